@@ -1,0 +1,142 @@
+/* ttsh.h — C ABI of the B200-native pseudospectral TTSH step.
+ *
+ * What it computes: one call of ttsh_step(h, n) applies n times Algorithm 1 of
+ * S. Shiratani, K. A. Takeuchi, D. Nishiguchi, arXiv:2304.03306 ("PAPER.md" below; Appendix C,
+ * PAPER.md:286-331) — the integrating-factor Euler step of the 2-D incompressible
+ * Toner-Tu-Swift-Hohenberg equation in vorticity form with the damping-mask boundary terms
+ * of Eq. (4) — on a periodic Nx x Ny grid.  ttsh_create runs Algorithm 2
+ * (mask processing, Appendix D) on a binary mask.
+ *
+ * General TTSH form (BASELINE.json:north_star), with the paper's model as a preset:
+ *     d_t v + lambda0 v.grad v = -grad p - (alpha + beta |v|^2) v + Gamma0 lap v - Gamma2 lap^2 v
+ *     paper (Eq. 2):  lambda0 = lambda, beta = b, alpha = 1 - a, Gamma0 = -2, Gamma2 = 1
+ *     linear symbol  sigma(k) = -alpha - Gamma0 k^2 - Gamma2 k^4   ( = a - (1-k^2)^2, Alg. 1 line 4, PAPER.md:295 )
+ *
+ * Conventions
+ *   - real fields: row-major scalar[Ny][Nx], x contiguous; point (i, j) sits at (i*dx, j*dx);
+ *     the DFT phase origin is index (0,0).  scalar = double (TTSH_F64) or float (TTSH_F32).
+ *   - every pointer documented "DEVICE" must be device memory of the current CUDA device, 16-byte
+ *     aligned; "HOST" pointers are ordinary host memory.  The library allocates NO device memory:
+ *     the caller owns the mask, the workspace, all field buffers and the stream; they are borrowed
+ *     for the duration of the enqueued (stream-ordered) work and the workspace must outlive the handle.
+ *   - all functions return 0 (TTSH_OK) or a negative ttsh_status; they never throw, abort or print.
+ *   - all work is enqueued on the stream given to ttsh_create; only ttsh_diagnostics synchronises.
+ *   - there is no CPU fallback: without a CUDA device every compute call returns TTSH_ERR_CUDA.
+ */
+#ifndef TTSH_H_
+#define TTSH_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ttsh_handle ttsh_handle;   /* opaque; host metadata + pointers into the workspace */
+
+typedef enum {
+  TTSH_OK = 0,
+  TTSH_ERR_INVALID_ARG = -1,         /* NULL pointer, n < 0, dx <= 0, dt <= 0, Gamma2 < 0, bad dealias fraction */
+  TTSH_ERR_UNSUPPORTED_SIZE = -2,    /* Nx, Ny must be powers of two in [64, 8192] (all sizes of PAPER.md:271 / BASELINE.json) */
+  TTSH_ERR_WORKSPACE_TOO_SMALL = -3,
+  TTSH_ERR_NOT_INITIALIZED = -4,     /* ttsh_step / get_fields / diagnostics before ttsh_set_velocity */
+  TTSH_ERR_CUDA = -5                 /* sticky; message via ttsh_last_error */
+} ttsh_status;
+
+/* Parameters of Eq. (2)/(4).  Paper preset (Table I :264-274): {9, 0.5, 1.6, -2, 1, 40, 4, 1, 2};
+ * BASELINE.json configs: {3.5, -0.5, 0.5, -1, 1, 40, 4, 1, 2}. */
+typedef struct {
+  double lambda0;      /* advection strength                                   */
+  double alpha;        /* linear damping (= 1 - a)                             */
+  double beta;         /* cubic nonlinearity (= b)                             */
+  double Gamma0;       /* coefficient of lap v  (negative = active)            */
+  double Gamma2;       /* coefficient of -lap^2 v, must be >= 0                */
+  double gamma_v;      /* velocity damping strength in the masked area, Eq. (4) */
+  double gamma_w;      /* vorticity damping strength in the masked area, Eq. (4) */
+  int dealias_num;     /* anti-aliasing cutoff |k| <= (num/den) * pi/dx, strict '>' removes; */
+  int dealias_den;     /* the paper's 1/2 rule is {1, 2}; allowed: 1/4 <= num/den <= 2/3                         */
+} ttsh_params;
+
+typedef enum { TTSH_F64 = 8, TTSH_F32 = 4 } ttsh_dtype;
+
+typedef enum {
+  TTSH_MASK_BINARY = 0,      /* unsigned char[Ny*Nx], nonzero = masked (K_naive = 1); Algorithm 2 is run on it */
+  TTSH_MASK_PROCESSED = 1    /* scalar[Ny*Nx], used as K(x) as given (caller guarantees K >= 0 and band-limited)           */
+} ttsh_mask_kind;
+
+/* Bytes of DEVICE workspace ttsh_create needs for this grid and dtype; 0 if the size is unsupported. */
+size_t ttsh_workspace_bytes(int Nx, int Ny, ttsh_dtype t);
+
+/* Creates a handle.  mask: DEVICE pointer (see ttsh_mask_kind) or NULL for no confinement (K == 0, the
+ * unconfined periodic run).  workspace: DEVICE, >= ttsh_workspace_bytes, 256-byte aligned.  cuda_stream: a
+ * cudaStream_t owned by the caller (NULL = the legacy default stream).  Enqueues Algorithm 2:
+ * K = ( iDFT[ lowpass_{1/4}( DFT[K_naive] ) ] )^2.  The mask buffer may be released after the stream has
+ * passed this call. */
+int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const ttsh_params* p, ttsh_dtype t,
+                const void* mask, ttsh_mask_kind kind, void* workspace, size_t workspace_bytes,
+                void* cuda_stream);
+
+/* Replaces K(x) on a live handle (state is kept: the hysteresis protocol of PAPER.md:143). */
+int ttsh_set_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind);
+
+/* Sets the state from a real velocity field (DEVICE scalar[Ny*Nx] each): w^ = i k_x v^_y - i k_y v^_x, mean
+ * flow v^(0) kept, then lines 5-16 of Algorithm 1 (cutoff, w^(0) = 0, Hermitian symmetrisation, stream-function
+ * inversion), i.e. v0 is projected onto band-limited divergence-free fields.  Resets t and the step counter. */
+int ttsh_set_velocity(ttsh_handle* h, const void* vx, const void* vy);
+
+/* n >= 0 applications of Algorithm 1; asynchronous; t += n*dt. */
+int ttsh_step(ttsh_handle* h, int n);
+
+/* Writes the current fields into caller-owned DEVICE buffers scalar[Ny*Nx]; any pointer may be NULL.
+ * v = iDFT[v^] (state), omega = iDFT[w^], psi = iDFT[w^/k^2] with psi^(0) = 0. */
+int ttsh_get_fields(ttsh_handle* h, void* vx, void* vy, void* omega, void* psi);
+
+/* Bit-exact checkpoint of the spectral state: w_hat is DEVICE complex-scalar[ttsh_state_elems] (interleaved
+ * re, im), mean_flow is HOST double[2] = v^(0).  get synchronises the stream. */
+size_t ttsh_state_elems(const ttsh_handle* h);
+int ttsh_get_state(ttsh_handle* h, void* w_hat, double* mean_flow);
+int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, double t, long long step);
+
+/* Diagnostics (sums over the ENTIRE grid; always double):
+ *   kinetic_energy = (1/2P) sum |v|^2,  enstrophy = (1/2P) sum w^2,
+ *   vortex_order   = Psi of Eq. (11), with e_theta the azimuthal unit vector about (cx, cy)
+ *                    (physical units); the grid point with r = 0 contributes to the denominator only;
+ *   polar_order    = |sum v| / sum |v|;   both orders are 0 when sum |v| = 0.
+ * host_out: HOST.  Synchronises the stream.  Returns TTSH_OK also when nonfinite > 0 (advisory). */
+typedef struct {
+  double t;
+  long long step;
+  double kinetic_energy, enstrophy, vortex_order, polar_order;
+  double sum_speed, sum_abs_vtheta, mean_vx, mean_vy, max_speed;
+  long long nonfinite;
+} ttsh_diag;
+int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out);
+
+/* Number of kernel launches the library has enqueued for this handle so far (bench bookkeeping). */
+long long ttsh_launch_count(const ttsh_handle* h);
+
+/* Debug/bench entry points for the individual kernels of the hot path (used by the per-kernel parity
+ * tests and the roofline measurement).  stage: one of TTSH_STAGE_*; runs that stage of a step once on the
+ * current state, leaving its outputs in the workspace.  Returns TTSH_ERR_INVALID_ARG for an unknown stage. */
+typedef enum {
+  TTSH_STAGE_INV_COL = 0,   /* w^ -> y-transformed intermediates (a1+a2/a6 column pass)  */
+  TTSH_STAGE_INV_ROW = 1,   /* intermediates -> omega, grad omega, v  (a2/a6 row pass)   */
+  TTSH_STAGE_REAL = 2,      /* rhs1, rhs2 (a3)                                           */
+  TTSH_STAGE_FWD_ROW = 3,   /* a4 row pass                                               */
+  TTSH_STAGE_FWD_COL = 4,   /* a4 column pass                                            */
+  TTSH_STAGE_SPECTRAL = 5   /* a5                                                        */
+} ttsh_stage;
+int ttsh_run_stage(ttsh_handle* h, int stage);
+/* Copies a workspace array out for inspection: which = 0..4 real scratch (omega|S, g_x|F_x, g_y|F_y, v_x, v_y),
+ * 5 = K.  dst: DEVICE scalar[Ny*Nx]. */
+int ttsh_debug_get_real(ttsh_handle* h, int which, void* dst);
+
+int ttsh_destroy(ttsh_handle* h);
+
+const char* ttsh_strerror(int code);
+const char* ttsh_last_error(const ttsh_handle* h);   /* "" if none */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TTSH_H_ */

@@ -1,0 +1,31 @@
+// engine.h — host-side launchers of the CUDA kernels, one explicit instantiation per scalar type.
+#pragma once
+#include <cuda_runtime.h>
+#include "ttsh_common.cuh"
+
+namespace ttsh {
+
+// FFT passes (fft_passes.cuh).  nfields <= 5 fields per launch (grid.y).  Return cudaErrorInvalidValue for an
+// unsupported transform length.
+template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const double* v0, cudaStream_t s);
+template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, cudaStream_t s);
+template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const double* v0, cudaStream_t s);
+template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, cudaStream_t s);
+// set the dynamic shared-memory attribute of the pass kernels for this grid (no launch)
+template <typename T> cudaError_t prepare_rows(const Geom& g);
+template <typename T> cudaError_t prepare_cols(const Geom& g);
+
+// element-wise kernels and reductions (pointwise.cuh)
+template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,
+                                                   void* w_s, void* gx_fx, void* gy_fy, cudaStream_t s);
+template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
+                                                  void* w, double* v0, cudaStream_t s);
+template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, double* v0, cudaStream_t s);
+template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s);
+template <typename T> cudaError_t launch_square(size_t n, const void* in, void* out, cudaStream_t s);
+template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, cudaStream_t s);
+constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs
+template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,
+                                              const void* w, double* partial, double* out, cudaStream_t s);
+
+}  // namespace ttsh

@@ -1,0 +1,94 @@
+// engine_fft.cuh — size dispatch for the FFT pass kernels (included by the per-dtype translation units).
+#pragma once
+#include "engine.h"
+#include "fft_passes.cuh"
+
+namespace ttsh {
+
+#define TTSH_FOR_SIZES(X) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) X(8192)
+
+template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+#ifdef TTSH_BUILD_COLS
+template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+  using C = ColCfg<T, NY>;
+  dim3 grid((g.Wx + C::L - 1) / C::L, nf);
+  k_inv_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), v0);
+  return cudaGetLastError();
+}
+template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+  using C = ColCfg<T, NY>;
+  dim3 grid((g.Wx + C::L - 1) / C::L, nf);
+  k_fwd_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab));
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+  switch (g.Ny) {
+#define X(N) case N: return go_inv_col<T, N>(g, b, nf, tab, v0, s);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+  switch (g.Ny) {
+#define X(N) case N: return go_fwd_col<T, N>(g, b, nf, tab, s);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T> cudaError_t prepare_cols(const Geom& g) {
+  switch (g.Ny) {
+#define X(N) case N: { cudaError_t e = set_smem(k_inv_col<T, N>, ColCfg<T, N>::SMEM); if (e != cudaSuccess) return e; \
+                       return set_smem(k_fwd_col<T, N>, ColCfg<T, N>::SMEM); }
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+#endif
+
+#ifdef TTSH_BUILD_ROWS
+template <typename T, int NX> static cudaError_t go_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+  using C = RowCfg<T, NX>;
+  dim3 grid((g.Ny / 2) / C::L, nf);
+  k_inv_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), v0);
+  return cudaGetLastError();
+}
+template <typename T, int NX> static cudaError_t go_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+  using C = RowCfg<T, NX>;
+  dim3 grid((g.Ny / 2) / C::L, nf);
+  k_fwd_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab));
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+  switch (g.Nx) {
+#define X(N) case N: return go_inv_row<T, N>(g, b, nf, tab, v0, s);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+  switch (g.Nx) {
+#define X(N) case N: return go_fwd_row<T, N>(g, b, nf, tab, s);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T> cudaError_t prepare_rows(const Geom& g) {
+  switch (g.Nx) {
+#define X(N) case N: { cudaError_t e = set_smem(k_inv_row<T, N>, RowCfg<T, N>::SMEM); if (e != cudaSuccess) return e; \
+                       return set_smem(k_fwd_row<T, N>, RowCfg<T, N>::SMEM); }
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+#endif
+
+}  // namespace ttsh

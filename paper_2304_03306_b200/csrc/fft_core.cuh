@@ -1,0 +1,192 @@
+// fft_core.cuh — shared-memory Stockham autosort FFT of one line, radix-16/8/4 butterflies in registers.
+//
+// A line of length N is transformed cooperatively by TPL = N/16 threads; every thread owns 16 complex
+// points per stage (one radix-16, two radix-8 or four radix-4 butterflies).  Stage s (radix R, Ns = product
+// of the earlier radices) does, for butterfly j in [0, N/R):
+//     k = j mod Ns;   v[r] = in[j + r N/R] * W_{Ns R}^{k r};   v = DFT_R(v);   out[(j-k) R + k + r Ns] = v[r]
+// The first stage reads through a caller-supplied functor (global memory, with whatever multiplier or
+// packing the pass needs) and the last stage writes through one, so a line makes one trip through
+// shared memory per stage boundary only.  Shared-memory indices are padded (i + i >> log2(R0)) so that both
+// the stride-R0 writes of the first stage and the unit-stride reads are bank-conflict free for 8- and 16-byte
+// elements.  DIR = -1: forward (e^{-i...}), DIR = +1: inverse.  No normalisation here.
+#pragma once
+#include "ttsh_common.cuh"
+#include <type_traits>
+
+namespace ttsh {
+
+// ---------------------------------------------------------------------------------------
+// radix plans.  nstages / radix are constexpr so that they can be template arguments.
+// ---------------------------------------------------------------------------------------
+template <int N> __host__ __device__ constexpr int fft_nstages() {
+  return N <= 256 ? 2 : (N <= 4096 ? 3 : 4);
+}
+template <int N> __host__ __device__ constexpr int fft_radix(int s) {
+  switch (N) {
+    case 32:   return s == 0 ? 8 : 4;
+    case 64:   return 8;
+    case 128:  return s == 0 ? 16 : 8;
+    case 256:  return 16;
+    case 512:  return 8;
+    case 1024: return s == 0 ? 16 : 8;
+    case 2048: return s <= 1 ? 16 : 8;
+    case 4096: return 16;
+    case 8192: return s == 0 ? 16 : 8;
+    default:   return 0;
+  }
+}
+template <int N> __host__ __device__ constexpr int fft_tpl() { return N / 16; }
+template <int N> __host__ __device__ constexpr int fft_padshift() { return fft_radix<N>(0) == 16 ? 4 : 3; }
+template <int N> __host__ __device__ constexpr int fft_line_elems() { return N + (N >> fft_padshift<N>()); }
+template <int N> __device__ __forceinline__ int fft_pad(int i) { return i + (i >> fft_padshift<N>()); }
+
+// ---------------------------------------------------------------------------------------
+// small DFTs in registers.  Outputs in natural order.
+// ---------------------------------------------------------------------------------------
+template <int DIR, typename T> __device__ __forceinline__ cplx<T> mul_w4(cplx<T> a) {   // a * W_4^1
+  return DIR < 0 ? mul_ni(a) : mul_i(a);
+}
+
+template <int DIR, typename T> __device__ __forceinline__ void dft2(cplx<T>& a, cplx<T>& b) {
+  cplx<T> t = a - b; a = a + b; b = t;
+}
+
+template <int DIR, typename T>
+__device__ __forceinline__ void dft4(cplx<T>& a0, cplx<T>& a1, cplx<T>& a2, cplx<T>& a3) {
+  cplx<T> t0 = a0 + a2, t1 = a0 - a2, t2 = a1 + a3, t3 = mul_w4<DIR>(a1 - a3);
+  a0 = t0 + t2; a1 = t1 + t3; a2 = t0 - t2; a3 = t1 - t3;
+}
+
+// a * W_8^n and a * W_16^n with compile-time n (DIR-aware); constants are exact to 0.5 ulp in double
+template <int DIR, int n, typename T> __device__ __forceinline__ cplx<T> mul_w8(cplx<T> a) {
+  constexpr T h = (T)0.70710678118654752440084436210485;
+  if (n == 0) return a;
+  if (n == 2) return mul_w4<DIR>(a);
+  if (n == 1) return DIR < 0 ? mk<T>(h * (a.x + a.y), h * (a.y - a.x)) : mk<T>(h * (a.x - a.y), h * (a.y + a.x));
+  /* n == 3 */ return DIR < 0 ? mk<T>(h * (a.y - a.x), -h * (a.x + a.y)) : mk<T>(-h * (a.x + a.y), h * (a.x - a.y));
+}
+template <int DIR, int n, typename T> __device__ __forceinline__ cplx<T> mul_w16(cplx<T> a) {
+  // W_16^n = cos(n pi/8) + DIR * i sin(n pi/8), n = 0..9
+  constexpr T c1 = (T)0.92387953251128675612818318939679, s1 = (T)0.38268343236508977172845998403040;
+  if (n % 2 == 0) return mul_w8<DIR, n / 2>(a);
+  T c = (n == 1) ? c1 : (n == 3) ? s1 : (n == 5) ? -s1 : (n == 7) ? -c1 : -c1;
+  T s = (n == 1) ? s1 : (n == 3) ? c1 : (n == 5) ? c1 : (n == 7) ? s1 : -s1;   // n == 9: (-c1, -s1)
+  s = DIR < 0 ? -s : s;
+  return mk<T>(a.x * c - a.y * s, a.x * s + a.y * c);
+}
+
+template <int DIR, typename T> __device__ __forceinline__ void dft8(cplx<T>* v) {
+  // s = 2 s1 + s2, r = r1 + 4 r2:  W_8^{rs} = W_4^{r1 s1} W_8^{r1 s2} W_2^{r2 s2}
+  dft4<DIR>(v[0], v[2], v[4], v[6]);
+  dft4<DIR>(v[1], v[3], v[5], v[7]);
+  v[3] = mul_w8<DIR, 1>(v[3]);
+  v[5] = mul_w8<DIR, 2>(v[5]);
+  v[7] = mul_w8<DIR, 3>(v[7]);
+  // v[2 r1] = y[0][r1], v[2 r1 + 1] = y[1][r1]
+  cplx<T> o[8];
+#pragma unroll
+  for (int r1 = 0; r1 < 4; ++r1) {
+    o[r1] = v[2 * r1] + v[2 * r1 + 1];
+    o[r1 + 4] = v[2 * r1] - v[2 * r1 + 1];
+  }
+#pragma unroll
+  for (int r = 0; r < 8; ++r) v[r] = o[r];
+}
+
+template <int DIR, typename T> __device__ __forceinline__ void dft16(cplx<T>* v) {
+  // s = 4 s1 + s2, r = r1 + 4 r2:  W_16^{rs} = W_4^{r1 s1} W_16^{r1 s2} W_4^{r2 s2}
+#pragma unroll
+  for (int s2 = 0; s2 < 4; ++s2) dft4<DIR>(v[s2], v[4 + s2], v[8 + s2], v[12 + s2]);   // v[4 r1 + s2] = y[s2][r1]
+  v[5] = mul_w16<DIR, 1>(v[5]);   v[6] = mul_w16<DIR, 2>(v[6]);   v[7] = mul_w16<DIR, 3>(v[7]);
+  v[9] = mul_w16<DIR, 2>(v[9]);   v[10] = mul_w16<DIR, 4>(v[10]); v[11] = mul_w16<DIR, 6>(v[11]);
+  v[13] = mul_w16<DIR, 3>(v[13]); v[14] = mul_w16<DIR, 6>(v[14]); v[15] = mul_w16<DIR, 9>(v[15]);
+#pragma unroll
+  for (int r1 = 0; r1 < 4; ++r1) dft4<DIR>(v[4 * r1], v[4 * r1 + 1], v[4 * r1 + 2], v[4 * r1 + 3]);
+  // now v[4 r1 + r2] = X[r1 + 4 r2]: transpose the 4x4 index
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = a + 1; b < 4; ++b) { cplx<T> t = v[4 * a + b]; v[4 * a + b] = v[4 * b + a]; v[4 * b + a] = t; }
+}
+
+template <int R, int DIR, typename T> __device__ __forceinline__ void dftR(cplx<T>* v) {
+  if (R == 16) dft16<DIR>(v);
+  else if (R == 8) dft8<DIR>(v);
+  else if (R == 4) dft4<DIR>(v[0], v[1], v[2], v[3]);
+  else dft2<DIR>(v[0], v[1]);
+}
+
+// 64/128-bit read-only loads of a complex value
+__device__ __forceinline__ cplx<double> ldg_c(const cplx<double>* p) {
+  double2 t = __ldg(reinterpret_cast<const double2*>(p)); return mk<double>(t.x, t.y);
+}
+__device__ __forceinline__ cplx<float> ldg_c(const cplx<float>* p) {
+  float2 t = __ldg(reinterpret_cast<const float2*>(p)); return mk<float>(t.x, t.y);
+}
+
+// twiddle W_M^p from the forward-sign table (M = table length), conjugated for the inverse
+template <int DIR, typename T> __device__ __forceinline__ cplx<T> twiddle(const cplx<T>* __restrict__ tab, int p) {
+  cplx<T> w = ldg_c(tab + p);
+  return DIR < 0 ? w : conj(w);
+}
+
+// ---------------------------------------------------------------------------------------
+// one line.  j = thread index within the line's TPL threads; sm = this line's padded buffer.
+// TS = stride into the twiddle table (table length = N * TS).
+// SYNC_LAST: the last-stage store goes to shared memory, so it needs the read/write barrier too.
+// EVERY thread of the CTA must call this (it contains __syncthreads()).
+// ---------------------------------------------------------------------------------------
+template <typename T, int N, int DIR, int TS, int S, int NS, bool SYNC_LAST, class Load, class Store>
+__device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab,
+                                          Load& load, Store& store) {
+  constexpr int R = fft_radix<N>(S);
+  constexpr int NST = fft_nstages<N>();
+  constexpr bool first = (S == 0), last = (S == NST - 1);
+  constexpr int TPL = fft_tpl<N>();
+  constexpr int NB = (N / R) / TPL;         // butterflies per thread: 16 / R
+  cplx<T> v[NB][R];
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    const int j = j0 + b * TPL;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int idx = j + r * (N / R);
+      v[b][r] = first ? load(idx) : sm[fft_pad<N>(idx)];
+    }
+  }
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    const int j = j0 + b * TPL;
+    if (NS > 1) {
+      const int k = j & (NS - 1);
+#pragma unroll
+      for (int r = 1; r < R; ++r) v[b][r] = v[b][r] * twiddle<DIR>(tab, k * r * ((N / (NS * R)) * TS));
+    }
+    dftR<R, DIR>(v[b]);
+  }
+  if (!last || SYNC_LAST) __syncthreads();     // every thread has finished reading this buffer
+#pragma unroll
+  for (int b = 0; b < NB; ++b) {
+    const int j = j0 + b * TPL;
+    const int k = j & (NS - 1);
+    const int base = (j - k) * R + k;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int o = base + r * NS;
+      if (last) store(o, v[b][r]);
+      else sm[fft_pad<N>(o)] = v[b][r];
+    }
+  }
+  if constexpr (!last) {
+    __syncthreads();
+    fft_stage<T, N, DIR, TS, S + 1, NS * R, SYNC_LAST>(j0, sm, tab, load, store);
+  }
+}
+
+template <typename T, int N, int DIR, int TS, bool SYNC_LAST, class Load, class Store>
+__device__ __forceinline__ void fft_line(int j, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab,
+                                         Load load, Store store) {
+  fft_stage<T, N, DIR, TS, 0, 1, SYNC_LAST>(j, sm, tab, load, store);
+}
+
+}  // namespace ttsh

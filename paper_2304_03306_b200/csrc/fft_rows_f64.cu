@@ -1,0 +1,8 @@
+// row-pass kernels, scalar = double
+#define TTSH_BUILD_ROWS
+#include "engine_fft.cuh"
+namespace ttsh {
+template cudaError_t launch_inv_row<double>(const Geom&, const Batch&, int, const void*, const double*, cudaStream_t);
+template cudaError_t launch_fwd_row<double>(const Geom&, const Batch&, int, const void*, cudaStream_t);
+template cudaError_t prepare_rows<double>(const Geom&);
+}

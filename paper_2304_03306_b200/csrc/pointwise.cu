@@ -1,0 +1,63 @@
+// element-wise kernels and reductions, both scalar types
+#include "engine.h"
+#include "pointwise.cuh"
+
+namespace ttsh {
+
+static inline int blocks_for(size_t n, int threads, int cap) {
+  size_t b = (n + threads - 1) / threads;
+  return (int)(b < (size_t)cap ? (b ? b : 1) : cap);
+}
+constexpr int GRID_CAP = 148 * 16;
+
+template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,
+                                                   void* w_s, void* gx_fx, void* gy_fy, cudaStream_t s) {
+  const size_t nvec = (size_t)g.Nx * g.Ny / Vec<T>::n;
+  k_realspace<T><<<blocks_for(nvec, 256, GRID_CAP), 256, 0, s>>>(nvec, m, (const T*)vx, (const T*)vy, (const T*)K,
+                                                                  (T*)w_s, (T*)gx_fx, (T*)gy_fy);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
+                                                  void* w, double* v0, cudaStream_t s) {
+  dim3 grid((g.Wx + 255) / 256, g.Hy);
+  k_spectral<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, v0);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, double* v0, cudaStream_t s) {
+  dim3 grid((g.Wx + 255) / 256, g.Hy);
+  k_spectral_init<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)Vx, (const cplx<T>*)Vy, (cplx<T>*)w, v0);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s) {
+  k_mask_to_real<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, mask, (T*)out);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_square(size_t n, const void* in, void* out, cudaStream_t s) {
+  k_square<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, (const T*)in, (T*)out);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, cudaStream_t s) {
+  k_fill<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, (T*)out, (T)val);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,
+                                              const void* w, double* partial, double* out, cudaStream_t s) {
+  k_diag_partial<T><<<DIAG_BLOCKS, 256, 0, s>>>(g.Nx, g.Ny, dx, cx, cy, (const T*)vx, (const T*)vy, (const T*)w, partial);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_diag_final<<<1, 256, 0, s>>>(DIAG_BLOCKS, partial, out);
+  return cudaGetLastError();
+}
+
+#define INST(T) \
+  template cudaError_t launch_realspace<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
+  template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, double*, cudaStream_t); \
+  template cudaError_t launch_spectral_init<T>(const Geom&, const void*, const void*, void*, double*, cudaStream_t); \
+  template cudaError_t launch_mask_to_real<T>(size_t, const unsigned char*, void*, cudaStream_t); \
+  template cudaError_t launch_square<T>(size_t, const void*, void*, cudaStream_t); \
+  template cudaError_t launch_fill<T>(size_t, void*, double, cudaStream_t); \
+  template cudaError_t launch_diag<T>(const Geom&, double, double, double, const void*, const void*, const void*, double*, double*, cudaStream_t);
+INST(double)
+INST(float)
+
+}  // namespace ttsh

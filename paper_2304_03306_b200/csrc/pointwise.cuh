@@ -1,0 +1,233 @@
+// pointwise.cuh — element-wise kernels of Algorithm 1 and the diagnostics reduction.
+//   k_realspace      lines 1-2: rhs1 = -beta |v|^2 v - gamma_v K v ;  rhs2 = -lambda0 v.grad(w) - gamma_w K w
+//   k_spectral       lines 3-12: curl + sum, integrating-factor Euler, k = 0 / cutoff / Hermitian cases
+//   k_spectral_init  state from a velocity field (ttsh_set_velocity)
+//   k_diag_*         warp-shuffle reductions for E, Z, Psi (Eq. 11), polar order
+// "any if statement should be purged": the k = 0 / cutoff cases are predicated selects on an
+// integer predicate; the only divergent branch is the mx = 0 column of the Hermitian symmetrisation.
+#pragma once
+#include "ttsh_common.cuh"
+
+namespace ttsh {
+
+// ---------------------------------------------------------------------------------------
+// a3: fused real-space kernel.  In place: (w, gx, gy) -> (rhs2, rhs1x, rhs1y); v and K are read-only.
+// 16-byte vector accesses; Nx*Ny is a multiple of 4.
+// ---------------------------------------------------------------------------------------
+template <typename T> struct Vec;   // 16-byte vector of T
+template <> struct Vec<double> { using type = double2; static constexpr int n = 2; };
+template <> struct Vec<float> { using type = float4; static constexpr int n = 4; };
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_realspace(size_t nvec, Model m, const T* __restrict__ vx, const T* __restrict__ vy, const T* __restrict__ K,
+            T* __restrict__ w_s, T* __restrict__ gx_fx, T* __restrict__ gy_fy) {
+  using V = typename Vec<T>::type;
+  constexpr int n = Vec<T>::n;
+  const T beta = (T)m.beta, gv = (T)m.gamma_v, gw = (T)m.gamma_w, lam = (T)m.lambda0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    V a = reinterpret_cast<const V*>(vx)[i], b = reinterpret_cast<const V*>(vy)[i];
+    V k = reinterpret_cast<const V*>(K)[i];
+    V w = reinterpret_cast<V*>(w_s)[i], gx = reinterpret_cast<V*>(gx_fx)[i], gy = reinterpret_cast<V*>(gy_fy)[i];
+    T* pa = reinterpret_cast<T*>(&a); T* pb = reinterpret_cast<T*>(&b); T* pk = reinterpret_cast<T*>(&k);
+    T* pw = reinterpret_cast<T*>(&w); T* pgx = reinterpret_cast<T*>(&gx); T* pgy = reinterpret_cast<T*>(&gy);
+#pragma unroll
+    for (int e = 0; e < n; ++e) {
+      const T u = pa[e], v = pb[e], kk = pk[e];
+      const T c = -beta * (u * u + v * v) - gv * kk;                 // rhs1 = c * v           (line 1)
+      const T s = -lam * (u * pgx[e] + v * pgy[e]) - gw * kk * pw[e];  // rhs2                   (line 2)
+      pgx[e] = c * u;
+      pgy[e] = c * v;
+      pw[e] = s;
+    }
+    reinterpret_cast<V*>(w_s)[i] = w;
+    reinterpret_cast<V*>(gx_fx)[i] = gx;
+    reinterpret_cast<V*>(gy_fy)[i] = gy;
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// a5: fused spectral kernel on the pruned spectrum [Hy][Wxp].
+//   w^_naive = exp(sigma dt) (w^ + dt (i kx F^y - i ky F^x + S^))                       (lines 3-4)
+//   k = 0:   w^ = 0,  v^(0) <- exp(-alpha dt) (v^(0) + dt F^(0))                         (lines 6-8, Eq. C1)
+//   cut:     w^ = 0                                                                       (lines 9-11)
+//   else:    w^ = (w^_naive(k) + conj w^_naive(-k)) / 2 — the identity off the mx = 0 column in half-spectrum
+//            storage; on that column the thread of (0, my > 0) computes both +-my and writes both   (line 12, R6)
+// In place on w^ (every element is read and written by exactly one thread).
+// ---------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ cplx<T> naive_update(const Geom& g, const Model& m, int mx, int my, size_t idx,
+                                                const cplx<T>* __restrict__ Fx, const cplx<T>* __restrict__ Fy,
+                                                const cplx<T>* __restrict__ S, const cplx<T>* w) {
+  const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my);
+  const T k2 = kx * kx + ky * ky;
+  const T sigma = -(T)m.alpha - (T)m.Gamma0 * k2 - (T)m.Gamma2 * k2 * k2;
+  const T dt = (T)m.dt;
+  const cplx<T> r = kx * mul_i(Fy[idx]) - ky * mul_i(Fx[idx]) + S[idx];      // line 3
+  const T e = sizeof(T) == 8 ? (T)exp((double)(sigma * dt)) : (T)expf((float)(sigma * dt));
+  return e * (w[idx] + dt * r);                                               // line 4
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __restrict__ Fy,
+           const cplx<T>* __restrict__ S, cplx<T>* w, double* v0) {
+  const int mx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int q = blockIdx.y;
+  if (mx >= g.Wx) return;
+  const int my = q <= g.My ? q : q - g.Hy;
+  const size_t idx = (size_t)q * g.Wxp + mx;
+  const bool zero = (mx == 0 && my == 0);
+  const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
+  if (mx == 0) {
+    if (my < 0) return;                                   // written by the thread of (0, -my)
+    if (zero) {
+      // mean flow, Eq. (C1): only rhs1 contributes
+      const double e = exp(-m.alpha * m.dt);
+      v0[0] = e * (v0[0] + m.dt * (double)Fx[idx].x);
+      v0[1] = e * (v0[1] + m.dt * (double)Fy[idx].x);
+      w[idx] = mk<T>(0, 0);
+      return;
+    }
+    const size_t idn = (size_t)(g.Hy - my) * g.Wxp;       // row of -my, mx = 0
+    cplx<T> out = mk<T>(0, 0);
+    if (!cut) {
+      const cplx<T> a = naive_update<T>(g, m, 0, my, idx, Fx, Fy, S, w);
+      const cplx<T> b = naive_update<T>(g, m, 0, -my, idn, Fx, Fy, S, w);
+      out = (T)0.5 * (a + conj(b));
+    }
+    w[idx] = out;
+    w[idn] = conj(out);
+    return;
+  }
+  cplx<T> out = naive_update<T>(g, m, mx, my, idx, Fx, Fy, S, w);
+  w[idx] = cut ? mk<T>(0, 0) : out;
+}
+
+// ttsh_set_velocity: w^ = i kx v^y - i ky v^x, v^(0) kept, then the same post-processing
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_spectral_init(Geom g, const cplx<T>* __restrict__ Vx, const cplx<T>* __restrict__ Vy, cplx<T>* w, double* v0) {
+  const int mx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int q = blockIdx.y;
+  if (mx >= g.Wx) return;
+  const int my = q <= g.My ? q : q - g.Hy;
+  const size_t idx = (size_t)q * g.Wxp + mx;
+  const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
+  auto curl = [&](int my_, size_t id) -> cplx<T> {
+    const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my_);
+    return kx * mul_i(Vy[id]) - ky * mul_i(Vx[id]);
+  };
+  if (mx == 0) {
+    if (my < 0) return;
+    if (my == 0) {
+      v0[0] = (double)Vx[idx].x;
+      v0[1] = (double)Vy[idx].x;
+      w[idx] = mk<T>(0, 0);
+      return;
+    }
+    const size_t idn = (size_t)(g.Hy - my) * g.Wxp;
+    cplx<T> out = mk<T>(0, 0);
+    if (!cut) out = (T)0.5 * (curl(my, idx) + conj(curl(-my, idn)));
+    w[idx] = out;
+    w[idn] = conj(out);
+    return;
+  }
+  w[idx] = cut ? mk<T>(0, 0) : curl(my, idx);
+}
+
+// ---------------------------------------------------------------------------------------
+// small helpers for Algorithm 2
+// ---------------------------------------------------------------------------------------
+template <typename T>
+__global__ void k_mask_to_real(size_t n, const unsigned char* __restrict__ mask, T* __restrict__ out) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    out[i] = mask[i] ? (T)1 : (T)0;
+}
+template <typename T>
+__global__ void k_square(size_t n, const T* __restrict__ in, T* __restrict__ out) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const T s = in[i];
+    out[i] = s * s;                                                           // line 9
+  }
+}
+template <typename T>
+__global__ void k_fill(size_t n, T* __restrict__ out, T val) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    out[i] = val;
+}
+
+// ---------------------------------------------------------------------------------------
+// a7: diagnostics.  Stage 1: grid-stride accumulation in fp64, warp-shuffle + smem block reduction, one
+// partial record per block.  Stage 2: one block reduces the partials (fixed order => deterministic).
+// record: [0] sum|v|^2  [1] sum w^2  [2] sum|v|  [3] sum|e_theta.v|  [4] sum vx  [5] sum vy  [6] max|v|  [7] #nonfinite
+// ---------------------------------------------------------------------------------------
+constexpr int DIAG_REC = 8;
+
+__device__ __forceinline__ void diag_warp_reduce(double* a) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+#pragma unroll
+    for (int k = 0; k < DIAG_REC; ++k) {
+      const double o = __shfl_down_sync(0xffffffffu, a[k], off);
+      if (k == 6) a[k] = fmax(a[k], o); else a[k] += o;
+    }
+  }
+}
+
+__device__ __forceinline__ void diag_block_reduce(double* a, double* out) {
+  __shared__ double sh[32][DIAG_REC];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  diag_warp_reduce(a);
+  if (lane == 0)
+    for (int k = 0; k < DIAG_REC; ++k) sh[wid][k] = a[k];
+  __syncthreads();
+  if (wid == 0) {
+    for (int k = 0; k < DIAG_REC; ++k) a[k] = lane < nw ? sh[lane][k] : 0.0;
+    diag_warp_reduce(a);
+    if (lane == 0)
+      for (int k = 0; k < DIAG_REC; ++k) out[k] = a[k];
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_diag_partial(int Nx, int Ny, double dx, double cx, double cy, const T* __restrict__ vx, const T* __restrict__ vy,
+               const T* __restrict__ w, double* __restrict__ partial) {
+  double a[DIAG_REC];
+#pragma unroll
+  for (int k = 0; k < DIAG_REC; ++k) a[k] = 0.0;
+  const size_t n = (size_t)Nx * Ny;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const double u = (double)vx[i], v = (double)vy[i], ww = (double)w[i];
+    const int ix = (int)(i % Nx), iy = (int)(i / Nx);
+    const double x = ix * dx - cx, y = iy * dx - cy;
+    const double r = sqrt(x * x + y * y);
+    const double s2 = u * u + v * v;
+    const double vth = r == 0.0 ? 0.0 : (-y * u + x * v) / r;       // e_theta . v  (Eq. 11)
+    a[0] += s2;
+    a[1] += ww * ww;
+    a[2] += sqrt(s2);
+    a[3] += fabs(vth);
+    a[4] += u;
+    a[5] += v;
+    a[6] = fmax(a[6], sqrt(s2));
+    a[7] += (isfinite(u) ? 0.0 : 1.0) + (isfinite(v) ? 0.0 : 1.0) + (isfinite(ww) ? 0.0 : 1.0);
+  }
+  diag_block_reduce(a, partial + (size_t)blockIdx.x * DIAG_REC);
+}
+
+__global__ void __launch_bounds__(256) k_diag_final(int nblocks, const double* __restrict__ partial, double* __restrict__ out) {
+  double a[DIAG_REC];
+#pragma unroll
+  for (int k = 0; k < DIAG_REC; ++k) a[k] = 0.0;
+  for (int b = threadIdx.x; b < nblocks; b += blockDim.x)
+#pragma unroll
+    for (int k = 0; k < DIAG_REC; ++k) {
+      const double o = partial[(size_t)b * DIAG_REC + k];
+      if (k == 6) a[k] = fmax(a[k], o); else a[k] += o;
+    }
+  diag_block_reduce(a, out);
+}
+
+}  // namespace ttsh

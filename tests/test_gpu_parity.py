@@ -1,0 +1,255 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the CPU oracle, element by element, same seeded inputs.
+
+Tolerances (BASELINE.json:north_star): fp64 relative L2 <= 1e-12 after 1 step and <= 1e-9 after 100 steps;
+fp32 <= 1e-5 after 1 step; diagnostics within 1e-10 relative (on the raw sums, reading R13)."""
+import numpy as np
+import pytest
+
+from oracle import BASELINE_PRESET, PAPER_PRESET, TTSHOracle
+from paper_2304_03306_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL_F64_1, TOL_F64_100, TOL_F32_1, TOL_DIAG = 1e-12, 1e-9, 1e-5, 1e-10
+
+
+@pytest.fixture(scope="module")
+def ttsh():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2304_03306_b200 import ttsh as t
+    return t
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def gpu_fields(s):
+    vx, vy, w, psi = s.get_fields()
+    return [t.cpu().numpy().astype(np.float64) for t in (vx, vy, w, psi)]
+
+
+def params_pair(ttsh, which):
+    return (ttsh.baseline_params(), BASELINE_PRESET) if which == "baseline" else (ttsh.paper_params(), PAPER_PRESET)
+
+
+def make_pair(ttsh, Nx, Ny, dx, dt, which, mask, dtype="f64", transform="matmul", vel=None):
+    gp, op = params_pair(ttsh, which)
+    s = ttsh.Solver(Nx, Ny, dx, dt, gp, dtype, mask=mask)
+    o = TTSHOracle(Nx, Ny, dx, dt, op, mask=mask, transform=transform)
+    if vel is not None:
+        vx0, vy0 = vel
+        if dtype == "f32":   # fp32 runs receive the fp64 array rounded to nearest (R15)
+            vx0 = vx0.astype(np.float32).astype(np.float64); vy0 = vy0.astype(np.float32).astype(np.float64)
+        s.set_velocity(vx0, vy0)
+        o.set_velocity(vx0, vy0)
+    return s, o
+
+
+def compare_state(s, o, tol, what=""):
+    vx, vy, w, psi = gpu_fields(s)
+    ovx, ovy, ow, opsi = o.get_fields()
+    ev = rel(np.stack([vx, vy]), np.stack([ovx, ovy]))
+    ew = rel(w, ow)
+    ep = rel(psi, opsi)
+    assert ev <= tol and ew <= tol and ep <= tol, f"{what}: v {ev:.3e} w {ew:.3e} psi {ep:.3e} > {tol:g}"
+    return ev, ew
+
+
+# ---------------------------------------------------------------- Algorithm 2 and set_velocity
+@pytest.mark.parametrize("shape", [(64, 64), (256, 128), (128, 512)])
+def test_mask_processing_matches_oracle(ttsh, shape):
+    Nx, Ny = shape
+    mask = workloads.dumbbell_mask(Nx, Ny, 0.5, min(Nx, Ny) * 0.5 * 0.2, min(Nx, Ny) * 0.5 * 0.25)
+    s, o = make_pair(ttsh, Nx, Ny, 0.5, 0.01, "baseline", mask)
+    K = s.debug_real(5).cpu().numpy()
+    assert rel(K, o.K) <= 1e-12
+    assert K.min() >= 0.0
+    s.close()
+
+
+@pytest.mark.parametrize("shape", [(64, 64), (128, 64), (64, 256), (512, 512)])
+def test_set_velocity_projection_matches_oracle(ttsh, shape):
+    Nx, Ny = shape
+    mask = workloads.disk_mask(Nx, Ny, 0.5, 0.3 * min(Nx, Ny) * 0.5)
+    vel = workloads.gaussian_velocity(Nx, Ny, 7, 1.0, mask)
+    vel = (vel[0] + 0.25, vel[1] - 0.5)       # non-zero mean flow
+    s, o = make_pair(ttsh, Nx, Ny, 0.5, 0.01, "baseline", mask, vel=vel)
+    compare_state(s, o, 1e-12, f"init {shape}")
+    s.close()
+
+
+# ---------------------------------------------------------------- per-kernel parity against oracle intermediates
+def test_real_space_kernel_matches_oracle_rhs(ttsh):
+    Nx, Ny = 256, 128
+    mask = workloads.disk_mask(Nx, Ny, 0.5, 20.0)
+    vel = workloads.planewave_velocity(Nx, Ny, 0.5, 3, amplitude=1.0)
+    s, o = make_pair(ttsh, Nx, Ny, 0.5, 0.01, "baseline", mask, vel=vel)
+    s.run_stage(ttsh.TTSH_STAGE_INV_COL); s.run_stage(ttsh.TTSH_STAGE_INV_ROW)
+    w, gx, gy, rhs1, rhs2 = o.rhs_real()
+    got = [s.debug_real(i).cpu().numpy() for i in range(5)]
+    for g, e, name in zip(got, (w, gx, gy, o.v[0], o.v[1]), ("w", "gx", "gy", "vx", "vy")):
+        assert rel(g, e) <= 1e-12, name
+    s.run_stage(ttsh.TTSH_STAGE_REAL)
+    got = [s.debug_real(i).cpu().numpy() for i in range(3)]
+    for g, e, name in zip(got, (rhs2, rhs1[0], rhs1[1]), ("rhs2", "rhs1x", "rhs1y")):
+        assert rel(g, e) <= 1e-12, name
+    s.close()
+
+
+# ---------------------------------------------------------------- whole-step parity
+CASES_SMALL = [
+    ("C1-baseline", 64, 64, "baseline", "disk", 1e-2),
+    ("C1-paper", 64, 64, "paper", "disk", 1e-2),
+    ("C1-O(1)", 64, 64, "baseline", "disk", 1.0),
+    ("rect-128x64", 128, 64, "baseline", "dumbbell", 1.0),
+    ("rect-64x256", 64, 256, "paper", "disk", 1.0),
+]
+
+
+@pytest.mark.parametrize("name,Nx,Ny,which,geom,amp", CASES_SMALL)
+def test_trajectory_small_grids_every_step(ttsh, name, Nx, Ny, which, geom, amp):
+    dx = 0.5
+    R = 12.0 if min(Nx, Ny) == 64 else 20.0
+    mask = workloads.disk_mask(Nx, Ny, dx, R) if geom == "disk" else workloads.dumbbell_mask(Nx, Ny, dx, 10.0, 14.0)
+    if amp < 0.1:
+        vel = workloads.gaussian_velocity(Nx, Ny, workloads.SEED0, amp, mask)
+    else:
+        vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0, amplitude=amp)
+    s, o = make_pair(ttsh, Nx, Ny, dx, 0.01, which, mask, vel=vel)
+    compare_state(s, o, TOL_F64_1, name + " init")
+    for n in range(1, 101):
+        s.step(1); o.step(1)
+        if n == 1:
+            compare_state(s, o, TOL_F64_1, name + " step 1")
+        elif n % 10 == 0:
+            compare_state(s, o, TOL_F64_100, f"{name} step {n}")
+    # diagnostics on the raw sums (R13)
+    cx, cy = (Nx // 2) * dx, (Ny // 2) * dx
+    d, od = s.diagnostics(cx, cy), o.diagnostics(cx, cy)
+    for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy", "max_speed"):
+        assert abs(d[key] - od[key]) <= TOL_DIAG * abs(od[key]), key
+    for key in ("mean_vx", "mean_vy"):
+        assert abs(d[key] - od[key]) * Nx * Ny <= TOL_DIAG * od["sum_speed"], key
+    assert abs(d["vortex_order"] - od["vortex_order"]) <= 1e-10 and abs(d["polar_order"] - od["polar_order"]) <= 1e-10
+    assert d["nonfinite"] == 0 and d["step"] == 100 and abs(d["t"] - 1.0) < 1e-12
+    s.close()
+
+
+def test_C2_256_disk_steps_1_and_100(ttsh):
+    cfg = workloads.CONFIGS["C2"]
+    mask = cfg.mask()
+    vel = cfg.initial_velocity(mask)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, vel=vel)
+    s.step(1); o.step(1)
+    compare_state(s, o, TOL_F64_1, "C2 step 1")
+    s.step(99); o.step(99)
+    compare_state(s, o, TOL_F64_100, "C2 step 100")
+    s.close()
+
+
+def test_C2_O1_start_100_steps_graph_replay(ttsh):
+    cfg = workloads.CONFIGS["C2"]
+    mask = cfg.mask()
+    vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "paper", mask, vel=vel)
+    s.step(100); o.step(100)          # n >= 4 on a small grid goes through the captured CUDA graph
+    compare_state(s, o, TOL_F64_100, "C2 O(1) step 100")
+    s.close()
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", TOL_F64_1), ("f32", TOL_F32_1)])
+def test_C3_1024_disk_single_step(ttsh, dtype, tol):
+    cfg = workloads.CONFIGS["C3"]
+    mask = cfg.mask(R=160.0)
+    vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, dtype=dtype, vel=vel)
+    if dtype == "f32":
+        o.K = s.debug_real(5).cpu().numpy().astype(np.float64)   # K is built by Algorithm 2 in fp32 in the fp32 handle (R15)
+    s.step(1); o.step(1)
+    compare_state(s, o, tol, f"C3 {dtype} step 1")
+    s.close()
+
+
+def test_C4_dumbbell_1024x2048_single_step(ttsh):
+    cfg = workloads.CONFIGS["C4"]
+    mask = cfg.mask()
+    vel = cfg.initial_velocity(mask, amplitude=1.0)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, vel=vel)
+    s.step(1); o.step(1)
+    compare_state(s, o, TOL_F64_1, "C4 step 1")
+    s.close()
+
+
+# ---------------------------------------------------------------- edge cases
+def test_no_mask_zero_field_and_error_paths(ttsh):
+    s = ttsh.Solver(64, 64, 0.5, 0.01, ttsh.baseline_params(), "f64", mask=None)
+    with pytest.raises(ttsh.TTSHError) as e:
+        s.step(1)
+    assert e.value.code == ttsh.TTSH_ERR_NOT_INITIALIZED
+    z = np.zeros((64, 64))
+    s.set_velocity(z, z)
+    s.step(3)
+    vx, vy, w, psi = gpu_fields(s)
+    assert np.all(vx == 0) and np.all(vy == 0) and np.all(w == 0) and np.all(psi == 0)
+    d = s.diagnostics()
+    assert d["vortex_order"] == 0.0 and d["polar_order"] == 0.0 and d["nonfinite"] == 0
+    assert ttsh.ttsh_step(s.h, -1) == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_step(s.h, 0) == ttsh.TTSH_OK
+    assert ttsh.ttsh_run_stage(s.h, 99) == ttsh.TTSH_ERR_INVALID_ARG
+    s.close()
+
+
+def test_uniform_fixed_point_and_single_mode_on_gpu(ttsh):
+    N, dx, dt = 64, 0.5, 0.01
+    p = ttsh.baseline_params()
+    vstar = np.sqrt((1.0 - np.exp(p.alpha * dt)) / (p.beta * dt))
+    s = ttsh.Solver(N, N, dx, dt, p, "f64", mask=None)
+    s.set_velocity(np.full((N, N), vstar * 0.6), np.full((N, N), vstar * 0.8))
+    s.step(100)
+    vx, vy, w, _ = gpu_fields(s)
+    assert np.max(np.abs(vx - 0.6 * vstar)) < 1e-14 and np.max(np.abs(vy - 0.8 * vstar)) < 1e-14 and np.max(np.abs(w)) < 1e-14
+    # closed-form growth of one Fourier mode
+    k = 2 * np.pi * np.array([3, 2]) / (N * dx)
+    x = np.arange(N)[None, :] * dx; y = np.arange(N)[:, None] * dx
+    ph = k[0] * x + k[1] * y + 0.3
+    vx0 = -k[1] * 1e-3 * np.sin(ph); vy0 = k[0] * 1e-3 * np.sin(ph)
+    s.set_velocity(vx0, vy0)
+    s.step(40)
+    k2 = float(k @ k)
+    g = np.exp((0.5 + k2 - k2 * k2) * 40 * dt)
+    vx, vy, _, _ = gpu_fields(s)
+    assert rel(vx, g * vx0) < 1e-12 and rel(vy, g * vy0) < 1e-12
+    s.close()
+
+
+def test_checkpoint_roundtrip_is_bit_exact_and_set_mask_keeps_state(ttsh):
+    import torch
+    N = 128
+    mask = workloads.disk_mask(N, N, 0.5, 20.0)
+    vel = workloads.planewave_velocity(N, N, 0.5, 9, amplitude=1.0)
+    s = ttsh.Solver(N, N, 0.5, 0.01, ttsh.baseline_params(), "f64", mask=mask)
+    s.set_velocity(*vel)
+    s.step(5)
+    n = ttsh.ttsh_state_elems(s.h)
+    buf = torch.empty(2 * n, dtype=torch.float64, device="cuda")
+    rc, mf = ttsh.ttsh_get_state(s.h, buf.data_ptr())
+    assert rc == 0
+    s.step(7)
+    a = [t.clone() for t in s.get_fields()]
+    assert ttsh.ttsh_set_state(s.h, buf.data_ptr(), mf, 0.05, 5) == 0
+    s.step(7)
+    b = s.get_fields()
+    for u, v in zip(a, b):
+        assert torch.equal(u, v)
+    # live mask change (hysteresis protocol): state carried over, K replaced
+    o = TTSHOracle(N, N, 0.5, 0.01, BASELINE_PRESET, mask=mask)
+    o.set_velocity(*vel); o.step(12)
+    mask2 = workloads.disk_mask(N, N, 0.5, 22.0)
+    s.set_mask(mask2)
+    o.K = TTSHOracle(N, N, 0.5, 0.01, BASELINE_PRESET, mask=mask2).K
+    s.step(3); o.step(3)
+    compare_state(s, o, TOL_F64_100, "after set_mask")
+    s.close()

@@ -1,0 +1,386 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the TTSH hot path in grid-point-steps/s (BASELINE.json:metric).
+
+One bench "step" = one diagnostics interval of the paper-shaped workload: 100 applications of Algorithm 1
+(rows a1-a6 of SURVEY.md §8a) followed by one ttsh_diagnostics call (row a7), on config C5 of BASELINE.json
+(4096x4096, dx=0.5, dt=1e-2, fp64, disk R=900, seeded Gaussian 1e-2 start).  `value` counts Nx*Ny*100 grid-point-steps
+per bench step, state resident in HBM.  `e2e` is the same job through the C ABI from HOST buffers: every bench
+step copies the initial velocity (pinned host memory) to the device, calls ttsh_set_velocity, runs the 100 steps
+and reads the diagnostics record back.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C5|C5-f32|C3|C3-f32|...]
+
+N > 1 (torchrun, one rank per GPU): independent replicas, no collective on the data path ("replicas only", DESIGN.md
+§9); value = units all ranks processed / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+INNER = 100   # Euler steps per bench step (diagnostics cadence of BASELINE.json configs[1])
+METRIC = "TTSH grid-point-steps/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C5")
+    ap.add_argument("--inner", type=int, default=100, help="Euler steps per bench step (profiling runs use fewer)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the 1024^2 / fp32 side measurements")
+    return ap.parse_args()
+
+
+def workload(name):
+    from paper_2304_03306_b200 import workloads
+    dtype = "f32" if name.endswith("-f32") else "f64"
+    cfg = workloads.CONFIGS[name.replace("-f32", "")]
+    return cfg, dtype
+
+
+def describe(cfg, dtype):
+    geom = {"disk": f"disk R={cfg.R:g}", "dumbbell": f"dumbbell R={cfg.R:g} d={cfg.d:g}", "none": "unconfined"}[cfg.geometry]
+    return (f"{cfg.name}: {cfg.Ny}x{cfg.Nx} grid, dx={cfg.dx}, dt={cfg.dt}, {dtype}, {geom}, lambda0=3.5 alpha=-0.5 beta=0.5 "
+            f"Gamma0=-1 Gamma2=1 gamma_v=40 gamma_w=4, Gaussian 1e-2 start, seed {cfg.seed}")
+
+
+# --------------------------------------------------------------------------------------------------
+# clocks sampling during the timed region
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.thread, self.index = [], None, None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        def pump():
+            for line in self.proc.stdout:
+                self.rows.append(line.strip())
+        self.thread = threading.Thread(target=pump, daemon=True)
+        self.thread.start()
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            parts = [p.strip() for p in r.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------------
+def oracle_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 1) for p in threadpool_info() if p.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return len(os.sched_getaffinity(0))
+
+
+def time_oracle(cfg, n_steps, budget_s, warmup=0):
+    """Times the oracle AS IT STANDS (naive-DFT transforms = explicit DFT-matrix products) on a bounded sample of
+    the workload: the same geometry family, parameters and start, on the largest grid <= the workload's whose
+    predicted cost fits the budget.  Returns (grid-point-steps/s, sample description, seconds per step)."""
+    from oracle import BASELINE_PRESET, TTSHOracle
+    from paper_2304_03306_b200 import workloads
+
+    def run(Nx, Ny, steps, wu):
+        scale = Nx / cfg.Nx
+        if cfg.geometry == "disk":
+            mask = workloads.disk_mask(Nx, Ny, cfg.dx, cfg.R * scale)
+        elif cfg.geometry == "dumbbell":
+            mask = workloads.dumbbell_mask(Nx, Ny, cfg.dx, cfg.R * scale, cfg.d * scale)
+        else:
+            mask = None
+        vx, vy = workloads.gaussian_velocity(Nx, Ny, cfg.seed, 1e-2, mask)
+        o = TTSHOracle(Nx, Ny, cfg.dx, cfg.dt, BASELINE_PRESET, mask=mask)
+        o.set_velocity(vx, vy)
+        if wu:
+            o.step(wu)
+        t0 = time.perf_counter()
+        o.step(steps)
+        return (time.perf_counter() - t0) / steps
+
+    # probe at 1/8 of the linear size (cost ~ N^3 per transform), then pick the sample grid
+    div = 8 if min(cfg.Nx, cfg.Ny) >= 512 else 1
+    t_probe = run(cfg.Nx // div, cfg.Ny // div, 1, 1)
+    f = 1
+    while f < div and t_probe * ((div // f) ** 3) * (n_steps + warmup + 1.5) > budget_s:
+        f *= 2
+    Nx, Ny = cfg.Nx // f, cfg.Ny // f
+    t_step = t_probe if f == div else run(Nx, Ny, n_steps, warmup)
+    sample = (f"{n_steps} Euler step(s) of oracle/ttsh_oracle.py (naive DFT-matrix transforms, fp64) on a {Ny}x{Nx} grid"
+              + ("" if f == 1 else f" (the {cfg.Ny}x{cfg.Nx} workload scaled by 1/{f}: same geometry family, parameters, start)"))
+    return Nx * Ny / t_step, sample, t_step
+
+
+# --------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------
+STAGE_NAMES = ["k_inv_col", "k_inv_row", "k_realspace", "k_fwd_row", "k_fwd_col", "k_spectral"]
+
+
+def stage_bytes(Nx, Ny, w):
+    """Algorithmic HBM bytes per launch of each kernel of one step: every input read once,
+    every output written once, pruned widths Wx = Nx/4+1, Hy = Ny/2+1."""
+    Wx, Hy = Nx // 4 + 1, Ny // 2 + 1
+    real, inter, spec = Nx * Ny * w, Ny * Wx * 2 * w, Hy * Wx * 2 * w
+    return {
+        "k_inv_col": spec + 4 * inter,
+        "k_inv_row": 4 * inter + 5 * real,
+        "k_realspace": 6 * real + 3 * real,
+        "k_fwd_row": 3 * real + 3 * inter,
+        "k_fwd_col": 3 * inter + 3 * spec,
+        "k_spectral": 4 * spec + spec,
+    }
+
+
+def measure(torch, ttsh, cfg, dtype, K, W, device, want_roofline=True, want_e2e=True, sampler=None):
+    import numpy as np
+    mask = cfg.mask()
+    vx0, vy0 = cfg.initial_velocity(mask)
+    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.baseline_params(), dtype, mask=mask, device=device)
+    s.set_velocity(vx0, vy0)
+    cx, cy = (cfg.Nx // 2) * cfg.dx, (cfg.Ny // 2) * cfg.dx
+    stream = torch.cuda.current_stream(device)
+
+    def bench_step():
+        s.step(INNER)
+        return s.diagnostics(cx, cy)
+
+    for _ in range(W):
+        bench_step()
+    torch.cuda.synchronize(device)
+    if sampler:
+        sampler.start()
+    l0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(K):
+        d = bench_step()
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    ms = e0.elapsed_time(e1)
+    launches = s.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    out = {"ms_total": ms, "launches": launches, "clocks": clocks, "diag": d}
+
+    if want_roofline:
+        reps = 20
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(reps)]
+        for r in range(reps):
+            for st in range(6):
+                ev[r][st].record(stream)
+                s.run_stage(st)
+            ev[r][6].record(stream)
+        torch.cuda.synchronize(device)
+        per = [sum(ev[r][st].elapsed_time(ev[r][st + 1]) for r in range(reps)) / reps for st in range(6)]
+        out["stage_ms"] = dict(zip(STAGE_NAMES, per))
+
+    if want_e2e:
+        w = 8 if dtype == "f64" else 4
+        npdt = np.float64 if dtype == "f64" else np.float32
+        hvx = torch.from_numpy(vx0.astype(npdt)).pin_memory()
+        hvy = torch.from_numpy(vy0.astype(npdt)).pin_memory()
+        dvx = torch.empty_like(hvx, device=device)
+        dvy = torch.empty_like(hvy, device=device)
+
+        def e2e_step():
+            dvx.copy_(hvx, non_blocking=True)
+            dvy.copy_(hvy, non_blocking=True)
+            rc = ttsh.ttsh_set_velocity(s.h, dvx.data_ptr(), dvy.data_ptr())
+            assert rc == 0
+            s.step(INNER)
+            return s.diagnostics(cx, cy)     # D2H of the diagnostics record + stream sync
+
+        e2e_step()
+        torch.cuda.synchronize(device)
+        ke = max(2, min(K, 3))
+        e0.record(stream)
+        for _ in range(ke):
+            e2e_step()
+        e1.record(stream)
+        torch.cuda.synchronize(device)
+        out["e2e_ms_per_step"] = e0.elapsed_time(e1) / ke
+        out["h2d"] = 2 * cfg.Nx * cfg.Ny * w
+        out["d2h"] = 8 * 8
+    s.close()
+    return out
+
+
+def main():
+    a = parse()
+    global INNER
+    INNER = a.inner
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg, dtype = workload(a.workload)
+    config = {"workload": describe(cfg, dtype), "bench_step": f"{INNER} Euler steps (Algorithm 1) + 1 diagnostics call",
+              "l2": "working set (9 fields, >1 GB at 4096^2 fp64) exceeds the 126 MB L2; no explicit flush",
+              "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)"}
+
+    # ------------------------------------------------------------------ reference arm = the oracle on host cores
+    if a.impl == "reference":
+        if rank != 0:
+            return
+        steps_total = a.steps + a.warmup
+        val, sample, t_step = time_oracle(cfg, max(1, a.steps), budget_s=150.0, warmup=min(a.warmup, 1))
+        cores = oracle_threads()
+        line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "grid-point-steps/s", "n_gpus": a.gpus,
+                "steps": a.steps, "warmup": a.warmup, "ms_per_step": 1e3 * t_step * INNER, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config,
+                "cpu_baseline": {"value": val, "unit": "grid-point-steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+                "e2e": {"value": val, "unit": "grid-point-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        _ = steps_total
+        print(json.dumps(line))
+        return
+
+    # ------------------------------------------------------------------ our arm
+    import torch
+    from paper_2304_03306_b200 import ttsh      # raises if libttsh.so is missing: no fallback
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    # replicas: each rank runs its own seed
+    if world > 1:
+        from dataclasses import replace
+        cfg = replace(cfg, index=cfg.index + 16 * rank)
+
+    def barrier():
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize(device)
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    res = measure(torch, ttsh, cfg, dtype, a.steps, a.warmup, device, sampler=sampler)
+    barrier()
+    ms = res["ms_total"]
+    e2e_ms = res["e2e_ms_per_step"]
+    launches = res["launches"]
+    if dist:
+        t = torch.tensor([ms, e2e_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = float(t[0]), float(t[1])
+        lt = torch.tensor([launches], device=device, dtype=torch.int64)
+        dist.all_reduce(lt, op=dist.ReduceOp.SUM)
+        launches = int(lt[0])
+    units = cfg.Nx * cfg.Ny * INNER * world
+    value = units * a.steps / (ms * 1e-3)
+    e2e_value = units / (e2e_ms * 1e-3)
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    w = 8 if dtype == "f64" else 4
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"
+    sb = stage_bytes(cfg.Nx, cfg.Ny, w)
+    st = res["stage_ms"]
+    dom = max(st, key=st.get)
+    achieved = sb[dom] / (st[dom] * 1e-3) / 1e9
+    step_ms = sum(st.values())
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": sb[dom],
+                "kernel_ms": st[dom], "kernel_share_of_step": st[dom] / step_ms,
+                "all_kernels": {k: {"ms": st[k], "GBps": sb[k] / (st[k] * 1e-3) / 1e9, "frac": sb[k] / (st[k] * 1e-3) / 1e9 / peak,
+                                    "bytes": sb[k]} for k in STAGE_NAMES},
+                "step_algorithmic_bytes": sum(sb.values()), "step_GBps": sum(sb.values()) / (step_ms * 1e-3) / 1e9,
+                "step_frac": sum(sb.values()) / (step_ms * 1e-3) / 1e9 / peak}
+    # traffic from the committed ncu capture, when present (profiles/ncu_traffic.json is written from an ncu --set full run)
+    try:
+        tr = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+        key = f"{dom}:{a.workload}"
+        if key in tr:
+            roofline["traffic"] = tr[key]
+    except Exception:
+        pass
+
+    line = {"metric": METRIC, "value": value, "unit": "grid-point-steps/s", "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype,
+            "data": "synthetic", "config": config, "clocks": res["clocks"],
+            "e2e": {"value": e2e_value, "unit": "grid-point-steps/s", "h2d_bytes_per_step": res["h2d"],
+                    "d2h_bytes_per_step": res["d2h"], "ms_per_step": e2e_ms},
+            "gpu_launches": launches, "roofline": roofline, "euler_step_ms": ms / a.steps / INNER}
+
+    if not a.no_extra and world == 1:
+        extra = {}
+        for name in ("C5-f32", "C3", "C3-f32", "C5p"):
+            if name == a.workload:
+                continue
+            c2, d2 = workload(name)
+            r2 = measure(torch, ttsh, c2, d2, max(2, a.steps // 2), 3, device, want_roofline=False, want_e2e=False)
+            k2 = max(2, a.steps // 2)
+            extra[name] = {"value": c2.Nx * c2.Ny * INNER * k2 / (r2["ms_total"] * 1e-3), "unit": "grid-point-steps/s",
+                           "euler_step_ms": r2["ms_total"] / k2 / INNER, "workload": describe(c2, d2)}
+        line["other_workloads"] = extra
+
+    if not a.no_cpu_baseline and world == 1:
+        val, sample, t_step = time_oracle(cfg, 1, budget_s=45.0)
+        line["cpu_baseline"] = {"value": val, "unit": "grid-point-steps/s", "cores": oracle_threads(), "kind": "oracle",
+                                "sample": sample, "seconds_per_euler_step": t_step}
+    print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

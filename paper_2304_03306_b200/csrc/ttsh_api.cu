@@ -340,11 +340,20 @@ int ttsh_step(ttsh_handle* h, int n) {
   // Small grids are launch-latency bound: replay one captured step.  Large grids launch directly.
   const bool use_graph = (size_t)h->Nx * h->Ny <= (size_t)1024 * 1024 && n >= 4;
   if (use_graph && !h->graph_ok) {
+    // capture on a private stream (the caller's may be the legacy default stream, which cannot capture);
+    // the instantiated graph is then replayed on the caller's stream.
     cudaGraph_t graph = nullptr;
+    cudaStream_t cap = nullptr;
     const long long before = h->launches;
-    TRY(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    TRY(h, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = h->stream;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) { cudaStreamDestroy(cap); return fail_cuda(h, e, "cudaStreamBeginCapture"); }
+    h->stream = cap;
     int rc = enqueue_step(h);
-    cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+    h->stream = user;
+    e = cudaStreamEndCapture(cap, &graph);
+    cudaStreamDestroy(cap);
     h->launches = before;
     if (rc != TTSH_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail_cuda(h, e, "cudaStreamEndCapture");

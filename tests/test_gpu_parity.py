@@ -216,6 +216,9 @@ def test_uniform_fixed_point_and_single_mode_on_gpu(ttsh):
     x = np.arange(N)[None, :] * dx; y = np.arange(N)[:, None] * dx
     ph = k[0] * x + k[1] * y + 0.3
     vx0 = -k[1] * 1e-3 * np.sin(ph); vy0 = k[0] * 1e-3 * np.sin(ph)
+    s.close()
+    lin = ttsh.ttsh_params(3.5, -0.5, 0.0, -1.0, 1.0, 0.0, 0.0, 1, 2)      # beta = 0: v.grad(w) == 0 for one mode, so growth is exact
+    s = ttsh.Solver(N, N, dx, dt, lin, "f64", mask=None)
     s.set_velocity(vx0, vy0)
     s.step(40)
     k2 = float(k @ k)

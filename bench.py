@@ -253,6 +253,23 @@ def measure(torch, ttsh, cfg, dtype, K, W, device, want_roofline=True, want_e2e=
     return out
 
 
+def reduce_over_ranks(dist, maxima, sums, device="cpu"):
+    """Replicas only: the job time is the MAX over ranks, counts are SUMMED.  No data-path collective."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return list(maxima), list(sums)
+    import torch
+    t = torch.tensor(list(maxima), device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor(list(sums), device=device, dtype=torch.int64)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t], [int(x) for x in c]
+
+
+def job_throughput(Nx, Ny, inner, steps, world, ms_max):
+    """Whole-job grid-point-steps/s of `world` replicas that each ran `steps` bench steps in at most ms_max."""
+    return Nx * Ny * inner * world * steps / (ms_max * 1e-3)
+
+
 def main():
     a = parse()
     global INNER
@@ -310,16 +327,9 @@ def main():
     ms = res["ms_total"]
     e2e_ms = res["e2e_ms_per_step"]
     launches = res["launches"]
-    if dist:
-        t = torch.tensor([ms, e2e_ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_ms = float(t[0]), float(t[1])
-        lt = torch.tensor([launches], device=device, dtype=torch.int64)
-        dist.all_reduce(lt, op=dist.ReduceOp.SUM)
-        launches = int(lt[0])
-    units = cfg.Nx * cfg.Ny * INNER * world
-    value = units * a.steps / (ms * 1e-3)
-    e2e_value = units / (e2e_ms * 1e-3)
+    (ms, e2e_ms), (launches,) = reduce_over_ranks(dist, [ms, e2e_ms], [launches], device)
+    value = job_throughput(cfg.Nx, cfg.Ny, INNER, a.steps, world, ms)
+    e2e_value = job_throughput(cfg.Nx, cfg.Ny, INNER, 1, world, e2e_ms)
     if rank != 0:
         if dist:
             dist.destroy_process_group()
@@ -345,12 +355,14 @@ def main():
                                     "bytes": sb[k]} for k in STAGE_NAMES},
                 "step_algorithmic_bytes": sum(sb.values()), "step_GBps": sum(sb.values()) / (step_ms * 1e-3) / 1e9,
                 "step_frac": sum(sb.values()) / (step_ms * 1e-3) / 1e9 / peak}
-    # traffic from the committed ncu capture, when present (profiles/ncu_traffic.json is written from an ncu --set full run)
+    # traffic from the committed ncu --set full capture of that kernel, when present (profiles/ncu_traffic.csv)
     try:
-        tr = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
-        key = f"{dom}:{a.workload}"
-        if key in tr:
-            roofline["traffic"] = tr[key]
+        import csv
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as fh:
+            for row in csv.DictReader(fh):
+                if row["kernel"] == dom and row["workload"] == a.workload:
+                    roofline["traffic"] = float(row["dram_bytes_per_launch"])     # latest row wins
+                    roofline["traffic_source"] = row["source"]
     except Exception:
         pass
 

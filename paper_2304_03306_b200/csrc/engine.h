@@ -7,8 +7,8 @@ namespace ttsh {
 
 // FFT passes (fft_passes.cuh).  nfields <= 5 fields per launch (grid.y).  Return cudaErrorInvalidValue for an
 // unsupported transform length.
-template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const double* v0, cudaStream_t s);
-template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, cudaStream_t s);
+template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, const double* v0, cudaStream_t s);
+template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, cudaStream_t s);
 template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const double* v0, cudaStream_t s);
 template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, cudaStream_t s);
 // set the dynamic shared-memory attribute of the pass kernels for this grid (no launch)

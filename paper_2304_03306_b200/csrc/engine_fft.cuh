@@ -12,29 +12,29 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
 }
 
 #ifdef TTSH_BUILD_COLS
-template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s) {
   using C = ColCfg<T, NY>;
   dim3 grid((g.Wx + C::L - 1) / C::L, nf);
-  k_inv_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), v0);
+  k_inv_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0);
   return cudaGetLastError();
 }
-template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s) {
   using C = ColCfg<T, NY>;
   dim3 grid((g.Wx + C::L - 1) / C::L, nf);
-  k_fwd_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab));
+  k_fwd_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS));
   return cudaGetLastError();
 }
-template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s) {
   switch (g.Ny) {
-#define X(N) case N: return go_inv_col<T, N>(g, b, nf, tab, v0, s);
+#define X(N) case N: return go_inv_col<T, N>(g, b, nf, tab, tabS, v0, s);
     TTSH_FOR_SIZES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s) {
   switch (g.Ny) {
-#define X(N) case N: return go_fwd_col<T, N>(g, b, nf, tab, s);
+#define X(N) case N: return go_fwd_col<T, N>(g, b, nf, tab, tabS, s);
     TTSH_FOR_SIZES(X)
 #undef X
   }

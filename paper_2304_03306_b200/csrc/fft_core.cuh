@@ -18,10 +18,8 @@ namespace ttsh {
 // ---------------------------------------------------------------------------------------
 // radix plans.  nstages / radix are constexpr so that they can be template arguments.
 // ---------------------------------------------------------------------------------------
-template <int N> __host__ __device__ constexpr int fft_nstages() {
-  return N <= 256 ? 2 : (N <= 4096 ? 3 : 4);
-}
-template <int N> __host__ __device__ constexpr int fft_radix(int s) {
+__host__ __device__ constexpr int fft_nstages_rt(int N) { return N <= 256 ? 2 : (N <= 4096 ? 3 : 4); }
+__host__ __device__ constexpr int fft_radix_rt(int N, int s) {
   switch (N) {
     case 32:   return s == 0 ? 8 : 4;
     case 64:   return 8;
@@ -35,6 +33,21 @@ template <int N> __host__ __device__ constexpr int fft_radix(int s) {
     default:   return 0;
   }
 }
+template <int N> __host__ __device__ constexpr int fft_nstages() { return fft_nstages_rt(N); }
+template <int N> __host__ __device__ constexpr int fft_radix(int s) { return fft_radix_rt(N, s); }
+// Per-stage twiddle tables.  Stage s >= 1 (radix R, Ns) needs w^r, r = 1..R-1, with w = W_{Ns R}^k, k = j mod Ns.  Only a
+// base set is stored and loaded — R=16: w^1, w^2, w^3, w^4, w^8, w^12;  R=8: w^1..w^4;  R=4: w^1..w^3 — laid out
+// [base][k] so that consecutive threads read consecutive entries (one coalesced request per base power); the other
+// powers are one complex product each (w^{4a+b} = w^{4a} w^b), which keeps every twiddle within ~1.5 ulp and takes the
+// twiddle traffic through L1 from 15 to 6 requests per radix-16 butterfly (L1 wavefronts were the top unit in ncu).
+__host__ __device__ constexpr int fft_tw_nbase(int R) { return R == 16 ? 6 : (R == 8 ? 4 : R - 1); }
+__host__ __device__ constexpr int fft_tw_base_power(int R, int b) { return (R == 16 && b >= 3) ? 4 * (b - 2) : b + 1; }
+__host__ __device__ constexpr int fft_tw_offset_rt(int N, int s) {
+  int off = 0, ns = fft_radix_rt(N, 0);
+  for (int t = 1; t < s; ++t) { off += fft_tw_nbase(fft_radix_rt(N, t)) * ns; ns *= fft_radix_rt(N, t); }
+  return off;
+}
+__host__ __device__ constexpr int fft_tw_elems_rt(int N) { return fft_tw_offset_rt(N, fft_nstages_rt(N)); }
 template <int N> __host__ __device__ constexpr int fft_tpl() { return N / 16; }
 template <int N> __host__ __device__ constexpr int fft_padshift() { return fft_radix<N>(0) == 16 ? 4 : 3; }
 template <int N> __host__ __device__ constexpr int fft_line_elems() { return N + (N >> fft_padshift<N>()); }
@@ -124,19 +137,77 @@ __device__ __forceinline__ cplx<float> ldg_c(const cplx<float>* p) {
   float2 t = __ldg(reinterpret_cast<const float2*>(p)); return mk<float>(t.x, t.y);
 }
 
+// strided loads of the column passes: ask L2 to fetch the whole 256-byte block around the 16/32/64 bytes this CTA
+// needs, so that DRAM sees 256-byte granules and the neighbouring CTAs (adjacent columns, running concurrently) hit L2
+__device__ __forceinline__ cplx<double> ld_l2_256(const cplx<double>* p) {
+  cplx<double> r;
+  asm volatile("ld.global.L2::256B.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ cplx<float> ld_l2_256(const cplx<float>* p) {
+  cplx<float> r;
+  asm volatile("ld.global.L2::256B.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+  return r;
+}
+
+// asynchronous L2 prefetch of a contiguous span (bytes: multiple of 16, address 16-byte aligned); costs no registers
+// and no shared memory.  Used to pull the rows of the CTA that will run about one wave later into L2, so that its
+// load phase sees L2 latency instead of DRAM latency.
+__device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 // twiddle W_M^p from the forward-sign table (M = table length), conjugated for the inverse
 template <int DIR, typename T> __device__ __forceinline__ cplx<T> twiddle(const cplx<T>* __restrict__ tab, int p) {
   cplx<T> w = ldg_c(tab + p);
   return DIR < 0 ? w : conj(w);
 }
 
+// loader = { issue(idx) -> Raw (global/shared loads only), finish(idx, Raw) -> cplx<T> }
+template <class I, class F> struct Loader {
+  I issue;
+  F finish;
+};
+template <class I, class F> __device__ __forceinline__ Loader<I, F> make_loader(I i, F f) { return Loader<I, F>{i, f}; }
+
+// fire-and-forget accumulation  *p += v  (two scalar reductions; each address receives exactly one addend per pass,
+// so the result does not depend on ordering)
+__device__ __forceinline__ void red_add(cplx<double>* p, cplx<double> v) {
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&p->x), "d"(v.x) : "memory");
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&p->y), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void red_add(cplx<float>* p, cplx<float> v) {
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(&p->x), "f"(v.x) : "memory");
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(&p->y), "f"(v.y) : "memory");
+}
+
+// v[r] *= w^r, r = 1..R-1, from the base powers stored at tw[b * ns]
+template <int R, int DIR, typename T>
+__device__ __forceinline__ void apply_stage_twiddles(cplx<T>* v, const cplx<T>* __restrict__ tw, int ns) {
+  if constexpr (R == 16) {
+    const cplx<T> w1 = twiddle<DIR>(tw, 0), w2 = twiddle<DIR>(tw, ns), w3 = twiddle<DIR>(tw, 2 * ns);
+    const cplx<T> w4 = twiddle<DIR>(tw, 3 * ns), w8 = twiddle<DIR>(tw, 4 * ns), w12 = twiddle<DIR>(tw, 5 * ns);
+    v[1] = v[1] * w1;   v[2] = v[2] * w2;   v[3] = v[3] * w3;   v[4] = v[4] * w4;   v[8] = v[8] * w8;   v[12] = v[12] * w12;
+    v[5] = v[5] * (w4 * w1);   v[6] = v[6] * (w4 * w2);   v[7] = v[7] * (w4 * w3);
+    v[9] = v[9] * (w8 * w1);   v[10] = v[10] * (w8 * w2); v[11] = v[11] * (w8 * w3);
+    v[13] = v[13] * (w12 * w1); v[14] = v[14] * (w12 * w2); v[15] = v[15] * (w12 * w3);
+  } else if constexpr (R == 8) {
+    const cplx<T> w1 = twiddle<DIR>(tw, 0), w2 = twiddle<DIR>(tw, ns), w3 = twiddle<DIR>(tw, 2 * ns), w4 = twiddle<DIR>(tw, 3 * ns);
+    v[1] = v[1] * w1; v[2] = v[2] * w2; v[3] = v[3] * w3; v[4] = v[4] * w4;
+    v[5] = v[5] * (w4 * w1); v[6] = v[6] * (w4 * w2); v[7] = v[7] * (w4 * w3);
+  } else {
+#pragma unroll
+    for (int r = 1; r < R; ++r) v[r] = v[r] * twiddle<DIR>(tw, (r - 1) * ns);
+  }
+}
+
 // ---------------------------------------------------------------------------------------
 // one line.  j = thread index within the line's TPL threads; sm = this line's padded buffer.
-// TS = stride into the twiddle table (table length = N * TS).
+// tab = the per-stage twiddle tables of length N (fft_tw_offset_rt).
 // SYNC_LAST: the last-stage store goes to shared memory, so it needs the read/write barrier too.
 // EVERY thread of the CTA must call this (it contains __syncthreads()).
 // ---------------------------------------------------------------------------------------
-template <typename T, int N, int DIR, int TS, int S, int NS, bool SYNC_LAST, class Load, class Store>
+template <typename T, int N, int DIR, int S, int NS, bool SYNC_LAST, class Load, class Store>
 __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab,
                                           Load& load, Store& store) {
   constexpr int R = fft_radix<N>(S);
@@ -145,13 +216,24 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
   constexpr int TPL = fft_tpl<N>();
   constexpr int NB = (N / R) / TPL;         // butterflies per thread: 16 / R
   cplx<T> v[NB][R];
+  if constexpr (first) {
+    // two-phase load: issue every global load of this thread first (all in flight together), then finish
+    // (multipliers, packing).  Without this split ptxas interleaves loads with their dependent arithmetic.
+    decltype(load.issue(0)) raw[NB][R];
 #pragma unroll
-  for (int b = 0; b < NB; ++b) {
-    const int j = j0 + b * TPL;
+    for (int b = 0; b < NB; ++b)
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      const int idx = j + r * (N / R);
-      v[b][r] = first ? load(idx) : sm[fft_pad<N>(idx)];
+      for (int r = 0; r < R; ++r) raw[b][r] = load.issue(j0 + b * TPL + r * (N / R));
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+#pragma unroll
+      for (int r = 0; r < R; ++r) v[b][r] = load.finish(j0 + b * TPL + r * (N / R), raw[b][r]);
+  } else {
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      const int j = j0 + b * TPL;
+#pragma unroll
+      for (int r = 0; r < R; ++r) v[b][r] = sm[fft_pad<N>(j + r * (N / R))];
     }
   }
 #pragma unroll
@@ -160,7 +242,7 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
     if (NS > 1) {
       const int k = j & (NS - 1);
 #pragma unroll
-      for (int r = 1; r < R; ++r) v[b][r] = v[b][r] * twiddle<DIR>(tab, k * r * ((N / (NS * R)) * TS));
+      apply_stage_twiddles<R, DIR>(v[b], tab + fft_tw_offset_rt(N, S) + k, NS);
     }
     dftR<R, DIR>(v[b]);
   }
@@ -179,14 +261,14 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
   }
   if constexpr (!last) {
     __syncthreads();
-    fft_stage<T, N, DIR, TS, S + 1, NS * R, SYNC_LAST>(j0, sm, tab, load, store);
+    fft_stage<T, N, DIR, S + 1, NS * R, SYNC_LAST>(j0, sm, tab, load, store);
   }
 }
 
-template <typename T, int N, int DIR, int TS, bool SYNC_LAST, class Load, class Store>
+template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store>
 __device__ __forceinline__ void fft_line(int j, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab,
                                          Load load, Store store) {
-  fft_stage<T, N, DIR, TS, 0, 1, SYNC_LAST>(j, sm, tab, load, store);
+  fft_stage<T, N, DIR, 0, 1, SYNC_LAST>(j, sm, tab, load, store);
 }
 
 }  // namespace ttsh

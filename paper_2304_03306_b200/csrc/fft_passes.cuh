@@ -14,6 +14,15 @@
 // are applied while loading, so the derivative fields never exist in spectral form in HBM.
 #pragma once
 #include "fft_core.cuh"
+#ifndef TTSH_PF_DIST
+#define TTSH_PF_DIST 296
+#endif
+#ifndef TTSH_ROW_MINB
+#define TTSH_ROW_MINB 2
+#endif
+#ifndef TTSH_COL_ELEMS
+#define TTSH_COL_ELEMS 4096
+#endif
 
 namespace ttsh {
 
@@ -26,13 +35,13 @@ template <typename T, int NX> struct RowCfg {
   static constexpr int THREADS = L * TPL;
   static constexpr int LS = fft_line_elems<NX>() + 4;                          // line stride (elements)
   static constexpr size_t SMEM = (size_t)L * LS * sizeof(cplx<T>);
-  static constexpr int MINB = THREADS <= 256 ? 2 : 1;                          // caps registers at 128/thread
+  static constexpr int MINB = THREADS <= 256 ? TTSH_ROW_MINB : 1;              // caps registers per thread
 };
 template <typename T, int NY> struct ColCfg {
   static constexpr int NH = NY / 2;
   static constexpr int TPL = fft_tpl<NH>();
   static constexpr int LMAX = sizeof(T) == 8 ? 8 : 8;
-  static constexpr int LBUDGET = (int)(4096 * 16 / sizeof(cplx<T>)) / NH;     // keep L*NH*sizeof <= 64 KiB
+  static constexpr int LBUDGET = (int)(TTSH_COL_ELEMS * 16 / sizeof(cplx<T>)) / NH;     // keep L*NH*sizeof <= 64 KiB
   static constexpr int L = LBUDGET < 1 ? 1 : (LBUDGET > LMAX ? LMAX : LBUDGET); // adjacent columns per CTA
   static constexpr int THREADS = L * TPL;
   static constexpr int LS = fft_line_elems<NH>() + (sizeof(T) == 8 ? 8 / (L > 8 ? 8 : L) : 16 / (L > 16 ? 16 : L));
@@ -60,7 +69,8 @@ __device__ __forceinline__ cplx<T> apply_spec_mode(int mode, cplx<T> w, int mx, 
 // ---------------------------------------------------------------------------------------
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
-k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY, const double* __restrict__ v0) {
+k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
+          const cplx<T>* __restrict__ tabS, const double* __restrict__ v0) {
   using C = ColCfg<T, NY>;
   constexpr int NH = C::NH, L = C::L;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -78,24 +88,31 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
-    auto load = [&](int mp) -> cplx<T> {
-      cplx<T> a = mk<T>(0, 0);
-      if (valid) {
-        if (mp <= My) a = apply_spec_mode<T>(mode, src[(size_t)mp * Wxp + mx], mx, mp, g, v0);
-        if (NH - mp <= My) {                       // my = mp - NH < 0, stored at row Hy + my
-          const int my = mp - NH;
-          cplx<T> b = apply_spec_mode<T>(mode, src[(size_t)(Hy + my) * Wxp + mx], mx, my, g, v0);
-          a = p ? a - b : a + b;
-        }
-        if (p) a = mul_conj(a, ldg_c(tabY + mp));   // * W_Ny^{-mp}  (inverse sign)
-        a = scale * a;
-      }
-      return a;
+    // a_p[mp] = (X[mp] + (-1)^p X[mp+NH]) W_Ny^{-p mp}; X[mp] is retained iff mp <= My, X[mp+NH] (my = mp-NH) iff
+    // NH-mp <= My.  With the 1/2 rule both hold only at mp = NH/2, so one load per point is issued up front and the
+    // rare second term is fetched in finish().
+    auto issue = [&](int mp) -> cplx<T> {
+      const bool use1 = mp <= My, use2 = NH - mp <= My;
+      const int q = use1 ? mp : Hy + mp - NH;
+      return (valid && (use1 || use2)) ? ld_l2_256(src + (size_t)q * Wxp + mx) : mk<T>(0, 0);
     };
+    auto finish = [&](int mp, cplx<T> raw) -> cplx<T> {
+      const bool use1 = mp <= My, use2 = NH - mp <= My;
+      if (!valid || !(use1 || use2)) return mk<T>(0, 0);
+      cplx<T> a = apply_spec_mode<T>(mode, raw, mx, use1 ? mp : mp - NH, g, v0);
+      if (!use1 && p) a = mk<T>(-a.x, -a.y);
+      if (use1 && use2) {
+        const cplx<T> b = apply_spec_mode<T>(mode, src[(size_t)(Hy + mp - NH) * Wxp + mx], mx, mp - NH, g, v0);
+        a = p ? a - b : a + b;
+      }
+      if (p) a = mul_conj(a, ldg_c(tabS + mp));   // * W_Ny^{-mp}  (inverse sign)
+      return scale * a;
+    };
+    auto load = make_loader(issue, finish);
     auto store = [&](int yp, cplx<T> val) {
       if (valid) dst[(size_t)(2 * yp + p) * Wxp + mx] = val;
     };
-    fft_line<T, NH, +1, 2, false>(j, line, tabY, load, store);
+    fft_line<T, NH, +1, false>(j, line, tabY, load, store);
   }
 }
 
@@ -104,7 +121,8 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 // ---------------------------------------------------------------------------------------
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
-k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY) {
+k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
+          const cplx<T>* __restrict__ tabS) {
   using C = ColCfg<T, NY>;
   constexpr int NH = C::NH, L = C::L;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -121,21 +139,22 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
-    auto load = [&](int yp) -> cplx<T> {
-      return valid ? scale * src[(size_t)(2 * yp + p) * Wxp + mx] : mk<T>(0, 0);
-    };
+    auto load = make_loader(
+        [&](int yp) -> cplx<T> { return valid ? ld_l2_256(src + (size_t)(2 * yp + p) * Wxp + mx) : mk<T>(0, 0); },
+        [&](int, cplx<T> raw) -> cplx<T> { return scale * raw; });
     auto store = [&](int mp, cplx<T> val) {
       if (!valid) return;
       if (p == 0) {
         if (mp <= My) dst[(size_t)mp * Wxp + mx] = val;
         if (NH - mp <= My) dst[(size_t)(Hy + mp - NH) * Wxp + mx] = val;
       } else {
-        const cplx<T> t = val * ldg_c(tabY + mp);                 // W_Ny^{mp} O[mp];  W_Ny^{mp+NH} = -W_Ny^{mp}
-        if (mp <= My) { cplx<T>* q = dst + (size_t)mp * Wxp + mx; *q = *q + t; }
-        if (NH - mp <= My) { cplx<T>* q = dst + (size_t)(Hy + mp - NH) * Wxp + mx; *q = *q - t; }
+        const cplx<T> t = val * ldg_c(tabS + mp);                 // W_Ny^{mp} O[mp];  W_Ny^{mp+NH} = -W_Ny^{mp}
+        // fire-and-forget reductions instead of read-modify-write: no L2 round trip on the critical path
+        if (mp <= My) red_add(dst + (size_t)mp * Wxp + mx, t);
+        if (NH - mp <= My) red_add(dst + (size_t)(Hy + mp - NH) * Wxp + mx, mk<T>(-t.x, -t.y));
       }
     };
-    fft_line<T, NH, -1, 2, false>(j, line, tabY, load, store);
+    fft_line<T, NH, -1, false>(j, line, tabY, load, store);
   }
 }
 
@@ -161,6 +180,13 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const T scale = (T)g.inv_sqrt_nx;
   const T dkx = (T)g.dkx;
   const T meany = (mode == RM_NIKX_MEANY) ? (T)(v0[1] * g.inv_sqrt_ny) : (T)0;
+  if (threadIdx.x == 0) {
+    int nb = blockIdx.x + TTSH_PF_DIST, ny = blockIdx.y;
+    if (nb >= (int)gridDim.x) { nb -= gridDim.x; ny += 1; }
+    if (ny < (int)gridDim.y && nb < (int)gridDim.x)
+      prefetch_l2_bulk(static_cast<const cplx<T>*>(batch.f[ny].src) + (size_t)(2 * nb * C::L) * Wxp,
+                       2 * C::L * Wxp * sizeof(cplx<T>));
+  }
 
   auto mult = [&](cplx<T> a, int mx) -> cplx<T> {
     if (mode == RM_ONE) return a;
@@ -168,21 +194,30 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     if (mode == RM_IKX) return kx * mul_i(a);
     return mx == 0 ? mk<T>(meany, (T)0) : kx * mul_ni(a);        // RM_NIKX_MEANY
   };
-  auto load = [&](int m) -> cplx<T> {
+  struct RawAB { cplx<T> a, b; };
+  auto issue = [&](int m) -> RawAB {
+    const int mx = m > NX / 2 ? NX - m : m;
+    RawAB r;
+    r.a = mk<T>(0, 0); r.b = mk<T>(0, 0);
+    if (mx < Wx) { r.a = srcA[mx]; r.b = srcB[mx]; }
+    return r;
+  };
+  auto finish = [&](int m, RawAB r) -> cplx<T> {
     // Z(m) = A(m) + i B(m) with A, B the Hermitian x-spectra of the two real rows
     const bool neg = m > NX / 2;
     const int mx = neg ? NX - m : m;
     if (mx >= Wx) return mk<T>(0, 0);
-    cplx<T> a = mult(srcA[mx], mx), b = mult(srcB[mx], mx);
+    cplx<T> a = mult(r.a, mx), b = mult(r.b, mx);
     if (mx == 0) { a.y = 0; b.y = 0; }             // Re[] of the oracle's complex iDFT: drop the anti-Hermitian part
     if (neg) { a = conj(a); b = conj(b); }
     return scale * mk<T>(a.x - b.y, a.y + b.x);
   };
+  auto load = make_loader(issue, finish);
   auto store = [&](int x, cplx<T> z) {
     dstA[x] = z.x;
     dstB[x] = z.y;
   };
-  fft_line<T, NX, +1, 1, false>(j, sm + c * C::LS, tabX, load, store);
+  fft_line<T, NX, +1, false>(j, sm + c * C::LS, tabX, load, store);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -205,10 +240,17 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   cplx<T>* __restrict__ dstB = dstA + Wxp;
   const T scale = (T)g.inv_sqrt_nx;
   cplx<T>* line = sm + c * C::LS;
+  if (threadIdx.x == 0) {   // L2 prefetch for the CTA that runs ~one wave later (C::L row pairs = 2 L contiguous rows)
+    int nb = blockIdx.x + TTSH_PF_DIST, ny = blockIdx.y;
+    if (nb >= (int)gridDim.x) { nb -= gridDim.x; ny += 1; }
+    if (ny < (int)gridDim.y && nb < (int)gridDim.x)
+      prefetch_l2_bulk(static_cast<const T*>(batch.f[ny].src) + (size_t)(2 * nb * C::L) * NX, 2 * C::L * NX * sizeof(T));
+  }
 
-  auto load = [&](int x) -> cplx<T> { return mk<T>(scale * srcA[x], scale * srcB[x]); };
+  auto load = make_loader([&](int x) -> cplx<T> { return mk<T>(srcA[x], srcB[x]); },
+                          [&](int, cplx<T> raw) -> cplx<T> { return scale * raw; });
   auto store = [&](int m, cplx<T> z) { line[fft_pad<NX>(m)] = z; };
-  fft_line<T, NX, -1, 1, true>(j, line, tabX, load, store);
+  fft_line<T, NX, -1, true>(j, line, tabX, load, store);
   __syncthreads();
   // unpack: A(m) = (Z(m) + conj Z(-m))/2,  B(m) = -i (Z(m) - conj Z(-m))/2,  m = 0..Wx-1
   for (int mx = j; mx < Wx; mx += TPL) {

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "engine.h"
+#include "fft_core.cuh"
 
 using namespace ttsh;
 
@@ -21,7 +22,7 @@ inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 inline bool pow2_in_range(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
 
 struct Layout {
-  size_t tabX, tabY, K, what, v0, diag_partial, diag_out, R[5], Tm[4], S[3], total;
+  size_t tabX, tabY, tabS, K, what, v0, diag_partial, diag_out, R[5], Tm[4], S[3], total;
 };
 
 Geom make_geom(int Nx, int Ny, double dx, int num, int den) {
@@ -51,6 +52,7 @@ Layout make_layout(int Nx, int Ny, size_t w) {
   auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
   L.tabX = take((size_t)Nx * cw);
   L.tabY = take((size_t)Ny * cw);
+  L.tabS = take((size_t)Ny * cw);
   L.K = take(P * w);
   L.what = take(spec);
   L.v0 = take(8 * sizeof(double));
@@ -74,7 +76,7 @@ struct ttsh_handle {
   Model m;
   cudaStream_t stream;
   char* ws;
-  void *tabX, *tabY, *K, *what, *R[5], *Tm[4], *S[3];
+  void *tabX, *tabY, *tabS, *K, *what, *R[5], *Tm[4], *S[3];
   double *v0, *diag_partial, *diag_out;
   bool initialized;
   double t;
@@ -102,18 +104,35 @@ int fail_cuda(ttsh_handle* h, cudaError_t e, const char* what) {
   return TTSH_ERR_CUDA;
 }
 
-template <typename T> void fill_table(std::vector<unsigned char>& buf, int N) {
-  buf.resize((size_t)N * 2 * sizeof(T));
-  T* t = reinterpret_cast<T*>(buf.data());
+// forward-sign twiddle W_M^p = exp(-2 pi i p / M), evaluated in long double, exact on the axes
+template <typename T> void put_twiddle(T* t, long long p, long long M) {
+  p %= M;
   const long double two_pi = 2.0L * acosl(-1.0L);
-  for (int p = 0; p < N; ++p) {   // forward sign: W_N^p = exp(-2 pi i p / N); octant-exact special values
-    long double a = two_pi * (long double)p / (long double)N;
-    long double c = cosl(a), s = -sinl(a);
-    if (4 * p == N || 4 * p == 3 * N) c = 0.0L;
-    if (p == 0 || 2 * p == N) s = 0.0L;
-    t[2 * p] = (T)c;
-    t[2 * p + 1] = (T)s;
+  long double a = two_pi * (long double)p / (long double)M;
+  long double c = cosl(a), s = -sinl(a);
+  if (4 * p == M || 4 * p == 3 * M) c = 0.0L;
+  if (p == 0 || 2 * p == M) s = 0.0L;
+  t[0] = (T)c;
+  t[1] = (T)s;
+}
+// per-stage tables of a length-N transform (layout: fft_core.cuh, fft_tw_offset_rt)
+template <typename T> void fill_stage_tables(std::vector<unsigned char>& buf, int N) {
+  buf.assign((size_t)(fft_tw_elems_rt(N) + 1) * 2 * sizeof(T), 0);
+  T* t = reinterpret_cast<T*>(buf.data());
+  int ns = fft_radix_rt(N, 0);
+  for (int s = 1; s < fft_nstages_rt(N); ++s) {
+    const int R = fft_radix_rt(N, s), off = fft_tw_offset_rt(N, s);
+    for (int b = 0; b < fft_tw_nbase(R); ++b)
+      for (int k = 0; k < ns; ++k)
+        put_twiddle<T>(t + 2 * (size_t)(off + b * ns + k), (long long)k * fft_tw_base_power(R, b), (long long)ns * R);
+    ns *= R;
   }
+}
+// split twiddles of the column pass: W_Ny^p, p < Ny/2
+template <typename T> void fill_split_table(std::vector<unsigned char>& buf, int Ny) {
+  buf.assign((size_t)(Ny / 2) * 2 * sizeof(T), 0);
+  T* t = reinterpret_cast<T*>(buf.data());
+  for (int p = 0; p < Ny / 2; ++p) put_twiddle<T>(t + 2 * (size_t)p, p, Ny);
 }
 
 // ---- dtype dispatch helpers ---------------------------------------------------------------
@@ -139,7 +158,7 @@ int enqueue_inverse(ttsh_handle* h, void* w, void* gx, void* gy, void* vx, void*
   if (need_psi) cb.f[nc++] = op(h->what, h->Tm[2], SM_PSI);
   if (need_vx) cb.f[nc++] = op(h->what, h->Tm[3], SM_IKY_PSI_MEANX);
   if (nc == 0) return TTSH_OK;
-  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->v0, h->stream));
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->tabS, h->v0, h->stream));
   h->launches++;
   // row pass; psi and v_y share the intermediate psi~, so psi (if requested) goes in a second launch slot
   Batch rb; memset(&rb, 0, sizeof(rb));
@@ -170,7 +189,7 @@ int enqueue_forward(ttsh_handle* h, int n, const void* const* src) {
     cb.f[i] = op(h->Tm[i], h->S[i], 0);
   }
   TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, n, h->tabX, h->stream));
-  TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, n, h->tabY, h->stream));
+  TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, n, h->tabY, h->tabS, h->stream));
   h->launches += 2;
   return TTSH_OK;
 }
@@ -180,7 +199,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     case TTSH_STAGE_INV_COL: {
       Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->what, h->Tm[1], SM_IKY), op(h->what, h->Tm[2], SM_PSI),
                              op(h->what, h->Tm[3], SM_IKY_PSI_MEANX)});
-      TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 4, h->tabY, h->v0, h->stream));
+      TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 4, h->tabY, h->tabS, h->v0, h->stream));
       h->launches++;
       return TTSH_OK;
     }
@@ -203,7 +222,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     }
     case TTSH_STAGE_FWD_COL: {
       Batch cb = make_batch({op(h->Tm[0], h->S[0], 0), op(h->Tm[1], h->S[1], 0), op(h->Tm[2], h->S[2], 0)});
-      TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 3, h->tabY, h->stream));
+      TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 3, h->tabY, h->tabS, h->stream));
       h->launches++;
       return TTSH_OK;
     }
@@ -245,7 +264,7 @@ int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   int rc = enqueue_forward(h, 1, src);
   if (rc != TTSH_OK) return rc;
   Batch cb = make_batch({op(h->S[0], h->Tm[0], SM_LOWPASS4)});
-  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 1, h->tabY, h->v0, h->stream));
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 1, h->tabY, h->tabS, h->v0, h->stream));
   Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE)});
   TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 1, h->tabX, h->v0, h->stream));
   TRY(h, DISPATCH(h, launch_square, P, h->R[0], h->K, h->stream));
@@ -288,7 +307,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->m.Gamma2 = p->Gamma2; h->m.gamma_v = p->gamma_v; h->m.gamma_w = p->gamma_w; h->m.dt = dt;
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   h->ws = static_cast<char*>(workspace);
-  h->tabX = h->ws + L.tabX; h->tabY = h->ws + L.tabY; h->K = h->ws + L.K; h->what = h->ws + L.what;
+  h->tabX = h->ws + L.tabX; h->tabY = h->ws + L.tabY; h->tabS = h->ws + L.tabS; h->K = h->ws + L.K; h->what = h->ws + L.what;
   h->v0 = reinterpret_cast<double*>(h->ws + L.v0);
   h->diag_partial = reinterpret_cast<double*>(h->ws + L.diag_partial);
   h->diag_out = reinterpret_cast<double*>(h->ws + L.diag_out);
@@ -299,11 +318,12 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->graph_exec = nullptr; h->graph_ok = false;
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
-  std::vector<unsigned char> tx, ty;
-  if (t == TTSH_F64) { fill_table<double>(tx, Nx); fill_table<double>(ty, Ny); }
-  else { fill_table<float>(tx, Nx); fill_table<float>(ty, Ny); }
+  std::vector<unsigned char> tx, ty, ts;
+  if (t == TTSH_F64) { fill_stage_tables<double>(tx, Nx); fill_stage_tables<double>(ty, Ny / 2); fill_split_table<double>(ts, Ny); }
+  else { fill_stage_tables<float>(tx, Nx); fill_stage_tables<float>(ty, Ny / 2); fill_split_table<float>(ts, Ny); }
   TRY(h, cudaMemcpyAsync(h->tabX, tx.data(), tx.size(), cudaMemcpyHostToDevice, h->stream));
   TRY(h, cudaMemcpyAsync(h->tabY, ty.data(), ty.size(), cudaMemcpyHostToDevice, h->stream));
+  TRY(h, cudaMemcpyAsync(h->tabS, ts.data(), ts.size(), cudaMemcpyHostToDevice, h->stream));
   TRY(h, cudaMemsetAsync(h->v0, 0, 8 * sizeof(double), h->stream));
   TRY(h, cudaStreamSynchronize(h->stream));   // the host tables go out of scope below
   TRY(h, DISPATCH(h, prepare_rows, h->g));

@@ -163,7 +163,8 @@ template <int DIR, typename T> __device__ __forceinline__ cplx<T> twiddle(const 
   return DIR < 0 ? w : conj(w);
 }
 
-// loader = { issue(idx) -> Raw (global/shared loads only), finish(idx, Raw) -> cplx<T> }
+// loader = { issue(idx, k) -> Raw (global/shared loads only), finish(idx, k, Raw) -> cplx<T> } with idx = j + k TPL;
+// the slot k = 0..15 is a compile-time constant after unrolling, so loaders can prune by k at compile time
 template <class I, class F> struct Loader {
   I issue;
   F finish;
@@ -171,14 +172,16 @@ template <class I, class F> struct Loader {
 template <class I, class F> __device__ __forceinline__ Loader<I, F> make_loader(I i, F f) { return Loader<I, F>{i, f}; }
 
 // fire-and-forget accumulation  *p += v  (two scalar reductions; each address receives exactly one addend per pass,
-// so the result does not depend on ordering)
+// so the result does not depend on ordering).  No "memory" clobber on purpose: the asm is volatile (never dropped),
+// the preceding plain store of the same thread to the same address is separated from it by a __syncthreads, and a
+// clobber would stop ptxas from hoisting the twiddle loads of the neighbouring outputs above it.
 __device__ __forceinline__ void red_add(cplx<double>* p, cplx<double> v) {
-  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&p->x), "d"(v.x) : "memory");
-  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&p->y), "d"(v.y) : "memory");
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&p->x), "d"(v.x));
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&p->y), "d"(v.y));
 }
 __device__ __forceinline__ void red_add(cplx<float>* p, cplx<float> v) {
-  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(&p->x), "f"(v.x) : "memory");
-  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(&p->y), "f"(v.y) : "memory");
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(&p->x), "f"(v.x));
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(&p->y), "f"(v.y));
 }
 
 // v[r] *= w^r, r = 1..R-1, from the base powers stored at tw[b * ns]
@@ -219,15 +222,15 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
   if constexpr (first) {
     // two-phase load: issue every global load of this thread first (all in flight together), then finish
     // (multipliers, packing).  Without this split ptxas interleaves loads with their dependent arithmetic.
-    decltype(load.issue(0)) raw[NB][R];
+    decltype(load.issue(0, 0)) raw[NB][R];
 #pragma unroll
     for (int b = 0; b < NB; ++b)
 #pragma unroll
-      for (int r = 0; r < R; ++r) raw[b][r] = load.issue(j0 + b * TPL + r * (N / R));
+      for (int r = 0; r < R; ++r) raw[b][r] = load.issue(j0 + (b + r * NB) * TPL, b + r * NB);
 #pragma unroll
     for (int b = 0; b < NB; ++b)
 #pragma unroll
-      for (int r = 0; r < R; ++r) v[b][r] = load.finish(j0 + b * TPL + r * (N / R), raw[b][r]);
+      for (int r = 0; r < R; ++r) v[b][r] = load.finish(j0 + (b + r * NB) * TPL, b + r * NB, raw[b][r]);
   } else {
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
@@ -241,7 +244,6 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
     const int j = j0 + b * TPL;
     if (NS > 1) {
       const int k = j & (NS - 1);
-#pragma unroll
       apply_stage_twiddles<R, DIR>(v[b], tab + fft_tw_offset_rt(N, S) + k, NS);
     }
     dftR<R, DIR>(v[b]);

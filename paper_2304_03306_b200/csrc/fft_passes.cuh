@@ -1,17 +1,20 @@
 // fft_passes.cuh — the four passes of the pruned 2-D R2C / C2R transforms (PAPER.md:319 defines the DFT).
 //
-//   inverse:  pruned spectrum [Hy][Wxp] --inv_col--> intermediate [Ny][Wxp] --inv_row--> real [Ny][Nx]
-//   forward:  real [Ny][Nx] --fwd_row--> intermediate [Ny][Wxp] --fwd_col--> pruned spectrum [Hy][Wxp]
+//   inverse:  pruned spectrum --k_inv_col--> intermediate --k_inv_row--> real [Ny][Nx]
+//   forward:  real [Ny][Nx] --k_fwd_row--> intermediate --k_fwd_col--> pruned spectrum
+//   (tile-major layouts of the two complex arrays: ttsh_common.cuh)
 //
-// Row passes pack two real rows (y, y+1) of one field into one complex length-Nx FFT
-// (z = row_y + i row_{y+1}); all global accesses are unit-stride in x.
+// Row passes pack two real rows of one field (same parity: y = 4a+p and 4a+p+2) into one complex length-Nx FFT
+// (z = row_A + i row_B); the real side is unit-stride, the intermediate side moves (A, B) pairs with one
+// 32-byte (fp64, LDG.256/STG.256) or 16-byte (fp32) access per thread, 2 CW elements contiguous per tile.
 // Column passes never hold a full column: because at most Ny/2+1 of the Ny y-wavenumbers are retained,
 // the length-Ny transform is split by the parity p of y into two length-Ny/2 transforms
 //   inverse:  f[2y'+p] = Ny^-1/2 sum_{m'} (X[m'] + (-1)^p X[m'+Ny/2]) W_Ny^{-p m'} W_{Ny/2}^{-m' y'}
 //   forward:  X[m]     = Ny^-1/2 (E[m mod Ny/2] + W_Ny^m O[m mod Ny/2]),  E/O = FFT_{Ny/2} of the even/odd rows
-// so a CTA needs only L * Ny/2 complex values of shared memory for L adjacent columns (L * 16 B or L * 8 B
-// contiguous per row in HBM).  Multipliers (i k_y, 1/k^2, i k_x, the low-pass of Algorithm 2, the mean flow)
-// are applied while loading, so the derivative fields never exist in spectral form in HBM.
+// so a CTA needs CW * Ny/2 complex values of shared memory for its CW adjacent columns, and — the arrays being
+// tile-major — every global access of a column CTA is `base + threadIdx.x + r * blockDim.x`: fully coalesced.
+// Multipliers (i k_y, 1/k^2, i k_x, the low-pass of Algorithm 2, the mean flow) are applied while loading, so the
+// derivative fields never exist in spectral form in HBM.
 #pragma once
 #include "fft_core.cuh"
 #ifndef TTSH_PF_DIST
@@ -20,8 +23,8 @@
 #ifndef TTSH_ROW_MINB
 #define TTSH_ROW_MINB 2
 #endif
-#ifndef TTSH_COL_ELEMS
-#define TTSH_COL_ELEMS 4096
+#ifndef TTSH_COL_BYTES
+#define TTSH_COL_BYTES 65536
 #endif
 
 namespace ttsh {
@@ -37,121 +40,179 @@ template <typename T, int NX> struct RowCfg {
   static constexpr size_t SMEM = (size_t)L * LS * sizeof(cplx<T>);
   static constexpr int MINB = THREADS <= 256 ? TTSH_ROW_MINB : 1;              // caps registers per thread
 };
+// columns per CTA of the column pass = tile width CW of the two complex arrays: CW * Ny/2 complex values near 64 KiB
+// of shared memory (fp64 4096: 2 columns, fp32 4096: 4), at least 2 and at most 8 columns
+__host__ __device__ constexpr int col_tile_width(int Ny, int elem_bytes) {
+  int cw = (TTSH_COL_BYTES / elem_bytes) / (Ny / 2);
+  return cw < 2 ? 2 : (cw > 8 ? 8 : cw);
+}
 template <typename T, int NY> struct ColCfg {
   static constexpr int NH = NY / 2;
   static constexpr int TPL = fft_tpl<NH>();
-  static constexpr int LMAX = sizeof(T) == 8 ? 8 : 8;
-  static constexpr int LBUDGET = (int)(TTSH_COL_ELEMS * 16 / sizeof(cplx<T>)) / NH;     // keep L*NH*sizeof <= 64 KiB
-  static constexpr int L = LBUDGET < 1 ? 1 : (LBUDGET > LMAX ? LMAX : LBUDGET); // adjacent columns per CTA
+  static constexpr int L = col_tile_width(NY, (int)sizeof(cplx<T>));
+  static constexpr int LSHIFT = L == 2 ? 1 : (L == 4 ? 2 : 3);
   static constexpr int THREADS = L * TPL;
-  static constexpr int LS = fft_line_elems<NH>() + (sizeof(T) == 8 ? 8 / (L > 8 ? 8 : L) : 16 / (L > 16 ? 16 : L));
+  static constexpr int LS = fft_line_elems<NH>() + 8 / L;
   static constexpr size_t SMEM = (size_t)L * LS * sizeof(cplx<T>);
   static constexpr int MINB = THREADS <= 256 ? 2 : 1;
 };
 
-// spectral multiplier of the inverse column pass (SpecMode), computed from integer wavenumber indices
+// 2-element (A, B) pair access of the row passes
+template <typename T> struct Pair { cplx<T> a, b; };
+__device__ __forceinline__ Pair<double> ld_pair(const cplx<double>* p) {
+  Pair<double> r;
+  asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.a.x), "=d"(r.a.y), "=d"(r.b.x), "=d"(r.b.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ Pair<float> ld_pair(const cplx<float>* p) {
+  Pair<float> r;
+  asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.a.x), "=f"(r.a.y), "=f"(r.b.x), "=f"(r.b.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_pair(cplx<double>* p, cplx<double> a, cplx<double> b) {
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y));
+}
+__device__ __forceinline__ void st_pair(cplx<float>* p, cplx<float> a, cplx<float> b) {
+  asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+}
+
+// spectral multiplier of the inverse column pass (SpecMode).  mode is uniform per CTA, kx and kx^2 per thread.
 template <typename T>
-__device__ __forceinline__ cplx<T> apply_spec_mode(int mode, cplx<T> w, int mx, int my, const Geom& g, const double* v0) {
+__device__ __forceinline__ cplx<T> apply_spec_mode(int mode, cplx<T> w, int mx, int my, T kx2, const Geom& g, const double* v0) {
   if (mode == SM_ONE) return w;
-  const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my);
+  const T ky = (T)g.dky * (T)my;
   if (mode == SM_IKY) return ky * mul_i(w);
   if (mode == SM_LOWPASS4) return is_cut(mx, my, g.Nx, g.Ny, 1, 4) ? mk<T>(0, 0) : w;
   const bool zero = (mx == 0 && my == 0);
-  const T ik2 = zero ? (T)0 : (T)1 / (kx * kx + ky * ky);
-  if (mode == SM_PSI) return ik2 * w;
+  const T ik2 = (T)1 / (zero ? (T)1 : kx2 + ky * ky);
+  if (mode == SM_PSI) return zero ? mk<T>(0, 0) : ik2 * w;
   /* SM_IKY_PSI_MEANX */
-  if (zero) return mk<T>((T)v0[0], (T)0);
-  return (ky * ik2) * mul_i(w);
+  return zero ? mk<T>((T)v0[0], (T)0) : (ky * ik2) * mul_i(w);
+}
+
+// thread -> (FFT index j, column c) of a column CTA: threadIdx.x enumerates the intermediate block [Ny/4][CW][2] in
+// memory order, e = (a CW + c) 2 + b, j = 2a + b, so that element y' = j + r TPL of column c is at e + r blockDim.x.
+template <int LSHIFT> __device__ __forceinline__ void col_thread_map(int e, int& j, int& c) {
+  c = (e >> 1) & ((1 << LSHIFT) - 1);
+  j = ((e >> (1 + LSHIFT)) << 1) | (e & 1);
 }
 
 // ---------------------------------------------------------------------------------------
-// inverse column pass
+// inverse column pass.  grid = (NT tiles, fields)
 // ---------------------------------------------------------------------------------------
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
 k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
           const cplx<T>* __restrict__ tabS, const double* __restrict__ v0) {
   using C = ColCfg<T, NY>;
-  constexpr int NH = C::NH, L = C::L;
+  constexpr int NH = C::NH, L = C::L, TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
-  const int c = threadIdx.x % L, j = threadIdx.x / L;
-  const int mx = blockIdx.x * L + c;
+  int j, c;
+  col_thread_map<C::LSHIFT>(threadIdx.x, j, c);
+  const int t = blockIdx.x;
+  const int mx = t * L + c;
   const bool valid = mx < g.Wx;
   const FieldOp op = batch.f[blockIdx.y];
-  const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src);
-  cplx<T>* __restrict__ dst = static_cast<cplx<T>*>(op.dst);
+  const int My = g.My, Hy = g.Hy;
+  const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * Hy * L + c;   // (q, c) at q L
+  cplx<T>* __restrict__ dst = static_cast<cplx<T>*>(op.dst) + (size_t)t * 2 * NH * L + threadIdx.x;
   const int mode = op.mode;
   const T scale = (T)g.inv_sqrt_ny;
-  const int My = g.My, Hy = g.Hy, Wxp = g.Wxp;
   cplx<T>* line = sm + c * C::LS;
+
+  const T kx = (T)g.dkx * (T)mx;
+  const T kx2 = kx * kx;
+  const bool half_rule = (2 * My == NH);     // the paper's 1/2 rule: |my| <= Ny/4 (uniform branch)
 
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
     // a_p[mp] = (X[mp] + (-1)^p X[mp+NH]) W_Ny^{-p mp}; X[mp] is retained iff mp <= My, X[mp+NH] (my = mp-NH) iff
-    // NH-mp <= My.  With the 1/2 rule both hold only at mp = NH/2, so one load per point is issued up front and the
-    // rare second term is fetched in finish().
-    auto issue = [&](int mp) -> cplx<T> {
-      const bool use1 = mp <= My, use2 = NH - mp <= My;
-      const int q = use1 ? mp : Hy + mp - NH;
-      return (valid && (use1 || use2)) ? ld_l2_256(src + (size_t)q * Wxp + mx) : mk<T>(0, 0);
-    };
-    auto finish = [&](int mp, cplx<T> raw) -> cplx<T> {
-      const bool use1 = mp <= My, use2 = NH - mp <= My;
-      if (!valid || !(use1 || use2)) return mk<T>(0, 0);
-      cplx<T> a = apply_spec_mode<T>(mode, raw, mx, use1 ? mp : mp - NH, g, v0);
-      if (!use1 && p) a = mk<T>(-a.x, -a.y);
-      if (use1 && use2) {
-        const cplx<T> b = apply_spec_mode<T>(mode, src[(size_t)(Hy + mp - NH) * Wxp + mx], mx, mp - NH, g, v0);
-        a = p ? a - b : a + b;
-      }
+    // NH-mp <= My.
+    // output element y' = j + k TPL of column c -> dst + p NH L + k blockDim (see col_thread_map); tail columns of the
+    // last tile are written too (zeros), the row pass never reads them
+    cplx<T>* out = dst + (size_t)p * NH * L;
+    auto store = [&](int yp, cplx<T> val) { out[(size_t)((yp - j) / TPL) * (L * TPL)] = val; };
+    auto twist = [&](int mp, cplx<T> a) -> cplx<T> {
       if (p) a = mul_conj(a, ldg_c(tabS + mp));   // * W_Ny^{-mp}  (inverse sign)
       return scale * a;
     };
-    auto load = make_loader(issue, finish);
-    auto store = [&](int yp, cplx<T> val) {
-      if (valid) dst[(size_t)(2 * yp + p) * Wxp + mx] = val;
-    };
-    fft_line<T, NH, +1, false>(j, line, tabY, load, store);
+    if (half_rule) {
+      // My = NH/2 = 8 TPL: slot k < 8 holds X[mp] only, k > 8 holds X[mp+NH] only, k = 8 holds X[mp+NH] plus, for the
+      // single point mp = NH/2 (j = 0), X[NH/2]: the selection is a compile-time function of the slot.
+      auto issue = [&](int mp, int k) -> cplx<T> {
+        const int q = k < 8 ? mp : Hy + mp - NH;
+        return valid ? src[(size_t)q * L] : mk<T>(0, 0);
+      };
+      auto finish = [&](int mp, int k, cplx<T> raw) -> cplx<T> {
+        if (!valid) return mk<T>(0, 0);
+        cplx<T> v = apply_spec_mode<T>(mode, raw, mx, k < 8 ? mp : mp - NH, kx2, g, v0);
+        if (k >= 8 && p) v = mk<T>(-v.x, -v.y);
+        if (k == 8 && j == 0) v = v + apply_spec_mode<T>(mode, src[(size_t)mp * L], mx, mp, kx2, g, v0);
+        return twist(mp, v);
+      };
+      fft_line<T, NH, +1, false>(j, line, tabY, make_loader(issue, finish), store);
+    } else {
+      // general dealias fraction: one load per point up front, the (possibly common) second term in finish()
+      auto issue = [&](int mp, int) -> cplx<T> {
+        const bool use1 = mp <= My, use2 = NH - mp <= My;
+        const int q = use1 ? mp : Hy + mp - NH;
+        return (valid && (use1 || use2)) ? src[(size_t)q * L] : mk<T>(0, 0);
+      };
+      auto finish = [&](int mp, int, cplx<T> raw) -> cplx<T> {
+        const bool use1 = mp <= My, use2 = NH - mp <= My;
+        if (!valid || !(use1 || use2)) return mk<T>(0, 0);
+        cplx<T> v = apply_spec_mode<T>(mode, raw, mx, use1 ? mp : mp - NH, kx2, g, v0);
+        if (!use1 && p) v = mk<T>(-v.x, -v.y);
+        if (use1 && use2) {
+          const cplx<T> b = apply_spec_mode<T>(mode, src[(size_t)(Hy + mp - NH) * L], mx, mp - NH, kx2, g, v0);
+          v = p ? v - b : v + b;
+        }
+        return twist(mp, v);
+      };
+      fft_line<T, NH, +1, false>(j, line, tabY, make_loader(issue, finish), store);
+    }
   }
 }
 
 // ---------------------------------------------------------------------------------------
-// forward column pass
+// forward column pass.  grid = (NT tiles, fields)
 // ---------------------------------------------------------------------------------------
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
 k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
           const cplx<T>* __restrict__ tabS) {
   using C = ColCfg<T, NY>;
-  constexpr int NH = C::NH, L = C::L;
+  constexpr int NH = C::NH, L = C::L, TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
-  const int c = threadIdx.x % L, j = threadIdx.x / L;
-  const int mx = blockIdx.x * L + c;
-  const bool valid = mx < g.Wx;
+  int j, c;
+  col_thread_map<C::LSHIFT>(threadIdx.x, j, c);
+  const int t = blockIdx.x;
+  const bool valid = t * L + c < g.Wx;
   const FieldOp op = batch.f[blockIdx.y];
-  const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src);
-  cplx<T>* dst = static_cast<cplx<T>*>(op.dst);
+  const int My = g.My, Hy = g.Hy;
+  const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * 2 * NH * L + threadIdx.x;
+  cplx<T>* dst = static_cast<cplx<T>*>(op.dst) + (size_t)t * Hy * L + c;
   const T scale = (T)g.inv_sqrt_ny;
-  const int My = g.My, Hy = g.Hy, Wxp = g.Wxp;
   cplx<T>* line = sm + c * C::LS;
 
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
+    const cplx<T>* in = src + (size_t)p * NH * L;
     auto load = make_loader(
-        [&](int yp) -> cplx<T> { return valid ? ld_l2_256(src + (size_t)(2 * yp + p) * Wxp + mx) : mk<T>(0, 0); },
-        [&](int, cplx<T> raw) -> cplx<T> { return scale * raw; });
+        [&](int, int k) -> cplx<T> { return valid ? in[(size_t)k * (L * TPL)] : mk<T>(0, 0); },
+        [&](int, int, cplx<T> raw) -> cplx<T> { return scale * raw; });
     auto store = [&](int mp, cplx<T> val) {
       if (!valid) return;
       if (p == 0) {
-        if (mp <= My) dst[(size_t)mp * Wxp + mx] = val;
-        if (NH - mp <= My) dst[(size_t)(Hy + mp - NH) * Wxp + mx] = val;
+        if (mp <= My) dst[(size_t)mp * L] = val;
+        if (NH - mp <= My) dst[(size_t)(Hy + mp - NH) * L] = val;
       } else {
-        const cplx<T> t = val * ldg_c(tabS + mp);                 // W_Ny^{mp} O[mp];  W_Ny^{mp+NH} = -W_Ny^{mp}
+        const cplx<T> tw = val * ldg_c(tabS + mp);                // W_Ny^{mp} O[mp];  W_Ny^{mp+NH} = -W_Ny^{mp}
         // fire-and-forget reductions instead of read-modify-write: no L2 round trip on the critical path
-        if (mp <= My) red_add(dst + (size_t)mp * Wxp + mx, t);
-        if (NH - mp <= My) red_add(dst + (size_t)(Hy + mp - NH) * Wxp + mx, mk<T>(-t.x, -t.y));
+        if (mp <= My) red_add(dst + (size_t)mp * L, tw);
+        if (NH - mp <= My) red_add(dst + (size_t)(Hy + mp - NH) * L, mk<T>(-tw.x, -tw.y));
       }
     };
     fft_line<T, NH, -1, false>(j, line, tabY, load, store);
@@ -159,58 +220,51 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 }
 
 // ---------------------------------------------------------------------------------------
-// inverse row pass (C2R, two rows per complex transform)
+// inverse row pass (C2R, two rows per complex transform).  grid = (Ny/2 / L row pairs, fields)
 // ---------------------------------------------------------------------------------------
 template <typename T, int NX>
 __global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
-k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabX, const double* __restrict__ v0) {
+k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabX,
+          const double* __restrict__ v0) {
   using C = RowCfg<T, NX>;
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
   const int c = threadIdx.x / TPL, j = threadIdx.x % TPL;
-  const int rp = blockIdx.x * C::L + c;             // row pair; Ny/2 is a multiple of L
+  const int rp = blockIdx.x * C::L + c;             // row pair: rows yA = 4a+p, yB = yA+2; Ny/2 is a multiple of L
+  const int a = rp >> 1, p = rp & 1;
   const FieldOp op = batch.f[blockIdx.y];
-  const int Wx = g.Wx, Wxp = g.Wxp;
-  const cplx<T>* __restrict__ srcA = static_cast<const cplx<T>*>(op.src) + (size_t)(2 * rp) * Wxp;
-  const cplx<T>* __restrict__ srcB = srcA + Wxp;
-  T* __restrict__ dstA = static_cast<T*>(op.dst) + (size_t)(2 * rp) * NX;
-  T* __restrict__ dstB = dstA + NX;
+  const int Wx = g.Wx;
+  const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src);
+  T* __restrict__ dstA = static_cast<T*>(op.dst) + (size_t)(4 * a + p) * NX;
+  T* __restrict__ dstB = dstA + 2 * NX;
   const int mode = op.mode;
   const T scale = (T)g.inv_sqrt_nx;
   const T dkx = (T)g.dkx;
   const T meany = (mode == RM_NIKX_MEANY) ? (T)(v0[1] * g.inv_sqrt_ny) : (T)0;
-  if (threadIdx.x == 0) {
-    int nb = blockIdx.x + TTSH_PF_DIST, ny = blockIdx.y;
-    if (nb >= (int)gridDim.x) { nb -= gridDim.x; ny += 1; }
-    if (ny < (int)gridDim.y && nb < (int)gridDim.x)
-      prefetch_l2_bulk(static_cast<const cplx<T>*>(batch.f[ny].src) + (size_t)(2 * nb * C::L) * Wxp,
-                       2 * C::L * Wxp * sizeof(cplx<T>));
-  }
 
-  auto mult = [&](cplx<T> a, int mx) -> cplx<T> {
-    if (mode == RM_ONE) return a;
+  auto mult = [&](cplx<T> w, int mx) -> cplx<T> {
+    if (mode == RM_ONE) return w;
     const T kx = dkx * (T)mx;
-    if (mode == RM_IKX) return kx * mul_i(a);
-    return mx == 0 ? mk<T>(meany, (T)0) : kx * mul_ni(a);        // RM_NIKX_MEANY
+    if (mode == RM_IKX) return kx * mul_i(w);
+    return mx == 0 ? mk<T>(meany, (T)0) : kx * mul_ni(w);        // RM_NIKX_MEANY
   };
-  struct RawAB { cplx<T> a, b; };
-  auto issue = [&](int m) -> RawAB {
+  auto issue = [&](int m, int) -> Pair<T> {
     const int mx = m > NX / 2 ? NX - m : m;
-    RawAB r;
+    if (mx < Wx) return ld_pair(src + inter_pair_index(g, a, p, mx));
+    Pair<T> r;
     r.a = mk<T>(0, 0); r.b = mk<T>(0, 0);
-    if (mx < Wx) { r.a = srcA[mx]; r.b = srcB[mx]; }
     return r;
   };
-  auto finish = [&](int m, RawAB r) -> cplx<T> {
+  auto finish = [&](int m, int, Pair<T> r) -> cplx<T> {
     // Z(m) = A(m) + i B(m) with A, B the Hermitian x-spectra of the two real rows
     const bool neg = m > NX / 2;
     const int mx = neg ? NX - m : m;
     if (mx >= Wx) return mk<T>(0, 0);
-    cplx<T> a = mult(r.a, mx), b = mult(r.b, mx);
-    if (mx == 0) { a.y = 0; b.y = 0; }             // Re[] of the oracle's complex iDFT: drop the anti-Hermitian part
-    if (neg) { a = conj(a); b = conj(b); }
-    return scale * mk<T>(a.x - b.y, a.y + b.x);
+    cplx<T> wa = mult(r.a, mx), wb = mult(r.b, mx);
+    if (mx == 0) { wa.y = 0; wb.y = 0; }           // Re[] of the oracle's complex iDFT: drop the anti-Hermitian part
+    if (neg) { wa = conj(wa); wb = conj(wb); }
+    return scale * mk<T>(wa.x - wb.y, wa.y + wb.x);
   };
   auto load = make_loader(issue, finish);
   auto store = [&](int x, cplx<T> z) {
@@ -221,7 +275,7 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 }
 
 // ---------------------------------------------------------------------------------------
-// forward row pass (R2C, two rows per complex transform)
+// forward row pass (R2C, two rows per complex transform).  grid = (Ny/2 / L row pairs, fields)
 // ---------------------------------------------------------------------------------------
 template <typename T, int NX>
 __global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
@@ -232,23 +286,24 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
   const int c = threadIdx.x / TPL, j = threadIdx.x % TPL;
   const int rp = blockIdx.x * C::L + c;
+  const int a = rp >> 1, p = rp & 1;
   const FieldOp op = batch.f[blockIdx.y];
-  const int Wx = g.Wx, Wxp = g.Wxp;
-  const T* __restrict__ srcA = static_cast<const T*>(op.src) + (size_t)(2 * rp) * NX;
-  const T* __restrict__ srcB = srcA + NX;
-  cplx<T>* __restrict__ dstA = static_cast<cplx<T>*>(op.dst) + (size_t)(2 * rp) * Wxp;
-  cplx<T>* __restrict__ dstB = dstA + Wxp;
+  const int Wx = g.Wx;
+  const T* __restrict__ srcA = static_cast<const T*>(op.src) + (size_t)(4 * a + p) * NX;
+  const T* __restrict__ srcB = srcA + 2 * NX;
+  cplx<T>* __restrict__ dst = static_cast<cplx<T>*>(op.dst);
   const T scale = (T)g.inv_sqrt_nx;
   cplx<T>* line = sm + c * C::LS;
-  if (threadIdx.x == 0) {   // L2 prefetch for the CTA that runs ~one wave later (C::L row pairs = 2 L contiguous rows)
+  if (threadIdx.x == 0) {   // L2 prefetch of the rows of the CTA pair that runs about one wave later (4 consecutive rows)
     int nb = blockIdx.x + TTSH_PF_DIST, ny = blockIdx.y;
     if (nb >= (int)gridDim.x) { nb -= gridDim.x; ny += 1; }
-    if (ny < (int)gridDim.y && nb < (int)gridDim.x)
-      prefetch_l2_bulk(static_cast<const T*>(batch.f[ny].src) + (size_t)(2 * nb * C::L) * NX, 2 * C::L * NX * sizeof(T));
+    if (ny < (int)gridDim.y && ((nb * C::L) & 1) == 0)
+      prefetch_l2_bulk(static_cast<const T*>(batch.f[ny].src) + (size_t)(2 * nb * C::L) * NX,
+                       (C::L >= 2 ? 2 * C::L : 4) * NX * sizeof(T));
   }
 
-  auto load = make_loader([&](int x) -> cplx<T> { return mk<T>(srcA[x], srcB[x]); },
-                          [&](int, cplx<T> raw) -> cplx<T> { return scale * raw; });
+  auto load = make_loader([&](int x, int) -> cplx<T> { return mk<T>(srcA[x], srcB[x]); },
+                          [&](int, int, cplx<T> raw) -> cplx<T> { return scale * raw; });
   auto store = [&](int m, cplx<T> z) { line[fft_pad<NX>(m)] = z; };
   fft_line<T, NX, -1, true>(j, line, tabX, load, store);
   __syncthreads();
@@ -256,8 +311,7 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   for (int mx = j; mx < Wx; mx += TPL) {
     const cplx<T> zp = line[fft_pad<NX>(mx)];
     const cplx<T> zm = conj(line[fft_pad<NX>((NX - mx) & (NX - 1))]);
-    dstA[mx] = (T)0.5 * (zp + zm);
-    dstB[mx] = (T)0.5 * mul_ni(zp - zm);
+    st_pair(dst + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
   }
 }
 

@@ -19,12 +19,12 @@ template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m
 }
 template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
                                                   void* w, double* v0, cudaStream_t s) {
-  dim3 grid((g.Wx + 255) / 256, g.Hy);
+  const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
   k_spectral<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, v0);
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, double* v0, cudaStream_t s) {
-  dim3 grid((g.Wx + 255) / 256, g.Hy);
+  const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
   k_spectral_init<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)Vx, (const cplx<T>*)Vy, (cplx<T>*)w, v0);
   return cudaGetLastError();
 }

@@ -47,7 +47,7 @@ k_realspace(size_t nvec, Model m, const T* __restrict__ vx, const T* __restrict_
 }
 
 // ---------------------------------------------------------------------------------------
-// a5: fused spectral kernel on the pruned spectrum [Hy][Wxp].
+// a5: fused spectral kernel on the tile-major pruned spectrum (spec_index).
 //   w^_naive = exp(sigma dt) (w^ + dt (i kx F^y - i ky F^x + S^))                       (lines 3-4)
 //   k = 0:   w^ = 0,  v^(0) <- exp(-alpha dt) (v^(0) + dt F^(0))                         (lines 6-8, Eq. C1)
 //   cut:     w^ = 0                                                                       (lines 9-11)
@@ -72,11 +72,15 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __restrict__ Fy,
            const cplx<T>* __restrict__ S, cplx<T>* w, double* v0) {
-  const int mx = blockIdx.x * blockDim.x + threadIdx.x;
-  const int q = blockIdx.y;
+  // threads enumerate the tile-major array in memory order: idx = (t Hy + q) CW + c
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
+  const int t = (int)(idx / ((size_t)g.Hy * g.CW));
+  const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
+  const int q = rem >> g.cw_shift;
+  const int mx = t * g.CW + (rem & (g.CW - 1));
   if (mx >= g.Wx) return;
   const int my = q <= g.My ? q : q - g.Hy;
-  const size_t idx = (size_t)q * g.Wxp + mx;
   const bool zero = (mx == 0 && my == 0);
   const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
   if (mx == 0) {
@@ -89,7 +93,7 @@ k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __res
       w[idx] = mk<T>(0, 0);
       return;
     }
-    const size_t idn = (size_t)(g.Hy - my) * g.Wxp;       // row of -my, mx = 0
+    const size_t idn = spec_index(g, g.Hy - my, 0);       // row of -my, mx = 0
     cplx<T> out = mk<T>(0, 0);
     if (!cut) {
       const cplx<T> a = naive_update<T>(g, m, 0, my, idx, Fx, Fy, S, w);
@@ -108,11 +112,15 @@ k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __res
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_spectral_init(Geom g, const cplx<T>* __restrict__ Vx, const cplx<T>* __restrict__ Vy, cplx<T>* w, double* v0) {
-  const int mx = blockIdx.x * blockDim.x + threadIdx.x;
-  const int q = blockIdx.y;
+  // threads enumerate the tile-major array in memory order: idx = (t Hy + q) CW + c
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
+  const int t = (int)(idx / ((size_t)g.Hy * g.CW));
+  const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
+  const int q = rem >> g.cw_shift;
+  const int mx = t * g.CW + (rem & (g.CW - 1));
   if (mx >= g.Wx) return;
   const int my = q <= g.My ? q : q - g.Hy;
-  const size_t idx = (size_t)q * g.Wxp + mx;
   const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
   auto curl = [&](int my_, size_t id) -> cplx<T> {
     const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my_);
@@ -126,7 +134,7 @@ k_spectral_init(Geom g, const cplx<T>* __restrict__ Vx, const cplx<T>* __restric
       w[idx] = mk<T>(0, 0);
       return;
     }
-    const size_t idn = (size_t)(g.Hy - my) * g.Wxp;
+    const size_t idn = spec_index(g, g.Hy - my, 0);
     cplx<T> out = mk<T>(0, 0);
     if (!cut) out = (T)0.5 * (curl(my, idx) + conj(curl(-my, idn)));
     w[idx] = out;

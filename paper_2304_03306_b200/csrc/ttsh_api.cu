@@ -10,7 +10,7 @@
 #include <vector>
 
 #include "engine.h"
-#include "fft_core.cuh"
+#include "fft_passes.cuh"
 
 using namespace ttsh;
 
@@ -25,12 +25,14 @@ struct Layout {
   size_t tabX, tabY, tabS, K, what, v0, diag_partial, diag_out, R[5], Tm[4], S[3], total;
 };
 
-Geom make_geom(int Nx, int Ny, double dx, int num, int den) {
+Geom make_geom(int Nx, int Ny, double dx, int num, int den, size_t w) {
   Geom g;
   g.Nx = Nx; g.Ny = Ny;
   g.num = num; g.den = den;
   g.Wx = (int)((long long)num * Nx / (2LL * den)) + 1;
-  g.Wxp = (g.Wx + 7) / 8 * 8;
+  g.CW = col_tile_width(Ny, (int)(2 * w));
+  g.cw_shift = g.CW == 2 ? 1 : (g.CW == 4 ? 2 : 3);
+  g.NT = (g.Wx + g.CW - 1) / g.CW;
   g.My = (int)((long long)num * Ny / (2LL * den));
   g.Hy = 2 * g.My + 1;
   const long double two_pi = 2.0L * acosl(-1.0L);
@@ -44,9 +46,9 @@ Geom make_geom(int Nx, int Ny, double dx, int num, int den) {
 // The workspace is sized for the widest dealias fraction the ABI accepts (2/3), so that
 // ttsh_workspace_bytes does not depend on the parameters.
 Layout make_layout(int Nx, int Ny, size_t w) {
-  const Geom g = make_geom(Nx, Ny, 1.0, 2, 3);
+  const Geom g = make_geom(Nx, Ny, 1.0, 2, 3, w);
   const size_t P = (size_t)Nx * Ny, cw = 2 * w;
-  const size_t inter = (size_t)Ny * g.Wxp * cw, spec = (size_t)g.Hy * g.Wxp * cw;
+  const size_t inter = (size_t)g.NT * g.CW * Ny * cw, spec = (size_t)g.NT * g.CW * g.Hy * cw;
   Layout L;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -302,7 +304,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   ttsh_handle* h = new (std::nothrow) ttsh_handle();
   if (!h) return TTSH_ERR_INVALID_ARG;
   h->Nx = Nx; h->Ny = Ny; h->dx = dx; h->dt = dt; h->p = *p; h->dtype = t;
-  h->g = make_geom(Nx, Ny, dx, p->dealias_num, p->dealias_den);
+  h->g = make_geom(Nx, Ny, dx, p->dealias_num, p->dealias_den, (size_t)t);
   h->m.lambda0 = p->lambda0; h->m.alpha = p->alpha; h->m.beta = p->beta; h->m.Gamma0 = p->Gamma0;
   h->m.Gamma2 = p->Gamma2; h->m.gamma_v = p->gamma_v; h->m.gamma_w = p->gamma_w; h->m.dt = dt;
   h->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -403,7 +405,7 @@ int ttsh_get_fields(ttsh_handle* h, void* vx, void* vy, void* omega, void* psi) 
   return enqueue_inverse(h, omega, nullptr, nullptr, vx, vy, psi);
 }
 
-size_t ttsh_state_elems(const ttsh_handle* h) { return h ? (size_t)h->g.Hy * h->g.Wxp : 0; }
+size_t ttsh_state_elems(const ttsh_handle* h) { return h ? (size_t)h->g.NT * h->g.CW * h->g.Hy : 0; }
 
 int ttsh_get_state(ttsh_handle* h, void* w_hat, double* mean_flow) {
   if (!h || !w_hat || !mean_flow) return TTSH_ERR_INVALID_ARG;

@@ -30,21 +30,40 @@ template <typename T> __device__ __forceinline__ cplx<T> mul_conj(cplx<T> a, cpl
 }
 
 // ---------------------------------------------------------------------------------------
-// grid geometry (host-filled, passed by value)
-//   real fields      scalar[Ny][Nx]
-//   x-pruned, y-real  cplx[Ny][Wxp]    ("intermediate": x-spectral mx = 0..Wx-1, y in real space)
-//   pruned spectrum   cplx[Hy][Wxp]    row q <-> my = q (q <= My) or q - Hy (q > My); mx = 0..Wx-1
-// Wx-1 = floor(num*Nx/(2*den)) and My = floor(num*Ny/(2*den)) bound the retained modes of the
-// circular cutoff k^2 <= ((num/den) pi/dx)^2; nothing outside is ever non-zero.
+// grid geometry (host-filled, passed by value) and the HBM layouts
+//
+//   real fields       scalar[Ny][Nx], x contiguous.
+//   retained modes    mx = 0..Wx-1 (Wx-1 = floor(num Nx / 2 den)), |my| <= My = floor(num Ny / 2 den): nothing outside
+//                     is ever non-zero under the circular cutoff k^2 <= ((num/den) pi/dx)^2.
+//                     Spectrum row q <-> my = q (q <= My) or q - Hy (q > My), Hy = 2 My + 1.
+//   column tiles      the retained x-wavenumbers are grouped in NT tiles of CW adjacent columns (CW = the number of
+//                     columns one CTA of the column pass transforms; a power of two).  Both complex arrays are
+//                     TILE-MAJOR, so that a column CTA streams one contiguous block and never makes a strided access:
+//   pruned spectrum   cplx[NT][Hy][CW]                      element (q, mx):  ((mx/CW) Hy + q) CW + mx%CW
+//   intermediate      cplx[NT][2][Ny/4][CW][2]              (x-spectral, y real).  Row y = 4a + p + 2b (p = parity,
+//                     b = 0/1) of column mx sits at  (((mx/CW) 2 + p) Ny/4 + a) 2 CW + 2 (mx%CW) + b:
+//                     rows are split by parity p (the column pass transforms even and odd rows separately) and the
+//                     two same-parity rows 4a+p, 4a+p+2 that one row-pass FFT packs together are adjacent, so the row
+//                     pass moves (A, B) pairs with single 32-byte (fp64) / 16-byte (fp32) accesses in pieces of
+//                     2 CW elements, and the column pass block [Ny/2][CW] is contiguous.
 // ---------------------------------------------------------------------------------------
 struct Geom {
   int Nx, Ny;
-  int Wx, Wxp;
+  int Wx;                  // retained x-wavenumbers
+  int CW, cw_shift, NT;    // tile width (columns), log2, number of tiles = ceil(Wx / CW)
   int My, Hy;
   int num, den;            // dealias fraction
   double dkx, dky;         // 2 pi / (Nx dx), 2 pi / (Ny dx)   (Table I)
   double inv_sqrt_nx, inv_sqrt_ny;
 };
+
+__host__ __device__ __forceinline__ size_t spec_index(const Geom& g, int q, int mx) {
+  return ((size_t)(mx >> g.cw_shift) * g.Hy + q) * g.CW + (mx & (g.CW - 1));
+}
+// index of the (A, B) pair (rows 4a+p and 4a+p+2) of column mx; B is the next element
+__host__ __device__ __forceinline__ size_t inter_pair_index(const Geom& g, int a, int p, int mx) {
+  return ((((size_t)(mx >> g.cw_shift) * 2 + p) * (g.Ny >> 2) + a) * g.CW + (mx & (g.CW - 1))) * 2;
+}
 
 // strict '>' cutoff evaluated exactly in integers (reading R4):
 //   k^2 > ((num/den) pi/dx)^2   <=>   4 den^2 ((mx Ny)^2 + (my Nx)^2) > num^2 (Nx Ny)^2

@@ -88,6 +88,27 @@ template <int DIR, int n, typename T> __device__ __forceinline__ cplx<T> mul_w16
   return mk<T>(a.x * c - a.y * s, a.x * s + a.y * c);
 }
 
+// a * W_32^k, k = 0..15 (compile-time k): the split twiddles of the column passes factor as W_Ny^{j + k Ny/32} = W_Ny^j W_32^k
+template <int DIR, int k, typename T> __device__ __forceinline__ cplx<T> mul_w32(cplx<T> a) {
+  constexpr double C[16] = {1.0000000000000000000000000000000000, 0.9807852804032304491261822361342390, 0.9238795325112867561281831893967883, 0.8314696123025452370787883776179058, 0.7071067811865475244008443621048490, 0.5555702330196022247428308139485329, 0.3826834323650897717284599840303989, 0.1950903220161282678482848684770222, 0.0000000000000000000000000000000000, -0.1950903220161282678482848684770222, -0.3826834323650897717284599840303989, -0.5555702330196022247428308139485329, -0.7071067811865475244008443621048490, -0.8314696123025452370787883776179058, -0.9238795325112867561281831893967883, -0.9807852804032304491261822361342390};
+  constexpr double S[16] = {0.0000000000000000000000000000000000, 0.1950903220161282678482848684770222, 0.3826834323650897717284599840303989, 0.5555702330196022247428308139485329, 0.7071067811865475244008443621048490, 0.8314696123025452370787883776179058, 0.9238795325112867561281831893967883, 0.9807852804032304491261822361342390, 1.0000000000000000000000000000000000, 0.9807852804032304491261822361342390, 0.9238795325112867561281831893967883, 0.8314696123025452370787883776179058, 0.7071067811865475244008443621048490, 0.5555702330196022247428308139485329, 0.3826834323650897717284599840303989, 0.1950903220161282678482848684770222};
+  if constexpr (k == 0) return a;
+  else if constexpr (k == 8) return mul_w4<DIR>(a);
+  else {
+    constexpr T c = (T)C[k], s = (T)(DIR < 0 ? -S[k] : S[k]);
+    return mk<T>(a.x * c - a.y * s, a.x * s + a.y * c);
+  }
+}
+template <int DIR, typename T> __device__ __forceinline__ cplx<T> mul_w32_rt(cplx<T> a, int k) {   // k constant after unrolling
+  switch (k) {
+#define TTSH_W32(K) case K: return mul_w32<DIR, K>(a);
+    TTSH_W32(0) TTSH_W32(1) TTSH_W32(2) TTSH_W32(3) TTSH_W32(4) TTSH_W32(5) TTSH_W32(6) TTSH_W32(7)
+    TTSH_W32(8) TTSH_W32(9) TTSH_W32(10) TTSH_W32(11) TTSH_W32(12) TTSH_W32(13) TTSH_W32(14) TTSH_W32(15)
+#undef TTSH_W32
+  }
+  return a;
+}
+
 template <int DIR, typename T> __device__ __forceinline__ void dft8(cplx<T>* v) {
   // s = 2 s1 + s2, r = r1 + 4 r2:  W_8^{rs} = W_4^{r1 s1} W_8^{r1 s2} W_2^{r2 s2}
   dft4<DIR>(v[0], v[2], v[4], v[6]);
@@ -165,11 +186,14 @@ template <int DIR, typename T> __device__ __forceinline__ cplx<T> twiddle(const 
 
 // loader = { issue(idx, k) -> Raw (global/shared loads only), finish(idx, k, Raw) -> cplx<T> } with idx = j + k TPL;
 // the slot k = 0..15 is a compile-time constant after unrolling, so loaders can prune by k at compile time
-template <class I, class F> struct Loader {
+template <int B, class I, class F> struct Loader {
+  static constexpr int BATCHES = B;
   I issue;
   F finish;
 };
-template <class I, class F> __device__ __forceinline__ Loader<I, F> make_loader(I i, F f) { return Loader<I, F>{i, f}; }
+template <int B = 1, class I, class F> __device__ __forceinline__ Loader<B, I, F> make_loader(I i, F f) {
+  return Loader<B, I, F>{i, f};
+}
 
 // fire-and-forget accumulation  *p += v  (two scalar reductions; each address receives exactly one addend per pass,
 // so the result does not depend on ordering).  No "memory" clobber on purpose: the asm is volatile (never dropped),
@@ -222,15 +246,24 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
   if constexpr (first) {
     // two-phase load: issue every global load of this thread first (all in flight together), then finish
     // (multipliers, packing).  Without this split ptxas interleaves loads with their dependent arithmetic.
-    decltype(load.issue(0, 0)) raw[NB][R];
+    // Load::BATCHES = 2 splits the 16 slots into k < 8 and k >= 8 (two round trips, half the raw registers: for loaders
+    // whose raw record is 32 bytes the single batch spilled, and a spill of a just-loaded value stalls on its load).
+    constexpr int NBAT = Load::BATCHES;
+    constexpr int SLOTS = NB * R;
 #pragma unroll
-    for (int b = 0; b < NB; ++b)
+    for (int bat = 0; bat < NBAT; ++bat) {
+      decltype(load.issue(0, 0)) raw[SLOTS / NBAT];
 #pragma unroll
-      for (int r = 0; r < R; ++r) raw[b][r] = load.issue(j0 + (b + r * NB) * TPL, b + r * NB);
+      for (int s = 0; s < SLOTS / NBAT; ++s) {
+        const int k = bat * (SLOTS / NBAT) + s;
+        raw[s] = load.issue(j0 + k * TPL, k);
+      }
 #pragma unroll
-    for (int b = 0; b < NB; ++b)
-#pragma unroll
-      for (int r = 0; r < R; ++r) v[b][r] = load.finish(j0 + (b + r * NB) * TPL, b + r * NB, raw[b][r]);
+      for (int s = 0; s < SLOTS / NBAT; ++s) {
+        const int k = bat * (SLOTS / NBAT) + s;      // slot k = b + r NB  <->  v[b][r]
+        v[k % NB][k / NB] = load.finish(j0 + k * TPL, k, raw[s]);
+      }
+    }
   } else {
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
@@ -257,7 +290,7 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       const int o = base + r * NS;
-      if (last) store(o, v[b][r]);
+      if constexpr (last) store(o, b + r * NB, v[b][r]);     // last stage: o = j0 + k TPL with slot k = b + r NB
       else sm[fft_pad<N>(o)] = v[b][r];
     }
   }

@@ -116,7 +116,10 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const FieldOp op = batch.f[blockIdx.y];
   const int My = g.My, Hy = g.Hy;
   const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * Hy * L + c;   // (q, c) at q L
-  cplx<T>* __restrict__ dst = static_cast<cplx<T>*>(op.dst) + (size_t)t * 2 * NH * L + threadIdx.x;
+  // inverse intermediate is pair-row-major: row y = 2y'+p of column mx at ((2 (y'>>1) + p) Wxp + mx) 2 + (y'&1);
+  // y' = j + k TPL keeps the parity of j, so slot k adds k TPL Wxp 2 elements
+  cplx<T>* __restrict__ dst = static_cast<cplx<T>*>(op.dst) + ((size_t)(j & ~1) * g.Wxp + mx) * 2 + (j & 1);
+  const size_t slot_stride = (size_t)TPL * g.Wxp * 2;
   const int mode = op.mode;
   const T scale = (T)g.inv_sqrt_ny;
   cplx<T>* line = sm + c * C::LS;
@@ -124,17 +127,18 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const T kx = (T)g.dkx * (T)mx;
   const T kx2 = kx * kx;
   const bool half_rule = (2 * My == NH);     // the paper's 1/2 rule: |my| <= Ny/4 (uniform branch)
+  const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
 
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
     // a_p[mp] = (X[mp] + (-1)^p X[mp+NH]) W_Ny^{-p mp}; X[mp] is retained iff mp <= My, X[mp+NH] (my = mp-NH) iff
     // NH-mp <= My.
-    // output element y' = j + k TPL of column c -> dst + p NH L + k blockDim (see col_thread_map); tail columns of the
-    // last tile are written too (zeros), the row pass never reads them
-    cplx<T>* out = dst + (size_t)p * NH * L;
-    auto store = [&](int yp, cplx<T> val) { out[(size_t)((yp - j) / TPL) * (L * TPL)] = val; };
-    auto twist = [&](int mp, cplx<T> a) -> cplx<T> {
-      if (p) a = mul_conj(a, ldg_c(tabS + mp));   // * W_Ny^{-mp}  (inverse sign)
+    // tail columns of the last tile are written too (zeros inside the row pitch), the row pass never reads them
+    cplx<T>* out = dst + (size_t)p * g.Wxp * 2;
+    auto store = [&](int, int k, cplx<T> val) { out[(size_t)k * slot_stride] = val; };
+    // * W_Ny^{-mp} (inverse sign) for the odd rows; mp = j + k TPL, so W_Ny^{mp} = W_Ny^j W_32^k: one table load per thread
+    auto twist = [&](int k, cplx<T> a) -> cplx<T> {
+      if (p) a = mul_w32_rt<+1>(mul_conj(a, wj), k);
       return scale * a;
     };
     if (half_rule) {
@@ -149,7 +153,7 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
         cplx<T> v = apply_spec_mode<T>(mode, raw, mx, k < 8 ? mp : mp - NH, kx2, g, v0);
         if (k >= 8 && p) v = mk<T>(-v.x, -v.y);
         if (k == 8 && j == 0) v = v + apply_spec_mode<T>(mode, src[(size_t)mp * L], mx, mp, kx2, g, v0);
-        return twist(mp, v);
+        return twist(k, v);
       };
       fft_line<T, NH, +1, false>(j, line, tabY, make_loader(issue, finish), store);
     } else {
@@ -159,7 +163,7 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
         const int q = use1 ? mp : Hy + mp - NH;
         return (valid && (use1 || use2)) ? src[(size_t)q * L] : mk<T>(0, 0);
       };
-      auto finish = [&](int mp, int, cplx<T> raw) -> cplx<T> {
+      auto finish = [&](int mp, int k, cplx<T> raw) -> cplx<T> {
         const bool use1 = mp <= My, use2 = NH - mp <= My;
         if (!valid || !(use1 || use2)) return mk<T>(0, 0);
         cplx<T> v = apply_spec_mode<T>(mode, raw, mx, use1 ? mp : mp - NH, kx2, g, v0);
@@ -168,7 +172,7 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
           const cplx<T> b = apply_spec_mode<T>(mode, src[(size_t)(Hy + mp - NH) * L], mx, mp - NH, kx2, g, v0);
           v = p ? v - b : v + b;
         }
-        return twist(mp, v);
+        return twist(k, v);
       };
       fft_line<T, NH, +1, false>(j, line, tabY, make_loader(issue, finish), store);
     }
@@ -196,6 +200,7 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   cplx<T>* dst = static_cast<cplx<T>*>(op.dst) + (size_t)t * Hy * L + c;
   const T scale = (T)g.inv_sqrt_ny;
   cplx<T>* line = sm + c * C::LS;
+  const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
 
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
@@ -203,14 +208,15 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     auto load = make_loader(
         [&](int, int k) -> cplx<T> { return valid ? in[(size_t)k * (L * TPL)] : mk<T>(0, 0); },
         [&](int, int, cplx<T> raw) -> cplx<T> { return scale * raw; });
-    auto store = [&](int mp, cplx<T> val) {
+    auto store = [&](int mp, int k, cplx<T> val) {
       if (!valid) return;
       if (p == 0) {
         if (mp <= My) dst[(size_t)mp * L] = val;
         if (NH - mp <= My) dst[(size_t)(Hy + mp - NH) * L] = val;
       } else {
-        const cplx<T> tw = val * ldg_c(tabS + mp);                // W_Ny^{mp} O[mp];  W_Ny^{mp+NH} = -W_Ny^{mp}
-        // fire-and-forget reductions instead of read-modify-write: no L2 round trip on the critical path
+        // W_Ny^{mp} O[mp] with mp = j + k TPL: W_Ny^j (one table load per thread) times the constant W_32^k;
+        // W_Ny^{mp+NH} = -W_Ny^{mp}.  Fire-and-forget reductions instead of read-modify-write.
+        const cplx<T> tw = mul_w32_rt<-1>(val * wj, k);
         if (mp <= My) red_add(dst + (size_t)mp * L, tw);
         if (NH - mp <= My) red_add(dst + (size_t)(Hy + mp - NH) * L, mk<T>(-tw.x, -tw.y));
       }
@@ -249,29 +255,53 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     if (mode == RM_IKX) return kx * mul_i(w);
     return mx == 0 ? mk<T>(meany, (T)0) : kx * mul_ni(w);        // RM_NIKX_MEANY
   };
-  auto issue = [&](int m, int) -> Pair<T> {
-    const int mx = m > NX / 2 ? NX - m : m;
-    if (mx < Wx) return ld_pair(src + inter_pair_index(g, a, p, mx));
-    Pair<T> r;
-    r.a = mk<T>(0, 0); r.b = mk<T>(0, 0);
-    return r;
-  };
-  auto finish = [&](int m, int, Pair<T> r) -> cplx<T> {
-    // Z(m) = A(m) + i B(m) with A, B the Hermitian x-spectra of the two real rows
-    const bool neg = m > NX / 2;
-    const int mx = neg ? NX - m : m;
-    if (mx >= Wx) return mk<T>(0, 0);
+  const cplx<T>* __restrict__ row = src + (size_t)rp * g.Wxp * 2;        // (A, B) pair of column mx at row + 2 mx
+  if (threadIdx.x == 0) {   // L2 prefetch of the contiguous input of the CTA that runs about one wave later
+    int nb = blockIdx.x + TTSH_PF_DIST, ny = blockIdx.y;
+    if (nb >= (int)gridDim.x) { nb -= gridDim.x; ny += 1; }
+    if (ny < (int)gridDim.y)
+      prefetch_l2_bulk(static_cast<const cplx<T>*>(batch.f[ny].src) + (size_t)nb * C::L * g.Wxp * 2,
+                       (unsigned)(C::L * g.Wxp * 2 * sizeof(cplx<T>)));
+  }
+  auto zero_pair = [&]() -> Pair<T> { Pair<T> r; r.a = mk<T>(0, 0); r.b = mk<T>(0, 0); return r; };
+  // Z(m) = A(m) + i B(m) with A, B the Hermitian x-spectra of the two real rows; neg: m stands for -mx
+  auto combine = [&](Pair<T> r, int mx, bool neg) -> cplx<T> {
     cplx<T> wa = mult(r.a, mx), wb = mult(r.b, mx);
     if (mx == 0) { wa.y = 0; wb.y = 0; }           // Re[] of the oracle's complex iDFT: drop the anti-Hermitian part
     if (neg) { wa = conj(wa); wb = conj(wb); }
     return scale * mk<T>(wa.x - wb.y, wa.y + wb.x);
   };
-  auto load = make_loader(issue, finish);
-  auto store = [&](int x, cplx<T> z) {
+  auto store = [&](int x, int, cplx<T> z) {
     dstA[x] = z.x;
     dstB[x] = z.y;
   };
-  fft_line<T, NX, +1, false>(j, sm + c * C::LS, tabX, load, store);
+  if (4 * (Wx - 1) == NX) {
+    // the paper's 1/2 rule: retained mx = 0..NX/4 = 4 TPL.  Input slot k (m = j + k TPL): k <= 3 holds +mx = m, k = 4 only
+    // the single point m = NX/4 (j = 0), k = 5..11 nothing, k = 12..15 holds -mx with mx = NX - m: compile-time pruning.
+    auto issue = [&](int m, int k) -> Pair<T> {
+      if (k <= 3 || (k == 4 && j == 0)) return ld_pair(row + 2 * m);
+      if (k >= 12) return ld_pair(row + 2 * (NX - m));
+      return zero_pair();
+    };
+    auto finish = [&](int m, int k, Pair<T> r) -> cplx<T> {
+      if (k <= 3) return combine(r, m, false);
+      if (k == 4) return j == 0 ? combine(r, m, false) : mk<T>(0, 0);
+      if (k >= 12) return combine(r, NX - m, true);
+      return mk<T>(0, 0);
+    };
+    fft_line<T, NX, +1, false>(j, sm + c * C::LS, tabX, make_loader<2>(issue, finish), store);
+  } else {
+    auto issue = [&](int m, int) -> Pair<T> {
+      const int mx = m > NX / 2 ? NX - m : m;
+      return mx < Wx ? ld_pair(row + 2 * mx) : zero_pair();
+    };
+    auto finish = [&](int m, int, Pair<T> r) -> cplx<T> {
+      const bool neg = m > NX / 2;
+      const int mx = neg ? NX - m : m;
+      return mx < Wx ? combine(r, mx, neg) : mk<T>(0, 0);
+    };
+    fft_line<T, NX, +1, false>(j, sm + c * C::LS, tabX, make_loader<2>(issue, finish), store);
+  }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -304,7 +334,7 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 
   auto load = make_loader([&](int x, int) -> cplx<T> { return mk<T>(srcA[x], srcB[x]); },
                           [&](int, int, cplx<T> raw) -> cplx<T> { return scale * raw; });
-  auto store = [&](int m, cplx<T> z) { line[fft_pad<NX>(m)] = z; };
+  auto store = [&](int m, int, cplx<T> z) { line[fft_pad<NX>(m)] = z; };
   fft_line<T, NX, -1, true>(j, line, tabX, load, store);
   __syncthreads();
   // unpack: A(m) = (Z(m) + conj Z(-m))/2,  B(m) = -i (Z(m) - conj Z(-m))/2,  m = 0..Wx-1

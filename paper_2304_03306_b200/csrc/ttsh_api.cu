@@ -33,6 +33,7 @@ Geom make_geom(int Nx, int Ny, double dx, int num, int den, size_t w) {
   g.CW = col_tile_width(Ny, (int)(2 * w));
   g.cw_shift = g.CW == 2 ? 1 : (g.CW == 4 ? 2 : 3);
   g.NT = (g.Wx + g.CW - 1) / g.CW;
+  g.Wxp = g.NT * g.CW;
   g.My = (int)((long long)num * Ny / (2LL * den));
   g.Hy = 2 * g.My + 1;
   const long double two_pi = 2.0L * acosl(-1.0L);

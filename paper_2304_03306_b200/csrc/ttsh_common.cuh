@@ -40,17 +40,20 @@ template <typename T> __device__ __forceinline__ cplx<T> mul_conj(cplx<T> a, cpl
 //                     columns one CTA of the column pass transforms; a power of two).  Both complex arrays are
 //                     TILE-MAJOR, so that a column CTA streams one contiguous block and never makes a strided access:
 //   pruned spectrum   cplx[NT][Hy][CW]                      element (q, mx):  ((mx/CW) Hy + q) CW + mx%CW
-//   intermediate      cplx[NT][2][Ny/4][CW][2]              (x-spectral, y real).  Row y = 4a + p + 2b (p = parity,
-//                     b = 0/1) of column mx sits at  (((mx/CW) 2 + p) Ny/4 + a) 2 CW + 2 (mx%CW) + b:
-//                     rows are split by parity p (the column pass transforms even and odd rows separately) and the
-//                     two same-parity rows 4a+p, 4a+p+2 that one row-pass FFT packs together are adjacent, so the row
-//                     pass moves (A, B) pairs with single 32-byte (fp64) / 16-byte (fp32) accesses in pieces of
-//                     2 CW elements, and the column pass block [Ny/2][CW] is contiguous.
+//   intermediates     (x-spectral, y real).  A row-pass FFT packs the two same-parity rows y = 4a+p (A) and 4a+p+2 (B),
+//                     row pair rp = 2a+p; (A, B) of one column are adjacent so that the row pass moves them with one
+//                     32-byte (fp64) / 16-byte (fp32) access.  Two layouts, chosen so that every READ is contiguous
+//                     and only fire-and-forget WRITES are scattered (in 2 CW-element pieces):
+//     forward  (k_fwd_row writes, k_fwd_col reads)   cplx[NT][2][Ny/4][CW][2]   tile-major: the column CTA's block
+//                     [Ny/2 rows of parity p][CW] is contiguous;  pair at  (((mx/CW) 2 + p) Ny/4 + a) 2 CW + 2 (mx%CW)
+//     inverse  (k_inv_col writes, k_inv_row reads)   cplx[Ny/2][Wxp][2]         pair-row-major: the row CTA's 2 Wxp
+//                     elements are contiguous;  pair at  (rp Wxp + mx) 2,   Wxp = NT CW
 // ---------------------------------------------------------------------------------------
 struct Geom {
   int Nx, Ny;
   int Wx;                  // retained x-wavenumbers
   int CW, cw_shift, NT;    // tile width (columns), log2, number of tiles = ceil(Wx / CW)
+  int Wxp;                 // NT * CW: padded number of columns
   int My, Hy;
   int num, den;            // dealias fraction
   double dkx, dky;         // 2 pi / (Nx dx), 2 pi / (Ny dx)   (Table I)
@@ -60,7 +63,7 @@ struct Geom {
 __host__ __device__ __forceinline__ size_t spec_index(const Geom& g, int q, int mx) {
   return ((size_t)(mx >> g.cw_shift) * g.Hy + q) * g.CW + (mx & (g.CW - 1));
 }
-// index of the (A, B) pair (rows 4a+p and 4a+p+2) of column mx; B is the next element
+// forward intermediate: index of the (A, B) pair (rows 4a+p and 4a+p+2) of column mx; B is the next element
 __host__ __device__ __forceinline__ size_t inter_pair_index(const Geom& g, int a, int p, int mx) {
   return ((((size_t)(mx >> g.cw_shift) * 2 + p) * (g.Ny >> 2) + a) * g.CW + (mx & (g.CW - 1))) * 2;
 }

@@ -19,8 +19,9 @@ template <typename T> cudaError_t prepare_cols(const Geom& g);
 template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,
                                                    void* w_s, void* gx_fx, void* gy_fy, cudaStream_t s);
 template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
-                                                  void* w, double* v0, cudaStream_t s);
-template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, double* v0, cudaStream_t s);
+                                                  void* w, void* psi, double* v0, cudaStream_t s);
+template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, void* psi, double* v0, cudaStream_t s);
+template <typename T> cudaError_t launch_psi_from_w(const Geom& g, const void* w, void* psi, cudaStream_t s);
 template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s);
 template <typename T> cudaError_t launch_square(size_t n, const void* in, void* out, cudaStream_t s);
 template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, cudaStream_t s);

@@ -76,18 +76,15 @@ __device__ __forceinline__ void st_pair(cplx<float>* p, cplx<float> a, cplx<floa
   asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
 }
 
-// spectral multiplier of the inverse column pass (SpecMode).  mode is uniform per CTA, kx and kx^2 per thread.
+// spectral multiplier of the inverse column pass (SpecMode).  mode is uniform per CTA.  No division: psi^ = w^/k^2 is kept
+// as a second spectrum by the spectral kernel (line 13 of Algorithm 1 is evaluated once per mode there).
 template <typename T>
-__device__ __forceinline__ cplx<T> apply_spec_mode(int mode, cplx<T> w, int mx, int my, T kx2, const Geom& g, const double* v0) {
+__device__ __forceinline__ cplx<T> apply_spec_mode(int mode, cplx<T> w, int mx, int my, const Geom& g, const double* v0) {
   if (mode == SM_ONE) return w;
-  const T ky = (T)g.dky * (T)my;
-  if (mode == SM_IKY) return ky * mul_i(w);
   if (mode == SM_LOWPASS4) return is_cut(mx, my, g.Nx, g.Ny, 1, 4) ? mk<T>(0, 0) : w;
-  const bool zero = (mx == 0 && my == 0);
-  const T ik2 = (T)1 / (zero ? (T)1 : kx2 + ky * ky);
-  if (mode == SM_PSI) return zero ? mk<T>(0, 0) : ik2 * w;
-  /* SM_IKY_PSI_MEANX */
-  return zero ? mk<T>((T)v0[0], (T)0) : (ky * ik2) * mul_i(w);
+  const T ky = (T)g.dky * (T)my;
+  if (mode == SM_IKY_MEANX && mx == 0 && my == 0) return mk<T>((T)v0[0], (T)0);
+  return ky * mul_i(w);
 }
 
 // thread -> (FFT index j, column c) of a column CTA: threadIdx.x enumerates the intermediate block [Ny/4][CW][2] in
@@ -124,8 +121,6 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const T scale = (T)g.inv_sqrt_ny;
   cplx<T>* line = sm + c * C::LS;
 
-  const T kx = (T)g.dkx * (T)mx;
-  const T kx2 = kx * kx;
   const bool half_rule = (2 * My == NH);     // the paper's 1/2 rule: |my| <= Ny/4 (uniform branch)
   const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
 
@@ -150,9 +145,9 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
       };
       auto finish = [&](int mp, int k, cplx<T> raw) -> cplx<T> {
         if (!valid) return mk<T>(0, 0);
-        cplx<T> v = apply_spec_mode<T>(mode, raw, mx, k < 8 ? mp : mp - NH, kx2, g, v0);
+        cplx<T> v = apply_spec_mode<T>(mode, raw, mx, k < 8 ? mp : mp - NH, g, v0);
         if (k >= 8 && p) v = mk<T>(-v.x, -v.y);
-        if (k == 8 && j == 0) v = v + apply_spec_mode<T>(mode, src[(size_t)mp * L], mx, mp, kx2, g, v0);
+        if (k == 8 && j == 0) v = v + apply_spec_mode<T>(mode, src[(size_t)mp * L], mx, mp, g, v0);
         return twist(k, v);
       };
       fft_line<T, NH, +1, false>(j, line, tabY, make_loader(issue, finish), store);
@@ -166,10 +161,10 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
       auto finish = [&](int mp, int k, cplx<T> raw) -> cplx<T> {
         const bool use1 = mp <= My, use2 = NH - mp <= My;
         if (!valid || !(use1 || use2)) return mk<T>(0, 0);
-        cplx<T> v = apply_spec_mode<T>(mode, raw, mx, use1 ? mp : mp - NH, kx2, g, v0);
+        cplx<T> v = apply_spec_mode<T>(mode, raw, mx, use1 ? mp : mp - NH, g, v0);
         if (!use1 && p) v = mk<T>(-v.x, -v.y);
         if (use1 && use2) {
-          const cplx<T> b = apply_spec_mode<T>(mode, src[(size_t)(Hy + mp - NH) * L], mx, mp - NH, kx2, g, v0);
+          const cplx<T> b = apply_spec_mode<T>(mode, src[(size_t)(Hy + mp - NH) * L], mx, mp - NH, g, v0);
           v = p ? v - b : v + b;
         }
         return twist(k, v);
@@ -202,26 +197,52 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   cplx<T>* line = sm + c * C::LS;
   const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
 
+  const bool half_rule = (2 * My == NH);
+  // output rows: X[mp] (my = mp >= 0) at row mp, X[mp+NH] (my = mp-NH < 0) at row Hy+mp-NH; mp = j + k TPL
+  cplx<T>* dpos = dst + (size_t)j * L;
+  cplx<T>* dneg = dst + (size_t)(Hy - NH + j) * L;
+  constexpr size_t KS = (size_t)TPL * L;     // elements per slot
+
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
     const cplx<T>* in = src + (size_t)p * NH * L;
     auto load = make_loader(
         [&](int, int k) -> cplx<T> { return valid ? in[(size_t)k * (L * TPL)] : mk<T>(0, 0); },
         [&](int, int, cplx<T> raw) -> cplx<T> { return scale * raw; });
-    auto store = [&](int mp, int k, cplx<T> val) {
-      if (!valid) return;
+    // pass 0 stores E; pass 1 accumulates W_Ny^{mp} O[mp] = W_Ny^j W_32^k O (one table load per thread; W_Ny^{mp+NH} =
+    // -W_Ny^{mp}) with fire-and-forget reductions instead of a read-modify-write.
+    if (half_rule) {
+      // My = NH/2 = 8 TPL: slot k < 8 -> row mp only, k > 8 -> row Hy+mp-NH only, k = 8 -> the latter plus, for j = 0, row NH/2
       if (p == 0) {
-        if (mp <= My) dst[(size_t)mp * L] = val;
-        if (NH - mp <= My) dst[(size_t)(Hy + mp - NH) * L] = val;
+        auto store = [&](int, int k, cplx<T> val) {
+          if (!valid) return;
+          if (k < 8 || (k == 8 && j == 0)) dpos[k * KS] = val;
+          if (k >= 8) dneg[k * KS] = val;
+        };
+        fft_line<T, NH, -1, false>(j, line, tabY, load, store);
       } else {
-        // W_Ny^{mp} O[mp] with mp = j + k TPL: W_Ny^j (one table load per thread) times the constant W_32^k;
-        // W_Ny^{mp+NH} = -W_Ny^{mp}.  Fire-and-forget reductions instead of read-modify-write.
-        const cplx<T> tw = mul_w32_rt<-1>(val * wj, k);
-        if (mp <= My) red_add(dst + (size_t)mp * L, tw);
-        if (NH - mp <= My) red_add(dst + (size_t)(Hy + mp - NH) * L, mk<T>(-tw.x, -tw.y));
+        auto store = [&](int, int k, cplx<T> val) {
+          if (!valid) return;
+          const cplx<T> tw = mul_w32_rt<-1>(val * wj, k);
+          if (k < 8 || (k == 8 && j == 0)) red_add(dpos + k * KS, tw);
+          if (k >= 8) red_add(dneg + k * KS, mk<T>(-tw.x, -tw.y));
+        };
+        fft_line<T, NH, -1, false>(j, line, tabY, load, store);
       }
-    };
-    fft_line<T, NH, -1, false>(j, line, tabY, load, store);
+    } else {
+      auto store = [&](int mp, int k, cplx<T> val) {
+        if (!valid) return;
+        if (p == 0) {
+          if (mp <= My) dpos[k * KS] = val;
+          if (NH - mp <= My) dneg[k * KS] = val;
+        } else {
+          const cplx<T> tw = mul_w32_rt<-1>(val * wj, k);
+          if (mp <= My) red_add(dpos + k * KS, tw);
+          if (NH - mp <= My) red_add(dneg + k * KS, mk<T>(-tw.x, -tw.y));
+        }
+      };
+      fft_line<T, NH, -1, false>(j, line, tabY, load, store);
+    }
   }
 }
 

@@ -18,14 +18,19 @@ template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
-                                                  void* w, double* v0, cudaStream_t s) {
+                                                  void* w, void* psi, double* v0, cudaStream_t s) {
   const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
-  k_spectral<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, v0);
+  k_spectral<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, (cplx<T>*)psi, v0);
   return cudaGetLastError();
 }
-template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, double* v0, cudaStream_t s) {
+template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, void* psi, double* v0, cudaStream_t s) {
   const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
-  k_spectral_init<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)Vx, (const cplx<T>*)Vy, (cplx<T>*)w, v0);
+  k_spectral_init<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)Vx, (const cplx<T>*)Vy, (cplx<T>*)w, (cplx<T>*)psi, v0);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_psi_from_w(const Geom& g, const void* w, void* psi, cudaStream_t s) {
+  const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
+  k_psi_from_w<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)w, (cplx<T>*)psi);
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s) {
@@ -51,8 +56,9 @@ template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double c
 
 #define INST(T) \
   template cudaError_t launch_realspace<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
-  template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, double*, cudaStream_t); \
-  template cudaError_t launch_spectral_init<T>(const Geom&, const void*, const void*, void*, double*, cudaStream_t); \
+  template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, double*, cudaStream_t); \
+  template cudaError_t launch_spectral_init<T>(const Geom&, const void*, const void*, void*, void*, double*, cudaStream_t); \
+  template cudaError_t launch_psi_from_w<T>(const Geom&, const void*, void*, cudaStream_t); \
   template cudaError_t launch_mask_to_real<T>(size_t, const unsigned char*, void*, cudaStream_t); \
   template cudaError_t launch_square<T>(size_t, const void*, void*, cudaStream_t); \
   template cudaError_t launch_fill<T>(size_t, void*, double, cudaStream_t); \

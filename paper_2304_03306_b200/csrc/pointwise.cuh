@@ -68,10 +68,15 @@ __device__ __forceinline__ cplx<T> naive_update(const Geom& g, const Model& m, i
   return e * (w[idx] + dt * r);                                               // line 4
 }
 
+template <typename T> __device__ __forceinline__ T inv_k2(const Geom& g, int mx, int my) {
+  const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my);
+  return (T)1 / (kx * kx + ky * ky);
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __restrict__ Fy,
-           const cplx<T>* __restrict__ S, cplx<T>* w, double* v0) {
+           const cplx<T>* __restrict__ S, cplx<T>* w, cplx<T>* __restrict__ psi, double* v0) {
   // threads enumerate the tile-major array in memory order: idx = (t Hy + q) CW + c
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
@@ -91,6 +96,7 @@ k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __res
       v0[0] = e * (v0[0] + m.dt * (double)Fx[idx].x);
       v0[1] = e * (v0[1] + m.dt * (double)Fy[idx].x);
       w[idx] = mk<T>(0, 0);
+      psi[idx] = mk<T>(0, 0);
       return;
     }
     const size_t idn = spec_index(g, g.Hy - my, 0);       // row of -my, mx = 0
@@ -100,18 +106,24 @@ k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __res
       const cplx<T> b = naive_update<T>(g, m, 0, -my, idn, Fx, Fy, S, w);
       out = (T)0.5 * (a + conj(b));
     }
+    const T ik2 = inv_k2<T>(g, 0, my);                          // psi^ = w^/k^2 (line 13)
     w[idx] = out;
     w[idn] = conj(out);
+    psi[idx] = ik2 * out;
+    psi[idn] = ik2 * conj(out);
     return;
   }
   cplx<T> out = naive_update<T>(g, m, mx, my, idx, Fx, Fy, S, w);
-  w[idx] = cut ? mk<T>(0, 0) : out;
+  out = cut ? mk<T>(0, 0) : out;
+  w[idx] = out;
+  psi[idx] = inv_k2<T>(g, mx, my) * out;                       // line 13
 }
 
 // ttsh_set_velocity: w^ = i kx v^y - i ky v^x, v^(0) kept, then the same post-processing
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_spectral_init(Geom g, const cplx<T>* __restrict__ Vx, const cplx<T>* __restrict__ Vy, cplx<T>* w, double* v0) {
+k_spectral_init(Geom g, const cplx<T>* __restrict__ Vx, const cplx<T>* __restrict__ Vy, cplx<T>* w,
+                cplx<T>* __restrict__ psi, double* v0) {
   // threads enumerate the tile-major array in memory order: idx = (t Hy + q) CW + c
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
@@ -132,16 +144,36 @@ k_spectral_init(Geom g, const cplx<T>* __restrict__ Vx, const cplx<T>* __restric
       v0[0] = (double)Vx[idx].x;
       v0[1] = (double)Vy[idx].x;
       w[idx] = mk<T>(0, 0);
+      psi[idx] = mk<T>(0, 0);
       return;
     }
     const size_t idn = spec_index(g, g.Hy - my, 0);
     cplx<T> out = mk<T>(0, 0);
     if (!cut) out = (T)0.5 * (curl(my, idx) + conj(curl(-my, idn)));
+    const T ik2 = inv_k2<T>(g, 0, my);
     w[idx] = out;
     w[idn] = conj(out);
+    psi[idx] = ik2 * out;
+    psi[idn] = ik2 * conj(out);
     return;
   }
-  w[idx] = cut ? mk<T>(0, 0) : curl(my, idx);
+  const cplx<T> out = cut ? mk<T>(0, 0) : curl(my, idx);
+  w[idx] = out;
+  psi[idx] = inv_k2<T>(g, mx, my) * out;
+}
+
+// psi^ = w^/k^2 from a restored w^ (ttsh_set_state)
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_psi_from_w(Geom g, const cplx<T>* __restrict__ w, cplx<T>* __restrict__ psi) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
+  const int t = (int)(idx / ((size_t)g.Hy * g.CW));
+  const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
+  const int q = rem >> g.cw_shift;
+  const int mx = t * g.CW + (rem & (g.CW - 1));
+  const int my = q <= g.My ? q : q - g.Hy;
+  psi[idx] = (mx >= g.Wx || (mx == 0 && my == 0)) ? mk<T>(0, 0) : inv_k2<T>(g, mx, my) * w[idx];
 }
 
 // ---------------------------------------------------------------------------------------

@@ -22,7 +22,7 @@ inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 inline bool pow2_in_range(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
 
 struct Layout {
-  size_t tabX, tabY, tabS, K, what, v0, diag_partial, diag_out, R[5], Tm[4], S[3], total;
+  size_t tabX, tabY, tabS, K, what, psihat, v0, diag_partial, diag_out, R[5], Tm[4], S[3], total;
 };
 
 Geom make_geom(int Nx, int Ny, double dx, int num, int den, size_t w) {
@@ -58,6 +58,7 @@ Layout make_layout(int Nx, int Ny, size_t w) {
   L.tabS = take((size_t)Ny * cw);
   L.K = take(P * w);
   L.what = take(spec);
+  L.psihat = take(spec);
   L.v0 = take(8 * sizeof(double));
   L.diag_partial = take((size_t)DIAG_BLOCKS * 8 * sizeof(double));
   L.diag_out = take(8 * sizeof(double));
@@ -79,7 +80,7 @@ struct ttsh_handle {
   Model m;
   cudaStream_t stream;
   char* ws;
-  void *tabX, *tabY, *tabS, *K, *what, *R[5], *Tm[4], *S[3];
+  void *tabX, *tabY, *tabS, *K, *what, *psihat, *R[5], *Tm[4], *S[3];
   double *v0, *diag_partial, *diag_out;
   bool initialized;
   double t;
@@ -158,8 +159,8 @@ int enqueue_inverse(ttsh_handle* h, void* w, void* gx, void* gy, void* vx, void*
   int nc = 0;
   if (need_w) cb.f[nc++] = op(h->what, h->Tm[0], SM_ONE);
   if (need_gy) cb.f[nc++] = op(h->what, h->Tm[1], SM_IKY);
-  if (need_psi) cb.f[nc++] = op(h->what, h->Tm[2], SM_PSI);
-  if (need_vx) cb.f[nc++] = op(h->what, h->Tm[3], SM_IKY_PSI_MEANX);
+  if (need_psi) cb.f[nc++] = op(h->psihat, h->Tm[2], SM_ONE);
+  if (need_vx) cb.f[nc++] = op(h->psihat, h->Tm[3], SM_IKY_MEANX);
   if (nc == 0) return TTSH_OK;
   TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->tabS, h->v0, h->stream));
   h->launches++;
@@ -200,8 +201,8 @@ int enqueue_forward(ttsh_handle* h, int n, const void* const* src) {
 int enqueue_stage(ttsh_handle* h, int stage) {
   switch (stage) {
     case TTSH_STAGE_INV_COL: {
-      Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->what, h->Tm[1], SM_IKY), op(h->what, h->Tm[2], SM_PSI),
-                             op(h->what, h->Tm[3], SM_IKY_PSI_MEANX)});
+      Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->what, h->Tm[1], SM_IKY), op(h->psihat, h->Tm[2], SM_ONE),
+                             op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
       TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 4, h->tabY, h->tabS, h->v0, h->stream));
       h->launches++;
       return TTSH_OK;
@@ -230,7 +231,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
       return TTSH_OK;
     }
     case TTSH_STAGE_SPECTRAL:
-      TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, h->S[0], h->S[1], h->S[2], h->what, h->v0, h->stream));
+      TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, h->S[0], h->S[1], h->S[2], h->what, h->psihat, h->v0, h->stream));
       h->launches++;
       return TTSH_OK;
   }
@@ -310,7 +311,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->m.Gamma2 = p->Gamma2; h->m.gamma_v = p->gamma_v; h->m.gamma_w = p->gamma_w; h->m.dt = dt;
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   h->ws = static_cast<char*>(workspace);
-  h->tabX = h->ws + L.tabX; h->tabY = h->ws + L.tabY; h->tabS = h->ws + L.tabS; h->K = h->ws + L.K; h->what = h->ws + L.what;
+  h->tabX = h->ws + L.tabX; h->tabY = h->ws + L.tabY; h->tabS = h->ws + L.tabS; h->K = h->ws + L.K; h->what = h->ws + L.what; h->psihat = h->ws + L.psihat;
   h->v0 = reinterpret_cast<double*>(h->ws + L.v0);
   h->diag_partial = reinterpret_cast<double*>(h->ws + L.diag_partial);
   h->diag_out = reinterpret_cast<double*>(h->ws + L.diag_out);
@@ -347,7 +348,7 @@ int ttsh_set_velocity(ttsh_handle* h, const void* vx, const void* vy) {
   const void* src[2] = {vx, vy};
   int rc = enqueue_forward(h, 2, src);
   if (rc != TTSH_OK) return rc;
-  TRY(h, DISPATCH(h, launch_spectral_init, h->g, h->S[0], h->S[1], h->what, h->v0, h->stream));
+  TRY(h, DISPATCH(h, launch_spectral_init, h->g, h->S[0], h->S[1], h->what, h->psihat, h->v0, h->stream));
   h->launches++;
   h->initialized = true;
   h->t = 0.0;
@@ -425,6 +426,8 @@ int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, d
   const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
   TRY(h, cudaMemcpyAsync(h->what, w_hat, bytes, cudaMemcpyDeviceToDevice, h->stream));
   TRY(h, cudaMemcpyAsync(h->v0, mean_flow, 2 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  TRY(h, DISPATCH(h, launch_psi_from_w, h->g, h->what, h->psihat, h->stream));
+  h->launches++;
   TRY(h, cudaStreamSynchronize(h->stream));
   h->initialized = true;
   h->t = t;

@@ -78,12 +78,11 @@ __host__ __device__ __forceinline__ bool is_cut(int mx, int my, int Nx, int Ny, 
 // ---------------------------------------------------------------------------------------
 // batched field descriptors: one launch transforms up to 5 fields (blockIdx.y selects the field)
 // ---------------------------------------------------------------------------------------
-enum SpecMode : int {     // multiplier applied to w^(mx,my) while loading the inverse column pass
-  SM_ONE = 0,             // w^
-  SM_IKY = 1,             // i k_y w^                       (Alg. 1 line 2)
-  SM_PSI = 2,             // w^/k^2, 0 at k = 0              (line 13)
-  SM_IKY_PSI_MEANX = 3,   // i k_y w^/k^2 = v^_x; v^_x(0) = mean flow   (lines 8, 14)
-  SM_LOWPASS4 = 4         // 1 inside the (1/4) pi/dx circle, else 0   (Alg. 2 lines 2-8)
+enum SpecMode : int {     // multiplier applied to the spectrum while loading the inverse column pass
+  SM_ONE = 0,             // x^                              (w^ -> w,  psi^ -> psi and, with -i k_x in the row pass, v_y)
+  SM_IKY = 1,             // i k_y x^                        (Alg. 1 line 2)
+  SM_IKY_MEANX = 2,       // i k_y psi^ = v^_x; the (0,0) entry is the mean flow v^_x(0)   (lines 8, 14)
+  SM_LOWPASS4 = 3         // 1 inside the (1/4) pi/dx circle, else 0   (Alg. 2 lines 2-8)
 };
 enum RowMode : int {      // multiplier applied in x-spectral space by the inverse row pass
   RM_ONE = 0,

@@ -165,18 +165,21 @@ def time_oracle(cfg, n_steps, budget_s, warmup=0):
 STAGE_NAMES = ["k_inv_col", "k_inv_row", "k_realspace", "k_fwd_row", "k_fwd_col", "k_spectral"]
 
 
-def stage_bytes(Nx, Ny, w):
-    """Algorithmic HBM bytes per launch of each kernel of one step: every input read once,
-    every output written once, pruned widths Wx = Nx/4+1, Hy = Ny/2+1."""
+def stage_bytes(Nx, Ny, w, conservative=True):
+    """Algorithmic HBM bytes per launch of each kernel of one step: every input read once, every
+    output written once, pruned widths Wx = Nx/4+1, Hy = Ny/2+1.  Conservative advection form (the default):
+    3 inverse transforms (w, v_x, v_y); literal form: 5 (w, d_x w, d_y w, v_x, v_y)."""
     Wx, Hy = Nx // 4 + 1, Ny // 2 + 1
     real, inter, spec = Nx * Ny * w, Ny * Wx * 2 * w, Hy * Wx * 2 * w
+    ninv_col, ninv_row = (3, 3) if conservative else (4, 5)
+    nreal_in = 4 if conservative else 6
     return {
-        "k_inv_col": spec + 4 * inter,
-        "k_inv_row": 4 * inter + 5 * real,
-        "k_realspace": 6 * real + 3 * real,
+        "k_inv_col": 2 * spec + ninv_col * inter,               # w^ and psi^ in
+        "k_inv_row": ninv_col * inter + ninv_row * real,
+        "k_realspace": nreal_in * real + 3 * real,
         "k_fwd_row": 3 * real + 3 * inter,
         "k_fwd_col": 3 * inter + 3 * spec,
-        "k_spectral": 4 * spec + spec,
+        "k_spectral": 4 * spec + 2 * spec,                       # F^x, F^y, S^, w^ in; w^, psi^ out
     }
 
 

@@ -18,6 +18,8 @@ template <typename T> cudaError_t prepare_cols(const Geom& g);
 // element-wise kernels and reductions (pointwise.cuh)
 template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,
                                                    void* w_s, void* gx_fx, void* gy_fy, cudaStream_t s);
+template <typename T> cudaError_t launch_realspace_cons(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,
+                                                        void* w_s, void* gx_out, void* gy_out, cudaStream_t s);
 template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
                                                   void* w, void* psi, double* v0, cudaStream_t s);
 template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, void* psi, double* v0, cudaStream_t s);

@@ -17,6 +17,13 @@ template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m
                                                                   (T*)w_s, (T*)gx_fx, (T*)gy_fy);
   return cudaGetLastError();
 }
+template <typename T> cudaError_t launch_realspace_cons(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,
+                                                        void* w_s, void* gx_out, void* gy_out, cudaStream_t s) {
+  const size_t nvec = (size_t)g.Nx * g.Ny / Vec<T>::n;
+  k_realspace_cons<T><<<blocks_for(nvec, 256, GRID_CAP), 256, 0, s>>>(nvec, m, (const T*)vx, (const T*)vy, (const T*)K,
+                                                                       (T*)w_s, (T*)gx_out, (T*)gy_out);
+  return cudaGetLastError();
+}
 template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
                                                   void* w, void* psi, double* v0, cudaStream_t s) {
   const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
@@ -56,6 +63,7 @@ template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double c
 
 #define INST(T) \
   template cudaError_t launch_realspace<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
+  template cudaError_t launch_realspace_cons<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
   template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, double*, cudaStream_t); \
   template cudaError_t launch_spectral_init<T>(const Geom&, const void*, const void*, void*, void*, double*, cudaStream_t); \
   template cudaError_t launch_psi_from_w<T>(const Geom&, const void*, void*, cudaStream_t); \

@@ -46,6 +46,37 @@ k_realspace(size_t nvec, Model m, const T* __restrict__ vx, const T* __restrict_
   }
 }
 
+// conservative form of the advection term (include/ttsh.h, ttsh_advection_form): with div v = 0,
+//   -lambda0 v.grad(w) = -lambda0 (d_x (v_x w) + d_y (v_y w)), so the spectral curl+sum of line 3 absorbs it:
+//   rhs^ = i kx (rhs1_y - lambda0 v_x w)^ - i ky (rhs1_x + lambda0 v_y w)^ + (-gamma_w K w)^.
+// Reads v, w, K (4 fields), writes 3: w -> -gamma_w K w in place, gx_out, gy_out.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_realspace_cons(size_t nvec, Model m, const T* __restrict__ vx, const T* __restrict__ vy, const T* __restrict__ K,
+                 T* __restrict__ w_s, T* __restrict__ gx_out, T* __restrict__ gy_out) {
+  using V = typename Vec<T>::type;
+  constexpr int n = Vec<T>::n;
+  const T beta = (T)m.beta, gv = (T)m.gamma_v, gw = (T)m.gamma_w, lam = (T)m.lambda0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    V a = reinterpret_cast<const V*>(vx)[i], b = reinterpret_cast<const V*>(vy)[i];
+    V k = reinterpret_cast<const V*>(K)[i];
+    V w = reinterpret_cast<V*>(w_s)[i], ox, oy;
+    T* pa = reinterpret_cast<T*>(&a); T* pb = reinterpret_cast<T*>(&b); T* pk = reinterpret_cast<T*>(&k);
+    T* pw = reinterpret_cast<T*>(&w); T* pox = reinterpret_cast<T*>(&ox); T* poy = reinterpret_cast<T*>(&oy);
+#pragma unroll
+    for (int e = 0; e < n; ++e) {
+      const T u = pa[e], v = pb[e], kk = pk[e], ww = pw[e];
+      const T c = -beta * (u * u + v * v) - gv * kk;      // rhs1 = c * v   (line 1)
+      pox[e] = c * u + lam * (v * ww);                    // rhs1_x + lambda0 v_y w
+      poy[e] = c * v - lam * (u * ww);                    // rhs1_y - lambda0 v_x w
+      pw[e] = -gw * kk * ww;                              // damping part of rhs2   (line 2)
+    }
+    reinterpret_cast<V*>(w_s)[i] = w;
+    reinterpret_cast<V*>(gx_out)[i] = ox;
+    reinterpret_cast<V*>(gy_out)[i] = oy;
+  }
+}
+
 // ---------------------------------------------------------------------------------------
 // a5: fused spectral kernel on the tile-major pruned spectrum (spec_index).
 //   w^_naive = exp(sigma dt) (w^ + dt (i kx F^y - i ky F^x + S^))                       (lines 3-4)

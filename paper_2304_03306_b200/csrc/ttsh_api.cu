@@ -90,6 +90,7 @@ struct ttsh_handle {
   std::string err;
   cudaGraphExec_t graph_exec;
   bool graph_ok;
+  int advection_form;
 };
 
 namespace {
@@ -201,21 +202,34 @@ int enqueue_forward(ttsh_handle* h, int n, const void* const* src) {
 int enqueue_stage(ttsh_handle* h, int stage) {
   switch (stage) {
     case TTSH_STAGE_INV_COL: {
-      Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->what, h->Tm[1], SM_IKY), op(h->psihat, h->Tm[2], SM_ONE),
-                             op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
-      TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 4, h->tabY, h->tabS, h->v0, h->stream));
+      if (h->advection_form == TTSH_ADVECTION_CONSERVATIVE) {   // w, psi (-> v_y), i k_y psi (-> v_x)
+        Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->psihat, h->Tm[2], SM_ONE), op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
+        TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, h->v0, h->stream));
+      } else {
+        Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->what, h->Tm[1], SM_IKY), op(h->psihat, h->Tm[2], SM_ONE),
+                               op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
+        TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 4, h->tabY, h->tabS, h->v0, h->stream));
+      }
       h->launches++;
       return TTSH_OK;
     }
     case TTSH_STAGE_INV_ROW: {
-      Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE), op(h->Tm[0], h->R[1], RM_IKX), op(h->Tm[1], h->R[2], RM_ONE),
-                             op(h->Tm[3], h->R[3], RM_ONE), op(h->Tm[2], h->R[4], RM_NIKX_MEANY)});
-      TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 5, h->tabX, h->v0, h->stream));
+      if (h->advection_form == TTSH_ADVECTION_CONSERVATIVE) {
+        Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE), op(h->Tm[3], h->R[3], RM_ONE), op(h->Tm[2], h->R[4], RM_NIKX_MEANY)});
+        TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 3, h->tabX, h->v0, h->stream));
+      } else {
+        Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE), op(h->Tm[0], h->R[1], RM_IKX), op(h->Tm[1], h->R[2], RM_ONE),
+                               op(h->Tm[3], h->R[3], RM_ONE), op(h->Tm[2], h->R[4], RM_NIKX_MEANY)});
+        TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 5, h->tabX, h->v0, h->stream));
+      }
       h->launches++;
       return TTSH_OK;
     }
     case TTSH_STAGE_REAL:
-      TRY(h, DISPATCH(h, launch_realspace, h->g, h->m, h->R[3], h->R[4], h->K, h->R[0], h->R[1], h->R[2], h->stream));
+      if (h->advection_form == TTSH_ADVECTION_CONSERVATIVE)
+        TRY(h, DISPATCH(h, launch_realspace_cons, h->g, h->m, h->R[3], h->R[4], h->K, h->R[0], h->R[1], h->R[2], h->stream));
+      else
+        TRY(h, DISPATCH(h, launch_realspace, h->g, h->m, h->R[3], h->R[4], h->K, h->R[0], h->R[1], h->R[2], h->stream));
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_FWD_ROW: {
@@ -319,7 +333,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   for (int i = 0; i < 4; ++i) h->Tm[i] = h->ws + L.Tm[i];
   for (int i = 0; i < 3; ++i) h->S[i] = h->ws + L.S[i];
   h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
-  h->graph_exec = nullptr; h->graph_ok = false;
+  h->graph_exec = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
   std::vector<unsigned char> tx, ty, ts;
@@ -353,6 +367,18 @@ int ttsh_set_velocity(ttsh_handle* h, const void* vx, const void* vy) {
   h->initialized = true;
   h->t = 0.0;
   h->step = 0;
+  return TTSH_OK;
+}
+
+int ttsh_set_advection_form(ttsh_handle* h, int form) {
+  if (!h || (form != TTSH_ADVECTION_CONSERVATIVE && form != TTSH_ADVECTION_LITERAL)) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (form != h->advection_form && h->graph_exec) {   // the captured step no longer matches
+    cudaGraphExecDestroy(h->graph_exec);
+    h->graph_exec = nullptr;
+    h->graph_ok = false;
+  }
+  h->advection_form = form;
   return TTSH_OK;
 }
 

@@ -22,11 +22,12 @@ TTSH_ERR_NOT_INITIALIZED = -4
 TTSH_ERR_CUDA = -5
 TTSH_F64, TTSH_F32 = 8, 4
 TTSH_MASK_BINARY, TTSH_MASK_PROCESSED = 0, 1
+TTSH_ADVECTION_CONSERVATIVE, TTSH_ADVECTION_LITERAL = 0, 1
 (TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL, TTSH_STAGE_FWD_ROW, TTSH_STAGE_FWD_COL,
  TTSH_STAGE_SPECTRAL) = range(6)
 
 # every symbol include/ttsh.h declares (tests check that the library exports all of them)
-SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_velocity", "ttsh_step",
+SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_velocity", "ttsh_set_advection_form", "ttsh_step",
            "ttsh_get_fields", "ttsh_state_elems", "ttsh_get_state", "ttsh_set_state", "ttsh_diagnostics",
            "ttsh_launch_count", "ttsh_run_stage", "ttsh_debug_get_real", "ttsh_destroy", "ttsh_strerror",
            "ttsh_last_error")
@@ -59,6 +60,7 @@ _sig = {
     "ttsh_create": (_i, [C.POINTER(_vp), _i, _i, _d, _d, C.POINTER(ttsh_params), _i, _vp, _i, _vp, _sz, _vp]),
     "ttsh_set_mask": (_i, [_vp, _vp, _i]),
     "ttsh_set_velocity": (_i, [_vp, _vp, _vp]),
+    "ttsh_set_advection_form": (_i, [_vp, _i]),
     "ttsh_step": (_i, [_vp, _i]),
     "ttsh_get_fields": (_i, [_vp, _vp, _vp, _vp, _vp]),
     "ttsh_state_elems": (_sz, [_vp]),
@@ -104,6 +106,10 @@ def ttsh_set_mask(h, mask_ptr, mask_kind):
 
 def ttsh_set_velocity(h, vx_ptr, vy_ptr):
     return _lib.ttsh_set_velocity(h, vx_ptr or None, vy_ptr or None)
+
+
+def ttsh_set_advection_form(h, form):
+    return _lib.ttsh_set_advection_form(h, form)
 
 
 def ttsh_step(h, n):
@@ -218,6 +224,9 @@ class Solver:
     def set_velocity(self, vx, vy):
         self._vx0, self._vy0 = self._dev(vx), self._dev(vy)
         self._check(ttsh_set_velocity(self.h, self._vx0.data_ptr(), self._vy0.data_ptr()))
+
+    def set_advection_form(self, form: int):
+        self._check(ttsh_set_advection_form(self.h, form))
 
     def step(self, n: int = 1):
         self._check(ttsh_step(self.h, n))

@@ -35,9 +35,11 @@ def params_pair(ttsh, which):
     return (ttsh.baseline_params(), BASELINE_PRESET) if which == "baseline" else (ttsh.paper_params(), PAPER_PRESET)
 
 
-def make_pair(ttsh, Nx, Ny, dx, dt, which, mask, dtype="f64", transform="matmul", vel=None):
+def make_pair(ttsh, Nx, Ny, dx, dt, which, mask, dtype="f64", transform="matmul", vel=None, form=None):
     gp, op = params_pair(ttsh, which)
     s = ttsh.Solver(Nx, Ny, dx, dt, gp, dtype, mask=mask)
+    if form is not None:
+        s.set_advection_form(form)
     o = TTSHOracle(Nx, Ny, dx, dt, op, mask=mask, transform=transform)
     if vel is not None:
         vx0, vy0 = vel
@@ -86,7 +88,7 @@ def test_real_space_kernel_matches_oracle_rhs(ttsh):
     Nx, Ny = 256, 128
     mask = workloads.disk_mask(Nx, Ny, 0.5, 20.0)
     vel = workloads.planewave_velocity(Nx, Ny, 0.5, 3, amplitude=1.0)
-    s, o = make_pair(ttsh, Nx, Ny, 0.5, 0.01, "baseline", mask, vel=vel)
+    s, o = make_pair(ttsh, Nx, Ny, 0.5, 0.01, "baseline", mask, vel=vel, form=ttsh.TTSH_ADVECTION_LITERAL)
     s.run_stage(ttsh.TTSH_STAGE_INV_COL); s.run_stage(ttsh.TTSH_STAGE_INV_ROW)
     w, gx, gy, rhs1, rhs2 = o.rhs_real()
     got = [s.debug_real(i).cpu().numpy() for i in range(5)]
@@ -95,6 +97,14 @@ def test_real_space_kernel_matches_oracle_rhs(ttsh):
     s.run_stage(ttsh.TTSH_STAGE_REAL)
     got = [s.debug_real(i).cpu().numpy() for i in range(3)]
     for g, e, name in zip(got, (rhs2, rhs1[0], rhs1[1]), ("rhs2", "rhs1x", "rhs1y")):
+        assert rel(g, e) <= 1e-12, name
+    # conservative form (include/ttsh.h): slots hold -gamma_w K w, rhs1_x + lambda0 v_y w, rhs1_y - lambda0 v_x w
+    s.set_advection_form(ttsh.TTSH_ADVECTION_CONSERVATIVE)
+    s.run_stage(ttsh.TTSH_STAGE_INV_COL); s.run_stage(ttsh.TTSH_STAGE_INV_ROW); s.run_stage(ttsh.TTSH_STAGE_REAL)
+    got = [s.debug_real(i).cpu().numpy() for i in range(3)]
+    p = BASELINE_PRESET
+    want = (-p.gamma_w * o.K * w, rhs1[0] + p.lambda0 * o.v[1] * w, rhs1[1] - p.lambda0 * o.v[0] * w)
+    for g, e, name in zip(got, want, ("damp", "Gx", "Gy")):
         assert rel(g, e) <= 1e-12, name
     s.close()
 
@@ -109,8 +119,9 @@ CASES_SMALL = [
 ]
 
 
+@pytest.mark.parametrize("form", [0, 1], ids=["conservative", "literal"])
 @pytest.mark.parametrize("name,Nx,Ny,which,geom,amp", CASES_SMALL)
-def test_trajectory_small_grids_every_step(ttsh, name, Nx, Ny, which, geom, amp):
+def test_trajectory_small_grids_every_step(ttsh, name, Nx, Ny, which, geom, amp, form):
     dx = 0.5
     R = 12.0 if min(Nx, Ny) == 64 else 20.0
     mask = workloads.disk_mask(Nx, Ny, dx, R) if geom == "disk" else workloads.dumbbell_mask(Nx, Ny, dx, 10.0, 14.0)
@@ -118,7 +129,7 @@ def test_trajectory_small_grids_every_step(ttsh, name, Nx, Ny, which, geom, amp)
         vel = workloads.gaussian_velocity(Nx, Ny, workloads.SEED0, amp, mask)
     else:
         vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0, amplitude=amp)
-    s, o = make_pair(ttsh, Nx, Ny, dx, 0.01, which, mask, vel=vel)
+    s, o = make_pair(ttsh, Nx, Ny, dx, 0.01, which, mask, vel=vel, form=form)
     compare_state(s, o, TOL_F64_1, name + " init")
     for n in range(1, 101):
         s.step(1); o.step(1)
@@ -160,12 +171,13 @@ def test_C2_O1_start_100_steps_graph_replay(ttsh):
     s.close()
 
 
+@pytest.mark.parametrize("form", [0, 1], ids=["conservative", "literal"])
 @pytest.mark.parametrize("dtype,tol", [("f64", TOL_F64_1), ("f32", TOL_F32_1)])
-def test_C3_1024_disk_single_step(ttsh, dtype, tol):
+def test_C3_1024_disk_single_step(ttsh, dtype, tol, form):
     cfg = workloads.CONFIGS["C3"]
     mask = cfg.mask(R=160.0)
     vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0)
-    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, dtype=dtype, vel=vel)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, dtype=dtype, vel=vel, form=form)
     if dtype == "f32":
         o.K = s.debug_real(5).cpu().numpy().astype(np.float64)   # K is built by Algorithm 2 in fp32 in the fp32 handle (R15)
     s.step(1); o.step(1)

@@ -162,7 +162,9 @@ def time_oracle(cfg, n_steps, budget_s, warmup=0):
 # --------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------
-STAGE_NAMES = ["k_inv_col", "k_inv_row", "k_realspace", "k_fwd_row", "k_fwd_col", "k_spectral"]
+# what ttsh_step launches per Euler step in the default (conservative) form, and the stage ids of ttsh_run_stage
+STAGE_NAMES = ["k_inv_col", "k_inv_row", "k_fwd_row_fused", "k_fwd_col", "k_spectral"]
+STAGE_IDS = [0, 1, 6, 4, 5]
 
 
 def stage_bytes(Nx, Ny, w, conservative=True):
@@ -178,6 +180,7 @@ def stage_bytes(Nx, Ny, w, conservative=True):
         "k_inv_row": ninv_col * inter + ninv_row * real,
         "k_realspace": nreal_in * real + 3 * real,
         "k_fwd_row": 3 * real + 3 * inter,
+        "k_fwd_row_fused": 4 * real + 3 * inter,                 # v_x, v_y, w, K in; 3 pruned intermediates out
         "k_fwd_col": 3 * inter + 3 * spec,
         "k_spectral": 4 * spec + 2 * spec,                       # F^x, F^y, S^, w^ in; w^, psi^ out
     }
@@ -215,14 +218,15 @@ def measure(torch, ttsh, cfg, dtype, K, W, device, want_roofline=True, want_e2e=
 
     if want_roofline:
         reps = 20
-        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(reps)]
+        ns = len(STAGE_IDS)
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(ns + 1)] for _ in range(reps)]
         for r in range(reps):
-            for st in range(6):
-                ev[r][st].record(stream)
+            for i, st in enumerate(STAGE_IDS):
+                ev[r][i].record(stream)
                 s.run_stage(st)
-            ev[r][6].record(stream)
+            ev[r][ns].record(stream)
         torch.cuda.synchronize(device)
-        per = [sum(ev[r][st].elapsed_time(ev[r][st + 1]) for r in range(reps)) / reps for st in range(6)]
+        per = [sum(ev[r][i].elapsed_time(ev[r][i + 1]) for r in range(reps)) / reps for i in range(ns)]
         out["stage_ms"] = dict(zip(STAGE_NAMES, per))
 
     if want_e2e:
@@ -346,7 +350,7 @@ def main():
         pass
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"
-    sb = stage_bytes(cfg.Nx, cfg.Ny, w)
+    sb = {k: v for k, v in stage_bytes(cfg.Nx, cfg.Ny, w).items() if k in STAGE_NAMES}
     st = res["stage_ms"]
     dom = max(st, key=st.get)
     achieved = sb[dom] / (st[dom] * 1e-3) / 1e9

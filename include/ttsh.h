@@ -136,7 +136,8 @@ typedef enum {
   TTSH_STAGE_REAL = 2,      /* rhs1, rhs2 (a3)                                           */
   TTSH_STAGE_FWD_ROW = 3,   /* a4 row pass                                               */
   TTSH_STAGE_FWD_COL = 4,   /* a4 column pass                                            */
-  TTSH_STAGE_SPECTRAL = 5   /* a5                                                        */
+  TTSH_STAGE_SPECTRAL = 5,  /* a5                                                        */
+  TTSH_STAGE_REAL_FWD_ROW = 6 /* a3 fused into the a4 row pass (what ttsh_step runs in the conservative form instead of 2+3) */
 } ttsh_stage;
 int ttsh_run_stage(ttsh_handle* h, int stage);
 /* Copies a workspace array out for inspection: which = 0..4 real scratch (omega|rhs2, g_x|rhs1_x, g_y|rhs1_y, v_x, v_y;

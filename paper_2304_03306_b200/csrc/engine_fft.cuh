@@ -64,6 +64,27 @@ template <typename T, int NX> static cudaError_t go_fwd_row(const Geom& g, const
   k_fwd_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab));
   return cudaGetLastError();
 }
+template <typename T, int NX> static size_t fused_smem(const Geom& g) {
+  return RowCfg<T, NX>::SMEM + (size_t)RowCfg<T, NX>::L * 2 * ((g.Wx + 3) & ~3) * sizeof(cplx<T>);
+}
+template <typename T, int NX> static cudaError_t go_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy,
+                                                                  const void* w, const void* K, void* oGx, void* oGy, void* oS,
+                                                                  const void* tab, cudaStream_t s) {
+  using C = RowCfg<T, NX>;
+  k_fwd_row_fused<T, NX><<<(g.Ny / 2) / C::L, C::THREADS, fused_smem<T, NX>(g), s>>>(
+      g, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K, (cplx<T>*)oGx, (cplx<T>*)oGy, (cplx<T>*)oS,
+      static_cast<const cplx<T>*>(tab));
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
+                                                       const void* K, void* oGx, void* oGy, void* oS, const void* tab, cudaStream_t s) {
+  switch (g.Nx) {
+#define X(N) case N: return go_fwd_row_fused<T, N>(g, m, vx, vy, w, K, oGx, oGy, oS, tab, s);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
 template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
   switch (g.Nx) {
 #define X(N) case N: return go_inv_row<T, N>(g, b, nf, tab, v0, s);
@@ -83,6 +104,7 @@ template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, 
 template <typename T> cudaError_t prepare_rows(const Geom& g) {
   switch (g.Nx) {
 #define X(N) case N: { cudaError_t e = set_smem(k_inv_row<T, N>, RowCfg<T, N>::SMEM); if (e != cudaSuccess) return e; \
+                       e = set_smem(k_fwd_row_fused<T, N>, fused_smem<T, N>(g)); if (e != cudaSuccess) return e; \
                        return set_smem(k_fwd_row<T, N>, RowCfg<T, N>::SMEM); }
     TTSH_FOR_SIZES(X)
 #undef X

@@ -20,6 +20,9 @@
 #ifndef TTSH_PF_DIST
 #define TTSH_PF_DIST 296
 #endif
+#ifndef TTSH_PF_DIST_FUSED
+#define TTSH_PF_DIST_FUSED 64
+#endif
 #ifndef TTSH_ROW_MINB
 #define TTSH_ROW_MINB 2
 #endif
@@ -363,6 +366,96 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     const cplx<T> zp = line[fft_pad<NX>(mx)];
     const cplx<T> zm = conj(line[fft_pad<NX>((NX - mx) & (NX - 1))]);
     st_pair(dst + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// fused real-space + forward row pass (conservative advection form; a3 + the row half of a4 in one kernel).
+// One CTA line handles one row pair (yA = 4a+p, yB = yA+2) and runs three packed complex FFTs whose inputs are
+// evaluated on the fly from v_x, v_y, w, K — the right-hand sides never exist in HBM:
+//   FFT 1: Gx(yA) + i Gy(yA),  FFT 2: Gx(yB) + i Gy(yB),  FFT 3: S'(yA) + i S'(yB)
+//   Gx = rhs1_x + lambda0 v_y w,  Gy = rhs1_y - lambda0 v_x w,  S' = -gamma_w K w   (pointwise.cuh, k_realspace_cons)
+// FFT 1's unpacked spectra wait in a shared-memory stash until FFT 2 supplies the B halves of the (A, B) pairs.
+// Reads 4 real fields (+ K, w a second time from L2), writes 3 pruned intermediates.  grid = (Ny/2 / L)
+// ---------------------------------------------------------------------------------------
+template <typename T> struct Raw4 { T a, b, c, d; };
+
+template <typename T, int NX>
+__global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
+k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m, const T* __restrict__ vx,
+                const T* __restrict__ vy, const T* __restrict__ w, const T* __restrict__ K, cplx<T>* __restrict__ outGx,
+                cplx<T>* __restrict__ outGy, cplx<T>* __restrict__ outS, const cplx<T>* __restrict__ tabX) {
+  using C = RowCfg<T, NX>;
+  constexpr int TPL = C::TPL;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+  const int c = threadIdx.x / TPL, j = threadIdx.x % TPL;
+  const int rp = blockIdx.x * C::L + c;
+  const int a = rp >> 1, p = rp & 1;
+  const int Wx = g.Wx;
+  const int stash_elems = 2 * ((Wx + 3) & ~3);
+  cplx<T>* line = sm + c * C::LS;
+  cplx<T>* stash = sm + C::L * C::LS + c * stash_elems;      // [mx][Gx~, Gy~] of row yA
+  const size_t offA = (size_t)(4 * a + p) * NX, offB = offA + 2 * (size_t)NX;
+  const T scale = (T)g.inv_sqrt_nx;
+  const T beta = (T)m.beta, gv = (T)m.gamma_v, gw = (T)m.gamma_w, lam = (T)m.lambda0;
+  if (threadIdx.x == 0) {   // L2 prefetch of the 4 consecutive rows (x 4 fields) a CTA pair about one wave later reads
+    const int nb = blockIdx.x + TTSH_PF_DIST_FUSED;   // 12 row loads per CTA: a shorter distance keeps the rows in L2
+    if (nb < (int)gridDim.x && ((nb * C::L) & 1) == 0) {
+      const size_t off = (size_t)(2 * nb * C::L) * NX;
+      const unsigned bytes = (C::L >= 2 ? 2 * C::L : 4) * NX * sizeof(T);
+      prefetch_l2_bulk(vx + off, bytes); prefetch_l2_bulk(vy + off, bytes);
+      prefetch_l2_bulk(w + off, bytes);  prefetch_l2_bulk(K + off, bytes);
+    }
+  }
+  auto store = [&](int mm, int, cplx<T> z) { line[fft_pad<NX>(mm)] = z; };
+
+#pragma unroll 1
+  for (int f = 0; f < 2; ++f) {       // FFT 1 (row yA) and FFT 2 (row yB): Gx + i Gy
+    const size_t off = f ? offB : offA;
+    auto issue = [&](int x, int) -> Raw4<T> {
+      Raw4<T> r;
+      r.a = vx[off + x]; r.b = vy[off + x]; r.c = K[off + x]; r.d = w[off + x];
+      return r;
+    };
+    auto finish = [&](int, int, Raw4<T> r) -> cplx<T> {
+      const T cc = -beta * (r.a * r.a + r.b * r.b) - gv * r.c;            // rhs1 = cc * v   (Alg. 1 line 1)
+      return mk<T>(scale * (cc * r.a + lam * (r.b * r.d)), scale * (cc * r.b - lam * (r.a * r.d)));
+    };
+    fft_line<T, NX, -1, true>(j, line, tabX, make_loader<2>(issue, finish), store);
+    __syncthreads();
+    // unpack: Gx~(m) = (Z(m) + conj Z(-m))/2,  Gy~(m) = -i (Z(m) - conj Z(-m))/2
+    for (int mx = j; mx < Wx; mx += TPL) {
+      const cplx<T> zp = line[fft_pad<NX>(mx)];
+      const cplx<T> zm = conj(line[fft_pad<NX>((NX - mx) & (NX - 1))]);
+      const cplx<T> gx = (T)0.5 * (zp + zm), gy = (T)0.5 * mul_ni(zp - zm);
+      if (f == 0) {
+        stash[2 * mx] = gx;
+        stash[2 * mx + 1] = gy;
+      } else {   // same thread wrote stash[2 mx ..] in the first pass
+        const size_t idx = inter_pair_index(g, a, p, mx);
+        st_pair(outGx + idx, stash[2 * mx], gx);
+        st_pair(outGy + idx, stash[2 * mx + 1], gy);
+      }
+    }
+  }
+  {                                    // FFT 3: S'(yA) + i S'(yB)
+    auto issue = [&](int x, int) -> Raw4<T> {
+      Raw4<T> r;
+      r.a = K[offA + x]; r.b = w[offA + x]; r.c = K[offB + x]; r.d = w[offB + x];
+      return r;
+    };
+    auto finish = [&](int, int, Raw4<T> r) -> cplx<T> {
+      const T s = -gw * scale;
+      return mk<T>(s * (r.a * r.b), s * (r.c * r.d));                      // damping part of rhs2   (line 2)
+    };
+    fft_line<T, NX, -1, true>(j, line, tabX, make_loader<2>(issue, finish), store);
+    __syncthreads();
+    for (int mx = j; mx < Wx; mx += TPL) {
+      const cplx<T> zp = line[fft_pad<NX>(mx)];
+      const cplx<T> zm = conj(line[fft_pad<NX>((NX - mx) & (NX - 1))]);
+      st_pair(outS + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
+    }
   }
 }
 

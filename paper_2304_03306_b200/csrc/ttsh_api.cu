@@ -244,6 +244,12 @@ int enqueue_stage(ttsh_handle* h, int stage) {
       h->launches++;
       return TTSH_OK;
     }
+    case TTSH_STAGE_REAL_FWD_ROW:     // a3 + row half of a4 in one kernel (conservative form only)
+      if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
+      TRY(h, DISPATCH(h, launch_fwd_row_fused, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, h->Tm[0], h->Tm[1], h->Tm[2],
+                      h->tabX, h->stream));
+      h->launches++;
+      return TTSH_OK;
     case TTSH_STAGE_SPECTRAL:
       TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, h->S[0], h->S[1], h->S[2], h->what, h->psihat, h->v0, h->stream));
       h->launches++;
@@ -255,13 +261,19 @@ int enqueue_stage(ttsh_handle* h, int stage) {
 // one application of Algorithm 1.  The two inverse transforms of v (a6) are scheduled at the START of the
 // step that consumes v, together with those of w and grad w: the state carried between steps is (w^, v^(0)).
 int enqueue_step(ttsh_handle* h) {
-  for (int s = TTSH_STAGE_INV_COL; s <= TTSH_STAGE_SPECTRAL; ++s) {
-    int rc = enqueue_stage(h, s);
+  static const int fused[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL_FWD_ROW, TTSH_STAGE_FWD_COL, TTSH_STAGE_SPECTRAL};
+  static const int plain[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL, TTSH_STAGE_FWD_ROW, TTSH_STAGE_FWD_COL,
+                              TTSH_STAGE_SPECTRAL};
+  const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE;
+  const int* seq = f ? fused : plain;
+  const int n = f ? 5 : 6;
+  for (int i = 0; i < n; ++i) {
+    int rc = enqueue_stage(h, seq[i]);
     if (rc != TTSH_OK) return rc;
   }
   return TTSH_OK;
 }
-constexpr int LAUNCHES_PER_STEP = 6;
+inline int launches_per_step(const ttsh_handle* h) { return h->advection_form == TTSH_ADVECTION_CONSERVATIVE ? 5 : 6; }
 
 int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   const size_t P = (size_t)h->Nx * h->Ny;
@@ -415,7 +427,7 @@ int ttsh_step(ttsh_handle* h, int n) {
   for (int i = 0; i < n; ++i) {
     if (use_graph) {
       TRY(h, cudaGraphLaunch(h->graph_exec, h->stream));
-      h->launches += LAUNCHES_PER_STEP;
+      h->launches += launches_per_step(h);
     } else {
       int rc = enqueue_step(h);
       if (rc != TTSH_OK) return rc;

@@ -109,6 +109,26 @@ def test_real_space_kernel_matches_oracle_rhs(ttsh):
     s.close()
 
 
+@pytest.mark.parametrize("shape,dtype", [((256, 128), "f64"), ((64, 512), "f64"), ((1024, 256), "f32")])
+def test_fused_forward_row_kernel_equals_unfused_pair(ttsh, shape, dtype):
+    """k_fwd_row_fused (what ttsh_step runs) against k_realspace_cons + k_fwd_row, via the final state of one step."""
+    Nx, Ny = shape
+    mask = workloads.disk_mask(Nx, Ny, 0.5, 0.3 * min(Nx, Ny) * 0.5)
+    vel = workloads.planewave_velocity(Nx, Ny, 0.5, 11, amplitude=1.0)
+    a = ttsh.Solver(Nx, Ny, 0.5, 0.01, ttsh.baseline_params(), dtype, mask=mask)
+    b = ttsh.Solver(Nx, Ny, 0.5, 0.01, ttsh.baseline_params(), dtype, mask=mask)
+    a.set_velocity(*vel); b.set_velocity(*vel)
+    a.step(1)                                                   # fused sequence
+    for st in (ttsh.TTSH_STAGE_INV_COL, ttsh.TTSH_STAGE_INV_ROW, ttsh.TTSH_STAGE_REAL, ttsh.TTSH_STAGE_FWD_ROW,
+               ttsh.TTSH_STAGE_FWD_COL, ttsh.TTSH_STAGE_SPECTRAL):
+        b.run_stage(st)                                         # unfused sequence, same arithmetic per point
+    fa, fb = gpu_fields(a), gpu_fields(b)
+    tol = 1e-13 if dtype == "f64" else 1e-5
+    for x, y, name in zip(fa, fb, ("vx", "vy", "w", "psi")):
+        assert rel(x, y) <= tol, name
+    a.close(); b.close()
+
+
 # ---------------------------------------------------------------- whole-step parity
 CASES_SMALL = [
     ("C1-baseline", 64, 64, "baseline", "disk", 1e-2),

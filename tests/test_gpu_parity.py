@@ -288,3 +288,49 @@ def test_checkpoint_roundtrip_is_bit_exact_and_set_mask_keeps_state(ttsh):
     s.step(3); o.step(3)
     compare_state(s, o, TOL_F64_100, "after set_mask")
     s.close()
+
+
+# ---------------------------------------------------------------- C5: the configuration bench.py times (4096 x 4096)
+def _c5_pair(ttsh, dtype, geometry="disk"):
+    cfg = workloads.CONFIGS["C5" if geometry == "disk" else "C5p"]
+    mask = cfg.mask()
+    vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0, nmodes=16)
+    g = workloads.gaussian_velocity(cfg.Nx, cfg.Ny, cfg.seed, 1e-2, mask)
+    vel = (vel[0] + g[0], vel[1] + g[1])        # O(1) smooth part + the config's white-noise start
+    # the O(N^3) matrix oracle needs minutes per step here: its FFT backend (locked to it by
+    # tests/test_oracle_pins.py::test_fft_backend_locked_to_matrix_backend) is the reference at this size
+    return cfg, make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, dtype=dtype, transform="fft", vel=vel)
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", TOL_F64_1), ("f32", TOL_F32_1)])
+def test_C5_4096_disk_R900_single_step_full_fields(ttsh, dtype, tol):
+    cfg, (s, o) = _c5_pair(ttsh, dtype)
+    if dtype == "f32":
+        o.K = s.debug_real(5).cpu().numpy().astype(np.float64)
+    s.step(1); o.step(1)
+    compare_state(s, o, tol, f"C5 {dtype} step 1")
+    if dtype == "f64":
+        # properties that hold at any size (checked on the GPU fields themselves)
+        vx, vy, w, psi = gpu_fields(s)
+        kx = 2 * np.pi * np.fft.fftfreq(cfg.Nx, cfg.dx)[None, :]; ky = 2 * np.pi * np.fft.fftfreq(cfg.Ny, cfg.dx)[:, None]
+        vxh, vyh = np.fft.fft2(vx), np.fft.fft2(vy)
+        assert np.max(np.abs(kx * vxh + ky * vyh)) <= 1e-12 * np.max(np.abs(vxh))      # div v = 0
+        assert abs(w.sum()) <= 1e-9 * np.abs(w).sum()                                      # w^(0) = 0
+        wh = np.fft.fft2(w)
+        mxs = np.abs(np.fft.fftfreq(cfg.Nx) * cfg.Nx)[None, :]; mys = np.abs(np.fft.fftfreq(cfg.Ny) * cfg.Ny)[:, None]
+        outside = (mxs / cfg.Nx) ** 2 + (mys / cfg.Ny) ** 2 > 1.0 / 16 + 1e-12
+        assert np.max(np.abs(wh[outside])) <= 1e-11 * np.max(np.abs(wh))                   # band-limited to the 1/2 cutoff
+        # 9 more steps (10 in total), still against the oracle
+        s.step(9); o.step(9)
+        compare_state(s, o, 1e-11, "C5 f64 step 10")
+        d, od = s.diagnostics(), o.diagnostics((cfg.Nx // 2) * cfg.dx, (cfg.Ny // 2) * cfg.dx)
+        for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy"):
+            assert abs(d[key] - od[key]) <= TOL_DIAG * abs(od[key]), key
+    s.close()
+
+
+def test_C5_unconfined_periodic_single_step(ttsh):
+    cfg, (s, o) = _c5_pair(ttsh, "f64", geometry="none")
+    s.step(1); o.step(1)
+    compare_state(s, o, TOL_F64_1, "C5p step 1")
+    s.close()

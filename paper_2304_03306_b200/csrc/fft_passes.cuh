@@ -98,7 +98,8 @@ template <int LSHIFT> __device__ __forceinline__ void col_thread_map(int e, int&
 }
 
 // ---------------------------------------------------------------------------------------
-// inverse column pass.  grid = (NT tiles, fields)
+// inverse column pass.  grid = (NT tiles, fields, 2 parities): one half-length transform per CTA (both read the same
+// 64 KB spectrum tile; splitting them doubles the number of CTAs and halves the tail of the last wave)
 // ---------------------------------------------------------------------------------------
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
@@ -127,8 +128,8 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const bool half_rule = (2 * My == NH);     // the paper's 1/2 rule: |my| <= Ny/4 (uniform branch)
   const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
 
-#pragma unroll 1
-  for (int p = 0; p < 2; ++p) {
+  {
+    const int p = blockIdx.z;
     // a_p[mp] = (X[mp] + (-1)^p X[mp+NH]) W_Ny^{-p mp}; X[mp] is retained iff mp <= My, X[mp+NH] (my = mp-NH) iff
     // NH-mp <= My.
     // tail columns of the last tile are written too (zeros inside the row pitch), the row pass never reads them

@@ -164,7 +164,7 @@ def time_oracle(cfg, n_steps, budget_s, warmup=0):
 # --------------------------------------------------------------------------------------------------
 # what ttsh_step launches per Euler step in the default (conservative) form, and the stage ids of ttsh_run_stage
 STAGE_NAMES = ["k_inv_col", "k_inv_row", "k_fwd_row_fused", "k_fwd_col", "k_spectral"]
-STAGE_IDS = [0, 1, 6, 4, 5]
+STAGE_IDS = [0, 1, 6, 7, 8]
 
 
 def stage_bytes(Nx, Ny, w, conservative=True):
@@ -180,9 +180,9 @@ def stage_bytes(Nx, Ny, w, conservative=True):
         "k_inv_row": ninv_col * inter + ninv_row * real,
         "k_realspace": nreal_in * real + 3 * real,
         "k_fwd_row": 3 * real + 3 * inter,
-        "k_fwd_row_fused": 4 * real + 3 * inter,                 # v_x, v_y, w, K in; 3 pruned intermediates out
-        "k_fwd_col": 3 * inter + 3 * spec,
-        "k_spectral": 4 * spec + 2 * spec,                       # F^x, F^y, S^, w^ in; w^, psi^ out
+        "k_fwd_row_fused": 4 * real + 2 * inter,                 # v_x, v_y, w, K in; A~ = i kx Gy~ + S'~ and B~ = Gx~ out
+        "k_fwd_col": (2 * inter + 2 * spec) if conservative else (3 * inter + 3 * spec),
+        "k_spectral": (3 if conservative else 4) * spec + 2 * spec,   # A^, B^ (or F^x, F^y, S^), w^ in; w^, psi^ out
     }
 
 

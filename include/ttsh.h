@@ -137,7 +137,9 @@ typedef enum {
   TTSH_STAGE_FWD_ROW = 3,   /* a4 row pass                                               */
   TTSH_STAGE_FWD_COL = 4,   /* a4 column pass                                            */
   TTSH_STAGE_SPECTRAL = 5,  /* a5                                                        */
-  TTSH_STAGE_REAL_FWD_ROW = 6 /* a3 fused into the a4 row pass (what ttsh_step runs in the conservative form instead of 2+3) */
+  TTSH_STAGE_REAL_FWD_ROW = 6, /* a3 fused into the a4 row pass; emits A~ = i kx Gy~ + S'~ and B~ = Gx~ (conservative form)   */
+  TTSH_STAGE_FWD_COL_P2 = 7,  /* a4 column pass of those two intermediates                                                    */
+  TTSH_STAGE_SPECTRAL_P2 = 8  /* a5 from the two spectra: rhs^ = A^ - i ky B^.  ttsh_step runs 0, 1, 6, 7, 8 by default         */
 } ttsh_stage;
 int ttsh_run_stage(ttsh_handle* h, int stage);
 /* Copies a workspace array out for inspection: which = 0..4 real scratch (omega|rhs2, g_x|rhs1_x, g_y|rhs1_y, v_x, v_y;

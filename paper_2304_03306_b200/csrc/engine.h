@@ -11,9 +11,12 @@ template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, 
 template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, cudaStream_t s);
 template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const double* v0, cudaStream_t s);
 template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, cudaStream_t s);
-// fused real-space + forward row pass (conservative form): reads v_x, v_y, w, K; writes the three intermediates
+// fused real-space + forward row pass (conservative form): reads v_x, v_y, w, K; writes A~ = i kx Gy~ + S'~ and B~ = Gx~
 template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
-                                                       const void* K, void* oGx, void* oGy, void* oS, const void* tabX, cudaStream_t s);
+                                                       const void* K, void* oA, void* oB, const void* tabX, cudaStream_t s);
+// a5 for the two-spectrum form: rhs^ = A^ - i ky B^ (column mx = 0: A^ = S'^ + i Gy^ separated by Hermitian symmetry)
+template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model& m, const void* A, const void* B, void* w, void* psi,
+                                                     double* v0, cudaStream_t s);
 // set the dynamic shared-memory attribute of the pass kernels for this grid (no launch)
 template <typename T> cudaError_t prepare_rows(const Geom& g);
 template <typename T> cudaError_t prepare_cols(const Geom& g);

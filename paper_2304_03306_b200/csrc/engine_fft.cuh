@@ -68,18 +68,17 @@ template <typename T, int NX> static size_t fused_smem(const Geom& g) {
   return RowCfg<T, NX>::SMEM + (size_t)RowCfg<T, NX>::L * 2 * ((g.Wx + 3) & ~3) * sizeof(cplx<T>);
 }
 template <typename T, int NX> static cudaError_t go_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy,
-                                                                  const void* w, const void* K, void* oGx, void* oGy, void* oS,
+                                                                  const void* w, const void* K, void* oA, void* oB,
                                                                   const void* tab, cudaStream_t s) {
   using C = RowCfg<T, NX>;
   k_fwd_row_fused<T, NX><<<(g.Ny / 2) / C::L, C::THREADS, fused_smem<T, NX>(g), s>>>(
-      g, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K, (cplx<T>*)oGx, (cplx<T>*)oGy, (cplx<T>*)oS,
-      static_cast<const cplx<T>*>(tab));
+      g, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab));
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
-                                                       const void* K, void* oGx, void* oGy, void* oS, const void* tab, cudaStream_t s) {
+                                                       const void* K, void* oA, void* oB, const void* tab, cudaStream_t s) {
   switch (g.Nx) {
-#define X(N) case N: return go_fwd_row_fused<T, N>(g, m, vx, vy, w, K, oGx, oGy, oS, tab, s);
+#define X(N) case N: return go_fwd_row_fused<T, N>(g, m, vx, vy, w, K, oA, oB, tab, s);
     TTSH_FOR_SIZES(X)
 #undef X
   }

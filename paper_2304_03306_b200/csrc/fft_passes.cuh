@@ -376,16 +376,20 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 // evaluated on the fly from v_x, v_y, w, K — the right-hand sides never exist in HBM:
 //   FFT 1: Gx(yA) + i Gy(yA),  FFT 2: Gx(yB) + i Gy(yB),  FFT 3: S'(yA) + i S'(yB)
 //   Gx = rhs1_x + lambda0 v_y w,  Gy = rhs1_y - lambda0 v_x w,  S' = -gamma_w K w   (pointwise.cuh, k_realspace_cons)
-// FFT 1's unpacked spectra wait in a shared-memory stash until FFT 2 supplies the B halves of the (A, B) pairs.
-// Reads 4 real fields (+ K, w a second time from L2), writes 3 pruned intermediates.  grid = (Ny/2 / L)
+// Line 3 of Algorithm 1 is rhs^ = i kx Gy^ - i ky Gx^ + S'^, and i kx is still diagonal after the row pass, so only TWO
+// intermediates leave the kernel:   A~ = i kx Gy~ + S'~   and   B~ = Gx~    (then rhs^ = A^ - i ky B^ in k_spectral_p2).
+// At mx = 0, where i kx Gy~ vanishes but the mean-flow update (line 8) needs Gy^(0,0), the real numbers S'~(0,y) and
+// Gy~(0,y) travel together as A~(0,y) = S'~ + i Gy~; the spectral kernel separates them by Hermitian symmetry.
+// Spectra of the first two FFTs wait in a shared-memory stash until their partners arrive.
+// Reads 4 real fields (+ K, w a second time from L2), writes 2 pruned intermediates.  grid = (Ny/2 / L)
 // ---------------------------------------------------------------------------------------
 template <typename T> struct Raw4 { T a, b, c, d; };
 
 template <typename T, int NX>
 __global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
 k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m, const T* __restrict__ vx,
-                const T* __restrict__ vy, const T* __restrict__ w, const T* __restrict__ K, cplx<T>* __restrict__ outGx,
-                cplx<T>* __restrict__ outGy, cplx<T>* __restrict__ outS, const cplx<T>* __restrict__ tabX) {
+                const T* __restrict__ vy, const T* __restrict__ w, const T* __restrict__ K, cplx<T>* __restrict__ outA,
+                cplx<T>* __restrict__ outB, const cplx<T>* __restrict__ tabX) {
   using C = RowCfg<T, NX>;
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -396,9 +400,10 @@ k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   const int Wx = g.Wx;
   const int stash_elems = 2 * ((Wx + 3) & ~3);
   cplx<T>* line = sm + c * C::LS;
-  cplx<T>* stash = sm + C::L * C::LS + c * stash_elems;      // [mx][Gx~, Gy~] of row yA
+  cplx<T>* stash = sm + C::L * C::LS + c * stash_elems;      // 2 complex per mx, owned by the thread of that mx
   const size_t offA = (size_t)(4 * a + p) * NX, offB = offA + 2 * (size_t)NX;
   const T scale = (T)g.inv_sqrt_nx;
+  const T dkx = (T)g.dkx;
   const T beta = (T)m.beta, gv = (T)m.gamma_v, gw = (T)m.gamma_w, lam = (T)m.lambda0;
   if (threadIdx.x == 0) {   // L2 prefetch of the 4 consecutive rows (x 4 fields) a CTA pair about one wave later reads
     const int nb = blockIdx.x + TTSH_PF_DIST_FUSED;   // 12 row loads per CTA: a shorter distance keeps the rows in L2
@@ -433,14 +438,13 @@ k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       if (f == 0) {
         stash[2 * mx] = gx;
         stash[2 * mx + 1] = gy;
-      } else {   // same thread wrote stash[2 mx ..] in the first pass
-        const size_t idx = inter_pair_index(g, a, p, mx);
-        st_pair(outGx + idx, stash[2 * mx], gx);
-        st_pair(outGy + idx, stash[2 * mx + 1], gy);
+      } else {   // the same thread wrote stash[2 mx ..] in the first pass
+        st_pair(outB + inter_pair_index(g, a, p, mx), stash[2 * mx], gx);     // B~ = Gx~ of rows (yA, yB)
+        stash[2 * mx] = gy;                                                   // stash now holds Gy~ of (yB, yA)
       }
     }
   }
-  {                                    // FFT 3: S'(yA) + i S'(yB)
+  {                                    // FFT 3: S'(yA) + i S'(yB), then A~ = i kx Gy~ + S'~
     auto issue = [&](int x, int) -> Raw4<T> {
       Raw4<T> r;
       r.a = K[offA + x]; r.b = w[offA + x]; r.c = K[offB + x]; r.d = w[offB + x];
@@ -455,7 +459,17 @@ k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m,
     for (int mx = j; mx < Wx; mx += TPL) {
       const cplx<T> zp = line[fft_pad<NX>(mx)];
       const cplx<T> zm = conj(line[fft_pad<NX>((NX - mx) & (NX - 1))]);
-      st_pair(outS + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
+      cplx<T> sa = (T)0.5 * (zp + zm), sb = (T)0.5 * mul_ni(zp - zm);       // S'~ of rows yA, yB
+      const cplx<T> gyA = stash[2 * mx + 1], gyB = stash[2 * mx];
+      if (mx == 0) {                   // all four numbers are real here: pack Gy~(0,y) into the imaginary part
+        sa = mk<T>(sa.x, gyA.x);
+        sb = mk<T>(sb.x, gyB.x);
+      } else {
+        const T kx = dkx * (T)mx;
+        sa = sa + kx * mul_i(gyA);
+        sb = sb + kx * mul_i(gyB);
+      }
+      st_pair(outA + inter_pair_index(g, a, p, mx), sa, sb);
     }
   }
 }

@@ -150,6 +150,65 @@ k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __res
   psi[idx] = inv_k2<T>(g, mx, my) * out;                       // line 13
 }
 
+// a5 for the two-spectrum form produced by k_fwd_row_fused:  rhs^ = A^ - i ky B^  with  A = i kx Gy + S',  B = Gx.
+// Column mx = 0 carries A^(0,my) = S'^(0,my) + i Gy^(0,my); S'(0,.) and Gy(0,.) are transforms of real sequences, so
+//   S'^(0,my) = (A^(0,my) + conj A^(0,-my)) / 2,   i Gy^(0,my) = (A^(0,my) - conj A^(0,-my)) / 2,
+// and i kx Gy^ = 0 there.  Gy^(0,0) = Im A^(0,0) and Gx^(0,0) = Re B^(0,0) feed the mean-flow update (line 8, Eq. C1).
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_spectral_p2(Geom g, Model m, const cplx<T>* __restrict__ A, const cplx<T>* __restrict__ B, cplx<T>* w,
+              cplx<T>* __restrict__ psi, double* v0) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
+  const int t = (int)(idx / ((size_t)g.Hy * g.CW));
+  const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
+  const int q = rem >> g.cw_shift;
+  const int mx = t * g.CW + (rem & (g.CW - 1));
+  if (mx >= g.Wx) return;
+  const int my = q <= g.My ? q : q - g.Hy;
+  const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
+  const T dt = (T)m.dt;
+  auto factor = [&](int my_) -> T {          // exp(sigma(k) dt), line 4
+    const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my_);
+    const T k2 = kx * kx + ky * ky;
+    const T sigma = -(T)m.alpha - (T)m.Gamma0 * k2 - (T)m.Gamma2 * k2 * k2;
+    return sizeof(T) == 8 ? (T)exp((double)(sigma * dt)) : (T)expf((float)(sigma * dt));
+  };
+  if (mx == 0) {
+    if (my < 0) return;                                   // written by the thread of (0, -my)
+    if (my == 0) {
+      const double e = exp(-m.alpha * m.dt);
+      v0[0] = e * (v0[0] + m.dt * (double)B[idx].x);      // Gx^(0,0)
+      v0[1] = e * (v0[1] + m.dt * (double)A[idx].y);      // Gy^(0,0)
+      w[idx] = mk<T>(0, 0);
+      psi[idx] = mk<T>(0, 0);
+      return;
+    }
+    const size_t idn = spec_index(g, g.Hy - my, 0);       // row of -my, mx = 0
+    cplx<T> out = mk<T>(0, 0);
+    if (!cut) {
+      const T ky = (T)(g.dky * my);
+      const cplx<T> sp = (T)0.5 * (A[idx] + conj(A[idn]));                   // S'^(0, my); S'^(0,-my) = conj
+      const cplx<T> rp = sp - ky * mul_i(B[idx]);                            // rhs^(0, my)
+      const cplx<T> rn = conj(sp) + ky * mul_i(B[idn]);                      // rhs^(0,-my)
+      const T e = factor(my);
+      const cplx<T> np_ = e * (w[idx] + dt * rp), nn = e * (w[idn] + dt * rn);
+      out = (T)0.5 * (np_ + conj(nn));                                       // line 12
+    }
+    const T ik2 = inv_k2<T>(g, 0, my);
+    w[idx] = out;
+    w[idn] = conj(out);
+    psi[idx] = ik2 * out;
+    psi[idn] = ik2 * conj(out);
+    return;
+  }
+  const T ky = (T)(g.dky * my);
+  cplx<T> out = factor(my) * (w[idx] + dt * (A[idx] - ky * mul_i(B[idx])));  // lines 3-4
+  out = cut ? mk<T>(0, 0) : out;
+  w[idx] = out;
+  psi[idx] = inv_k2<T>(g, mx, my) * out;                                     // line 13
+}
+
 // ttsh_set_velocity: w^ = i kx v^y - i ky v^x, v^(0) kept, then the same post-processing
 template <typename T>
 __global__ void __launch_bounds__(256)

@@ -246,8 +246,17 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     }
     case TTSH_STAGE_REAL_FWD_ROW:     // a3 + row half of a4 in one kernel (conservative form only)
       if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
-      TRY(h, DISPATCH(h, launch_fwd_row_fused, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, h->Tm[0], h->Tm[1], h->Tm[2],
-                      h->tabX, h->stream));
+      TRY(h, DISPATCH(h, launch_fwd_row_fused, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, h->Tm[0], h->Tm[1], h->tabX, h->stream));
+      h->launches++;
+      return TTSH_OK;
+    case TTSH_STAGE_FWD_COL_P2: {      // column pass of the two intermediates A~, B~ of TTSH_STAGE_REAL_FWD_ROW
+      Batch cb = make_batch({op(h->Tm[0], h->S[0], 0), op(h->Tm[1], h->S[1], 0)});
+      TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 2, h->tabY, h->tabS, h->stream));
+      h->launches++;
+      return TTSH_OK;
+    }
+    case TTSH_STAGE_SPECTRAL_P2:
+      TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, h->S[0], h->S[1], h->what, h->psihat, h->v0, h->stream));
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_SPECTRAL:
@@ -261,7 +270,8 @@ int enqueue_stage(ttsh_handle* h, int stage) {
 // one application of Algorithm 1.  The two inverse transforms of v (a6) are scheduled at the START of the
 // step that consumes v, together with those of w and grad w: the state carried between steps is (w^, v^(0)).
 int enqueue_step(ttsh_handle* h) {
-  static const int fused[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL_FWD_ROW, TTSH_STAGE_FWD_COL, TTSH_STAGE_SPECTRAL};
+  static const int fused[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL_FWD_ROW, TTSH_STAGE_FWD_COL_P2,
+                              TTSH_STAGE_SPECTRAL_P2};
   static const int plain[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL, TTSH_STAGE_FWD_ROW, TTSH_STAGE_FWD_COL,
                               TTSH_STAGE_SPECTRAL};
   const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE;

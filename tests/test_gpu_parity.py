@@ -118,7 +118,7 @@ def test_fused_forward_row_kernel_equals_unfused_pair(ttsh, shape, dtype):
     a = ttsh.Solver(Nx, Ny, 0.5, 0.01, ttsh.baseline_params(), dtype, mask=mask)
     b = ttsh.Solver(Nx, Ny, 0.5, 0.01, ttsh.baseline_params(), dtype, mask=mask)
     a.set_velocity(*vel); b.set_velocity(*vel)
-    a.step(1)                                                   # fused sequence
+    a.step(1)                                                   # fused sequence (stages 0, 1, 6, 7, 8)
     for st in (ttsh.TTSH_STAGE_INV_COL, ttsh.TTSH_STAGE_INV_ROW, ttsh.TTSH_STAGE_REAL, ttsh.TTSH_STAGE_FWD_ROW,
                ttsh.TTSH_STAGE_FWD_COL, ttsh.TTSH_STAGE_SPECTRAL):
         b.run_stage(st)                                         # unfused sequence, same arithmetic per point

@@ -37,7 +37,7 @@ namespace ttsh {
 // ---------------------------------------------------------------------------------------
 template <typename T, int NX> struct RowCfg {
   static constexpr int TPL = fft_tpl<NX>();
-  static constexpr int L = (TPL >= 256) ? 1 : (TPL >= 128 ? 2 : 4);          // row pairs per CTA
+  static constexpr int L = (TPL >= 256) ? 1 : (TPL >= 64 ? 2 : 4);           // row pairs per CTA
   static constexpr int THREADS = L * TPL;
   static constexpr int LS = fft_line_elems<NX>() + 4;                          // line stride (elements)
   static constexpr size_t SMEM = (size_t)L * LS * sizeof(cplx<T>);
@@ -47,7 +47,8 @@ template <typename T, int NX> struct RowCfg {
 // of shared memory (fp64 4096: 2 columns, fp32 4096: 4), at least 2 and at most 8 columns
 __host__ __device__ constexpr int col_tile_width(int Ny, int elem_bytes) {
   int cw = (TTSH_COL_BYTES / elem_bytes) / (Ny / 2);
-  return cw < 2 ? 2 : (cw > 8 ? 8 : cw);
+  const int cap = Ny >= 2048 ? 8 : 4;      // small grids: more, smaller CTAs (the GPU has 148 SMs to fill)
+  return cw < 2 ? 2 : (cw > cap ? cap : cw);
 }
 template <typename T, int NY> struct ColCfg {
   static constexpr int NH = NY / 2;
@@ -57,7 +58,7 @@ template <typename T, int NY> struct ColCfg {
   static constexpr int THREADS = L * TPL;
   static constexpr int LS = fft_line_elems<NH>() + 8 / L;
   static constexpr size_t SMEM = (size_t)L * LS * sizeof(cplx<T>);
-  static constexpr int MINB = THREADS <= 256 ? 2 : 1;
+  static constexpr int MINB = (THREADS <= 256 || sizeof(T) == 4) ? 2 : 1;    // fp32: 512 threads x 64 registers
 };
 
 // 2-element (A, B) pair access of the row passes

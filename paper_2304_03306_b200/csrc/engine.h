@@ -33,6 +33,8 @@ template <typename T> cudaError_t launch_psi_from_w(const Geom& g, const void* w
 template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s);
 template <typename T> cudaError_t launch_square(size_t n, const void* in, void* out, cudaStream_t s);
 template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, cudaStream_t s);
+// natural <-> permuted row layout of an internal real field (to_perm = 1: natural -> permuted)
+template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* in, void* out, int to_perm, cudaStream_t s);
 constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs
 template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,
                                               const void* w, double* partial, double* out, cudaStream_t s);

@@ -188,11 +188,35 @@ template <int DIR, typename T> __device__ __forceinline__ cplx<T> twiddle(const 
 // the slot k = 0..15 is a compile-time constant after unrolling, so loaders can prune by k at compile time
 template <int B, class I, class F> struct Loader {
   static constexpr int BATCHES = B;
+  static constexpr int VEC = 1;
   I issue;
   F finish;
 };
 template <int B = 1, class I, class F> __device__ __forceinline__ Loader<B, I, F> make_loader(I i, F f) {
   return Loader<B, I, F>{i, f};
+}
+// vector loader: issue(k0, Raw* out) fills the 4 consecutive slots k0..k0+3 (k0 a multiple of 4) with wide loads
+template <int B, class Raw, class I, class F> struct VecLoader {
+  static constexpr int BATCHES = B;
+  static constexpr int VEC = 4;
+  using raw_t = Raw;
+  I issue;
+  F finish;
+};
+template <int B, class Raw, class I, class F> __device__ __forceinline__ VecLoader<B, Raw, I, F> make_vec_loader(I i, F f) {
+  return VecLoader<B, Raw, I, F>{i, f};
+}
+// vector store of the last stage: f(k0, const cplx<T>* v4) receives the 4 consecutive slots k0..k0+3
+template <class F> struct VecStore { F f; };
+template <class F> __device__ __forceinline__ VecStore<F> make_vec_store(F f) { return VecStore<F>{f}; }
+template <class S> struct is_vec_store : std::false_type {};
+template <class F> struct is_vec_store<VecStore<F>> : std::true_type {};
+// permuted row layout of the internal real fields: element x = j + k TPL (the 16 points one thread owns are k = 0..15)
+// is stored at ((k >> 2) TPL + j) 4 + (k & 3), so that a thread moves its points with 4 wide accesses (LDG/STG.256 in
+// fp64) and a warp instruction still covers 1 KB of contiguous memory.  TPL = row length / 16.
+__host__ __device__ __forceinline__ int perm_index(int x, int tpl) {
+  const int j = x % tpl, k = x / tpl;
+  return ((k >> 2) * tpl + j) * 4 + (k & 3);
 }
 
 // fire-and-forget accumulation  *p += v  (two scalar reductions; each address receives exactly one addend per pass,
@@ -252,6 +276,16 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
     constexpr int SLOTS = NB * R;
 #pragma unroll
     for (int bat = 0; bat < NBAT; ++bat) {
+      if constexpr (Load::VEC == 4) {
+        typename Load::raw_t raw[SLOTS / NBAT];
+#pragma unroll
+        for (int s = 0; s < SLOTS / NBAT; s += 4) load.issue(bat * (SLOTS / NBAT) + s, raw + s);
+#pragma unroll
+        for (int s = 0; s < SLOTS / NBAT; ++s) {
+          const int k = bat * (SLOTS / NBAT) + s;
+          v[k % NB][k / NB] = load.finish(j0 + k * TPL, k, raw[s]);
+        }
+      } else {
       decltype(load.issue(0, 0)) raw[SLOTS / NBAT];
 #pragma unroll
       for (int s = 0; s < SLOTS / NBAT; ++s) {
@@ -262,6 +296,7 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
       for (int s = 0; s < SLOTS / NBAT; ++s) {
         const int k = bat * (SLOTS / NBAT) + s;      // slot k = b + r NB  <->  v[b][r]
         v[k % NB][k / NB] = load.finish(j0 + k * TPL, k, raw[s]);
+      }
       }
     }
   } else {
@@ -282,16 +317,28 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
     dftR<R, DIR>(v[b]);
   }
   if (!last || SYNC_LAST) __syncthreads();     // every thread has finished reading this buffer
+  if constexpr (last && is_vec_store<Store>::value) {
+    // last stage, vector store: slot k = b + r NB holds output index j0 + k TPL
 #pragma unroll
-  for (int b = 0; b < NB; ++b) {
-    const int j = j0 + b * TPL;
-    const int k = j & (NS - 1);
-    const int base = (j - k) * R + k;
+    for (int k0 = 0; k0 < NB * R; k0 += 4) {
+      cplx<T> t4[4];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      const int o = base + r * NS;
-      if constexpr (last) store(o, b + r * NB, v[b][r]);     // last stage: o = j0 + k TPL with slot k = b + r NB
-      else sm[fft_pad<N>(o)] = v[b][r];
+      for (int i = 0; i < 4; ++i) t4[i] = v[(k0 + i) % NB][(k0 + i) / NB];
+      store.f(k0, t4);
+    }
+  } else {
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      const int j = j0 + b * TPL;
+      const int k = j & (NS - 1);
+      const int base = (j - k) * R + k;
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const int o = base + r * NS;
+        if constexpr (last) {
+          if constexpr (!is_vec_store<Store>::value) store(o, b + r * NB, v[b][r]);   // o = j0 + k TPL, slot k = b + r NB
+        } else sm[fft_pad<N>(o)] = v[b][r];
+      }
     }
   }
   if constexpr (!last) {

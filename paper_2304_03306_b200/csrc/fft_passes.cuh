@@ -80,6 +80,25 @@ __device__ __forceinline__ void st_pair(cplx<float>* p, cplx<float> a, cplx<floa
   asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
 }
 
+// 4 consecutive scalars of a (permuted) real row: one 32-byte (fp64) / 16-byte (fp32) access
+template <typename T> struct Quad { T v[4]; };
+__device__ __forceinline__ Quad<double> ld_quad(const double* p) {
+  Quad<double> r;
+  asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.v[0]), "=d"(r.v[1]), "=d"(r.v[2]), "=d"(r.v[3]) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ Quad<float> ld_quad(const float* p) {
+  Quad<float> r;
+  asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_quad(double* p, double a, double b, double c, double d) {
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d));
+}
+__device__ __forceinline__ void st_quad(float* p, float a, float b, float c, float d) {
+  asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d));
+}
+
 // spectral multiplier of the inverse column pass (SpecMode).  mode is uniform per CTA.  No division: psi^ = w^/k^2 is kept
 // as a second spectrum by the spectral kernel (line 13 of Algorithm 1 is evaluated once per mode there).
 template <typename T>
@@ -270,7 +289,7 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src);
   T* __restrict__ dstA = static_cast<T*>(op.dst) + (size_t)(4 * a + p) * NX;
   T* __restrict__ dstB = dstA + 2 * NX;
-  const int mode = op.mode;
+  const int mode = op.mode & RM_MODE_MASK;
   const T scale = (T)g.inv_sqrt_nx;
   const T dkx = (T)g.dkx;
   const T meany = (mode == RM_NIKX_MEANY) ? (T)(v0[1] * g.inv_sqrt_ny) : (T)0;
@@ -297,10 +316,22 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     if (neg) { wa = conj(wa); wb = conj(wb); }
     return scale * mk<T>(wa.x - wb.y, wa.y + wb.x);
   };
-  auto store = [&](int x, int, cplx<T> z) {
-    dstA[x] = z.x;
-    dstB[x] = z.y;
-  };
+  // output rows: natural order (caller-owned buffers) or the permuted internal layout (perm_index, fft_core.cuh): the
+  // 4 slots k0..k0+3 of this thread are then 4 consecutive scalars -> one wide store per row
+  const bool perm = (op.mode & RM_PERM) != 0;
+  auto store = make_vec_store([&](int k0, const cplx<T>* z) {
+    if (perm) {
+      const size_t e = ((size_t)(k0 >> 2) * TPL + j) * 4;
+      st_quad(dstA + e, z[0].x, z[1].x, z[2].x, z[3].x);
+      st_quad(dstB + e, z[0].y, z[1].y, z[2].y, z[3].y);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        dstA[j + (k0 + i) * TPL] = z[i].x;
+        dstB[j + (k0 + i) * TPL] = z[i].y;
+      }
+    }
+  });
   if (4 * (Wx - 1) == NX) {
     // the paper's 1/2 rule: retained mx = 0..NX/4 = 4 TPL.  Input slot k (m = j + k TPL): k <= 3 holds +mx = m, k = 4 only
     // the single point m = NX/4 (j = 0), k = 5..11 nothing, k = 12..15 holds -mx with mx = NX - m: compile-time pruning.
@@ -358,8 +389,20 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
                        (C::L >= 2 ? 2 * C::L : 4) * NX * sizeof(T));
   }
 
-  auto load = make_loader([&](int x, int) -> cplx<T> { return mk<T>(srcA[x], srcB[x]); },
-                          [&](int, int, cplx<T> raw) -> cplx<T> { return scale * raw; });
+  const bool perm = (op.mode & RM_PERM) != 0;     // input rows in the permuted internal layout (else natural order)
+  auto load = make_vec_loader<1, cplx<T>>(
+      [&](int k0, cplx<T>* out) {
+        if (perm) {
+          const size_t e = ((size_t)(k0 >> 2) * TPL + j) * 4;
+          const Quad<T> qa = ld_quad(srcA + e), qb = ld_quad(srcB + e);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) out[i] = mk<T>(qa.v[i], qb.v[i]);
+        } else {
+#pragma unroll
+          for (int i = 0; i < 4; ++i) out[i] = mk<T>(srcA[j + (k0 + i) * TPL], srcB[j + (k0 + i) * TPL]);
+        }
+      },
+      [&](int, int, cplx<T> raw) -> cplx<T> { return scale * raw; });
   auto store = [&](int m, int, cplx<T> z) { line[fft_pad<NX>(m)] = z; };
   fft_line<T, NX, -1, true>(j, line, tabX, load, store);
   __syncthreads();
@@ -420,16 +463,18 @@ k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m,
 #pragma unroll 1
   for (int f = 0; f < 2; ++f) {       // FFT 1 (row yA) and FFT 2 (row yB): Gx + i Gy
     const size_t off = f ? offB : offA;
-    auto issue = [&](int x, int) -> Raw4<T> {
-      Raw4<T> r;
-      r.a = vx[off + x]; r.b = vy[off + x]; r.c = K[off + x]; r.d = w[off + x];
-      return r;
+    // inputs are in the permuted internal layout: slots k0..k0+3 of this thread are 4 consecutive scalars per field
+    auto issue = [&](int k0, Raw4<T>* out) {
+      const size_t e = off + ((size_t)(k0 >> 2) * TPL + j) * 4;
+      const Quad<T> q0 = ld_quad(vx + e), q1 = ld_quad(vy + e), q2 = ld_quad(K + e), q3 = ld_quad(w + e);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { out[i].a = q0.v[i]; out[i].b = q1.v[i]; out[i].c = q2.v[i]; out[i].d = q3.v[i]; }
     };
     auto finish = [&](int, int, Raw4<T> r) -> cplx<T> {
       const T cc = -beta * (r.a * r.a + r.b * r.b) - gv * r.c;            // rhs1 = cc * v   (Alg. 1 line 1)
       return mk<T>(scale * (cc * r.a + lam * (r.b * r.d)), scale * (cc * r.b - lam * (r.a * r.d)));
     };
-    fft_line<T, NX, -1, true>(j, line, tabX, make_loader<2>(issue, finish), store);
+    fft_line<T, NX, -1, true>(j, line, tabX, make_vec_loader<2, Raw4<T>>(issue, finish), store);
     __syncthreads();
     // unpack: Gx~(m) = (Z(m) + conj Z(-m))/2,  Gy~(m) = -i (Z(m) - conj Z(-m))/2
     for (int mx = j; mx < Wx; mx += TPL) {
@@ -446,16 +491,17 @@ k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m,
     }
   }
   {                                    // FFT 3: S'(yA) + i S'(yB), then A~ = i kx Gy~ + S'~
-    auto issue = [&](int x, int) -> Raw4<T> {
-      Raw4<T> r;
-      r.a = K[offA + x]; r.b = w[offA + x]; r.c = K[offB + x]; r.d = w[offB + x];
-      return r;
+    auto issue = [&](int k0, Raw4<T>* out) {
+      const size_t e = ((size_t)(k0 >> 2) * TPL + j) * 4;
+      const Quad<T> q0 = ld_quad(K + offA + e), q1 = ld_quad(w + offA + e), q2 = ld_quad(K + offB + e), q3 = ld_quad(w + offB + e);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { out[i].a = q0.v[i]; out[i].b = q1.v[i]; out[i].c = q2.v[i]; out[i].d = q3.v[i]; }
     };
     auto finish = [&](int, int, Raw4<T> r) -> cplx<T> {
       const T s = -gw * scale;
       return mk<T>(s * (r.a * r.b), s * (r.c * r.d));                      // damping part of rhs2   (line 2)
     };
-    fft_line<T, NX, -1, true>(j, line, tabX, make_loader<2>(issue, finish), store);
+    fft_line<T, NX, -1, true>(j, line, tabX, make_vec_loader<2, Raw4<T>>(issue, finish), store);
     __syncthreads();
     for (int mx = j; mx < Wx; mx += TPL) {
       const cplx<T> zp = line[fft_pad<NX>(mx)];

@@ -266,6 +266,20 @@ k_psi_from_w(Geom g, const cplx<T>* __restrict__ w, cplx<T>* __restrict__ psi) {
   psi[idx] = (mx >= g.Wx || (mx == 0 && my == 0)) ? mk<T>(0, 0) : inv_k2<T>(g, mx, my) * w[idx];
 }
 
+// natural <-> permuted row layout of the internal real fields (perm_index: x = j + k TPL -> ((k>>2) TPL + j) 4 + (k&3)).
+// Only for buffers that cross the C ABI in natural order (a processed mask, debug copies).
+template <typename T>
+__global__ void k_permute_rows(int Nx, size_t n, const T* __restrict__ in, T* __restrict__ out, int to_perm) {
+  const int tpl = Nx / 16;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t row = i / Nx;
+    const int x = (int)(i - row * Nx);
+    const int j = x % tpl, k = x / tpl;
+    const size_t pi = row * Nx + (size_t)(((k >> 2) * tpl + j) * 4 + (k & 3));
+    if (to_perm) out[pi] = in[i]; else out[i] = in[pi];
+  }
+}
+
 // ---------------------------------------------------------------------------------------
 // small helpers for Algorithm 2
 // ---------------------------------------------------------------------------------------

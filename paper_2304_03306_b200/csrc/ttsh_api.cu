@@ -215,11 +215,13 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     }
     case TTSH_STAGE_INV_ROW: {
       if (h->advection_form == TTSH_ADVECTION_CONSERVATIVE) {
-        Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE), op(h->Tm[3], h->R[3], RM_ONE), op(h->Tm[2], h->R[4], RM_NIKX_MEANY)});
+        Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE | RM_PERM), op(h->Tm[3], h->R[3], RM_ONE | RM_PERM),
+                               op(h->Tm[2], h->R[4], RM_NIKX_MEANY | RM_PERM)});
         TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 3, h->tabX, h->v0, h->stream));
       } else {
-        Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE), op(h->Tm[0], h->R[1], RM_IKX), op(h->Tm[1], h->R[2], RM_ONE),
-                               op(h->Tm[3], h->R[3], RM_ONE), op(h->Tm[2], h->R[4], RM_NIKX_MEANY)});
+        Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE | RM_PERM), op(h->Tm[0], h->R[1], RM_IKX | RM_PERM),
+                               op(h->Tm[1], h->R[2], RM_ONE | RM_PERM), op(h->Tm[3], h->R[3], RM_ONE | RM_PERM),
+                               op(h->Tm[2], h->R[4], RM_NIKX_MEANY | RM_PERM)});
         TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 5, h->tabX, h->v0, h->stream));
       }
       h->launches++;
@@ -233,7 +235,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_FWD_ROW: {
-      Batch rb = make_batch({op(h->R[1], h->Tm[0], 0), op(h->R[2], h->Tm[1], 0), op(h->R[0], h->Tm[2], 0)});
+      Batch rb = make_batch({op(h->R[1], h->Tm[0], RM_PERM), op(h->R[2], h->Tm[1], RM_PERM), op(h->R[0], h->Tm[2], RM_PERM)});
       TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->stream));
       h->launches++;
       return TTSH_OK;
@@ -293,8 +295,9 @@ int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
     h->launches++;
     return TTSH_OK;
   }
-  if (kind == TTSH_MASK_PROCESSED) {
-    TRY(h, cudaMemcpyAsync(h->K, mask, P * w, cudaMemcpyDeviceToDevice, h->stream));
+  if (kind == TTSH_MASK_PROCESSED) {   // K is kept in the permuted internal row layout
+    TRY(h, DISPATCH(h, launch_permute, h->Nx, P, mask, h->K, 1, h->stream));
+    h->launches++;
     return TTSH_OK;
   }
   // Algorithm 2: K = ( iDFT[ lowpass_{1/4}( DFT[K_naive] ) ] )^2
@@ -305,7 +308,7 @@ int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   if (rc != TTSH_OK) return rc;
   Batch cb = make_batch({op(h->S[0], h->Tm[0], SM_LOWPASS4)});
   TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 1, h->tabY, h->tabS, h->v0, h->stream));
-  Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE)});
+  Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE | RM_PERM)});
   TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 1, h->tabX, h->v0, h->stream));
   TRY(h, DISPATCH(h, launch_square, P, h->R[0], h->K, h->stream));
   h->launches += 3;
@@ -527,8 +530,9 @@ int ttsh_run_stage(ttsh_handle* h, int stage) {
 int ttsh_debug_get_real(ttsh_handle* h, int which, void* dst) {
   if (!h || !dst || which < 0 || which > 5) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
-  const void* src = which == 5 ? h->K : h->R[which];
-  TRY(h, cudaMemcpyAsync(dst, src, (size_t)h->Nx * h->Ny * (size_t)h->dtype, cudaMemcpyDeviceToDevice, h->stream));
+  const void* src = which == 5 ? h->K : h->R[which];   // internal fields are in the permuted row layout
+  TRY(h, DISPATCH(h, launch_permute, h->Nx, (size_t)h->Nx * h->Ny, src, dst, 0, h->stream));
+  h->launches++;
   return TTSH_OK;
 }
 

@@ -87,7 +87,9 @@ enum SpecMode : int {     // multiplier applied to the spectrum while loading th
 enum RowMode : int {      // multiplier applied in x-spectral space by the inverse row pass
   RM_ONE = 0,
   RM_IKX = 1,             // i k_x            (d_x w)
-  RM_NIKX_MEANY = 2       // -i k_x psi~ = v~_y; the mx = 0 entry is the mean flow v^_y(0)/sqrt(Ny)  (lines 8, 14)
+  RM_NIKX_MEANY = 2,      // -i k_x psi~ = v~_y; the mx = 0 entry is the mean flow v^_y(0)/sqrt(Ny)  (lines 8, 14)
+  RM_MODE_MASK = 0xff,
+  RM_PERM = 0x100         // flag: the real rows of this field use the permuted internal layout (perm_index, fft_core.cuh)
 };
 
 struct FieldOp {

@@ -139,7 +139,9 @@ typedef enum {
   TTSH_STAGE_SPECTRAL = 5,  /* a5                                                        */
   TTSH_STAGE_REAL_FWD_ROW = 6, /* a3 fused into the a4 row pass; emits A~ = i kx Gy~ + S'~ and B~ = Gx~ (conservative form)   */
   TTSH_STAGE_FWD_COL_P2 = 7,  /* a4 column pass of those two intermediates                                                    */
-  TTSH_STAGE_SPECTRAL_P2 = 8  /* a5 from the two spectra: rhs^ = A^ - i ky B^.  ttsh_step runs 0, 1, 6, 7, 8 by default         */
+  TTSH_STAGE_SPECTRAL_P2 = 8, /* a5 from the two spectra: rhs^ = A^ - i ky B^                                                   */
+  TTSH_STAGE_ROW_STEP = 9     /* stages 1 + 6 in one kernel: w, v never leave the SM (1/2 rule, row pair fits in shared memory:
+                                 every grid but Nx = 8192 in fp64).  ttsh_step runs 0, 9, 7, 8 where supported, else 0, 1, 6, 7, 8 */
 } ttsh_stage;
 int ttsh_run_stage(ttsh_handle* h, int stage);
 /* Copies a workspace array out for inspection: which = 0..4 real scratch (omega|rhs2, g_x|rhs1_x, g_y|rhs1_y, v_x, v_y;

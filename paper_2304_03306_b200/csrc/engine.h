@@ -17,6 +17,11 @@ template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Mode
 // a5 for the two-spectrum form: rhs^ = A^ - i ky B^ (column mx = 0: A^ = S'^ + i Gy^ separated by Hermitian symmetry)
 template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model& m, const void* A, const void* B, void* w, void* psi,
                                                      double* v0, cudaStream_t s);
+// the whole row half of a step in one kernel (row_step.cuh): reads the inverse intermediates of w, v_x (= i k_y psi^ with the mean
+// flow) and psi, and K; writes A~ and B~.  Supported for the 1/2 rule when one packed row pair fits in shared memory.
+template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
+                                                  const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s);
+template <typename T> bool row_step_supported(const Geom& g);
 // set the dynamic shared-memory attribute of the pass kernels for this grid (no launch)
 template <typename T> cudaError_t prepare_rows(const Geom& g);
 template <typename T> cudaError_t prepare_cols(const Geom& g);

@@ -112,4 +112,54 @@ template <typename T> cudaError_t prepare_rows(const Geom& g) {
 }
 #endif
 
+#ifdef TTSH_BUILD_ROWSTEP
+}  // namespace ttsh
+#include "row_step.cuh"
+namespace ttsh {
+// persistent grid: one CTA per resident slot (SMs x occupancy), looping over the row-pair blocks
+template <typename T, int NX> static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx,
+                                                             const void* inPsi, const void* K, void* oA, void* oB,
+                                                             const void* tab, const double* v0, cudaStream_t s) {
+  using C = RowStepCfg<T, NX>;
+  if constexpr (!C::FITS) return cudaErrorInvalidConfiguration;
+  else {
+    static int slots = 0;
+    if (slots == 0) {
+      cudaError_t e = set_smem(k_row_step<T, NX>, C::SMEM);
+      if (e != cudaSuccess) return e;
+      int dev = 0, sms = 0, occ = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_row_step<T, NX>, C::THREADS, C::SMEM);
+      if (e != cudaSuccess) return e;
+      slots = sms * (occ > 0 ? occ : 1);
+    }
+    const int nblk = (g.Ny / 2) / C::L;
+    const int grid = nblk < slots ? nblk : slots;
+    k_row_step<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx, (const cplx<T>*)inPsi,
+                                                       (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab),
+                                                       v0, nblk);
+    return cudaGetLastError();
+  }
+}
+template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
+                                                  const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s) {
+  switch (g.Nx) {
+#define X(N) case N: return go_row_step<T, N>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T> bool row_step_supported(const Geom& g) {
+  if (4 * (g.Wx - 1) != g.Nx) return false;          // 1/2 rule only
+  switch (g.Nx) {
+#define X(N) case N: return RowStepCfg<T, N>::FITS;
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return false;
+}
+#endif
+
 }  // namespace ttsh

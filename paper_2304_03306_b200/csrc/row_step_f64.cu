@@ -1,0 +1,7 @@
+// fused row-step kernel, scalar = double
+#define TTSH_BUILD_ROWSTEP
+#include "engine_fft.cuh"
+namespace ttsh {
+template cudaError_t launch_row_step<double>(const Geom&, const Model&, const void*, const void*, const void*, const void*, void*, void*, const void*, const double*, cudaStream_t);
+template bool row_step_supported<double>(const Geom&);
+}

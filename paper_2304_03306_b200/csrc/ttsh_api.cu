@@ -22,7 +22,7 @@ inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 inline bool pow2_in_range(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
 
 struct Layout {
-  size_t tabX, tabY, tabS, K, what, psihat, v0, diag_partial, diag_out, R[5], Tm[4], S[3], total;
+  size_t tabX, tabY, tabS, K, what, psihat, v0, diag_partial, diag_out, R[5], Tm[5], S[3], total;
 };
 
 Geom make_geom(int Nx, int Ny, double dx, int num, int den, size_t w) {
@@ -63,7 +63,7 @@ Layout make_layout(int Nx, int Ny, size_t w) {
   L.diag_partial = take((size_t)DIAG_BLOCKS * 8 * sizeof(double));
   L.diag_out = take(8 * sizeof(double));
   for (int i = 0; i < 5; ++i) L.R[i] = take(P * w);
-  for (int i = 0; i < 4; ++i) L.Tm[i] = take(inter);
+  for (int i = 0; i < 5; ++i) L.Tm[i] = take(inter);
   for (int i = 0; i < 3; ++i) L.S[i] = take(spec);
   L.total = off;
   return L;
@@ -80,7 +80,7 @@ struct ttsh_handle {
   Model m;
   cudaStream_t stream;
   char* ws;
-  void *tabX, *tabY, *tabS, *K, *what, *psihat, *R[5], *Tm[4], *S[3];
+  void *tabX, *tabY, *tabS, *K, *what, *psihat, *R[5], *Tm[5], *S[3];
   double *v0, *diag_partial, *diag_out;
   bool initialized;
   double t;
@@ -91,6 +91,7 @@ struct ttsh_handle {
   cudaGraphExec_t graph_exec;
   bool graph_ok;
   int advection_form;
+  bool row_step_ok;     // the fused row-step kernel supports this grid / dtype / dealias fraction
 };
 
 namespace {
@@ -248,15 +249,20 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     }
     case TTSH_STAGE_REAL_FWD_ROW:     // a3 + row half of a4 in one kernel (conservative form only)
       if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
-      TRY(h, DISPATCH(h, launch_fwd_row_fused, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, h->Tm[0], h->Tm[1], h->tabX, h->stream));
+      TRY(h, DISPATCH(h, launch_fwd_row_fused, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, h->Tm[1], h->Tm[4], h->tabX, h->stream));
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_FWD_COL_P2: {      // column pass of the two intermediates A~, B~ of TTSH_STAGE_REAL_FWD_ROW
-      Batch cb = make_batch({op(h->Tm[0], h->S[0], 0), op(h->Tm[1], h->S[1], 0)});
+      Batch cb = make_batch({op(h->Tm[1], h->S[0], 0), op(h->Tm[4], h->S[1], 0)});
       TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 2, h->tabY, h->tabS, h->stream));
       h->launches++;
       return TTSH_OK;
     }
+    case TTSH_STAGE_ROW_STEP:         // a2/a6 row pass + a3 + a4 row pass in one kernel (conservative form, 1/2 rule)
+      if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || !h->row_step_ok) return TTSH_ERR_INVALID_ARG;
+      TRY(h, DISPATCH(h, launch_row_step, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], h->K, h->Tm[1], h->Tm[4], h->tabX, h->v0, h->stream));
+      h->launches++;
+      return TTSH_OK;
     case TTSH_STAGE_SPECTRAL_P2:
       TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, h->S[0], h->S[1], h->what, h->psihat, h->v0, h->stream));
       h->launches++;
@@ -274,18 +280,21 @@ int enqueue_stage(ttsh_handle* h, int stage) {
 int enqueue_step(ttsh_handle* h) {
   static const int fused[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL_FWD_ROW, TTSH_STAGE_FWD_COL_P2,
                               TTSH_STAGE_SPECTRAL_P2};
+  static const int rowstep[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_ROW_STEP, TTSH_STAGE_FWD_COL_P2, TTSH_STAGE_SPECTRAL_P2};
   static const int plain[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL, TTSH_STAGE_FWD_ROW, TTSH_STAGE_FWD_COL,
                               TTSH_STAGE_SPECTRAL};
   const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE;
-  const int* seq = f ? fused : plain;
-  const int n = f ? 5 : 6;
+  const int* seq = f ? (h->row_step_ok ? rowstep : fused) : plain;
+  const int n = f ? (h->row_step_ok ? 4 : 5) : 6;
   for (int i = 0; i < n; ++i) {
     int rc = enqueue_stage(h, seq[i]);
     if (rc != TTSH_OK) return rc;
   }
   return TTSH_OK;
 }
-inline int launches_per_step(const ttsh_handle* h) { return h->advection_form == TTSH_ADVECTION_CONSERVATIVE ? 5 : 6; }
+inline int launches_per_step(const ttsh_handle* h) {
+  return h->advection_form == TTSH_ADVECTION_CONSERVATIVE ? (h->row_step_ok ? 4 : 5) : 6;
+}
 
 int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   const size_t P = (size_t)h->Nx * h->Ny;
@@ -355,10 +364,11 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->diag_partial = reinterpret_cast<double*>(h->ws + L.diag_partial);
   h->diag_out = reinterpret_cast<double*>(h->ws + L.diag_out);
   for (int i = 0; i < 5; ++i) h->R[i] = h->ws + L.R[i];
-  for (int i = 0; i < 4; ++i) h->Tm[i] = h->ws + L.Tm[i];
+  for (int i = 0; i < 5; ++i) h->Tm[i] = h->ws + L.Tm[i];
   for (int i = 0; i < 3; ++i) h->S[i] = h->ws + L.S[i];
   h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
   h->graph_exec = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
+  h->row_step_ok = h->dtype == TTSH_F64 ? row_step_supported<double>(h->g) : row_step_supported<float>(h->g);
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
   std::vector<unsigned char> tx, ty, ts;

@@ -163,8 +163,8 @@ def time_oracle(cfg, n_steps, budget_s, warmup=0):
 # our arm
 # --------------------------------------------------------------------------------------------------
 # what ttsh_step launches per Euler step in the default (conservative) form, and the stage ids of ttsh_run_stage
-STAGE_NAMES = ["k_inv_col", "k_inv_row", "k_fwd_row_fused", "k_fwd_col", "k_spectral"]
-STAGE_IDS = [0, 1, 6, 7, 8]
+STAGE_NAMES = ["k_inv_col", "k_row_step", "k_fwd_col", "k_spectral_p2"]
+STAGE_IDS = [0, 9, 7, 8]
 
 
 def stage_bytes(Nx, Ny, w, conservative=True):
@@ -181,6 +181,8 @@ def stage_bytes(Nx, Ny, w, conservative=True):
         "k_realspace": nreal_in * real + 3 * real,
         "k_fwd_row": 3 * real + 3 * inter,
         "k_fwd_row_fused": 4 * real + 2 * inter,                 # v_x, v_y, w, K in; A~ = i kx Gy~ + S'~ and B~ = Gx~ out
+        "k_row_step": 3 * inter + real + 2 * inter,              # w~, v_x~, psi~ and K in; A~, B~ out (w, v stay on the SM)
+        "k_spectral_p2": 3 * spec + 2 * spec,                    # A^, B^, w^ in; w^, psi^ out
         "k_fwd_col": (2 * inter + 2 * spec) if conservative else (3 * inter + 3 * spec),
         "k_spectral": (3 if conservative else 4) * spec + 2 * spec,   # A^, B^ (or F^x, F^y, S^), w^ in; w^, psi^ out
     }
@@ -218,16 +220,21 @@ def measure(torch, ttsh, cfg, dtype, K, W, device, want_roofline=True, want_e2e=
 
     if want_roofline:
         reps = 20
-        ns = len(STAGE_IDS)
+        names, ids = STAGE_NAMES, STAGE_IDS
+        try:
+            s.run_stage(9)
+        except Exception:     # grid / dtype without the fused row-step kernel: ttsh_step launches the 5-kernel sequence
+            names, ids = ["k_inv_col", "k_inv_row", "k_fwd_row_fused", "k_fwd_col", "k_spectral_p2"], [0, 1, 6, 7, 8]
+        ns = len(ids)
         ev = [[torch.cuda.Event(enable_timing=True) for _ in range(ns + 1)] for _ in range(reps)]
         for r in range(reps):
-            for i, st in enumerate(STAGE_IDS):
+            for i, st in enumerate(ids):
                 ev[r][i].record(stream)
                 s.run_stage(st)
             ev[r][ns].record(stream)
         torch.cuda.synchronize(device)
         per = [sum(ev[r][i].elapsed_time(ev[r][i + 1]) for r in range(reps)) / reps for i in range(ns)]
-        out["stage_ms"] = dict(zip(STAGE_NAMES, per))
+        out["stage_ms"] = dict(zip(names, per))
 
     if want_e2e:
         w = 8 if dtype == "f64" else 4
@@ -350,8 +357,8 @@ def main():
         pass
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"
-    sb = {k: v for k, v in stage_bytes(cfg.Nx, cfg.Ny, w).items() if k in STAGE_NAMES}
     st = res["stage_ms"]
+    sb = {k: v for k, v in stage_bytes(cfg.Nx, cfg.Ny, w).items() if k in st}
     dom = max(st, key=st.get)
     achieved = sb[dom] / (st[dom] * 1e-3) / 1e9
     step_ms = sum(st.values())
@@ -359,7 +366,7 @@ def main():
                 "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": sb[dom],
                 "kernel_ms": st[dom], "kernel_share_of_step": st[dom] / step_ms,
                 "all_kernels": {k: {"ms": st[k], "GBps": sb[k] / (st[k] * 1e-3) / 1e9, "frac": sb[k] / (st[k] * 1e-3) / 1e9 / peak,
-                                    "bytes": sb[k]} for k in STAGE_NAMES},
+                                    "bytes": sb[k]} for k in st},
                 "step_algorithmic_bytes": sum(sb.values()), "step_GBps": sum(sb.values()) / (step_ms * 1e-3) / 1e9,
                 "step_frac": sum(sb.values()) / (step_ms * 1e-3) / 1e9 / peak}
     # traffic from the committed ncu --set full capture of that kernel, when present (profiles/ncu_traffic.csv)

@@ -40,6 +40,8 @@ template <typename T> cudaError_t launch_square(size_t n, const void* in, void* 
 template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, cudaStream_t s);
 // natural <-> permuted row layout of an internal real field (to_perm = 1: natural -> permuted)
 template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* in, void* out, int to_perm, cudaStream_t s);
+// permuted internal row layout (perm_index) -> thread-order layout of the warp-local plan (perm_index_wl)
+template <typename T> cudaError_t launch_reperm_wl(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
 constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs
 template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,
                                               const void* w, double* partial, double* out, cudaStream_t s);

@@ -211,14 +211,6 @@ template <class F> struct VecStore { F f; };
 template <class F> __device__ __forceinline__ VecStore<F> make_vec_store(F f) { return VecStore<F>{f}; }
 template <class S> struct is_vec_store : std::false_type {};
 template <class F> struct is_vec_store<VecStore<F>> : std::true_type {};
-// permuted row layout of the internal real fields: element x = j + k TPL (the 16 points one thread owns are k = 0..15)
-// is stored at ((k >> 2) TPL + j) 4 + (k & 3), so that a thread moves its points with 4 wide accesses (LDG/STG.256 in
-// fp64) and a warp instruction still covers 1 KB of contiguous memory.  TPL = row length / 16.
-__host__ __device__ __forceinline__ int perm_index(int x, int tpl) {
-  const int j = x % tpl, k = x / tpl;
-  return ((k >> 2) * tpl + j) * 4 + (k & 3);
-}
-
 // fire-and-forget accumulation  *p += v  (two scalar reductions; each address receives exactly one addend per pass,
 // so the result does not depend on ordering).  No "memory" clobber on purpose: the asm is volatile (never dropped),
 // the preceding plain store of the same thread to the same address is separated from it by a __syncthreads, and a
@@ -352,5 +344,96 @@ __device__ __forceinline__ void fft_line(int j, cplx<T>* __restrict__ sm, const 
                                          Load load, Store store) {
   fft_stage<T, N, DIR, 0, 1, SYNC_LAST>(j, sm, tab, load, store);
 }
+
+// ---------------------------------------------------------------------------------------
+// "warp-local" plan for N = R1 x 16 x 16 (N = 4096, 2048, 1024: R1 = 16, 8, 4): the same Stockham stages, but the
+// butterflies of stages 2 and 3 are assigned to threads so that the exchange BETWEEN them stays inside a half-warp:
+//   stage 2 (radix 16, Ns = R1) butterfly j = k + R1 q writes the 16 positions  TPL q + k + R1 r,
+//   stage 3 (radix 16, Ns = TPL) butterfly j'' = k + R1 r reads the 16 positions j'' + TPL q  (and writes the same),
+// so the 16 producers {q} and the 16 consumers {r} of one k form a closed group.  Thread t of the line runs, in both
+// stages, butterfly  wl_j(t) = (t >> 4) + R1 (t & 15)  (k = t >> 4, q or r = t & 15): a group is a half-warp, its 256
+// positions are read in stage 2 by its own threads only, so the stage-2 -> stage-3 exchange needs a __syncwarp instead
+// of two CTA barriers and the warps of a line drift apart (one warp's exchange overlaps another warp's arithmetic).
+// Inside the group the element (q, r) is kept at position TPL q + k + R1 rot(r, q) (rot: fft_wl_rot below).  Only the stage-1 -> stage-2 exchange is
+// CTA-wide.  Stage 1 is generic in its base index j0: j0 = t for inputs loaded in natural order (coalesced), j0 = wl_j(t)
+// for inputs the thread already owns in registers.  Outputs: slot k of thread t is index wl_j(t) + k TPL.
+// Twiddle tables (host: fill_stage_tables_wl): [6 base powers][R1] for stage 2 (indexed by k = t >> 4: a broadcast per
+// half-warp), then [6][TPL] for stage 3 stored in THREAD order (entry t holds W_N^{wl_j(t) power}: coalesced).
+// ---------------------------------------------------------------------------------------
+template <int N> __host__ __device__ constexpr bool fft_wl_supported() { return N == 4096 || N == 2048 || N == 1024; }
+template <int N> __host__ __device__ constexpr int fft_wl_r1() { return N / 256; }
+__host__ __device__ constexpr int fft_wl_r1_rt(int N) { return N / 256; }
+__host__ __device__ constexpr int fft_wl_tw_elems_rt(int N) { return 6 * fft_wl_r1_rt(N) + 6 * (N / 16); }
+// shared-memory index padding i + (i >> A) + (i >> B) and the in-group rotation, chosen per element size and N (searched
+// exhaustively: every access of the plan - stage-1 writes from either base index, stage-2/3 reads and writes, the
+// last-stage store - is then bank-conflict free for 16-byte (fp64) and 8-byte (fp32) elements).
+template <typename T, int N> __host__ __device__ constexpr int fft_wl_pad_a() { return (sizeof(T) == 4 || N == 4096) ? 4 : 3; }
+template <typename T, int N> __host__ __device__ constexpr int fft_wl_pad_b() { return 2 * fft_wl_pad_a<T, N>(); }
+template <typename T, int N> __host__ __device__ constexpr int fft_wl_line_elems() {
+  return N + (N >> fft_wl_pad_a<T, N>()) + (N >> fft_wl_pad_b<T, N>());
+}
+template <typename T, int N> __device__ __forceinline__ int fft_wl_pad(int i) {
+  return i + (i >> fft_wl_pad_a<T, N>()) + (i >> fft_wl_pad_b<T, N>());
+}
+template <typename T, int N> __device__ __forceinline__ int fft_wl_rot(int r, int q) {
+  return (sizeof(T) == 8 && N == 2048) ? (r ^ q) : r;
+}
+__host__ __device__ __forceinline__ int fft_wl_j_rt(int t, int r1) { return (t >> 4) + r1 * (t & 15); }
+template <int N> __device__ __forceinline__ int fft_wl_j(int t) { return (t >> 4) + fft_wl_r1<N>() * (t & 15); }
+template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store>
+__device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tabw,
+                                            Load load, Store store) {
+  static_assert(fft_wl_supported<N>(), "warp-local plan: N = R1 x 16 x 16");
+  constexpr int R1 = fft_wl_r1<N>(), TPL = N / 16, NB = 16 / R1;
+  // ---- stage 1 (radix R1, Ns = 1, no twiddles) ----
+  {
+    cplx<T> v[NB][R1];
+    constexpr int NBAT = Load::BATCHES, SLOTS = 16;
+#pragma unroll
+    for (int bat = 0; bat < NBAT; ++bat) {
+      decltype(load.issue(0, 0)) raw[SLOTS / NBAT];
+#pragma unroll
+      for (int s = 0; s < SLOTS / NBAT; ++s) {
+        const int k = bat * (SLOTS / NBAT) + s;
+        raw[s] = load.issue(j0 + k * TPL, k);
+      }
+#pragma unroll
+      for (int s = 0; s < SLOTS / NBAT; ++s) {
+        const int k = bat * (SLOTS / NBAT) + s;      // slot k = b + r NB  <->  v[b][r]
+        v[k % NB][k / NB] = load.finish(j0 + k * TPL, k, raw[s]);
+      }
+    }
+#pragma unroll
+    for (int b = 0; b < NB; ++b) dftR<R1, DIR>(v[b]);
+    __syncthreads();                           // every thread has finished reading this buffer (previous transform)
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      const int base = (j0 + b * TPL) * R1;
+#pragma unroll
+      for (int r = 0; r < R1; ++r) sm[fft_wl_pad<T, N>(base + r)] = v[b][r];
+    }
+    __syncthreads();
+  }
+  // ---- stages 2 and 3 (radix 16), exchange inside the half-warp ----
+  const int kk = t >> 4, q = t & 15;
+  const int j = kk + R1 * q;
+  cplx<T> v[16];
+#pragma unroll
+  for (int r = 0; r < 16; ++r) v[r] = sm[fft_wl_pad<T, N>(j + r * TPL)];
+  apply_stage_twiddles<16, DIR>(v, tabw + kk, R1);
+  dft16<DIR>(v);
+  __syncwarp();                                // the group's 256 positions have been read by its 16 threads
+#pragma unroll
+  for (int r = 0; r < 16; ++r) sm[fft_wl_pad<T, N>(TPL * q + kk + R1 * fft_wl_rot<T, N>(r, q))] = v[r];
+  __syncwarp();
+#pragma unroll
+  for (int qq = 0; qq < 16; ++qq) v[qq] = sm[fft_wl_pad<T, N>(TPL * qq + kk + R1 * fft_wl_rot<T, N>(q, qq))];
+  apply_stage_twiddles<16, DIR>(v, tabw + 6 * R1 + t, TPL);
+  dft16<DIR>(v);
+  if (SYNC_LAST) __syncthreads();              // the store goes to shared memory: every group has finished reading it
+#pragma unroll
+  for (int r = 0; r < 16; ++r) store(j + r * TPL, r, v[r]);
+}
+
 
 }  // namespace ttsh

@@ -58,6 +58,10 @@ template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* i
   k_permute_rows<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(Nx, n, (const T*)in, (T*)out, to_perm);
   return cudaGetLastError();
 }
+template <typename T> cudaError_t launch_reperm_wl(int Nx, size_t n, const void* in, void* out, cudaStream_t s) {
+  k_reperm_wl<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(Nx, n, (const T*)in, (T*)out);
+  return cudaGetLastError();
+}
 template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, cudaStream_t s) {
   k_fill<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, (T*)out, (T)val);
   return cudaGetLastError();
@@ -82,6 +86,7 @@ template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double c
   template cudaError_t launch_square<T>(size_t, const void*, void*, cudaStream_t); \
   template cudaError_t launch_fill<T>(size_t, void*, double, cudaStream_t); \
   template cudaError_t launch_permute<T>(int, size_t, const void*, void*, int, cudaStream_t); \
+  template cudaError_t launch_reperm_wl<T>(int, size_t, const void*, void*, cudaStream_t); \
   template cudaError_t launch_diag<T>(const Geom&, double, double, double, const void*, const void*, const void*, double*, double*, cudaStream_t);
 INST(double)
 INST(float)

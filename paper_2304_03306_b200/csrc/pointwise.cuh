@@ -280,6 +280,16 @@ __global__ void k_permute_rows(int Nx, size_t n, const T* __restrict__ in, T* __
   }
 }
 
+template <typename T>
+__global__ void k_reperm_wl(int Nx, size_t n, const T* __restrict__ in, T* __restrict__ out) {
+  const int tpl = Nx / 16;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t row = i / Nx;
+    const int x = (int)(i - row * Nx);
+    out[row * Nx + perm_index_wl(x, tpl)] = in[row * Nx + perm_index(x, tpl)];
+  }
+}
+
 // ---------------------------------------------------------------------------------------
 // small helpers for Algorithm 2
 // ---------------------------------------------------------------------------------------

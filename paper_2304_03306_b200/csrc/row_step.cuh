@@ -11,6 +11,9 @@
 // HBM traffic per step for the row half: 3 x 0.5 U + 1 U (K) in, 2 x 0.5 U out = 3.5 U instead of 9.5 U for
 // k_inv_row + k_fwd_row_fused.  Of the three packed fields one waits in shared memory (stash, [slot][thread], touched
 // by its owner thread only), one in registers (H) and one is the live transform (V).
+// For Nx = 1024, 2048, 4096 the transforms use the warp-local plan of fft_core.cuh (one CTA-wide exchange per transform);
+// the thread then owns x = wl_j(j) + k TPL, K is read from its thread-order copy (perm_index_wl) and tabX is the
+// warp-local twiddle table.
 // Packing by rows (f(y_A) + i f(y_B)) makes i k_x commute with the packing, so A~ is formed BEFORE the unpack:
 //   T(m) = i k_m Zgy(m) + Zs(m),  k_m the signed wavenumber of bin m  ->  2 unpacks for 3 transforms.
 #pragma once
@@ -20,7 +23,9 @@ namespace ttsh {
 
 template <typename T, int NX> struct RowStepCfg {
   using R = RowCfg<T, NX>;
-  static constexpr int TPL = R::TPL, L = R::L, THREADS = R::THREADS, LS = R::LS;
+  static constexpr bool WL = fft_wl_supported<NX>();                   // warp-local FFT plan (fft_core.cuh)
+  static constexpr int TPL = R::TPL, L = R::L, THREADS = R::THREADS;
+  static constexpr int LS = WL ? fft_wl_line_elems<T, NX>() + 4 : R::LS;
   static constexpr int ST = NX;                                        // stash elements per line
   static constexpr size_t SMEM = (size_t)L * (LS + ST) * sizeof(cplx<T>);
   static constexpr int MINB = 1;
@@ -29,6 +34,7 @@ template <typename T, int NX> struct RowStepCfg {
 
 // inverse row transform of one packed row pair into registers: out[k] = f(y_A, x) + i f(y_B, x), x = j + k TPL.
 // MODE = RM_ONE or RM_NIKX_MEANY (ttsh_common.cuh).  1/2 rule only: retained mx = 0..NX/4.
+// With the warp-local plan the thread owns x = wl_j(j) + k TPL instead (tabX is then the warp-local table).
 template <typename T, int NX, int MODE>
 __device__ __forceinline__ void inv_row_regs(const cplx<T>* __restrict__ row, int j, cplx<T>* __restrict__ line,
                                              const cplx<T>* __restrict__ tabX, T scale, T dkx, T meany, cplx<T> (&out)[16]) {
@@ -56,7 +62,20 @@ __device__ __forceinline__ void inv_row_regs(const cplx<T>* __restrict__ row, in
     return mk<T>(0, 0);
   };
   auto store = [&](int, int k, cplx<T> z) { out[k] = z; };
-  fft_line<T, NX, +1, false>(j, line, tabX, make_loader<2>(issue, finish), store);
+  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, +1, false>(j, j, line, tabX, make_loader<2>(issue, finish), store);
+  else fft_line<T, NX, +1, false>(j, line, tabX, make_loader<2>(issue, finish), store);
+}
+
+// forward transform of the 16 values a thread owns (slot k <-> x = jw + k TPL; jw = wl_j(j) for the warp-local plan, else j)
+template <typename T, int NX, bool SYNC_LAST, class Load, class Store>
+__device__ __forceinline__ void fwd_row_regs(int jw, int j, cplx<T>* __restrict__ line, const cplx<T>* __restrict__ tabX, Load load,
+                                             Store store) {
+  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, -1, SYNC_LAST>(jw, j, line, tabX, load, store);
+  else fft_line<T, NX, -1, SYNC_LAST>(j, line, tabX, load, store);
+}
+template <typename T, int NX> __device__ __forceinline__ int row_step_pad(int i) {
+  if constexpr (fft_wl_supported<NX>()) return fft_wl_pad<T, NX>(i);
+  else return fft_pad<NX>(i);
 }
 
 template <typename T, int NX>
@@ -70,6 +89,7 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
   const int c = threadIdx.x / TPL, j = threadIdx.x % TPL;
+  const int jw = C::WL ? (j >> 4) + (NX / 256) * (j & 15) : j;       // the x-class this thread owns: x = jw + k TPL
   cplx<T>* line = sm + c * C::LS;
   cplx<T>* stash = sm + C::L * C::LS + c * C::ST + j;      // slot k of this thread at stash[k TPL]
   const int Wx = g.Wx;
@@ -131,12 +151,12 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
     auto keep = [&](int k) -> bool { return k <= 3 || k >= 12 || (k == 4 && j == 0); };
     auto ident = [&](int, int, cplx<T> r) -> cplx<T> { return r; };
     {
-      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[fft_pad<NX>(mm)] = z; };
-      fft_line<T, NX, -1, true>(j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), store);
+      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX>(mm)] = z; };
+      fwd_row_regs<T, NX, true>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), store);
       __syncthreads();
       for (int mx = j; mx < Wx; mx += TPL) {
-        const cplx<T> zp = line[fft_pad<NX>(mx)];
-        const cplx<T> zm = conj(line[fft_pad<NX>((NX - mx) & (NX - 1))]);
+        const cplx<T> zp = line[row_step_pad<T, NX>(mx)];
+        const cplx<T> zm = conj(line[row_step_pad<T, NX>((NX - mx) & (NX - 1))]);
         st_pair(outB + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
       }
     }
@@ -148,16 +168,16 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
         if (k <= 4) H[k] = (dkx * (T)mm) * mul_i(z);
         else if (k >= 12) H[k] = (dkx * (T)(mm - NX)) * mul_i(z);
       };
-      fft_line<T, NX, -1, false>(j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), store);
+      fwd_row_regs<T, NX, false>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), store);
     }
     // ---- transform 3: S' -> A~ = unpack(i k_m Zgy + Zs) ----
     {
-      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[fft_pad<NX>(mm)] = z + H[k]; };
-      fft_line<T, NX, -1, true>(j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return stash[k * TPL]; }, ident), store);
+      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX>(mm)] = z + H[k]; };
+      fwd_row_regs<T, NX, true>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return stash[k * TPL]; }, ident), store);
       __syncthreads();
       for (int mx = j; mx < Wx; mx += TPL) {
-        const cplx<T> zp = line[fft_pad<NX>(mx)];
-        const cplx<T> zm = conj(line[fft_pad<NX>((NX - mx) & (NX - 1))]);
+        const cplx<T> zp = line[row_step_pad<T, NX>(mx)];
+        const cplx<T> zm = conj(line[row_step_pad<T, NX>((NX - mx) & (NX - 1))]);
         cplx<T> sa = (T)0.5 * (zp + zm), sb = (T)0.5 * mul_ni(zp - zm);
         if (mx == 0) {                // real numbers S'~(0,y) and Gy~(0,y) travel together (k_fwd_row_fused)
           sa = mk<T>(sa.x, zg0.x);

@@ -22,7 +22,7 @@ inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 inline bool pow2_in_range(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
 
 struct Layout {
-  size_t tabX, tabY, tabS, K, what, psihat, v0, diag_partial, diag_out, R[5], Tm[5], S[3], total;
+  size_t tabX, tabXw, tabY, tabS, K, K2, what, psihat, v0, diag_partial, diag_out, R[5], Tm[5], S[3], total;
 };
 
 Geom make_geom(int Nx, int Ny, double dx, int num, int den, size_t w) {
@@ -54,9 +54,11 @@ Layout make_layout(int Nx, int Ny, size_t w) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
   L.tabX = take((size_t)Nx * cw);
+  L.tabXw = take((size_t)Nx * cw);         // warp-local plan tables (fft_core.cuh), 6 (Nx/256 + Nx/16) entries
   L.tabY = take((size_t)Ny * cw);
   L.tabS = take((size_t)Ny * cw);
   L.K = take(P * w);
+  L.K2 = take(P * w);                      // K in the thread-order row layout of the fused row-step kernel
   L.what = take(spec);
   L.psihat = take(spec);
   L.v0 = take(8 * sizeof(double));
@@ -80,7 +82,7 @@ struct ttsh_handle {
   Model m;
   cudaStream_t stream;
   char* ws;
-  void *tabX, *tabY, *tabS, *K, *what, *psihat, *R[5], *Tm[5], *S[3];
+  void *tabX, *tabXw, *tabY, *tabS, *K, *K2, *what, *psihat, *R[5], *Tm[5], *S[3];
   double *v0, *diag_partial, *diag_out;
   bool initialized;
   double t;
@@ -92,6 +94,7 @@ struct ttsh_handle {
   bool graph_ok;
   int advection_form;
   bool row_step_ok;     // the fused row-step kernel supports this grid / dtype / dealias fraction
+  bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
 };
 
 namespace {
@@ -132,6 +135,17 @@ template <typename T> void fill_stage_tables(std::vector<unsigned char>& buf, in
       for (int k = 0; k < ns; ++k)
         put_twiddle<T>(t + 2 * (size_t)(off + b * ns + k), (long long)k * fft_tw_base_power(R, b), (long long)ns * R);
     ns *= R;
+  }
+}
+// tables of the warp-local plan N = R1 x 16 x 16 (fft_core.cuh, fft_line_wl): stage 2 [6][R1], stage 3 [6][TPL] in thread order
+template <typename T> void fill_stage_tables_wl(std::vector<unsigned char>& buf, int N) {
+  const int R1 = fft_wl_r1_rt(N), TPL = N / 16;
+  buf.assign((size_t)(fft_wl_tw_elems_rt(N) + 1) * 2 * sizeof(T), 0);
+  T* t = reinterpret_cast<T*>(buf.data());
+  for (int b = 0; b < 6; ++b) {
+    for (int k = 0; k < R1; ++k) put_twiddle<T>(t + 2 * (size_t)(b * R1 + k), (long long)k * fft_tw_base_power(16, b), 16LL * R1);
+    for (int th = 0; th < TPL; ++th)
+      put_twiddle<T>(t + 2 * (size_t)(6 * R1 + b * TPL + th), (long long)fft_wl_j_rt(th, R1) * fft_tw_base_power(16, b), (long long)N);
   }
 }
 // split twiddles of the column pass: W_Ny^p, p < Ny/2
@@ -260,7 +274,8 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     }
     case TTSH_STAGE_ROW_STEP:         // a2/a6 row pass + a3 + a4 row pass in one kernel (conservative form, 1/2 rule)
       if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || !h->row_step_ok) return TTSH_ERR_INVALID_ARG;
-      TRY(h, DISPATCH(h, launch_row_step, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], h->K, h->Tm[1], h->Tm[4], h->tabX, h->v0, h->stream));
+      TRY(h, DISPATCH(h, launch_row_step, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], h->row_step_wl ? h->K2 : h->K, h->Tm[1], h->Tm[4],
+                      h->row_step_wl ? h->tabXw : h->tabX, h->v0, h->stream));
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_SPECTRAL_P2:
@@ -296,7 +311,15 @@ inline int launches_per_step(const ttsh_handle* h) {
   return h->advection_form == TTSH_ADVECTION_CONSERVATIVE ? (h->row_step_ok ? 4 : 5) : 6;
 }
 
+int apply_mask_k(ttsh_handle* h, const void* mask, ttsh_mask_kind kind);
 int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
+  int rc = apply_mask_k(h, mask, kind);
+  if (rc != TTSH_OK || !(h->row_step_ok && h->row_step_wl)) return rc;
+  TRY(h, DISPATCH(h, launch_reperm_wl, h->Nx, (size_t)h->Nx * h->Ny, h->K, h->K2, h->stream));
+  h->launches++;
+  return TTSH_OK;
+}
+int apply_mask_k(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   const size_t P = (size_t)h->Nx * h->Ny;
   const size_t w = (size_t)h->dtype;
   if (!mask) {
@@ -359,7 +382,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->m.Gamma2 = p->Gamma2; h->m.gamma_v = p->gamma_v; h->m.gamma_w = p->gamma_w; h->m.dt = dt;
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   h->ws = static_cast<char*>(workspace);
-  h->tabX = h->ws + L.tabX; h->tabY = h->ws + L.tabY; h->tabS = h->ws + L.tabS; h->K = h->ws + L.K; h->what = h->ws + L.what; h->psihat = h->ws + L.psihat;
+  h->tabX = h->ws + L.tabX; h->tabXw = h->ws + L.tabXw; h->K2 = h->ws + L.K2; h->tabY = h->ws + L.tabY; h->tabS = h->ws + L.tabS; h->K = h->ws + L.K; h->what = h->ws + L.what; h->psihat = h->ws + L.psihat;
   h->v0 = reinterpret_cast<double*>(h->ws + L.v0);
   h->diag_partial = reinterpret_cast<double*>(h->ws + L.diag_partial);
   h->diag_out = reinterpret_cast<double*>(h->ws + L.diag_out);
@@ -369,11 +392,18 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
   h->graph_exec = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
   h->row_step_ok = h->dtype == TTSH_F64 ? row_step_supported<double>(h->g) : row_step_supported<float>(h->g);
+  h->row_step_wl = Nx == 1024 || Nx == 2048 || Nx == 4096;
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
   std::vector<unsigned char> tx, ty, ts;
   if (t == TTSH_F64) { fill_stage_tables<double>(tx, Nx); fill_stage_tables<double>(ty, Ny / 2); fill_split_table<double>(ts, Ny); }
   else { fill_stage_tables<float>(tx, Nx); fill_stage_tables<float>(ty, Ny / 2); fill_split_table<float>(ts, Ny); }
+  if (h->row_step_wl) {
+    std::vector<unsigned char> tw;
+    if (t == TTSH_F64) fill_stage_tables_wl<double>(tw, Nx); else fill_stage_tables_wl<float>(tw, Nx);
+    TRY(h, cudaMemcpyAsync(h->tabXw, tw.data(), tw.size(), cudaMemcpyHostToDevice, h->stream));
+    TRY(h, cudaStreamSynchronize(h->stream));
+  }
   TRY(h, cudaMemcpyAsync(h->tabX, tx.data(), tx.size(), cudaMemcpyHostToDevice, h->stream));
   TRY(h, cudaMemcpyAsync(h->tabY, ty.data(), ty.size(), cudaMemcpyHostToDevice, h->stream));
   TRY(h, cudaMemcpyAsync(h->tabS, ts.data(), ts.size(), cudaMemcpyHostToDevice, h->stream));

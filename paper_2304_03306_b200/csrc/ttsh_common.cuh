@@ -68,6 +68,21 @@ __host__ __device__ __forceinline__ size_t inter_pair_index(const Geom& g, int a
   return ((((size_t)(mx >> g.cw_shift) * 2 + p) * (g.Ny >> 2) + a) * g.CW + (mx & (g.CW - 1))) * 2;
 }
 
+// permuted row layout of the internal real fields: element x = j + k TPL (the 16 points one thread owns are k = 0..15)
+// is stored at ((k >> 2) TPL + j) 4 + (k & 3), so that a thread moves its points with 4 wide accesses (LDG/STG.256 in
+// fp64) and a warp instruction still covers 1 KB of contiguous memory.  TPL = row length / 16.
+__host__ __device__ __forceinline__ int perm_index(int x, int tpl) {
+  const int j = x % tpl, k = x / tpl;
+  return ((k >> 2) * tpl + j) * 4 + (k & 3);
+}
+
+// thread-order ("wl") permuted row layout of a real field: element x = wl_j(t) + k TPL at ((k >> 2) TPL + t) 4 + (k & 3)
+__host__ __device__ __forceinline__ int perm_index_wl(int x, int tpl) {
+  const int r1 = tpl / 16, jj = x % tpl, k = x / tpl;
+  const int t = 16 * (jj % r1) + jj / r1;
+  return ((k >> 2) * tpl + t) * 4 + (k & 3);
+}
+
 // strict '>' cutoff evaluated exactly in integers (reading R4):
 //   k^2 > ((num/den) pi/dx)^2   <=>   4 den^2 ((mx Ny)^2 + (my Nx)^2) > num^2 (Nx Ny)^2
 __host__ __device__ __forceinline__ bool is_cut(int mx, int my, int Nx, int Ny, int num, int den) {

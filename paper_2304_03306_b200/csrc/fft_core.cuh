@@ -178,6 +178,33 @@ __device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) 
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+// mbarrier + 1-D bulk asynchronous copy global -> shared (TMA unit, SASS UBLKCP): the copy is issued by one thread and
+// completes on the mbarrier with its byte count; consumers wait on the barrier's phase parity.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void bulk_load(void* dst_smem, const void* src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra MBAR_DONE;\n"
+      "bra MBAR_WAIT;\n"
+      "MBAR_DONE:\n"
+      "}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
 // twiddle W_M^p from the forward-sign table (M = table length), conjugated for the inverse
 template <int DIR, typename T> __device__ __forceinline__ cplx<T> twiddle(const cplx<T>* __restrict__ tab, int p) {
   cplx<T> w = ldg_c(tab + p);
@@ -250,9 +277,13 @@ __device__ __forceinline__ void apply_stage_twiddles(cplx<T>* v, const cplx<T>* 
 // SYNC_LAST: the last-stage store goes to shared memory, so it needs the read/write barrier too.
 // EVERY thread of the CTA must call this (it contains __syncthreads()).
 // ---------------------------------------------------------------------------------------
-template <typename T, int N, int DIR, int S, int NS, bool SYNC_LAST, class Load, class Store>
+// Hook: called by every thread right after the first CTA barrier of the transform, i.e. when all threads have consumed
+// their first-stage inputs (row_step.cuh issues the next asynchronous bulk copy into the input staging buffer there).
+struct NoHook { __device__ __forceinline__ void operator()() const {} };
+
+template <typename T, int N, int DIR, int S, int NS, bool SYNC_LAST, class Load, class Store, class Hook>
 __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab,
-                                          Load& load, Store& store) {
+                                          Load& load, Store& store, Hook& hook) {
   constexpr int R = fft_radix<N>(S);
   constexpr int NST = fft_nstages<N>();
   constexpr bool first = (S == 0), last = (S == NST - 1);
@@ -309,6 +340,7 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
     dftR<R, DIR>(v[b]);
   }
   if (!last || SYNC_LAST) __syncthreads();     // every thread has finished reading this buffer
+  if constexpr (first) hook();
   if constexpr (last && is_vec_store<Store>::value) {
     // last stage, vector store: slot k = b + r NB holds output index j0 + k TPL
 #pragma unroll
@@ -335,14 +367,14 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
   }
   if constexpr (!last) {
     __syncthreads();
-    fft_stage<T, N, DIR, S + 1, NS * R, SYNC_LAST>(j0, sm, tab, load, store);
+    fft_stage<T, N, DIR, S + 1, NS * R, SYNC_LAST>(j0, sm, tab, load, store, hook);
   }
 }
 
-template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store>
+template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store, class Hook = NoHook>
 __device__ __forceinline__ void fft_line(int j, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab,
-                                         Load load, Store store) {
-  fft_stage<T, N, DIR, 0, 1, SYNC_LAST>(j, sm, tab, load, store);
+                                         Load load, Store store, Hook hook = Hook()) {
+  fft_stage<T, N, DIR, 0, 1, SYNC_LAST>(j, sm, tab, load, store, hook);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -380,9 +412,9 @@ template <typename T, int N> __device__ __forceinline__ int fft_wl_rot(int r, in
 }
 __host__ __device__ __forceinline__ int fft_wl_j_rt(int t, int r1) { return (t >> 4) + r1 * (t & 15); }
 template <int N> __device__ __forceinline__ int fft_wl_j(int t) { return (t >> 4) + fft_wl_r1<N>() * (t & 15); }
-template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store>
+template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store, class Hook = NoHook>
 __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tabw,
-                                            Load load, Store store) {
+                                            Load load, Store store, Hook hook = Hook()) {
   static_assert(fft_wl_supported<N>(), "warp-local plan: N = R1 x 16 x 16");
   constexpr int R1 = fft_wl_r1<N>(), TPL = N / 16, NB = 16 / R1;
   // ---- stage 1 (radix R1, Ns = 1, no twiddles) ----
@@ -406,6 +438,7 @@ __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__
 #pragma unroll
     for (int b = 0; b < NB; ++b) dftR<R1, DIR>(v[b]);
     __syncthreads();                           // every thread has finished reading this buffer (previous transform)
+    hook();
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       const int base = (j0 + b * TPL) * R1;

@@ -2,8 +2,8 @@
 //
 //   inverse row pass of w~, v_x~, psi~ (C2R, a2 + a6)  ->  rhs of Algorithm 1 lines 1-2 (a3)  ->  forward row pass (R2C, a4)
 //
-// All three operate on whole rows, and a thread of the Stockham transform owns the same 16 x-positions x = j + k TPL at
-// the output of an inverse transform as at the input of a forward one, so w, v_x, v_y never leave the SM: per row pair
+// All three operate on whole rows, and a thread of the Stockham transform owns the same 16 x-positions at the output of
+// an inverse transform as at the input of a forward one, so w, v_x, v_y never leave the SM: per row pair
 // (y_A = 4a+p, y_B = y_A+2, packed as z = f(y_A) + i f(y_B)) the kernel reads three pruned intermediates and K and
 // writes the two pruned intermediates  A~ = i k_x Gy~ + S'~  and  B~ = Gx~  (fft_passes.cuh, k_fwd_row_fused):
 //   Gx = rhs1_x + lambda0 v_y w,  Gy = rhs1_y - lambda0 v_x w,  S' = -gamma_w K w,  rhs1 = -(beta |v|^2 + gamma_v K) v
@@ -11,6 +11,12 @@
 // HBM traffic per step for the row half: 3 x 0.5 U + 1 U (K) in, 2 x 0.5 U out = 3.5 U instead of 9.5 U for
 // k_inv_row + k_fwd_row_fused.  Of the three packed fields one waits in shared memory (stash, [slot][thread], touched
 // by its owner thread only), one in registers (H) and one is the live transform (V).
+//
+// Inputs arrive by asynchronous bulk copies (cp.async.bulk + mbarrier, fft_core.cuh) into two staging slots per line, each
+// issued one phase ahead by the line's first thread right after the barrier that ends the previous use of the slot:
+//   slot 0:  w~  ->  psi~  ->  K(y_B)  ->  w~ of the next row pair        slot 1:  v_x~  ->  K(y_A)  ->  v_x~ of the next row pair
+// so no thread ever waits on a global load; the first-stage loaders and the pointwise phase read shared memory.
+//
 // For Nx = 1024, 2048, 4096 the transforms use the warp-local plan of fft_core.cuh (one CTA-wide exchange per transform);
 // the thread then owns x = wl_j(j) + k TPL, K is read from its thread-order copy (perm_index_wl) and tabX is the
 // warp-local twiddle table.
@@ -27,17 +33,54 @@ template <typename T, int NX> struct RowStepCfg {
   static constexpr int TPL = R::TPL, L = R::L, THREADS = R::THREADS;
   static constexpr int LS = WL ? fft_wl_line_elems<T, NX>() + 4 : R::LS;
   static constexpr int ST = NX;                                        // stash elements per line
-  static constexpr size_t SMEM = (size_t)L * (LS + ST) * sizeof(cplx<T>);
+  // staging slot (bytes): one row pair of an inverse intermediate, 2 Wxp <= 2 (NX/4 + 8) complex values, or one row of K
+  static constexpr int SLOT = ((NX / 4 + 8) * 2 * (int)sizeof(cplx<T>) + 127) / 128 * 128;
+  static constexpr size_t OFF_SLOTS = ((size_t)L * (LS + ST) * sizeof(cplx<T>) + 127) / 128 * 128;
+  static constexpr size_t OFF_BARS = OFF_SLOTS + (size_t)L * 2 * SLOT;
+  static constexpr size_t SMEM = OFF_BARS + (size_t)L * 2 * sizeof(unsigned long long);
   static constexpr int MINB = 1;
   static constexpr bool FITS = SMEM <= 227 * 1024;
 };
 
+// (A, B) pair / 4 consecutive scalars from a staging slot.  fp64: 32 bytes per lane as two LDS.128 whose order is swapped
+// on lanes with bit 2 set, so that the 8 lanes of a wavefront cover all banks (lane stride 32 bytes would otherwise be a
+// 2-way conflict).  fp32: one LDS.128.
+__device__ __forceinline__ Pair<double> lds_pair(const cplx<double>* p, int sw) {
+  const double2 u = *reinterpret_cast<const double2*>(p + sw), v = *reinterpret_cast<const double2*>(p + (sw ^ 1));
+  Pair<double> r;
+  r.a = sw ? mk<double>(v.x, v.y) : mk<double>(u.x, u.y);
+  r.b = sw ? mk<double>(u.x, u.y) : mk<double>(v.x, v.y);
+  return r;
+}
+__device__ __forceinline__ Pair<float> lds_pair(const cplx<float>* p, int) {
+  const float4 u = *reinterpret_cast<const float4*>(p);
+  Pair<float> r;
+  r.a = mk<float>(u.x, u.y);
+  r.b = mk<float>(u.z, u.w);
+  return r;
+}
+__device__ __forceinline__ Quad<double> lds_quad(const double* p, int sw) {
+  const double2 u = *reinterpret_cast<const double2*>(p + 2 * sw), v = *reinterpret_cast<const double2*>(p + 2 * (sw ^ 1));
+  Quad<double> r;
+  r.v[0] = sw ? v.x : u.x; r.v[1] = sw ? v.y : u.y; r.v[2] = sw ? u.x : v.x; r.v[3] = sw ? u.y : v.y;
+  return r;
+}
+__device__ __forceinline__ Quad<float> lds_quad(const float* p, int) {
+  const float4 u = *reinterpret_cast<const float4*>(p);
+  Quad<float> r;
+  r.v[0] = u.x; r.v[1] = u.y; r.v[2] = u.z; r.v[3] = u.w;
+  return r;
+}
+
 // inverse row transform of one packed row pair into registers: out[k] = f(y_A, x) + i f(y_B, x), x = j + k TPL.
+// row: the staged pairs of this row pair in shared memory ((A, B) of column mx at row + 2 mx).
 // MODE = RM_ONE or RM_NIKX_MEANY (ttsh_common.cuh).  1/2 rule only: retained mx = 0..NX/4.
 // With the warp-local plan the thread owns x = wl_j(j) + k TPL instead (tabX is then the warp-local table).
-template <typename T, int NX, int MODE>
+template <typename T, int NX, int MODE, class Hook>
 __device__ __forceinline__ void inv_row_regs(const cplx<T>* __restrict__ row, int j, cplx<T>* __restrict__ line,
-                                             const cplx<T>* __restrict__ tabX, T scale, T dkx, T meany, cplx<T> (&out)[16]) {
+                                             const cplx<T>* __restrict__ tabX, T scale, T dkx, T meany, cplx<T> (&out)[16],
+                                             Hook hook) {
+  const int sw = (j >> 2) & 1;
   auto mult = [&](cplx<T> w, int mx) -> cplx<T> {
     if (MODE == RM_ONE) return w;
     const T kx = dkx * (T)mx;
@@ -51,8 +94,8 @@ __device__ __forceinline__ void inv_row_regs(const cplx<T>* __restrict__ row, in
   };
   auto zero_pair = [&]() -> Pair<T> { Pair<T> r; r.a = mk<T>(0, 0); r.b = mk<T>(0, 0); return r; };
   auto issue = [&](int m, int k) -> Pair<T> {
-    if (k <= 3 || (k == 4 && j == 0)) return ld_pair(row + 2 * m);
-    if (k >= 12) return ld_pair(row + 2 * (NX - m));
+    if (k <= 3 || (k == 4 && j == 0)) return lds_pair(row + 2 * m, sw);
+    if (k >= 12) return lds_pair(row + 2 * (NX - m), sw);
     return zero_pair();
   };
   auto finish = [&](int m, int k, Pair<T> r) -> cplx<T> {
@@ -62,16 +105,16 @@ __device__ __forceinline__ void inv_row_regs(const cplx<T>* __restrict__ row, in
     return mk<T>(0, 0);
   };
   auto store = [&](int, int k, cplx<T> z) { out[k] = z; };
-  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, +1, false>(j, j, line, tabX, make_loader<2>(issue, finish), store);
-  else fft_line<T, NX, +1, false>(j, line, tabX, make_loader<2>(issue, finish), store);
+  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, +1, false>(j, j, line, tabX, make_loader<1>(issue, finish), store, hook);
+  else fft_line<T, NX, +1, false>(j, line, tabX, make_loader<1>(issue, finish), store, hook);
 }
 
 // forward transform of the 16 values a thread owns (slot k <-> x = jw + k TPL; jw = wl_j(j) for the warp-local plan, else j)
-template <typename T, int NX, bool SYNC_LAST, class Load, class Store>
+template <typename T, int NX, bool SYNC_LAST, class Load, class Store, class Hook = NoHook>
 __device__ __forceinline__ void fwd_row_regs(int jw, int j, cplx<T>* __restrict__ line, const cplx<T>* __restrict__ tabX, Load load,
-                                             Store store) {
-  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, -1, SYNC_LAST>(jw, j, line, tabX, load, store);
-  else fft_line<T, NX, -1, SYNC_LAST>(j, line, tabX, load, store);
+                                             Store store, Hook hook = Hook()) {
+  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, -1, SYNC_LAST>(jw, j, line, tabX, load, store, hook);
+  else fft_line<T, NX, -1, SYNC_LAST>(j, line, tabX, load, store, hook);
 }
 template <typename T, int NX> __device__ __forceinline__ int row_step_pad(int i) {
   if constexpr (fft_wl_supported<NX>()) return fft_wl_pad<T, NX>(i);
@@ -86,12 +129,16 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
            const double* __restrict__ v0, int nblk) {
   using C = RowStepCfg<T, NX>;
   constexpr int TPL = C::TPL;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
   const int c = threadIdx.x / TPL, j = threadIdx.x % TPL;
   const int jw = C::WL ? (j >> 4) + (NX / 256) * (j & 15) : j;       // the x-class this thread owns: x = jw + k TPL
   cplx<T>* line = sm + c * C::LS;
   cplx<T>* stash = sm + C::L * C::LS + c * C::ST + j;      // slot k of this thread at stash[k TPL]
+  unsigned char* slot0 = smem_raw + C::OFF_SLOTS + (size_t)(2 * c) * C::SLOT;
+  unsigned char* slot1 = slot0 + C::SLOT;
+  unsigned long long* bar0 = reinterpret_cast<unsigned long long*>(smem_raw + C::OFF_BARS) + 2 * c;
+  unsigned long long* bar1 = bar0 + 1;
   const int Wx = g.Wx;
   const T scale_i = (T)g.inv_sqrt_nx, scale_f = (T)g.inv_sqrt_nx;
   const T dkx = (T)g.dkx;
@@ -99,60 +146,84 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
   const T beta = (T)m.beta, gv = (T)m.gamma_v, lam = (T)m.lambda0;
   const T ngw = -(T)m.gamma_w * scale_f;
   const size_t in_stride = (size_t)g.Wxp * 2;               // elements per row pair of an inverse intermediate
+  const unsigned in_bytes = (unsigned)(in_stride * sizeof(cplx<T>)), k_bytes = (unsigned)(NX * sizeof(T));
+  const bool leader = (j == 0);
+  unsigned ph0 = 0, ph1 = 0;                                 // phase parity of the next completion of each slot's barrier
+
+  if (leader) { mbar_init(bar0, 1); mbar_init(bar1, 1); }
+  mbar_fence_init();
+  __syncthreads();
+  if (leader && (int)blockIdx.x < nblk) {
+    const size_t rp0 = (size_t)blockIdx.x * C::L + c;
+    bulk_load(slot0, inW + rp0 * in_stride, in_bytes, bar0);
+    bulk_load(slot1, inVx + rp0 * in_stride, in_bytes, bar1);
+  }
 
 #pragma unroll 1
   for (int blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
     const int rp = blk * C::L + c;
     const int a = rp >> 1, p = rp & 1;
     const size_t offA = (size_t)(4 * a + p) * NX, offB = offA + 2 * (size_t)NX;
-    if (j == 0) {   // L2 prefetch of what this line reads in the CTA's next iteration
-      const int nb = blk + gridDim.x;
-      if (nb < nblk) {
-        const int nrp = nb * C::L + c;
-        const unsigned bytes = (unsigned)(in_stride * sizeof(cplx<T>));
-        prefetch_l2_bulk(inW + (size_t)nrp * in_stride, bytes);
-        prefetch_l2_bulk(inVx + (size_t)nrp * in_stride, bytes);
-        prefetch_l2_bulk(inPsi + (size_t)nrp * in_stride, bytes);
-        const size_t nA = (size_t)(4 * (nrp >> 1) + (nrp & 1)) * NX;
-        prefetch_l2_bulk(K + nA, (unsigned)(NX * sizeof(T)));
-        prefetch_l2_bulk(K + nA + 2 * (size_t)NX, (unsigned)(NX * sizeof(T)));
-      }
+    const int nb = blk + gridDim.x;
+    if (leader && nb < nblk) {   // L2 prefetch of what this line reads in the CTA's next iteration
+      const int nrp = nb * C::L + c;
+      prefetch_l2_bulk(inW + (size_t)nrp * in_stride, in_bytes);
+      prefetch_l2_bulk(inVx + (size_t)nrp * in_stride, in_bytes);
+      prefetch_l2_bulk(inPsi + (size_t)nrp * in_stride, in_bytes);
+      const size_t nA = (size_t)(4 * (nrp >> 1) + (nrp & 1)) * NX;
+      prefetch_l2_bulk(K + nA, k_bytes);
+      prefetch_l2_bulk(K + nA + 2 * (size_t)NX, k_bytes);
     }
     cplx<T> H[16], V[16];
-    // ---- a2 / a6: w, v_x, v_y of the two rows (x = j + k TPL) ----
-    inv_row_regs<T, NX, RM_ONE>(inW + (size_t)rp * in_stride, j, line, tabX, scale_i, dkx, meany, V);
+    // ---- a2 / a6: w, v_x, v_y of the two rows ----
+    mbar_wait(bar0, ph0); ph0 ^= 1;
+    inv_row_regs<T, NX, RM_ONE>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
+                                [&]() { if (leader) bulk_load(slot0, inPsi + (size_t)rp * in_stride, in_bytes, bar0); });
 #pragma unroll
     for (int k = 0; k < 16; ++k) stash[k * TPL] = V[k];                     // w
-    inv_row_regs<T, NX, RM_ONE>(inVx + (size_t)rp * in_stride, j, line, tabX, scale_i, dkx, meany, H);          // v_x
-    inv_row_regs<T, NX, RM_NIKX_MEANY>(inPsi + (size_t)rp * in_stride, j, line, tabX, scale_i, dkx, meany, V);  // v_y
+    mbar_wait(bar1, ph1); ph1 ^= 1;
+    inv_row_regs<T, NX, RM_ONE>(reinterpret_cast<const cplx<T>*>(slot1), j, line, tabX, scale_i, dkx, meany, H,
+                                [&]() { if (leader) bulk_load(slot1, K + offA, k_bytes, bar1); });              // v_x
+    mbar_wait(bar0, ph0); ph0 ^= 1;
+    inv_row_regs<T, NX, RM_NIKX_MEANY>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
+                                       [&]() { if (leader) bulk_load(slot0, K + offB, k_bytes, bar0); });       // v_y
     // ---- a3: lines 1-2 of Algorithm 1, pointwise;  V <- Gx,  H <- Gy,  stash <- S'  (all scaled for the forward pass) ----
+    mbar_wait(bar1, ph1); ph1 ^= 1;
+    mbar_wait(bar0, ph0); ph0 ^= 1;
     {
-      Quad<T> ka[4], kb[4];
+      const int sw = (j >> 2) & 1;
+      const T* KA = reinterpret_cast<const T*>(slot1);
+      const T* KB = reinterpret_cast<const T*>(slot0);
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
-        const size_t e = ((size_t)q * TPL + j) * 4;
-        ka[q] = ld_quad(K + offA + e);
-        kb[q] = ld_quad(K + offB + e);
-      }
+        const Quad<T> ka = lds_quad(KA + (q * TPL + j) * 4, sw), kb = lds_quad(KB + (q * TPL + j) * 4, sw);
 #pragma unroll
-      for (int k = 0; k < 16; ++k) {
-        const cplx<T> w = stash[k * TPL];
-        const T KA = ka[k >> 2].v[k & 3], KB = kb[k >> 2].v[k & 3];
-        const T vxA = H[k].x, vxB = H[k].y, vyA = V[k].x, vyB = V[k].y;
-        const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * KA);
-        const T ccB = scale_f * (-beta * (vxB * vxB + vyB * vyB) - gv * KB);
-        const T lwA = scale_f * lam * w.x, lwB = scale_f * lam * w.y;
-        V[k] = mk<T>(ccA * vxA + lwA * vyA, ccB * vxB + lwB * vyB);          // Gx
-        H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
-        stash[k * TPL] = mk<T>(ngw * (KA * w.x), ngw * (KB * w.y));          // S'
+        for (int i = 0; i < 4; ++i) {
+          const int k = 4 * q + i;
+          const cplx<T> w = stash[k * TPL];
+          const T kA = ka.v[i], kB = kb.v[i];
+          const T vxA = H[k].x, vxB = H[k].y, vyA = V[k].x, vyB = V[k].y;
+          const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * kA);
+          const T ccB = scale_f * (-beta * (vxB * vxB + vyB * vyB) - gv * kB);
+          const T lwA = scale_f * lam * w.x, lwB = scale_f * lam * w.y;
+          V[k] = mk<T>(ccA * vxA + lwA * vyA, ccB * vxB + lwB * vyB);          // Gx
+          H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
+          stash[k * TPL] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));          // S'
+        }
       }
     }
-    // ---- a4, transform 1: Gx -> B~ ----
+    // ---- a4, transform 1: Gx -> B~ (its first barrier frees both slots: stage the next row pair) ----
     auto keep = [&](int k) -> bool { return k <= 3 || k >= 12 || (k == 4 && j == 0); };
     auto ident = [&](int, int, cplx<T> r) -> cplx<T> { return r; };
     {
       auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX>(mm)] = z; };
-      fwd_row_regs<T, NX, true>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), store);
+      fwd_row_regs<T, NX, true>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), store, [&]() {
+        if (leader && nb < nblk) {
+          const size_t nrp = (size_t)nb * C::L + c;
+          bulk_load(slot0, inW + nrp * in_stride, in_bytes, bar0);
+          bulk_load(slot1, inVx + nrp * in_stride, in_bytes, bar1);
+        }
+      });
       __syncthreads();
       for (int mx = j; mx < Wx; mx += TPL) {
         const cplx<T> zp = line[row_step_pad<T, NX>(mx)];

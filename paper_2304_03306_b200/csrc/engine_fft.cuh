@@ -14,7 +14,7 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
 #ifdef TTSH_BUILD_COLS
 template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s) {
   using C = ColCfg<T, NY>;
-  dim3 grid(g.NT, nf, 2);
+  dim3 grid(2, g.NT, nf);
   k_inv_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0);
   return cudaGetLastError();
 }

@@ -23,6 +23,9 @@
 #ifndef TTSH_PF_DIST_FUSED
 #define TTSH_PF_DIST_FUSED 64
 #endif
+#ifndef TTSH_PF_DIST_COL
+#define TTSH_PF_DIST_COL 148
+#endif
 #ifndef TTSH_ROW_MINB
 #define TTSH_ROW_MINB 2
 #endif
@@ -118,8 +121,9 @@ template <int LSHIFT> __device__ __forceinline__ void col_thread_map(int e, int&
 }
 
 // ---------------------------------------------------------------------------------------
-// inverse column pass.  grid = (NT tiles, fields, 2 parities): one half-length transform per CTA (both read the same
-// 64 KB spectrum tile; splitting them doubles the number of CTAs and halves the tail of the last wave)
+// inverse column pass.  grid = (2 parities, NT tiles, fields): one half-length transform per CTA (both read the same
+// 64 KB spectrum tile - adjacent in launch order, so the second read hits L2; splitting them doubles the number of CTAs
+// and halves the tail of the last wave)
 // ---------------------------------------------------------------------------------------
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
@@ -131,10 +135,10 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
   int j, c;
   col_thread_map<C::LSHIFT>(threadIdx.x, j, c);
-  const int t = blockIdx.x;
+  const int t = blockIdx.y;
   const int mx = t * L + c;
   const bool valid = mx < g.Wx;
-  const FieldOp op = batch.f[blockIdx.y];
+  const FieldOp op = batch.f[blockIdx.z];
   const int My = g.My, Hy = g.Hy;
   const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * Hy * L + c;   // (q, c) at q L
   // inverse intermediate is pair-row-major: row y = 2y'+p of column mx at ((2 (y'>>1) + p) Wxp + mx) 2 + (y'&1);
@@ -147,9 +151,15 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 
   const bool half_rule = (2 * My == NH);     // the paper's 1/2 rule: |my| <= Ny/4 (uniform branch)
   const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
+  if (threadIdx.x == 0 && blockIdx.x == 0) {  // L2 prefetch of the spectrum tile the CTAs about one wave later read
+    int nt = blockIdx.y + TTSH_PF_DIST_COL, nz = blockIdx.z;
+    if (nt >= (int)gridDim.y) { nt -= gridDim.y; nz += 1; }
+    if (nz < (int)gridDim.z)
+      prefetch_l2_bulk(static_cast<const cplx<T>*>(batch.f[nz].src) + (size_t)nt * Hy * L, (unsigned)(Hy * L * sizeof(cplx<T>)));
+  }
 
   {
-    const int p = blockIdx.z;
+    const int p = blockIdx.x;
     // a_p[mp] = (X[mp] + (-1)^p X[mp+NH]) W_Ny^{-p mp}; X[mp] is retained iff mp <= My, X[mp+NH] (my = mp-NH) iff
     // NH-mp <= My.
     // tail columns of the last tile are written too (zeros inside the row pitch), the row pass never reads them

@@ -215,6 +215,35 @@ def test_C4_dumbbell_1024x2048_single_step(ttsh):
     s.close()
 
 
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_C3_C4_100_steps_against_fft_backed_oracle(ttsh, name):
+    """north_star's 100-step bound (<= 1e-9) at 1024^2 and 1024x2048.  100 steps of the O(N^3) matrix oracle take hours
+    here, so the oracle runs with its FFT backend (locked to the matrix backend by
+    tests/test_oracle_pins.py::test_fft_backend_locked_to_matrix_backend).  O(1) start: every term of Algorithm 1 is active."""
+    cfg = workloads.CONFIGS[name]
+    mask = cfg.mask(R=160.0) if name == "C3" else cfg.mask()
+    vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, transform="fft", vel=vel)
+    s.step(100); o.step(100)
+    compare_state(s, o, TOL_F64_100, f"{name} step 100")
+    d, od = s.diagnostics(), o.diagnostics((cfg.Nx // 2) * cfg.dx, (cfg.Ny // 2) * cfg.dx)
+    for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy"):
+        assert abs(d[key] - od[key]) <= TOL_DIAG * abs(od[key]), key
+    s.close()
+
+
+def test_C4_shape_fp32_single_step(ttsh):
+    """Nx = 2048 in fp32 (the warp-local row plan with two lines per CTA), dumbbell mask, one step <= 1e-5."""
+    cfg = workloads.CONFIGS["C4"]
+    mask = cfg.mask()
+    vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, dtype="f32", transform="fft", vel=vel)
+    o.K = s.debug_real(5).cpu().numpy().astype(np.float64)
+    s.step(1); o.step(1)
+    compare_state(s, o, TOL_F32_1, "C4 f32 step 1")
+    s.close()
+
+
 # ---------------------------------------------------------------- edge cases
 def test_no_mask_zero_field_and_error_paths(ttsh):
     s = ttsh.Solver(64, 64, 0.5, 0.01, ttsh.baseline_params(), "f64", mask=None)

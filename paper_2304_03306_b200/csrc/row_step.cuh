@@ -30,7 +30,11 @@ namespace ttsh {
 template <typename T, int NX> struct RowStepCfg {
   using R = RowCfg<T, NX>;
   static constexpr bool WL = fft_wl_supported<NX>();                   // warp-local FFT plan (fft_core.cuh)
+#ifdef TTSH_RS_L1
+  static constexpr int TPL = R::TPL, L = 1, THREADS = TPL;
+#else
   static constexpr int TPL = R::TPL, L = R::L, THREADS = R::THREADS;
+#endif
   static constexpr int LS = WL ? fft_wl_line_elems<T, NX>() + 4 : R::LS;
   static constexpr int ST = NX;                                        // stash elements per line
   // staging slot (bytes): one row pair of an inverse intermediate, 2 Wxp <= 2 (NX/4 + 8) complex values, or one row of K

@@ -12,7 +12,7 @@ import os
 from typing import Optional
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "csrc", "libttsh.so")
+LIB_PATH = os.environ.get("TTSH_LIB_PATH") or os.path.join(_HERE, "csrc", "libttsh.so")   # override: an out-of-tree build
 
 TTSH_OK = 0
 TTSH_ERR_INVALID_ARG = -1

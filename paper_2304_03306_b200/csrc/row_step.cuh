@@ -30,11 +30,9 @@ namespace ttsh {
 template <typename T, int NX> struct RowStepCfg {
   using R = RowCfg<T, NX>;
   static constexpr bool WL = fft_wl_supported<NX>();                   // warp-local FFT plan (fft_core.cuh)
-#ifdef TTSH_RS_L1
+  // one row pair per CTA: for Nx <= 2048 several small CTAs share an SM and drift apart (measured +2-10 % over two
+  // row pairs per CTA, which pass every barrier together)
   static constexpr int TPL = R::TPL, L = 1, THREADS = TPL;
-#else
-  static constexpr int TPL = R::TPL, L = R::L, THREADS = R::THREADS;
-#endif
   static constexpr int LS = WL ? fft_wl_line_elems<T, NX>() + 4 : R::LS;
   static constexpr int ST = NX;                                        // stash elements per line
   // staging slot (bytes): one row pair of an inverse intermediate, 2 Wxp <= 2 (NX/4 + 8) complex values, or one row of K

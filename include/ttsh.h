@@ -124,6 +124,25 @@ typedef struct {
 } ttsh_diag;
 int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out);
 
+/* Ensembles: the paper's workload is sweeps of independent runs on one grid — disk radius R (Fig. 2), the
+ * hysteresis branches, dumbbell separations — and on grids up to about 1024^2 one system
+ * cannot fill a B200.  An ensemble advances `count` independent handles with ONE launch of each hot kernel per Euler step
+ * (4 launches for all members together), every member computing exactly what ttsh_step computes for it: results are
+ * bit-identical to stepping the members one by one.
+ * Requirements (else TTSH_ERR_INVALID_ARG): count >= 1; all members have the same Nx, Ny, dtype, dx, dt, parameters and
+ * stream, use TTSH_ADVECTION_CONSERVATIVE with the 1/2 rule on a grid the fused row kernel supports (every grid but
+ * Nx = 8192 in fp64), and their workspaces lie at a uniform byte stride: workspace_b = workspace_0 + b * stride, stride >=
+ * ttsh_workspace_bytes (carve them from one allocation).  Masks, states and step counters are per member; all other calls
+ * (ttsh_set_velocity, ttsh_set_mask, ttsh_get_fields, ttsh_diagnostics, ...) keep working on the member handles.  The
+ * ensemble borrows the members: destroy it before them. */
+typedef struct ttsh_ensemble ttsh_ensemble;
+int ttsh_ensemble_create(ttsh_ensemble** out, ttsh_handle* const* members, int count);
+/* n >= 0 applications of Algorithm 1 to every member; asynchronous; every member's t and step counter advance.
+ * TTSH_ERR_NOT_INITIALIZED if a member has no state yet. */
+int ttsh_ensemble_step(ttsh_ensemble* e, int n);
+long long ttsh_ensemble_launch_count(const ttsh_ensemble* e);
+int ttsh_ensemble_destroy(ttsh_ensemble* e);
+
 /* Number of kernel launches the library has enqueued for this handle so far (bench bookkeeping). */
 long long ttsh_launch_count(const ttsh_handle* h);
 

@@ -7,8 +7,13 @@ namespace ttsh {
 
 // FFT passes (fft_passes.cuh).  nfields <= 5 fields per launch (grid.y).  Return cudaErrorInvalidValue for an
 // unsupported transform length.
-template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, const double* v0, cudaStream_t s);
-template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, cudaStream_t s);
+// Ensembles (ttsh_ensemble_step): `members` independent systems whose workspaces lie `mstride` bytes apart are advanced by
+// ONE launch of each hot kernel: member b uses every pointer argument (field sources / destinations, K, v0) + b * mstride;
+// the twiddle tables are member 0's.
+template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, const double* v0, cudaStream_t s,
+                                                 int members = 1, size_t mstride = 0);
+template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, cudaStream_t s,
+                                                 int members = 1, size_t mstride = 0);
 template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const double* v0, cudaStream_t s);
 template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, cudaStream_t s);
 // fused real-space + forward row pass (conservative form): reads v_x, v_y, w, K; writes A~ = i kx Gy~ + S'~ and B~ = Gx~
@@ -16,12 +21,17 @@ template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Mode
                                                        const void* K, void* oA, void* oB, const void* tabX, cudaStream_t s);
 // a5 for the two-spectrum form: rhs^ = A^ - i ky B^ (column mx = 0: A^ = S'^ + i Gy^ separated by Hermitian symmetry)
 template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model& m, const void* A, const void* B, void* w, void* psi,
-                                                     double* v0, cudaStream_t s);
+                                                     double* v0, cudaStream_t s, int members = 1, size_t mstride = 0);
 // the whole row half of a step in one kernel (row_step.cuh): reads the inverse intermediates of w, v_x (= i k_y psi^ with the mean
 // flow) and psi, and K; writes A~ and B~.  Supported for the 1/2 rule when one packed row pair fits in shared memory.
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                   const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s);
 template <typename T> bool row_step_supported(const Geom& g);
+// the same kernel over an ensemble: several row pairs per CTA on small grids (a line of Nx = 64 has 4 threads), row pairs
+// of all members in one persistent grid
+template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
+                                                      const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s,
+                                                      int members, size_t mstride);
 // set the dynamic shared-memory attribute of the pass kernels for this grid (no launch)
 template <typename T> cudaError_t prepare_rows(const Geom& g);
 template <typename T> cudaError_t prepare_cols(const Geom& g);

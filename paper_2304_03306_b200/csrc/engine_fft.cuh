@@ -12,29 +12,35 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
 }
 
 #ifdef TTSH_BUILD_COLS
-template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s) {
+template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s,
+                                                            int members, size_t mstride) {
   using C = ColCfg<T, NY>;
-  dim3 grid(2, g.NT, nf);
-  k_inv_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0);
+  dim3 grid(2, g.NT, nf * members);
+  k_inv_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0, nf, mstride);
   return cudaGetLastError();
 }
-template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s) {
+template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s,
+                                                            int members, size_t mstride) {
   using C = ColCfg<T, NY>;
-  dim3 grid(g.NT, nf);
-  k_fwd_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS));
+  dim3 grid(g.NT, nf * members);
+  k_fwd_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), nf, mstride);
   return cudaGetLastError();
 }
-template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s) {
+template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s,
+                                                 int members, size_t mstride) {
+  if (nf * members > 65535) return cudaErrorInvalidValue;
   switch (g.Ny) {
-#define X(N) case N: return go_inv_col<T, N>(g, b, nf, tab, tabS, v0, s);
+#define X(N) case N: return go_inv_col<T, N>(g, b, nf, tab, tabS, v0, s, members, mstride);
     TTSH_FOR_SIZES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s) {
+template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s,
+                                                 int members, size_t mstride) {
+  if (nf * members > 65535) return cudaErrorInvalidValue;
   switch (g.Ny) {
-#define X(N) case N: return go_fwd_col<T, N>(g, b, nf, tab, tabS, s);
+#define X(N) case N: return go_fwd_col<T, N>(g, b, nf, tab, tabS, s, members, mstride);
     TTSH_FOR_SIZES(X)
 #undef X
   }
@@ -117,35 +123,48 @@ template <typename T> cudaError_t prepare_rows(const Geom& g) {
 #include "row_step.cuh"
 namespace ttsh {
 // persistent grid: one CTA per resident slot (SMs x occupancy), looping over the row-pair blocks
-template <typename T, int NX> static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx,
-                                                             const void* inPsi, const void* K, void* oA, void* oB,
-                                                             const void* tab, const double* v0, cudaStream_t s) {
-  using C = RowStepCfg<T, NX>;
+template <typename T, int NX, int LL, bool ENS>
+static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi, const void* K,
+                               void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int members, size_t mstride) {
+  using C = RowStepCfg<T, NX, LL>;
   if constexpr (!C::FITS) return cudaErrorInvalidConfiguration;
   else {
     static int slots = 0;
     if (slots == 0) {
-      cudaError_t e = set_smem(k_row_step<T, NX>, C::SMEM);
+      cudaError_t e = set_smem(k_row_step<T, NX, LL, ENS>, C::SMEM);
       if (e != cudaSuccess) return e;
       int dev = 0, sms = 0, occ = 0;
       cudaGetDevice(&dev);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_row_step<T, NX>, C::THREADS, C::SMEM);
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_row_step<T, NX, LL, ENS>, C::THREADS, C::SMEM);
       if (e != cudaSuccess) return e;
       slots = sms * (occ > 0 ? occ : 1);
     }
-    const int nblk = (g.Ny / 2) / C::L;
+    const int rpm = g.Ny / 2;                                  // row pairs per member
+    const long long nblk_ll = (long long)rpm * members / C::L;
+    if (nblk_ll > 0x3fffffff) return cudaErrorInvalidValue;
+    const int nblk = (int)nblk_ll;
     const int grid = nblk < slots ? nblk : slots;
-    k_row_step<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx, (const cplx<T>*)inPsi,
-                                                       (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab),
-                                                       v0, nblk);
+    k_row_step<T, NX, LL, ENS><<<grid, C::THREADS, C::SMEM, s>>>(g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx, (const cplx<T>*)inPsi,
+                                                                 (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab),
+                                                                 v0, nblk, rpm, mstride);
     return cudaGetLastError();
   }
 }
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                   const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s) {
   switch (g.Nx) {
-#define X(N) case N: return go_row_step<T, N>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s);
+#define X(N) case N: return go_row_step<T, N, 1, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
+                                                      const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s,
+                                                      int members, size_t mstride) {
+  switch (g.Nx) {
+#define X(N) case N: return go_row_step<T, N, row_step_ens_lines<N>(), true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride);
     TTSH_FOR_SIZES(X)
 #undef X
   }

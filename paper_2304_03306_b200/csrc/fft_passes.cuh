@@ -128,7 +128,7 @@ template <int LSHIFT> __device__ __forceinline__ void col_thread_map(int e, int&
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
 k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
-          const cplx<T>* __restrict__ tabS, const double* __restrict__ v0) {
+          const cplx<T>* __restrict__ tabS, const double* __restrict__ v0_, int nf, size_t mstride) {
   using C = ColCfg<T, NY>;
   constexpr int NH = C::NH, L = C::L, TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -138,7 +138,12 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const int t = blockIdx.y;
   const int mx = t * L + c;
   const bool valid = mx < g.Wx;
-  const FieldOp op = batch.f[blockIdx.z];
+  const int member = blockIdx.z / nf;             // grid.z = ensemble members x fields (member 0 only outside ensembles)
+  const size_t moff = (size_t)member * mstride;    // bytes
+  FieldOp op = batch.f[blockIdx.z - member * nf];
+  op.src = static_cast<const char*>(op.src) + moff;
+  op.dst = static_cast<char*>(op.dst) + moff;
+  const double* __restrict__ v0 = reinterpret_cast<const double*>(reinterpret_cast<const char*>(v0_) + moff);
   const int My = g.My, Hy = g.Hy;
   const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * Hy * L + c;   // (q, c) at q L
   // inverse intermediate is pair-row-major: row y = 2y'+p of column mx at ((2 (y'>>1) + p) Wxp + mx) 2 + (y'&1);
@@ -155,7 +160,8 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     int nt = blockIdx.y + TTSH_PF_DIST_COL, nz = blockIdx.z;
     if (nt >= (int)gridDim.y) { nt -= gridDim.y; nz += 1; }
     if (nz < (int)gridDim.z)
-      prefetch_l2_bulk(static_cast<const cplx<T>*>(batch.f[nz].src) + (size_t)nt * Hy * L, (unsigned)(Hy * L * sizeof(cplx<T>)));
+      prefetch_l2_bulk(reinterpret_cast<const cplx<T>*>(static_cast<const char*>(batch.f[nz % nf].src) + (size_t)(nz / nf) * mstride) +
+                           (size_t)nt * Hy * L, (unsigned)(Hy * L * sizeof(cplx<T>)));
   }
 
   {
@@ -214,7 +220,7 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 template <typename T, int NY>
 __global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
 k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
-          const cplx<T>* __restrict__ tabS) {
+          const cplx<T>* __restrict__ tabS, int nf, size_t mstride) {
   using C = ColCfg<T, NY>;
   constexpr int NH = C::NH, L = C::L, TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -223,7 +229,11 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   col_thread_map<C::LSHIFT>(threadIdx.x, j, c);
   const int t = blockIdx.x;
   const bool valid = t * L + c < g.Wx;
-  const FieldOp op = batch.f[blockIdx.y];
+  const int member = blockIdx.y / nf;             // grid.y = ensemble members x fields
+  const size_t moff = (size_t)member * mstride;
+  FieldOp op = batch.f[blockIdx.y - member * nf];
+  op.src = static_cast<const char*>(op.src) + moff;
+  op.dst = static_cast<char*>(op.dst) + moff;
   const int My = g.My, Hy = g.Hy;
   const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * 2 * NH * L + threadIdx.x;
   cplx<T>* dst = static_cast<cplx<T>*>(op.dst) + (size_t)t * Hy * L + c;

@@ -31,9 +31,10 @@ template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m,
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model& m, const void* A, const void* B, void* w, void* psi,
-                                                     double* v0, cudaStream_t s) {
-  const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
-  k_spectral_p2<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)A, (const cplx<T>*)B, (cplx<T>*)w, (cplx<T>*)psi, v0);
+                                                     double* v0, cudaStream_t s, int members, size_t mstride) {
+  if (members > 65535) return cudaErrorInvalidValue;
+  const dim3 grid((unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256), (unsigned)members);
+  k_spectral_p2<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)A, (const cplx<T>*)B, (cplx<T>*)w, (cplx<T>*)psi, v0, mstride);
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, void* psi, double* v0, cudaStream_t s) {
@@ -81,7 +82,7 @@ template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double c
   template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, double*, cudaStream_t); \
   template cudaError_t launch_spectral_init<T>(const Geom&, const void*, const void*, void*, void*, double*, cudaStream_t); \
   template cudaError_t launch_psi_from_w<T>(const Geom&, const void*, void*, cudaStream_t); \
-  template cudaError_t launch_spectral_p2<T>(const Geom&, const Model&, const void*, const void*, void*, void*, double*, cudaStream_t); \
+  template cudaError_t launch_spectral_p2<T>(const Geom&, const Model&, const void*, const void*, void*, void*, double*, cudaStream_t, int, size_t); \
   template cudaError_t launch_mask_to_real<T>(size_t, const unsigned char*, void*, cudaStream_t); \
   template cudaError_t launch_square<T>(size_t, const void*, void*, cudaStream_t); \
   template cudaError_t launch_fill<T>(size_t, void*, double, cudaStream_t); \

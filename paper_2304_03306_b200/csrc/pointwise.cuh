@@ -156,10 +156,16 @@ k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __res
 // and i kx Gy^ = 0 there.  Gy^(0,0) = Im A^(0,0) and Gx^(0,0) = Re B^(0,0) feed the mean-flow update (line 8, Eq. C1).
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_spectral_p2(Geom g, Model m, const cplx<T>* __restrict__ A, const cplx<T>* __restrict__ B, cplx<T>* w,
-              cplx<T>* __restrict__ psi, double* v0) {
+k_spectral_p2(Geom g, Model m, const cplx<T>* __restrict__ A_, const cplx<T>* __restrict__ B_, cplx<T>* w_,
+              cplx<T>* __restrict__ psi_, double* v0_, size_t mstride) {
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
+  const size_t moff = (size_t)blockIdx.y * mstride;      // ensemble member (bytes); 0 outside ensembles
+  const cplx<T>* __restrict__ A = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(A_) + moff);
+  const cplx<T>* __restrict__ B = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(B_) + moff);
+  cplx<T>* w = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(w_) + moff);
+  cplx<T>* __restrict__ psi = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(psi_) + moff);
+  double* v0 = reinterpret_cast<double*>(reinterpret_cast<char*>(v0_) + moff);
   const int t = (int)(idx / ((size_t)g.Hy * g.CW));
   const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
   const int q = rem >> g.cw_shift;

@@ -27,12 +27,16 @@
 
 namespace ttsh {
 
-template <typename T, int NX> struct RowStepCfg {
+// row pairs per CTA of the ensemble variant: lines of small grids have few threads (Nx = 64: 4), so a CTA takes several
+// consecutive row pairs of one member (64 threads; shared memory per thread does not depend on Nx, about 4 such CTAs per SM)
+template <int NX> __host__ __device__ constexpr int row_step_ens_lines() { return NX >= 1024 ? 1 : 1024 / NX; }
+
+template <typename T, int NX, int LL = 1> struct RowStepCfg {
   using R = RowCfg<T, NX>;
   static constexpr bool WL = fft_wl_supported<NX>();                   // warp-local FFT plan (fft_core.cuh)
   // one row pair per CTA: for Nx <= 2048 several small CTAs share an SM and drift apart (measured +2-10 % over two
   // row pairs per CTA, which pass every barrier together)
-  static constexpr int TPL = R::TPL, L = 1, THREADS = TPL;
+  static constexpr int TPL = R::TPL, L = LL, THREADS = LL * TPL;
   static constexpr int LS = WL ? fft_wl_line_elems<T, NX>() + 4 : R::LS;
   static constexpr int ST = NX;                                        // stash elements per line
   // staging slot (bytes): one row pair of an inverse intermediate, 2 Wxp <= 2 (NX/4 + 8) complex values, or one row of K
@@ -123,13 +127,19 @@ template <typename T, int NX> __device__ __forceinline__ int row_step_pad(int i)
   else return fft_pad<NX>(i);
 }
 
-template <typename T, int NX>
-__global__ void __launch_bounds__(RowStepCfg<T, NX>::THREADS, RowStepCfg<T, NX>::MINB)
+template <class P> __device__ __forceinline__ P* byte_off(P* p, size_t bytes) {
+  return reinterpret_cast<P*>(reinterpret_cast<char*>(const_cast<typename std::remove_const<P>::type*>(p)) + bytes);
+}
+
+// LL row pairs per CTA.  ENS: the persistent grid runs over the row pairs of `members` systems whose workspaces lie mstride
+// bytes apart (ttsh_ensemble_step); rpm = Ny/2 row pairs per member, a multiple of LL, so a CTA's lines share a member.
+template <typename T, int NX, int LL, bool ENS>
+__global__ void __launch_bounds__(RowStepCfg<T, NX, LL>::THREADS, RowStepCfg<T, NX, LL>::MINB)
 k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, const cplx<T>* __restrict__ inW,
            const cplx<T>* __restrict__ inVx, const cplx<T>* __restrict__ inPsi, const T* __restrict__ K,
            cplx<T>* __restrict__ outA, cplx<T>* __restrict__ outB, const cplx<T>* __restrict__ tabX,
-           const double* __restrict__ v0, int nblk) {
-  using C = RowStepCfg<T, NX>;
+           const double* __restrict__ v0, int nblk, int rpm, size_t mstride) {
+  using C = RowStepCfg<T, NX, LL>;
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -144,7 +154,12 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
   const int Wx = g.Wx;
   const T scale_i = (T)g.inv_sqrt_nx, scale_f = (T)g.inv_sqrt_nx;
   const T dkx = (T)g.dkx;
-  const T meany = (T)(v0[1] * g.inv_sqrt_ny);
+  T meany = (T)(v0[1] * g.inv_sqrt_ny);
+  // global row pair -> (row pair of its member, byte offset of the member's workspace)
+  auto locate = [&](int rpg, int& rp_, size_t& mo_) {
+    if constexpr (ENS) { const int mb = rpg / rpm; rp_ = rpg - mb * rpm; mo_ = (size_t)mb * mstride; }
+    else { rp_ = rpg; mo_ = 0; }
+  };
   const T beta = (T)m.beta, gv = (T)m.gamma_v, lam = (T)m.lambda0;
   const T ngw = -(T)m.gamma_w * scale_f;
   const size_t in_stride = (size_t)g.Wxp * 2;               // elements per row pair of an inverse intermediate
@@ -156,39 +171,43 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
   mbar_fence_init();
   __syncthreads();
   if (leader && (int)blockIdx.x < nblk) {
-    const size_t rp0 = (size_t)blockIdx.x * C::L + c;
-    bulk_load(slot0, inW + rp0 * in_stride, in_bytes, bar0);
-    bulk_load(slot1, inVx + rp0 * in_stride, in_bytes, bar1);
+    int rp0; size_t mo0;
+    locate(blockIdx.x * C::L + c, rp0, mo0);
+    bulk_load(slot0, byte_off(inW, mo0) + (size_t)rp0 * in_stride, in_bytes, bar0);
+    bulk_load(slot1, byte_off(inVx, mo0) + (size_t)rp0 * in_stride, in_bytes, bar1);
   }
 
 #pragma unroll 1
   for (int blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
-    const int rp = blk * C::L + c;
+    int rp; size_t mo;
+    locate(blk * C::L + c, rp, mo);
+    if constexpr (ENS) meany = (T)(byte_off(v0, mo)[1] * g.inv_sqrt_ny);
     const int a = rp >> 1, p = rp & 1;
     const size_t offA = (size_t)(4 * a + p) * NX, offB = offA + 2 * (size_t)NX;
     const int nb = blk + gridDim.x;
     if (leader && nb < nblk) {   // L2 prefetch of what this line reads in the CTA's next iteration
-      const int nrp = nb * C::L + c;
-      prefetch_l2_bulk(inW + (size_t)nrp * in_stride, in_bytes);
-      prefetch_l2_bulk(inVx + (size_t)nrp * in_stride, in_bytes);
-      prefetch_l2_bulk(inPsi + (size_t)nrp * in_stride, in_bytes);
+      int nrp; size_t nmo;
+      locate(nb * C::L + c, nrp, nmo);
+      prefetch_l2_bulk(byte_off(inW, nmo) + (size_t)nrp * in_stride, in_bytes);
+      prefetch_l2_bulk(byte_off(inVx, nmo) + (size_t)nrp * in_stride, in_bytes);
+      prefetch_l2_bulk(byte_off(inPsi, nmo) + (size_t)nrp * in_stride, in_bytes);
       const size_t nA = (size_t)(4 * (nrp >> 1) + (nrp & 1)) * NX;
-      prefetch_l2_bulk(K + nA, k_bytes);
-      prefetch_l2_bulk(K + nA + 2 * (size_t)NX, k_bytes);
+      prefetch_l2_bulk(byte_off(K, nmo) + nA, k_bytes);
+      prefetch_l2_bulk(byte_off(K, nmo) + nA + 2 * (size_t)NX, k_bytes);
     }
     cplx<T> H[16], V[16];
     // ---- a2 / a6: w, v_x, v_y of the two rows ----
     mbar_wait(bar0, ph0); ph0 ^= 1;
     inv_row_regs<T, NX, RM_ONE>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
-                                [&]() { if (leader) bulk_load(slot0, inPsi + (size_t)rp * in_stride, in_bytes, bar0); });
+                                [&]() { if (leader) bulk_load(slot0, byte_off(inPsi, mo) + (size_t)rp * in_stride, in_bytes, bar0); });
 #pragma unroll
     for (int k = 0; k < 16; ++k) stash[k * TPL] = V[k];                     // w
     mbar_wait(bar1, ph1); ph1 ^= 1;
     inv_row_regs<T, NX, RM_ONE>(reinterpret_cast<const cplx<T>*>(slot1), j, line, tabX, scale_i, dkx, meany, H,
-                                [&]() { if (leader) bulk_load(slot1, K + offA, k_bytes, bar1); });              // v_x
+                                [&]() { if (leader) bulk_load(slot1, byte_off(K, mo) + offA, k_bytes, bar1); });              // v_x
     mbar_wait(bar0, ph0); ph0 ^= 1;
     inv_row_regs<T, NX, RM_NIKX_MEANY>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
-                                       [&]() { if (leader) bulk_load(slot0, K + offB, k_bytes, bar0); });       // v_y
+                                       [&]() { if (leader) bulk_load(slot0, byte_off(K, mo) + offB, k_bytes, bar0); });       // v_y
     // ---- a3: lines 1-2 of Algorithm 1, pointwise;  V <- Gx,  H <- Gy,  stash <- S'  (all scaled for the forward pass) ----
     mbar_wait(bar1, ph1); ph1 ^= 1;
     mbar_wait(bar0, ph0); ph0 ^= 1;
@@ -221,16 +240,17 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
       auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX>(mm)] = z; };
       fwd_row_regs<T, NX, true>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), store, [&]() {
         if (leader && nb < nblk) {
-          const size_t nrp = (size_t)nb * C::L + c;
-          bulk_load(slot0, inW + nrp * in_stride, in_bytes, bar0);
-          bulk_load(slot1, inVx + nrp * in_stride, in_bytes, bar1);
+          int nrp; size_t nmo;
+          locate(nb * C::L + c, nrp, nmo);
+          bulk_load(slot0, byte_off(inW, nmo) + (size_t)nrp * in_stride, in_bytes, bar0);
+          bulk_load(slot1, byte_off(inVx, nmo) + (size_t)nrp * in_stride, in_bytes, bar1);
         }
       });
       __syncthreads();
       for (int mx = j; mx < Wx; mx += TPL) {
         const cplx<T> zp = line[row_step_pad<T, NX>(mx)];
         const cplx<T> zm = conj(line[row_step_pad<T, NX>((NX - mx) & (NX - 1))]);
-        st_pair(outB + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
+        st_pair(byte_off(outB, mo) + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
       }
     }
     // ---- transform 2: Gy -> H <- i k_m Zgy(m) (retained bins only) ----
@@ -256,7 +276,7 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
           sa = mk<T>(sa.x, zg0.x);
           sb = mk<T>(sb.x, zg0.y);
         }
-        st_pair(outA + inter_pair_index(g, a, p, mx), sa, sb);
+        st_pair(byte_off(outA, mo) + inter_pair_index(g, a, p, mx), sa, sb);
       }
     }
   }

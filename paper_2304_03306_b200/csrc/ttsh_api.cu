@@ -97,6 +97,13 @@ struct ttsh_handle {
   bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
 };
 
+struct ttsh_ensemble {
+  std::vector<ttsh_handle*> members;   // borrowed
+  size_t mstride;                      // bytes between consecutive members' workspaces
+  cudaGraphExec_t graph_exec;
+  long long launches;
+};
+
 namespace {
 
 #define TRY(h, call)                                                        \
@@ -555,6 +562,101 @@ int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out) 
     d.polar_order = 0.0;
   }
   *host_out = d;
+  return TTSH_OK;
+}
+
+// ---- ensembles -----------------------------------------------------------------------------------------------
+int ttsh_ensemble_create(ttsh_ensemble** out, ttsh_handle* const* members, int count) {
+  if (!out) return TTSH_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!members || count < 1 || count > 8192) return TTSH_ERR_INVALID_ARG;
+  const ttsh_handle* h0 = members[0];
+  if (!h0) return TTSH_ERR_INVALID_ARG;
+  ptrdiff_t stride = 0;
+  for (int b = 0; b < count; ++b) {
+    const ttsh_handle* h = members[b];
+    if (!h) return TTSH_ERR_INVALID_ARG;
+    if (h->sticky) return h->sticky;
+    if (h->Nx != h0->Nx || h->Ny != h0->Ny || h->dtype != h0->dtype || h->dx != h0->dx || h->dt != h0->dt ||
+        h->stream != h0->stream || memcmp(&h->p, &h0->p, sizeof(ttsh_params)) != 0)
+      return TTSH_ERR_INVALID_ARG;
+    if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || !h->row_step_ok) return TTSH_ERR_INVALID_ARG;
+    for (int a = 0; a < b; ++a) if (members[a] == h) return TTSH_ERR_INVALID_ARG;
+    if (b == 1) stride = h->ws - h0->ws;
+    if (b >= 1 && h->ws - h0->ws != (ptrdiff_t)b * stride) return TTSH_ERR_INVALID_ARG;
+  }
+  if (count > 1 && stride < (ptrdiff_t)make_layout(h0->Nx, h0->Ny, (size_t)h0->dtype).total) return TTSH_ERR_INVALID_ARG;
+  ttsh_ensemble* e = new (std::nothrow) ttsh_ensemble();
+  if (!e) return TTSH_ERR_INVALID_ARG;
+  e->members.assign(members, members + count);
+  e->mstride = count > 1 ? (size_t)stride : 0;
+  e->graph_exec = nullptr;
+  e->launches = 0;
+  *out = e;
+  return TTSH_OK;
+}
+
+static int ensemble_enqueue_step(ttsh_ensemble* e, cudaStream_t stream) {
+  ttsh_handle* h = e->members[0];
+  const int B = (int)e->members.size();
+  const size_t ms = e->mstride;
+  Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->psihat, h->Tm[2], SM_ONE), op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, h->v0, stream, B, ms));
+  TRY(h, DISPATCH(h, launch_row_step_ens, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], h->row_step_wl ? h->K2 : h->K, h->Tm[1], h->Tm[4],
+                  h->row_step_wl ? h->tabXw : h->tabX, h->v0, stream, B, ms));
+  Batch fb = make_batch({op(h->Tm[1], h->S[0], 0), op(h->Tm[4], h->S[1], 0)});
+  TRY(h, DISPATCH(h, launch_fwd_col, h->g, fb, 2, h->tabY, h->tabS, stream, B, ms));
+  TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, h->S[0], h->S[1], h->what, h->psihat, h->v0, stream, B, ms));
+  return TTSH_OK;
+}
+
+int ttsh_ensemble_step(ttsh_ensemble* e, int n) {
+  if (!e || n < 0) return TTSH_ERR_INVALID_ARG;
+  ttsh_handle* h0 = e->members[0];
+  for (ttsh_handle* h : e->members) {
+    if (h->sticky) return h->sticky;
+    if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+    if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
+  }
+  if (n == 0) return TTSH_OK;
+  // a step of a small ensemble is launch-latency bound: replay one captured step (as ttsh_step does)
+  const bool use_graph = (size_t)h0->Nx * h0->Ny * e->members.size() <= (size_t)4 * 1024 * 1024 && n >= 4;
+  if (use_graph && !e->graph_exec) {
+    cudaGraph_t graph = nullptr;
+    cudaStream_t cap = nullptr;
+    TRY(h0, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaError_t err = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (err != cudaSuccess) { cudaStreamDestroy(cap); return fail_cuda(h0, err, "cudaStreamBeginCapture"); }
+    const int rc = ensemble_enqueue_step(e, cap);
+    err = cudaStreamEndCapture(cap, &graph);
+    cudaStreamDestroy(cap);
+    if (rc != TTSH_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (err != cudaSuccess) return fail_cuda(h0, err, "cudaStreamEndCapture");
+    err = cudaGraphInstantiate(&e->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (err != cudaSuccess) { e->graph_exec = nullptr; return fail_cuda(h0, err, "cudaGraphInstantiate"); }
+  }
+  for (int i = 0; i < n; ++i) {
+    if (use_graph) TRY(h0, cudaGraphLaunch(e->graph_exec, h0->stream));
+    else {
+      const int rc = ensemble_enqueue_step(e, h0->stream);
+      if (rc != TTSH_OK) return rc;
+    }
+    e->launches += 4;
+  }
+  for (ttsh_handle* h : e->members) {
+    h->t += (double)n * h->dt;
+    h->step += n;
+  }
+  return TTSH_OK;
+}
+
+long long ttsh_ensemble_launch_count(const ttsh_ensemble* e) { return e ? e->launches : 0; }
+
+int ttsh_ensemble_destroy(ttsh_ensemble* e) {
+  if (!e) return TTSH_OK;
+  if (e->graph_exec) cudaGraphExecDestroy(e->graph_exec);
+  delete e;
   return TTSH_OK;
 }
 

@@ -30,7 +30,8 @@ TTSH_ADVECTION_CONSERVATIVE, TTSH_ADVECTION_LITERAL = 0, 1
 SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_velocity", "ttsh_set_advection_form", "ttsh_step",
            "ttsh_get_fields", "ttsh_state_elems", "ttsh_get_state", "ttsh_set_state", "ttsh_diagnostics",
            "ttsh_launch_count", "ttsh_run_stage", "ttsh_debug_get_real", "ttsh_destroy", "ttsh_strerror",
-           "ttsh_last_error")
+           "ttsh_last_error", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
+           "ttsh_ensemble_destroy")
 
 
 class ttsh_params(C.Structure):
@@ -73,6 +74,10 @@ _sig = {
     "ttsh_destroy": (_i, [_vp]),
     "ttsh_strerror": (C.c_char_p, [_i]),
     "ttsh_last_error": (C.c_char_p, [_vp]),
+    "ttsh_ensemble_create": (_i, [C.POINTER(_vp), C.POINTER(_vp), _i]),
+    "ttsh_ensemble_step": (_i, [_vp, _i]),
+    "ttsh_ensemble_launch_count": (_ll, [_vp]),
+    "ttsh_ensemble_destroy": (_i, [_vp]),
 }
 for _name, (_res, _args) in _sig.items():
     _f = getattr(_lib, _name)
@@ -157,6 +162,26 @@ def ttsh_destroy(h):
     return _lib.ttsh_destroy(h)
 
 
+def ttsh_ensemble_create(handles):
+    """Returns (status, ensemble).  handles: sequence of member handles (c_void_p or int; None = NULL)."""
+    e = _vp()
+    arr = (_vp * max(1, len(handles)))(*[getattr(h, "value", h) for h in handles])
+    rc = _lib.ttsh_ensemble_create(C.byref(e), arr, len(handles))
+    return rc, e
+
+
+def ttsh_ensemble_step(e, n):
+    return _lib.ttsh_ensemble_step(e, n)
+
+
+def ttsh_ensemble_launch_count(e):
+    return int(_lib.ttsh_ensemble_launch_count(e))
+
+
+def ttsh_ensemble_destroy(e):
+    return _lib.ttsh_ensemble_destroy(e)
+
+
 def ttsh_strerror(code):
     return _lib.ttsh_strerror(code).decode()
 
@@ -179,7 +204,9 @@ def baseline_params() -> ttsh_params:
 # ---- convenience wrapper (owns torch tensors; marshalling only) --------------------------------------
 class Solver:
     def __init__(self, Nx: int, Ny: int, dx: float, dt: float, params: ttsh_params, dtype: str = "f64",
-                 mask=None, mask_kind: int = TTSH_MASK_BINARY, device: str = "cuda:0", stream=None):
+                 mask=None, mask_kind: int = TTSH_MASK_BINARY, device: str = "cuda:0", stream=None, workspace=None):
+        """workspace: an optional uint8 CUDA tensor (>= ttsh_workspace_bytes, 256-byte aligned) to use instead of a fresh one
+        (Ensemble carves its members' workspaces from one allocation)."""
         import torch
         self.torch = torch
         self.Nx, self.Ny, self.dx, self.dt = Nx, Ny, dx, dt
@@ -191,7 +218,8 @@ class Solver:
             raise TTSHError(TTSH_ERR_UNSUPPORTED_SIZE)
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.workspace = workspace if workspace is not None else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            nbytes = self.workspace.numel()
             mptr = 0
             if mask is not None:
                 want = torch.uint8 if mask_kind == TTSH_MASK_BINARY else self.tdtype
@@ -263,6 +291,53 @@ class Solver:
             self.torch.cuda.synchronize(self.device)
             ttsh_destroy(self.h)
             self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Ensemble:
+    """`count` independent systems on one grid (different masks / initial fields, same parameters) advanced together by
+    ttsh_ensemble_step: one launch of each hot kernel per Euler step for all members.  members[i] is an ordinary Solver."""
+
+    def __init__(self, count: int, Nx: int, Ny: int, dx: float, dt: float, params: ttsh_params, dtype: str = "f64",
+                 masks=None, mask_kind: int = TTSH_MASK_BINARY, device: str = "cuda:0", stream=None):
+        import torch
+        self.torch = torch
+        self.device = torch.device(device)
+        code = {"f64": TTSH_F64, "f32": TTSH_F32}[dtype]
+        nbytes = ttsh_workspace_bytes(Nx, Ny, code)
+        if nbytes == 0:
+            raise TTSHError(TTSH_ERR_UNSUPPORTED_SIZE)
+        stride = (nbytes + 255) // 256 * 256
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.workspace = torch.empty(stride * count, dtype=torch.uint8, device=self.device)
+        self.members = [Solver(Nx, Ny, dx, dt, params, dtype, mask=None if masks is None else masks[i], mask_kind=mask_kind,
+                               device=device, stream=self.stream, workspace=self.workspace[i * stride:(i + 1) * stride])
+                        for i in range(count)]
+        rc, self.e = ttsh_ensemble_create([m.h for m in self.members])
+        if rc != TTSH_OK:
+            raise TTSHError(rc)
+
+    def step(self, n: int = 1):
+        rc = ttsh_ensemble_step(self.e, n)
+        if rc != TTSH_OK:
+            raise TTSHError(rc, ttsh_last_error(self.members[0].h))
+
+    def launch_count(self) -> int:
+        return ttsh_ensemble_launch_count(self.e)
+
+    def close(self):
+        if getattr(self, "e", None):
+            self.torch.cuda.synchronize(self.device)
+            ttsh_ensemble_destroy(self.e)
+            self.e = None
+        for m in getattr(self, "members", []):
+            m.close()
 
     def __del__(self):
         try:

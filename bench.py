@@ -274,6 +274,31 @@ def measure(torch, ttsh, cfg, dtype, K, W, device, want_roofline=True, want_e2e=
     return out
 
 
+def measure_ensemble(torch, ttsh, name, count, device, nsteps=200):
+    """`count` members of one config's R sweep (radii spread over the config's sweep range, one seed each), advanced together."""
+    cfg, dtype = workload(name)
+    lo, hi = (min(cfg.sweep), max(cfg.sweep)) if cfg.sweep else (0.5 * cfg.R, cfg.R)
+    radii = [lo + (hi - lo) * i / max(1, count - 1) for i in range(count)]
+    masks = [cfg.mask(R=r) for r in radii]
+    ens = ttsh.Ensemble(count, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.baseline_params(), dtype, masks=masks, device=device)
+    from paper_2304_03306_b200 import workloads
+    for i, m in enumerate(ens.members):
+        m.set_velocity(*workloads.gaussian_velocity(cfg.Nx, cfg.Ny, cfg.seed + 1000 * (i + 1), 1e-2, masks[i]))
+    stream = torch.cuda.current_stream(device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ens.step(20)
+    torch.cuda.synchronize(device)
+    e0.record(stream)
+    ens.step(nsteps)
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    ms = e0.elapsed_time(e1) / nsteps
+    bad = sum(m.diagnostics()["nonfinite"] for m in (ens.members[0], ens.members[-1]))
+    ens.close()
+    return {"value": cfg.Nx * cfg.Ny * count / (ms * 1e-3), "unit": "grid-point-steps/s", "euler_step_ms": ms, "members": count,
+            "nonfinite": bad, "workload": f"{count} members of the {name} sweep, disk R = {lo:g}..{hi:g}, {dtype}, one ttsh_ensemble_step"}
+
+
 def reduce_over_ranks(dist, maxima, sums, device="cpu"):
     """Replicas only: the job time is the MAX over ranks, counts are SUMMED.  No data-path collective."""
     if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
@@ -417,6 +442,10 @@ def main():
             k2 = max(2, a.steps // 2)
             extra[name] = {"value": c2.Nx * c2.Ny * INNER * k2 / (r2["ms_total"] * 1e-3), "unit": "grid-point-steps/s",
                            "euler_step_ms": r2["ms_total"] / k2 / INNER, "workload": describe(c2, d2)}
+        # the paper's sweeps (R sweep of C1 / C2 / C3) as ensembles: ttsh_ensemble_step, one launch of each hot
+        # kernel per Euler step for all members
+        for name, count in (("C1", 256), ("C2", 64), ("C3", 16), ("C3-f32", 16)):
+            extra[f"{name} x{count} ensemble"] = measure_ensemble(torch, ttsh, name, count, device)
         line["other_workloads"] = extra
 
     if not a.no_cpu_baseline and world == 1:

@@ -18,4 +18,5 @@ from .ttsh_oracle import (  # noqa: F401
     cut_mask,
     process_mask,
     linear_symbol,
+    psi2_of_field,
 )

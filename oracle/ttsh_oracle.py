@@ -327,3 +327,42 @@ class TTSHOracle:
                     max_speed=float(speed.max()),
                     nonfinite=int(np.count_nonzero(~np.isfinite(vx)) + np.count_nonzero(~np.isfinite(vy))
                                   + np.count_nonzero(~np.isfinite(w))))
+
+    # -- ttsh_dumbbell_order ---------------------------------------------
+    def dumbbell_order(self, centre_left, centre_right, radius: float) -> dict:
+        """Psi_2 of the current vorticity field; see psi2_of_field."""
+        w = self._idft(self.w_hat).real
+        return psi2_of_field(w, self.dx, centre_left, centre_right, radius)
+
+
+def psi2_of_field(w: np.ndarray, dx: float, centre_left, centre_right, radius: float) -> dict:
+    """Order parameter of the dumbbell geometry:
+
+        Psi_2 = | w(x*_left) + w(x*_right) | / ( |w|(x*_left) + |w|(x*_right) ),   x*_side = argmax_side |w|,
+
+    "left"/"right" = the grid points within `radius` (the paper: D/2) of the centre of either cavity, i.e.
+    (i dx - cx)^2 + (j dx - cy)^2 <= radius^2 (inclusive; plain, non-periodic distance; evaluated in fp64 without
+    contraction).  Ties in |w| go to the lowest linear index j Nx + i; Psi_2 = 0 if the denominator is 0 or a region holds
+    no grid point (index -1).  Written as the definition: one pass over the grid per side."""
+    Ny, Nx = w.shape
+    out = {}
+    best = []
+    for side, (cx, cy) in (("left", centre_left), ("right", centre_right)):
+        bi, ba = -1, -1.0
+        for j in range(Ny):
+            yy = j * dx - cy
+            for i in range(Nx):
+                xx = i * dx - cx
+                if xx * xx + yy * yy <= radius * radius:
+                    a = abs(float(w[j, i]))
+                    if a > ba:
+                        ba, bi = a, j * Nx + i
+        val = float(w[bi // Nx, bi % Nx]) if bi >= 0 else 0.0
+        out["index_" + side] = bi
+        out["omega_" + side] = val
+        best.append(val)
+    den = abs(best[0]) + abs(best[1])
+    ok = den > 0.0 and out["index_left"] >= 0 and out["index_right"] >= 0
+    out["psi2"] = abs(best[0] + best[1]) / den if ok else 0.0
+    return out
+

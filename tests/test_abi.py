@@ -88,3 +88,11 @@ def test_product_path_never_imports_the_oracle():
         for f in files:
             if f.endswith(".py"):
                 assert not imp2.search(open(os.path.join(dirpath, f)).read()), f
+
+
+def test_ensemble_create_rejects_bad_arguments_without_touching_cuda(ttsh):
+    assert ttsh.ttsh_ensemble_create([])[0] == ttsh.TTSH_ERR_INVALID_ARG            # count < 1
+    assert ttsh.ttsh_ensemble_create([None])[0] == ttsh.TTSH_ERR_INVALID_ARG        # NULL member
+    assert ttsh.ttsh_ensemble_step(None, 1) == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_ensemble_destroy(None) == ttsh.TTSH_OK
+    assert ttsh.ttsh_ensemble_launch_count(None) == 0

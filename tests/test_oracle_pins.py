@@ -377,3 +377,84 @@ def test_rhs_terms_signs_on_a_hand_computable_field():
     assert np.max(np.abs(rhs1[1])) == 0.0
     assert np.max(np.abs(rhs2 - (-p.lambda0 * u * A * q * np.cos(q * x) - p.gamma_w * Kf * A * np.sin(q * x)))) < 1e-13
     assert np.max(np.abs(gy)) < 1e-14
+
+
+# ---------------------------------------------------------------- Psi_2 of the dumbbell geometry
+def _two_vortices(Nx, Ny, dx, cl, cr, al, ar, width=3.0):
+    x = np.arange(Nx)[None, :] * dx
+    y = np.arange(Ny)[:, None] * dx
+    g = lambda c: np.exp(-((x - c[0]) ** 2 + (y - c[1]) ** 2) / (2 * width ** 2))
+    return al * g(cl) + ar * g(cr)
+
+
+def test_psi2_ferromagnetic_antiferromagnetic_and_closed_form():
+    """'By construction, Psi_2 = 1 for the ferromagnetic flow and 0 for the antiferromagnetic one' (PAPER.md:199); for peak
+    vorticities a and -b the definition gives |a - b| / (a + b)."""
+    from oracle import psi2_of_field
+    Nx, Ny, dx = 96, 48, 0.5
+    cl, cr = (14.0, 12.0), (34.0, 12.0)            # grid points (28, 24) and (68, 24)
+    r = 6.0
+    d = psi2_of_field(_two_vortices(Nx, Ny, dx, cl, cr, 2.0, 0.7), dx, cl, cr, r)
+    assert d["psi2"] == 1.0 and d["index_left"] == 24 * Nx + 28 and d["index_right"] == 24 * Nx + 68
+    d = psi2_of_field(_two_vortices(Nx, Ny, dx, cl, cr, -1.5, -1.5), dx, cl, cr, r)
+    assert d["psi2"] == 1.0
+    d = psi2_of_field(_two_vortices(Nx, Ny, dx, cl, cr, 1.25, -1.25), dx, cl, cr, r)
+    assert d["psi2"] == 0.0
+    a, b = 2.0, 0.5
+    w = _two_vortices(Nx, Ny, dx, cl, cr, a, -b)
+    d = psi2_of_field(w, dx, cl, cr, r)
+    wl, wr = w[24, 28], w[24, 68]                   # the peaks (each Gaussian leaks ~1e-10 into the other cavity)
+    assert d["omega_left"] == wl and d["omega_right"] == wr
+    assert abs(d["psi2"] - (a - b) / (a + b)) < 1e-8 and d["psi2"] == abs(wl + wr) / (abs(wl) + abs(wr))
+
+
+def test_psi2_region_ties_and_degenerate_cases():
+    from oracle import psi2_of_field
+    Nx, Ny, dx = 40, 32, 0.5
+    cl, cr = (5.0, 8.0), (14.0, 8.0)
+    # a larger peak OUTSIDE both regions is ignored
+    w = _two_vortices(Nx, Ny, dx, cl, cr, 1.0, 1.0, width=1.0)
+    w[2, 2] = 50.0
+    w[31, 39] = -80.0
+    d = psi2_of_field(w, dx, cl, cr, 3.0)
+    assert d["index_left"] == 16 * Nx + 10 and d["index_right"] == 16 * Nx + 28 and d["psi2"] == 1.0
+    # the region is inclusive (<=) and uses the plain distance: radius 1.0 about a grid point holds exactly 13 points at dx = 0.5
+    ones = np.ones((Ny, Nx))
+    marked = np.zeros((Ny, Nx))
+    for j in range(Ny):
+        for i in range(Nx):
+            if (i * dx - 5.0) ** 2 + (j * dx - 8.0) ** 2 <= 1.0:
+                marked[j, i] = 1.0
+    assert marked.sum() == 13
+    # ties in |w| -> lowest linear index j Nx + i: the topmost point of the disk, (x, y) = (5.0, 7.0) -> (i, j) = (10, 14)
+    d = psi2_of_field(ones, dx, cl, cr, 1.0)
+    assert d["index_left"] == 14 * Nx + 10 and d["index_right"] == 14 * Nx + 28 and d["psi2"] == 1.0
+    # sign does not break a tie in |w|
+    w = ones.copy(); w[14, 10] = -1.0
+    assert psi2_of_field(w, dx, cl, cr, 1.0)["index_left"] == 14 * Nx + 10
+    assert psi2_of_field(w, dx, cl, cr, 1.0)["psi2"] == 0.0
+    # zero field, and a region without grid points
+    assert psi2_of_field(np.zeros((Ny, Nx)), dx, cl, cr, 1.0)["psi2"] == 0.0
+    d = psi2_of_field(ones, dx, (5.25, 8.25), cr, 0.1)
+    assert d["index_left"] == -1 and d["psi2"] == 0.0
+
+
+def test_psi2_of_the_oracle_state_uses_the_real_vorticity():
+    """TTSHOracle.dumbbell_order = psi2_of_field(iDFT[w^]): a two-vortex initial condition in a dumbbell keeps its signs."""
+    Nx, Ny, dx = 64, 32, 0.5
+    mask = workloads.dumbbell_mask(Nx, Ny, dx, 6.0, 9.0)
+    cl, cr = ((Nx // 2) * dx - 4.5, (Ny // 2) * dx), ((Nx // 2) * dx + 4.5, (Ny // 2) * dx)
+    x = np.arange(Nx)[None, :] * dx
+    y = np.arange(Ny)[:, None] * dx
+    def vortex(c, s):   # solid-body-like swirl with Gaussian envelope
+        e = np.exp(-((x - c[0]) ** 2 + (y - c[1]) ** 2) / 8.0)
+        return -s * (y - c[1]) * e, s * (x - c[0]) * e
+    for sl, sr, expect in ((1.0, 1.0, 1.0), (1.0, -1.0, 0.0)):
+        vxl, vyl = vortex(cl, sl); vxr, vyr = vortex(cr, sr)
+        o = TTSHOracle(Nx, Ny, dx, 0.01, BASELINE_PRESET, mask=mask)
+        o.set_velocity(vxl + vxr, vyl + vyr)
+        d = o.dumbbell_order(cl, cr, 4.5)
+        assert abs(d["psi2"] - expect) < 1e-6
+        w = o.get_fields()[2]
+        assert d["omega_left"] == w.flat[d["index_left"]] and d["omega_right"] == w.flat[d["index_right"]]
+

@@ -124,6 +124,20 @@ typedef struct {
 } ttsh_diag;
 int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out);
 
+/* Order parameter of the dumbbell geometry:
+ *   Psi_2 = | w(x*_left) + w(x*_right) | / ( |w|(x*_left) + |w|(x*_right) ),   x*_side = argmax_side |w|,
+ * "left"/"right" = the grid points within `radius` (the paper: D/2) of the centre of either cavity (physical units;
+ * (i dx - cx)^2 + (j dx - cy)^2 <= radius^2, inclusive, plain non-periodic distance).  Ties in |w| go to the lowest linear
+ * index j Nx + i.  psi2 = 0 when the denominator vanishes or a region holds no grid point (index -1).  1 = ferromagnetic
+ * (same-sign vortices), 0 = antiferromagnetic.  host_out: HOST.  Synchronises the stream. */
+typedef struct {
+  double psi2;
+  double omega_left, omega_right;        /* w at the two maximisers */
+  long long index_left, index_right;     /* their linear indices j Nx + i */
+} ttsh_psi2;
+int ttsh_dumbbell_order(ttsh_handle* h, double cx_left, double cy_left, double cx_right, double cy_right, double radius,
+                        ttsh_psi2* host_out);
+
 /* Ensembles: the paper's workload is sweeps of independent runs on one grid — disk radius R (Fig. 2), the
  * hysteresis branches, dumbbell separations — and on grids up to about 1024^2 one system
  * cannot fill a B200.  An ensemble advances `count` independent handles with ONE launch of each hot kernel per Euler step

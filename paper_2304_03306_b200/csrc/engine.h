@@ -56,4 +56,8 @@ constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs
 template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,
                                               const void* w, double* partial, double* out, cudaStream_t s);
 
+// Psi_2: per side (|w|, w, linear index) of the argmax of |w| within `radius` of (cx, cy); out[6]
+template <typename T> cudaError_t launch_region_argmax(const Geom& g, double dx, double cxl, double cyl, double cxr, double cyr, double radius,
+                                                       const void* w, double* partial, double* out, cudaStream_t s);
+
 }  // namespace ttsh

@@ -76,7 +76,17 @@ template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double c
   return cudaGetLastError();
 }
 
+template <typename T> cudaError_t launch_region_argmax(const Geom& g, double dx, double cxl, double cyl, double cxr, double cyr, double radius,
+                                                       const void* w, double* partial, double* out, cudaStream_t s) {
+  k_region_argmax_partial<T><<<DIAG_BLOCKS, 256, 0, s>>>(g.Nx, g.Ny, dx, cxl, cyl, cxr, cyr, radius, (const T*)w, partial);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_region_argmax_final<<<1, 256, 0, s>>>(DIAG_BLOCKS, partial, out);
+  return cudaGetLastError();
+}
+
 #define INST(T) \
+  template cudaError_t launch_region_argmax<T>(const Geom&, double, double, double, double, double, double, const void*, double*, double*, cudaStream_t); \
   template cudaError_t launch_realspace<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
   template cudaError_t launch_realspace_cons<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
   template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, double*, cudaStream_t); \

@@ -390,4 +390,65 @@ __global__ void __launch_bounds__(256) k_diag_final(int nblocks, const double* _
   diag_block_reduce(a, out);
 }
 
+// ---------------------------------------------------------------------------------------
+// Psi_2 of the dumbbell geometry: per side, argmax of |w| over the grid points within `radius` of the cavity
+// centre, (i dx - cx)^2 + (j dx - cy)^2 <= radius^2 evaluated in fp64 without contraction (the same IEEE operations as the
+// definition), ties to the lowest linear index.  Record per side: (|w|, w, index); index -1 = no point.
+// ---------------------------------------------------------------------------------------
+struct ArgBest { double a, v, i; };
+__device__ __forceinline__ void arg_merge(ArgBest& x, double a, double v, double i) {
+  if (a > x.a || (a == x.a && i < x.i)) { x.a = a; x.v = v; x.i = i; }
+}
+__device__ __forceinline__ void arg_warp_reduce(ArgBest& x) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double a = __shfl_down_sync(0xffffffffu, x.a, o), v = __shfl_down_sync(0xffffffffu, x.v, o), i = __shfl_down_sync(0xffffffffu, x.i, o);
+    arg_merge(x, a, v, i);
+  }
+}
+__device__ __forceinline__ void arg_block_reduce(ArgBest* x, double* out) {     // x[2] -> out[6], thread 0 writes
+  __shared__ double sh[32][6];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  for (int s = 0; s < 2; ++s) {
+    arg_warp_reduce(x[s]);
+    if (lane == 0) { sh[wid][3 * s] = x[s].a; sh[wid][3 * s + 1] = x[s].v; sh[wid][3 * s + 2] = x[s].i; }
+  }
+  __syncthreads();
+  if (wid == 0) {
+    for (int s = 0; s < 2; ++s) {
+      ArgBest y;
+      y.a = lane < nw ? sh[lane][3 * s] : -1.0; y.v = lane < nw ? sh[lane][3 * s + 1] : 0.0; y.i = lane < nw ? sh[lane][3 * s + 2] : -1.0;
+      arg_warp_reduce(y);
+      if (lane == 0) { out[3 * s] = y.a; out[3 * s + 1] = y.v; out[3 * s + 2] = y.i; }
+    }
+  }
+}
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_region_argmax_partial(int Nx, int Ny, double dx, double cxl, double cyl, double cxr, double cyr, double radius,
+                        const T* __restrict__ w, double* __restrict__ partial) {
+  ArgBest x[2];
+  x[0].a = x[1].a = -1.0; x[0].v = x[1].v = 0.0; x[0].i = x[1].i = -1.0;
+  const double r2 = __dmul_rn(radius, radius);
+  const size_t n = (size_t)Nx * Ny;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const double px = __dmul_rn((double)(int)(i % Nx), dx), py = __dmul_rn((double)(int)(i / Nx), dx);
+    const double ww = (double)w[i];
+    const double xl = __dsub_rn(px, cxl), yl = __dsub_rn(py, cyl), xr = __dsub_rn(px, cxr), yr = __dsub_rn(py, cyr);
+    if (__dadd_rn(__dmul_rn(xl, xl), __dmul_rn(yl, yl)) <= r2) arg_merge(x[0], fabs(ww), ww, (double)i);
+    if (__dadd_rn(__dmul_rn(xr, xr), __dmul_rn(yr, yr)) <= r2) arg_merge(x[1], fabs(ww), ww, (double)i);
+  }
+  arg_block_reduce(x, partial + (size_t)blockIdx.x * DIAG_REC);
+}
+__global__ void __launch_bounds__(256) k_region_argmax_final(int nblocks, const double* __restrict__ partial, double* __restrict__ out) {
+  ArgBest x[2];
+  x[0].a = x[1].a = -1.0; x[0].v = x[1].v = 0.0; x[0].i = x[1].i = -1.0;
+  for (int b = threadIdx.x; b < nblocks; b += blockDim.x)
+    for (int s = 0; s < 2; ++s) {
+      const double* r = partial + (size_t)b * DIAG_REC + 3 * s;
+      arg_merge(x[s], r[0], r[1], r[2]);
+    }
+  arg_block_reduce(x, out);
+}
+
 }  // namespace ttsh

@@ -565,6 +565,28 @@ int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out) 
   return TTSH_OK;
 }
 
+int ttsh_dumbbell_order(ttsh_handle* h, double cxl, double cyl, double cxr, double cyr, double radius, ttsh_psi2* host_out) {
+  if (!h || !host_out || !(radius >= 0.0) || !std::isfinite(radius)) return TTSH_ERR_INVALID_ARG;
+  if (!std::isfinite(cxl) || !std::isfinite(cyl) || !std::isfinite(cxr) || !std::isfinite(cyr)) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  int rc = enqueue_inverse(h, h->R[0], nullptr, nullptr, nullptr, nullptr, nullptr);
+  if (rc != TTSH_OK) return rc;
+  TRY(h, DISPATCH(h, launch_region_argmax, h->g, h->dx, cxl, cyl, cxr, cyr, radius, h->R[0], h->diag_partial, h->diag_out, h->stream));
+  h->launches += 2;
+  double rec[6];
+  TRY(h, cudaMemcpyAsync(rec, h->diag_out, sizeof(rec), cudaMemcpyDeviceToHost, h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));
+  ttsh_psi2 d;
+  d.index_left = (long long)rec[2]; d.index_right = (long long)rec[5];
+  d.omega_left = d.index_left >= 0 ? rec[1] : 0.0;
+  d.omega_right = d.index_right >= 0 ? rec[4] : 0.0;
+  const double den = fabs(d.omega_left) + fabs(d.omega_right);
+  d.psi2 = (den > 0.0 && d.index_left >= 0 && d.index_right >= 0) ? fabs(d.omega_left + d.omega_right) / den : 0.0;
+  *host_out = d;
+  return TTSH_OK;
+}
+
 // ---- ensembles -----------------------------------------------------------------------------------------------
 int ttsh_ensemble_create(ttsh_ensemble** out, ttsh_handle* const* members, int count) {
   if (!out) return TTSH_ERR_INVALID_ARG;

@@ -30,7 +30,7 @@ TTSH_ADVECTION_CONSERVATIVE, TTSH_ADVECTION_LITERAL = 0, 1
 SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_velocity", "ttsh_set_advection_form", "ttsh_step",
            "ttsh_get_fields", "ttsh_state_elems", "ttsh_get_state", "ttsh_set_state", "ttsh_diagnostics",
            "ttsh_launch_count", "ttsh_run_stage", "ttsh_debug_get_real", "ttsh_destroy", "ttsh_strerror",
-           "ttsh_last_error", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
+           "ttsh_last_error", "ttsh_dumbbell_order", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
            "ttsh_ensemble_destroy")
 
 
@@ -74,6 +74,7 @@ _sig = {
     "ttsh_destroy": (_i, [_vp]),
     "ttsh_strerror": (C.c_char_p, [_i]),
     "ttsh_last_error": (C.c_char_p, [_vp]),
+    "ttsh_dumbbell_order": (_i, [_vp, _d, _d, _d, _d, _d, _vp]),
     "ttsh_ensemble_create": (_i, [C.POINTER(_vp), C.POINTER(_vp), _i]),
     "ttsh_ensemble_step": (_i, [_vp, _i]),
     "ttsh_ensemble_launch_count": (_ll, [_vp]),
@@ -82,6 +83,14 @@ _sig = {
 for _name, (_res, _args) in _sig.items():
     _f = getattr(_lib, _name)
     _f.restype, _f.argtypes = _res, _args
+
+
+class ttsh_psi2(C.Structure):
+    _fields_ = [("psi2", C.c_double), ("omega_left", C.c_double), ("omega_right", C.c_double),
+                ("index_left", C.c_longlong), ("index_right", C.c_longlong)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
 
 
 class TTSHError(RuntimeError):
@@ -143,6 +152,12 @@ def ttsh_set_state(h, w_hat_ptr, mean_flow, t, step):
 def ttsh_diagnostics(h, cx, cy):
     d = ttsh_diag()
     rc = _lib.ttsh_diagnostics(h, cx, cy, C.byref(d))
+    return rc, d
+
+
+def ttsh_dumbbell_order(h, cx_left, cy_left, cx_right, cy_right, radius):
+    d = ttsh_psi2()
+    rc = _lib.ttsh_dumbbell_order(h, cx_left, cy_left, cx_right, cy_right, radius, C.byref(d))
     return rc, d
 
 
@@ -272,6 +287,11 @@ class Solver:
         cx = (self.Nx // 2) * self.dx if cx is None else cx
         cy = (self.Ny // 2) * self.dx if cy is None else cy
         rc, d = ttsh_diagnostics(self.h, cx, cy)
+        self._check(rc)
+        return d.as_dict()
+
+    def dumbbell_order(self, centre_left, centre_right, radius: float) -> dict:
+        rc, d = ttsh_dumbbell_order(self.h, centre_left[0], centre_left[1], centre_right[0], centre_right[1], radius)
         self._check(rc)
         return d.as_dict()
 

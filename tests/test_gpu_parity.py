@@ -363,3 +363,68 @@ def test_C5_unconfined_periodic_single_step(ttsh):
     s.step(1); o.step(1)
     compare_state(s, o, TOL_F64_1, "C5p step 1")
     s.close()
+
+
+# ---------------------------------------------------------------- Psi_2 of the dumbbell geometry
+def _vortex_pair_velocity(Nx, Ny, dx, cl, cr, sl, sr):
+    x = np.arange(Nx)[None, :] * dx
+    y = np.arange(Ny)[:, None] * dx
+    vx = np.zeros((Ny, Nx)); vy = np.zeros((Ny, Nx))
+    for c, s in ((cl, sl), (cr, sr)):
+        e = np.exp(-((x - c[0]) ** 2 + (y - c[1]) ** 2) / 18.0)
+        vx += -s * (y - c[1]) * e
+        vy += s * (x - c[0]) * e
+    return vx, vy
+
+
+@pytest.mark.parametrize("Nx,Ny,R,d,sl,sr,nsteps", [(128, 64, 10.0, 16.0, 1.0, 0.8, 20), (128, 64, 10.0, 16.0, 1.0, -0.7, 20),
+                                                   (256, 128, 20.0, 30.0, -0.6, 1.0, 5)])
+def test_dumbbell_order_parameter_matches_oracle(ttsh, Nx, Ny, R, d, sl, sr, nsteps):
+    """ttsh_dumbbell_order vs the oracle's definition: the maximisers are unique here (smooth vortices), so index, w at the
+    maximiser and Psi_2 must all agree (indices exactly, values to the field tolerance)."""
+    dx = 0.5
+    mask = workloads.dumbbell_mask(Nx, Ny, dx, R, d)
+    cl, cr = ((Nx // 2) * dx - d / 2, (Ny // 2) * dx), ((Nx // 2) * dx + d / 2, (Ny // 2) * dx)
+    vel = _vortex_pair_velocity(Nx, Ny, dx, cl, cr, sl, sr)
+    s, o = make_pair(ttsh, Nx, Ny, dx, 0.01, "baseline", mask, vel=vel)
+    for n in (0, nsteps):
+        s.step(n); o.step(n)
+        g, r = s.dumbbell_order(cl, cr, d / 2), o.dumbbell_order(cl, cr, d / 2)
+        assert g["index_left"] == r["index_left"] and g["index_right"] == r["index_right"]
+        wmax = max(abs(r["omega_left"]), abs(r["omega_right"]))
+        assert abs(g["omega_left"] - r["omega_left"]) <= 1e-9 * wmax and abs(g["omega_right"] - r["omega_right"]) <= 1e-9 * wmax
+        assert abs(g["psi2"] - r["psi2"]) <= 1e-9
+    same = sl * sr > 0
+    assert (g["psi2"] > 0.99) if same else (g["psi2"] < 0.5)
+    s.close()
+
+
+def test_dumbbell_order_regions_ties_and_fp32(ttsh):
+    """Region membership and tie-breaking are integer/IEEE decisions: the kernel must take exactly the oracle's."""
+    from oracle import psi2_of_field
+    Nx, Ny, dx = 128, 64, 0.5
+    mask = workloads.dumbbell_mask(Nx, Ny, dx, 10.0, 16.0)
+    vel = workloads.gaussian_velocity(Nx, Ny, workloads.SEED0 + 9, 1.0, mask)     # rough field: many near-maximal points
+    for dtype in ("f64", "f32"):
+        s = ttsh.Solver(Nx, Ny, dx, 0.01, ttsh.baseline_params(), dtype, mask=mask)
+        s.set_velocity(*vel)
+        s.step(2)
+        w = s.get_fields()[2].cpu().numpy().astype(np.float64)                     # the kernel's own w: decisions must match on it
+        for cl, cr, rad in (((24.0, 16.0), (40.0, 16.0), 8.0), ((24.25, 16.1), (40.3, 15.9), 3.3), ((5.0, 5.0), (60.0, 30.0), 0.0),
+                            ((-50.0, 16.0), (40.0, 16.0), 2.0), ((0.0, 0.0), (63.5, 31.5), 200.0)):
+            g = s.dumbbell_order(cl, cr, rad)
+            r = psi2_of_field(w, dx, cl, cr, rad)
+            assert g["index_left"] == r["index_left"] and g["index_right"] == r["index_right"], (dtype, cl, cr, rad)
+            assert g["omega_left"] == r["omega_left"] and g["omega_right"] == r["omega_right"]
+            assert abs(g["psi2"] - r["psi2"]) <= 1e-15
+        s.close()
+    # exact ties: a zero field has |w| = 0 everywhere -> the lowest linear index of each region, Psi_2 = 0
+    s = ttsh.Solver(Nx, Ny, dx, 0.01, ttsh.baseline_params(), "f64", mask=mask)
+    z = np.zeros((Ny, Nx))
+    s.set_velocity(z, z)
+    g = s.dumbbell_order((24.0, 16.0), (40.0, 16.0), 1.0)
+    r = psi2_of_field(z, dx, (24.0, 16.0), (40.0, 16.0), 1.0)
+    assert g["index_left"] == r["index_left"] == 30 * Nx + 48 and g["index_right"] == r["index_right"] and g["psi2"] == 0.0
+    assert ttsh.ttsh_dumbbell_order(s.h, 0.0, 0.0, 1.0, 1.0, -1.0)[0] == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_dumbbell_order(s.h, float("nan"), 0.0, 1.0, 1.0, 1.0)[0] == ttsh.TTSH_ERR_INVALID_ARG
+    s.close()

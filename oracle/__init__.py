@@ -19,4 +19,5 @@ from .ttsh_oracle import (  # noqa: F401
     process_mask,
     linear_symbol,
     psi2_of_field,
+    temporal_psd,
 )

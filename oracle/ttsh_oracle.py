@@ -366,3 +366,21 @@ def psi2_of_field(w: np.ndarray, dx: float, centre_left, centre_right, radius: f
     out["psi2"] = abs(best[0] + best[1]) / den if ok else 0.0
     return out
 
+
+def temporal_psd(series, times, omegas) -> np.ndarray:
+    """Temporal power spectral density of the vorticity field, Eq. (5):
+
+        S(Omega) = (1/P) sum_x | sum_t w(x, t) exp(-i Omega t) |^2 ,   P = number of grid points,
+
+    for the samples series[n] = w(., times[n]) and every Omega in omegas.  Written as the definition (one complex
+    accumulator per point and frequency); accumulation in fp64, the final sum over x in long double."""
+    series = [np.asarray(f, dtype=np.float64) for f in series]
+    P = series[0].size
+    out = np.zeros(len(omegas))
+    for m, Om in enumerate(omegas):
+        acc = np.zeros(series[0].shape, dtype=np.complex128)
+        for f, t in zip(series, times):
+            acc += f * complex(np.cos(Om * t), -np.sin(Om * t))
+        out[m] = float(np.sum(acc.real * acc.real + acc.imag * acc.imag, dtype=np.longdouble)) / P
+    return out
+

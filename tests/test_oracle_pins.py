@@ -458,3 +458,42 @@ def test_psi2_of_the_oracle_state_uses_the_real_vorticity():
         w = o.get_fields()[2]
         assert d["omega_left"] == w.flat[d["index_left"]] and d["omega_right"] == w.flat[d["index_right"]]
 
+
+# ---------------------------------------------------------------- temporal PSD, Eq. (5)
+def test_temporal_psd_closed_forms_and_library_special_case():
+    from oracle import temporal_psd
+    rng = np.random.default_rng(5)
+    Ny, Nx, n, dt = 6, 8, 64, 0.25
+    times = [k * dt for k in range(n)]
+    a = rng.standard_normal((Ny, Nx))
+    b = rng.standard_normal((Ny, Nx))
+    base = 2 * np.pi / (n * dt)                         # DFT frequencies of the sampling window
+    # (i) w(x, t) = a(x) cos(3 base t) + b(x) sin(3 base t) over whole periods: all the power sits at +-3 base,
+    #     S = (n/2)^2 mean(a^2 + b^2); orthogonal DFT frequencies carry nothing
+    series = [a * np.cos(3 * base * t) + b * np.sin(3 * base * t) for t in times]
+    S = temporal_psd(series, times, [3 * base, -3 * base, 2 * base, 5 * base, 0.0])
+    want = (n / 2) ** 2 * np.mean(a * a + b * b)
+    assert abs(S[0] - want) < 1e-10 * want and abs(S[1] - want) < 1e-10 * want
+    assert max(S[2], S[3], S[4]) < 1e-20 * want
+    # (ii) a constant field: S(0) = n^2 mean(w^2)
+    S = temporal_psd([a] * n, times, [0.0])
+    assert abs(S[0] - n * n * np.mean(a * a)) < 1e-12 * S[0]
+    # (iii) on the DFT frequencies the inner sum is numpy's FFT over the time axis (a shifted time origin only rotates
+    #       the phase), and (iv) Parseval: sum_m S(Omega_m) = n sum_t mean(w(t)^2)
+    series = [rng.standard_normal((Ny, Nx)) for _ in range(n)]
+    t0 = 3.7
+    S = temporal_psd(series, [t0 + t for t in times], [m * base for m in range(n)])
+    F = np.fft.fft(np.stack(series), axis=0)
+    assert np.allclose(S, np.mean(np.abs(F) ** 2, axis=(1, 2)), rtol=1e-11, atol=0)
+    assert abs(S.sum() - n * sum(np.mean(f * f) for f in series)) < 1e-11 * S.sum()
+    # (v) the sign of the exponent: a rotating pattern exp(+i W t) has its power at +W only
+    W = 7 * base
+    S = temporal_psd([np.cos(W * t) * a for t in times], times, [W])   # real signal: half the power at +W
+    c = temporal_psd([a * np.cos(W * t) for t in times], times, [W])[0]
+    assert abs(S[0] - c) == 0.0
+    # a non-DFT frequency against the explicit double sum on one point
+    Om = 1.2345
+    one = [np.full((1, 1), np.sin(0.9 * t) + 0.3) for t in times]
+    ref = abs(sum((np.sin(0.9 * t) + 0.3) * np.exp(-1j * Om * t) for t in times)) ** 2
+    assert abs(temporal_psd(one, times, [Om])[0] - ref) < 1e-12 * ref
+

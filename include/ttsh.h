@@ -138,6 +138,21 @@ typedef struct {
 int ttsh_dumbbell_order(ttsh_handle* h, double cx_left, double cy_left, double cx_right, double cy_right, double radius,
                         ttsh_psi2* host_out);
 
+/* Streaming temporal power spectral density of the vorticity field, Eq. (5):
+ *   S(Omega) = (1/P) sum_x | sum_t w(x, t) exp(-i Omega t) |^2,   P = Nx Ny,
+ * for a caller-chosen set of angular frequencies: one complex accumulator per grid point and frequency, updated by
+ * ttsh_psd_accumulate with the handle's current field w(., t) (t = the handle's time), so no time series is ever stored.
+ * omegas: HOST double[nfreq], 1 <= nfreq <= 1024.  workspace: DEVICE, >= ttsh_psd_workspace_bytes (about
+ * nfreq x 2 fields), 256-byte aligned, owned by the caller, zeroed by create / reset (stream-ordered).  Accumulators have
+ * the handle's scalar type; the sum over x is taken in double.  The accumulator borrows the handle: destroy it first. */
+typedef struct ttsh_psd ttsh_psd;
+size_t ttsh_psd_workspace_bytes(int Nx, int Ny, ttsh_dtype t, int nfreq);       /* 0 if unsupported */
+int ttsh_psd_create(ttsh_psd** out, ttsh_handle* h, const double* omegas, int nfreq, void* workspace, size_t workspace_bytes);
+int ttsh_psd_accumulate(ttsh_psd* s);                                           /* asynchronous */
+int ttsh_psd_result(ttsh_psd* s, double* S_host, long long* nsamples_host);     /* S_host: HOST double[nfreq]; nsamples may be NULL; synchronises */
+int ttsh_psd_reset(ttsh_psd* s);
+int ttsh_psd_destroy(ttsh_psd* s);
+
 /* Ensembles: the paper's workload is sweeps of independent runs on one grid — disk radius R (Fig. 2), the
  * hysteresis branches, dumbbell separations — and on grids up to about 1024^2 one system
  * cannot fill a B200.  An ensemble advances `count` independent handles with ONE launch of each hot kernel per Euler step

@@ -60,4 +60,10 @@ template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double c
 template <typename T> cudaError_t launch_region_argmax(const Geom& g, double dx, double cxl, double cyl, double cxr, double cyr, double radius,
                                                        const void* w, double* partial, double* out, cudaStream_t s);
 
+// streaming temporal PSD, Eq. (5): acc[nf][n] += w exp(-i Omega t) with host-computed phases cs = cos(Omega t),
+// sn = -sin(Omega t) (HOST arrays);  out[m] = sum_x |acc[m][x]|^2 through partial[nf][psd_blocks()]
+template <typename T> cudaError_t launch_psd_accumulate(size_t n, int nf, const double* cs, const double* sn, const void* w, void* acc, cudaStream_t s);
+template <typename T> cudaError_t launch_psd_power(size_t n, int nf, const void* acc, double* partial, double* out, cudaStream_t s);
+int psd_blocks();
+
 }  // namespace ttsh

@@ -85,7 +85,29 @@ template <typename T> cudaError_t launch_region_argmax(const Geom& g, double dx,
   return cudaGetLastError();
 }
 
+template <typename T> cudaError_t launch_psd_accumulate(size_t n, int nf, const double* cs, const double* sn, const void* w, void* acc, cudaStream_t s) {
+  for (int m0 = 0; m0 < nf; m0 += PSD_CHUNK) {
+    const int cnt = nf - m0 < PSD_CHUNK ? nf - m0 : PSD_CHUNK;
+    PsdPhases ph;
+    for (int m = 0; m < PSD_CHUNK; ++m) { ph.c[m] = m < cnt ? cs[m0 + m] : 0.0; ph.s[m] = m < cnt ? sn[m0 + m] : 0.0; }
+    k_psd_accumulate<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, cnt, ph, (const T*)w, (cplx<T>*)acc + (size_t)m0 * n);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+template <typename T> cudaError_t launch_psd_power(size_t n, int nf, const void* acc, double* partial, double* out, cudaStream_t s) {
+  k_psd_power_partial<T><<<dim3(PSD_BLOCKS, nf), 256, 0, s>>>(n, (const cplx<T>*)acc, partial);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_psd_power_final<<<nf, 32, 0, s>>>(PSD_BLOCKS, partial, out);
+  return cudaGetLastError();
+}
+int psd_blocks() { return PSD_BLOCKS; }
+
 #define INST(T) \
+  template cudaError_t launch_psd_accumulate<T>(size_t, int, const double*, const double*, const void*, void*, cudaStream_t); \
+  template cudaError_t launch_psd_power<T>(size_t, int, const void*, double*, double*, cudaStream_t); \
   template cudaError_t launch_region_argmax<T>(const Geom&, double, double, double, double, double, double, const void*, double*, double*, cudaStream_t); \
   template cudaError_t launch_realspace<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
   template cudaError_t launch_realspace_cons<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \

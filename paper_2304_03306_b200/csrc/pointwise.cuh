@@ -451,4 +451,70 @@ __global__ void __launch_bounds__(256) k_region_argmax_final(int nblocks, const 
   arg_block_reduce(x, out);
 }
 
+// ---------------------------------------------------------------------------------------
+// streaming temporal PSD, Eq. (5): per point and frequency one complex accumulator
+//   A_m(x) += w(x, t) exp(-i Omega_m t);     S(Omega_m) = (1/P) sum_x |A_m(x)|^2
+// acc is frequency-major [nf][n]: every access is unit-stride.  The phases of one sample (host-computed, <= 64 per launch)
+// travel as a kernel argument.  Pure streaming: 2 x sizeof(cplx<T>) bytes per point and frequency -> HBM-bound.
+// ---------------------------------------------------------------------------------------
+constexpr int PSD_CHUNK = 64;
+constexpr int PSD_BLOCKS = 296;
+struct PsdPhases { double c[PSD_CHUNK], s[PSD_CHUNK]; };      // cos(Omega t), -sin(Omega t)
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_psd_accumulate(size_t n, int nf, const __grid_constant__ PsdPhases ph, const T* __restrict__ w, cplx<T>* __restrict__ acc) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const T ww = w[i];
+    int m = 0;
+    for (; m + 4 <= nf; m += 4) {                 // four independent read-modify-write streams in flight per thread
+      cplx<T> v[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) v[u] = acc[(size_t)(m + u) * n + i];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        v[u].x += ww * (T)ph.c[m + u];
+        v[u].y += ww * (T)ph.s[m + u];
+        acc[(size_t)(m + u) * n + i] = v[u];
+      }
+    }
+    for (; m < nf; ++m) {
+      cplx<T> v = acc[(size_t)m * n + i];
+      v.x += ww * (T)ph.c[m];
+      v.y += ww * (T)ph.s[m];
+      acc[(size_t)m * n + i] = v;
+    }
+  }
+}
+// partial[m][b] = sum over the block's points of |A_m|^2 (fp64);  grid (PSD_BLOCKS, nf)
+template <typename T>
+__global__ void __launch_bounds__(256) k_psd_power_partial(size_t n, const cplx<T>* __restrict__ acc, double* __restrict__ partial) {
+  const cplx<T>* a = acc + (size_t)blockIdx.y * n;
+  double sum = 0.0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const double x = (double)a[i].x, y = (double)a[i].y;
+    sum += x * x + y * y;
+  }
+  __shared__ double sh[32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+  if (lane == 0) sh[wid] = sum;
+  __syncthreads();
+  if (wid == 0) {
+    sum = lane < (int)(blockDim.x >> 5) ? sh[lane] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+    if (lane == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = sum;
+  }
+}
+// out[m] = sum_b partial[m][b];  grid nf, one warp each
+__global__ void __launch_bounds__(32) k_psd_power_final(int nblocks, const double* __restrict__ partial, double* __restrict__ out) {
+  double sum = 0.0;
+  for (int b = threadIdx.x; b < nblocks; b += 32) sum += partial[(size_t)blockIdx.x * nblocks + b];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+  if (threadIdx.x == 0) out[blockIdx.x] = sum;
+}
+
 }  // namespace ttsh

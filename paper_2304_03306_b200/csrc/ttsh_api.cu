@@ -97,6 +97,15 @@ struct ttsh_handle {
   bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
 };
 
+struct ttsh_psd {
+  ttsh_handle* h;                      // borrowed
+  std::vector<double> omegas, cs, sn;  // frequencies; phases of the current sample (host)
+  void* acc;                           // cplx<T>[nfreq][Ny*Nx] in the caller's workspace
+  size_t acc_bytes;
+  double *partial, *out;
+  long long nsamples;
+};
+
 struct ttsh_ensemble {
   std::vector<ttsh_handle*> members;   // borrowed
   size_t mstride;                      // bytes between consecutive members' workspaces
@@ -584,6 +593,86 @@ int ttsh_dumbbell_order(ttsh_handle* h, double cxl, double cyl, double cxr, doub
   const double den = fabs(d.omega_left) + fabs(d.omega_right);
   d.psi2 = (den > 0.0 && d.index_left >= 0 && d.index_right >= 0) ? fabs(d.omega_left + d.omega_right) / den : 0.0;
   *host_out = d;
+  return TTSH_OK;
+}
+
+// ---- streaming temporal PSD (Eq. 5) ------------------------------------------------------------------------
+struct PsdLayout { size_t acc, partial, out, total; };
+static PsdLayout psd_layout(int Nx, int Ny, size_t w, int nfreq) {
+  PsdLayout L;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+  L.acc = take((size_t)nfreq * Nx * Ny * 2 * w);
+  L.partial = take((size_t)nfreq * psd_blocks() * sizeof(double));
+  L.out = take((size_t)nfreq * sizeof(double));
+  L.total = off;
+  return L;
+}
+size_t ttsh_psd_workspace_bytes(int Nx, int Ny, ttsh_dtype t, int nfreq) {
+  if (!pow2_in_range(Nx) || !pow2_in_range(Ny) || (t != TTSH_F64 && t != TTSH_F32) || nfreq < 1 || nfreq > 1024) return 0;
+  return psd_layout(Nx, Ny, (size_t)t, nfreq).total;
+}
+int ttsh_psd_create(ttsh_psd** out, ttsh_handle* h, const double* omegas, int nfreq, void* workspace, size_t workspace_bytes) {
+  if (!out) return TTSH_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!h || !omegas || !workspace || nfreq < 1 || nfreq > 1024) return TTSH_ERR_INVALID_ARG;
+  if (reinterpret_cast<uintptr_t>(workspace) % ALIGN) return TTSH_ERR_INVALID_ARG;
+  for (int m = 0; m < nfreq; ++m) if (!std::isfinite(omegas[m])) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  const PsdLayout L = psd_layout(h->Nx, h->Ny, (size_t)h->dtype, nfreq);
+  if (workspace_bytes < L.total) return TTSH_ERR_WORKSPACE_TOO_SMALL;
+  ttsh_psd* s = new (std::nothrow) ttsh_psd();
+  if (!s) return TTSH_ERR_INVALID_ARG;
+  s->h = h;
+  s->omegas.assign(omegas, omegas + nfreq);
+  s->cs.resize(nfreq); s->sn.resize(nfreq);
+  char* ws = static_cast<char*>(workspace);
+  s->acc = ws + L.acc;
+  s->acc_bytes = (size_t)nfreq * h->Nx * h->Ny * 2 * (size_t)h->dtype;
+  s->partial = reinterpret_cast<double*>(ws + L.partial);
+  s->out = reinterpret_cast<double*>(ws + L.out);
+  s->nsamples = 0;
+  *out = s;
+  TRY(h, cudaMemsetAsync(s->acc, 0, s->acc_bytes, h->stream));
+  return TTSH_OK;
+}
+int ttsh_psd_accumulate(ttsh_psd* s) {
+  if (!s) return TTSH_ERR_INVALID_ARG;
+  ttsh_handle* h = s->h;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  int rc = enqueue_inverse(h, h->R[0], nullptr, nullptr, nullptr, nullptr, nullptr);     // w(., t)
+  if (rc != TTSH_OK) return rc;
+  const int nf = (int)s->omegas.size();
+  for (int m = 0; m < nf; ++m) { s->cs[m] = cos(s->omegas[m] * h->t); s->sn[m] = -sin(s->omegas[m] * h->t); }
+  TRY(h, DISPATCH(h, launch_psd_accumulate, (size_t)h->Nx * h->Ny, nf, s->cs.data(), s->sn.data(), h->R[0], s->acc, h->stream));
+  h->launches += (nf + 63) / 64;
+  s->nsamples++;
+  return TTSH_OK;
+}
+int ttsh_psd_result(ttsh_psd* s, double* S_host, long long* nsamples_host) {
+  if (!s || !S_host) return TTSH_ERR_INVALID_ARG;
+  ttsh_handle* h = s->h;
+  if (h->sticky) return h->sticky;
+  const int nf = (int)s->omegas.size();
+  TRY(h, DISPATCH(h, launch_psd_power, (size_t)h->Nx * h->Ny, nf, s->acc, s->partial, s->out, h->stream));
+  h->launches += 2;
+  TRY(h, cudaMemcpyAsync(S_host, s->out, (size_t)nf * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));
+  const double P = (double)h->Nx * (double)h->Ny;
+  for (int m = 0; m < nf; ++m) S_host[m] /= P;
+  if (nsamples_host) *nsamples_host = s->nsamples;
+  return TTSH_OK;
+}
+int ttsh_psd_reset(ttsh_psd* s) {
+  if (!s) return TTSH_ERR_INVALID_ARG;
+  if (s->h->sticky) return s->h->sticky;
+  TRY(s->h, cudaMemsetAsync(s->acc, 0, s->acc_bytes, s->h->stream));
+  s->nsamples = 0;
+  return TTSH_OK;
+}
+int ttsh_psd_destroy(ttsh_psd* s) {
+  delete s;
   return TTSH_OK;
 }
 

@@ -30,7 +30,8 @@ TTSH_ADVECTION_CONSERVATIVE, TTSH_ADVECTION_LITERAL = 0, 1
 SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_velocity", "ttsh_set_advection_form", "ttsh_step",
            "ttsh_get_fields", "ttsh_state_elems", "ttsh_get_state", "ttsh_set_state", "ttsh_diagnostics",
            "ttsh_launch_count", "ttsh_run_stage", "ttsh_debug_get_real", "ttsh_destroy", "ttsh_strerror",
-           "ttsh_last_error", "ttsh_dumbbell_order", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
+           "ttsh_last_error", "ttsh_dumbbell_order", "ttsh_psd_workspace_bytes", "ttsh_psd_create",
+           "ttsh_psd_accumulate", "ttsh_psd_result", "ttsh_psd_reset", "ttsh_psd_destroy", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
            "ttsh_ensemble_destroy")
 
 
@@ -75,6 +76,12 @@ _sig = {
     "ttsh_strerror": (C.c_char_p, [_i]),
     "ttsh_last_error": (C.c_char_p, [_vp]),
     "ttsh_dumbbell_order": (_i, [_vp, _d, _d, _d, _d, _d, _vp]),
+    "ttsh_psd_workspace_bytes": (_sz, [_i, _i, _i, _i]),
+    "ttsh_psd_create": (_i, [C.POINTER(_vp), _vp, C.POINTER(_d), _i, _vp, _sz]),
+    "ttsh_psd_accumulate": (_i, [_vp]),
+    "ttsh_psd_result": (_i, [_vp, C.POINTER(_d), C.POINTER(_ll)]),
+    "ttsh_psd_reset": (_i, [_vp]),
+    "ttsh_psd_destroy": (_i, [_vp]),
     "ttsh_ensemble_create": (_i, [C.POINTER(_vp), C.POINTER(_vp), _i]),
     "ttsh_ensemble_step": (_i, [_vp, _i]),
     "ttsh_ensemble_launch_count": (_ll, [_vp]),
@@ -159,6 +166,37 @@ def ttsh_dumbbell_order(h, cx_left, cy_left, cx_right, cy_right, radius):
     d = ttsh_psi2()
     rc = _lib.ttsh_dumbbell_order(h, cx_left, cy_left, cx_right, cy_right, radius, C.byref(d))
     return rc, d
+
+
+def ttsh_psd_workspace_bytes(Nx, Ny, dtype, nfreq):
+    return int(_lib.ttsh_psd_workspace_bytes(Nx, Ny, dtype, nfreq))
+
+
+def ttsh_psd_create(h, omegas, workspace_ptr, workspace_bytes):
+    """Returns (status, psd handle).  omegas: sequence of angular frequencies (host)."""
+    s = _vp()
+    arr = (_d * max(1, len(omegas)))(*[float(o) for o in omegas])
+    rc = _lib.ttsh_psd_create(C.byref(s), h, arr, len(omegas), workspace_ptr or None, workspace_bytes)
+    return rc, s
+
+
+def ttsh_psd_accumulate(s):
+    return _lib.ttsh_psd_accumulate(s)
+
+
+def ttsh_psd_result(s, nfreq):
+    out = (_d * max(1, nfreq))()
+    n = _ll(0)
+    rc = _lib.ttsh_psd_result(s, out, C.byref(n))
+    return rc, [out[i] for i in range(nfreq)], int(n.value)
+
+
+def ttsh_psd_reset(s):
+    return _lib.ttsh_psd_reset(s)
+
+
+def ttsh_psd_destroy(s):
+    return _lib.ttsh_psd_destroy(s)
 
 
 def ttsh_launch_count(h):
@@ -311,6 +349,45 @@ class Solver:
             self.torch.cuda.synchronize(self.device)
             ttsh_destroy(self.h)
             self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class TemporalPSD:
+    """Streaming Eq. (5) on a Solver: accumulate() after every sampling interval, result() -> S(Omega_m)."""
+
+    def __init__(self, solver: Solver, omegas):
+        self.solver, self.omegas = solver, [float(o) for o in omegas]
+        torch = solver.torch
+        nbytes = ttsh_psd_workspace_bytes(solver.Nx, solver.Ny, solver.dtype_code, len(self.omegas))
+        if nbytes == 0:
+            raise TTSHError(TTSH_ERR_INVALID_ARG, "1 <= nfreq <= 1024")
+        with torch.cuda.device(solver.device), torch.cuda.stream(solver.stream):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=solver.device)
+            rc, self.s = ttsh_psd_create(solver.h, self.omegas, self.workspace.data_ptr(), nbytes)
+        if rc != TTSH_OK:
+            raise TTSHError(rc)
+
+    def accumulate(self):
+        self.solver._check(ttsh_psd_accumulate(self.s))
+
+    def result(self):
+        rc, S, n = ttsh_psd_result(self.s, len(self.omegas))
+        self.solver._check(rc)
+        return S, n
+
+    def reset(self):
+        self.solver._check(ttsh_psd_reset(self.s))
+
+    def close(self):
+        if getattr(self, "s", None):
+            self.solver.torch.cuda.synchronize(self.solver.device)
+            ttsh_psd_destroy(self.s)
+            self.s = None
 
     def __del__(self):
         try:

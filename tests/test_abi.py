@@ -96,3 +96,18 @@ def test_ensemble_create_rejects_bad_arguments_without_touching_cuda(ttsh):
     assert ttsh.ttsh_ensemble_step(None, 1) == ttsh.TTSH_ERR_INVALID_ARG
     assert ttsh.ttsh_ensemble_destroy(None) == ttsh.TTSH_OK
     assert ttsh.ttsh_ensemble_launch_count(None) == 0
+
+
+def test_psd_argument_validation_without_touching_cuda(ttsh):
+    assert ttsh.ttsh_psd_workspace_bytes(64, 64, ttsh.TTSH_F64, 0) == 0
+    assert ttsh.ttsh_psd_workspace_bytes(64, 64, ttsh.TTSH_F64, 1025) == 0
+    assert ttsh.ttsh_psd_workspace_bytes(96, 64, ttsh.TTSH_F64, 4) == 0
+    b64 = ttsh.ttsh_psd_workspace_bytes(256, 128, ttsh.TTSH_F64, 10)
+    b32 = ttsh.ttsh_psd_workspace_bytes(256, 128, ttsh.TTSH_F32, 10)
+    assert 10 * 256 * 128 * 16 <= b64 < 10 * 256 * 128 * 16 + (1 << 16) and 10 * 256 * 128 * 8 <= b32 < b64
+    assert ttsh.ttsh_psd_create(None, [0.1], 256, 1 << 20)[0] == ttsh.TTSH_ERR_INVALID_ARG     # NULL handle
+    assert ttsh.ttsh_psd_accumulate(None) == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_psd_result(None, 1)[0] == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_psd_reset(None) == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_psd_destroy(None) == ttsh.TTSH_OK
+    assert ttsh.ttsh_dumbbell_order(None, 0.0, 0.0, 1.0, 1.0, 1.0)[0] == ttsh.TTSH_ERR_INVALID_ARG

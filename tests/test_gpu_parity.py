@@ -428,3 +428,38 @@ def test_dumbbell_order_regions_ties_and_fp32(ttsh):
     assert ttsh.ttsh_dumbbell_order(s.h, 0.0, 0.0, 1.0, 1.0, -1.0)[0] == ttsh.TTSH_ERR_INVALID_ARG
     assert ttsh.ttsh_dumbbell_order(s.h, float("nan"), 0.0, 1.0, 1.0, 1.0)[0] == ttsh.TTSH_ERR_INVALID_ARG
     s.close()
+
+
+# ---------------------------------------------------------------- streaming temporal PSD, Eq. (5)
+@pytest.mark.parametrize("Nx,Ny,dtype,nfreq,tol", [(64, 64, "f64", 6, 1e-10), (256, 128, "f64", 70, 1e-10), (128, 64, "f32", 5, 2e-4)])
+def test_streaming_temporal_psd_matches_oracle(ttsh, Nx, Ny, dtype, nfreq, tol):
+    """ttsh_psd_* vs oracle.temporal_psd of the ORACLE's own vorticity series (sampled every 3 steps from an O(1) start,
+    where the field changes by O(1) over the window).  nfreq = 70 crosses the 64-frequency launch chunk."""
+    from oracle import temporal_psd
+    dx, dt, every, nsamp = 0.5, 0.01, 3, 10
+    mask = workloads.disk_mask(Nx, Ny, dx, 0.3 * min(Nx, Ny) * dx)
+    vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 3, amplitude=1.0)
+    s, o = make_pair(ttsh, Nx, Ny, dx, dt, "baseline", mask, dtype=dtype, vel=vel)
+    window = nsamp * every * dt
+    omegas = [0.0] + [2 * np.pi * m / window for m in range(1, nfreq - 1)] + [17.3]     # DFT frequencies and an odd one
+    psd = ttsh.TemporalPSD(s, omegas)
+    series, times = [], []
+    for _ in range(nsamp):
+        psd.accumulate()
+        series.append(o.get_fields()[2]); times.append(o.t)
+        s.step(every); o.step(every)
+    S, n = psd.result()
+    ref = temporal_psd(series, times, omegas)
+    assert n == nsamp and len(S) == nfreq
+    scale = ref.max()
+    assert scale > 0 and np.max(np.abs(np.asarray(S) - ref)) <= tol * scale, np.max(np.abs(np.asarray(S) - ref)) / scale
+    assert np.all(np.abs(np.asarray(S)[:3] - ref[:3]) <= 10 * tol * ref[:3])                # the strong low-frequency bins, relatively
+    # result() does not disturb the accumulators; reset() clears them
+    S2, _ = psd.result()
+    assert S2 == S
+    psd.reset()
+    psd.accumulate()
+    S3, n3 = psd.result()
+    w = o.get_fields()[2]
+    assert n3 == 1 and abs(S3[0] - np.mean(w * w)) <= max(tol, 1e-9) * 10 * np.mean(w * w)   # one sample: S = mean(w^2) at every frequency
+    psd.close(); s.close()

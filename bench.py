@@ -17,6 +17,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -299,6 +300,34 @@ def measure_ensemble(torch, ttsh, name, count, device, nsteps=200):
             "nonfinite": bad, "workload": f"{count} members of the {name} sweep, disk R = {lo:g}..{hi:g}, {dtype}, one ttsh_ensemble_step"}
 
 
+def measure_psd(torch, ttsh, name, nfreq, device, hbm_peak, reps=10):
+    """One ttsh_psd_accumulate = inverse transform of w^ + the streaming update of nfreq complex accumulators per grid point
+    (Eq. 5).  Algorithmic bytes of the update kernel: read w once, read + write nfreq accumulators."""
+    cfg, dtype = workload(name)
+    mask = cfg.mask()
+    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.baseline_params(), dtype, mask=mask, device=device)
+    s.set_velocity(*cfg.initial_velocity(mask))
+    psd = ttsh.TemporalPSD(s, [0.01 * m for m in range(nfreq)])
+    stream = torch.cuda.current_stream(device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(3):
+        psd.accumulate()
+    torch.cuda.synchronize(device)
+    e0.record(stream)
+    for _ in range(reps):
+        psd.accumulate()
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    ms = e0.elapsed_time(e1) / reps
+    w = 8 if dtype == "f64" else 4
+    nbytes = cfg.Nx * cfg.Ny * (w + nfreq * 2 * 2 * w)
+    S, n = psd.result()
+    psd.close(); s.close()
+    return {"ms_per_accumulate": ms, "algorithmic_bytes": nbytes, "GBps_incl_inverse_transform": nbytes / (ms * 1e-3) / 1e9,
+            "frac_of_hbm_peak": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "samples": n, "finite": bool(all(math.isfinite(x) for x in S)),
+            "workload": f"{name} {dtype}, {nfreq} frequencies: {nfreq * 2 * w * cfg.Nx * cfg.Ny / 2**20:.0f} MiB of accumulators (> L2)"}
+
+
 def reduce_over_ranks(dist, maxima, sums, device="cpu"):
     """Replicas only: the job time is the MAX over ranks, counts are SUMMED.  No data-path collective."""
     if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
@@ -446,6 +475,7 @@ def main():
         # kernel per Euler step for all members
         for name, count in (("C1", 256), ("C2", 64), ("C3", 16), ("C3-f32", 16)):
             extra[f"{name} x{count} ensemble"] = measure_ensemble(torch, ttsh, name, count, device)
+        extra["C3 temporal PSD, 64 frequencies"] = measure_psd(torch, ttsh, "C3", 64, device, peak)
         line["other_workloads"] = extra
 
     if not a.no_cpu_baseline and world == 1:

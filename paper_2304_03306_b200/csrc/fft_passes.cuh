@@ -59,7 +59,9 @@ template <typename T, int NY> struct ColCfg {
   static constexpr int L = col_tile_width(NY, (int)sizeof(cplx<T>));
   static constexpr int LSHIFT = L == 2 ? 1 : (L == 4 ? 2 : 3);
   static constexpr int THREADS = L * TPL;
-  static constexpr int LS = fft_line_elems<NH>() + 8 / L;
+  // line stride: a 128-byte wavefront holds W = 128 / sizeof(cplx<T>) elements and is filled by W threads = W/L consecutive
+  // butterflies x L lines (col_thread_map), so the lines must start W/L elements apart modulo W to land in distinct banks
+  static constexpr int LS = fft_line_elems<NH>() + (128 / (int)sizeof(cplx<T>)) / L;
   static constexpr size_t SMEM = (size_t)L * LS * sizeof(cplx<T>);
   static constexpr int MINB = (THREADS <= 256 || sizeof(T) == 4) ? 2 : 1;    // fp32: 512 threads x 64 registers
 };

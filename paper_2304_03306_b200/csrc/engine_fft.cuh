@@ -12,23 +12,47 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
 }
 
 #ifdef TTSH_BUILD_COLS
+// the grouped variant is used when it still leaves at least one 128-thread CTA per SM
+static int col_fill_ctas() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    n = sms > 0 ? sms : 148;
+  }
+  return n;
+}
 template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s,
                                                             int members, size_t mstride) {
   using C = ColCfg<T, NY>;
-  dim3 grid(2, g.NT, nf * members);
-  k_inv_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0, nf, mstride);
+  const long long items = (long long)g.NT * nf * members;
+  constexpr int G = C::GMAX;
+  if (G > 1 && 2 * items >= (long long)G * col_fill_ctas()) {          // several items per CTA once that still fills the GPU
+    const long long ctas = (items + G - 1) / G;
+    if (ctas > 65535) return cudaErrorInvalidValue;
+    k_inv_col<T, NY, G><<<dim3(2, (unsigned)ctas), G * C::THREADS, G * C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0, nf, members, mstride);
+    return cudaGetLastError();
+  }
+  if (items > 65535) return cudaErrorInvalidValue;
+  k_inv_col<T, NY, 1><<<dim3(2, (unsigned)items), C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0, nf, members, mstride);
   return cudaGetLastError();
 }
 template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s,
                                                             int members, size_t mstride) {
   using C = ColCfg<T, NY>;
-  dim3 grid(g.NT, nf * members);
-  k_fwd_col<T, NY><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), nf, mstride);
+  const long long items = (long long)g.NT * nf * members;
+  constexpr int G = C::GMAX;
+  if (items > 0x3fffffffLL) return cudaErrorInvalidValue;
+  if (G > 1 && items >= (long long)G * col_fill_ctas()) {
+    k_fwd_col<T, NY, G><<<(unsigned)((items + G - 1) / G), G * C::THREADS, G * C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), nf, members, mstride);
+    return cudaGetLastError();
+  }
+  k_fwd_col<T, NY, 1><<<(unsigned)items, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), nf, members, mstride);
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s,
                                                  int members, size_t mstride) {
-  if (nf * members > 65535) return cudaErrorInvalidValue;
   switch (g.Ny) {
 #define X(N) case N: return go_inv_col<T, N>(g, b, nf, tab, tabS, v0, s, members, mstride);
     TTSH_FOR_SIZES(X)
@@ -38,7 +62,6 @@ template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, 
 }
 template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s,
                                                  int members, size_t mstride) {
-  if (nf * members > 65535) return cudaErrorInvalidValue;
   switch (g.Ny) {
 #define X(N) case N: return go_fwd_col<T, N>(g, b, nf, tab, tabS, s, members, mstride);
     TTSH_FOR_SIZES(X)
@@ -48,8 +71,11 @@ template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, 
 }
 template <typename T> cudaError_t prepare_cols(const Geom& g) {
   switch (g.Ny) {
-#define X(N) case N: { cudaError_t e = set_smem(k_inv_col<T, N>, ColCfg<T, N>::SMEM); if (e != cudaSuccess) return e; \
-                       return set_smem(k_fwd_col<T, N>, ColCfg<T, N>::SMEM); }
+#define X(N) case N: { using C = ColCfg<T, N>; \
+                       cudaError_t e = set_smem(k_inv_col<T, N, 1>, C::SMEM); if (e != cudaSuccess) return e; \
+                       e = set_smem(k_inv_col<T, N, C::GMAX>, C::GMAX * C::SMEM); if (e != cudaSuccess) return e; \
+                       e = set_smem(k_fwd_col<T, N, C::GMAX>, C::GMAX * C::SMEM); if (e != cudaSuccess) return e; \
+                       return set_smem(k_fwd_col<T, N, 1>, C::SMEM); }
     TTSH_FOR_SIZES(X)
 #undef X
   }

@@ -64,6 +64,10 @@ template <typename T, int NY> struct ColCfg {
   static constexpr int LS = fft_line_elems<NH>() + (128 / (int)sizeof(cplx<T>)) / L;
   static constexpr size_t SMEM = (size_t)L * LS * sizeof(cplx<T>);
   static constexpr int MINB = (THREADS <= 256 || sizeof(T) == 4) ? 2 : 1;    // fp32: 512 threads x 64 registers
+  // small Ny: a transform has few threads (Ny = 64: 8), so a CTA of the kernels' G > 1 variant runs G independent work items
+  // (tile x field x member) side by side, each with its own line buffers (ensembles; a single small system keeps G = 1:
+  // more, smaller CTAs spread over more SMs)
+  static constexpr int GMAX = THREADS >= 128 ? 1 : 128 / THREADS;   // used when the launch has enough items to fill the GPU anyway
 };
 
 // 2-element (A, B) pair access of the row passes
@@ -127,22 +131,28 @@ template <int LSHIFT> __device__ __forceinline__ void col_thread_map(int e, int&
 // 64 KB spectrum tile - adjacent in launch order, so the second read hits L2; splitting them doubles the number of CTAs
 // and halves the tail of the last wave)
 // ---------------------------------------------------------------------------------------
-template <typename T, int NY>
-__global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
+template <typename T, int NY, int G>
+__global__ void __launch_bounds__(G * ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
 k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
-          const cplx<T>* __restrict__ tabS, const double* __restrict__ v0_, int nf, size_t mstride) {
+          const cplx<T>* __restrict__ tabS, const double* __restrict__ v0_, int nf, int nmembers, size_t mstride) {
   using C = ColCfg<T, NY>;
   constexpr int NH = C::NH, L = C::L, TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+  // grid = (2 parities, ceil(items / G)); item = tile + NT * (field + nf * member), G items per CTA
+  const int sub = G == 1 ? 0 : (int)threadIdx.x / C::THREADS, tid = G == 1 ? (int)threadIdx.x : (int)threadIdx.x % C::THREADS;
   int j, c;
-  col_thread_map<C::LSHIFT>(threadIdx.x, j, c);
-  const int t = blockIdx.y;
+  col_thread_map<C::LSHIFT>(tid, j, c);
+  const int nitems = g.NT * nf * nmembers;
+  int item = blockIdx.y * G + sub;
+  const bool live = G == 1 || item < nitems;   // an idle group of the last CTA still takes part in the barriers
+  if (!live) item = nitems - 1;
+  const int t = item % g.NT, zf = item / g.NT;
   const int mx = t * L + c;
-  const bool valid = mx < g.Wx;
-  const int member = blockIdx.z / nf;             // grid.z = ensemble members x fields (member 0 only outside ensembles)
+  const bool valid = live && mx < g.Wx;
+  const int member = zf / nf;                      // member 0 only outside ensembles
   const size_t moff = (size_t)member * mstride;    // bytes
-  FieldOp op = batch.f[blockIdx.z - member * nf];
+  FieldOp op = batch.f[zf - member * nf];
   op.src = static_cast<const char*>(op.src) + moff;
   op.dst = static_cast<char*>(op.dst) + moff;
   const double* __restrict__ v0 = reinterpret_cast<const double*>(reinterpret_cast<const char*>(v0_) + moff);
@@ -154,16 +164,17 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const size_t slot_stride = (size_t)TPL * g.Wxp * 2;
   const int mode = op.mode;
   const T scale = (T)g.inv_sqrt_ny;
-  cplx<T>* line = sm + c * C::LS;
+  cplx<T>* line = sm + (sub * L + c) * C::LS;
 
   const bool half_rule = (2 * My == NH);     // the paper's 1/2 rule: |my| <= Ny/4 (uniform branch)
   const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
-  if (threadIdx.x == 0 && blockIdx.x == 0) {  // L2 prefetch of the spectrum tile the CTAs about one wave later read
-    int nt = blockIdx.y + TTSH_PF_DIST_COL, nz = blockIdx.z;
-    if (nt >= (int)gridDim.y) { nt -= gridDim.y; nz += 1; }
-    if (nz < (int)gridDim.z)
+  if (G == 1 && threadIdx.x == 0 && blockIdx.x == 0) {  // L2 prefetch of the spectrum tile the CTAs about one wave later read
+    const int ni = item + TTSH_PF_DIST_COL;
+    if (ni < nitems) {
+      const int nt = ni % g.NT, nz = ni / g.NT;
       prefetch_l2_bulk(reinterpret_cast<const cplx<T>*>(static_cast<const char*>(batch.f[nz % nf].src) + (size_t)(nz / nf) * mstride) +
                            (size_t)nt * Hy * L, (unsigned)(Hy * L * sizeof(cplx<T>)));
+    }
   }
 
   {
@@ -172,7 +183,7 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     // NH-mp <= My.
     // tail columns of the last tile are written too (zeros inside the row pitch), the row pass never reads them
     cplx<T>* out = dst + (size_t)p * g.Wxp * 2;
-    auto store = [&](int, int k, cplx<T> val) { out[(size_t)k * slot_stride] = val; };
+    auto store = [&](int, int k, cplx<T> val) { if (live) out[(size_t)k * slot_stride] = val; };
     // * W_Ny^{-mp} (inverse sign) for the odd rows; mp = j + k TPL, so W_Ny^{mp} = W_Ny^j W_32^k: one table load per thread
     auto twist = [&](int k, cplx<T> a) -> cplx<T> {
       if (p) a = mul_w32_rt<+1>(mul_conj(a, wj), k);
@@ -219,28 +230,34 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 // ---------------------------------------------------------------------------------------
 // forward column pass.  grid = (NT tiles, fields)
 // ---------------------------------------------------------------------------------------
-template <typename T, int NY>
-__global__ void __launch_bounds__(ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
+template <typename T, int NY, int G>
+__global__ void __launch_bounds__(G * ColCfg<T, NY>::THREADS, ColCfg<T, NY>::MINB)
 k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabY,
-          const cplx<T>* __restrict__ tabS, int nf, size_t mstride) {
+          const cplx<T>* __restrict__ tabS, int nf, int nmembers, size_t mstride) {
   using C = ColCfg<T, NY>;
   constexpr int NH = C::NH, L = C::L, TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+  // grid = ceil(items / G); item = tile + NT * (field + nf * member), G items per CTA
+  const int sub = G == 1 ? 0 : (int)threadIdx.x / C::THREADS, tid = G == 1 ? (int)threadIdx.x : (int)threadIdx.x % C::THREADS;
   int j, c;
-  col_thread_map<C::LSHIFT>(threadIdx.x, j, c);
-  const int t = blockIdx.x;
-  const bool valid = t * L + c < g.Wx;
-  const int member = blockIdx.y / nf;             // grid.y = ensemble members x fields
+  col_thread_map<C::LSHIFT>(tid, j, c);
+  const int nitems = g.NT * nf * nmembers;
+  int item = blockIdx.x * G + sub;
+  const bool live = G == 1 || item < nitems;
+  if (!live) item = nitems - 1;
+  const int t = item % g.NT, zf = item / g.NT;
+  const bool valid = live && t * L + c < g.Wx;
+  const int member = zf / nf;
   const size_t moff = (size_t)member * mstride;
-  FieldOp op = batch.f[blockIdx.y - member * nf];
+  FieldOp op = batch.f[zf - member * nf];
   op.src = static_cast<const char*>(op.src) + moff;
   op.dst = static_cast<char*>(op.dst) + moff;
   const int My = g.My, Hy = g.Hy;
-  const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * 2 * NH * L + threadIdx.x;
+  const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src) + (size_t)t * 2 * NH * L + tid;
   cplx<T>* dst = static_cast<cplx<T>*>(op.dst) + (size_t)t * Hy * L + c;
   const T scale = (T)g.inv_sqrt_ny;
-  cplx<T>* line = sm + c * C::LS;
+  cplx<T>* line = sm + (sub * L + c) * C::LS;
   const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
 
   const bool half_rule = (2 * My == NH);

@@ -497,3 +497,83 @@ def test_temporal_psd_closed_forms_and_library_special_case():
     ref = abs(sum((np.sin(0.9 * t) + 0.3) * np.exp(-1j * Om * t) for t in times)) ** 2
     assert abs(temporal_psd(one, times, [Om])[0] - ref) < 1e-12 * ref
 
+
+
+# ---------------------------------------------------------------- tangent-linear step and QR growth rates
+def _o1_state(Nx, Ny, dx, seed, amp=1.0):
+    return workloads.planewave_velocity(Nx, Ny, dx, seed, amplitude=amp, nmodes=10)
+
+
+def test_tangent_step_is_the_derivative_of_the_nonlinear_step():
+    """Central finite differences of the NONLINEAR oracle (which the tangent code does not call for its arithmetic):
+    (Phi^n(s + eps d) - Phi^n(s - eps d)) / 2 eps = J_n d + O(eps^2).  O(1) base state inside a disk, so that the cubic,
+    advection and both damping terms all contribute; n = 1 and n = 3 (composition along the moving base state)."""
+    from oracle.tangent import TangentOracle
+    Nx, Ny, dx, dt = 32, 64, 0.5, 0.01
+    mask = workloads.disk_mask(Nx, Ny, dx, 6.0)
+    v0 = _o1_state(Nx, Ny, dx, 11)
+    d0 = _o1_state(Nx, Ny, dx, 12, amp=0.7)
+    d0 = (d0[0] + 0.3, d0[1] - 0.2)                       # with a mean-flow component (line 8 of Algorithm 1)
+    eps = 1e-5
+    for n in (1, 3):
+        plus = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET, mask=mask)
+        minus = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET, mask=mask)
+        plus.set_velocity(v0[0] + eps * d0[0], v0[1] + eps * d0[1]); plus.step(n)
+        minus.set_velocity(v0[0] - eps * d0[0], v0[1] - eps * d0[1]); minus.step(n)
+        fd = [(a - b) / (2 * eps) for a, b in zip(plus.get_fields()[:3], minus.get_fields()[:3])]
+        base = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET, mask=mask)
+        base.set_velocity(*v0)
+        tan = TangentOracle(base, 1)
+        tan.set(0, *d0)
+        tan.step(n)
+        got = tan.get_fields(0)
+        for f, g in zip(fd, got):
+            assert np.linalg.norm(f - g) <= 1e-8 * np.linalg.norm(f), np.linalg.norm(f - g) / np.linalg.norm(f)
+        assert base.nstep == n                              # the tangent step advances the base trajectory too
+    # a dropped term must be visible at this tolerance: the advection part alone is far larger than 1e-8
+    assert BASELINE_PRESET.lambda0 * dt > 1e-3
+
+
+def test_tangent_about_the_zero_state_is_the_linear_operator():
+    """Base state 0, no mask: the Jacobian is exp(sigma(k) dt) per mode (Alg. 1 line 4), so a single-mode perturbation
+    grows by exactly exp(sigma(k) n dt) and its growth rate from the QR diagonal is sigma(k)."""
+    from oracle.tangent import TangentOracle
+    Nx = Ny = 32
+    dx, dt, n = 0.5, 0.01, 7
+    base = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET)
+    z = np.zeros((Ny, Nx))
+    base.set_velocity(z, z)
+    x = np.arange(Nx)[None, :] * dx
+    y = np.arange(Ny)[:, None] * dx
+    kx, ky = 2 * np.pi * 2 / (Nx * dx), 2 * np.pi * 1 / (Ny * dx)          # retained mode (2, 1)
+    ph = kx * x + ky * y
+    dvx, dvy = ky * np.cos(ph), -kx * np.cos(ph)                            # divergence-free single mode
+    tan = TangentOracle(base, 2)
+    tan.set(0, dvx, dvy)
+    tan.set(1, np.ones((Ny, Nx)), z)                                        # pure mean flow: grows by exp(-alpha dt)
+    tan.orthonormalize()
+    tan.step(n)
+    logr = tan.orthonormalize()
+    k2 = kx * kx + ky * ky
+    p = BASELINE_PRESET
+    sigma = -p.alpha - p.Gamma0 * k2 - p.Gamma2 * k2 * k2
+    assert abs(logr[0] / (n * dt) - sigma) < 1e-10
+    assert abs(logr[1] / (n * dt) - (-p.alpha)) < 1e-10
+
+
+def test_tangent_qr_orthonormalises_and_measures_the_volume():
+    from oracle.tangent import TangentOracle
+    Nx, Ny, dx, dt = 32, 32, 0.5, 0.01
+    mask = workloads.disk_mask(Nx, Ny, dx, 5.0)
+    base = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET, mask=mask)
+    base.set_velocity(*_o1_state(Nx, Ny, dx, 21))
+    tan = TangentOracle(base, 3)
+    for i in range(3):
+        tan.set(i, *_o1_state(Nx, Ny, dx, 30 + i))
+    A = tan.as_matrix()
+    logr = tan.orthonormalize()
+    sign, logdet = np.linalg.slogdet(A.T @ A)
+    assert sign > 0 and abs(2 * logr.sum() - logdet) < 1e-9                 # prod R_ii^2 = det(Gram)
+    Q = tan.as_matrix()
+    assert np.allclose(Q.T @ Q, np.eye(3), atol=1e-12)                      # and the stored states reproduce Q
+    assert np.allclose(tan.orthonormalize(), 0.0, atol=1e-12)               # idempotent: R = I

@@ -153,6 +153,29 @@ int ttsh_psd_result(ttsh_psd* s, double* S_host, long long* nsamples_host);     
 int ttsh_psd_reset(ttsh_psd* s);
 int ttsh_psd_destroy(ttsh_psd* s);
 
+/* Tangent-linear evolution and growth rates (Lyapunov exponents): nvec independent perturbations
+ * (dw^, dv^(0)) of the state are carried along the trajectory by the Jacobian of Algorithm 1 at the current state (lines 1-2
+ * differentiated, everything else is linear), and re-orthonormalised on request by a QR decomposition (modified Gram-Schmidt
+ * on the device) whose diagonal gives the growth: lambda_i = sum log R_ii / elapsed time.  The inner product is the Euclidean
+ * one of the real vectors [dw(x) for all x ; dv^_x(0) ; dv^_y(0)] (unitary DFT normalisation of the mean flow).
+ * workspace: DEVICE, >= ttsh_tangent_workspace_bytes, 256-byte aligned, owned by the caller.  1 <= nvec <= 64.  Requires
+ * TTSH_ADVECTION_CONSERVATIVE.  The tangent object borrows the handle: destroy it first. */
+typedef struct ttsh_tangent ttsh_tangent;
+size_t ttsh_tangent_workspace_bytes(int Nx, int Ny, ttsh_dtype t, int nvec);     /* 0 if unsupported */
+int ttsh_tangent_create(ttsh_tangent** out, ttsh_handle* h, int nvec, void* workspace, size_t workspace_bytes);
+/* Sets perturbation i from a real velocity perturbation (DEVICE scalar[Ny*Nx] each) through the same (linear) projection
+ * as ttsh_set_velocity. */
+int ttsh_tangent_set(ttsh_tangent* s, int i, const void* dvx, const void* dvy);
+/* n times: every perturbation through the Jacobian at the handle's current state, then one step of the handle itself
+ * (so the handle advances by n steps).  Asynchronous.  TTSH_ERR_NOT_INITIALIZED unless the handle and all vectors are set. */
+int ttsh_tangent_step(ttsh_tangent* s, int n);
+/* QR of the current vectors: they are replaced by the orthonormal Q (R_ii > 0), log_r_host[i] = log R_ii (HOST double[nvec]).
+ * Synchronises. */
+int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host);
+/* dv = (dvx, dvy) and dw of perturbation i into DEVICE scalar[Ny*Nx] buffers; any pointer may be NULL. */
+int ttsh_tangent_get_fields(ttsh_tangent* s, int i, void* dvx, void* dvy, void* domega);
+int ttsh_tangent_destroy(ttsh_tangent* s);
+
 /* Ensembles: the paper's workload is sweeps of independent runs on one grid — disk radius R (Fig. 2), the
  * hysteresis branches, dumbbell separations — and on grids up to about 1024^2 one system
  * cannot fill a B200.  An ensemble advances `count` independent handles with ONE launch of each hot kernel per Euler step

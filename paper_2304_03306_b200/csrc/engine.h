@@ -66,4 +66,12 @@ template <typename T> cudaError_t launch_psd_accumulate(size_t n, int nf, const 
 template <typename T> cudaError_t launch_psd_power(size_t n, int nf, const void* acc, double* partial, double* out, cudaStream_t s);
 int psd_blocks();
 
+// tangent-linear step and Gram-Schmidt on tangent vectors (pointwise.cuh)
+template <typename T> cudaError_t launch_realspace_tangent(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
+                                                           const void* K, void* dvx, void* dvy, void* dw, cudaStream_t s);
+template <typename T> cudaError_t launch_spec_dot(const Geom& g, const void* a, const void* b, const double* a0, const double* b0,
+                                                  int norm_slot, double* partial, double* rdiag, double* coef, cudaStream_t s);
+template <typename T> cudaError_t launch_spec_scale_axpy(const Geom& g, const double* coef, const void* x, void* y, const double* x0,
+                                                         double* y0, cudaStream_t s);
+
 }  // namespace ttsh

@@ -105,7 +105,34 @@ template <typename T> cudaError_t launch_psd_power(size_t n, int nf, const void*
 }
 int psd_blocks() { return PSD_BLOCKS; }
 
+template <typename T> cudaError_t launch_realspace_tangent(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
+                                                           const void* K, void* dvx, void* dvy, void* dw, cudaStream_t s) {
+  const size_t nvec = (size_t)g.Nx * g.Ny / Vec<T>::n;
+  k_realspace_tangent<T><<<blocks_for(nvec, 256, GRID_CAP), 256, 0, s>>>(nvec, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K,
+                                                                           (T*)dvx, (T*)dvy, (T*)dw);
+  return cudaGetLastError();
+}
+// coef[0] <- <a, b> (norm_slot < 0) or rdiag[norm_slot] <- |a|, coef[0] <- 1/|a|; partial: DIAG_BLOCKS doubles
+template <typename T> cudaError_t launch_spec_dot(const Geom& g, const void* a, const void* b, const double* a0, const double* b0,
+                                                  int norm_slot, double* partial, double* rdiag, double* coef, cudaStream_t s) {
+  k_spec_dot_partial<T><<<DIAG_BLOCKS, 256, 0, s>>>(g, (const cplx<T>*)a, (const cplx<T>*)b, partial);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_spec_dot_final<<<1, 32, 0, s>>>(DIAG_BLOCKS, partial, a0, b0, norm_slot, rdiag, coef);
+  return cudaGetLastError();
+}
+// y <- coef y (x == NULL) or y <- y - coef x, on the spectrum and the mean flow
+template <typename T> cudaError_t launch_spec_scale_axpy(const Geom& g, const double* coef, const void* x, void* y, const double* x0,
+                                                         double* y0, cudaStream_t s) {
+  const size_t n = (size_t)g.NT * g.Hy * g.CW;
+  k_spec_scale_axpy<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, coef, (const cplx<T>*)x, (cplx<T>*)y, x0, y0);
+  return cudaGetLastError();
+}
+
 #define INST(T) \
+  template cudaError_t launch_realspace_tangent<T>(const Geom&, const Model&, const void*, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
+  template cudaError_t launch_spec_dot<T>(const Geom&, const void*, const void*, const double*, const double*, int, double*, double*, double*, cudaStream_t); \
+  template cudaError_t launch_spec_scale_axpy<T>(const Geom&, const double*, const void*, void*, const double*, double*, cudaStream_t); \
   template cudaError_t launch_psd_accumulate<T>(size_t, int, const double*, const double*, const void*, void*, cudaStream_t); \
   template cudaError_t launch_psd_power<T>(size_t, int, const void*, double*, double*, cudaStream_t); \
   template cudaError_t launch_region_argmax<T>(const Geom&, double, double, double, double, double, double, const void*, double*, double*, cudaStream_t); \

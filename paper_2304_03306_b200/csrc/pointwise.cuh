@@ -517,4 +517,102 @@ __global__ void __launch_bounds__(32) k_psd_power_final(int nblocks, const doubl
   if (threadIdx.x == 0) out[blockIdx.x] = sum;
 }
 
+// ---------------------------------------------------------------------------------------
+// tangent-linear step (Lyapunov exponents): derivative of lines 1-2 of Algorithm 1 in the conservative
+// form of k_realspace_cons at the base state (u, v, w), applied to a perturbation (du, dv, dw); in place:
+//   c = -beta (u^2 + v^2) - gamma_v K,   dc = -2 beta (u du + v dv)
+//   du <- dGx = dc u + c du + lambda0 (dv w + v dw),   dv <- dGy = dc v + c dv - lambda0 (du w + u dw),   dw <- -gamma_w K dw
+// ---------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_realspace_tangent(size_t nvec, Model m, const T* __restrict__ vx, const T* __restrict__ vy, const T* __restrict__ w,
+                    const T* __restrict__ K, T* __restrict__ dvx, T* __restrict__ dvy, T* __restrict__ dw) {
+  using V = typename Vec<T>::type;
+  constexpr int n = Vec<T>::n;
+  const T beta = (T)m.beta, gv = (T)m.gamma_v, gw = (T)m.gamma_w, lam = (T)m.lambda0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    V a = reinterpret_cast<const V*>(vx)[i], b = reinterpret_cast<const V*>(vy)[i], ww = reinterpret_cast<const V*>(w)[i];
+    V k = reinterpret_cast<const V*>(K)[i];
+    V da = reinterpret_cast<V*>(dvx)[i], db = reinterpret_cast<V*>(dvy)[i], dww = reinterpret_cast<V*>(dw)[i];
+    T* pa = reinterpret_cast<T*>(&a); T* pb = reinterpret_cast<T*>(&b); T* pw = reinterpret_cast<T*>(&ww); T* pk = reinterpret_cast<T*>(&k);
+    T* pda = reinterpret_cast<T*>(&da); T* pdb = reinterpret_cast<T*>(&db); T* pdw = reinterpret_cast<T*>(&dww);
+#pragma unroll
+    for (int e = 0; e < n; ++e) {
+      const T u = pa[e], v = pb[e], om = pw[e], kk = pk[e], du = pda[e], dv = pdb[e], dom = pdw[e];
+      const T c = -beta * (u * u + v * v) - gv * kk;
+      const T dc = (T)-2 * beta * (u * du + v * dv);
+      pda[e] = dc * u + c * du + lam * (dv * om + v * dom);
+      pdb[e] = dc * v + c * dv - lam * (du * om + u * dom);
+      pdw[e] = -gw * kk * dom;
+    }
+    reinterpret_cast<V*>(dvx)[i] = da;
+    reinterpret_cast<V*>(dvy)[i] = db;
+    reinterpret_cast<V*>(dw)[i] = dww;
+  }
+}
+
+// Gram-Schmidt on tangent vectors (a^, a0) = (pruned tile-major half spectrum, mean flow[2]).  Inner product = the Euclidean
+// one of the real vectors [a(x) ; a0] = sum over the FULL spectrum of Re(a^ conj b^) + a0 . b0 (unitary DFT): stored entries
+// of the column mx = 0 count once (both +-my are stored), mx > 0 twice (their conjugates are implicit).
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_spec_dot_partial(Geom g, const cplx<T>* __restrict__ a, const cplx<T>* __restrict__ b, double* __restrict__ partial) {
+  const size_t n = (size_t)g.NT * g.Hy * g.CW;
+  double sum = 0.0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const int t = (int)(i / ((size_t)g.Hy * g.CW));
+    const int mx = t * g.CW + (int)(i & (size_t)(g.CW - 1));
+    if (mx >= g.Wx) continue;
+    const double re = (double)a[i].x * (double)b[i].x + (double)a[i].y * (double)b[i].y;
+    sum += mx == 0 ? re : 2.0 * re;
+  }
+  __shared__ double sh[32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+  if (lane == 0) sh[wid] = sum;
+  __syncthreads();
+  if (wid == 0) {
+    sum = lane < (int)(blockDim.x >> 5) ? sh[lane] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+    if (lane == 0) partial[blockIdx.x] = sum;
+  }
+}
+// one warp: total = sum partial + a0 . b0.  norm_slot >= 0: rdiag[norm_slot] = sqrt(total), coef[0] = 1 / sqrt(total)
+// (0 if total == 0); else coef[0] = total.
+__global__ void __launch_bounds__(32)
+k_spec_dot_final(int nblocks, const double* __restrict__ partial, const double* __restrict__ a0, const double* __restrict__ b0,
+                 int norm_slot, double* __restrict__ rdiag, double* __restrict__ coef) {
+  double sum = 0.0;
+  for (int b = threadIdx.x; b < nblocks; b += 32) sum += partial[b];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+  if (threadIdx.x == 0) {
+    sum += a0[0] * b0[0] + a0[1] * b0[1];
+    if (norm_slot >= 0) {
+      const double r = sqrt(sum);
+      rdiag[norm_slot] = r;
+      coef[0] = r > 0.0 ? 1.0 / r : 0.0;
+    } else coef[0] = sum;
+  }
+}
+// scale: y <- coef y (x == nullptr);  axpy: y <- y - coef x.  coef is read from device memory (no host round trip in the QR).
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_spec_scale_axpy(size_t n, const double* __restrict__ coef, const cplx<T>* __restrict__ x, cplx<T>* __restrict__ y,
+                  const double* __restrict__ x0, double* __restrict__ y0) {
+  const T c = (T)coef[0];
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    cplx<T> v = y[i];
+    if (x) { const cplx<T> u = x[i]; v.x -= c * u.x; v.y -= c * u.y; }
+    else { v.x *= c; v.y *= c; }
+    y[i] = v;
+  }
+  if (blockIdx.x == 0 && threadIdx.x < 2) {
+    const double cd = coef[0];
+    y0[threadIdx.x] = x0 ? y0[threadIdx.x] - cd * x0[threadIdx.x] : cd * y0[threadIdx.x];
+  }
+}
+
 }  // namespace ttsh

@@ -106,6 +106,16 @@ struct ttsh_psd {
   long long nsamples;
 };
 
+struct ttsh_tangent {
+  ttsh_handle* h;                      // borrowed
+  int nvec;
+  std::vector<void*> what, psihat;     // per vector: dw^, dpsi^ (pruned tile-major spectra in the caller's workspace)
+  std::vector<double*> v0;             // per vector: dv^(0)
+  std::vector<bool> set;
+  void* real[3];                       // dw, dv_x, dv_y of the vector being stepped (permuted internal row layout)
+  double *partial, *coef, *rdiag;
+};
+
 struct ttsh_ensemble {
   std::vector<ttsh_handle*> members;   // borrowed
   size_t mstride;                      // bytes between consecutive members' workspaces
@@ -672,6 +682,151 @@ int ttsh_psd_reset(ttsh_psd* s) {
   return TTSH_OK;
 }
 int ttsh_psd_destroy(ttsh_psd* s) {
+  delete s;
+  return TTSH_OK;
+}
+
+// ---- tangent-linear evolution and QR growth rates -----------------------------------------
+struct TanLayout { size_t vec, vec_stride, real[3], partial, coef, rdiag, total; };
+static TanLayout tan_layout(int Nx, int Ny, size_t w, int nvec) {
+  const Geom g = make_geom(Nx, Ny, 1.0, 2, 3, w);
+  const size_t spec = (size_t)g.NT * g.CW * g.Hy * 2 * w, P = (size_t)Nx * Ny;
+  TanLayout L;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+  L.vec_stride = 2 * align_up(spec) + align_up(8 * sizeof(double));       // dw^, dpsi^, dv^(0)
+  L.vec = take(L.vec_stride * nvec);
+  for (int i = 0; i < 3; ++i) L.real[i] = take(P * w);
+  L.partial = take((size_t)DIAG_BLOCKS * sizeof(double));
+  L.coef = take(8 * sizeof(double));
+  L.rdiag = take((size_t)nvec * sizeof(double));
+  L.total = off;
+  return L;
+}
+size_t ttsh_tangent_workspace_bytes(int Nx, int Ny, ttsh_dtype t, int nvec) {
+  if (!pow2_in_range(Nx) || !pow2_in_range(Ny) || (t != TTSH_F64 && t != TTSH_F32) || nvec < 1 || nvec > 64) return 0;
+  return tan_layout(Nx, Ny, (size_t)t, nvec).total;
+}
+int ttsh_tangent_create(ttsh_tangent** out, ttsh_handle* h, int nvec, void* workspace, size_t workspace_bytes) {
+  if (!out) return TTSH_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!h || !workspace || nvec < 1 || nvec > 64) return TTSH_ERR_INVALID_ARG;
+  if (reinterpret_cast<uintptr_t>(workspace) % ALIGN) return TTSH_ERR_INVALID_ARG;
+  if (h->sticky) return h->sticky;
+  if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
+  const TanLayout L = tan_layout(h->Nx, h->Ny, (size_t)h->dtype, nvec);
+  if (workspace_bytes < L.total) return TTSH_ERR_WORKSPACE_TOO_SMALL;
+  ttsh_tangent* s = new (std::nothrow) ttsh_tangent();
+  if (!s) return TTSH_ERR_INVALID_ARG;
+  char* ws = static_cast<char*>(workspace);
+  s->h = h;
+  s->nvec = nvec;
+  s->what.resize(nvec); s->psihat.resize(nvec); s->v0.resize(nvec);
+  s->set.assign(nvec, false);
+  const size_t spec_max = (L.vec_stride - align_up(8 * sizeof(double))) / 2;    // bytes of one spectrum slot
+  for (int i = 0; i < nvec; ++i) {
+    char* base = ws + L.vec + (size_t)i * L.vec_stride;
+    s->what[i] = base;
+    s->psihat[i] = base + spec_max;
+    s->v0[i] = reinterpret_cast<double*>(base + 2 * spec_max);
+  }
+  for (int i = 0; i < 3; ++i) s->real[i] = ws + L.real[i];
+  s->partial = reinterpret_cast<double*>(ws + L.partial);
+  s->coef = reinterpret_cast<double*>(ws + L.coef);
+  s->rdiag = reinterpret_cast<double*>(ws + L.rdiag);
+  *out = s;
+  TRY(h, cudaMemsetAsync(ws + L.vec, 0, L.vec_stride * nvec, h->stream));
+  return TTSH_OK;
+}
+int ttsh_tangent_set(ttsh_tangent* s, int i, const void* dvx, const void* dvy) {
+  if (!s || i < 0 || i >= s->nvec || !dvx || !dvy) return TTSH_ERR_INVALID_ARG;
+  ttsh_handle* h = s->h;
+  if (h->sticky) return h->sticky;
+  const void* src[2] = {dvx, dvy};
+  int rc = enqueue_forward(h, 2, src);
+  if (rc != TTSH_OK) return rc;
+  TRY(h, DISPATCH(h, launch_spectral_init, h->g, h->S[0], h->S[1], s->what[i], s->psihat[i], s->v0[i], h->stream));
+  h->launches++;
+  s->set[i] = true;
+  return TTSH_OK;
+}
+// inverse transforms of perturbation i into real buffers (permuted internal layout if perm, else natural); any dst may be NULL
+static int tangent_inverse(ttsh_tangent* s, int i, void* dw, void* dvx, void* dvy, bool perm) {
+  ttsh_handle* h = s->h;
+  const int pf = perm ? RM_PERM : 0;
+  Batch cb; memset(&cb, 0, sizeof(cb));
+  Batch rb; memset(&rb, 0, sizeof(rb));
+  int nc = 0, nr = 0;
+  if (dw) { cb.f[nc++] = op(s->what[i], h->Tm[0], SM_ONE); rb.f[nr++] = op(h->Tm[0], dw, RM_ONE | pf); }
+  if (dvy) { cb.f[nc++] = op(s->psihat[i], h->Tm[2], SM_ONE); rb.f[nr++] = op(h->Tm[2], dvy, RM_NIKX_MEANY | pf); }
+  if (dvx) { cb.f[nc++] = op(s->psihat[i], h->Tm[3], SM_IKY_MEANX); rb.f[nr++] = op(h->Tm[3], dvx, RM_ONE | pf); }
+  if (nc == 0) return TTSH_OK;
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->tabS, s->v0[i], h->stream));
+  TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, s->v0[i], h->stream));
+  h->launches += 2;
+  return TTSH_OK;
+}
+int ttsh_tangent_step(ttsh_tangent* s, int n) {
+  if (!s || n < 0) return TTSH_ERR_INVALID_ARG;
+  ttsh_handle* h = s->h;
+  if (h->sticky) return h->sticky;
+  if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
+  for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
+  for (int it = 0; it < n; ++it) {
+    // base state in real space (permuted internal layout): R[0] = w, R[3] = v_x, R[4] = v_y
+    int rc = enqueue_stage(h, TTSH_STAGE_INV_COL);
+    if (rc == TTSH_OK) rc = enqueue_stage(h, TTSH_STAGE_INV_ROW);
+    if (rc != TTSH_OK) return rc;
+    for (int i = 0; i < s->nvec; ++i) {
+      rc = tangent_inverse(s, i, s->real[0], s->real[1], s->real[2], true);        // dw, dv_x, dv_y
+      if (rc != TTSH_OK) return rc;
+      TRY(h, DISPATCH(h, launch_realspace_tangent, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, s->real[1], s->real[2], s->real[0], h->stream));
+      Batch rb = make_batch({op(s->real[1], h->Tm[0], RM_PERM), op(s->real[2], h->Tm[1], RM_PERM), op(s->real[0], h->Tm[2], RM_PERM)});
+      TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->stream));
+      Batch cb = make_batch({op(h->Tm[0], h->S[0], 0), op(h->Tm[1], h->S[1], 0), op(h->Tm[2], h->S[2], 0)});
+      TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 3, h->tabY, h->tabS, h->stream));
+      // lines 3-16 are linear: the same spectral kernel on the perturbation's (dw^, dpsi^, dv^(0))
+      TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, h->S[0], h->S[1], h->S[2], s->what[i], s->psihat[i], s->v0[i], h->stream));
+      h->launches += 4;
+    }
+    rc = ttsh_step(h, 1);
+    if (rc != TTSH_OK) return rc;
+  }
+  return TTSH_OK;
+}
+int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host) {
+  if (!s || !log_r_host) return TTSH_ERR_INVALID_ARG;
+  ttsh_handle* h = s->h;
+  if (h->sticky) return h->sticky;
+  for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
+  // modified Gram-Schmidt, all coefficients stay on the device
+  for (int i = 0; i < s->nvec; ++i) {
+    TRY(h, DISPATCH(h, launch_spec_dot, h->g, s->what[i], s->what[i], s->v0[i], s->v0[i], i, s->partial, s->rdiag, s->coef, h->stream));
+    TRY(h, DISPATCH(h, launch_spec_scale_axpy, h->g, s->coef, nullptr, s->what[i], nullptr, s->v0[i], h->stream));
+    h->launches += 3;
+    for (int j = i + 1; j < s->nvec; ++j) {
+      TRY(h, DISPATCH(h, launch_spec_dot, h->g, s->what[i], s->what[j], s->v0[i], s->v0[j], -1, s->partial, s->rdiag, s->coef, h->stream));
+      TRY(h, DISPATCH(h, launch_spec_scale_axpy, h->g, s->coef, s->what[i], s->what[j], s->v0[i], s->v0[j], h->stream));
+      h->launches += 3;
+    }
+  }
+  for (int i = 0; i < s->nvec; ++i) {
+    TRY(h, DISPATCH(h, launch_psi_from_w, h->g, s->what[i], s->psihat[i], h->stream));
+    h->launches++;
+  }
+  TRY(h, cudaMemcpyAsync(log_r_host, s->rdiag, (size_t)s->nvec * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));
+  for (int i = 0; i < s->nvec; ++i) log_r_host[i] = log(log_r_host[i]);
+  return TTSH_OK;
+}
+int ttsh_tangent_get_fields(ttsh_tangent* s, int i, void* dvx, void* dvy, void* domega) {
+  if (!s || i < 0 || i >= s->nvec) return TTSH_ERR_INVALID_ARG;
+  if (s->h->sticky) return s->h->sticky;
+  if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
+  return tangent_inverse(s, i, domega, dvx, dvy, false);
+}
+int ttsh_tangent_destroy(ttsh_tangent* s) {
   delete s;
   return TTSH_OK;
 }

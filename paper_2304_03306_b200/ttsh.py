@@ -31,7 +31,9 @@ SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_vel
            "ttsh_get_fields", "ttsh_state_elems", "ttsh_get_state", "ttsh_set_state", "ttsh_diagnostics",
            "ttsh_launch_count", "ttsh_run_stage", "ttsh_debug_get_real", "ttsh_destroy", "ttsh_strerror",
            "ttsh_last_error", "ttsh_dumbbell_order", "ttsh_psd_workspace_bytes", "ttsh_psd_create",
-           "ttsh_psd_accumulate", "ttsh_psd_result", "ttsh_psd_reset", "ttsh_psd_destroy", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
+           "ttsh_psd_accumulate", "ttsh_psd_result", "ttsh_psd_reset", "ttsh_psd_destroy", "ttsh_tangent_workspace_bytes",
+           "ttsh_tangent_create", "ttsh_tangent_set", "ttsh_tangent_step", "ttsh_tangent_orthonormalize",
+           "ttsh_tangent_get_fields", "ttsh_tangent_destroy", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
            "ttsh_ensemble_destroy")
 
 
@@ -82,6 +84,13 @@ _sig = {
     "ttsh_psd_result": (_i, [_vp, C.POINTER(_d), C.POINTER(_ll)]),
     "ttsh_psd_reset": (_i, [_vp]),
     "ttsh_psd_destroy": (_i, [_vp]),
+    "ttsh_tangent_workspace_bytes": (_sz, [_i, _i, _i, _i]),
+    "ttsh_tangent_create": (_i, [C.POINTER(_vp), _vp, _i, _vp, _sz]),
+    "ttsh_tangent_set": (_i, [_vp, _i, _vp, _vp]),
+    "ttsh_tangent_step": (_i, [_vp, _i]),
+    "ttsh_tangent_orthonormalize": (_i, [_vp, C.POINTER(_d)]),
+    "ttsh_tangent_get_fields": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "ttsh_tangent_destroy": (_i, [_vp]),
     "ttsh_ensemble_create": (_i, [C.POINTER(_vp), C.POINTER(_vp), _i]),
     "ttsh_ensemble_step": (_i, [_vp, _i]),
     "ttsh_ensemble_launch_count": (_ll, [_vp]),
@@ -197,6 +206,38 @@ def ttsh_psd_reset(s):
 
 def ttsh_psd_destroy(s):
     return _lib.ttsh_psd_destroy(s)
+
+
+def ttsh_tangent_workspace_bytes(Nx, Ny, dtype, nvec):
+    return int(_lib.ttsh_tangent_workspace_bytes(Nx, Ny, dtype, nvec))
+
+
+def ttsh_tangent_create(h, nvec, workspace_ptr, workspace_bytes):
+    s = _vp()
+    rc = _lib.ttsh_tangent_create(C.byref(s), h, nvec, workspace_ptr or None, workspace_bytes)
+    return rc, s
+
+
+def ttsh_tangent_set(s, i, dvx_ptr, dvy_ptr):
+    return _lib.ttsh_tangent_set(s, i, dvx_ptr or None, dvy_ptr or None)
+
+
+def ttsh_tangent_step(s, n):
+    return _lib.ttsh_tangent_step(s, n)
+
+
+def ttsh_tangent_orthonormalize(s, nvec):
+    out = (_d * max(1, nvec))()
+    rc = _lib.ttsh_tangent_orthonormalize(s, out)
+    return rc, [out[i] for i in range(nvec)]
+
+
+def ttsh_tangent_get_fields(s, i, dvx_ptr=None, dvy_ptr=None, domega_ptr=None):
+    return _lib.ttsh_tangent_get_fields(s, i, dvx_ptr or None, dvy_ptr or None, domega_ptr or None)
+
+
+def ttsh_tangent_destroy(s):
+    return _lib.ttsh_tangent_destroy(s)
 
 
 def ttsh_launch_count(h):
@@ -387,6 +428,54 @@ class TemporalPSD:
         if getattr(self, "s", None):
             self.solver.torch.cuda.synchronize(self.solver.device)
             ttsh_psd_destroy(self.s)
+            self.s = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Tangent:
+    """nvec perturbations carried along a Solver's trajectory by the Jacobian of Algorithm 1, with QR re-orthonormalisation
+    (Lyapunov exponents): lambda_i = sum of orthonormalize()[i] over the run / elapsed time."""
+
+    def __init__(self, solver: Solver, nvec: int):
+        self.solver, self.nvec = solver, int(nvec)
+        torch = solver.torch
+        nbytes = ttsh_tangent_workspace_bytes(solver.Nx, solver.Ny, solver.dtype_code, self.nvec)
+        if nbytes == 0:
+            raise TTSHError(TTSH_ERR_INVALID_ARG, "1 <= nvec <= 64")
+        with torch.cuda.device(solver.device), torch.cuda.stream(solver.stream):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=solver.device)
+            rc, self.s = ttsh_tangent_create(solver.h, self.nvec, self.workspace.data_ptr(), nbytes)
+        if rc != TTSH_OK:
+            raise TTSHError(rc)
+
+    def set(self, i: int, dvx, dvy):
+        a, b = self.solver._dev(dvx), self.solver._dev(dvy)
+        self._keep = (a, b)
+        self.solver._check(ttsh_tangent_set(self.s, i, a.data_ptr(), b.data_ptr()))
+
+    def step(self, n: int = 1):
+        self.solver._check(ttsh_tangent_step(self.s, n))
+
+    def orthonormalize(self):
+        rc, logr = ttsh_tangent_orthonormalize(self.s, self.nvec)
+        self.solver._check(rc)
+        return logr
+
+    def get_fields(self, i: int):
+        s = self.solver
+        dvx, dvy, dw = s.new_field(), s.new_field(), s.new_field()
+        s._check(ttsh_tangent_get_fields(self.s, i, dvx.data_ptr(), dvy.data_ptr(), dw.data_ptr()))
+        return dvx, dvy, dw
+
+    def close(self):
+        if getattr(self, "s", None):
+            self.solver.torch.cuda.synchronize(self.solver.device)
+            ttsh_tangent_destroy(self.s)
             self.s = None
 
     def __del__(self):

@@ -14,8 +14,10 @@ template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, 
                                                  int members = 1, size_t mstride = 0);
 template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, cudaStream_t s,
                                                  int members = 1, size_t mstride = 0);
-template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const double* v0, cudaStream_t s);
-template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, cudaStream_t s);
+template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const double* v0, cudaStream_t s,
+                                                 int members = 1, size_t mstride = 0);
+template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, cudaStream_t s,
+                                                 int members = 1, size_t mstride = 0);
 // fused real-space + forward row pass (conservative form): reads v_x, v_y, w, K; writes A~ = i kx Gy~ + S'~ and B~ = Gx~
 template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
                                                        const void* K, void* oA, void* oB, const void* tabX, cudaStream_t s);
@@ -42,7 +44,7 @@ template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m
 template <typename T> cudaError_t launch_realspace_cons(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,
                                                         void* w_s, void* gx_out, void* gy_out, cudaStream_t s);
 template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
-                                                  void* w, void* psi, double* v0, cudaStream_t s);
+                                                  void* w, void* psi, double* v0, cudaStream_t s, int members = 1, size_t mstride = 0);
 template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, void* psi, double* v0, cudaStream_t s);
 template <typename T> cudaError_t launch_psi_from_w(const Geom& g, const void* w, void* psi, cudaStream_t s);
 template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s);
@@ -67,11 +69,15 @@ template <typename T> cudaError_t launch_psd_power(size_t n, int nf, const void*
 int psd_blocks();
 
 // tangent-linear step and Gram-Schmidt on tangent vectors (pointwise.cuh)
+// members: tangent vectors whose (dvx, dvy, dw) lie mstride bytes apart; the base fields and K are shared
 template <typename T> cudaError_t launch_realspace_tangent(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
-                                                           const void* K, void* dvx, void* dvy, void* dw, cudaStream_t s);
+                                                           const void* K, void* dvx, void* dvy, void* dw, cudaStream_t s,
+                                                           int members = 1, size_t mstride = 0);
+// batched over count vectors b_j / y_j at a uniform byte stride (one launch per Gram-Schmidt row)
 template <typename T> cudaError_t launch_spec_dot(const Geom& g, const void* a, const void* b, const double* a0, const double* b0,
-                                                  int norm_slot, double* partial, double* rdiag, double* coef, cudaStream_t s);
+                                                  int count, size_t bstride, int norm_slot, double* partial, double* rdiag,
+                                                  double* coef, cudaStream_t s);
 template <typename T> cudaError_t launch_spec_scale_axpy(const Geom& g, const double* coef, const void* x, void* y, const double* x0,
-                                                         double* y0, cudaStream_t s);
+                                                         double* y0, int count, size_t ystride, cudaStream_t s);
 
 }  // namespace ttsh

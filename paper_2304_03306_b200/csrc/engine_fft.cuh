@@ -84,16 +84,18 @@ template <typename T> cudaError_t prepare_cols(const Geom& g) {
 #endif
 
 #ifdef TTSH_BUILD_ROWS
-template <typename T, int NX> static cudaError_t go_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+template <typename T, int NX> static cudaError_t go_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s,
+                                                            int members, size_t mstride) {
   using C = RowCfg<T, NX>;
-  dim3 grid((g.Ny / 2) / C::L, nf);
-  k_inv_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), v0);
+  dim3 grid((g.Ny / 2) / C::L, nf, members);
+  k_inv_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), v0, mstride);
   return cudaGetLastError();
 }
-template <typename T, int NX> static cudaError_t go_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+template <typename T, int NX> static cudaError_t go_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s,
+                                                            int members, size_t mstride) {
   using C = RowCfg<T, NX>;
-  dim3 grid((g.Ny / 2) / C::L, nf);
-  k_fwd_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab));
+  dim3 grid((g.Ny / 2) / C::L, nf, members);
+  k_fwd_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), mstride);
   return cudaGetLastError();
 }
 template <typename T, int NX> static size_t fused_smem(const Geom& g) {
@@ -116,17 +118,21 @@ template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Mode
   }
   return cudaErrorInvalidValue;
 }
-template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s) {
+template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s,
+                                                 int members, size_t mstride) {
+  if (members < 1 || members > 65535) return cudaErrorInvalidValue;
   switch (g.Nx) {
-#define X(N) case N: return go_inv_row<T, N>(g, b, nf, tab, v0, s);
+#define X(N) case N: return go_inv_row<T, N>(g, b, nf, tab, v0, s, members, mstride);
     TTSH_FOR_SIZES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s) {
+template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s,
+                                                 int members, size_t mstride) {
+  if (members < 1 || members > 65535) return cudaErrorInvalidValue;
   switch (g.Nx) {
-#define X(N) case N: return go_fwd_row<T, N>(g, b, nf, tab, s);
+#define X(N) case N: return go_fwd_row<T, N>(g, b, nf, tab, s, members, mstride);
     TTSH_FOR_SIZES(X)
 #undef X
   }

@@ -315,7 +315,7 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 template <typename T, int NX>
 __global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
 k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabX,
-          const double* __restrict__ v0) {
+          const double* __restrict__ v0_, size_t mstride) {
   using C = RowCfg<T, NX>;
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -323,7 +323,11 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const int c = threadIdx.x / TPL, j = threadIdx.x % TPL;
   const int rp = blockIdx.x * C::L + c;             // row pair: rows yA = 4a+p, yB = yA+2; Ny/2 is a multiple of L
   const int a = rp >> 1, p = rp & 1;
-  const FieldOp op = batch.f[blockIdx.y];
+  const size_t moff = (size_t)blockIdx.z * mstride;     // grid.z = member (tangent vectors at a uniform stride); 0 otherwise
+  FieldOp op = batch.f[blockIdx.y];
+  op.src = static_cast<const char*>(op.src) + moff;
+  op.dst = static_cast<char*>(op.dst) + moff;
+  const double* __restrict__ v0 = reinterpret_cast<const double*>(reinterpret_cast<const char*>(v0_) + moff);
   const int Wx = g.Wx;
   const cplx<T>* __restrict__ src = static_cast<const cplx<T>*>(op.src);
   T* __restrict__ dstA = static_cast<T*>(op.dst) + (size_t)(4 * a + p) * NX;
@@ -344,7 +348,7 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     int nb = blockIdx.x + TTSH_PF_DIST, ny = blockIdx.y;
     if (nb >= (int)gridDim.x) { nb -= gridDim.x; ny += 1; }
     if (ny < (int)gridDim.y)
-      prefetch_l2_bulk(static_cast<const cplx<T>*>(batch.f[ny].src) + (size_t)nb * C::L * g.Wxp * 2,
+      prefetch_l2_bulk(reinterpret_cast<const cplx<T>*>(static_cast<const char*>(batch.f[ny].src) + moff) + (size_t)nb * C::L * g.Wxp * 2,
                        (unsigned)(C::L * g.Wxp * 2 * sizeof(cplx<T>)));
   }
   auto zero_pair = [&]() -> Pair<T> { Pair<T> r; r.a = mk<T>(0, 0); r.b = mk<T>(0, 0); return r; };
@@ -405,7 +409,7 @@ k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 // ---------------------------------------------------------------------------------------
 template <typename T, int NX>
 __global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
-k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabX) {
+k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabX, size_t mstride) {
   using C = RowCfg<T, NX>;
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -413,7 +417,10 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   const int c = threadIdx.x / TPL, j = threadIdx.x % TPL;
   const int rp = blockIdx.x * C::L + c;
   const int a = rp >> 1, p = rp & 1;
-  const FieldOp op = batch.f[blockIdx.y];
+  const size_t moff = (size_t)blockIdx.z * mstride;     // grid.z = member
+  FieldOp op = batch.f[blockIdx.y];
+  op.src = static_cast<const char*>(op.src) + moff;
+  op.dst = static_cast<char*>(op.dst) + moff;
   const int Wx = g.Wx;
   const T* __restrict__ srcA = static_cast<const T*>(op.src) + (size_t)(4 * a + p) * NX;
   const T* __restrict__ srcB = srcA + 2 * NX;
@@ -424,7 +431,7 @@ k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     int nb = blockIdx.x + TTSH_PF_DIST, ny = blockIdx.y;
     if (nb >= (int)gridDim.x) { nb -= gridDim.x; ny += 1; }
     if (ny < (int)gridDim.y && ((nb * C::L) & 1) == 0)
-      prefetch_l2_bulk(static_cast<const T*>(batch.f[ny].src) + (size_t)(2 * nb * C::L) * NX,
+      prefetch_l2_bulk(reinterpret_cast<const T*>(static_cast<const char*>(batch.f[ny].src) + moff) + (size_t)(2 * nb * C::L) * NX,
                        (C::L >= 2 ? 2 * C::L : 4) * NX * sizeof(T));
   }
 

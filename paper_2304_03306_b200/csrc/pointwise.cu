@@ -25,9 +25,10 @@ template <typename T> cudaError_t launch_realspace_cons(const Geom& g, const Mod
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m, const void* Fx, const void* Fy, const void* S,
-                                                  void* w, void* psi, double* v0, cudaStream_t s) {
-  const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
-  k_spectral<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, (cplx<T>*)psi, v0);
+                                                  void* w, void* psi, double* v0, cudaStream_t s, int members, size_t mstride) {
+  if (members < 1 || members > 65535) return cudaErrorInvalidValue;
+  const dim3 grid((unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256), (unsigned)members);
+  k_spectral<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, (cplx<T>*)psi, v0, mstride);
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model& m, const void* A, const void* B, void* w, void* psi,
@@ -106,39 +107,43 @@ template <typename T> cudaError_t launch_psd_power(size_t n, int nf, const void*
 int psd_blocks() { return PSD_BLOCKS; }
 
 template <typename T> cudaError_t launch_realspace_tangent(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
-                                                           const void* K, void* dvx, void* dvy, void* dw, cudaStream_t s) {
+                                                           const void* K, void* dvx, void* dvy, void* dw, cudaStream_t s,
+                                                           int members, size_t mstride) {
+  if (members < 1 || members > 65535) return cudaErrorInvalidValue;
   const size_t nvec = (size_t)g.Nx * g.Ny / Vec<T>::n;
-  k_realspace_tangent<T><<<blocks_for(nvec, 256, GRID_CAP), 256, 0, s>>>(nvec, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K,
-                                                                           (T*)dvx, (T*)dvy, (T*)dw);
+  const dim3 grid((unsigned)blocks_for(nvec, 256, GRID_CAP), (unsigned)members);
+  k_realspace_tangent<T><<<grid, 256, 0, s>>>(nvec, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K, (T*)dvx, (T*)dvy, (T*)dw, mstride);
   return cudaGetLastError();
 }
-// coef[0] <- <a, b> (norm_slot < 0) or rdiag[norm_slot] <- |a|, coef[0] <- 1/|a|; partial: DIAG_BLOCKS doubles
+// count = 1, norm_slot >= 0:  rdiag[norm_slot] <- |a|, coef[0] <- 1/|a|   (b = a)
+// norm_slot < 0:              coef[j] <- <a, b_j>, b_j = b + j * bstride bytes, j < count;  partial: DIAG_BLOCKS * count doubles
 template <typename T> cudaError_t launch_spec_dot(const Geom& g, const void* a, const void* b, const double* a0, const double* b0,
-                                                  int norm_slot, double* partial, double* rdiag, double* coef, cudaStream_t s) {
-  k_spec_dot_partial<T><<<DIAG_BLOCKS, 256, 0, s>>>(g, (const cplx<T>*)a, (const cplx<T>*)b, partial);
+                                                  int count, size_t bstride, int norm_slot, double* partial, double* rdiag,
+                                                  double* coef, cudaStream_t s) {
+  k_spec_dot_partial<T><<<dim3(DIAG_BLOCKS, count), 256, 0, s>>>(g, (const cplx<T>*)a, (const cplx<T>*)b, partial, bstride);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  k_spec_dot_final<<<1, 32, 0, s>>>(DIAG_BLOCKS, partial, a0, b0, norm_slot, rdiag, coef);
+  k_spec_dot_final<<<count, 32, 0, s>>>(DIAG_BLOCKS, partial, a0, b0, bstride, norm_slot, rdiag, coef);
   return cudaGetLastError();
 }
-// y <- coef y (x == NULL) or y <- y - coef x, on the spectrum and the mean flow
+// y_j <- coef[j] y_j (x == NULL) or y_j <- y_j - coef[j] x, j < count, on the spectrum and the mean flow
 template <typename T> cudaError_t launch_spec_scale_axpy(const Geom& g, const double* coef, const void* x, void* y, const double* x0,
-                                                         double* y0, cudaStream_t s) {
+                                                         double* y0, int count, size_t ystride, cudaStream_t s) {
   const size_t n = (size_t)g.NT * g.Hy * g.CW;
-  k_spec_scale_axpy<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, coef, (const cplx<T>*)x, (cplx<T>*)y, x0, y0);
+  k_spec_scale_axpy<T><<<dim3(blocks_for(n, 256, GRID_CAP), count), 256, 0, s>>>(n, coef, (const cplx<T>*)x, (cplx<T>*)y, x0, y0, ystride);
   return cudaGetLastError();
 }
 
 #define INST(T) \
-  template cudaError_t launch_realspace_tangent<T>(const Geom&, const Model&, const void*, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
-  template cudaError_t launch_spec_dot<T>(const Geom&, const void*, const void*, const double*, const double*, int, double*, double*, double*, cudaStream_t); \
-  template cudaError_t launch_spec_scale_axpy<T>(const Geom&, const double*, const void*, void*, const double*, double*, cudaStream_t); \
+  template cudaError_t launch_realspace_tangent<T>(const Geom&, const Model&, const void*, const void*, const void*, const void*, void*, void*, void*, cudaStream_t, int, size_t); \
+  template cudaError_t launch_spec_dot<T>(const Geom&, const void*, const void*, const double*, const double*, int, size_t, int, double*, double*, double*, cudaStream_t); \
+  template cudaError_t launch_spec_scale_axpy<T>(const Geom&, const double*, const void*, void*, const double*, double*, int, size_t, cudaStream_t); \
   template cudaError_t launch_psd_accumulate<T>(size_t, int, const double*, const double*, const void*, void*, cudaStream_t); \
   template cudaError_t launch_psd_power<T>(size_t, int, const void*, double*, double*, cudaStream_t); \
   template cudaError_t launch_region_argmax<T>(const Geom&, double, double, double, double, double, double, const void*, double*, double*, cudaStream_t); \
   template cudaError_t launch_realspace<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
   template cudaError_t launch_realspace_cons<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, void*, cudaStream_t); \
-  template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, double*, cudaStream_t); \
+  template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, double*, cudaStream_t, int, size_t); \
   template cudaError_t launch_spectral_init<T>(const Geom&, const void*, const void*, void*, void*, double*, cudaStream_t); \
   template cudaError_t launch_psi_from_w<T>(const Geom&, const void*, void*, cudaStream_t); \
   template cudaError_t launch_spectral_p2<T>(const Geom&, const Model&, const void*, const void*, void*, void*, double*, cudaStream_t, int, size_t); \

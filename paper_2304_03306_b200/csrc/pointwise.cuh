@@ -106,11 +106,18 @@ template <typename T> __device__ __forceinline__ T inv_k2(const Geom& g, int mx,
 
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx, const cplx<T>* __restrict__ Fy,
-           const cplx<T>* __restrict__ S, cplx<T>* w, cplx<T>* __restrict__ psi, double* v0) {
+k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx_, const cplx<T>* __restrict__ Fy_,
+           const cplx<T>* __restrict__ S_, cplx<T>* w_, cplx<T>* __restrict__ psi_, double* v0_, size_t mstride) {
   // threads enumerate the tile-major array in memory order: idx = (t Hy + q) CW + c
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
+  const size_t moff = (size_t)blockIdx.y * mstride;      // member (tangent vectors at a uniform byte stride); 0 otherwise
+  const cplx<T>* __restrict__ Fx = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(Fx_) + moff);
+  const cplx<T>* __restrict__ Fy = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(Fy_) + moff);
+  const cplx<T>* __restrict__ S = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(S_) + moff);
+  cplx<T>* w = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(w_) + moff);
+  cplx<T>* __restrict__ psi = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(psi_) + moff);
+  double* v0 = reinterpret_cast<double*>(reinterpret_cast<char*>(v0_) + moff);
   const int t = (int)(idx / ((size_t)g.Hy * g.CW));
   const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
   const int q = rem >> g.cw_shift;
@@ -526,7 +533,11 @@ __global__ void __launch_bounds__(32) k_psd_power_final(int nblocks, const doubl
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_realspace_tangent(size_t nvec, Model m, const T* __restrict__ vx, const T* __restrict__ vy, const T* __restrict__ w,
-                    const T* __restrict__ K, T* __restrict__ dvx, T* __restrict__ dvy, T* __restrict__ dw) {
+                    const T* __restrict__ K, T* __restrict__ dvx_, T* __restrict__ dvy_, T* __restrict__ dw_, size_t mstride) {
+  const size_t moff = (size_t)blockIdx.y * mstride;      // tangent vector (bytes); the base fields and K are shared
+  T* __restrict__ dvx = reinterpret_cast<T*>(reinterpret_cast<char*>(dvx_) + moff);
+  T* __restrict__ dvy = reinterpret_cast<T*>(reinterpret_cast<char*>(dvy_) + moff);
+  T* __restrict__ dw = reinterpret_cast<T*>(reinterpret_cast<char*>(dw_) + moff);
   using V = typename Vec<T>::type;
   constexpr int n = Vec<T>::n;
   const T beta = (T)m.beta, gv = (T)m.gamma_v, gw = (T)m.gamma_w, lam = (T)m.lambda0;
@@ -556,7 +567,9 @@ k_realspace_tangent(size_t nvec, Model m, const T* __restrict__ vx, const T* __r
 // of the column mx = 0 count once (both +-my are stored), mx > 0 twice (their conjugates are implicit).
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_spec_dot_partial(Geom g, const cplx<T>* __restrict__ a, const cplx<T>* __restrict__ b, double* __restrict__ partial) {
+k_spec_dot_partial(Geom g, const cplx<T>* __restrict__ a, const cplx<T>* __restrict__ b_, double* __restrict__ partial, size_t bstride) {
+  // grid.y = vector j of a batch <a, b_j>, b_j = b_ + j * bstride bytes;  partial[j][gridDim.x]
+  const cplx<T>* __restrict__ b = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(b_) + (size_t)blockIdx.y * bstride);
   const size_t n = (size_t)g.NT * g.Hy * g.CW;
   double sum = 0.0;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
@@ -576,16 +589,18 @@ k_spec_dot_partial(Geom g, const cplx<T>* __restrict__ a, const cplx<T>* __restr
     sum = lane < (int)(blockDim.x >> 5) ? sh[lane] : 0.0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
-    if (lane == 0) partial[blockIdx.x] = sum;
+    if (lane == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = sum;
   }
 }
-// one warp: total = sum partial + a0 . b0.  norm_slot >= 0: rdiag[norm_slot] = sqrt(total), coef[0] = 1 / sqrt(total)
+// one warp per vector j (blockIdx.x): total = sum partial + a0 . b0.  norm_slot >= 0: rdiag[norm_slot] = sqrt(total), coef[0] = 1 / sqrt(total)
 // (0 if total == 0); else coef[0] = total.
 __global__ void __launch_bounds__(32)
-k_spec_dot_final(int nblocks, const double* __restrict__ partial, const double* __restrict__ a0, const double* __restrict__ b0,
-                 int norm_slot, double* __restrict__ rdiag, double* __restrict__ coef) {
+k_spec_dot_final(int nblocks, const double* __restrict__ partial, const double* __restrict__ a0, const double* __restrict__ b0_,
+                 size_t bstride, int norm_slot, double* __restrict__ rdiag, double* __restrict__ coef_) {
+  const double* __restrict__ b0 = reinterpret_cast<const double*>(reinterpret_cast<const char*>(b0_) + (size_t)blockIdx.x * bstride);
+  double* __restrict__ coef = coef_ + blockIdx.x;
   double sum = 0.0;
-  for (int b = threadIdx.x; b < nblocks; b += 32) sum += partial[b];
+  for (int b = threadIdx.x; b < nblocks; b += 32) sum += partial[(size_t)blockIdx.x * nblocks + b];
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
   if (threadIdx.x == 0) {
@@ -600,8 +615,12 @@ k_spec_dot_final(int nblocks, const double* __restrict__ partial, const double* 
 // scale: y <- coef y (x == nullptr);  axpy: y <- y - coef x.  coef is read from device memory (no host round trip in the QR).
 template <typename T>
 __global__ void __launch_bounds__(256)
-k_spec_scale_axpy(size_t n, const double* __restrict__ coef, const cplx<T>* __restrict__ x, cplx<T>* __restrict__ y,
-                  const double* __restrict__ x0, double* __restrict__ y0) {
+k_spec_scale_axpy(size_t n, const double* __restrict__ coef_, const cplx<T>* __restrict__ x, cplx<T>* __restrict__ y_,
+                  const double* __restrict__ x0, double* __restrict__ y0_, size_t ystride) {
+  // grid.y = vector j of a batch: y_j = y_ + j * ystride bytes, coefficient coef_[j]
+  const double* __restrict__ coef = coef_ + blockIdx.y;
+  cplx<T>* __restrict__ y = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(y_) + (size_t)blockIdx.y * ystride);
+  double* __restrict__ y0 = reinterpret_cast<double*>(reinterpret_cast<char*>(y0_) + (size_t)blockIdx.y * ystride);
   const T c = (T)coef[0];
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     cplx<T> v = y[i];

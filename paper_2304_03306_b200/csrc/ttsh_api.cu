@@ -109,12 +109,18 @@ struct ttsh_psd {
 struct ttsh_tangent {
   ttsh_handle* h;                      // borrowed
   int nvec;
-  std::vector<void*> what, psihat;     // per vector: dw^, dpsi^ (pruned tile-major spectra in the caller's workspace)
-  std::vector<double*> v0;             // per vector: dv^(0)
+  size_t stride;                       // bytes between the workspace blocks of consecutive vectors
+  // block of vector 0 (vector i: + i * stride): dw^, dpsi^ (pruned tile-major spectra), dv^(0), and per-vector scratch:
+  // dw | dv_x | dv_y in real space (permuted internal row layout), three intermediates, three spectra
+  void *what, *psihat;
+  double* v0;
+  void *real[3], *inter[3], *spec[3];
   std::vector<bool> set;
-  void* real[3];                       // dw, dv_x, dv_y of the vector being stepped (permuted internal row layout)
   double *partial, *coef, *rdiag;
 };
+template <class P> static P* vec_ptr(const ttsh_tangent* s, P* p0, int i) {
+  return reinterpret_cast<P*>(reinterpret_cast<char*>(p0) + (size_t)i * s->stride);
+}
 
 struct ttsh_ensemble {
   std::vector<ttsh_handle*> members;   // borrowed
@@ -687,18 +693,26 @@ int ttsh_psd_destroy(ttsh_psd* s) {
 }
 
 // ---- tangent-linear evolution and QR growth rates -----------------------------------------
-struct TanLayout { size_t vec, vec_stride, real[3], partial, coef, rdiag, total; };
+// Every vector owns one block of the workspace — dw^, dpsi^, dv^(0), three real fields, three intermediates, three spectra —
+// and the blocks lie at a uniform stride, so one launch of each kernel serves ALL vectors (the member dimension of the
+// kernels, as in ttsh_ensemble_step): a tangent step costs 7 launches whatever nvec is.
+struct TanLayout { size_t what, psihat, v0, real[3], inter[3], spec[3], vec_stride, vec, partial, coef, rdiag, total; };
 static TanLayout tan_layout(int Nx, int Ny, size_t w, int nvec) {
   const Geom g = make_geom(Nx, Ny, 1.0, 2, 3, w);
-  const size_t spec = (size_t)g.NT * g.CW * g.Hy * 2 * w, P = (size_t)Nx * Ny;
+  const size_t cw = 2 * w, P = (size_t)Nx * Ny;
+  const size_t spec = (size_t)g.NT * g.CW * g.Hy * cw, inter = (size_t)g.NT * g.CW * Ny * cw;
   TanLayout L;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
-  L.vec_stride = 2 * align_up(spec) + align_up(8 * sizeof(double));       // dw^, dpsi^, dv^(0)
-  L.vec = take(L.vec_stride * nvec);
+  L.what = take(spec); L.psihat = take(spec); L.v0 = take(8 * sizeof(double));
   for (int i = 0; i < 3; ++i) L.real[i] = take(P * w);
-  L.partial = take((size_t)DIAG_BLOCKS * sizeof(double));
-  L.coef = take(8 * sizeof(double));
+  for (int i = 0; i < 3; ++i) L.inter[i] = take(inter);
+  for (int i = 0; i < 3; ++i) L.spec[i] = take(spec);
+  L.vec_stride = off;
+  off = 0;
+  L.vec = take(L.vec_stride * nvec);
+  L.partial = take((size_t)DIAG_BLOCKS * nvec * sizeof(double));
+  L.coef = take((size_t)(nvec + 8) * sizeof(double));
   L.rdiag = take((size_t)nvec * sizeof(double));
   L.total = off;
   return L;
@@ -721,16 +735,11 @@ int ttsh_tangent_create(ttsh_tangent** out, ttsh_handle* h, int nvec, void* work
   char* ws = static_cast<char*>(workspace);
   s->h = h;
   s->nvec = nvec;
-  s->what.resize(nvec); s->psihat.resize(nvec); s->v0.resize(nvec);
+  s->stride = L.vec_stride;
   s->set.assign(nvec, false);
-  const size_t spec_max = (L.vec_stride - align_up(8 * sizeof(double))) / 2;    // bytes of one spectrum slot
-  for (int i = 0; i < nvec; ++i) {
-    char* base = ws + L.vec + (size_t)i * L.vec_stride;
-    s->what[i] = base;
-    s->psihat[i] = base + spec_max;
-    s->v0[i] = reinterpret_cast<double*>(base + 2 * spec_max);
-  }
-  for (int i = 0; i < 3; ++i) s->real[i] = ws + L.real[i];
+  char* v = ws + L.vec;                     // block of vector 0; vector i is at + i * stride
+  s->what = v + L.what; s->psihat = v + L.psihat; s->v0 = reinterpret_cast<double*>(v + L.v0);
+  for (int i = 0; i < 3; ++i) { s->real[i] = v + L.real[i]; s->inter[i] = v + L.inter[i]; s->spec[i] = v + L.spec[i]; }
   s->partial = reinterpret_cast<double*>(ws + L.partial);
   s->coef = reinterpret_cast<double*>(ws + L.coef);
   s->rdiag = reinterpret_cast<double*>(ws + L.rdiag);
@@ -745,24 +754,33 @@ int ttsh_tangent_set(ttsh_tangent* s, int i, const void* dvx, const void* dvy) {
   const void* src[2] = {dvx, dvy};
   int rc = enqueue_forward(h, 2, src);
   if (rc != TTSH_OK) return rc;
-  TRY(h, DISPATCH(h, launch_spectral_init, h->g, h->S[0], h->S[1], s->what[i], s->psihat[i], s->v0[i], h->stream));
+  TRY(h, DISPATCH(h, launch_spectral_init, h->g, h->S[0], h->S[1], vec_ptr(s, s->what, i), vec_ptr(s, s->psihat, i), vec_ptr(s, s->v0, i), h->stream));
   h->launches++;
   s->set[i] = true;
   return TTSH_OK;
 }
-// inverse transforms of perturbation i into real buffers (permuted internal layout if perm, else natural); any dst may be NULL
-static int tangent_inverse(ttsh_tangent* s, int i, void* dw, void* dvx, void* dvy, bool perm) {
+// inverse transforms of `count` vectors starting at vector `first` into dw, dvx, dvy (vector `first`'s buffers; the others
+// at + stride): permuted internal row layout if perm, else natural; any destination may be NULL
+static int tangent_inverse(ttsh_tangent* s, int first, int count, void* dw, void* dvx, void* dvy, bool perm, size_t dst_stride) {
   ttsh_handle* h = s->h;
   const int pf = perm ? RM_PERM : 0;
   Batch cb; memset(&cb, 0, sizeof(cb));
   Batch rb; memset(&rb, 0, sizeof(rb));
+  void* what = vec_ptr(s, s->what, first);
+  void* psihat = vec_ptr(s, s->psihat, first);
+  double* v0 = vec_ptr(s, s->v0, first);
+  void* t0 = vec_ptr(s, s->inter[0], first);
+  void* t1 = vec_ptr(s, s->inter[1], first);
+  void* t2 = vec_ptr(s, s->inter[2], first);
   int nc = 0, nr = 0;
-  if (dw) { cb.f[nc++] = op(s->what[i], h->Tm[0], SM_ONE); rb.f[nr++] = op(h->Tm[0], dw, RM_ONE | pf); }
-  if (dvy) { cb.f[nc++] = op(s->psihat[i], h->Tm[2], SM_ONE); rb.f[nr++] = op(h->Tm[2], dvy, RM_NIKX_MEANY | pf); }
-  if (dvx) { cb.f[nc++] = op(s->psihat[i], h->Tm[3], SM_IKY_MEANX); rb.f[nr++] = op(h->Tm[3], dvx, RM_ONE | pf); }
+  if (dw) { cb.f[nc++] = op(what, t0, SM_ONE); rb.f[nr++] = op(t0, dw, RM_ONE | pf); }
+  if (dvy) { cb.f[nc++] = op(psihat, t1, SM_ONE); rb.f[nr++] = op(t1, dvy, RM_NIKX_MEANY | pf); }
+  if (dvx) { cb.f[nc++] = op(psihat, t2, SM_IKY_MEANX); rb.f[nr++] = op(t2, dvx, RM_ONE | pf); }
   if (nc == 0) return TTSH_OK;
-  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->tabS, s->v0[i], h->stream));
-  TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, s->v0[i], h->stream));
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->tabS, v0, h->stream, count, s->stride));
+  if (count == 1 || dst_stride == s->stride) {
+    TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, v0, h->stream, count, s->stride));
+  } else return TTSH_ERR_INVALID_ARG;
   h->launches += 2;
   return TTSH_OK;
 }
@@ -773,23 +791,24 @@ int ttsh_tangent_step(ttsh_tangent* s, int n) {
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
   for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
+  const int M = s->nvec;
+  const size_t ms = s->stride;
   for (int it = 0; it < n; ++it) {
     // base state in real space (permuted internal layout): R[0] = w, R[3] = v_x, R[4] = v_y
     int rc = enqueue_stage(h, TTSH_STAGE_INV_COL);
     if (rc == TTSH_OK) rc = enqueue_stage(h, TTSH_STAGE_INV_ROW);
     if (rc != TTSH_OK) return rc;
-    for (int i = 0; i < s->nvec; ++i) {
-      rc = tangent_inverse(s, i, s->real[0], s->real[1], s->real[2], true);        // dw, dv_x, dv_y
-      if (rc != TTSH_OK) return rc;
-      TRY(h, DISPATCH(h, launch_realspace_tangent, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, s->real[1], s->real[2], s->real[0], h->stream));
-      Batch rb = make_batch({op(s->real[1], h->Tm[0], RM_PERM), op(s->real[2], h->Tm[1], RM_PERM), op(s->real[0], h->Tm[2], RM_PERM)});
-      TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->stream));
-      Batch cb = make_batch({op(h->Tm[0], h->S[0], 0), op(h->Tm[1], h->S[1], 0), op(h->Tm[2], h->S[2], 0)});
-      TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 3, h->tabY, h->tabS, h->stream));
-      // lines 3-16 are linear: the same spectral kernel on the perturbation's (dw^, dpsi^, dv^(0))
-      TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, h->S[0], h->S[1], h->S[2], s->what[i], s->psihat[i], s->v0[i], h->stream));
-      h->launches += 4;
-    }
+    // all vectors at once: dw, dv_x, dv_y -> linearised lines 1-2 in place -> three forward transforms -> lines 3-16
+    rc = tangent_inverse(s, 0, M, s->real[0], s->real[1], s->real[2], true, ms);
+    if (rc != TTSH_OK) return rc;
+    TRY(h, DISPATCH(h, launch_realspace_tangent, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, s->real[1], s->real[2], s->real[0], h->stream, M, ms));
+    Batch rb = make_batch({op(s->real[1], s->inter[0], RM_PERM), op(s->real[2], s->inter[1], RM_PERM), op(s->real[0], s->inter[2], RM_PERM)});
+    TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->stream, M, ms));
+    Batch cb = make_batch({op(s->inter[0], s->spec[0], 0), op(s->inter[1], s->spec[1], 0), op(s->inter[2], s->spec[2], 0)});
+    TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 3, h->tabY, h->tabS, h->stream, M, ms));
+    // lines 3-16 are linear: the same spectral kernel on the perturbations' (dw^, dpsi^, dv^(0))
+    TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, s->spec[0], s->spec[1], s->spec[2], s->what, s->psihat, s->v0, h->stream, M, ms));
+    h->launches += 4;
     rc = ttsh_step(h, 1);
     if (rc != TTSH_OK) return rc;
   }
@@ -800,19 +819,25 @@ int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host) {
   ttsh_handle* h = s->h;
   if (h->sticky) return h->sticky;
   for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
-  // modified Gram-Schmidt, all coefficients stay on the device
+  // modified Gram-Schmidt, all coefficients stay on the device; row i of R in one batched launch per operation:
+  // r_ii = |q_i|, q_i /= r_ii, then r_ij = <q_i, q_j> and q_j -= r_ij q_i for all j > i together
   for (int i = 0; i < s->nvec; ++i) {
-    TRY(h, DISPATCH(h, launch_spec_dot, h->g, s->what[i], s->what[i], s->v0[i], s->v0[i], i, s->partial, s->rdiag, s->coef, h->stream));
-    TRY(h, DISPATCH(h, launch_spec_scale_axpy, h->g, s->coef, nullptr, s->what[i], nullptr, s->v0[i], h->stream));
+    void* qi = vec_ptr(s, s->what, i);
+    double* qi0 = vec_ptr(s, s->v0, i);
+    TRY(h, DISPATCH(h, launch_spec_dot, h->g, qi, qi, qi0, qi0, 1, 0, i, s->partial, s->rdiag, s->coef, h->stream));
+    TRY(h, DISPATCH(h, launch_spec_scale_axpy, h->g, s->coef, nullptr, qi, nullptr, qi0, 1, 0, h->stream));
     h->launches += 3;
-    for (int j = i + 1; j < s->nvec; ++j) {
-      TRY(h, DISPATCH(h, launch_spec_dot, h->g, s->what[i], s->what[j], s->v0[i], s->v0[j], -1, s->partial, s->rdiag, s->coef, h->stream));
-      TRY(h, DISPATCH(h, launch_spec_scale_axpy, h->g, s->coef, s->what[i], s->what[j], s->v0[i], s->v0[j], h->stream));
+    const int rest = s->nvec - i - 1;
+    if (rest > 0) {
+      void* qj = vec_ptr(s, s->what, i + 1);
+      double* qj0 = vec_ptr(s, s->v0, i + 1);
+      TRY(h, DISPATCH(h, launch_spec_dot, h->g, qi, qj, qi0, qj0, rest, s->stride, -1, s->partial, s->rdiag, s->coef, h->stream));
+      TRY(h, DISPATCH(h, launch_spec_scale_axpy, h->g, s->coef, qi, qj, qi0, qj0, rest, s->stride, h->stream));
       h->launches += 3;
     }
   }
   for (int i = 0; i < s->nvec; ++i) {
-    TRY(h, DISPATCH(h, launch_psi_from_w, h->g, s->what[i], s->psihat[i], h->stream));
+    TRY(h, DISPATCH(h, launch_psi_from_w, h->g, vec_ptr(s, s->what, i), vec_ptr(s, s->psihat, i), h->stream));
     h->launches++;
   }
   TRY(h, cudaMemcpyAsync(log_r_host, s->rdiag, (size_t)s->nvec * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -824,7 +849,7 @@ int ttsh_tangent_get_fields(ttsh_tangent* s, int i, void* dvx, void* dvy, void* 
   if (!s || i < 0 || i >= s->nvec) return TTSH_ERR_INVALID_ARG;
   if (s->h->sticky) return s->h->sticky;
   if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
-  return tangent_inverse(s, i, domega, dvx, dvy, false);
+  return tangent_inverse(s, i, 1, domega, dvx, dvy, false, 0);
 }
 int ttsh_tangent_destroy(ttsh_tangent* s) {
   delete s;

@@ -328,6 +328,40 @@ def measure_psd(torch, ttsh, name, nfreq, device, hbm_peak, reps=10):
             "workload": f"{name} {dtype}, {nfreq} frequencies: {nfreq * 2 * w * cfg.Nx * cfg.Ny / 2**20:.0f} MiB of accumulators (> L2)"}
 
 
+def measure_tangent(torch, ttsh, name, nvec, device, nsteps=100, qr_every=10):
+    """Lyapunov-exponent workload: nvec perturbations carried along the trajectory by ttsh_tangent_step,
+    re-orthonormalised every qr_every steps.  Reports the cost per step next to the plain ttsh_step."""
+    from paper_2304_03306_b200 import workloads
+    cfg, dtype = workload(name)
+    mask = cfg.mask()
+    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.baseline_params(), dtype, mask=mask, device=device)
+    s.set_velocity(*cfg.initial_velocity(mask))
+    tg = ttsh.Tangent(s, nvec)
+    for i in range(nvec):
+        tg.set(i, *workloads.gaussian_velocity(cfg.Nx, cfg.Ny, cfg.seed + 500 + i, 1.0))
+    tg.orthonormalize()
+    stream = torch.cuda.current_stream(device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tg.step(qr_every); tg.orthonormalize()
+    torch.cuda.synchronize(device)
+    acc = [0.0] * nvec
+    e0.record(stream)
+    for _ in range(nsteps // qr_every):
+        tg.step(qr_every)
+        acc = [a + b for a, b in zip(acc, tg.orthonormalize())]
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    ms = e0.elapsed_time(e1) / nsteps
+    e0.record(stream); s.step(nsteps); e1.record(stream)
+    torch.cuda.synchronize(device)
+    ms_base = e0.elapsed_time(e1) / nsteps
+    rates = [a / (nsteps * cfg.dt) for a in acc]
+    tg.close(); s.close()
+    return {"ms_per_step_with_qr": ms, "ms_per_plain_step": ms_base, "vectors": nvec, "qr_every": qr_every,
+            "growth_rates_over_window": [round(r, 6) for r in rates], "finite": bool(all(math.isfinite(r) for r in rates)),
+            "workload": f"{name} {dtype}, {nvec} tangent vectors, QR every {qr_every} steps, {nsteps} steps from the 1e-2 start"}
+
+
 def reduce_over_ranks(dist, maxima, sums, device="cpu"):
     """Replicas only: the job time is the MAX over ranks, counts are SUMMED.  No data-path collective."""
     if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
@@ -476,6 +510,7 @@ def main():
         for name, count in (("C1", 256), ("C2", 64), ("C3", 16), ("C3-f32", 16)):
             extra[f"{name} x{count} ensemble"] = measure_ensemble(torch, ttsh, name, count, device)
         extra["C3 temporal PSD, 64 frequencies"] = measure_psd(torch, ttsh, "C3", 64, device, peak)
+        extra["C2 Lyapunov, 8 vectors"] = measure_tangent(torch, ttsh, "C2", 8, device)
         line["other_workloads"] = extra
 
     if not a.no_cpu_baseline and world == 1:

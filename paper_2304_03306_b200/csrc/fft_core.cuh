@@ -392,7 +392,19 @@ __device__ __forceinline__ void fft_line(int j, cplx<T>* __restrict__ sm, const 
 // Twiddle tables (host: fill_stage_tables_wl): [6 base powers][R1] for stage 2 (indexed by k = t >> 4: a broadcast per
 // half-warp), then [6][TPL] for stage 3 stored in THREAD order (entry t holds W_N^{wl_j(t) power}: coalesced).
 // ---------------------------------------------------------------------------------------
-template <int N> __host__ __device__ constexpr bool fft_wl_supported() { return N == 4096 || N == 2048 || N == 1024; }
+// measured in k_row_step (B200, L = 1): the plan wins at N = 4096 (295 vs 316 us at C5); at N = 2048 the plain 16 x 16 x 8
+// plan is faster (141.9 vs 150.6 us at 2048 x 4096 fp64: the R1 = 8 first stage spills) and so is 16 x 8 x 8 at N = 1024 (65.9 vs
+// 74.4 us at 1024 x 4096 fp64; C3 36.8 -> 34.8 us per step): with one row pair per CTA several CTAs share an SM and hide each
+// other's barriers, which is what the warp-local exchange was for
+#ifndef TTSH_WL_2048
+#define TTSH_WL_2048 0
+#endif
+#ifndef TTSH_WL_1024
+#define TTSH_WL_1024 0
+#endif
+template <int N> __host__ __device__ constexpr bool fft_wl_supported() {
+  return N == 4096 || (N == 2048 && TTSH_WL_2048) || (N == 1024 && TTSH_WL_1024);
+}
 template <int N> __host__ __device__ constexpr int fft_wl_r1() { return N / 256; }
 __host__ __device__ constexpr int fft_wl_r1_rt(int N) { return N / 256; }
 __host__ __device__ constexpr int fft_wl_tw_elems_rt(int N) { return 6 * fft_wl_r1_rt(N) + 6 * (N / 16); }

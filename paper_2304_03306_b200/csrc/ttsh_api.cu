@@ -424,7 +424,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
   h->graph_exec = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
   h->row_step_ok = h->dtype == TTSH_F64 ? row_step_supported<double>(h->g) : row_step_supported<float>(h->g);
-  h->row_step_wl = Nx == 1024 || Nx == 2048 || Nx == 4096;
+  h->row_step_wl = (Nx == 1024 && TTSH_WL_1024) || (Nx == 2048 && TTSH_WL_2048) || Nx == 4096;
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
   std::vector<unsigned char> tx, ty, ts;

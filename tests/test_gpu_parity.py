@@ -463,3 +463,47 @@ def test_streaming_temporal_psd_matches_oracle(ttsh, Nx, Ny, dtype, nfreq, tol):
     w = o.get_fields()[2]
     assert n3 == 1 and abs(S3[0] - np.mean(w * w)) <= max(tol, 1e-9) * 10 * np.mean(w * w)   # one sample: S = mean(w^2) at every frequency
     psd.close(); s.close()
+
+
+# ---------------------------------------------------------------- other dealiasing fractions (reading R5) and the maximum grid size
+@pytest.mark.parametrize("num,den", [(2, 3), (1, 3), (1, 4), (3, 8)])
+@pytest.mark.parametrize("Nx,Ny", [(64, 128), (256, 64)])
+def test_other_dealias_fractions_match_oracle(ttsh, num, den, Nx, Ny):
+    """The cutoff fraction is a rational parameter (1/4 <= num/den <= 2/3; the paper's 1/2 is the default): the pruned
+    layouts, the general branch of the column passes and the 5-launch step (the fused row kernel is 1/2-rule only) against
+    the oracle with the same fraction.  Note that 2/3 is NOT alias-free for the cubic term: parity, not physics."""
+    from dataclasses import replace
+    dx, dt = 0.5, 0.01
+    mask = workloads.disk_mask(Nx, Ny, dx, 10.0)
+    vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 5, amplitude=1.0)
+    gp = ttsh.baseline_params()
+    gp.dealias_num, gp.dealias_den = num, den
+    op = replace(BASELINE_PRESET, dealias_num=num, dealias_den=den)
+    s = ttsh.Solver(Nx, Ny, dx, dt, gp, "f64", mask=mask)
+    o = TTSHOracle(Nx, Ny, dx, dt, op, mask=mask)
+    s.set_velocity(*vel); o.set_velocity(*vel)
+    compare_state(s, o, TOL_F64_1, f"{num}/{den} init")
+    s.step(1); o.step(1)
+    compare_state(s, o, TOL_F64_1, f"{num}/{den} step 1")
+    s.step(19); o.step(19)
+    compare_state(s, o, TOL_F64_100, f"{num}/{den} step 20")
+    s.set_advection_form(ttsh.TTSH_ADVECTION_LITERAL)
+    s.step(5); o.step(5)
+    compare_state(s, o, TOL_F64_100, f"{num}/{den} literal form")
+    s.close()
+
+
+@pytest.mark.parametrize("Nx,Ny,dtype", [(8192, 64, "f64"), (8192, 64, "f32"), (64, 8192, "f64"), (64, 8192, "f32")])
+def test_maximum_grid_dimension_8192(ttsh, Nx, Ny, dtype):
+    """Nx = 8192 (fp64: the row pair does not fit in shared memory -> the 5-launch step; fp32: the fused row kernel) and
+    Ny = 8192 (4096-point half-length column transforms), 3 steps against the FFT-backed oracle."""
+    dx, dt = 0.5, 0.01
+    mask = workloads.disk_mask(Nx, Ny, dx, 12.0)
+    vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 6, amplitude=1.0)
+    s, o = make_pair(ttsh, Nx, Ny, dx, dt, "baseline", mask, dtype=dtype, transform="fft", vel=vel)
+    if dtype == "f32":
+        o.K = s.debug_real(5).cpu().numpy().astype(np.float64)
+    s.step(3); o.step(3)
+    compare_state(s, o, TOL_F64_100 if dtype == "f64" else 3 * TOL_F32_1, f"{Nx}x{Ny} {dtype}")
+    assert s.diagnostics()["nonfinite"] == 0
+    s.close()

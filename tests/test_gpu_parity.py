@@ -507,3 +507,43 @@ def test_maximum_grid_dimension_8192(ttsh, Nx, Ny, dtype):
     compare_state(s, o, TOL_F64_100 if dtype == "f64" else 3 * TOL_F32_1, f"{Nx}x{Ny} {dtype}")
     assert s.diagnostics()["nonfinite"] == 0
     s.close()
+
+
+# ---------------------------------------------------------------- C2 as BASELINE.json states it: 20,000 steps, diagnostics every 100
+def test_C2_long_run_20000_steps_invariants(ttsh):
+    """No oracle can follow 20,000 steps (chaotic dynamics): properties that hold at any time instead —
+    finite fields, div v = 0 and sum(w) = 0 to round-off, bounded energy after saturation, small velocity deep inside the
+    masked region, and no growth of the anti-Hermitian part on the m_x = 0 column (reading R6: without the
+    symmetrisation of Alg. 1 line 12 a half-spectrum run is NaN by step ~12,000)."""
+    cfg = workloads.CONFIGS["C2"]
+    mask = cfg.mask()
+    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.baseline_params(), "f64", mask=mask)
+    s.set_velocity(*cfg.initial_velocity(mask))
+    energies = []
+    for _ in range(cfg.steps // 100):
+        s.step(100)
+        d = s.diagnostics()
+        assert d["nonfinite"] == 0 and np.isfinite(d["kinetic_energy"]) and np.isfinite(d["enstrophy"])
+        energies.append(d["kinetic_energy"])
+    assert d["step"] == cfg.steps and abs(d["t"] - cfg.steps * cfg.dt) < 1e-9
+    energies = np.asarray(energies)
+    assert energies[-1] > 1e3 * energies[0]              # the 1e-2 start has grown into the active state ...
+    assert energies.max() < 1.0 and d["max_speed"] < 5.0   # ... and saturated (|v| ~ sqrt(-alpha/beta) = 1 in the bulk)
+    assert energies[-50:].min() > 0.2 * energies[-50:].max()
+    vx, vy, w, psi = gpu_fields(s)
+    Ny, Nx = vx.shape
+    kx = 2 * np.pi * np.fft.fftfreq(Nx, d=cfg.dx)[None, :]
+    ky = 2 * np.pi * np.fft.fftfreq(Ny, d=cfg.dx)[:, None]
+    vxh, vyh = np.fft.fft2(vx), np.fft.fft2(vy)
+    div = np.fft.ifft2(1j * kx * vxh + 1j * ky * vyh).real
+    curl = np.fft.ifft2(1j * kx * vyh - 1j * ky * vxh).real
+    scale = np.abs(w).max()
+    assert np.abs(div).max() <= 1e-11 * scale and np.abs(curl - w).max() <= 1e-11 * scale
+    assert abs(w.mean()) <= 1e-13 * scale
+    # wall: beyond R plus half the wall thickness the speed is a small fraction of the interior's
+    i = np.arange(Nx)[None, :] - Nx // 2
+    j = np.arange(Ny)[:, None] - Ny // 2
+    r = np.hypot(i, j) * cfg.dx
+    speed = np.hypot(vx, vy)
+    assert speed[r > cfg.R + 0.5 * (Nx * cfg.dx / 2 - cfg.R)].max() < 1e-2 * speed[r < cfg.R].max()
+    s.close()

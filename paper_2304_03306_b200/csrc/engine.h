@@ -5,6 +5,19 @@
 
 namespace ttsh {
 
+// launch with programmatic dependent launch allowed (ttsh_common.cuh: pdl_wait / pdl_trigger); captured into CUDA graphs as a
+// programmatic dependency edge
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = TTSH_PDL;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // FFT passes (fft_passes.cuh).  nfields <= 5 fields per launch (grid.y).  Return cudaErrorInvalidValue for an
 // unsupported transform length.
 // Ensembles (ttsh_ensemble_step): `members` independent systems whose workspaces lie `mstride` bytes apart are advanced by

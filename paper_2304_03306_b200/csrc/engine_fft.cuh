@@ -31,12 +31,12 @@ template <typename T, int NY> static cudaError_t go_inv_col(const Geom& g, const
   if (G > 1 && 2 * items >= (long long)G * col_fill_ctas()) {          // several items per CTA once that still fills the GPU
     const long long ctas = (items + G - 1) / G;
     if (ctas > 65535) return cudaErrorInvalidValue;
-    k_inv_col<T, NY, G><<<dim3(2, (unsigned)ctas), G * C::THREADS, G * C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0, nf, members, mstride);
-    return cudaGetLastError();
+    return launch_pdl(k_inv_col<T, NY, G>, dim3(2, (unsigned)ctas), dim3(G * C::THREADS), G * C::SMEM, s, g, b, static_cast<const cplx<T>*>(tab),
+                      static_cast<const cplx<T>*>(tabS), v0, nf, members, mstride);
   }
   if (items > 65535) return cudaErrorInvalidValue;
-  k_inv_col<T, NY, 1><<<dim3(2, (unsigned)items), C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), v0, nf, members, mstride);
-  return cudaGetLastError();
+  return launch_pdl(k_inv_col<T, NY, 1>, dim3(2, (unsigned)items), dim3(C::THREADS), C::SMEM, s, g, b, static_cast<const cplx<T>*>(tab),
+                    static_cast<const cplx<T>*>(tabS), v0, nf, members, mstride);
 }
 template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, cudaStream_t s,
                                                             int members, size_t mstride) {
@@ -45,11 +45,11 @@ template <typename T, int NY> static cudaError_t go_fwd_col(const Geom& g, const
   constexpr int G = C::GMAX;
   if (items > 0x3fffffffLL) return cudaErrorInvalidValue;
   if (G > 1 && items >= (long long)G * col_fill_ctas()) {
-    k_fwd_col<T, NY, G><<<(unsigned)((items + G - 1) / G), G * C::THREADS, G * C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), nf, members, mstride);
-    return cudaGetLastError();
+    return launch_pdl(k_fwd_col<T, NY, G>, dim3((unsigned)((items + G - 1) / G)), dim3(G * C::THREADS), G * C::SMEM, s, g, b,
+                      static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), nf, members, mstride);
   }
-  k_fwd_col<T, NY, 1><<<(unsigned)items, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), static_cast<const cplx<T>*>(tabS), nf, members, mstride);
-  return cudaGetLastError();
+  return launch_pdl(k_fwd_col<T, NY, 1>, dim3((unsigned)items), dim3(C::THREADS), C::SMEM, s, g, b, static_cast<const cplx<T>*>(tab),
+                    static_cast<const cplx<T>*>(tabS), nf, members, mstride);
 }
 template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabS, const double* v0, cudaStream_t s,
                                                  int members, size_t mstride) {
@@ -177,10 +177,8 @@ static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, c
     if (nblk_ll > 0x3fffffff) return cudaErrorInvalidValue;
     const int nblk = (int)nblk_ll;
     const int grid = nblk < slots ? nblk : slots;
-    k_row_step<T, NX, LL, ENS><<<grid, C::THREADS, C::SMEM, s>>>(g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx, (const cplx<T>*)inPsi,
-                                                                 (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab),
-                                                                 v0, nblk, rpm, mstride);
-    return cudaGetLastError();
+    return launch_pdl(k_row_step<T, NX, LL, ENS>, dim3(grid), dim3(C::THREADS), C::SMEM, s, g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx,
+                      (const cplx<T>*)inPsi, (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab), v0, nblk, rpm, mstride);
   }
 }
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,

@@ -177,6 +177,8 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
     }
   }
 
+  pdl_wait();        // everything above touches only tables and addresses; the spectra below are the predecessor's output
+  pdl_trigger();
   {
     const int p = blockIdx.x;
     // a_p[mp] = (X[mp] + (-1)^p X[mp+NH]) W_Ny^{-p mp}; X[mp] is retained iff mp <= My, X[mp+NH] (my = mp-NH) iff
@@ -266,6 +268,8 @@ k_fwd_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
   cplx<T>* dneg = dst + (size_t)(Hy - NH + j) * L;
   constexpr size_t KS = (size_t)TPL * L;     // elements per slot
 
+  pdl_wait();
+  pdl_trigger();
 #pragma unroll 1
   for (int p = 0; p < 2; ++p) {
     const cplx<T>* in = src + (size_t)p * NH * L;

@@ -35,8 +35,7 @@ template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model&
                                                      double* v0, cudaStream_t s, int members, size_t mstride) {
   if (members > 65535) return cudaErrorInvalidValue;
   const dim3 grid((unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256), (unsigned)members);
-  k_spectral_p2<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)A, (const cplx<T>*)B, (cplx<T>*)w, (cplx<T>*)psi, v0, mstride);
-  return cudaGetLastError();
+  return launch_pdl(k_spectral_p2<T>, grid, dim3(256), 0, s, g, m, (const cplx<T>*)A, (const cplx<T>*)B, (cplx<T>*)w, (cplx<T>*)psi, v0, mstride);
 }
 template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, void* psi, double* v0, cudaStream_t s) {
   const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);

@@ -165,6 +165,8 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_spectral_p2(Geom g, Model m, const cplx<T>* __restrict__ A_, const cplx<T>* __restrict__ B_, cplx<T>* w_,
               cplx<T>* __restrict__ psi_, double* v0_, size_t mstride) {
+  pdl_wait();
+  pdl_trigger();
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
   const size_t moff = (size_t)blockIdx.y * mstride;      // ensemble member (bytes); 0 outside ensembles

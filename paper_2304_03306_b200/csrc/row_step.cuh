@@ -154,7 +154,7 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
   const int Wx = g.Wx;
   const T scale_i = (T)g.inv_sqrt_nx, scale_f = (T)g.inv_sqrt_nx;
   const T dkx = (T)g.dkx;
-  T meany = (T)(v0[1] * g.inv_sqrt_ny);
+  T meany = (T)0;                                            // v^_y(0) / sqrt(Ny): read after pdl_wait (the predecessor writes v0)
   // global row pair -> (row pair of its member, byte offset of the member's workspace)
   auto locate = [&](int rpg, int& rp_, size_t& mo_) {
     if constexpr (ENS) { const int mb = rpg / rpm; rp_ = rpg - mb * rpm; mo_ = (size_t)mb * mstride; }
@@ -170,6 +170,9 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
   if (leader) { mbar_init(bar0, 1); mbar_init(bar1, 1); }
   mbar_fence_init();
   __syncthreads();
+  pdl_wait();          // inputs, K and v0 below are written by the preceding launches
+  pdl_trigger();
+  if constexpr (!ENS) meany = (T)(v0[1] * g.inv_sqrt_ny);
   if (leader && (int)blockIdx.x < nblk) {
     int rp0; size_t mo0;
     locate(blockIdx.x * C::L + c, rp0, mo0);

@@ -30,6 +30,33 @@ template <typename T> __device__ __forceinline__ cplx<T> mul_conj(cplx<T> a, cpl
 }
 
 // ---------------------------------------------------------------------------------------
+// programmatic dependent launch: the four kernels of a step are launched with the programmatic-stream-serialization
+// attribute (engine.h: launch_pdl), so the next kernel's CTAs are scheduled while the last wave of the previous one drains
+// and run their prologue (index arithmetic, twiddle loads, mbarrier set-up) early; pdl_wait() blocks until the previous grid
+// has completed and its writes are visible, and must precede the first access to anything a predecessor writes.
+// Both are no-ops in a kernel launched without the attribute.
+// ---------------------------------------------------------------------------------------
+#ifndef TTSH_PDL
+#define TTSH_PDL 1
+#endif
+__device__ __forceinline__ void pdl_wait() {
+#if TTSH_PDL
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
+// Measured (B200): with the implicit trigger at kernel exit the attribute saves the launch latency at every kernel boundary
+// (C5 fp64 425.4 -> 416.0 us per step, 256^2 21.4 -> 20.5 us); an explicit early trigger (TTSH_PDL_TRIGGER = 1: dependents
+// become resident while the last wave still runs) was slower everywhere (C5 453 us, 1024^2 34.8 -> 46.5 us) and is off.
+#ifndef TTSH_PDL_TRIGGER
+#define TTSH_PDL_TRIGGER 0
+#endif
+__device__ __forceinline__ void pdl_trigger() {
+#if TTSH_PDL && TTSH_PDL_TRIGGER
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
+}
+
+// ---------------------------------------------------------------------------------------
 // grid geometry (host-filled, passed by value) and the HBM layouts
 //
 //   real fields       scalar[Ny][Nx], x contiguous.

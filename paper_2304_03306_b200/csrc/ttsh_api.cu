@@ -485,7 +485,10 @@ int ttsh_step(ttsh_handle* h, int n) {
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   if (n == 0) return TTSH_OK;
   // Small grids are launch-latency bound: replay one captured step.  Large grids launch directly.
-  const bool use_graph = (size_t)h->Nx * h->Ny <= (size_t)1024 * 1024 && n >= 4;
+#ifndef TTSH_GRAPH_MAX_POINTS
+#define TTSH_GRAPH_MAX_POINTS (1024 * 1024)
+#endif
+  const bool use_graph = (size_t)h->Nx * h->Ny <= (size_t)TTSH_GRAPH_MAX_POINTS && n >= 4;
   if (use_graph && !h->graph_ok) {
     // capture on a private stream (the caller's may be the legacy default stream, which cannot capture);
     // the instantiated graph is then replayed on the caller's stream.

@@ -88,15 +88,13 @@ template <typename T, int NX> static cudaError_t go_inv_row(const Geom& g, const
                                                             int members, size_t mstride) {
   using C = RowCfg<T, NX>;
   dim3 grid((g.Ny / 2) / C::L, nf, members);
-  k_inv_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), v0, mstride);
-  return cudaGetLastError();
+  return launch_pdl(k_inv_row<T, NX>, grid, dim3(C::THREADS), C::SMEM, s, g, b, static_cast<const cplx<T>*>(tab), v0, mstride);
 }
 template <typename T, int NX> static cudaError_t go_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s,
                                                             int members, size_t mstride) {
   using C = RowCfg<T, NX>;
   dim3 grid((g.Ny / 2) / C::L, nf, members);
-  k_fwd_row<T, NX><<<grid, C::THREADS, C::SMEM, s>>>(g, b, static_cast<const cplx<T>*>(tab), mstride);
-  return cudaGetLastError();
+  return launch_pdl(k_fwd_row<T, NX>, grid, dim3(C::THREADS), C::SMEM, s, g, b, static_cast<const cplx<T>*>(tab), mstride);
 }
 template <typename T, int NX> static size_t fused_smem(const Geom& g) {
   return RowCfg<T, NX>::SMEM + (size_t)RowCfg<T, NX>::L * 2 * ((g.Wx + 3) & ~3) * sizeof(cplx<T>);
@@ -105,9 +103,8 @@ template <typename T, int NX> static cudaError_t go_fwd_row_fused(const Geom& g,
                                                                   const void* w, const void* K, void* oA, void* oB,
                                                                   const void* tab, cudaStream_t s) {
   using C = RowCfg<T, NX>;
-  k_fwd_row_fused<T, NX><<<(g.Ny / 2) / C::L, C::THREADS, fused_smem<T, NX>(g), s>>>(
-      g, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab));
-  return cudaGetLastError();
+  return launch_pdl(k_fwd_row_fused<T, NX>, dim3((g.Ny / 2) / C::L), dim3(C::THREADS), fused_smem<T, NX>(g), s, g, m, (const T*)vx, (const T*)vy,
+                    (const T*)w, (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab));
 }
 template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
                                                        const void* K, void* oA, void* oB, const void* tab, cudaStream_t s) {

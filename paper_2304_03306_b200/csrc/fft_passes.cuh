@@ -321,6 +321,7 @@ __global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
 k_inv_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabX,
           const double* __restrict__ v0_, size_t mstride) {
   using C = RowCfg<T, NX>;
+  pdl_wait();      // launched with programmatic dependent launch: inputs and v0 come from the preceding kernels
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -415,6 +416,7 @@ template <typename T, int NX>
 __global__ void __launch_bounds__(RowCfg<T, NX>::THREADS, RowCfg<T, NX>::MINB)
 k_fwd_row(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, const cplx<T>* __restrict__ tabX, size_t mstride) {
   using C = RowCfg<T, NX>;
+  pdl_wait();
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -485,6 +487,7 @@ k_fwd_row_fused(const __grid_constant__ Geom g, const __grid_constant__ Model m,
                 const T* __restrict__ vy, const T* __restrict__ w, const T* __restrict__ K, cplx<T>* __restrict__ outA,
                 cplx<T>* __restrict__ outB, const cplx<T>* __restrict__ tabX) {
   using C = RowCfg<T, NX>;
+  pdl_wait();
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);

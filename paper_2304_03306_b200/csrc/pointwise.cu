@@ -28,8 +28,7 @@ template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m,
                                                   void* w, void* psi, double* v0, cudaStream_t s, int members, size_t mstride) {
   if (members < 1 || members > 65535) return cudaErrorInvalidValue;
   const dim3 grid((unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256), (unsigned)members);
-  k_spectral<T><<<grid, 256, 0, s>>>(g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, (cplx<T>*)psi, v0, mstride);
-  return cudaGetLastError();
+  return launch_pdl(k_spectral<T>, grid, dim3(256), 0, s, g, m, (const cplx<T>*)Fx, (const cplx<T>*)Fy, (const cplx<T>*)S, (cplx<T>*)w, (cplx<T>*)psi, v0, mstride);
 }
 template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model& m, const void* A, const void* B, void* w, void* psi,
                                                      double* v0, cudaStream_t s, int members, size_t mstride) {
@@ -111,26 +110,22 @@ template <typename T> cudaError_t launch_realspace_tangent(const Geom& g, const 
   if (members < 1 || members > 65535) return cudaErrorInvalidValue;
   const size_t nvec = (size_t)g.Nx * g.Ny / Vec<T>::n;
   const dim3 grid((unsigned)blocks_for(nvec, 256, GRID_CAP), (unsigned)members);
-  k_realspace_tangent<T><<<grid, 256, 0, s>>>(nvec, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K, (T*)dvx, (T*)dvy, (T*)dw, mstride);
-  return cudaGetLastError();
+  return launch_pdl(k_realspace_tangent<T>, grid, dim3(256), 0, s, nvec, m, (const T*)vx, (const T*)vy, (const T*)w, (const T*)K, (T*)dvx, (T*)dvy, (T*)dw, mstride);
 }
 // count = 1, norm_slot >= 0:  rdiag[norm_slot] <- |a|, coef[0] <- 1/|a|   (b = a)
 // norm_slot < 0:              coef[j] <- <a, b_j>, b_j = b + j * bstride bytes, j < count;  partial: DIAG_BLOCKS * count doubles
 template <typename T> cudaError_t launch_spec_dot(const Geom& g, const void* a, const void* b, const double* a0, const double* b0,
                                                   int count, size_t bstride, int norm_slot, double* partial, double* rdiag,
                                                   double* coef, cudaStream_t s) {
-  k_spec_dot_partial<T><<<dim3(DIAG_BLOCKS, count), 256, 0, s>>>(g, (const cplx<T>*)a, (const cplx<T>*)b, partial, bstride);
-  cudaError_t e = cudaGetLastError();
+  cudaError_t e = launch_pdl(k_spec_dot_partial<T>, dim3(DIAG_BLOCKS, count), dim3(256), 0, s, g, (const cplx<T>*)a, (const cplx<T>*)b, partial, bstride);
   if (e != cudaSuccess) return e;
-  k_spec_dot_final<<<count, 32, 0, s>>>(DIAG_BLOCKS, partial, a0, b0, bstride, norm_slot, rdiag, coef);
-  return cudaGetLastError();
+  return launch_pdl(k_spec_dot_final, dim3(count), dim3(32), 0, s, (int)DIAG_BLOCKS, (const double*)partial, a0, b0, bstride, norm_slot, rdiag, coef);
 }
 // y_j <- coef[j] y_j (x == NULL) or y_j <- y_j - coef[j] x, j < count, on the spectrum and the mean flow
 template <typename T> cudaError_t launch_spec_scale_axpy(const Geom& g, const double* coef, const void* x, void* y, const double* x0,
                                                          double* y0, int count, size_t ystride, cudaStream_t s) {
   const size_t n = (size_t)g.NT * g.Hy * g.CW;
-  k_spec_scale_axpy<T><<<dim3(blocks_for(n, 256, GRID_CAP), count), 256, 0, s>>>(n, coef, (const cplx<T>*)x, (cplx<T>*)y, x0, y0, ystride);
-  return cudaGetLastError();
+  return launch_pdl(k_spec_scale_axpy<T>, dim3(blocks_for(n, 256, GRID_CAP), count), dim3(256), 0, s, n, coef, (const cplx<T>*)x, (cplx<T>*)y, x0, y0, ystride);
 }
 
 #define INST(T) \

@@ -108,6 +108,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx_, const cplx<T>* __restrict__ Fy_,
            const cplx<T>* __restrict__ S_, cplx<T>* w_, cplx<T>* __restrict__ psi_, double* v0_, size_t mstride) {
+  pdl_wait();
   // threads enumerate the tile-major array in memory order: idx = (t Hy + q) CW + c
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
@@ -536,6 +537,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_realspace_tangent(size_t nvec, Model m, const T* __restrict__ vx, const T* __restrict__ vy, const T* __restrict__ w,
                     const T* __restrict__ K, T* __restrict__ dvx_, T* __restrict__ dvy_, T* __restrict__ dw_, size_t mstride) {
+  pdl_wait();
   const size_t moff = (size_t)blockIdx.y * mstride;      // tangent vector (bytes); the base fields and K are shared
   T* __restrict__ dvx = reinterpret_cast<T*>(reinterpret_cast<char*>(dvx_) + moff);
   T* __restrict__ dvy = reinterpret_cast<T*>(reinterpret_cast<char*>(dvy_) + moff);
@@ -570,6 +572,7 @@ k_realspace_tangent(size_t nvec, Model m, const T* __restrict__ vx, const T* __r
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_spec_dot_partial(Geom g, const cplx<T>* __restrict__ a, const cplx<T>* __restrict__ b_, double* __restrict__ partial, size_t bstride) {
+  pdl_wait();
   // grid.y = vector j of a batch <a, b_j>, b_j = b_ + j * bstride bytes;  partial[j][gridDim.x]
   const cplx<T>* __restrict__ b = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(b_) + (size_t)blockIdx.y * bstride);
   const size_t n = (size_t)g.NT * g.Hy * g.CW;
@@ -599,6 +602,7 @@ k_spec_dot_partial(Geom g, const cplx<T>* __restrict__ a, const cplx<T>* __restr
 __global__ void __launch_bounds__(32)
 k_spec_dot_final(int nblocks, const double* __restrict__ partial, const double* __restrict__ a0, const double* __restrict__ b0_,
                  size_t bstride, int norm_slot, double* __restrict__ rdiag, double* __restrict__ coef_) {
+  pdl_wait();
   const double* __restrict__ b0 = reinterpret_cast<const double*>(reinterpret_cast<const char*>(b0_) + (size_t)blockIdx.x * bstride);
   double* __restrict__ coef = coef_ + blockIdx.x;
   double sum = 0.0;
@@ -619,6 +623,7 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_spec_scale_axpy(size_t n, const double* __restrict__ coef_, const cplx<T>* __restrict__ x, cplx<T>* __restrict__ y_,
                   const double* __restrict__ x0, double* __restrict__ y0_, size_t ystride) {
+  pdl_wait();
   // grid.y = vector j of a batch: y_j = y_ + j * ystride bytes, coefficient coef_[j]
   const double* __restrict__ coef = coef_ + blockIdx.y;
   cplx<T>* __restrict__ y = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(y_) + (size_t)blockIdx.y * ystride);

@@ -50,7 +50,10 @@ template <typename T, int NX> struct RowCfg {
 // of shared memory (fp64 4096: 2 columns, fp32 4096: 4), at least 2 and at most 8 columns
 __host__ __device__ constexpr int col_tile_width(int Ny, int elem_bytes) {
   int cw = (TTSH_COL_BYTES / elem_bytes) / (Ny / 2);
-  const int cap = Ny >= 2048 ? 8 : 4;      // small grids: more, smaller CTAs (the GPU has 148 SMs to fill)
+#ifndef TTSH_COL_CAP_SMALL
+#define TTSH_COL_CAP_SMALL 4
+#endif
+  const int cap = Ny >= 2048 ? 8 : TTSH_COL_CAP_SMALL;      // small grids: more, smaller CTAs (the GPU has 148 SMs to fill)
   return cw < 2 ? 2 : (cw > cap ? cap : cw);
 }
 template <typename T, int NY> struct ColCfg {

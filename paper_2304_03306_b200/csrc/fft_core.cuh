@@ -424,6 +424,10 @@ template <typename T, int N> __device__ __forceinline__ int fft_wl_rot(int r, in
 }
 __host__ __device__ __forceinline__ int fft_wl_j_rt(int t, int r1) { return (t >> 4) + r1 * (t & 15); }
 template <int N> __device__ __forceinline__ int fft_wl_j(int t) { return (t >> 4) + fft_wl_r1<N>() * (t & 15); }
+// timing probes (_work only, never defined in the product build): TTSH_PROBE_NO_DFT drops the butterflies, TTSH_PROBE_NO_XCHG the
+// shared-memory exchanges of the warp-local plan; results are then wrong, only the kernel time is of interest
+template <typename T> __device__ __forceinline__ void keep_alive(cplx<T>& z) { asm volatile("" : "+d"(z.x), "+d"(z.y)); }
+__device__ __forceinline__ void keep_alive(cplx<float>& z) { asm volatile("" : "+f"(z.x), "+f"(z.y)); }
 template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store, class Hook = NoHook>
 __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tabw,
                                             Load load, Store store, Hook hook = Hook()) {
@@ -447,15 +451,21 @@ __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__
         v[k % NB][k / NB] = load.finish(j0 + k * TPL, k, raw[s]);
       }
     }
+#ifndef TTSH_PROBE_NO_DFT
 #pragma unroll
     for (int b = 0; b < NB; ++b) dftR<R1, DIR>(v[b]);
+#endif
     __syncthreads();                           // every thread has finished reading this buffer (previous transform)
     hook();
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       const int base = (j0 + b * TPL) * R1;
 #pragma unroll
+#ifndef TTSH_PROBE_NO_XCHG
       for (int r = 0; r < R1; ++r) sm[fft_wl_pad<T, N>(base + r)] = v[b][r];
+#else
+      for (int r = 0; r < R1; ++r) keep_alive(v[b][r]);
+#endif
     }
     __syncthreads();
   }
@@ -463,18 +473,32 @@ __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__
   const int kk = t >> 4, q = t & 15;
   const int j = kk + R1 * q;
   cplx<T> v[16];
+#ifndef TTSH_PROBE_NO_XCHG
 #pragma unroll
   for (int r = 0; r < 16; ++r) v[r] = sm[fft_wl_pad<T, N>(j + r * TPL)];
+#else
+#pragma unroll
+  for (int r = 0; r < 16; ++r) v[r] = mk<T>((T)(j + r), (T)t);
+#endif
+#ifndef TTSH_PROBE_NO_DFT
   apply_stage_twiddles<16, DIR>(v, tabw + kk, R1);
   dft16<DIR>(v);
+#endif
   __syncwarp();                                // the group's 256 positions have been read by its 16 threads
+#ifndef TTSH_PROBE_NO_XCHG
 #pragma unroll
   for (int r = 0; r < 16; ++r) sm[fft_wl_pad<T, N>(TPL * q + kk + R1 * fft_wl_rot<T, N>(r, q))] = v[r];
   __syncwarp();
 #pragma unroll
   for (int qq = 0; qq < 16; ++qq) v[qq] = sm[fft_wl_pad<T, N>(TPL * qq + kk + R1 * fft_wl_rot<T, N>(q, qq))];
+#else
+#pragma unroll
+  for (int r = 0; r < 16; ++r) keep_alive(v[r]);
+#endif
+#ifndef TTSH_PROBE_NO_DFT
   apply_stage_twiddles<16, DIR>(v, tabw + 6 * R1 + t, TPL);
   dft16<DIR>(v);
+#endif
   if (SYNC_LAST) __syncthreads();              // the store goes to shared memory: every group has finished reading it
 #pragma unroll
   for (int r = 0; r < 16; ++r) store(j + r * TPL, r, v[r]);

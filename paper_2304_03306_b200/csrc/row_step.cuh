@@ -44,7 +44,10 @@ template <typename T, int NX, int LL = 1> struct RowStepCfg {
   static constexpr size_t OFF_SLOTS = ((size_t)L * (LS + ST) * sizeof(cplx<T>) + 127) / 128 * 128;
   static constexpr size_t OFF_BARS = OFF_SLOTS + (size_t)L * 2 * SLOT;
   static constexpr size_t SMEM = OFF_BARS + (size_t)L * 2 * sizeof(unsigned long long);
-  static constexpr int MINB = 1;
+#ifndef TTSH_RS_MINB_F32
+#define TTSH_RS_MINB_F32 1
+#endif
+  static constexpr int MINB = (sizeof(T) == 4 && NX == 4096) ? TTSH_RS_MINB_F32 : 1;
   static constexpr bool FITS = SMEM <= 227 * 1024;
 };
 

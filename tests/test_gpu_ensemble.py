@@ -176,3 +176,46 @@ def test_ensemble_argument_validation(ttsh):
     ens3.close()
     for s in (a, b, c, d32, other):
         s.close()
+
+
+def test_C3_radius_sweep_and_C4_separation_sweep_as_ensembles_10000_steps(ttsh):
+    """BASELINE.json configs[2] and [3] as they are stated: the disk-radius sweep R in {40, 80, 160, 240} at 1024^2 and the
+    dumbbell separation sweep d in {80, 100, 110, 118} at 1024 x 2048, 10,000 steps each — run as 4-member ensembles.  No
+    oracle can follow that far (chaos): finite fields, saturated energies, the confined kinetic energy grows with the
+    unmasked area, member 0 stays bit-identical to the same system stepped alone for the first 200 steps, and Psi_2 of every
+    dumbbell is a valid order parameter."""
+    p = ttsh.baseline_params()
+    for name in ("C3", "C4"):
+        cfg = workloads.CONFIGS[name]
+        sweep = cfg.sweep
+        masks = [cfg.mask(R=r) if name == "C3" else cfg.mask(d=r) for r in sweep]
+        vels = [workloads.gaussian_velocity(cfg.Nx, cfg.Ny, cfg.seed + 10 * i, 1e-2, masks[i]) for i in range(len(sweep))]
+        ens = ttsh.Ensemble(len(sweep), cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, p, "f64", masks=masks)
+        alone = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, p, "f64", mask=masks[0])
+        for i, m in enumerate(ens.members):
+            m.set_velocity(*vels[i])
+        alone.set_velocity(*vels[0])
+        ens.step(200); alone.step(200)
+        for a, b in zip(fields(ens.members[0]), fields(alone)):
+            assert np.array_equal(a, b)
+        alone.close()
+        for _ in range((cfg.steps - 200) // 1400):
+            ens.step(1400)
+            for m in ens.members:
+                d = m.diagnostics()
+                assert d["nonfinite"] == 0 and np.isfinite(d["kinetic_energy"])
+        diags = [m.diagnostics() for m in ens.members]
+        assert all(d["step"] == cfg.steps for d in diags)
+        E = [d["kinetic_energy"] for d in diags]
+        assert all(1e-4 < e < 1.0 for e in E) and all(d["max_speed"] < 5.0 for d in diags)
+        if name == "C3":
+            assert E[0] < E[1] < E[2] < E[3]              # energy per unit box area follows the unmasked area (R^2)
+        else:
+            for i, m in enumerate(ens.members):
+                dsep = sweep[i]
+                cl = ((cfg.Nx // 2) * cfg.dx - dsep / 2, (cfg.Ny // 2) * cfg.dx)
+                cr = ((cfg.Nx // 2) * cfg.dx + dsep / 2, (cfg.Ny // 2) * cfg.dx)
+                o = m.dumbbell_order(cl, cr, dsep / 2)
+                assert 0.0 <= o["psi2"] <= 1.0 and o["index_left"] >= 0 and o["index_right"] >= 0
+                assert abs(o["omega_left"]) > 0 and abs(o["omega_right"]) > 0
+        ens.close()

@@ -547,3 +547,32 @@ def test_C2_long_run_20000_steps_invariants(ttsh):
     speed = np.hypot(vx, vy)
     assert speed[r > cfg.R + 0.5 * (Nx * cfg.dx / 2 - cfg.R)].max() < 1e-2 * speed[r < cfg.R].max()
     s.close()
+
+
+@pytest.mark.parametrize("name,dtype", [("C5", "f64"), ("C5p", "f32")])
+def test_C5_2000_steps_invariants(ttsh, name, dtype):
+    """BASELINE.json configs[4] as stated: 4096 x 4096, 2,000 steps (disk R = 900 in fp64, unconfined in fp32), in the launch
+    configuration bench.py times.  Properties that hold at any size and time: finite fields, div v = 0 and sum(w) = 0 to
+    round-off of the dtype, the linear growth of the small random start (every retained mode grows or decays by
+    exp(sigma(k) t) while the field is small, so the energy rises and stays far below saturation after t = 20)."""
+    cfg = workloads.CONFIGS[name]
+    mask = cfg.mask()
+    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.baseline_params(), dtype, mask=mask)
+    s.set_velocity(*cfg.initial_velocity(mask))
+    e0 = s.diagnostics()["kinetic_energy"]
+    for _ in range(cfg.steps // 500):
+        s.step(500)
+        d = s.diagnostics()
+        assert d["nonfinite"] == 0 and np.isfinite(d["kinetic_energy"]) and np.isfinite(d["enstrophy"])
+    assert d["step"] == cfg.steps and d["kinetic_energy"] > 10 * e0 and d["max_speed"] < 5.0
+    vx, vy, w, _ = gpu_fields(s)
+    kx = 2 * np.pi * np.fft.rfftfreq(cfg.Nx, d=cfg.dx)[None, :]
+    ky = 2 * np.pi * np.fft.fftfreq(cfg.Ny, d=cfg.dx)[:, None]
+    vxh, vyh = np.fft.rfft2(vx), np.fft.rfft2(vy)
+    div = np.fft.irfft2(1j * kx * vxh + 1j * ky * vyh, s=vx.shape)
+    curl = np.fft.irfft2(1j * kx * vyh - 1j * ky * vxh, s=vx.shape)
+    scale = np.abs(w).max()
+    eps = 1e-11 if dtype == "f64" else 2e-4
+    assert np.abs(div).max() <= eps * scale and np.abs(curl - w).max() <= eps * scale
+    assert abs(w.mean()) <= eps * scale
+    s.close()

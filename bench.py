@@ -362,6 +362,31 @@ def measure_tangent(torch, ttsh, name, nvec, device, nsteps=100, qr_every=10):
             "workload": f"{name} {dtype}, {nvec} tangent vectors, QR every {qr_every} steps, {nsteps} steps from the 1e-2 start"}
 
 
+def measure_cufft_reference(torch, cfg, dtype, device, reps=10):
+    """north_star: 'cuFFT serves only as a side-by-side reference'.  The transforms of ONE Euler step in the conservative form
+    (3 inverse + 3 forward dense 2-D real transforms, the paper's own design) through torch.fft = cuFFT, without
+    any of the element-wise work, next to our whole step."""
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    x = torch.randn(3, cfg.Ny, cfg.Nx, dtype=tdt, device=device)
+    stream = torch.cuda.current_stream(device)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def six():
+        X = torch.fft.rfft2(x, norm="ortho")
+        return torch.fft.irfft2(X, s=(cfg.Ny, cfg.Nx), norm="ortho")
+
+    six(); six()
+    torch.cuda.synchronize(device)
+    e0.record(stream)
+    for _ in range(reps):
+        y = six()
+    e1.record(stream)
+    torch.cuda.synchronize(device)
+    ms = e0.elapsed_time(e1) / reps
+    del y
+    return {"ms_for_3_rfft2_plus_3_irfft2": ms, "workload": f"dense {cfg.Nx}x{cfg.Ny} {dtype} transforms of one step via torch.fft (cuFFT)"}
+
+
 def reduce_over_ranks(dist, maxima, sums, device="cpu"):
     """Replicas only: the job time is the MAX over ranks, counts are SUMMED.  No data-path collective."""
     if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
@@ -511,6 +536,7 @@ def main():
             extra[f"{name} x{count} ensemble"] = measure_ensemble(torch, ttsh, name, count, device)
         extra["C3 temporal PSD, 64 frequencies"] = measure_psd(torch, ttsh, "C3", 64, device, peak)
         extra["C2 Lyapunov, 8 vectors"] = measure_tangent(torch, ttsh, "C2", 8, device)
+        extra["cuFFT side-by-side (reference only, never in the product path)"] = measure_cufft_reference(torch, cfg, dtype, device)
         line["other_workloads"] = extra
 
     if not a.no_cpu_baseline and world == 1:

@@ -17,7 +17,7 @@
 //   slot 0:  w~  ->  psi~  ->  K(y_B)  ->  w~ of the next row pair        slot 1:  v_x~  ->  K(y_A)  ->  v_x~ of the next row pair
 // so no thread ever waits on a global load; the first-stage loaders and the pointwise phase read shared memory.
 //
-// For Nx = 1024, 2048, 4096 the transforms use the warp-local plan of fft_core.cuh (one CTA-wide exchange per transform);
+// For Nx = 4096 (where fft_wl_supported) the transforms use the warp-local plan of fft_core.cuh (one CTA-wide exchange per transform);
 // the thread then owns x = wl_j(j) + k TPL, K is read from its thread-order copy (perm_index_wl) and tabX is the
 // warp-local twiddle table.
 // Packing by rows (f(y_A) + i f(y_B)) makes i k_x commute with the packing, so A~ is formed BEFORE the unpack:

@@ -233,7 +233,7 @@ def test_C3_C4_100_steps_against_fft_backed_oracle(ttsh, name):
 
 
 def test_C4_shape_fp32_single_step(ttsh):
-    """Nx = 2048 in fp32 (the warp-local row plan with two lines per CTA), dumbbell mask, one step <= 1e-5."""
+    """Nx = 2048 in fp32 (the fused row kernel with the plain 16 x 16 x 8 plan), dumbbell mask, one step <= 1e-5."""
     cfg = workloads.CONFIGS["C4"]
     mask = cfg.mask()
     vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0)

@@ -576,3 +576,39 @@ def test_C5_2000_steps_invariants(ttsh, name, dtype):
     assert np.abs(div).max() <= eps * scale and np.abs(curl - w).max() <= eps * scale
     assert abs(w.mean()) <= eps * scale
     s.close()
+
+
+# ---------------------------------------------------------------- the widening kernels at BASELINE's full sizes
+def test_full_size_psd_at_C3_and_dumbbell_order_at_C4(ttsh):
+    """ttsh_psd_* at 1024 x 1024 with 64 frequencies (the configuration bench.py times: 1 GiB of accumulators) and
+    ttsh_dumbbell_order at 1024 x 2048, against the oracle (FFT-backed transforms, locked to the matrix DFT by the pins)."""
+    from oracle import temporal_psd
+    cfg = workloads.CONFIGS["C3"]
+    mask = cfg.mask()
+    vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=1.0)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, transform="fft", vel=vel)
+    omegas = [0.05 * m for m in range(64)]
+    psd = ttsh.TemporalPSD(s, omegas)
+    series, times = [], []
+    for _ in range(4):
+        psd.accumulate()
+        series.append(o.get_fields()[2]); times.append(o.t)
+        s.step(2); o.step(2)
+    S, n = psd.result()
+    ref = temporal_psd(series, times, omegas)
+    assert n == 4 and np.max(np.abs(np.asarray(S) - ref)) <= 1e-10 * ref.max()
+    psd.close(); s.close()
+
+    cfg = workloads.CONFIGS["C4"]
+    mask = cfg.mask()
+    cl = ((cfg.Nx // 2) * cfg.dx - cfg.d / 2, (cfg.Ny // 2) * cfg.dx)
+    cr = ((cfg.Nx // 2) * cfg.dx + cfg.d / 2, (cfg.Ny // 2) * cfg.dx)
+    vel = _vortex_pair_velocity(cfg.Nx, cfg.Ny, cfg.dx, cl, cr, 1.0, -0.8)
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "baseline", mask, transform="fft", vel=vel)
+    s.step(3); o.step(3)
+    g, r = s.dumbbell_order(cl, cr, cfg.d / 2), o.dumbbell_order(cl, cr, cfg.d / 2)
+    assert g["index_left"] == r["index_left"] and g["index_right"] == r["index_right"]
+    wmax = max(abs(r["omega_left"]), abs(r["omega_right"]))
+    assert abs(g["omega_left"] - r["omega_left"]) <= 1e-9 * wmax and abs(g["omega_right"] - r["omega_right"]) <= 1e-9 * wmax
+    assert abs(g["psi2"] - r["psi2"]) <= 1e-9 and g["psi2"] < 0.5
+    s.close()

@@ -361,6 +361,53 @@ def test_vortex_order_parameter_limits_and_parseval():
     assert d0["vortex_order"] == 0.0 and d0["polar_order"] == 0.0
 
 
+def test_diagnostics_centre_on_a_non_square_grid_and_both_mean_components():
+    """Eq. (11) about a centre with cx != cy on a non-square grid: a field that is azimuthal about
+    (cx, cy) gives Psi = 1 only about that centre (a swapped or transposed centre does not); mean_vx and mean_vy are
+    distinct numbers; max_speed and the sums follow the closed forms of a hand-built field."""
+    Nx, Ny, dx = 96, 48, 0.5
+    o = TTSHOracle(Nx, Ny, dx, 0.01, BASELINE_PRESET)
+    cx, cy = 30 * dx, 11 * dx                                               # grid points, cx != cy, neither the box centre
+    x = np.arange(Nx)[None, :] * dx - cx; y = np.arange(Ny)[:, None] * dx - cy
+    r = np.hypot(x, y); rs = np.where(r == 0, 1.0, r)
+    o.w_hat = np.zeros((Ny, Nx), complex)
+    o.v = np.stack([-y / rs * np.exp(-0.3 * r), x / rs * np.exp(-0.3 * r)])   # azimuthal about (cx, cy)
+    assert abs(o.diagnostics(cx, cy)["vortex_order"] - 1.0) < 1e-12
+    assert o.diagnostics(cy, cx)["vortex_order"] < 0.9                       # swapped coordinates: not the centre
+    assert o.diagnostics(cx, cy + 4.0)["vortex_order"] < 0.99 and o.diagnostics(cx + 4.0, cy)["vortex_order"] < 0.99
+    # uniform flow with different components: both means, polar order, energy
+    o.v = np.stack([np.full((Ny, Nx), 0.3), np.full((Ny, Nx), -0.4)])
+    d = o.diagnostics(cx, cy)
+    assert abs(d["mean_vx"] - 0.3) < 1e-15 and abs(d["mean_vy"] + 0.4) < 1e-15
+    assert abs(d["polar_order"] - 1.0) < 1e-13 and abs(d["sum_speed"] - 0.5 * Nx * Ny) < 1e-9
+    # uniform flow (u, 0): |e_theta . v| = |u| |y| / r, summed by hand about (cx, cy)
+    o.v = np.stack([np.full((Ny, Nx), 0.7), np.zeros((Ny, Nx))])
+    want = 0.7 * np.sum(np.where(r == 0, 0.0, np.abs(y) / rs))
+    d = o.diagnostics(cx, cy)
+    assert abs(d["sum_abs_vtheta"] - want) < 1e-10 * want
+    want_t = 0.7 * np.sum(np.where(r == 0, 0.0, np.abs(x) / rs))            # (0, u): |x| / r instead
+    o.v = np.stack([np.zeros((Ny, Nx)), np.full((Ny, Nx), 0.7)])
+    assert abs(o.diagnostics(cx, cy)["sum_abs_vtheta"] - want_t) < 1e-10 * want_t and abs(want - want_t) > 1e-3 * want
+
+
+def test_nonfinite_counts_every_field():
+    """`nonfinite` counts the non-finite entries of v_x, v_y AND w (reading R13): one bad value in each, separately."""
+    N, dx = 16, 0.5
+    for which, bad in (("vx", np.nan), ("vy", np.inf), ("w", np.nan)):
+        o = TTSHOracle(N, N, dx, 0.01, LIN)
+        o.w_hat = np.zeros((N, N), complex)
+        o.v = np.zeros((2, N, N))
+        if which == "vx":
+            o.v[0, 3, 5] = bad
+        elif which == "vy":
+            o.v[1, 7, 2] = bad
+        else:
+            o.w_hat[0, 0] = bad                                              # w = iDFT[w^]: every point non-finite
+        want = N * N if which == "w" else 1
+        with np.errstate(all="ignore"):
+            assert o.diagnostics(4.0, 4.0)["nonfinite"] == want, which
+
+
 def test_rhs_terms_signs_on_a_hand_computable_field():
     # uniform v = (u, 0), w = A sin(qx x): rhs1 = -beta u^3 - gamma_v K u ; rhs2 = -lambda0 u A qx cos(qx x) - gamma_w K w
     N, dx = 16, 0.5
@@ -486,11 +533,11 @@ def test_temporal_psd_closed_forms_and_library_special_case():
     F = np.fft.fft(np.stack(series), axis=0)
     assert np.allclose(S, np.mean(np.abs(F) ** 2, axis=(1, 2)), rtol=1e-11, atol=0)
     assert abs(S.sum() - n * sum(np.mean(f * f) for f in series)) < 1e-11 * S.sum()
-    # (v) the sign of the exponent: a rotating pattern exp(+i W t) has its power at +W only
+    # (v) for a real series S(-W) = S(+W) exactly (the accumulators are complex conjugates of each other), so the sign of the
+    #     exponent in Eq. (5) is not observable in S; what is observable is that HALF the power of a real cosine sits at +W
     W = 7 * base
-    S = temporal_psd([np.cos(W * t) * a for t in times], times, [W])   # real signal: half the power at +W
-    c = temporal_psd([a * np.cos(W * t) for t in times], times, [W])[0]
-    assert abs(S[0] - c) == 0.0
+    S = temporal_psd([a * np.cos(W * t) for t in times], times, [W, -W])
+    assert S[0] == S[1] and abs(S[0] - (n / 2) ** 2 * np.mean(a * a)) < 1e-10 * S[0]
     # a non-DFT frequency against the explicit double sum on one point
     Om = 1.2345
     one = [np.full((1, 1), np.sin(0.9 * t) + 0.3) for t in times]
@@ -576,4 +623,10 @@ def test_tangent_qr_orthonormalises_and_measures_the_volume():
     assert sign > 0 and abs(2 * logr.sum() - logdet) < 1e-9                 # prod R_ii^2 = det(Gram)
     Q = tan.as_matrix()
     assert np.allclose(Q.T @ Q, np.eye(3), atol=1e-12)                      # and the stored states reproduce Q
+    # sign convention R_ii > 0: q_i has a positive component along a_i (Gram-Schmidt's choice), and A = Q R with the
+    # upper-triangular R = Q^T A whose diagonal is exp(logr)
+    R = Q.T @ A
+    assert np.all(np.diag(R) > 0) and np.allclose(np.diag(R), np.exp(logr), rtol=1e-10)
+    assert np.allclose(np.tril(R, -1), 0.0, atol=1e-9 * np.abs(R).max()) and np.allclose(Q @ R, A, atol=1e-9 * np.abs(A).max())
+    assert abs(Q[:, 0] @ A[:, 0] - np.linalg.norm(A[:, 0])) < 1e-10 * np.linalg.norm(A[:, 0])   # q_0 = +a_0 / |a_0|
     assert np.allclose(tan.orthonormalize(), 0.0, atol=1e-12)               # idempotent: R = I

@@ -41,7 +41,6 @@ def test_workspace_bytes_and_size_validation(ttsh):
     b32 = ttsh.ttsh_workspace_bytes(4096, 4096, ttsh.TTSH_F32)
     U = 4096 * 4096 * 8
     assert 6 * U < b64 < 13 * U and 0.45 * b64 < b32 < 0.55 * b64        # 7 real fields + pruned spectra and intermediates (1.7 GB of 180 GB HBM)
-    assert ttsh.ttsh_workspace_bytes(2048, 1024, ttsh.TTSH_F64) == ttsh.ttsh_workspace_bytes(1024, 2048, ttsh.TTSH_F64) or True
 
 
 def test_create_rejects_bad_arguments_without_touching_cuda(ttsh):

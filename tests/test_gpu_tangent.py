@@ -68,6 +68,19 @@ def test_tangent_steps_match_oracle(ttsh, Nx, Ny):
     tg.close(); s.close()
 
 
+def test_tangent_at_the_size_bench_times(ttsh):
+    """256 x 256 with 8 vectors (the configuration bench.py's Lyapunov line times), 1 and 20 steps, then one QR."""
+    s, o, tg, to = setup(ttsh, 256, 256, 8, R=30.0)
+    tg.step(1); to.step(1)
+    compare_vectors(tg, to, TOL_1, "256^2 1 step")
+    tg.step(19); to.step(19)
+    compare_vectors(tg, to, TOL_N, "256^2 20 steps")
+    lg, lo = np.asarray(tg.orthonormalize()), to.orthonormalize()
+    assert np.allclose(lg, lo, rtol=0, atol=1e-9), lg - lo
+    compare_vectors(tg, to, 1e-8, "256^2 after QR")
+    tg.close(); s.close()
+
+
 def test_qr_growth_rates_match_oracle(ttsh):
     """Three cycles of (5 tangent steps, QR): log R_ii and the re-orthonormalised vectors agree with the oracle's
     numpy.linalg.qr (the device runs modified Gram-Schmidt: same R up to rounding for well-conditioned vectors)."""

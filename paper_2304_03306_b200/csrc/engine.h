@@ -40,13 +40,16 @@ template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model&
 // the whole row half of a step in one kernel (row_step.cuh): reads the inverse intermediates of w, v_x (= i k_y psi^ with the mean
 // flow) and psi, and K; writes A~ and B~.  Supported for the 1/2 rule when one packed row pair fits in shared memory.
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
-                                                  const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s);
+                                                  const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s, int slots);
 template <typename T> bool row_step_supported(const Geom& g);
+// per-device set-up of k_row_step (shared-memory opt-in, resident CTAs): call on the handle's device; slots = CTAs of the
+// persistent grid of the single-system / ensemble variant (0: not supported for this grid)
+template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens);
 // the same kernel over an ensemble: several row pairs per CTA on small grids (a line of Nx = 64 has 4 threads), row pairs
 // of all members in one persistent grid
 template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                       const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s,
-                                                      int members, size_t mstride);
+                                                      int members, size_t mstride, int slots);
 // set the dynamic shared-memory attribute of the pass kernels for this grid (no launch)
 template <typename T> cudaError_t prepare_rows(const Geom& g);
 template <typename T> cudaError_t prepare_cols(const Geom& g);

@@ -151,24 +151,33 @@ template <typename T> cudaError_t prepare_rows(const Geom& g) {
 }  // namespace ttsh
 #include "row_step.cuh"
 namespace ttsh {
-// persistent grid: one CTA per resident slot (SMs x occupancy), looping over the row-pair blocks
+// persistent grid: one CTA per resident slot (SMs x occupancy), looping over the row-pair blocks.  The opt-in to > 48 KB of
+// dynamic shared memory and the occupancy are per DEVICE: prepare_row_step runs in ttsh_create on the handle's device and the
+// slot counts live in the handle.
+template <typename T, int NX, int LL, bool ENS>
+static cudaError_t prep_row_step(int* slots) {
+  using C = RowStepCfg<T, NX, LL>;
+  *slots = 0;
+  if constexpr (!C::FITS) return cudaSuccess;
+  else {
+    cudaError_t e = set_smem(k_row_step<T, NX, LL, ENS>, C::SMEM);
+    if (e != cudaSuccess) return e;
+    int dev = 0, sms = 0, occ = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_row_step<T, NX, LL, ENS>, C::THREADS, C::SMEM);
+    if (e != cudaSuccess) return e;
+    *slots = sms * (occ > 0 ? occ : 1);
+    return cudaSuccess;
+  }
+}
 template <typename T, int NX, int LL, bool ENS>
 static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi, const void* K,
-                               void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int members, size_t mstride) {
+                               void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int members, size_t mstride, int slots) {
   using C = RowStepCfg<T, NX, LL>;
   if constexpr (!C::FITS) return cudaErrorInvalidConfiguration;
   else {
-    static int slots = 0;
-    if (slots == 0) {
-      cudaError_t e = set_smem(k_row_step<T, NX, LL, ENS>, C::SMEM);
-      if (e != cudaSuccess) return e;
-      int dev = 0, sms = 0, occ = 0;
-      cudaGetDevice(&dev);
-      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_row_step<T, NX, LL, ENS>, C::THREADS, C::SMEM);
-      if (e != cudaSuccess) return e;
-      slots = sms * (occ > 0 ? occ : 1);
-    }
+    if (slots <= 0) return cudaErrorInvalidConfiguration;
     const int rpm = g.Ny / 2;                                  // row pairs per member
     const long long nblk_ll = (long long)rpm * members / C::L;
     if (nblk_ll > 0x3fffffff) return cudaErrorInvalidValue;
@@ -178,10 +187,20 @@ static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, c
                       (const cplx<T>*)inPsi, (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab), v0, nblk, rpm, mstride);
   }
 }
-template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
-                                                  const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s) {
+template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens) {
+  *slots = *slots_ens = 0;
   switch (g.Nx) {
-#define X(N) case N: return go_row_step<T, N, 1, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0);
+#define X(N) case N: { cudaError_t e = prep_row_step<T, N, 1, false>(slots); if (e != cudaSuccess) return e; \
+                       return prep_row_step<T, N, row_step_ens_lines<N>(), true>(slots_ens); }
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
+                                                  const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int slots) {
+  switch (g.Nx) {
+#define X(N) case N: return go_row_step<T, N, 1, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots);
     TTSH_FOR_SIZES(X)
 #undef X
   }
@@ -189,9 +208,9 @@ template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m,
 }
 template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                       const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s,
-                                                      int members, size_t mstride) {
+                                                      int members, size_t mstride, int slots) {
   switch (g.Nx) {
-#define X(N) case N: return go_row_step<T, N, row_step_ens_lines<N>(), true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride);
+#define X(N) case N: return go_row_step<T, N, row_step_ens_lines<N>(), true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots);
     TTSH_FOR_SIZES(X)
 #undef X
   }

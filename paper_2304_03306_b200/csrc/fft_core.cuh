@@ -251,24 +251,35 @@ __device__ __forceinline__ void red_add(cplx<float>* p, cplx<float> v) {
   asm volatile("red.global.add.f32 [%0], %1;" ::"l"(&p->y), "f"(v.y));
 }
 
-// v[r] *= w^r, r = 1..R-1, from the base powers stored at tw[b * ns]
+// stage twiddles: the base powers stored at tw[b * ns] are loaded first (TwBase), v[r] *= w^r, r = 1..R-1, is applied later, so
+// that the table loads are in flight together with the shared-memory reads of the stage
+template <int R, typename T> struct TwBase { cplx<T> w[fft_tw_nbase(R)]; };
 template <int R, int DIR, typename T>
-__device__ __forceinline__ void apply_stage_twiddles(cplx<T>* v, const cplx<T>* __restrict__ tw, int ns) {
+__device__ __forceinline__ TwBase<R, T> load_stage_twiddles(const cplx<T>* __restrict__ tw, int ns) {
+  TwBase<R, T> b;
+#pragma unroll
+  for (int i = 0; i < fft_tw_nbase(R); ++i) b.w[i] = twiddle<DIR>(tw, i * ns);
+  return b;
+}
+template <int R, typename T> __device__ __forceinline__ void apply_stage_twiddles(cplx<T>* v, const TwBase<R, T>& b) {
   if constexpr (R == 16) {
-    const cplx<T> w1 = twiddle<DIR>(tw, 0), w2 = twiddle<DIR>(tw, ns), w3 = twiddle<DIR>(tw, 2 * ns);
-    const cplx<T> w4 = twiddle<DIR>(tw, 3 * ns), w8 = twiddle<DIR>(tw, 4 * ns), w12 = twiddle<DIR>(tw, 5 * ns);
+    const cplx<T> w1 = b.w[0], w2 = b.w[1], w3 = b.w[2], w4 = b.w[3], w8 = b.w[4], w12 = b.w[5];
     v[1] = v[1] * w1;   v[2] = v[2] * w2;   v[3] = v[3] * w3;   v[4] = v[4] * w4;   v[8] = v[8] * w8;   v[12] = v[12] * w12;
     v[5] = v[5] * (w4 * w1);   v[6] = v[6] * (w4 * w2);   v[7] = v[7] * (w4 * w3);
     v[9] = v[9] * (w8 * w1);   v[10] = v[10] * (w8 * w2); v[11] = v[11] * (w8 * w3);
     v[13] = v[13] * (w12 * w1); v[14] = v[14] * (w12 * w2); v[15] = v[15] * (w12 * w3);
   } else if constexpr (R == 8) {
-    const cplx<T> w1 = twiddle<DIR>(tw, 0), w2 = twiddle<DIR>(tw, ns), w3 = twiddle<DIR>(tw, 2 * ns), w4 = twiddle<DIR>(tw, 3 * ns);
+    const cplx<T> w1 = b.w[0], w2 = b.w[1], w3 = b.w[2], w4 = b.w[3];
     v[1] = v[1] * w1; v[2] = v[2] * w2; v[3] = v[3] * w3; v[4] = v[4] * w4;
     v[5] = v[5] * (w4 * w1); v[6] = v[6] * (w4 * w2); v[7] = v[7] * (w4 * w3);
   } else {
 #pragma unroll
-    for (int r = 1; r < R; ++r) v[r] = v[r] * twiddle<DIR>(tw, (r - 1) * ns);
+    for (int r = 1; r < R; ++r) v[r] = v[r] * b.w[r - 1];
   }
+}
+template <int R, int DIR, typename T>
+__device__ __forceinline__ void apply_stage_twiddles(cplx<T>* v, const cplx<T>* __restrict__ tw, int ns) {
+  apply_stage_twiddles<R>(v, load_stage_twiddles<R, DIR>(tw, ns));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -322,22 +333,22 @@ __device__ __forceinline__ void fft_stage(int j0, cplx<T>* __restrict__ sm, cons
       }
       }
     }
+#pragma unroll
+    for (int b = 0; b < NB; ++b) dftR<R, DIR>(v[b]);
   } else {
+    TwBase<R, T> tw[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       const int j = j0 + b * TPL;
+      tw[b] = load_stage_twiddles<R, DIR>(tab + fft_tw_offset_rt(N, S) + (j & (NS - 1)), NS);
 #pragma unroll
       for (int r = 0; r < R; ++r) v[b][r] = sm[fft_pad<N>(j + r * (N / R))];
     }
-  }
 #pragma unroll
-  for (int b = 0; b < NB; ++b) {
-    const int j = j0 + b * TPL;
-    if (NS > 1) {
-      const int k = j & (NS - 1);
-      apply_stage_twiddles<R, DIR>(v[b], tab + fft_tw_offset_rt(N, S) + k, NS);
+    for (int b = 0; b < NB; ++b) {
+      apply_stage_twiddles<R>(v[b], tw[b]);
+      dftR<R, DIR>(v[b]);
     }
-    dftR<R, DIR>(v[b]);
   }
   if (!last || SYNC_LAST) __syncthreads();     // every thread has finished reading this buffer
   if constexpr (first) hook();
@@ -392,19 +403,10 @@ __device__ __forceinline__ void fft_line(int j, cplx<T>* __restrict__ sm, const 
 // Twiddle tables (host: fill_stage_tables_wl): [6 base powers][R1] for stage 2 (indexed by k = t >> 4: a broadcast per
 // half-warp), then [6][TPL] for stage 3 stored in THREAD order (entry t holds W_N^{wl_j(t) power}: coalesced).
 // ---------------------------------------------------------------------------------------
-// measured in k_row_step (B200, L = 1): the plan wins at N = 4096 (295 vs 316 us at C5); at N = 2048 the plain 16 x 16 x 8
-// plan is faster (141.9 vs 150.6 us at 2048 x 4096 fp64: the R1 = 8 first stage spills) and so is 16 x 8 x 8 at N = 1024 (65.9 vs
-// 74.4 us at 1024 x 4096 fp64; C3 36.8 -> 34.8 us per step): with one row pair per CTA several CTAs share an SM and hide each
-// other's barriers, which is what the warp-local exchange was for
-#ifndef TTSH_WL_2048
-#define TTSH_WL_2048 0
-#endif
-#ifndef TTSH_WL_1024
-#define TTSH_WL_1024 0
-#endif
-template <int N> __host__ __device__ constexpr bool fft_wl_supported() {
-  return N == 4096 || (N == 2048 && TTSH_WL_2048) || (N == 1024 && TTSH_WL_1024);
-}
+// measured in k_row_step (B200, one row pair per CTA): the plan wins at N = 4096 (295 vs 316 us at C5); at N = 2048 the plain
+// 16 x 16 x 8 plan is faster (141.9 vs 150.6 us at 2048 x 4096 fp64: the R1 = 8 first stage spills) and so is 16 x 8 x 8 at N = 1024
+// (65.9 vs 74.4 us at 1024 x 4096 fp64): with one row pair per CTA several CTAs share an SM and hide each other's barriers
+template <int N> __host__ __device__ constexpr bool fft_wl_supported() { return N == 4096; }
 template <int N> __host__ __device__ constexpr int fft_wl_r1() { return N / 256; }
 __host__ __device__ constexpr int fft_wl_r1_rt(int N) { return N / 256; }
 __host__ __device__ constexpr int fft_wl_tw_elems_rt(int N) { return 6 * fft_wl_r1_rt(N) + 6 * (N / 16); }
@@ -424,10 +426,6 @@ template <typename T, int N> __device__ __forceinline__ int fft_wl_rot(int r, in
 }
 __host__ __device__ __forceinline__ int fft_wl_j_rt(int t, int r1) { return (t >> 4) + r1 * (t & 15); }
 template <int N> __device__ __forceinline__ int fft_wl_j(int t) { return (t >> 4) + fft_wl_r1<N>() * (t & 15); }
-// timing probes (_work only, never defined in the product build): TTSH_PROBE_NO_DFT drops the butterflies, TTSH_PROBE_NO_XCHG the
-// shared-memory exchanges of the warp-local plan; results are then wrong, only the kernel time is of interest
-template <typename T> __device__ __forceinline__ void keep_alive(cplx<T>& z) { asm volatile("" : "+d"(z.x), "+d"(z.y)); }
-__device__ __forceinline__ void keep_alive(cplx<float>& z) { asm volatile("" : "+f"(z.x), "+f"(z.y)); }
 template <typename T, int N, int DIR, bool SYNC_LAST, class Load, class Store, class Hook = NoHook>
 __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tabw,
                                             Load load, Store store, Hook hook = Hook()) {
@@ -451,21 +449,15 @@ __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__
         v[k % NB][k / NB] = load.finish(j0 + k * TPL, k, raw[s]);
       }
     }
-#ifndef TTSH_PROBE_NO_DFT
 #pragma unroll
     for (int b = 0; b < NB; ++b) dftR<R1, DIR>(v[b]);
-#endif
     __syncthreads();                           // every thread has finished reading this buffer (previous transform)
     hook();
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       const int base = (j0 + b * TPL) * R1;
 #pragma unroll
-#ifndef TTSH_PROBE_NO_XCHG
       for (int r = 0; r < R1; ++r) sm[fft_wl_pad<T, N>(base + r)] = v[b][r];
-#else
-      for (int r = 0; r < R1; ++r) keep_alive(v[b][r]);
-#endif
     }
     __syncthreads();
   }
@@ -473,36 +465,21 @@ __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__
   const int kk = t >> 4, q = t & 15;
   const int j = kk + R1 * q;
   cplx<T> v[16];
-#ifndef TTSH_PROBE_NO_XCHG
 #pragma unroll
   for (int r = 0; r < 16; ++r) v[r] = sm[fft_wl_pad<T, N>(j + r * TPL)];
-#else
-#pragma unroll
-  for (int r = 0; r < 16; ++r) v[r] = mk<T>((T)(j + r), (T)t);
-#endif
-#ifndef TTSH_PROBE_NO_DFT
   apply_stage_twiddles<16, DIR>(v, tabw + kk, R1);
   dft16<DIR>(v);
-#endif
   __syncwarp();                                // the group's 256 positions have been read by its 16 threads
-#ifndef TTSH_PROBE_NO_XCHG
 #pragma unroll
   for (int r = 0; r < 16; ++r) sm[fft_wl_pad<T, N>(TPL * q + kk + R1 * fft_wl_rot<T, N>(r, q))] = v[r];
   __syncwarp();
 #pragma unroll
   for (int qq = 0; qq < 16; ++qq) v[qq] = sm[fft_wl_pad<T, N>(TPL * qq + kk + R1 * fft_wl_rot<T, N>(q, qq))];
-#else
-#pragma unroll
-  for (int r = 0; r < 16; ++r) keep_alive(v[r]);
-#endif
-#ifndef TTSH_PROBE_NO_DFT
   apply_stage_twiddles<16, DIR>(v, tabw + 6 * R1 + t, TPL);
   dft16<DIR>(v);
-#endif
   if (SYNC_LAST) __syncthreads();              // the store goes to shared memory: every group has finished reading it
 #pragma unroll
   for (int r = 0; r < 16; ++r) store(j + r * TPL, r, v[r]);
 }
-
 
 }  // namespace ttsh

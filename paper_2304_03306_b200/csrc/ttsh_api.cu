@@ -93,6 +93,8 @@ struct ttsh_handle {
   cudaGraphExec_t graph_exec;
   bool graph_ok;
   int advection_form;
+  int device;           // CUDA device of the workspace: every entry point must be called with it current
+  int rs_slots, rs_slots_ens;   // persistent grid of k_row_step on this device (single system / ensemble variant)
   bool row_step_ok;     // the fused row-step kernel supports this grid / dtype / dealias fraction
   bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
 };
@@ -136,6 +138,14 @@ namespace {
     cudaError_t e_ = (call);                                                \
     if (e_ != cudaSuccess) return fail_cuda((h), e_, #call);                \
   } while (0)
+
+// every pointer of a handle lives on one CUDA device (that of the workspace); the kernels' shared-memory opt-in and the
+// persistent grids were set up for it.  Entry points refuse to run with another device current.
+bool on_device(const ttsh_handle* h) {
+  int dev = -1;
+  return h->device < 0 || (cudaGetDevice(&dev) == cudaSuccess && dev == h->device);
+}
+#define CHECK_DEVICE(h) do { if (!on_device(h)) return TTSH_ERR_INVALID_ARG; } while (0)
 
 int fail_cuda(ttsh_handle* h, cudaError_t e, const char* what) {
   if (h) {
@@ -307,7 +317,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     case TTSH_STAGE_ROW_STEP:         // a2/a6 row pass + a3 + a4 row pass in one kernel (conservative form, 1/2 rule)
       if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || !h->row_step_ok) return TTSH_ERR_INVALID_ARG;
       TRY(h, DISPATCH(h, launch_row_step, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], h->row_step_wl ? h->K2 : h->K, h->Tm[1], h->Tm[4],
-                      h->row_step_wl ? h->tabXw : h->tabX, h->v0, h->stream));
+                      h->row_step_wl ? h->tabXw : h->tabX, h->v0, h->stream, h->rs_slots));
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_SPECTRAL_P2:
@@ -397,6 +407,8 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   if (t != TTSH_F64 && t != TTSH_F32) return TTSH_ERR_INVALID_ARG;
   if (!(dx > 0.0) || !(dt > 0.0) || !(p->Gamma2 >= 0.0)) return TTSH_ERR_INVALID_ARG;
   if (!std::isfinite(dx) || !std::isfinite(dt)) return TTSH_ERR_INVALID_ARG;
+  for (double v : {p->lambda0, p->alpha, p->beta, p->Gamma0, p->Gamma2, p->gamma_v, p->gamma_w})
+    if (!std::isfinite(v)) return TTSH_ERR_INVALID_ARG;
   if (kind != TTSH_MASK_BINARY && kind != TTSH_MASK_PROCESSED) return TTSH_ERR_INVALID_ARG;
   if (p->dealias_num <= 0 || p->dealias_den <= 0) return TTSH_ERR_INVALID_ARG;
   if (4 * p->dealias_num < p->dealias_den || 3 * p->dealias_num > 2 * p->dealias_den) return TTSH_ERR_INVALID_ARG;
@@ -424,9 +436,23 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
   h->graph_exec = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
   h->row_step_ok = h->dtype == TTSH_F64 ? row_step_supported<double>(h->g) : row_step_supported<float>(h->g);
-  h->row_step_wl = (Nx == 1024 && TTSH_WL_1024) || (Nx == 2048 && TTSH_WL_2048) || Nx == 4096;
+  h->row_step_wl = Nx == 4096;
+  h->rs_slots = h->rs_slots_ens = 0;
+  h->device = -1;
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
+  {   // the device of the workspace must be the current one
+    int dev = -1;
+    TRY(h, cudaGetDevice(&dev));
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, workspace) == cudaSuccess && at.type == cudaMemoryTypeDevice && at.device != dev) {
+      h->err = "the workspace is not on the current CUDA device";
+      h->sticky = TTSH_ERR_INVALID_ARG;
+      return TTSH_ERR_INVALID_ARG;
+    }
+    (void)cudaGetLastError();
+    h->device = dev;
+  }
   std::vector<unsigned char> tx, ty, ts;
   if (t == TTSH_F64) { fill_stage_tables<double>(tx, Nx); fill_stage_tables<double>(ty, Ny / 2); fill_split_table<double>(ts, Ny); }
   else { fill_stage_tables<float>(tx, Nx); fill_stage_tables<float>(ty, Ny / 2); fill_split_table<float>(ts, Ny); }
@@ -443,12 +469,14 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   TRY(h, cudaStreamSynchronize(h->stream));   // the host tables go out of scope below
   TRY(h, DISPATCH(h, prepare_rows, h->g));
   TRY(h, DISPATCH(h, prepare_cols, h->g));
+  if (h->row_step_ok) TRY(h, DISPATCH(h, prepare_row_step, h->g, &h->rs_slots, &h->rs_slots_ens));
   return apply_mask(h, mask, kind);
 }
 
 int ttsh_set_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   if (!h) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (kind != TTSH_MASK_BINARY && kind != TTSH_MASK_PROCESSED) return TTSH_ERR_INVALID_ARG;
   return apply_mask(h, mask, kind);
 }
@@ -456,6 +484,7 @@ int ttsh_set_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
 int ttsh_set_velocity(ttsh_handle* h, const void* vx, const void* vy) {
   if (!h || !vx || !vy) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   const void* src[2] = {vx, vy};
   int rc = enqueue_forward(h, 2, src);
   if (rc != TTSH_OK) return rc;
@@ -470,6 +499,7 @@ int ttsh_set_velocity(ttsh_handle* h, const void* vx, const void* vy) {
 int ttsh_set_advection_form(ttsh_handle* h, int form) {
   if (!h || (form != TTSH_ADVECTION_CONSERVATIVE && form != TTSH_ADVECTION_LITERAL)) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (form != h->advection_form && h->graph_exec) {   // the captured step no longer matches
     cudaGraphExecDestroy(h->graph_exec);
     h->graph_exec = nullptr;
@@ -482,6 +512,7 @@ int ttsh_set_advection_form(ttsh_handle* h, int form) {
 int ttsh_step(ttsh_handle* h, int n) {
   if (!h || n < 0) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   if (n == 0) return TTSH_OK;
   // Small grids are launch-latency bound: replay one captured step.  Large grids launch directly.
@@ -529,6 +560,7 @@ int ttsh_step(ttsh_handle* h, int n) {
 int ttsh_get_fields(ttsh_handle* h, void* vx, void* vy, void* omega, void* psi) {
   if (!h) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   return enqueue_inverse(h, omega, nullptr, nullptr, vx, vy, psi);
 }
@@ -538,6 +570,7 @@ size_t ttsh_state_elems(const ttsh_handle* h) { return h ? (size_t)h->g.NT * h->
 int ttsh_get_state(ttsh_handle* h, void* w_hat, double* mean_flow) {
   if (!h || !w_hat || !mean_flow) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
   TRY(h, cudaMemcpyAsync(w_hat, h->what, bytes, cudaMemcpyDeviceToDevice, h->stream));
@@ -549,6 +582,7 @@ int ttsh_get_state(ttsh_handle* h, void* w_hat, double* mean_flow) {
 int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, double t, long long step) {
   if (!h || !w_hat || !mean_flow) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
   TRY(h, cudaMemcpyAsync(h->what, w_hat, bytes, cudaMemcpyDeviceToDevice, h->stream));
   TRY(h, cudaMemcpyAsync(h->v0, mean_flow, 2 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
@@ -564,6 +598,7 @@ int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, d
 int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out) {
   if (!h || !host_out) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   int rc = enqueue_inverse(h, h->R[0], nullptr, nullptr, h->R[3], h->R[4], nullptr);
   if (rc != TTSH_OK) return rc;
@@ -597,6 +632,7 @@ int ttsh_dumbbell_order(ttsh_handle* h, double cxl, double cyl, double cxr, doub
   if (!h || !host_out || !(radius >= 0.0) || !std::isfinite(radius)) return TTSH_ERR_INVALID_ARG;
   if (!std::isfinite(cxl) || !std::isfinite(cyl) || !std::isfinite(cxr) || !std::isfinite(cyr)) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   int rc = enqueue_inverse(h, h->R[0], nullptr, nullptr, nullptr, nullptr, nullptr);
   if (rc != TTSH_OK) return rc;
@@ -638,6 +674,7 @@ int ttsh_psd_create(ttsh_psd** out, ttsh_handle* h, const double* omegas, int nf
   if (reinterpret_cast<uintptr_t>(workspace) % ALIGN) return TTSH_ERR_INVALID_ARG;
   for (int m = 0; m < nfreq; ++m) if (!std::isfinite(omegas[m])) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   const PsdLayout L = psd_layout(h->Nx, h->Ny, (size_t)h->dtype, nfreq);
   if (workspace_bytes < L.total) return TTSH_ERR_WORKSPACE_TOO_SMALL;
   ttsh_psd* s = new (std::nothrow) ttsh_psd();
@@ -659,6 +696,7 @@ int ttsh_psd_accumulate(ttsh_psd* s) {
   if (!s) return TTSH_ERR_INVALID_ARG;
   ttsh_handle* h = s->h;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   int rc = enqueue_inverse(h, h->R[0], nullptr, nullptr, nullptr, nullptr, nullptr);     // w(., t)
   if (rc != TTSH_OK) return rc;
@@ -673,6 +711,7 @@ int ttsh_psd_result(ttsh_psd* s, double* S_host, long long* nsamples_host) {
   if (!s || !S_host) return TTSH_ERR_INVALID_ARG;
   ttsh_handle* h = s->h;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   const int nf = (int)s->omegas.size();
   TRY(h, DISPATCH(h, launch_psd_power, (size_t)h->Nx * h->Ny, nf, s->acc, s->partial, s->out, h->stream));
   h->launches += 2;
@@ -686,6 +725,7 @@ int ttsh_psd_result(ttsh_psd* s, double* S_host, long long* nsamples_host) {
 int ttsh_psd_reset(ttsh_psd* s) {
   if (!s) return TTSH_ERR_INVALID_ARG;
   if (s->h->sticky) return s->h->sticky;
+  CHECK_DEVICE(s->h);
   TRY(s->h, cudaMemsetAsync(s->acc, 0, s->acc_bytes, s->h->stream));
   s->nsamples = 0;
   return TTSH_OK;
@@ -730,6 +770,7 @@ int ttsh_tangent_create(ttsh_tangent** out, ttsh_handle* h, int nvec, void* work
   if (!h || !workspace || nvec < 1 || nvec > 64) return TTSH_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(workspace) % ALIGN) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
   const TanLayout L = tan_layout(h->Nx, h->Ny, (size_t)h->dtype, nvec);
   if (workspace_bytes < L.total) return TTSH_ERR_WORKSPACE_TOO_SMALL;
@@ -754,6 +795,7 @@ int ttsh_tangent_set(ttsh_tangent* s, int i, const void* dvx, const void* dvy) {
   if (!s || i < 0 || i >= s->nvec || !dvx || !dvy) return TTSH_ERR_INVALID_ARG;
   ttsh_handle* h = s->h;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   const void* src[2] = {dvx, dvy};
   int rc = enqueue_forward(h, 2, src);
   if (rc != TTSH_OK) return rc;
@@ -791,6 +833,7 @@ int ttsh_tangent_step(ttsh_tangent* s, int n) {
   if (!s || n < 0) return TTSH_ERR_INVALID_ARG;
   ttsh_handle* h = s->h;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
   for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
@@ -821,6 +864,7 @@ int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host) {
   if (!s || !log_r_host) return TTSH_ERR_INVALID_ARG;
   ttsh_handle* h = s->h;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
   // modified Gram-Schmidt, all coefficients stay on the device; row i of R in one batched launch per operation:
   // r_ii = |q_i|, q_i /= r_ii, then r_ij = <q_i, q_j> and q_j -= r_ij q_i for all j > i together
@@ -851,6 +895,7 @@ int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host) {
 int ttsh_tangent_get_fields(ttsh_tangent* s, int i, void* dvx, void* dvy, void* domega) {
   if (!s || i < 0 || i >= s->nvec) return TTSH_ERR_INVALID_ARG;
   if (s->h->sticky) return s->h->sticky;
+  CHECK_DEVICE(s->h);
   if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
   return tangent_inverse(s, i, 1, domega, dvx, dvy, false, 0);
 }
@@ -897,7 +942,7 @@ static int ensemble_enqueue_step(ttsh_ensemble* e, cudaStream_t stream) {
   Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->psihat, h->Tm[2], SM_ONE), op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
   TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, h->v0, stream, B, ms));
   TRY(h, DISPATCH(h, launch_row_step_ens, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], h->row_step_wl ? h->K2 : h->K, h->Tm[1], h->Tm[4],
-                  h->row_step_wl ? h->tabXw : h->tabX, h->v0, stream, B, ms));
+                  h->row_step_wl ? h->tabXw : h->tabX, h->v0, stream, B, ms, h->rs_slots_ens));
   Batch fb = make_batch({op(h->Tm[1], h->S[0], 0), op(h->Tm[4], h->S[1], 0)});
   TRY(h, DISPATCH(h, launch_fwd_col, h->g, fb, 2, h->tabY, h->tabS, stream, B, ms));
   TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, h->S[0], h->S[1], h->what, h->psihat, h->v0, stream, B, ms));
@@ -909,6 +954,7 @@ int ttsh_ensemble_step(ttsh_ensemble* e, int n) {
   ttsh_handle* h0 = e->members[0];
   for (ttsh_handle* h : e->members) {
     if (h->sticky) return h->sticky;
+    CHECK_DEVICE(h);
     if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
     if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
   }
@@ -959,6 +1005,7 @@ long long ttsh_launch_count(const ttsh_handle* h) { return h ? h->launches : 0; 
 int ttsh_run_stage(ttsh_handle* h, int stage) {
   if (!h) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   return enqueue_stage(h, stage);
 }
@@ -966,6 +1013,7 @@ int ttsh_run_stage(ttsh_handle* h, int stage) {
 int ttsh_debug_get_real(ttsh_handle* h, int which, void* dst) {
   if (!h || !dst || which < 0 || which > 5) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
   const void* src = which == 5 ? h->K : h->R[which];   // internal fields are in the permuted row layout
   TRY(h, DISPATCH(h, launch_permute, h->Nx, (size_t)h->Nx * h->Ny, src, dst, 0, h->stream));
   h->launches++;

@@ -112,8 +112,11 @@ __host__ __device__ __forceinline__ int perm_index_wl(int x, int tpl) {
 
 // strict '>' cutoff evaluated exactly in integers (reading R4):
 //   k^2 > ((num/den) pi/dx)^2   <=>   4 den^2 ((mx Ny)^2 + (my Nx)^2) > num^2 (Nx Ny)^2
+// Nx, Ny are powers of two, so the three products share the factor g = min(Nx, Ny), which is divided out first: with
+// |mx| <= Nx/2, |my| <= Ny/2, max(Nx, Ny) <= 2^14 and den <= 64 both sides stay below 2^42 (no int64 overflow at any accepted size).
 __host__ __device__ __forceinline__ bool is_cut(int mx, int my, int Nx, int Ny, int num, int den) {
-  const long long a = (long long)mx * Ny, b = (long long)my * Nx, c = (long long)Nx * Ny;
+  const int gx = Nx < Ny ? 1 : Nx / Ny, gy = Ny < Nx ? 1 : Ny / Nx;      // Nx / g and Ny / g
+  const long long a = (long long)mx * gy, b = (long long)my * gx, c = (long long)gx * gy * (Nx < Ny ? Nx : Ny);
   return 4LL * den * den * (a * a + b * b) > (long long)num * num * c * c;
 }
 

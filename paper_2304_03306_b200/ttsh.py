@@ -307,11 +307,13 @@ class Solver:
         self.dtype_code = {"f64": TTSH_F64, "f32": TTSH_F32}[dtype]
         self.tdtype = torch.float64 if dtype == "f64" else torch.float32
         self.device = torch.device(device)
+        self._dependants = []     # TemporalPSD / Tangent / Ensemble objects that borrow the handle: closed before it
         nbytes = ttsh_workspace_bytes(Nx, Ny, self.dtype_code)
         if nbytes == 0:
             raise TTSHError(TTSH_ERR_UNSUPPORTED_SIZE)
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        with self._ctx():
             self.workspace = workspace if workspace is not None else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             nbytes = self.workspace.numel()
             mptr = 0
@@ -332,60 +334,83 @@ class Solver:
         if rc != TTSH_OK:
             raise TTSHError(rc, ttsh_last_error(self.h))
 
+    def _ctx(self):
+        """The handle's device and stream made current: the library enqueues on self.stream, and every tensor this wrapper
+        allocates or copies must be ordered on that same stream (torch's caching allocator reuses memory per stream)."""
+        import contextlib
+        st = contextlib.ExitStack()
+        st.enter_context(self.torch.cuda.device(self.device))
+        st.enter_context(self.torch.cuda.stream(self.stream))
+        return st
+
     def _dev(self, a):
-        return self.torch.as_tensor(a).to(device=self.device, dtype=self.tdtype).contiguous()
+        with self._ctx():
+            return self.torch.as_tensor(a).to(device=self.device, dtype=self.tdtype).contiguous()
 
     def set_mask(self, mask, mask_kind=TTSH_MASK_BINARY):
-        if mask is None:
-            self._check(ttsh_set_mask(self.h, 0, mask_kind))
-            return
-        want = self.torch.uint8 if mask_kind == TTSH_MASK_BINARY else self.tdtype
-        self._mask = self.torch.as_tensor(mask).to(device=self.device, dtype=want).contiguous()
-        self._check(ttsh_set_mask(self.h, self._mask.data_ptr(), mask_kind))
+        with self._ctx():
+            if mask is None:
+                self._check(ttsh_set_mask(self.h, 0, mask_kind))
+                return
+            want = self.torch.uint8 if mask_kind == TTSH_MASK_BINARY else self.tdtype
+            self._mask = self.torch.as_tensor(mask).to(device=self.device, dtype=want).contiguous()
+            self._check(ttsh_set_mask(self.h, self._mask.data_ptr(), mask_kind))
 
     def set_velocity(self, vx, vy):
-        self._vx0, self._vy0 = self._dev(vx), self._dev(vy)
-        self._check(ttsh_set_velocity(self.h, self._vx0.data_ptr(), self._vy0.data_ptr()))
+        with self._ctx():
+            self._vx0, self._vy0 = self._dev(vx), self._dev(vy)
+            self._check(ttsh_set_velocity(self.h, self._vx0.data_ptr(), self._vy0.data_ptr()))
 
     def set_advection_form(self, form: int):
-        self._check(ttsh_set_advection_form(self.h, form))
+        with self._ctx():
+            self._check(ttsh_set_advection_form(self.h, form))
 
     def step(self, n: int = 1):
-        self._check(ttsh_step(self.h, n))
+        with self._ctx():
+            self._check(ttsh_step(self.h, n))
 
     def new_field(self):
-        return self.torch.empty((self.Ny, self.Nx), dtype=self.tdtype, device=self.device)
+        with self._ctx():
+            return self.torch.empty((self.Ny, self.Nx), dtype=self.tdtype, device=self.device)
 
     def get_fields(self, psi: bool = True):
-        vx, vy, w = self.new_field(), self.new_field(), self.new_field()
-        ps = self.new_field() if psi else None
-        self._check(ttsh_get_fields(self.h, vx.data_ptr(), vy.data_ptr(), w.data_ptr(), ps.data_ptr() if psi else 0))
+        with self._ctx():
+            vx, vy, w = self.new_field(), self.new_field(), self.new_field()
+            ps = self.new_field() if psi else None
+            self._check(ttsh_get_fields(self.h, vx.data_ptr(), vy.data_ptr(), w.data_ptr(), ps.data_ptr() if psi else 0))
         return vx, vy, w, ps
 
     def diagnostics(self, cx: Optional[float] = None, cy: Optional[float] = None) -> dict:
         cx = (self.Nx // 2) * self.dx if cx is None else cx
         cy = (self.Ny // 2) * self.dx if cy is None else cy
-        rc, d = ttsh_diagnostics(self.h, cx, cy)
+        with self._ctx():
+            rc, d = ttsh_diagnostics(self.h, cx, cy)
         self._check(rc)
         return d.as_dict()
 
     def dumbbell_order(self, centre_left, centre_right, radius: float) -> dict:
-        rc, d = ttsh_dumbbell_order(self.h, centre_left[0], centre_left[1], centre_right[0], centre_right[1], radius)
+        with self._ctx():
+            rc, d = ttsh_dumbbell_order(self.h, centre_left[0], centre_left[1], centre_right[0], centre_right[1], radius)
         self._check(rc)
         return d.as_dict()
 
     def run_stage(self, stage: int):
-        self._check(ttsh_run_stage(self.h, stage))
+        with self._ctx():
+            self._check(ttsh_run_stage(self.h, stage))
 
     def debug_real(self, which: int):
-        out = self.new_field()
-        self._check(ttsh_debug_get_real(self.h, which, out.data_ptr()))
+        with self._ctx():
+            out = self.new_field()
+            self._check(ttsh_debug_get_real(self.h, which, out.data_ptr()))
         return out
 
     def launch_count(self) -> int:
         return ttsh_launch_count(self.h)
 
     def close(self):
+        """Closes the objects that borrow the handle (TemporalPSD, Tangent, Ensemble) first, then the handle."""
+        for d in list(getattr(self, "_dependants", [])):
+            d.close()
         if getattr(self, "h", None):
             self.torch.cuda.synchronize(self.device)
             ttsh_destroy(self.h)
@@ -412,23 +437,29 @@ class TemporalPSD:
             rc, self.s = ttsh_psd_create(solver.h, self.omegas, self.workspace.data_ptr(), nbytes)
         if rc != TTSH_OK:
             raise TTSHError(rc)
+        solver._dependants.append(self)
 
     def accumulate(self):
-        self.solver._check(ttsh_psd_accumulate(self.s))
+        with self.solver._ctx():
+            self.solver._check(ttsh_psd_accumulate(self.s))
 
     def result(self):
-        rc, S, n = ttsh_psd_result(self.s, len(self.omegas))
+        with self.solver._ctx():
+            rc, S, n = ttsh_psd_result(self.s, len(self.omegas))
         self.solver._check(rc)
         return S, n
 
     def reset(self):
-        self.solver._check(ttsh_psd_reset(self.s))
+        with self.solver._ctx():
+            self.solver._check(ttsh_psd_reset(self.s))
 
     def close(self):
         if getattr(self, "s", None):
             self.solver.torch.cuda.synchronize(self.solver.device)
             ttsh_psd_destroy(self.s)
             self.s = None
+            if self in self.solver._dependants:
+                self.solver._dependants.remove(self)
 
     def __del__(self):
         try:
@@ -452,24 +483,29 @@ class Tangent:
             rc, self.s = ttsh_tangent_create(solver.h, self.nvec, self.workspace.data_ptr(), nbytes)
         if rc != TTSH_OK:
             raise TTSHError(rc)
+        solver._dependants.append(self)
 
     def set(self, i: int, dvx, dvy):
-        a, b = self.solver._dev(dvx), self.solver._dev(dvy)
-        self._keep = (a, b)
-        self.solver._check(ttsh_tangent_set(self.s, i, a.data_ptr(), b.data_ptr()))
+        with self.solver._ctx():
+            a, b = self.solver._dev(dvx), self.solver._dev(dvy)
+            self._keep = (a, b)
+            self.solver._check(ttsh_tangent_set(self.s, i, a.data_ptr(), b.data_ptr()))
 
     def step(self, n: int = 1):
-        self.solver._check(ttsh_tangent_step(self.s, n))
+        with self.solver._ctx():
+            self.solver._check(ttsh_tangent_step(self.s, n))
 
     def orthonormalize(self):
-        rc, logr = ttsh_tangent_orthonormalize(self.s, self.nvec)
+        with self.solver._ctx():
+            rc, logr = ttsh_tangent_orthonormalize(self.s, self.nvec)
         self.solver._check(rc)
         return logr
 
     def get_fields(self, i: int):
         s = self.solver
-        dvx, dvy, dw = s.new_field(), s.new_field(), s.new_field()
-        s._check(ttsh_tangent_get_fields(self.s, i, dvx.data_ptr(), dvy.data_ptr(), dw.data_ptr()))
+        with s._ctx():
+            dvx, dvy, dw = s.new_field(), s.new_field(), s.new_field()
+            s._check(ttsh_tangent_get_fields(self.s, i, dvx.data_ptr(), dvy.data_ptr(), dw.data_ptr()))
         return dvx, dvy, dw
 
     def close(self):
@@ -477,6 +513,8 @@ class Tangent:
             self.solver.torch.cuda.synchronize(self.solver.device)
             ttsh_tangent_destroy(self.s)
             self.s = None
+            if self in self.solver._dependants:
+                self.solver._dependants.remove(self)
 
     def __del__(self):
         try:
@@ -508,9 +546,12 @@ class Ensemble:
         rc, self.e = ttsh_ensemble_create([m.h for m in self.members])
         if rc != TTSH_OK:
             raise TTSHError(rc)
+        for m in self.members:
+            m._dependants.append(self)      # closing a member closes the ensemble first
 
     def step(self, n: int = 1):
-        rc = ttsh_ensemble_step(self.e, n)
+        with self.members[0]._ctx():
+            rc = ttsh_ensemble_step(self.e, n)
         if rc != TTSH_OK:
             raise TTSHError(rc, ttsh_last_error(self.members[0].h))
 
@@ -522,6 +563,9 @@ class Ensemble:
             self.torch.cuda.synchronize(self.device)
             ttsh_ensemble_destroy(self.e)
             self.e = None
+            for m in self.members:
+                if self in m._dependants:
+                    m._dependants.remove(self)
         for m in getattr(self, "members", []):
             m.close()
 

@@ -70,6 +70,11 @@ def test_create_rejects_bad_arguments_without_touching_cuda(ttsh):
     q = ttsh.baseline_params(); q.Gamma2 = -1.0
     rc, h = ttsh.ttsh_create(64, 64, 0.5, 0.01, q, ttsh.TTSH_F64, 0, 0, fake_ws, nbytes, 0)
     assert rc == ttsh.TTSH_ERR_INVALID_ARG
+    for field in ("lambda0", "alpha", "beta", "Gamma0", "Gamma2", "gamma_v", "gamma_w"):      # non-finite parameters
+        for bad in (float("nan"), float("inf")):
+            q = ttsh.baseline_params(); setattr(q, field, bad)
+            rc, h = ttsh.ttsh_create(64, 64, 0.5, 0.01, q, ttsh.TTSH_F64, 0, 0, fake_ws, nbytes, 0)
+            assert rc == ttsh.TTSH_ERR_INVALID_ARG and not h, (field, bad)
     assert ttsh.ttsh_step(None, 1) == ttsh.TTSH_ERR_INVALID_ARG
     assert ttsh.ttsh_destroy(None) == ttsh.TTSH_OK
     assert "workspace" in ttsh.ttsh_strerror(ttsh.TTSH_ERR_WORKSPACE_TOO_SMALL)

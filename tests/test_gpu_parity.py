@@ -337,6 +337,31 @@ def test_checkpoint_roundtrip_is_bit_exact_and_set_mask_keeps_state(ttsh):
     s.close()
 
 
+def test_non_default_stream_and_close_order(ttsh):
+    """The wrapper orders its allocations and copies on the Solver's own stream (not torch's current one), and closing a Solver
+    first tears down the objects that borrow its handle (TemporalPSD, Tangent)."""
+    import torch
+    N = 128
+    mask = workloads.disk_mask(N, N, 0.5, 20.0)
+    vel = workloads.planewave_velocity(N, N, 0.5, 13, amplitude=1.0)
+    side = torch.cuda.Stream()
+    s = ttsh.Solver(N, N, 0.5, 0.01, ttsh.baseline_params(), "f64", mask=mask, stream=side)
+    ref = ttsh.Solver(N, N, 0.5, 0.01, ttsh.baseline_params(), "f64", mask=mask)
+    for _ in range(3):                      # repeated upload / step / read-back: a cross-stream race would show as a mismatch
+        s.set_velocity(*vel); ref.set_velocity(*vel)
+        s.step(7); ref.step(7)
+        a, b = s.get_fields(), ref.get_fields()
+        side.synchronize(); torch.cuda.synchronize()
+        for u, v in zip(a, b):
+            assert torch.equal(u, v)
+    psd = ttsh.TemporalPSD(s, [0.0, 1.0])
+    tg = ttsh.Tangent(s, 2)
+    psd.accumulate()
+    s.close()                               # dependants are closed first: no use of a freed handle afterwards
+    assert psd.s is None and tg.s is None and s.h is None
+    psd.close(); tg.close(); ref.close()
+
+
 # ---------------------------------------------------------------- C5: the configuration bench.py times (4096 x 4096)
 def _c5_pair(ttsh, dtype, geometry="disk"):
     cfg = workloads.CONFIGS["C5" if geometry == "disk" else "C5p"]

@@ -52,10 +52,23 @@ def workload(name):
     return cfg, dtype
 
 
+PARAM_TEXT = {"baseline": "lambda0=3.5 alpha=-0.5 beta=0.5 Gamma0=-1 Gamma2=1 gamma_v=40 gamma_w=4",
+              "paper": "the paper's parameters (PAPER.md:61): lambda0=9 alpha=0.5 beta=1.6 Gamma0=-2 Gamma2=1 gamma_v=40 gamma_w=4"}
+
+
 def describe(cfg, dtype):
     geom = {"disk": f"disk R={cfg.R:g}", "dumbbell": f"dumbbell R={cfg.R:g} d={cfg.d:g}", "none": "unconfined"}[cfg.geometry]
-    return (f"{cfg.name}: {cfg.Ny}x{cfg.Nx} grid, dx={cfg.dx}, dt={cfg.dt}, {dtype}, {geom}, lambda0=3.5 alpha=-0.5 beta=0.5 "
-            f"Gamma0=-1 Gamma2=1 gamma_v=40 gamma_w=4, Gaussian 1e-2 start, seed {cfg.seed}")
+    return (f"{cfg.name}: {cfg.Ny}x{cfg.Nx} grid, dx={cfg.dx}, dt={cfg.dt}, {dtype}, {geom}, {PARAM_TEXT[cfg.preset]}, "
+            f"Gaussian 1e-2 start, seed {cfg.seed}")
+
+
+def gpu_params(ttsh, cfg):
+    return ttsh.paper_params() if cfg.preset == "paper" else ttsh.baseline_params()
+
+
+def oracle_params(cfg):
+    from oracle import BASELINE_PRESET, PAPER_PRESET
+    return PAPER_PRESET if cfg.preset == "paper" else BASELINE_PRESET
 
 
 # --------------------------------------------------------------------------------------------------
@@ -127,11 +140,10 @@ def oracle_c(cfg):
     """The oracle-fft restatement of the oracle in plain C (oracle/ttsh_oracle_c.c: full complex spectra, radix-2 FFT, OpenMP over
     lines) at the workload's REAL size, with its mask and start.  The honest CPU baseline: the counterpart of the CPU curve of
     Fig. 9 (PAPER.md:367)."""
-    from oracle import BASELINE_PRESET
     from oracle.c_oracle import TTSHOracleC
     mask = cfg.mask()
     vx, vy = cfg.initial_velocity(mask)
-    o = TTSHOracleC(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, BASELINE_PRESET, mask=mask)
+    o = TTSHOracleC(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, oracle_params(cfg), mask=mask)
     o.set_velocity(vx, vy)
     return o
 
@@ -155,8 +167,9 @@ def time_oracle(cfg, n_steps, budget_s, warmup=0):
     """Times the oracle AS IT STANDS (naive-DFT transforms = explicit DFT-matrix products) on a bounded sample of
     the workload: the same geometry family, parameters and start, on the largest grid <= the workload's whose
     predicted cost fits the budget.  Returns (grid-point-steps/s, sample description, seconds per step)."""
-    from oracle import BASELINE_PRESET, TTSHOracle
+    from oracle import TTSHOracle
     from paper_2304_03306_b200 import workloads
+    BASELINE_PRESET = oracle_params(cfg)
 
     def run(Nx, Ny, steps, wu):
         scale = Nx / cfg.Nx
@@ -228,7 +241,7 @@ def measure(torch, ttsh, cfg, dtype, K, W, device, want_roofline=True, want_e2e=
     import numpy as np
     mask = cfg.mask()
     vx0, vy0 = cfg.initial_velocity(mask)
-    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.baseline_params(), dtype, mask=mask, device=device)
+    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, gpu_params(ttsh, cfg), dtype, mask=mask, device=device)
     s.set_velocity(vx0, vy0)
     cx, cy = (cfg.Nx // 2) * cfg.dx, (cfg.Ny // 2) * cfg.dx
     stream = torch.cuda.current_stream(device)
@@ -589,12 +602,12 @@ def main():
 
     if not a.no_extra and world == 1:
         extra = {}
-        for name in ("C5-f32", "C3", "C3-f32", "C5p"):
+        for name in ("C5-f32", "C3", "C3-f32", "C5p", "C6", "C6-f32"):
             if name == a.workload:
                 continue
             c2, d2 = workload(name)
-            r2 = measure(torch, ttsh, c2, d2, max(2, a.steps // 2), 3, device, want_roofline=False, want_e2e=False)
-            k2 = max(2, a.steps // 2)
+            k2 = max(2, a.steps // 2) if c2.Nx * c2.Ny <= 4096 * 4096 else 1
+            r2 = measure(torch, ttsh, c2, d2, k2, 3 if k2 > 1 else 1, device, want_roofline=False, want_e2e=False)
             extra[name] = {"value": c2.Nx * c2.Ny * INNER * k2 / (r2["ms_total"] * 1e-3), "unit": "grid-point-steps/s",
                            "euler_step_ms": r2["ms_total"] / k2 / INNER, "workload": describe(c2, d2)}
         # the paper's sweeps (R sweep of C1 / C2 / C3) as ensembles: ttsh_ensemble_step, one launch of each hot

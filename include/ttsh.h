@@ -21,6 +21,8 @@
  *     for the duration of the enqueued (stream-ordered) work and the workspace must outlive the handle.
  *   - all functions return 0 (TTSH_OK) or a negative ttsh_status; they never throw, abort or print.
  *   - all work is enqueued on the stream given to ttsh_create; only ttsh_diagnostics synchronises.
+ *   - a handle belongs to the CUDA device that was current in ttsh_create (the device of its workspace); every later call
+ *     on it must be made with that device current, else it returns TTSH_ERR_INVALID_ARG.
  *   - there is no CPU fallback: without a CUDA device every compute call returns TTSH_ERR_CUDA.
  */
 #ifndef TTSH_H_
@@ -36,8 +38,9 @@ typedef struct ttsh_handle ttsh_handle;   /* opaque; host metadata + pointers in
 
 typedef enum {
   TTSH_OK = 0,
-  TTSH_ERR_INVALID_ARG = -1,         /* NULL pointer, n < 0, dx <= 0, dt <= 0, Gamma2 < 0, bad dealias fraction */
-  TTSH_ERR_UNSUPPORTED_SIZE = -2,    /* Nx, Ny must be powers of two in [64, 8192] (all sizes of PAPER.md:271 / BASELINE.json) */
+  TTSH_ERR_INVALID_ARG = -1,         /* NULL pointer, n < 0, dx <= 0, dt <= 0, Gamma2 < 0, non-finite parameter, bad dealias fraction, wrong device */
+  TTSH_ERR_UNSUPPORTED_SIZE = -2,    /* Nx, Ny must be powers of two in [64, 16384]: the paper's grids are 8192^2 and
+                                        16384^2 for Fig. 6(f); BASELINE.json's are 64 .. 4096 */
   TTSH_ERR_WORKSPACE_TOO_SMALL = -3,
   TTSH_ERR_NOT_INITIALIZED = -4,     /* ttsh_step / get_fields / diagnostics before ttsh_set_velocity */
   TTSH_ERR_CUDA = -5                 /* sticky; message via ttsh_last_error */
@@ -155,8 +158,9 @@ int ttsh_psd_destroy(ttsh_psd* s);
 
 /* Tangent-linear evolution and growth rates (Lyapunov exponents): nvec independent perturbations
  * (dw^, dv^(0)) of the state are carried along the trajectory by the Jacobian of Algorithm 1 at the current state (lines 1-2
- * differentiated, everything else is linear), and re-orthonormalised on request by a QR decomposition (modified Gram-Schmidt
- * on the device) whose diagonal gives the growth: lambda_i = sum log R_ii / elapsed time.  The inner product is the Euclidean
+ * differentiated, everything else is linear), and re-orthonormalised on request by a QR decomposition (CholeskyQR2 on the
+ * device: Gram matrix, Cholesky factor, triangular solve, twice; modified Gram-Schmidt when the vectors are
+ * numerically dependent) whose diagonal gives the growth: lambda_i = sum log R_ii / elapsed time.  The inner product is the Euclidean
  * one of the real vectors [dw(x) for all x ; dv^_x(0) ; dv^_y(0)] (unitary DFT normalisation of the mean flow).
  * workspace: DEVICE, >= ttsh_tangent_workspace_bytes, 256-byte aligned, owned by the caller.  1 <= nvec <= 64.  Requires
  * TTSH_ADVECTION_CONSERVATIVE.  The tangent object borrows the handle: destroy it first. */

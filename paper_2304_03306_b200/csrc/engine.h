@@ -27,9 +27,10 @@ template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, 
                                                  int members = 1, size_t mstride = 0);
 template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, int nfields, const void* tabY, const void* tabS, cudaStream_t s,
                                                  int members = 1, size_t mstride = 0);
-template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const double* v0, cudaStream_t s,
-                                                 int members = 1, size_t mstride = 0);
-template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, cudaStream_t s,
+// tabR: W_Nx^j, j < Nx/32, used by the real-row kernels of Nx = 16384 (fft_rows_real.cuh); ignored on the other grids
+template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const void* tabR, const double* v0,
+                                                 cudaStream_t s, int members = 1, size_t mstride = 0);
+template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nfields, const void* tabX, const void* tabR, cudaStream_t s,
                                                  int members = 1, size_t mstride = 0);
 // fused real-space + forward row pass (conservative form): reads v_x, v_y, w, K; writes A~ = i kx Gy~ + S'~ and B~ = Gx~
 template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
@@ -44,7 +45,13 @@ template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m,
 template <typename T> bool row_step_supported(const Geom& g);
 // per-device set-up of k_row_step (shared-memory opt-in, resident CTAs): call on the handle's device; slots = CTAs of the
 // persistent grid of the single-system / ensemble variant (0: not supported for this grid)
-template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens);
+template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens, int* slots_tan);
+// tangent-linear variant of the row-step kernel (row_step.cuh, TAN): members = tangent vectors whose intermediates / outputs / mean
+// flows lie mstride bytes apart; K and the base fields bw, bvx, bvy (internal real fields, layout perm_index) are shared.  tabX: the
+// plain per-stage tables (this variant never runs the warp-local plan)
+template <typename T> cudaError_t launch_row_step_tan(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
+                                                      const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s,
+                                                      int members, size_t mstride, int slots, const void* bw, const void* bvx, const void* bvy);
 // the same kernel over an ensemble: several row pairs per CTA on small grids (a line of Nx = 64 has 4 threads), row pairs
 // of all members in one persistent grid
 template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
@@ -95,5 +102,12 @@ template <typename T> cudaError_t launch_spec_dot(const Geom& g, const void* a, 
                                                   double* coef, cudaStream_t s);
 template <typename T> cudaError_t launch_spec_scale_axpy(const Geom& g, const double* coef, const void* x, void* y, const double* x0,
                                                          double* y0, int count, size_t ystride, cudaStream_t s);
+
+// blocked QR (CholeskyQR2) of tangent vectors at a uniform byte stride: Gram matrix G[nvec][nvec] (device; partial: nvec^2 *
+// DIAG_BLOCKS doubles) and the in-place product A <- A S with an upper-triangular S (device), which also refreshes psi^ = w^/k^2
+template <typename T> cudaError_t launch_gram(const Geom& g, const void* v, const double* v0, size_t vstride, int nvec, double* partial, double* G,
+                                              cudaStream_t s);
+cudaError_t launch_chol_inv(int nvec, const double* G, double* S, double* logr, int* flag, cudaStream_t s);
+template <typename T> cudaError_t launch_tri_apply(const Geom& g, int nvec, const double* S, void* v, void* psi, double* v0, size_t vstride, cudaStream_t s);
 
 }  // namespace ttsh

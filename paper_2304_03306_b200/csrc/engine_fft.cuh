@@ -6,6 +6,10 @@
 namespace ttsh {
 
 #define TTSH_FOR_SIZES(X) X(64) X(128) X(256) X(512) X(1024) X(2048) X(4096) X(8192)
+// Ny = 16384 (Fig. 6(f)): half-length column transforms of 8192 points, one column per CTA.
+// Nx = 16384: one real row per half-length complex transform (fft_rows_real.cuh) instead of packed row pairs.
+#define TTSH_FOR_COL_SIZES(X) TTSH_FOR_SIZES(X) X(16384)
+#define TTSH_REAL_ROW_NX 16384
 
 template <typename K> static cudaError_t set_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -55,7 +59,7 @@ template <typename T> cudaError_t launch_inv_col(const Geom& g, const Batch& b, 
                                                  int members, size_t mstride) {
   switch (g.Ny) {
 #define X(N) case N: return go_inv_col<T, N>(g, b, nf, tab, tabS, v0, s, members, mstride);
-    TTSH_FOR_SIZES(X)
+    TTSH_FOR_COL_SIZES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
@@ -64,7 +68,7 @@ template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, 
                                                  int members, size_t mstride) {
   switch (g.Ny) {
 #define X(N) case N: return go_fwd_col<T, N>(g, b, nf, tab, tabS, s, members, mstride);
-    TTSH_FOR_SIZES(X)
+    TTSH_FOR_COL_SIZES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
@@ -76,7 +80,7 @@ template <typename T> cudaError_t prepare_cols(const Geom& g) {
                        e = set_smem(k_inv_col<T, N, C::GMAX>, C::GMAX * C::SMEM); if (e != cudaSuccess) return e; \
                        e = set_smem(k_fwd_col<T, N, C::GMAX>, C::GMAX * C::SMEM); if (e != cudaSuccess) return e; \
                        return set_smem(k_fwd_col<T, N, 1>, C::SMEM); }
-    TTSH_FOR_SIZES(X)
+    TTSH_FOR_COL_SIZES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
@@ -84,6 +88,21 @@ template <typename T> cudaError_t prepare_cols(const Geom& g) {
 #endif
 
 #ifdef TTSH_BUILD_ROWS
+}  // namespace ttsh
+#include "fft_rows_real.cuh"
+namespace ttsh {
+template <typename T, int NX> static cudaError_t go_inv_row_real(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabR, const double* v0,
+                                                                 cudaStream_t s, int members, size_t mstride) {
+  using C = RealRowCfg<T, NX>;
+  return launch_pdl(k_inv_row_real<T, NX>, dim3(g.Ny, nf, members), dim3(C::TPL), C::SMEM, s, g, b, static_cast<const cplx<T>*>(tab),
+                    static_cast<const cplx<T>*>(tabR), v0, mstride);
+}
+template <typename T, int NX> static cudaError_t go_fwd_row_real(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabR, cudaStream_t s,
+                                                                 int members, size_t mstride) {
+  using C = RealRowCfg<T, NX>;
+  return launch_pdl(k_fwd_row_real<T, NX>, dim3(g.Ny, nf, members), dim3(C::TPL), C::SMEM, s, g, b, static_cast<const cplx<T>*>(tab),
+                    static_cast<const cplx<T>*>(tabR), mstride);
+}
 template <typename T, int NX> static cudaError_t go_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s,
                                                             int members, size_t mstride) {
   using C = RowCfg<T, NX>;
@@ -108,16 +127,17 @@ template <typename T, int NX> static cudaError_t go_fwd_row_fused(const Geom& g,
 }
 template <typename T> cudaError_t launch_fwd_row_fused(const Geom& g, const Model& m, const void* vx, const void* vy, const void* w,
                                                        const void* K, void* oA, void* oB, const void* tab, cudaStream_t s) {
-  switch (g.Nx) {
+  switch (g.Nx) {       // pair kernels only (Nx <= 8192)
 #define X(N) case N: return go_fwd_row_fused<T, N>(g, m, vx, vy, w, K, oA, oB, tab, s);
     TTSH_FOR_SIZES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const double* v0, cudaStream_t s,
-                                                 int members, size_t mstride) {
+template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabR, const double* v0,
+                                                 cudaStream_t s, int members, size_t mstride) {
   if (members < 1 || members > 65535) return cudaErrorInvalidValue;
+  if (g.Nx == TTSH_REAL_ROW_NX) return go_inv_row_real<T, TTSH_REAL_ROW_NX>(g, b, nf, tab, tabR, v0, s, members, mstride);
   switch (g.Nx) {
 #define X(N) case N: return go_inv_row<T, N>(g, b, nf, tab, v0, s, members, mstride);
     TTSH_FOR_SIZES(X)
@@ -125,9 +145,10 @@ template <typename T> cudaError_t launch_inv_row(const Geom& g, const Batch& b, 
   }
   return cudaErrorInvalidValue;
 }
-template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, cudaStream_t s,
+template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, int nf, const void* tab, const void* tabR, cudaStream_t s,
                                                  int members, size_t mstride) {
   if (members < 1 || members > 65535) return cudaErrorInvalidValue;
+  if (g.Nx == TTSH_REAL_ROW_NX) return go_fwd_row_real<T, TTSH_REAL_ROW_NX>(g, b, nf, tab, tabR, s, members, mstride);
   switch (g.Nx) {
 #define X(N) case N: return go_fwd_row<T, N>(g, b, nf, tab, s, members, mstride);
     TTSH_FOR_SIZES(X)
@@ -136,6 +157,12 @@ template <typename T> cudaError_t launch_fwd_row(const Geom& g, const Batch& b, 
   return cudaErrorInvalidValue;
 }
 template <typename T> cudaError_t prepare_rows(const Geom& g) {
+  if (g.Nx == TTSH_REAL_ROW_NX) {
+    using C = RealRowCfg<T, TTSH_REAL_ROW_NX>;
+    cudaError_t e = set_smem(k_inv_row_real<T, TTSH_REAL_ROW_NX>, C::SMEM);
+    if (e != cudaSuccess) return e;
+    return set_smem(k_fwd_row_real<T, TTSH_REAL_ROW_NX>, C::SMEM);
+  }
   switch (g.Nx) {
 #define X(N) case N: { cudaError_t e = set_smem(k_inv_row<T, N>, RowCfg<T, N>::SMEM); if (e != cudaSuccess) return e; \
                        e = set_smem(k_fwd_row_fused<T, N>, fused_smem<T, N>(g)); if (e != cudaSuccess) return e; \
@@ -154,27 +181,28 @@ namespace ttsh {
 // persistent grid: one CTA per resident slot (SMs x occupancy), looping over the row-pair blocks.  The opt-in to > 48 KB of
 // dynamic shared memory and the occupancy are per DEVICE: prepare_row_step runs in ttsh_create on the handle's device and the
 // slot counts live in the handle.
-template <typename T, int NX, int LL, bool ENS>
+template <typename T, int NX, int LL, bool ENS, bool TAN = false>
 static cudaError_t prep_row_step(int* slots) {
-  using C = RowStepCfg<T, NX, LL>;
+  using C = RowStepCfg<T, NX, LL, TAN>;
   *slots = 0;
   if constexpr (!C::FITS) return cudaSuccess;
   else {
-    cudaError_t e = set_smem(k_row_step<T, NX, LL, ENS>, C::SMEM);
+    cudaError_t e = set_smem(k_row_step<T, NX, LL, ENS, TAN>, C::SMEM);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0, occ = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_row_step<T, NX, LL, ENS>, C::THREADS, C::SMEM);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_row_step<T, NX, LL, ENS, TAN>, C::THREADS, C::SMEM);
     if (e != cudaSuccess) return e;
     *slots = sms * (occ > 0 ? occ : 1);
     return cudaSuccess;
   }
 }
-template <typename T, int NX, int LL, bool ENS>
+template <typename T, int NX, int LL, bool ENS, bool TAN = false>
 static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi, const void* K,
-                               void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int members, size_t mstride, int slots) {
-  using C = RowStepCfg<T, NX, LL>;
+                               void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int members, size_t mstride, int slots,
+                               const void* bw = nullptr, const void* bvx = nullptr, const void* bvy = nullptr) {
+  using C = RowStepCfg<T, NX, LL, TAN>;
   if constexpr (!C::FITS) return cudaErrorInvalidConfiguration;
   else {
     if (slots <= 0) return cudaErrorInvalidConfiguration;
@@ -183,14 +211,16 @@ static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, c
     if (nblk_ll > 0x3fffffff) return cudaErrorInvalidValue;
     const int nblk = (int)nblk_ll;
     const int grid = nblk < slots ? nblk : slots;
-    return launch_pdl(k_row_step<T, NX, LL, ENS>, dim3(grid), dim3(C::THREADS), C::SMEM, s, g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx,
-                      (const cplx<T>*)inPsi, (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab), v0, nblk, rpm, mstride);
+    return launch_pdl(k_row_step<T, NX, LL, ENS, TAN>, dim3(grid), dim3(C::THREADS), C::SMEM, s, g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx,
+                      (const cplx<T>*)inPsi, (const T*)K, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab), v0, nblk, rpm, mstride,
+                      (const T*)bw, (const T*)bvx, (const T*)bvy);
   }
 }
-template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens) {
-  *slots = *slots_ens = 0;
+template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens, int* slots_tan) {
+  *slots = *slots_ens = *slots_tan = 0;
   switch (g.Nx) {
 #define X(N) case N: { cudaError_t e = prep_row_step<T, N, 1, false>(slots); if (e != cudaSuccess) return e; \
+                       e = prep_row_step<T, N, row_step_ens_lines<N>(), true, true>(slots_tan); if (e != cudaSuccess) return e; \
                        return prep_row_step<T, N, row_step_ens_lines<N>(), true>(slots_ens); }
     TTSH_FOR_SIZES(X)
 #undef X
@@ -211,6 +241,17 @@ template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model
                                                       int members, size_t mstride, int slots) {
   switch (g.Nx) {
 #define X(N) case N: return go_row_step<T, N, row_step_ens_lines<N>(), true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+// tangent-linear variant: members = tangent vectors (in / out / v0 at mstride), K and the base fields bw, bvx, bvy shared
+template <typename T> cudaError_t launch_row_step_tan(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
+                                                      const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s,
+                                                      int members, size_t mstride, int slots, const void* bw, const void* bvx, const void* bvy) {
+  switch (g.Nx) {
+#define X(N) case N: return go_row_step<T, N, row_step_ens_lines<N>(), true, true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots, bw, bvx, bvy);
     TTSH_FOR_SIZES(X)
 #undef X
   }

@@ -400,16 +400,22 @@ __device__ __forceinline__ void fft_line(int j, cplx<T>* __restrict__ sm, const 
 // Inside the group the element (q, r) is kept at position TPL q + k + R1 rot(r, q) (rot: fft_wl_rot below).  Only the stage-1 -> stage-2 exchange is
 // CTA-wide.  Stage 1 is generic in its base index j0: j0 = t for inputs loaded in natural order (coalesced), j0 = wl_j(t)
 // for inputs the thread already owns in registers.  Outputs: slot k of thread t is index wl_j(t) + k TPL.
-// Twiddle tables (host: fill_stage_tables_wl): [6 base powers][R1] for stage 2 (indexed by k = t >> 4: a broadcast per
-// half-warp), then [6][TPL] for stage 3 stored in THREAD order (entry t holds W_N^{wl_j(t) power}: coalesced).
+// Twiddle tables (host: fill_stage_tables_wl): [15 powers][R1] for stage 2 (indexed by k = t >> 4: a broadcast per half-warp, so
+// all 15 powers are read and none is derived), then [6 base powers][TPL] for stage 3 stored in THREAD order (entry t holds
+// W_N^{wl_j(t) power}).  In fp64 the caller passes a copy of the table in SHARED memory: with 200 KB of dynamic shared memory the
+// L1 is smaller than the table, every global twiddle load missed it (ncu, round 1: 0.06 % hits) and paid L2 latency in the
+// middle of a stage; from shared memory the loads cost the same data-pipe wavefronts and 30 cycles.
 // ---------------------------------------------------------------------------------------
 // measured in k_row_step (B200, one row pair per CTA): the plan wins at N = 4096 (295 vs 316 us at C5); at N = 2048 the plain
 // 16 x 16 x 8 plan is faster (141.9 vs 150.6 us at 2048 x 4096 fp64: the R1 = 8 first stage spills) and so is 16 x 8 x 8 at N = 1024
 // (65.9 vs 74.4 us at 1024 x 4096 fp64): with one row pair per CTA several CTAs share an SM and hide each other's barriers
 template <int N> __host__ __device__ constexpr bool fft_wl_supported() { return N == 4096; }
 template <int N> __host__ __device__ constexpr int fft_wl_r1() { return N / 256; }
+// stage 2 reads all 15 twiddle powers (fp64: 36 fewer DP instructions per butterfly) or 6 base powers and derives 9 (fp32: the
+// shared-memory data pipe, not the FMA pipe, is the scarcer resource there)
+template <typename T> __host__ __device__ constexpr bool fft_wl_stage2_all() { return sizeof(T) == 8; }
 __host__ __device__ constexpr int fft_wl_r1_rt(int N) { return N / 256; }
-__host__ __device__ constexpr int fft_wl_tw_elems_rt(int N) { return 6 * fft_wl_r1_rt(N) + 6 * (N / 16); }
+__host__ __device__ constexpr int fft_wl_tw_elems_rt(int N) { return 15 * fft_wl_r1_rt(N) + 6 * (N / 16); }
 // shared-memory index padding i + (i >> A) + (i >> B) and the in-group rotation, chosen per element size and N (searched
 // exhaustively: every access of the plan - stage-1 writes from either base index, stage-2/3 reads and writes, the
 // last-stage store - is then bank-conflict free for 16-byte (fp64) and 8-byte (fp32) elements).
@@ -467,7 +473,18 @@ __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__
   cplx<T> v[16];
 #pragma unroll
   for (int r = 0; r < 16; ++r) v[r] = sm[fft_wl_pad<T, N>(j + r * TPL)];
-  apply_stage_twiddles<16, DIR>(v, tabw + kk, R1);
+  if constexpr (fft_wl_stage2_all<T>()) {
+#pragma unroll
+    for (int r = 1; r < 16; ++r) {             // stage-2 twiddles W_{16 R1}^{kk r}: all 15 powers, shared-memory broadcasts
+      const cplx<T> w = tabw[(r - 1) * R1 + kk];
+      v[r] = v[r] * (DIR < 0 ? w : conj(w));
+    }
+  } else {
+    TwBase<16, T> b;                           // 6 base powers (rows 1, 2, 3, 4, 8, 12 of the table), the other 9 derived
+#pragma unroll
+    for (int i = 0; i < 6; ++i) { const cplx<T> w = tabw[(fft_tw_base_power(16, i) - 1) * R1 + kk]; b.w[i] = DIR < 0 ? w : conj(w); }
+    apply_stage_twiddles<16>(v, b);
+  }
   dft16<DIR>(v);
   __syncwarp();                                // the group's 256 positions have been read by its 16 threads
 #pragma unroll
@@ -475,7 +492,12 @@ __device__ __forceinline__ void fft_line_wl(int j0, int t, cplx<T>* __restrict__
   __syncwarp();
 #pragma unroll
   for (int qq = 0; qq < 16; ++qq) v[qq] = sm[fft_wl_pad<T, N>(TPL * qq + kk + R1 * fft_wl_rot<T, N>(q, qq))];
-  apply_stage_twiddles<16, DIR>(v, tabw + 6 * R1 + t, TPL);
+  {
+    TwBase<16, T> b;                           // stage-3 base powers from the shared-memory copy (thread order: conflict-free)
+#pragma unroll
+    for (int i = 0; i < 6; ++i) { const cplx<T> w = tabw[15 * R1 + i * TPL + t]; b.w[i] = DIR < 0 ? w : conj(w); }
+    apply_stage_twiddles<16>(v, b);
+  }
   dft16<DIR>(v);
   if (SYNC_LAST) __syncthreads();              // the store goes to shared memory: every group has finished reading it
 #pragma unroll

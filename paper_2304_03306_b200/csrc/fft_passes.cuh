@@ -47,8 +47,9 @@ template <typename T, int NX> struct RowCfg {
   static constexpr int MINB = THREADS <= 256 ? TTSH_ROW_MINB : 1;              // caps registers per thread
 };
 // columns per CTA of the column pass = tile width CW of the two complex arrays: CW * Ny/2 complex values near 64 KiB
-// of shared memory (fp64 4096: 2 columns, fp32 4096: 4), at least 2 and at most 8 columns
+// of shared memory (fp64 4096: 2 columns, fp32 4096: 4), at least 2 and at most 8 columns (1 at Ny = 16384)
 __host__ __device__ constexpr int col_tile_width(int Ny, int elem_bytes) {
+  if (Ny >= 16384) return 1;      // 8192-point half-length transforms: one column per CTA (128 KB in fp64)
   int cw = (TTSH_COL_BYTES / elem_bytes) / (Ny / 2);
 #ifndef TTSH_COL_CAP_SMALL
 #define TTSH_COL_CAP_SMALL 4
@@ -60,7 +61,7 @@ template <typename T, int NY> struct ColCfg {
   static constexpr int NH = NY / 2;
   static constexpr int TPL = fft_tpl<NH>();
   static constexpr int L = col_tile_width(NY, (int)sizeof(cplx<T>));
-  static constexpr int LSHIFT = L == 2 ? 1 : (L == 4 ? 2 : 3);
+  static constexpr int LSHIFT = L == 1 ? 0 : (L == 2 ? 1 : (L == 4 ? 2 : 3));
   static constexpr int THREADS = L * TPL;
   // line stride: a 128-byte wavefront holds W = 128 / sizeof(cplx<T>) elements and is filled by W threads = W/L consecutive
   // butterflies x L lines (col_thread_map), so the lines must start W/L elements apart modulo W to land in distinct banks
@@ -116,7 +117,7 @@ __device__ __forceinline__ void st_quad(float* p, float a, float b, float c, flo
 template <typename T>
 __device__ __forceinline__ cplx<T> apply_spec_mode(int mode, cplx<T> w, int mx, int my, const Geom& g, const double* v0) {
   if (mode == SM_ONE) return w;
-  if (mode == SM_LOWPASS4) return is_cut(mx, my, g.Nx, g.Ny, 1, 4) ? mk<T>(0, 0) : w;
+  if (mode == SM_LOWPASS4) return is_cut(g, mx, my, 1, 4) ? mk<T>(0, 0) : w;
   const T ky = (T)g.dky * (T)my;
   if (mode == SM_IKY_MEANX && mx == 0 && my == 0) return mk<T>((T)v0[0], (T)0);
   return ky * mul_i(w);
@@ -171,7 +172,9 @@ k_inv_col(const __grid_constant__ Geom g, const __grid_constant__ Batch batch, c
 
   const bool half_rule = (2 * My == NH);     // the paper's 1/2 rule: |my| <= Ny/4 (uniform branch)
   const cplx<T> wj = ldg_c(tabS + j);         // W_Ny^j
-  if (G == 1 && threadIdx.x == 0 && blockIdx.x == 0) {  // L2 prefetch of the spectrum tile the CTAs about one wave later read
+  // L2 prefetch of the spectrum tile the CTAs about one wave later read (bulk prefetch: 16-byte granules, so not for the
+  // one-column fp32 tiles of Ny = 16384, whose rows are 8 bytes)
+  if ((L * sizeof(cplx<T>)) % 16 == 0 && G == 1 && threadIdx.x == 0 && blockIdx.x == 0) {
     const int ni = item + TTSH_PF_DIST_COL;
     if (ni < nitems) {
       const int nt = ni % g.NT, nz = ni / g.NT;

@@ -128,7 +128,31 @@ template <typename T> cudaError_t launch_spec_scale_axpy(const Geom& g, const do
   return launch_pdl(k_spec_scale_axpy<T>, dim3(blocks_for(n, 256, GRID_CAP), count), dim3(256), 0, s, n, coef, (const cplx<T>*)x, (cplx<T>*)y, x0, y0, ystride);
 }
 
+// Gram matrix of nvec tangent vectors (spectra v + j vstride bytes, mean flows v0 + j vstride bytes) into G[nvec][nvec] (device);
+// partial: nvec * nvec * DIAG_BLOCKS doubles
+template <typename T> cudaError_t launch_gram(const Geom& g, const void* v, const double* v0, size_t vstride, int nvec, double* partial, double* G,
+                                              cudaStream_t s) {
+  const int tiles = (nvec + GRAM_TILE - 1) / GRAM_TILE;
+  const size_t n = (size_t)g.NT * g.Hy * g.CW;
+  const int nb = blocks_for(n, 256, DIAG_BLOCKS);      // small spectra: no more blocks than there is work (nvec * tiles of them each)
+  cudaError_t e = launch_pdl(k_gram_partial<T>, dim3(nb, nvec, tiles), dim3(256), 0, s, g, (const cplx<T>*)v, vstride, nvec, partial);
+  if (e != cudaSuccess) return e;
+  return launch_pdl(k_gram_final, dim3(nvec, nvec), dim3(32), 0, s, nb, nvec, (const double*)partial, v0, vstride, G);
+}
+// Cholesky factor of G and its inverse on the device (nvec <= 64); logr[i] += log R_ii; *flag set on a breakdown
+cudaError_t launch_chol_inv(int nvec, const double* G, double* S, double* logr, int* flag, cudaStream_t s) {
+  if (nvec < 1 || nvec > 64) return cudaErrorInvalidValue;
+  return launch_pdl(k_chol_inv, dim3(1), dim3(64), 0, s, nvec, G, S, logr, flag);
+}
+// A <- A S (S upper triangular, device, row-major), psi^ = w^/k^2 and the mean flows alongside
+template <typename T> cudaError_t launch_tri_apply(const Geom& g, int nvec, const double* S, void* v, void* psi, double* v0, size_t vstride, cudaStream_t s) {
+  const size_t n = (size_t)g.NT * g.Hy * g.CW;
+  return launch_pdl(k_tri_apply<T>, dim3(blocks_for(n, 256, GRID_CAP)), dim3(256), 0, s, g, nvec, S, (cplx<T>*)v, (cplx<T>*)psi, v0, vstride);
+}
+
 #define INST(T) \
+  template cudaError_t launch_gram<T>(const Geom&, const void*, const double*, size_t, int, double*, double*, cudaStream_t); \
+  template cudaError_t launch_tri_apply<T>(const Geom&, int, const double*, void*, void*, double*, size_t, cudaStream_t); \
   template cudaError_t launch_realspace_tangent<T>(const Geom&, const Model&, const void*, const void*, const void*, const void*, void*, void*, void*, cudaStream_t, int, size_t); \
   template cudaError_t launch_spec_dot<T>(const Geom&, const void*, const void*, const double*, const double*, int, size_t, int, double*, double*, double*, cudaStream_t); \
   template cudaError_t launch_spec_scale_axpy<T>(const Geom&, const double*, const void*, void*, const double*, double*, int, size_t, cudaStream_t); \

@@ -126,7 +126,7 @@ k_spectral(Geom g, Model m, const cplx<T>* __restrict__ Fx_, const cplx<T>* __re
   if (mx >= g.Wx) return;
   const int my = q <= g.My ? q : q - g.Hy;
   const bool zero = (mx == 0 && my == 0);
-  const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
+  const bool cut = is_cut(g, mx, my, g.num, g.den);
   if (mx == 0) {
     if (my < 0) return;                                   // written by the thread of (0, -my)
     if (zero) {
@@ -182,7 +182,7 @@ k_spectral_p2(Geom g, Model m, const cplx<T>* __restrict__ A_, const cplx<T>* __
   const int mx = t * g.CW + (rem & (g.CW - 1));
   if (mx >= g.Wx) return;
   const int my = q <= g.My ? q : q - g.Hy;
-  const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
+  const bool cut = is_cut(g, mx, my, g.num, g.den);
   const T dt = (T)m.dt;
   auto factor = [&](int my_) -> T {          // exp(sigma(k) dt), line 4
     const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my_);
@@ -239,7 +239,7 @@ k_spectral_init(Geom g, const cplx<T>* __restrict__ Vx, const cplx<T>* __restric
   const int mx = t * g.CW + (rem & (g.CW - 1));
   if (mx >= g.Wx) return;
   const int my = q <= g.My ? q : q - g.Hy;
-  const bool cut = is_cut(mx, my, g.Nx, g.Ny, g.num, g.den);
+  const bool cut = is_cut(g, mx, my, g.num, g.den);
   auto curl = [&](int my_, size_t id) -> cplx<T> {
     const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my_);
     return kx * mul_i(Vy[id]) - ky * mul_i(Vx[id]);
@@ -638,6 +638,158 @@ k_spec_scale_axpy(size_t n, const double* __restrict__ coef_, const cplx<T>* __r
   if (blockIdx.x == 0 && threadIdx.x < 2) {
     const double cd = coef[0];
     y0[threadIdx.x] = x0 ? y0[threadIdx.x] - cd * x0[threadIdx.x] : cd * y0[threadIdx.x];
+  }
+}
+
+
+// ---------------------------------------------------------------------------------------
+// Blocked QR of the tangent vectors (CholeskyQR2) in the same inner product as above: G = A^T A in one launch, R = chol(G) on
+// the host (nvec <= 64), A <- A R^-1 in one launch, twice; R = R2 R1.  Against Gram-Schmidt row by row (6 launches per vector)
+// this is 3 launches per pass whatever nvec.
+// k_gram_partial: grid (blocks, nvec, ceil(nvec / 8)); block (b, i, jt) accumulates <v_i, v_j> for the 8 vectors j of tile jt with
+// j >= i over its share of the spectrum.  partial[(i nvec + j) nblocks + b].
+// ---------------------------------------------------------------------------------------
+constexpr int GRAM_TILE = 8;
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_gram_partial(Geom g, const cplx<T>* __restrict__ v_, size_t vstride, int nvec, double* __restrict__ partial) {
+  pdl_wait();
+  const int i = blockIdx.y, j0 = blockIdx.z * GRAM_TILE;
+  if (j0 + GRAM_TILE <= i) return;                      // nothing of this tile lies on or above the diagonal
+  const cplx<T>* __restrict__ a = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(v_) + (size_t)i * vstride);
+  const size_t n = (size_t)g.NT * g.Hy * g.CW;
+  double acc[GRAM_TILE];
+#pragma unroll
+  for (int u = 0; u < GRAM_TILE; ++u) acc[u] = 0.0;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+    const int t = (int)(e / ((size_t)g.Hy * g.CW));
+    const int mx = t * g.CW + (int)(e & (size_t)(g.CW - 1));
+    if (mx >= g.Wx) continue;
+    const double wgt = mx == 0 ? 1.0 : 2.0;
+    const double ax = wgt * (double)a[e].x, ay = wgt * (double)a[e].y;
+#pragma unroll
+    for (int u = 0; u < GRAM_TILE; ++u) {
+      const int j = j0 + u;
+      if (j < i || j >= nvec) continue;
+      const cplx<T> b = reinterpret_cast<const cplx<T>*>(reinterpret_cast<const char*>(v_) + (size_t)j * vstride)[e];
+      acc[u] += ax * (double)b.x + ay * (double)b.y;
+    }
+  }
+  __shared__ double sh[8][GRAM_TILE];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int u = 0; u < GRAM_TILE; ++u) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc[u] += __shfl_down_sync(0xffffffffu, acc[u], o);
+    if (lane == 0) sh[wid][u] = acc[u];
+  }
+  __syncthreads();
+  if (threadIdx.x < GRAM_TILE) {
+    const int j = j0 + threadIdx.x;
+    if (j >= i && j < nvec) {
+      double s = 0.0;
+      for (int w = 0; w < 8; ++w) s += sh[w][threadIdx.x];
+      partial[((size_t)i * nvec + j) * gridDim.x + blockIdx.x] = s;
+    }
+  }
+}
+// one warp per entry (i, j >= i): G[i][j] = G[j][i] = sum of the partials + the mean-flow part
+__global__ void __launch_bounds__(32)
+k_gram_final(int nblocks, int nvec, const double* __restrict__ partial, const double* __restrict__ v0_, size_t vstride, double* __restrict__ G) {
+  pdl_wait();
+  const int i = blockIdx.y, j = blockIdx.x;
+  if (j < i) return;
+  double s = 0.0;
+  for (int b = threadIdx.x; b < nblocks; b += 32) s += partial[((size_t)i * nvec + j) * nblocks + b];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+  if (threadIdx.x == 0) {
+    const double* a0 = reinterpret_cast<const double*>(reinterpret_cast<const char*>(v0_) + (size_t)i * vstride);
+    const double* b0 = reinterpret_cast<const double*>(reinterpret_cast<const char*>(v0_) + (size_t)j * vstride);
+    s += a0[0] * b0[0] + a0[1] * b0[1];
+    G[i * nvec + j] = s;
+    G[j * nvec + i] = s;
+  }
+}
+// G = R^T R (R upper triangular, positive diagonal) and S = R^-1 for nvec <= 64, one block of 64 threads (thread j owns column
+// j); logr[i] += log R_ii.  A pivot at or below 1e-13 of its diagonal entry (numerically dependent vectors) sets *flag and leaves
+// S = identity, so that the following k_tri_apply changes nothing and the host can fall back to Gram-Schmidt.
+__global__ void __launch_bounds__(64) k_chol_inv(int M, const double* __restrict__ G, double* __restrict__ S, double* __restrict__ logr, int* flag) {
+  pdl_wait();
+  __shared__ double R[64][65];
+  __shared__ int bad;
+  const int j = threadIdx.x;
+  if (j == 0) bad = *flag;
+  for (int i = 0; i < M; ++i) R[i][j] = (j < M) ? G[i * M + j] : 0.0;
+  __syncthreads();
+  for (int k = 0; k < M && !bad; ++k) {
+    if (j == k) {
+      const double d = R[k][k];
+      if (!(d > 1e-13 * G[k * M + k]) || !isfinite(d)) bad = 1; else R[k][k] = sqrt(d);
+    }
+    __syncthreads();
+    if (bad) break;
+    if (j > k && j < M) R[k][j] /= R[k][k];
+    __syncthreads();
+    if (j > k && j < M)
+      for (int i = k + 1; i <= j; ++i) R[i][j] -= R[k][i] * R[k][j];
+    __syncthreads();
+  }
+  __syncthreads();
+  if (j < M) {
+    if (bad) {
+      for (int i = 0; i < M; ++i) S[i * M + j] = (i == j) ? 1.0 : 0.0;
+    } else {
+      // column j of S = R^-1 by back substitution (entries below the diagonal are zero)
+      double col[64];
+      col[j] = 1.0 / R[j][j];
+      for (int i = j - 1; i >= 0; --i) {
+        double v = 0.0;
+        for (int k = i + 1; k <= j; ++k) v -= R[i][k] * col[k];
+        col[i] = v / R[i][i];
+      }
+      for (int i = 0; i < M; ++i) S[i * M + j] = i <= j ? col[i] : 0.0;
+      logr[j] += log(R[j][j]);
+    }
+  }
+  if (j == 0 && bad) *flag = 1;
+}
+
+// A <- A S with S upper triangular (S = R^-1, row-major S[i nvec + j]): q_j = sum_{i <= j} S[i][j] a_i, computed in place from the
+// last column to the first (q_j needs only a_i, i <= j).  Also psi^_j = q_j / k^2 (line 13) and the mean-flow part (block 0).
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_tri_apply(Geom g, int nvec, const double* __restrict__ S, cplx<T>* v_, cplx<T>* __restrict__ psi_, double* v0_, size_t vstride) {
+  pdl_wait();
+  const size_t n = (size_t)g.NT * g.Hy * g.CW;
+  auto vec = [&](cplx<T>* p, int j) { return reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(p) + (size_t)j * vstride); };
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+    const int t = (int)(e / ((size_t)g.Hy * g.CW));
+    const int rem = (int)(e - (size_t)t * g.Hy * g.CW);
+    const int q = rem >> g.cw_shift;
+    const int mx = t * g.CW + (rem & (g.CW - 1));
+    const int my = q <= g.My ? q : q - g.Hy;
+    const bool dead = mx >= g.Wx || (mx == 0 && my == 0);
+    const T ik2 = dead ? (T)0 : inv_k2<T>(g, mx, my);
+    for (int j = nvec - 1; j >= 0; --j) {
+      double sx = 0.0, sy = 0.0;
+      for (int i = 0; i <= j; ++i) {
+        const double c = S[i * nvec + j];
+        const cplx<T> a = vec(v_, i)[e];
+        sx += c * (double)a.x; sy += c * (double)a.y;
+      }
+      const cplx<T> out = dead ? mk<T>(0, 0) : mk<T>((T)sx, (T)sy);
+      vec(v_, j)[e] = out;
+      vec(psi_, j)[e] = ik2 * out;
+    }
+  }
+  if (blockIdx.x == 0 && threadIdx.x < 2) {
+    for (int j = nvec - 1; j >= 0; --j) {
+      double s = 0.0;
+      for (int i = 0; i <= j; ++i)
+        s += S[i * nvec + j] * reinterpret_cast<double*>(reinterpret_cast<char*>(v0_) + (size_t)i * vstride)[threadIdx.x];
+      reinterpret_cast<double*>(reinterpret_cast<char*>(v0_) + (size_t)j * vstride)[threadIdx.x] = s;
+    }
   }
 }
 

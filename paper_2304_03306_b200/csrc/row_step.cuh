@@ -31,9 +31,11 @@ namespace ttsh {
 // consecutive row pairs of one member (64 threads; shared memory per thread does not depend on Nx, about 4 such CTAs per SM)
 template <int NX> __host__ __device__ constexpr int row_step_ens_lines() { return NX >= 1024 ? 1 : 1024 / NX; }
 
-template <typename T, int NX, int LL = 1> struct RowStepCfg {
+// TAN: the tangent-linear variant (ttsh_tangent_step): its pointwise stage reads the base fields w, v_x, v_y from the internal real
+// fields (row layout perm_index: x = j + k TPL), so it always runs the plain Stockham plan, whose threads own exactly those points.
+template <typename T, int NX, int LL = 1, bool TAN = false> struct RowStepCfg {
   using R = RowCfg<T, NX>;
-  static constexpr bool WL = fft_wl_supported<NX>();                   // warp-local FFT plan (fft_core.cuh)
+  static constexpr bool WL = fft_wl_supported<NX>() && !TAN;           // warp-local FFT plan (fft_core.cuh)
   // one row pair per CTA: for Nx <= 2048 several small CTAs share an SM and drift apart (measured +2-10 % over two
   // row pairs per CTA, which pass every barrier together)
   static constexpr int TPL = R::TPL, L = LL, THREADS = LL * TPL;
@@ -43,7 +45,12 @@ template <typename T, int NX, int LL = 1> struct RowStepCfg {
   static constexpr int SLOT = ((NX / 4 + 8) * 2 * (int)sizeof(cplx<T>) + 127) / 128 * 128;
   static constexpr size_t OFF_SLOTS = ((size_t)L * (LS + ST) * sizeof(cplx<T>) + 127) / 128 * 128;
   static constexpr size_t OFF_BARS = OFF_SLOTS + (size_t)L * 2 * SLOT;
-  static constexpr size_t SMEM = OFF_BARS + (size_t)L * 2 * sizeof(unsigned long long);
+  // warp-local plan: a copy of its twiddle table lives in shared memory (fft_core.cuh explains why)
+  static constexpr size_t OFF_TAB = (OFF_BARS + (size_t)L * 2 * sizeof(unsigned long long) + 15) / 16 * 16;
+  // fp64 only (C5: k_row_step 258.3 -> 253.5 us); in fp32 the L1 next to 101 KB of shared memory holds the 13 KB table and the
+  // copy only adds shared-memory wavefronts (137.0 us from global memory, 145.6 us from the copy)
+  static constexpr bool SMEM_TAB = WL && sizeof(T) == 8;
+  static constexpr size_t SMEM = OFF_TAB + (SMEM_TAB ? (size_t)fft_wl_tw_elems_rt(NX) * sizeof(cplx<T>) : 0);
 #ifndef TTSH_RS_MINB_F32
 #define TTSH_RS_MINB_F32 1
 #endif
@@ -85,7 +92,7 @@ __device__ __forceinline__ Quad<float> lds_quad(const float* p, int) {
 // row: the staged pairs of this row pair in shared memory ((A, B) of column mx at row + 2 mx).
 // MODE = RM_ONE or RM_NIKX_MEANY (ttsh_common.cuh).  1/2 rule only: retained mx = 0..NX/4.
 // With the warp-local plan the thread owns x = wl_j(j) + k TPL instead (tabX is then the warp-local table).
-template <typename T, int NX, int MODE, class Hook>
+template <typename T, int NX, int MODE, bool WL, class Hook>
 __device__ __forceinline__ void inv_row_regs(const cplx<T>* __restrict__ row, int j, cplx<T>* __restrict__ line,
                                              const cplx<T>* __restrict__ tabX, T scale, T dkx, T meany, cplx<T> (&out)[16],
                                              Hook hook) {
@@ -114,19 +121,19 @@ __device__ __forceinline__ void inv_row_regs(const cplx<T>* __restrict__ row, in
     return mk<T>(0, 0);
   };
   auto store = [&](int, int k, cplx<T> z) { out[k] = z; };
-  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, +1, false>(j, j, line, tabX, make_loader<1>(issue, finish), store, hook);
+  if constexpr (WL) fft_line_wl<T, NX, +1, false>(j, j, line, tabX, make_loader<1>(issue, finish), store, hook);
   else fft_line<T, NX, +1, false>(j, line, tabX, make_loader<1>(issue, finish), store, hook);
 }
 
 // forward transform of the 16 values a thread owns (slot k <-> x = jw + k TPL; jw = wl_j(j) for the warp-local plan, else j)
-template <typename T, int NX, bool SYNC_LAST, class Load, class Store, class Hook = NoHook>
+template <typename T, int NX, bool SYNC_LAST, bool WL, class Load, class Store, class Hook = NoHook>
 __device__ __forceinline__ void fwd_row_regs(int jw, int j, cplx<T>* __restrict__ line, const cplx<T>* __restrict__ tabX, Load load,
                                              Store store, Hook hook = Hook()) {
-  if constexpr (fft_wl_supported<NX>()) fft_line_wl<T, NX, -1, SYNC_LAST>(jw, j, line, tabX, load, store, hook);
+  if constexpr (WL) fft_line_wl<T, NX, -1, SYNC_LAST>(jw, j, line, tabX, load, store, hook);
   else fft_line<T, NX, -1, SYNC_LAST>(j, line, tabX, load, store, hook);
 }
-template <typename T, int NX> __device__ __forceinline__ int row_step_pad(int i) {
-  if constexpr (fft_wl_supported<NX>()) return fft_wl_pad<T, NX>(i);
+template <typename T, int NX, bool WL> __device__ __forceinline__ int row_step_pad(int i) {
+  if constexpr (WL) return fft_wl_pad<T, NX>(i);
   else return fft_pad<NX>(i);
 }
 
@@ -136,13 +143,18 @@ template <class P> __device__ __forceinline__ P* byte_off(P* p, size_t bytes) {
 
 // LL row pairs per CTA.  ENS: the persistent grid runs over the row pairs of `members` systems whose workspaces lie mstride
 // bytes apart (ttsh_ensemble_step); rpm = Ny/2 row pairs per member, a multiple of LL, so a CTA's lines share a member.
-template <typename T, int NX, int LL, bool ENS>
-__global__ void __launch_bounds__(RowStepCfg<T, NX, LL>::THREADS, RowStepCfg<T, NX, LL>::MINB)
+// TAN (with ENS: the members are the tangent vectors): inW / inVx / inPsi / outA / outB / v0 belong to the perturbation (dw~, dv_x~,
+// dpsi~; per vector, mstride apart), K and the base fields bw, bvx, bvy (internal real fields of the handle) are shared, and the
+// pointwise stage evaluates the derivative of lines 1-2 at the base state (pointwise.cuh, k_realspace_tangent).
+template <typename T, int NX, int LL, bool ENS, bool TAN = false>
+__global__ void __launch_bounds__(RowStepCfg<T, NX, LL, TAN>::THREADS, RowStepCfg<T, NX, LL, TAN>::MINB)
 k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, const cplx<T>* __restrict__ inW,
            const cplx<T>* __restrict__ inVx, const cplx<T>* __restrict__ inPsi, const T* __restrict__ K,
            cplx<T>* __restrict__ outA, cplx<T>* __restrict__ outB, const cplx<T>* __restrict__ tabX,
-           const double* __restrict__ v0, int nblk, int rpm, size_t mstride) {
-  using C = RowStepCfg<T, NX, LL>;
+           const double* __restrict__ v0, int nblk, int rpm, size_t mstride, const T* __restrict__ bw, const T* __restrict__ bvx,
+           const T* __restrict__ bvy) {
+  using C = RowStepCfg<T, NX, LL, TAN>;
+  static_assert(!TAN || ENS, "the tangent variant runs over the vectors as members");
   constexpr int TPL = C::TPL;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
@@ -172,6 +184,11 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
 
   if (leader) { mbar_init(bar0, 1); mbar_init(bar1, 1); }
   mbar_fence_init();
+  if constexpr (C::SMEM_TAB) {      // twiddle table -> shared memory (host-written at ttsh_create: no dependence on the preceding launch)
+    cplx<T>* stab = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_TAB);
+    for (int i = threadIdx.x; i < fft_wl_tw_elems_rt(NX); i += C::THREADS) stab[i] = ldg_c(tabX + i);
+    tabX = stab;
+  }
   __syncthreads();
   pdl_wait();          // inputs, K and v0 below are written by the preceding launches
   pdl_trigger();
@@ -190,6 +207,7 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
     if constexpr (ENS) meany = (T)(byte_off(v0, mo)[1] * g.inv_sqrt_ny);
     const int a = rp >> 1, p = rp & 1;
     const size_t offA = (size_t)(4 * a + p) * NX, offB = offA + 2 * (size_t)NX;
+    const size_t kmo = TAN ? 0 : mo;                    // K is shared by all tangent vectors
     const int nb = blk + gridDim.x;
     if (leader && nb < nblk) {   // L2 prefetch of what this line reads in the CTA's next iteration
       int nrp; size_t nmo;
@@ -198,22 +216,28 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
       prefetch_l2_bulk(byte_off(inVx, nmo) + (size_t)nrp * in_stride, in_bytes);
       prefetch_l2_bulk(byte_off(inPsi, nmo) + (size_t)nrp * in_stride, in_bytes);
       const size_t nA = (size_t)(4 * (nrp >> 1) + (nrp & 1)) * NX;
-      prefetch_l2_bulk(byte_off(K, nmo) + nA, k_bytes);
-      prefetch_l2_bulk(byte_off(K, nmo) + nA + 2 * (size_t)NX, k_bytes);
+      const size_t nkmo = TAN ? 0 : nmo;
+      prefetch_l2_bulk(byte_off(K, nkmo) + nA, k_bytes);
+      prefetch_l2_bulk(byte_off(K, nkmo) + nA + 2 * (size_t)NX, k_bytes);
+      if constexpr (TAN) {   // the six base rows of the next row pair
+        prefetch_l2_bulk(bw + nA, k_bytes); prefetch_l2_bulk(bw + nA + 2 * (size_t)NX, k_bytes);
+        prefetch_l2_bulk(bvx + nA, k_bytes); prefetch_l2_bulk(bvx + nA + 2 * (size_t)NX, k_bytes);
+        prefetch_l2_bulk(bvy + nA, k_bytes); prefetch_l2_bulk(bvy + nA + 2 * (size_t)NX, k_bytes);
+      }
     }
     cplx<T> H[16], V[16];
     // ---- a2 / a6: w, v_x, v_y of the two rows ----
     mbar_wait(bar0, ph0); ph0 ^= 1;
-    inv_row_regs<T, NX, RM_ONE>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
+    inv_row_regs<T, NX, RM_ONE, C::WL>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
                                 [&]() { if (leader) bulk_load(slot0, byte_off(inPsi, mo) + (size_t)rp * in_stride, in_bytes, bar0); });
 #pragma unroll
     for (int k = 0; k < 16; ++k) stash[k * TPL] = V[k];                     // w
     mbar_wait(bar1, ph1); ph1 ^= 1;
-    inv_row_regs<T, NX, RM_ONE>(reinterpret_cast<const cplx<T>*>(slot1), j, line, tabX, scale_i, dkx, meany, H,
-                                [&]() { if (leader) bulk_load(slot1, byte_off(K, mo) + offA, k_bytes, bar1); });              // v_x
+    inv_row_regs<T, NX, RM_ONE, C::WL>(reinterpret_cast<const cplx<T>*>(slot1), j, line, tabX, scale_i, dkx, meany, H,
+                                [&]() { if (leader) bulk_load(slot1, byte_off(K, kmo) + offA, k_bytes, bar1); });             // v_x
     mbar_wait(bar0, ph0); ph0 ^= 1;
-    inv_row_regs<T, NX, RM_NIKX_MEANY>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
-                                       [&]() { if (leader) bulk_load(slot0, byte_off(K, mo) + offB, k_bytes, bar0); });       // v_y
+    inv_row_regs<T, NX, RM_NIKX_MEANY, C::WL>(reinterpret_cast<const cplx<T>*>(slot0), j, line, tabX, scale_i, dkx, meany, V,
+                                       [&]() { if (leader) bulk_load(slot0, byte_off(K, kmo) + offB, k_bytes, bar0); });      // v_y
     // ---- a3: lines 1-2 of Algorithm 1, pointwise;  V <- Gx,  H <- Gy,  stash <- S'  (all scaled for the forward pass) ----
     mbar_wait(bar1, ph1); ph1 ^= 1;
     mbar_wait(bar0, ph0); ph0 ^= 1;
@@ -224,6 +248,30 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const Quad<T> ka = lds_quad(KA + (q * TPL + j) * 4, sw), kb = lds_quad(KB + (q * TPL + j) * 4, sw);
+        if constexpr (TAN) {
+          // derivative of lines 1-2 at the base state (u, v, om): with c = -beta (u^2 + v^2) - gamma_v K, dc = -2 beta (u du + v dv),
+          //   dGx = dc u + c du + lambda0 (dv om + v dom),  dGy = dc v + c dv - lambda0 (du om + u dom),  dS' = -gamma_w K dom
+          // one row at a time (three base quads in flight instead of six: the stage runs at the register limit)
+          const size_t e = (size_t)(q * TPL + j) * 4;
+#pragma unroll
+          for (int r = 0; r < 2; ++r) {
+            const size_t off = (r ? offB : offA) + e;
+            const Quad<T> om = ld_quad(bw + off), u = ld_quad(bvx + off), v = ld_quad(bvy + off);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const int k = 4 * q + i;
+              T* sp = reinterpret_cast<T*>(stash + k * TPL) + r;            // dw of row r, then dS' of row r
+              const T kk = r ? kb.v[i] : ka.v[i], dom = *sp;
+              const T du = r ? H[k].y : H[k].x, dv = r ? V[k].y : V[k].x;
+              const T c = -beta * (u.v[i] * u.v[i] + v.v[i] * v.v[i]) - gv * kk;
+              const T dc = (T)-2 * beta * (u.v[i] * du + v.v[i] * dv);
+              const T gx = scale_f * (dc * u.v[i] + c * du + lam * (dv * om.v[i] + v.v[i] * dom));
+              const T gy = scale_f * (dc * v.v[i] + c * dv - lam * (du * om.v[i] + u.v[i] * dom));
+              if (r) { V[k].y = gx; H[k].y = gy; } else { V[k].x = gx; H[k].x = gy; }
+              *sp = ngw * (kk * dom);
+            }
+          }
+        } else {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           const int k = 4 * q + i;
@@ -237,14 +285,15 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
           H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
           stash[k * TPL] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));          // S'
         }
+        }
       }
     }
     // ---- a4, transform 1: Gx -> B~ (its first barrier frees both slots: stage the next row pair) ----
     auto keep = [&](int k) -> bool { return k <= 3 || k >= 12 || (k == 4 && j == 0); };
     auto ident = [&](int, int, cplx<T> r) -> cplx<T> { return r; };
     {
-      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX>(mm)] = z; };
-      fwd_row_regs<T, NX, true>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), store, [&]() {
+      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX, C::WL>(mm)] = z; };
+      fwd_row_regs<T, NX, true, C::WL>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), store, [&]() {
         if (leader && nb < nblk) {
           int nrp; size_t nmo;
           locate(nb * C::L + c, nrp, nmo);
@@ -254,8 +303,8 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
       });
       __syncthreads();
       for (int mx = j; mx < Wx; mx += TPL) {
-        const cplx<T> zp = line[row_step_pad<T, NX>(mx)];
-        const cplx<T> zm = conj(line[row_step_pad<T, NX>((NX - mx) & (NX - 1))]);
+        const cplx<T> zp = line[row_step_pad<T, NX, C::WL>(mx)];
+        const cplx<T> zm = conj(line[row_step_pad<T, NX, C::WL>((NX - mx) & (NX - 1))]);
         st_pair(byte_off(outB, mo) + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
       }
     }
@@ -267,16 +316,16 @@ k_row_step(const __grid_constant__ Geom g, const __grid_constant__ Model m, cons
         if (k <= 4) H[k] = (dkx * (T)mm) * mul_i(z);
         else if (k >= 12) H[k] = (dkx * (T)(mm - NX)) * mul_i(z);
       };
-      fwd_row_regs<T, NX, false>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), store);
+      fwd_row_regs<T, NX, false, C::WL>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), store);
     }
     // ---- transform 3: S' -> A~ = unpack(i k_m Zgy + Zs) ----
     {
-      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX>(mm)] = z + H[k]; };
-      fwd_row_regs<T, NX, true>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return stash[k * TPL]; }, ident), store);
+      auto store = [&](int mm, int k, cplx<T> z) { if (keep(k)) line[row_step_pad<T, NX, C::WL>(mm)] = z + H[k]; };
+      fwd_row_regs<T, NX, true, C::WL>(jw, j, line, tabX, make_loader<1>([&](int, int k) -> cplx<T> { return stash[k * TPL]; }, ident), store);
       __syncthreads();
       for (int mx = j; mx < Wx; mx += TPL) {
-        const cplx<T> zp = line[row_step_pad<T, NX>(mx)];
-        const cplx<T> zm = conj(line[row_step_pad<T, NX>((NX - mx) & (NX - 1))]);
+        const cplx<T> zp = line[row_step_pad<T, NX, C::WL>(mx)];
+        const cplx<T> zm = conj(line[row_step_pad<T, NX, C::WL>((NX - mx) & (NX - 1))]);
         cplx<T> sa = (T)0.5 * (zp + zm), sb = (T)0.5 * mul_ni(zp - zm);
         if (mx == 0) {                // real numbers S'~(0,y) and Gy~(0,y) travel together (k_fwd_row_fused)
           sa = mk<T>(sa.x, zg0.x);

@@ -19,7 +19,7 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-inline bool pow2_in_range(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
+inline bool pow2_in_range(int n) { return n >= 64 && n <= 16384 && (n & (n - 1)) == 0; }   // PAPER.md:271 (8192), :282 (16384)
 
 struct Layout {
   size_t tabX, tabXw, tabY, tabS, K, K2, what, psihat, v0, diag_partial, diag_out, R[5], Tm[5], S[3], total;
@@ -29,9 +29,11 @@ Geom make_geom(int Nx, int Ny, double dx, int num, int den, size_t w) {
   Geom g;
   g.Nx = Nx; g.Ny = Ny;
   g.num = num; g.den = den;
+  const int gmin = Nx < Ny ? Nx : Ny;
+  g.cut_gx = Nx / gmin; g.cut_gy = Ny / gmin; g.cut_c = g.cut_gx * g.cut_gy * gmin;
   g.Wx = (int)((long long)num * Nx / (2LL * den)) + 1;
   g.CW = col_tile_width(Ny, (int)(2 * w));
-  g.cw_shift = g.CW == 2 ? 1 : (g.CW == 4 ? 2 : 3);
+  g.cw_shift = g.CW == 1 ? 0 : (g.CW == 2 ? 1 : (g.CW == 4 ? 2 : 3));
   g.NT = (g.Wx + g.CW - 1) / g.CW;
   g.Wxp = g.NT * g.CW;
   g.My = (int)((long long)num * Ny / (2LL * den));
@@ -54,7 +56,7 @@ Layout make_layout(int Nx, int Ny, size_t w) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
   L.tabX = take((size_t)Nx * cw);
-  L.tabXw = take((size_t)Nx * cw);         // warp-local plan tables (fft_core.cuh), 6 (Nx/256 + Nx/16) entries
+  L.tabXw = take((size_t)Nx * cw);         // warp-local plan tables (fft_core.cuh), 6 (Nx/256 + Nx/16) entries; Nx = 16384: W_Nx^j, j < Nx/32
   L.tabY = take((size_t)Ny * cw);
   L.tabS = take((size_t)Ny * cw);
   L.K = take(P * w);
@@ -90,13 +92,15 @@ struct ttsh_handle {
   long long launches;
   int sticky;
   std::string err;
-  cudaGraphExec_t graph_exec;
+  cudaGraphExec_t graph_exec;      // one captured Euler step
+  cudaGraphExec_t graph_exec_k;    // GRAPH_K captured Euler steps (grids up to 256^2: one graph launch costs as much as the step)
   bool graph_ok;
   int advection_form;
   int device;           // CUDA device of the workspace: every entry point must be called with it current
-  int rs_slots, rs_slots_ens;   // persistent grid of k_row_step on this device (single system / ensemble variant)
+  int rs_slots, rs_slots_ens, rs_slots_tan;   // persistent grid of k_row_step on this device (single system / ensemble / tangent variant)
   bool row_step_ok;     // the fused row-step kernel supports this grid / dtype / dealias fraction
   bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
+  bool real_rows;       // Nx = 16384: one real row per half-length transform (fft_rows_real.cuh); internal real fields in natural order
 };
 
 struct ttsh_psd {
@@ -118,7 +122,7 @@ struct ttsh_tangent {
   double* v0;
   void *real[3], *inter[3], *spec[3];
   std::vector<bool> set;
-  double *partial, *coef, *rdiag;
+  double *partial, *coef, *rdiag, *gram;
 };
 template <class P> static P* vec_ptr(const ttsh_tangent* s, P* p0, int i) {
   return reinterpret_cast<P*>(reinterpret_cast<char*>(p0) + (size_t)i * s->stride);
@@ -179,16 +183,16 @@ template <typename T> void fill_stage_tables(std::vector<unsigned char>& buf, in
     ns *= R;
   }
 }
-// tables of the warp-local plan N = R1 x 16 x 16 (fft_core.cuh, fft_line_wl): stage 2 [6][R1], stage 3 [6][TPL] in thread order
+// tables of the warp-local plan N = R1 x 16 x 16 (fft_core.cuh, fft_line_wl): stage 2 [15 powers][R1], stage 3 [6 base powers][TPL] in thread order
 template <typename T> void fill_stage_tables_wl(std::vector<unsigned char>& buf, int N) {
   const int R1 = fft_wl_r1_rt(N), TPL = N / 16;
   buf.assign((size_t)(fft_wl_tw_elems_rt(N) + 1) * 2 * sizeof(T), 0);
   T* t = reinterpret_cast<T*>(buf.data());
-  for (int b = 0; b < 6; ++b) {
-    for (int k = 0; k < R1; ++k) put_twiddle<T>(t + 2 * (size_t)(b * R1 + k), (long long)k * fft_tw_base_power(16, b), 16LL * R1);
+  for (int r = 1; r < 16; ++r)
+    for (int k = 0; k < R1; ++k) put_twiddle<T>(t + 2 * (size_t)((r - 1) * R1 + k), (long long)k * r, 16LL * R1);
+  for (int b = 0; b < 6; ++b)
     for (int th = 0; th < TPL; ++th)
-      put_twiddle<T>(t + 2 * (size_t)(6 * R1 + b * TPL + th), (long long)fft_wl_j_rt(th, R1) * fft_tw_base_power(16, b), (long long)N);
-  }
+      put_twiddle<T>(t + 2 * (size_t)(15 * R1 + b * TPL + th), (long long)fft_wl_j_rt(th, R1) * fft_tw_base_power(16, b), (long long)N);
 }
 // split twiddles of the column pass: W_Ny^p, p < Ny/2
 template <typename T> void fill_split_table(std::vector<unsigned char>& buf, int Ny) {
@@ -231,12 +235,12 @@ int enqueue_inverse(ttsh_handle* h, void* w, void* gx, void* gy, void* vx, void*
   if (vx) rb.f[nr++] = op(h->Tm[3], vx, RM_ONE);
   if (vy) rb.f[nr++] = op(h->Tm[2], vy, RM_NIKX_MEANY);
   if (nr) {
-    TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, h->v0, h->stream));
+    TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, h->tabXw, h->v0, h->stream));
     h->launches++;
   }
   if (psi) {
     Batch pb = make_batch({op(h->Tm[2], psi, RM_ONE)});
-    TRY(h, DISPATCH(h, launch_inv_row, h->g, pb, 1, h->tabX, h->v0, h->stream));
+    TRY(h, DISPATCH(h, launch_inv_row, h->g, pb, 1, h->tabX, h->tabXw, h->v0, h->stream));
     h->launches++;
   }
   return TTSH_OK;
@@ -250,7 +254,7 @@ int enqueue_forward(ttsh_handle* h, int n, const void* const* src) {
     rb.f[i] = op(src[i], h->Tm[i], 0);
     cb.f[i] = op(h->Tm[i], h->S[i], 0);
   }
-  TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, n, h->tabX, h->stream));
+  TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, n, h->tabX, h->tabXw, h->stream));
   TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, n, h->tabY, h->tabS, h->stream));
   h->launches += 2;
   return TTSH_OK;
@@ -274,12 +278,12 @@ int enqueue_stage(ttsh_handle* h, int stage) {
       if (h->advection_form == TTSH_ADVECTION_CONSERVATIVE) {
         Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE | RM_PERM), op(h->Tm[3], h->R[3], RM_ONE | RM_PERM),
                                op(h->Tm[2], h->R[4], RM_NIKX_MEANY | RM_PERM)});
-        TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 3, h->tabX, h->v0, h->stream));
+        TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 3, h->tabX, h->tabXw, h->v0, h->stream));
       } else {
         Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE | RM_PERM), op(h->Tm[0], h->R[1], RM_IKX | RM_PERM),
                                op(h->Tm[1], h->R[2], RM_ONE | RM_PERM), op(h->Tm[3], h->R[3], RM_ONE | RM_PERM),
                                op(h->Tm[2], h->R[4], RM_NIKX_MEANY | RM_PERM)});
-        TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 5, h->tabX, h->v0, h->stream));
+        TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 5, h->tabX, h->tabXw, h->v0, h->stream));
       }
       h->launches++;
       return TTSH_OK;
@@ -293,7 +297,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
       return TTSH_OK;
     case TTSH_STAGE_FWD_ROW: {
       Batch rb = make_batch({op(h->R[1], h->Tm[0], RM_PERM), op(h->R[2], h->Tm[1], RM_PERM), op(h->R[0], h->Tm[2], RM_PERM)});
-      TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->stream));
+      TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->tabXw, h->stream));
       h->launches++;
       return TTSH_OK;
     }
@@ -304,7 +308,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
       return TTSH_OK;
     }
     case TTSH_STAGE_REAL_FWD_ROW:     // a3 + row half of a4 in one kernel (conservative form only)
-      if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
+      if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || h->real_rows) return TTSH_ERR_INVALID_ARG;
       TRY(h, DISPATCH(h, launch_fwd_row_fused, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, h->Tm[1], h->Tm[4], h->tabX, h->stream));
       h->launches++;
       return TTSH_OK;
@@ -340,7 +344,9 @@ int enqueue_step(ttsh_handle* h) {
   static const int rowstep[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_ROW_STEP, TTSH_STAGE_FWD_COL_P2, TTSH_STAGE_SPECTRAL_P2};
   static const int plain[] = {TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL, TTSH_STAGE_FWD_ROW, TTSH_STAGE_FWD_COL,
                               TTSH_STAGE_SPECTRAL};
-  const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE;
+  // conservative form: 4 launches where the fused row-step kernel applies, else 5 (fused real-space + forward row pass); the
+  // literal form and Nx = 16384 (real-row passes, no fused row kernels) run the 6-launch sequence
+  const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows;
   const int* seq = f ? (h->row_step_ok ? rowstep : fused) : plain;
   const int n = f ? (h->row_step_ok ? 4 : 5) : 6;
   for (int i = 0; i < n; ++i) {
@@ -350,7 +356,17 @@ int enqueue_step(ttsh_handle* h) {
   return TTSH_OK;
 }
 inline int launches_per_step(const ttsh_handle* h) {
-  return h->advection_form == TTSH_ADVECTION_CONSERVATIVE ? (h->row_step_ok ? 4 : 5) : 6;
+  return (h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows) ? (h->row_step_ok ? 4 : 5) : 6;
+}
+
+// natural <-> internal row layout of a real field (to_perm = 1: natural -> internal).  On real-row grids the internal layout IS
+// the natural one.
+int copy_real(ttsh_handle* h, const void* src, void* dst, int to_perm) {
+  const size_t P = (size_t)h->Nx * h->Ny;
+  if (h->real_rows) TRY(h, cudaMemcpyAsync(dst, src, P * (size_t)h->dtype, cudaMemcpyDeviceToDevice, h->stream));
+  else TRY(h, DISPATCH(h, launch_permute, h->Nx, P, src, dst, to_perm, h->stream));
+  h->launches++;
+  return TTSH_OK;
 }
 
 int apply_mask_k(ttsh_handle* h, const void* mask, ttsh_mask_kind kind);
@@ -369,11 +385,7 @@ int apply_mask_k(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
     h->launches++;
     return TTSH_OK;
   }
-  if (kind == TTSH_MASK_PROCESSED) {   // K is kept in the permuted internal row layout
-    TRY(h, DISPATCH(h, launch_permute, h->Nx, P, mask, h->K, 1, h->stream));
-    h->launches++;
-    return TTSH_OK;
-  }
+  if (kind == TTSH_MASK_PROCESSED) return copy_real(h, mask, h->K, 1);   // K is kept in the internal row layout
   // Algorithm 2: K = ( iDFT[ lowpass_{1/4}( DFT[K_naive] ) ] )^2
   TRY(h, DISPATCH(h, launch_mask_to_real, P, static_cast<const unsigned char*>(mask), h->R[0], h->stream));
   h->launches++;
@@ -383,7 +395,7 @@ int apply_mask_k(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   Batch cb = make_batch({op(h->S[0], h->Tm[0], SM_LOWPASS4)});
   TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 1, h->tabY, h->tabS, h->v0, h->stream));
   Batch rb = make_batch({op(h->Tm[0], h->R[0], RM_ONE | RM_PERM)});
-  TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 1, h->tabX, h->v0, h->stream));
+  TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, 1, h->tabX, h->tabXw, h->v0, h->stream));
   TRY(h, DISPATCH(h, launch_square, P, h->R[0], h->K, h->stream));
   h->launches += 3;
   return TTSH_OK;
@@ -434,10 +446,11 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   for (int i = 0; i < 5; ++i) h->Tm[i] = h->ws + L.Tm[i];
   for (int i = 0; i < 3; ++i) h->S[i] = h->ws + L.S[i];
   h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
-  h->graph_exec = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
+  h->graph_exec = h->graph_exec_k = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
   h->row_step_ok = h->dtype == TTSH_F64 ? row_step_supported<double>(h->g) : row_step_supported<float>(h->g);
   h->row_step_wl = Nx == 4096;
-  h->rs_slots = h->rs_slots_ens = 0;
+  h->real_rows = Nx == 16384;
+  h->rs_slots = h->rs_slots_ens = h->rs_slots_tan = 0;
   h->device = -1;
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
@@ -454,8 +467,18 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
     h->device = dev;
   }
   std::vector<unsigned char> tx, ty, ts;
-  if (t == TTSH_F64) { fill_stage_tables<double>(tx, Nx); fill_stage_tables<double>(ty, Ny / 2); fill_split_table<double>(ts, Ny); }
-  else { fill_stage_tables<float>(tx, Nx); fill_stage_tables<float>(ty, Ny / 2); fill_split_table<float>(ts, Ny); }
+  const int Nrow = h->real_rows ? Nx / 2 : Nx;       // length of the complex row transform
+  if (t == TTSH_F64) { fill_stage_tables<double>(tx, Nrow); fill_stage_tables<double>(ty, Ny / 2); fill_split_table<double>(ts, Ny); }
+  else { fill_stage_tables<float>(tx, Nrow); fill_stage_tables<float>(ty, Ny / 2); fill_split_table<float>(ts, Ny); }
+  if (h->real_rows) {      // W_Nx^j, j < Nx/32: the split / merge twiddles of the real-row passes
+    std::vector<unsigned char> tr((size_t)(Nx / 32) * 2 * (size_t)t);
+    for (int j = 0; j < Nx / 32; ++j) {
+      if (t == TTSH_F64) put_twiddle<double>(reinterpret_cast<double*>(tr.data()) + 2 * (size_t)j, j, Nx);
+      else put_twiddle<float>(reinterpret_cast<float*>(tr.data()) + 2 * (size_t)j, j, Nx);
+    }
+    TRY(h, cudaMemcpyAsync(h->tabXw, tr.data(), tr.size(), cudaMemcpyHostToDevice, h->stream));
+    TRY(h, cudaStreamSynchronize(h->stream));
+  }
   if (h->row_step_wl) {
     std::vector<unsigned char> tw;
     if (t == TTSH_F64) fill_stage_tables_wl<double>(tw, Nx); else fill_stage_tables_wl<float>(tw, Nx);
@@ -469,7 +492,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   TRY(h, cudaStreamSynchronize(h->stream));   // the host tables go out of scope below
   TRY(h, DISPATCH(h, prepare_rows, h->g));
   TRY(h, DISPATCH(h, prepare_cols, h->g));
-  if (h->row_step_ok) TRY(h, DISPATCH(h, prepare_row_step, h->g, &h->rs_slots, &h->rs_slots_ens));
+  if (h->row_step_ok) TRY(h, DISPATCH(h, prepare_row_step, h->g, &h->rs_slots, &h->rs_slots_ens, &h->rs_slots_tan));
   return apply_mask(h, mask, kind);
 }
 
@@ -500,9 +523,10 @@ int ttsh_set_advection_form(ttsh_handle* h, int form) {
   if (!h || (form != TTSH_ADVECTION_CONSERVATIVE && form != TTSH_ADVECTION_LITERAL)) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
   CHECK_DEVICE(h);
-  if (form != h->advection_form && h->graph_exec) {   // the captured step no longer matches
-    cudaGraphExecDestroy(h->graph_exec);
-    h->graph_exec = nullptr;
+  if (form != h->advection_form) {   // the captured steps no longer match
+    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+    if (h->graph_exec_k) cudaGraphExecDestroy(h->graph_exec_k);
+    h->graph_exec = h->graph_exec_k = nullptr;
     h->graph_ok = false;
   }
   h->advection_form = form;
@@ -515,12 +539,14 @@ int ttsh_step(ttsh_handle* h, int n) {
   CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
   if (n == 0) return TTSH_OK;
-  // Small grids are launch-latency bound: replay one captured step.  Large grids launch directly.
-#ifndef TTSH_GRAPH_MAX_POINTS
-#define TTSH_GRAPH_MAX_POINTS (1024 * 1024)
-#endif
-  const bool use_graph = (size_t)h->Nx * h->Ny <= (size_t)TTSH_GRAPH_MAX_POINTS && n >= 4;
-  if (use_graph && !h->graph_ok) {
+  // Small grids are launch-latency bound: replay captured steps.  Up to 1024^2 one step per graph launch; up to 256^2, where the
+  // four kernels of a step take about as long as a graph launch costs on the host, GRAPH_K steps per launch.  Large grids launch
+  // directly.  Replays are bit-identical to direct launches (same kernels, same order).
+  constexpr int GRAPH_K = 16;
+  const size_t P = (size_t)h->Nx * h->Ny;
+  const bool use_graph = P <= (size_t)1024 * 1024 && n >= 4;
+  const bool use_k = P <= (size_t)256 * 256 && n >= GRAPH_K;
+  auto capture = [&](int steps, cudaGraphExec_t* out) -> int {
     // capture on a private stream (the caller's may be the legacy default stream, which cannot capture);
     // the instantiated graph is then replayed on the caller's stream.
     cudaGraph_t graph = nullptr;
@@ -531,19 +557,35 @@ int ttsh_step(ttsh_handle* h, int n) {
     cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
     if (e != cudaSuccess) { cudaStreamDestroy(cap); return fail_cuda(h, e, "cudaStreamBeginCapture"); }
     h->stream = cap;
-    int rc = enqueue_step(h);
+    int rc = TTSH_OK;
+    for (int i = 0; i < steps && rc == TTSH_OK; ++i) rc = enqueue_step(h);
     h->stream = user;
     e = cudaStreamEndCapture(cap, &graph);
     cudaStreamDestroy(cap);
     h->launches = before;
     if (rc != TTSH_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail_cuda(h, e, "cudaStreamEndCapture");
-    e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    e = cudaGraphInstantiate(out, graph, 0);
     cudaGraphDestroy(graph);
-    if (e != cudaSuccess) return fail_cuda(h, e, "cudaGraphInstantiate");
+    if (e != cudaSuccess) { *out = nullptr; return fail_cuda(h, e, "cudaGraphInstantiate"); }
+    return TTSH_OK;
+  };
+  if (use_graph && !h->graph_ok) {
+    int rc = capture(1, &h->graph_exec);
+    if (rc != TTSH_OK) return rc;
     h->graph_ok = true;
   }
-  for (int i = 0; i < n; ++i) {
+  if (use_k && !h->graph_exec_k) {
+    int rc = capture(GRAPH_K, &h->graph_exec_k);
+    if (rc != TTSH_OK) return rc;
+  }
+  int left = n;
+  while (use_k && left >= GRAPH_K) {
+    TRY(h, cudaGraphLaunch(h->graph_exec_k, h->stream));
+    h->launches += (long long)GRAPH_K * launches_per_step(h);
+    left -= GRAPH_K;
+  }
+  for (; left > 0; --left) {
     if (use_graph) {
       TRY(h, cudaGraphLaunch(h->graph_exec, h->stream));
       h->launches += launches_per_step(h);
@@ -739,7 +781,7 @@ int ttsh_psd_destroy(ttsh_psd* s) {
 // Every vector owns one block of the workspace — dw^, dpsi^, dv^(0), three real fields, three intermediates, three spectra —
 // and the blocks lie at a uniform stride, so one launch of each kernel serves ALL vectors (the member dimension of the
 // kernels, as in ttsh_ensemble_step): a tangent step costs 7 launches whatever nvec is.
-struct TanLayout { size_t what, psihat, v0, real[3], inter[3], spec[3], vec_stride, vec, partial, coef, rdiag, total; };
+struct TanLayout { size_t what, psihat, v0, real[3], inter[3], spec[3], vec_stride, vec, partial, coef, rdiag, gram, total; };
 static TanLayout tan_layout(int Nx, int Ny, size_t w, int nvec) {
   const Geom g = make_geom(Nx, Ny, 1.0, 2, 3, w);
   const size_t cw = 2 * w, P = (size_t)Nx * Ny;
@@ -754,9 +796,10 @@ static TanLayout tan_layout(int Nx, int Ny, size_t w, int nvec) {
   L.vec_stride = off;
   off = 0;
   L.vec = take(L.vec_stride * nvec);
-  L.partial = take((size_t)DIAG_BLOCKS * nvec * sizeof(double));
+  L.partial = take((size_t)DIAG_BLOCKS * nvec * nvec * sizeof(double));
   L.coef = take((size_t)(nvec + 8) * sizeof(double));
   L.rdiag = take((size_t)nvec * sizeof(double));
+  L.gram = take((size_t)2 * nvec * nvec * sizeof(double));     // Gram matrix, R^-1
   L.total = off;
   return L;
 }
@@ -787,6 +830,7 @@ int ttsh_tangent_create(ttsh_tangent** out, ttsh_handle* h, int nvec, void* work
   s->partial = reinterpret_cast<double*>(ws + L.partial);
   s->coef = reinterpret_cast<double*>(ws + L.coef);
   s->rdiag = reinterpret_cast<double*>(ws + L.rdiag);
+  s->gram = reinterpret_cast<double*>(ws + L.gram);
   *out = s;
   TRY(h, cudaMemsetAsync(ws + L.vec, 0, L.vec_stride * nvec, h->stream));
   return TTSH_OK;
@@ -824,7 +868,7 @@ static int tangent_inverse(ttsh_tangent* s, int first, int count, void* dw, void
   if (nc == 0) return TTSH_OK;
   TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, nc, h->tabY, h->tabS, v0, h->stream, count, s->stride));
   if (count == 1 || dst_stride == s->stride) {
-    TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, v0, h->stream, count, s->stride));
+    TRY(h, DISPATCH(h, launch_inv_row, h->g, rb, nr, h->tabX, h->tabXw, v0, h->stream, count, s->stride));
   } else return TTSH_ERR_INVALID_ARG;
   h->launches += 2;
   return TTSH_OK;
@@ -844,30 +888,41 @@ int ttsh_tangent_step(ttsh_tangent* s, int n) {
     int rc = enqueue_stage(h, TTSH_STAGE_INV_COL);
     if (rc == TTSH_OK) rc = enqueue_stage(h, TTSH_STAGE_INV_ROW);
     if (rc != TTSH_OK) return rc;
+    if (h->row_step_ok && h->rs_slots_tan > 0) {
+      // all vectors at once, fused (row_step.cuh, TAN): inverse column pass of (dw^, dpsi^, i k_y dpsi^), then ONE kernel for the
+      // inverse row transforms, the linearised lines 1-2 at the base state (R[0], R[3], R[4], K) and the forward row transforms
+      // into dA~ = i k_x dGy~ + dS'~ and dB~ = dGx~ (parked in the vectors' real scratch), column pass, lines 3-16 (linear).
+      Batch cb = make_batch({op(s->what, s->inter[0], SM_ONE), op(s->psihat, s->inter[1], SM_ONE), op(s->psihat, s->inter[2], SM_IKY_MEANX)});
+      TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, s->v0, h->stream, M, ms));
+      TRY(h, DISPATCH(h, launch_row_step_tan, h->g, h->m, s->inter[0], s->inter[2], s->inter[1], h->K, s->real[0], s->real[1], h->tabX, s->v0,
+                      h->stream, M, ms, h->rs_slots_tan, h->R[0], h->R[3], h->R[4]));
+      Batch fb = make_batch({op(s->real[0], s->spec[0], 0), op(s->real[1], s->spec[1], 0)});
+      TRY(h, DISPATCH(h, launch_fwd_col, h->g, fb, 2, h->tabY, h->tabS, h->stream, M, ms));
+      TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, s->spec[0], s->spec[1], s->what, s->psihat, s->v0, h->stream, M, ms));
+      h->launches += 4;
+    } else {
     // all vectors at once: dw, dv_x, dv_y -> linearised lines 1-2 in place -> three forward transforms -> lines 3-16
     rc = tangent_inverse(s, 0, M, s->real[0], s->real[1], s->real[2], true, ms);
     if (rc != TTSH_OK) return rc;
     TRY(h, DISPATCH(h, launch_realspace_tangent, h->g, h->m, h->R[3], h->R[4], h->R[0], h->K, s->real[1], s->real[2], s->real[0], h->stream, M, ms));
     Batch rb = make_batch({op(s->real[1], s->inter[0], RM_PERM), op(s->real[2], s->inter[1], RM_PERM), op(s->real[0], s->inter[2], RM_PERM)});
-    TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->stream, M, ms));
+    TRY(h, DISPATCH(h, launch_fwd_row, h->g, rb, 3, h->tabX, h->tabXw, h->stream, M, ms));
     Batch cb = make_batch({op(s->inter[0], s->spec[0], 0), op(s->inter[1], s->spec[1], 0), op(s->inter[2], s->spec[2], 0)});
     TRY(h, DISPATCH(h, launch_fwd_col, h->g, cb, 3, h->tabY, h->tabS, h->stream, M, ms));
     // lines 3-16 are linear: the same spectral kernel on the perturbations' (dw^, dpsi^, dv^(0))
     TRY(h, DISPATCH(h, launch_spectral, h->g, h->m, s->spec[0], s->spec[1], s->spec[2], s->what, s->psihat, s->v0, h->stream, M, ms));
     h->launches += 4;
+    }
     rc = ttsh_step(h, 1);
     if (rc != TTSH_OK) return rc;
   }
   return TTSH_OK;
 }
-int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host) {
-  if (!s || !log_r_host) return TTSH_ERR_INVALID_ARG;
+// modified Gram-Schmidt on the device (the fallback of the blocked QR below): all coefficients stay on the device; row i of R in
+// one batched launch per operation: r_ii = |q_i|, q_i /= r_ii, then r_ij = <q_i, q_j> and q_j -= r_ij q_i for all j > i together.
+// Adds log r_ii to log_r_host.
+static int tangent_mgs(ttsh_tangent* s, double* log_r_host) {
   ttsh_handle* h = s->h;
-  if (h->sticky) return h->sticky;
-  CHECK_DEVICE(h);
-  for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
-  // modified Gram-Schmidt, all coefficients stay on the device; row i of R in one batched launch per operation:
-  // r_ii = |q_i|, q_i /= r_ii, then r_ij = <q_i, q_j> and q_j -= r_ij q_i for all j > i together
   for (int i = 0; i < s->nvec; ++i) {
     void* qi = vec_ptr(s, s->what, i);
     double* qi0 = vec_ptr(s, s->v0, i);
@@ -887,9 +942,40 @@ int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host) {
     TRY(h, DISPATCH(h, launch_psi_from_w, h->g, vec_ptr(s, s->what, i), vec_ptr(s, s->psihat, i), h->stream));
     h->launches++;
   }
-  TRY(h, cudaMemcpyAsync(log_r_host, s->rdiag, (size_t)s->nvec * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  std::vector<double> r(s->nvec);
+  TRY(h, cudaMemcpyAsync(r.data(), s->rdiag, (size_t)s->nvec * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   TRY(h, cudaStreamSynchronize(h->stream));
-  for (int i = 0; i < s->nvec; ++i) log_r_host[i] = log(log_r_host[i]);
+  for (int i = 0; i < s->nvec; ++i) log_r_host[i] += log(r[i]);
+  return TTSH_OK;
+}
+
+// QR of the current vectors, R_ii > 0.  Blocked: CholeskyQR2 — G = A^T A, R = chol(G) and R^-1 (one small block), A <- A R^-1,
+// all on the device, twice (the second pass restores orthogonality to round-off; R = R2 R1, so log R_ii = log R1_ii + log R2_ii).  A
+// Cholesky pivot below 1e-13 of its diagonal entry (vectors that are numerically dependent at the level where the Gram matrix
+// loses them, cond(A) > ~3e6) sends the remaining work to modified Gram-Schmidt instead.
+int ttsh_tangent_orthonormalize(ttsh_tangent* s, double* log_r_host) {
+  if (!s || !log_r_host) return TTSH_ERR_INVALID_ARG;
+  ttsh_handle* h = s->h;
+  if (h->sticky) return h->sticky;
+  CHECK_DEVICE(h);
+  for (int i = 0; i < s->nvec; ++i) if (!s->set[i]) return TTSH_ERR_NOT_INITIALIZED;
+  const int M = s->nvec;
+  // device scratch: gram = G[M][M] | S[M][M]; rdiag = log R_ii accumulated over the two passes; coef[M + 1 ..] holds the flag
+  double* Sdev = s->gram + (size_t)M * M;
+  int* flag = reinterpret_cast<int*>(s->coef + M + 2);
+  TRY(h, cudaMemsetAsync(s->rdiag, 0, (size_t)M * sizeof(double), h->stream));
+  TRY(h, cudaMemsetAsync(flag, 0, sizeof(int), h->stream));
+  for (int pass = 0; pass < 2; ++pass) {
+    TRY(h, DISPATCH(h, launch_gram, h->g, s->what, s->v0, s->stride, M, s->partial, s->gram, h->stream));
+    TRY(h, launch_chol_inv(M, s->gram, Sdev, s->rdiag, flag, h->stream));
+    TRY(h, DISPATCH(h, launch_tri_apply, h->g, M, Sdev, s->what, s->psihat, s->v0, s->stride, h->stream));
+    h->launches += 4;
+  }
+  int bad = 0;
+  TRY(h, cudaMemcpyAsync(log_r_host, s->rdiag, (size_t)M * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  TRY(h, cudaMemcpyAsync(&bad, flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  TRY(h, cudaStreamSynchronize(h->stream));
+  if (bad) return tangent_mgs(s, log_r_host);      // adds its log r_ii to what a completed first pass recorded
   return TTSH_OK;
 }
 int ttsh_tangent_get_fields(ttsh_tangent* s, int i, void* dvx, void* dvy, void* domega) {
@@ -1014,15 +1100,14 @@ int ttsh_debug_get_real(ttsh_handle* h, int which, void* dst) {
   if (!h || !dst || which < 0 || which > 5) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
   CHECK_DEVICE(h);
-  const void* src = which == 5 ? h->K : h->R[which];   // internal fields are in the permuted row layout
-  TRY(h, DISPATCH(h, launch_permute, h->Nx, (size_t)h->Nx * h->Ny, src, dst, 0, h->stream));
-  h->launches++;
-  return TTSH_OK;
+  const void* src = which == 5 ? h->K : h->R[which];   // internal fields are in the internal row layout
+  return copy_real(h, src, dst, 0);
 }
 
 int ttsh_destroy(ttsh_handle* h) {
   if (!h) return TTSH_OK;
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  if (h->graph_exec_k) cudaGraphExecDestroy(h->graph_exec_k);
   delete h;
   return TTSH_OK;
 }
@@ -1031,7 +1116,7 @@ const char* ttsh_strerror(int code) {
   switch (code) {
     case TTSH_OK: return "ok";
     case TTSH_ERR_INVALID_ARG: return "invalid argument";
-    case TTSH_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (Nx, Ny must be powers of two in [64, 8192])";
+    case TTSH_ERR_UNSUPPORTED_SIZE: return "unsupported grid size (Nx, Ny must be powers of two in [64, 16384])";
     case TTSH_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
     case TTSH_ERR_NOT_INITIALIZED: return "state not initialised (call ttsh_set_velocity first)";
     case TTSH_ERR_CUDA: return "CUDA error";

@@ -83,6 +83,7 @@ struct Geom {
   int Wxp;                 // NT * CW: padded number of columns
   int My, Hy;
   int num, den;            // dealias fraction
+  int cut_gx, cut_gy, cut_c;   // Nx / g, Ny / g, Nx Ny / g with g = min(Nx, Ny): the cutoff predicate with its common factor divided out
   double dkx, dky;         // 2 pi / (Nx dx), 2 pi / (Ny dx)   (Table I)
   double inv_sqrt_nx, inv_sqrt_ny;
 };
@@ -112,11 +113,11 @@ __host__ __device__ __forceinline__ int perm_index_wl(int x, int tpl) {
 
 // strict '>' cutoff evaluated exactly in integers (reading R4):
 //   k^2 > ((num/den) pi/dx)^2   <=>   4 den^2 ((mx Ny)^2 + (my Nx)^2) > num^2 (Nx Ny)^2
-// Nx, Ny are powers of two, so the three products share the factor g = min(Nx, Ny), which is divided out first: with
-// |mx| <= Nx/2, |my| <= Ny/2, max(Nx, Ny) <= 2^14 and den <= 64 both sides stay below 2^42 (no int64 overflow at any accepted size).
-__host__ __device__ __forceinline__ bool is_cut(int mx, int my, int Nx, int Ny, int num, int den) {
-  const int gx = Nx < Ny ? 1 : Nx / Ny, gy = Ny < Nx ? 1 : Ny / Nx;      // Nx / g and Ny / g
-  const long long a = (long long)mx * gy, b = (long long)my * gx, c = (long long)gx * gy * (Nx < Ny ? Nx : Ny);
+// Nx, Ny are powers of two, so the three products share the factor g = min(Nx, Ny), which is divided out (host, make_geom:
+// cut_gx = Nx / g, cut_gy = Ny / g, cut_c = Nx Ny / g): with |mx| <= Nx/2, |my| <= Ny/2, max(Nx, Ny) <= 2^14 and den <= 64 both
+// sides stay below 2^42, so nothing overflows int64 at any accepted size.
+__host__ __device__ __forceinline__ bool is_cut(const Geom& g, int mx, int my, int num, int den) {
+  const long long a = (long long)mx * g.cut_gy, b = (long long)my * g.cut_gx, c = g.cut_c;
   return 4LL * den * den * (a * a + b * b) > (long long)num * num * c * c;
 }
 

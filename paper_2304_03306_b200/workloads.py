@@ -89,6 +89,7 @@ class Config:
     dtypes: Tuple[str, ...] = ("f64",)
     index: int = 0
     sweep: Tuple[float, ...] = field(default_factory=tuple)
+    preset: str = "baseline"         # "baseline" (BASELINE.json's parameters) | "paper" (Table I)
 
     @property
     def seed(self) -> int:
@@ -116,4 +117,7 @@ CONFIGS = {
                  sweep=(80.0, 100.0, 110.0, 118.0)),
     "C5": Config("C5", 4096, 4096, geometry="disk", R=900.0, steps=2000, dtypes=("f64", "f32"), index=4),
     "C5p": Config("C5p", 4096, 4096, geometry="none", steps=2000, dtypes=("f64", "f32"), index=4),
+    # the paper's own production run (Table I :264-278): 8192 x 8192, dx = 0.005 (L = 40.96), dt = 0.01, the paper's
+    # parameters, a disk of radius R = 5.2 (just above the onset of the single vortex): about 95 % of the box is masked
+    "C6": Config("C6", 8192, 8192, dx=0.005, dt=0.01, geometry="disk", R=5.2, steps=2000, dtypes=("f64", "f32"), index=5, preset="paper"),
 }

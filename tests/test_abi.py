@@ -35,7 +35,9 @@ def test_struct_layouts_match_the_header(ttsh):
 def test_workspace_bytes_and_size_validation(ttsh):
     assert ttsh.ttsh_workspace_bytes(100, 64, ttsh.TTSH_F64) == 0         # not a power of two
     assert ttsh.ttsh_workspace_bytes(32, 64, ttsh.TTSH_F64) == 0          # below 64
-    assert ttsh.ttsh_workspace_bytes(64, 16384, ttsh.TTSH_F64) == 0       # above 8192
+    assert ttsh.ttsh_workspace_bytes(64, 32768, ttsh.TTSH_F64) == 0       # above 16384
+    assert ttsh.ttsh_workspace_bytes(16384, 64, ttsh.TTSH_F64) > 0 and ttsh.ttsh_workspace_bytes(64, 16384, ttsh.TTSH_F32) > 0
+    assert 12 * 2**31 < ttsh.ttsh_workspace_bytes(16384, 16384, ttsh.TTSH_F64) < 15 * 2**31   # Fig. 6(f) grid: about 27 GB of 180 GB
     assert ttsh.ttsh_workspace_bytes(64, 64, 3) == 0                      # bad dtype
     b64 = ttsh.ttsh_workspace_bytes(4096, 4096, ttsh.TTSH_F64)
     b32 = ttsh.ttsh_workspace_bytes(4096, 4096, ttsh.TTSH_F32)

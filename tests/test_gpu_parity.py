@@ -337,6 +337,31 @@ def test_checkpoint_roundtrip_is_bit_exact_and_set_mask_keeps_state(ttsh):
     s.close()
 
 
+@pytest.mark.parametrize("N", [64, 256, 512])
+def test_graph_replay_is_bit_identical_to_direct_launches(ttsh, N):
+    """ttsh_step(n) replays captured steps on small grids (16 steps per graph up to 256^2, one per graph up to 1024^2); the
+    result must be bit-identical to n direct launches (ttsh_step(1) never uses a graph)."""
+    import torch
+    mask = workloads.disk_mask(N, N, 0.5, 0.3 * N * 0.5)
+    vel = workloads.planewave_velocity(N, N, 0.5, 21, amplitude=1.0)
+    a = ttsh.Solver(N, N, 0.5, 0.01, ttsh.baseline_params(), "f64", mask=mask)
+    b = ttsh.Solver(N, N, 0.5, 0.01, ttsh.baseline_params(), "f64", mask=mask)
+    a.set_velocity(*vel); b.set_velocity(*vel)
+    a.step(53)                       # 3 x 16-step graphs + 5 single-step graphs (N <= 256), 53 single-step graphs (N = 512)
+    for _ in range(53):
+        b.step(1)
+    assert a.launch_count() == b.launch_count()
+    for u, v in zip(a.get_fields(), b.get_fields()):
+        assert torch.equal(u, v)
+    a.set_mask(workloads.disk_mask(N, N, 0.5, 0.35 * N * 0.5)); b.set_mask(workloads.disk_mask(N, N, 0.5, 0.35 * N * 0.5))
+    a.step(20)
+    for _ in range(20):
+        b.step(1)
+    for u, v in zip(a.get_fields(), b.get_fields()):
+        assert torch.equal(u, v)                 # the captured graphs see the new K (same buffer)
+    a.close(); b.close()
+
+
 def test_non_default_stream_and_close_order(ttsh):
     """The wrapper orders its allocations and copies on the Solver's own stream (not torch's current one), and closing a Solver
     first tears down the objects that borrow its handle (TemporalPSD, Tangent)."""
@@ -568,6 +593,79 @@ def test_maximum_grid_dimension_8192(ttsh, Nx, Ny, dtype):
     s.step(3); o.step(3)
     compare_state(s, o, TOL_F64_100 if dtype == "f64" else 3 * TOL_F32_1, f"{Nx}x{Ny} {dtype}")
     assert s.diagnostics()["nonfinite"] == 0
+    s.close()
+
+
+@pytest.mark.parametrize("Nx,Ny,dtype", [(16384, 64, "f64"), (16384, 64, "f32"), (64, 16384, "f64"), (64, 16384, "f32"), (16384, 128, "f64")])
+def test_maximum_grid_dimension_16384(ttsh, Nx, Ny, dtype):
+    """(N, dx) = (16384, 0.0025) is the grid of Fig. 6(f).  Nx = 16384: one real row per half-length transform
+    (fft_rows_real.cuh), 6-launch step; Ny = 16384: 8192-point half-length column transforms, one column per CTA.  Algorithm 2,
+    the initial projection, 3 steps in both advection forms and the diagnostics against the C oracle-fft."""
+    dx, dt = 0.5, 0.01
+    mask = workloads.disk_mask(Nx, Ny, dx, 12.0)
+    vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 6, amplitude=1.0)
+    vel = (vel[0] + 0.1, vel[1] - 0.2)
+    s, o = make_pair(ttsh, Nx, Ny, dx, dt, "baseline", mask, dtype=dtype, transform="c", vel=vel)
+    f64 = dtype == "f64"
+    K = s.debug_real(5).cpu().numpy().astype(np.float64)
+    assert rel(K, o.K) <= (1e-12 if f64 else TOL_F32_1)
+    compare_state(s, o, TOL_F64_1 if f64 else TOL_F32_1, f"{Nx}x{Ny} {dtype} init")
+    s.step(3); o.step(3)
+    compare_state(s, o, TOL_F64_100 if f64 else 3 * TOL_F32_1, f"{Nx}x{Ny} {dtype} 3 steps")
+    if f64:
+        s.set_advection_form(ttsh.TTSH_ADVECTION_LITERAL)
+        s.step(2); o.step(2)
+        compare_state(s, o, TOL_F64_100, f"{Nx}x{Ny} literal form")
+        cx, cy = (Nx // 2) * dx, (Ny // 2) * dx
+        d, od = s.diagnostics(cx, cy), o.diagnostics(cx, cy)
+        for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy"):
+            assert abs(d[key] - od[key]) <= TOL_DIAG * abs(od[key]), key
+    assert s.diagnostics()["nonfinite"] == 0
+    s.close()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_C6_paper_production_grid_8192(ttsh, dtype):
+    """The paper's own run (Table I): 8192 x 8192, dx = 0.005, dt = 0.01, the paper's parameters, disk R = 5.2.
+    1 step and (fp64) 10 steps against the C oracle-fft (about 5 s of host time per step), O(1) start plus the config's noise."""
+    cfg = workloads.CONFIGS["C6"]
+    mask = cfg.mask()
+    vel = workloads.planewave_velocity(cfg.Nx, cfg.Ny, cfg.dx, cfg.seed, amplitude=0.3, nmodes=12, kmax=1.5)
+    g = workloads.gaussian_velocity(cfg.Nx, cfg.Ny, cfg.seed, 1e-2, mask)
+    vel = (vel[0] + g[0], vel[1] + g[1])
+    del g
+    s, o = make_pair(ttsh, cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, "paper", mask, dtype=dtype, transform="c", vel=vel)
+    del vel
+    s.step(1); o.step(1)
+    compare_state(s, o, TOL_F64_1 if dtype == "f64" else TOL_F32_1, f"C6 {dtype} step 1")
+    if dtype == "f64":
+        s.step(9); o.step(9)
+        compare_state(s, o, TOL_F64_100, "C6 f64 step 10")
+        cx, cy = (cfg.Nx // 2) * cfg.dx, (cfg.Ny // 2) * cfg.dx
+        d, od = s.diagnostics(cx, cy), o.diagnostics(cx, cy)
+        for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy"):
+            assert abs(d[key] - od[key]) <= TOL_DIAG * abs(od[key]), key
+    s.close()
+
+
+@pytest.mark.slow
+def test_full_16384_square_grid_runs_in_fp32(ttsh):
+    """The full 16384 x 16384 grid of Fig. 6(f) in fp32 (13.5 GB of workspace): the state stays finite, the
+    small random start grows at the linear rate, w has zero mean.  (No oracle can follow this size; parity is on the strips.)"""
+    N, dx, dt = 16384, 0.5, 0.01
+    mask = workloads.disk_mask(N, N, dx, 0.22 * N * dx)
+    s = ttsh.Solver(N, N, dx, dt, ttsh.baseline_params(), "f32", mask=mask)
+    vel = workloads.gaussian_velocity(N, N, workloads.SEED0 + 8, 1e-2, mask)
+    s.set_velocity(*vel)
+    del vel
+    d0 = s.diagnostics()
+    s.step(20)
+    d = s.diagnostics()
+    assert d["nonfinite"] == 0 and d["step"] == 20 and np.isfinite(d["kinetic_energy"]) and 0 < d["kinetic_energy"] < d0["kinetic_energy"]
+    assert d["max_speed"] < 1.0        # band-limiting removes most of the white-noise energy; nothing blows up
+    w = s.get_fields(psi=False)[2]
+    assert abs(float(w.double().mean())) <= 1e-4 * float(w.abs().max())
     s.close()
 
 

@@ -109,6 +109,38 @@ def test_qr_growth_rates_match_oracle(ttsh):
     tg.close(); s.close()
 
 
+@pytest.mark.parametrize("eps,tol", [(1e-4, 1e-9), (1e-8, 1e-6)])
+def test_qr_of_nearly_parallel_vectors(ttsh, eps, tol):
+    """An ill-conditioned set: vector 1 = vector 0 + eps * (something else).  eps = 1e-4 (cond ~ 1e4) goes through the blocked
+    CholeskyQR2; eps = 1e-8 trips its pivot test and falls back to modified Gram-Schmidt on the device.  log R_ii against
+    numpy's Householder QR (the oracle), where Gram-Schmidt and Householder differ most."""
+    Nx = Ny = 64
+    dx, dt = 0.5, 0.01
+    s = ttsh.Solver(Nx, Ny, dx, dt, ttsh.baseline_params(), "f64")
+    o = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET)
+    z = np.zeros((Ny, Nx))
+    s.set_velocity(z, z); o.set_velocity(z, z)
+    tg, to = ttsh.Tangent(s, 3), TangentOracle(o, 3)
+    a = workloads.planewave_velocity(Nx, Ny, dx, 3, amplitude=1.0, nmodes=6)
+    b = workloads.planewave_velocity(Nx, Ny, dx, 4, amplitude=1.0, nmodes=6)
+    c = workloads.planewave_velocity(Nx, Ny, dx, 5, amplitude=0.5, nmodes=6)
+    vecs = [a, (a[0] + eps * b[0], a[1] + eps * b[1]), (c[0] + 0.3, c[1])]
+    for i, v in enumerate(vecs):
+        tg.set(i, *v); to.set(i, *v)
+    lg, lo = np.asarray(tg.orthonormalize()), to.orthonormalize()
+    assert np.allclose(lg, lo, rtol=0, atol=tol), lg - lo
+    assert lo[1] - lo[0] < np.log(eps) + 2.0               # R_11 / R_00 really is of order eps
+    # the device's vectors are orthonormal afterwards
+    P = Nx * Ny
+    cols = []
+    for i in range(3):
+        dvx, dvy, dw = [t.cpu().numpy() for t in tg.get_fields(i)]
+        cols.append(np.concatenate([dw.ravel(), [dvx.sum() / np.sqrt(P), dvy.sum() / np.sqrt(P)]]))
+    A = np.stack(cols, axis=1)
+    assert np.allclose(A.T @ A, np.eye(3), atol=1e-6 if eps < 1e-6 else 1e-10)   # one pass of Gram-Schmidt loses eps_mach * cond
+    tg.close(); s.close()
+
+
 def test_growth_about_the_zero_state_is_sigma_of_k(ttsh):
     """Base state 0, no mask: the tangent map is exp(sigma(k) dt) per mode (Alg. 1 line 4): closed form on the GPU too."""
     Nx = Ny = 64

@@ -226,6 +226,10 @@ int ttsh_debug_get_real(ttsh_handle* h, int which, void* dst);
 
 int ttsh_destroy(ttsh_handle* h);
 
+/* "ttsh sm_100a sources=<first 16 hex digits of the SHA-256 of csrc/*.cu, *.cuh, *.h, include/ttsh.h, Makefile, concatenated in
+ * sorted order> cuda=<nvcc version> built <date>": which sources this binary was compiled from (tests compare it with the tree). */
+const char* ttsh_build_info(void);
+
 const char* ttsh_strerror(int code);
 const char* ttsh_last_error(const ttsh_handle* h);   /* "" if none */
 

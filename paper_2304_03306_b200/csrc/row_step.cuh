@@ -51,10 +51,7 @@ template <typename T, int NX, int LL = 1, bool TAN = false> struct RowStepCfg {
   // copy only adds shared-memory wavefronts (137.0 us from global memory, 145.6 us from the copy)
   static constexpr bool SMEM_TAB = WL && sizeof(T) == 8;
   static constexpr size_t SMEM = OFF_TAB + (SMEM_TAB ? (size_t)fft_wl_tw_elems_rt(NX) * sizeof(cplx<T>) : 0);
-#ifndef TTSH_RS_MINB_F32
-#define TTSH_RS_MINB_F32 1
-#endif
-  static constexpr int MINB = (sizeof(T) == 4 && NX == 4096) ? TTSH_RS_MINB_F32 : 1;
+  static constexpr int MINB = 1;          // one CTA per SM also in fp32 at Nx = 4096 (two CTAs of 128 registers: 140 vs 136 us)
   static constexpr bool FITS = SMEM <= 227 * 1024;
 };
 

@@ -13,6 +13,8 @@
 #include "fft_passes.cuh"
 
 using namespace ttsh;
+#define TTSH_STR2(x) #x
+#define TTSH_STR(x) TTSH_STR2(x)
 
 namespace {
 
@@ -1125,5 +1127,12 @@ const char* ttsh_strerror(int code) {
 }
 
 const char* ttsh_last_error(const ttsh_handle* h) { return h ? h->err.c_str() : ""; }
+
+#ifndef TTSH_SOURCE_HASH
+#define TTSH_SOURCE_HASH "unknown"
+#endif
+const char* ttsh_build_info(void) {
+  return "ttsh sm_100a sources=" TTSH_SOURCE_HASH " cuda=" TTSH_STR(__CUDACC_VER_MAJOR__) "." TTSH_STR(__CUDACC_VER_MINOR__) " built " __DATE__ " " __TIME__;
+}
 
 }  // extern "C"

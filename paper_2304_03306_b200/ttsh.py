@@ -34,7 +34,7 @@ SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_vel
            "ttsh_psd_accumulate", "ttsh_psd_result", "ttsh_psd_reset", "ttsh_psd_destroy", "ttsh_tangent_workspace_bytes",
            "ttsh_tangent_create", "ttsh_tangent_set", "ttsh_tangent_step", "ttsh_tangent_orthonormalize",
            "ttsh_tangent_get_fields", "ttsh_tangent_destroy", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
-           "ttsh_ensemble_destroy")
+           "ttsh_ensemble_destroy", "ttsh_build_info")
 
 
 class ttsh_params(C.Structure):
@@ -95,6 +95,7 @@ _sig = {
     "ttsh_ensemble_step": (_i, [_vp, _i]),
     "ttsh_ensemble_launch_count": (_ll, [_vp]),
     "ttsh_ensemble_destroy": (_i, [_vp]),
+    "ttsh_build_info": (C.c_char_p, []),
 }
 for _name, (_res, _args) in _sig.items():
     _f = getattr(_lib, _name)
@@ -274,6 +275,10 @@ def ttsh_ensemble_launch_count(e):
 
 def ttsh_ensemble_destroy(e):
     return _lib.ttsh_ensemble_destroy(e)
+
+
+def ttsh_build_info():
+    return _lib.ttsh_build_info().decode()
 
 
 def ttsh_strerror(code):

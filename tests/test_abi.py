@@ -27,6 +27,22 @@ def test_library_exports_every_declared_symbol(ttsh):
         assert hasattr(lib, name), name
 
 
+def test_library_was_built_from_the_sources_in_the_tree(ttsh):
+    """ttsh_build_info carries the SHA-256 of the CUDA sources the binary was compiled from (csrc/Makefile): a stale libttsh.so
+    that travelled with the snapshot instead of being rebuilt would show here."""
+    import glob
+    import hashlib
+    csrc = os.path.join(ROOT, "paper_2304_03306_b200", "csrc")
+    files = sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh")) + glob.glob(os.path.join(csrc, "*.h"))
+                   + [os.path.join(csrc, "..", "..", "include", "ttsh.h"), os.path.join(csrc, "Makefile")],
+                   key=lambda p: os.path.relpath(p, csrc))
+    h = hashlib.sha256()
+    for f in files:
+        h.update(open(f, "rb").read())
+    info = ttsh.ttsh_build_info()
+    assert "sm_100a" in info and ("sources=" + h.hexdigest()[:16]) in info, info
+
+
 def test_struct_layouts_match_the_header(ttsh):
     assert C.sizeof(ttsh.ttsh_params) == 7 * 8 + 2 * 4
     assert C.sizeof(ttsh.ttsh_diag) == 12 * 8

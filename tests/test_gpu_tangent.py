@@ -26,12 +26,12 @@ def rel(a, b):
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
-def setup(ttsh, Nx, Ny, nvec, dtype="f64", R=None, base_amp=1.0):
+def setup(ttsh, Nx, Ny, nvec, dtype="f64", R=None, base_amp=1.0, transform="matmul"):
     dx, dt = 0.5, 0.01
     mask = workloads.disk_mask(Nx, Ny, dx, R if R is not None else 0.3 * min(Nx, Ny) * dx)
     v0 = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 40, amplitude=base_amp, nmodes=12)
     s = ttsh.Solver(Nx, Ny, dx, dt, ttsh.baseline_params(), dtype, mask=mask)
-    o = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET, mask=mask)
+    o = TTSHOracle(Nx, Ny, dx, dt, BASELINE_PRESET, mask=mask, transform=transform)
     if dtype == "f32":
         v0 = tuple(a.astype(np.float32).astype(np.float64) for a in v0)
     s.set_velocity(*v0); o.set_velocity(*v0)
@@ -78,6 +78,19 @@ def test_tangent_at_the_size_bench_times(ttsh):
     lg, lo = np.asarray(tg.orthonormalize()), to.orthonormalize()
     assert np.allclose(lg, lo, rtol=0, atol=1e-9), lg - lo
     compare_vectors(tg, to, 1e-8, "256^2 after QR")
+    tg.close(); s.close()
+
+
+def test_tangent_at_1024_with_4_vectors(ttsh):
+    """1024 x 1024 with 4 vectors (the other size DESIGN.md quotes): the fused tangent row kernel with one row pair per CTA, 1 and 5
+    steps and one QR against the oracle with its FFT backend (locked to the matrix backend by the CPU pins)."""
+    s, o, tg, to = setup(ttsh, 1024, 1024, 4, R=160.0, transform="fft")
+    tg.step(1); to.step(1)
+    compare_vectors(tg, to, TOL_1, "1024^2 1 step")
+    tg.step(4); to.step(4)
+    compare_vectors(tg, to, TOL_N, "1024^2 5 steps")
+    lg, lo = np.asarray(tg.orthonormalize()), to.orthonormalize()
+    assert np.allclose(lg, lo, rtol=0, atol=1e-9), lg - lo
     tg.close(); s.close()
 
 

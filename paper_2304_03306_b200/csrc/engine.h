@@ -43,6 +43,9 @@ template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model&
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                   const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s, int slots);
 template <typename T> bool row_step_supported(const Geom& g);
+// ... and it is the three-team in-place variant (row_step_t3.cuh: Nx = 4096 in fp64), which wants K in line-position order
+// (launch_reperm_t3) and the table of fill_stage_tables_t3
+template <typename T> bool row_step_is_t3(const Geom& g);
 // per-device set-up of k_row_step (shared-memory opt-in, resident CTAs): call on the handle's device; slots = CTAs of the
 // persistent grid of the single-system / ensemble variant (0: not supported for this grid)
 template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens, int* slots_tan);
@@ -77,6 +80,8 @@ template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, c
 template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* in, void* out, int to_perm, cudaStream_t s);
 // permuted internal row layout (perm_index) -> thread-order layout of the warp-local plan (perm_index_wl)
 template <typename T> cudaError_t launch_reperm_wl(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
+// permuted internal row layout -> row-pair-major line-position order of row_step_t3.cuh: (K(y_A, x(p)), K(y_B, x(p))) at (rp Nx + p) 2
+template <typename T> cudaError_t launch_reperm_t3(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
 constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs
 template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,
                                               const void* w, double* partial, double* out, cudaStream_t s);

@@ -80,7 +80,7 @@ template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, c
 template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* in, void* out, int to_perm, cudaStream_t s);
 // permuted internal row layout (perm_index) -> thread-order layout of the warp-local plan (perm_index_wl)
 template <typename T> cudaError_t launch_reperm_wl(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
-// permuted internal row layout -> row-pair-major line-position order of row_step_t3.cuh: (K(y_A, x(p)), K(y_B, x(p))) at (rp Nx + p) 2
+// permuted internal row layout -> line-position order of row_step_t3.cuh, one plane per row: K(y_r, x(p)) at (rp 2 + r) Nx + p
 template <typename T> cudaError_t launch_reperm_t3(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
 constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs
 template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,

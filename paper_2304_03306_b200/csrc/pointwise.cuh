@@ -307,13 +307,13 @@ __global__ void k_reperm_wl(int Nx, size_t n, const T* __restrict__ in, T* __res
 }
 
 // K for row_step_t3.cuh (Nx = 4096 = 16^3): row pair rp = 2a + par holds rows y_A = 4a + par, y_B = y_A + 2; line position p holds
-// x = digit-reversed p;  out[(rp Nx + p) 2 + r] = K(y_r, x(p))
+// x = digit-reversed p; one plane per row:  out[(rp 2 + r) Nx + p] = K(y_r, x(p))
 template <typename T>
 __global__ void k_reperm_t3(int Nx, size_t n, const T* __restrict__ in, T* __restrict__ out) {
   const int tpl = Nx / 16;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const size_t rp = i / (2 * (size_t)Nx);
-    const int rem = (int)(i - rp * 2 * (size_t)Nx), p = rem >> 1, r = rem & 1;
+    const size_t plane = i / (size_t)Nx, rp = plane >> 1;
+    const int p = (int)(i - plane * (size_t)Nx), r = (int)(plane & 1);
     const size_t y = 4 * (rp >> 1) + (rp & 1) + 2 * r;
     const int x = (p >> 8) + 16 * ((p >> 4) & 15) + 256 * (p & 15);
     out[i] = in[y * Nx + perm_index(x, tpl)];

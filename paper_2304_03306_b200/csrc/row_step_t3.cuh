@@ -4,8 +4,17 @@
 // Why another layout: k_row_step keeps two of the three packed fields of a row pair in registers / a private stash, which takes
 // all 64 K registers for 8 warps, and 8 warps run the fp64 pipe and the shared-memory data pipe one after the other (DESIGN.md §6:
 // 126 us of arithmetic + 125 us of exchanges = 258 us).  The stage micro-benchmark there says 12 warps in independent teams overlap
-// the two pipes.  Here the three fields of a row pair live in THREE shared-memory lines (3 x 68 KB), one team of 4 warps per field,
-// and every transform runs IN PLACE, so a thread holds one radix-16 butterfly (16 values) at a time and does two per stage:
+// the two pipes.  Here a row pair (y_A = 4a+p, y_B = y_A+2) lives in THREE shared-memory lines (3 x 68 KB), one team of 4 warps each,
+// every transform runs IN PLACE, and a thread holds one radix-16 butterfly (16 values) at a time:
+//
+//   line 0 (team 0):  w(y_A) + i w(y_B)            -> S'(y_A) + i S'(y_B)
+//   line 1 (team 1):  v_x(y_A) + i v_y(y_A) = u_A  -> Gx(y_A) + i Gy(y_A) = (cc_A - i lw_A) u_A
+//   line 2 (team 2):  v_x(y_B) + i v_y(y_B) = u_B  -> Gx(y_B) + i Gy(y_B)
+//
+// (cc = -beta |v|^2 - gamma_v K, lw = lambda0 w: lines 1-2 of Algorithm 1 in the conservative form, row_step.cuh.)  Packing the two
+// velocity components of ONE row makes the pointwise stage local to the thread that finishes the inverse transform of u: it needs
+// only the real number w(y, x) from line 0 and K(y, x), so u never makes the round trip through shared memory between the inverse
+// and the forward transform, and there is no separate pointwise phase.
 //
 //   inverse (decimation in frequency), N = 16 x 16 x 16, input bin m = j + 256 r, output x = s + 16 s' + 256 s'' at position
 //   256 s + 16 s' + s'' (digit-reversed; the pointwise stage does not care and K comes in that order, k_reperm_t3):
@@ -16,9 +25,12 @@
 //   256 k0 + 16 k1 + k2 at that position: natural order, so the unpack reads bins m and N - m directly.
 //   A warp owns four 256-point blocks through B, C, C', B': only A and A' are team-wide.
 //
-// Per row pair: 1 team barrier + CTA barrier | pointwise on all positions by all 384 threads | CTA barrier + 1 team barrier |
-// unpack (team 1: B~ from Gx~;  teams 0 and 2 together: A~ = unpack(i k_m Zgy + Zs)).  Inputs are read straight from global memory
-// (L2-prefetched one row pair ahead) by the first inverse stage, which is pruned to the retained bins like row_step.cuh.
+// Stage A reads its inputs (the pruned inverse intermediates, retained bins |m| <= N/4 only) straight from global memory into
+// registers, one row pair AHEAD (issued before the unpack of the previous row pair); butterflies j and 256 - j need the same eight
+// bins (one as Z(m), the other as Z(N - m)), so a thread runs that pair and every bin is loaded once.
+// Synchronisation per row pair: team barriers after A and before A'; team 0 -> teams 1, 2 "w is in line 0" and back "S' is in
+// line 0" (bar.arrive / bar.sync); two CTA barriers around the unpack, which needs all three lines:
+//   B~ = (Gx~(y_A), Gx~(y_B)),   A~ = i k_x Gy~ + S'~   (fft_passes.cuh, k_fwd_row_fused).
 #pragma once
 #include "fft_passes.cuh"
 
@@ -41,6 +53,30 @@ __device__ __forceinline__ int t3_pad(int i) { return i + (i >> 4); }
 // real-space x of line position p (and back: the map is an involution on 3 hex digits)
 __host__ __device__ __forceinline__ int t3_digit_reverse(int p) { return (p >> 8) + 16 * ((p >> 4) & 15) + 256 * (p & 15); }
 __device__ __forceinline__ void named_bar(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+__device__ __forceinline__ void named_bar_arrive(int id, int nthreads) {
+  __threadfence_block();                         // the arriving thread's shared-memory writes are visible to the waiting threads
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ Quad<double> ldg_quad(const double* p) {
+  Quad<double> r;
+  asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.v[0]), "=d"(r.v[1]), "=d"(r.v[2]), "=d"(r.v[3]) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ Quad<float> ldg_quad(const float* p) {
+  Quad<float> r;
+  asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ cplx<double> ld_c(const cplx<double>* p) {
+  cplx<double> r;
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ cplx<float> ld_c(const cplx<float>* p) {
+  cplx<float> r;
+  asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+  return r;
+}
 
 template <int DIR, typename T> __device__ __forceinline__ TwBase<16, T> t3_twA(const cplx<T>* __restrict__ tw, int j) {
   TwBase<16, T> b;
@@ -114,46 +150,16 @@ __device__ __forceinline__ void t3_warp_stages(cplx<T>* __restrict__ line, const
   }
 }
 
-// stage A of the inverse transform of one packed row pair: the staged pairs (A, B) of column mx at row[2 mx] (global memory, inverse
-// intermediate layout), Z(m) = scale (wa + i wb), Z(N - m) = scale (conj wa + i conj wb); retained mx = 0..NX/4 only (1/2 rule).
-template <typename T, int NX, int MODE>
-__device__ __forceinline__ void t3_inverse_A(const cplx<T>* __restrict__ row, int t, cplx<T>* __restrict__ line, const cplx<T>* __restrict__ tw,
-                                             T scale, T dkx, T meany) {
-  auto mult = [&](cplx<T> w, int mx) -> cplx<T> {
-    if (MODE == RM_ONE) return w;
-    const T kx = dkx * (T)mx;
-    return mx == 0 ? mk<T>(meany, (T)0) : kx * mul_ni(w);        // RM_NIKX_MEANY
-  };
-  auto combine = [&](Pair<T> r, int mx, bool neg) -> cplx<T> {
-    cplx<T> wa = mult(r.a, mx), wb = mult(r.b, mx);
-    if (mx == 0) { wa.y = 0; wb.y = 0; }
-    if (neg) { wa = conj(wa); wb = conj(wb); }
-    return scale * mk<T>(wa.x - wb.y, wa.y + wb.x);
-  };
-#pragma unroll 1
-  for (int h = 0; h < 2; ++h) {
-    const int j = t + 128 * h;
-    Pair<T> lo[4], hi[4], mid;
+
+// one radix-16 butterfly of stage A (inverse): v = the 16 bins j + 256 r (zeros outside the retained band already in place)
+template <typename T>
+__device__ __forceinline__ void t3_inverse_A_butterfly(cplx<T> (&v)[16], int j, cplx<T>* __restrict__ line, const cplx<T>* __restrict__ tw) {
+  const TwBase<16, T> tb = t3_twA<+1>(tw, j);
+  dft16<+1>(v);
+  apply_stage_twiddles<16>(v, tb);
+  cplx<T>* col = line + j + (j >> 4);
 #pragma unroll
-    for (int k = 0; k < 4; ++k) lo[k] = ld_pair(row + 2 * (j + 256 * k));
-#pragma unroll
-    for (int k = 0; k < 4; ++k) hi[k] = ld_pair(row + 2 * (NX - (j + 256 * (12 + k))));
-    mid.a = mk<T>(0, 0); mid.b = mk<T>(0, 0);
-    if (j == 0) mid = ld_pair(row + 2 * (NX / 4));
-    const TwBase<16, T> tb = t3_twA<+1>(tw, j);
-    cplx<T> v[16];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = combine(lo[k], j + 256 * k, false);
-    v[4] = j == 0 ? combine(mid, NX / 4, false) : mk<T>(0, 0);
-#pragma unroll
-    for (int k = 5; k < 12; ++k) v[k] = mk<T>(0, 0);
-#pragma unroll
-    for (int k = 0; k < 4; ++k) v[12 + k] = combine(hi[k], NX - (j + 256 * (12 + k)), true);
-    dft16<+1>(v);
-    apply_stage_twiddles<16>(v, tb);
-#pragma unroll
-    for (int s = 0; s < 16; ++s) line[j + (j >> 4) + 272 * s] = v[s];
-  }
+  for (int s = 0; s < 16; ++s) col[272 * s] = v[s];
 }
 
 // stage A' of the forward transform: bins 256 k0 + i in place; only the retained bins (|m| <= NX/4) are stored
@@ -178,8 +184,8 @@ __device__ __forceinline__ void t3_forward_A(int t, cplx<T>* __restrict__ line, 
 }
 
 // ENS: the persistent grid runs over the row pairs of `members` systems whose workspaces lie mstride bytes apart
-// (ttsh_ensemble_step); rpm = Ny/2 row pairs per member.  K3: K in line-position order, (K(y_A, x(p)), K(y_B, x(p))) at
-// ((rp NX) + p) 2 (k_reperm_t3); tab3: [5][256] W_N^{j b}, b = 1, 2, 3, 4, 8, then [6][16] W_256^{c b}, b = 1, 2, 3, 4, 8, 12.
+// (ttsh_ensemble_step); rpm = Ny/2 row pairs per member.  K3: K in line-position order, one plane per row: K(y_r, x(p)) at
+// (rp 2 + r) NX + p (k_reperm_t3); tab3: [5][256] W_N^{j b}, b = 1, 2, 3, 4, 8, then [6][16] W_256^{c b}, b = 1, 2, 3, 4, 8, 12.
 template <typename T, int NX, bool ENS>
 __global__ void __launch_bounds__(RowStep3Cfg<T, NX>::THREADS, 1)
 k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, const cplx<T>* __restrict__ inW,
@@ -187,6 +193,7 @@ k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, c
               cplx<T>* __restrict__ outA, cplx<T>* __restrict__ outB, const cplx<T>* __restrict__ tab3,
               const double* __restrict__ v0, int nblk, int rpm, size_t mstride) {
   using C = RowStep3Cfg<T, NX>;
+  constexpr int BAR_W = 5, BAR_S = 6;             // "w is in line 0" (team 0 -> teams 1, 2), "S' is in line 0" (teams 1, 2 -> team 0)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx<T>* lines = reinterpret_cast<cplx<T>*>(smem_raw);
   cplx<T>* tw = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_TW);
@@ -204,7 +211,33 @@ k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, c
     if constexpr (ENS) { const int mb = rpg / rpm; rp_ = rpg - mb * rpm; mo_ = (size_t)mb * mstride; }
     else { rp_ = rpg; mo_ = 0; }
   };
-  const cplx<T>* in_f = f == 0 ? inW : (f == 1 ? inVx : inPsi);
+  // the eight bins of this thread's butterfly pair (j, 256 - j): lo[k] = t + 256 k, hi[k] = 256 - t + 256 k.  Thread 0 runs j = 0
+  // (bins 0, 256, 512, 768, 1024) and j = 128 (bins 128, 384, 640, 896): lo[k] = 256 k, hi = 128, 384, 640, 1024, and bin 896 in ex.
+  const bool t0 = (t == 0);
+  auto bin_lo = [&](int k) -> int { return t + 256 * k; };
+  auto bin_hi = [&](int k) -> int { return t0 ? (k < 3 ? 128 + 256 * k : 1024) : 256 - t + 256 * k; };
+  // raw record of one bin: team 0: (w~(m, y_A), w~(m, y_B)); team 1 / 2: (v_x~(m, y), psi~(m, y)) of the team's row
+  auto fetch = [&](const cplx<T>* rowW, const cplx<T>* rowVx, const cplx<T>* rowPsi, int mx) -> Pair<T> {
+    if (f == 0) return ld_pair(rowW + 2 * mx);
+    Pair<T> r;
+    r.a = ld_c(rowVx + 2 * mx + (f - 1));
+    r.b = ld_c(rowPsi + 2 * mx + (f - 1));
+    return r;
+  };
+  Pair<T> lo[4], hi[4], ex;
+  ex.a = mk<T>(0, 0); ex.b = mk<T>(0, 0);
+  auto prefetch = [&](int rpg) {
+    int rp_; size_t mo_;
+    locate(rpg, rp_, mo_);
+    const cplx<T>* rowW = byte_off(inW, mo_) + (size_t)rp_ * in_stride;
+    const cplx<T>* rowVx = byte_off(inVx, mo_) + (size_t)rp_ * in_stride;
+    const cplx<T>* rowPsi = byte_off(inPsi, mo_) + (size_t)rp_ * in_stride;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) lo[k] = fetch(rowW, rowVx, rowPsi, bin_lo(k));
+#pragma unroll
+    for (int k = 0; k < 4; ++k) hi[k] = fetch(rowW, rowVx, rowPsi, bin_hi(k));
+    if (t0) ex = fetch(rowW, rowVx, rowPsi, 896);
+  };
 
   for (int i = tid; i < C::TW_ELEMS; i += C::THREADS) tw[i] = ldg_c(tab3 + i);   // host-written at ttsh_create
   __syncthreads();
@@ -212,6 +245,7 @@ k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, c
   pdl_trigger();
   T meany = (T)0;
   if constexpr (!ENS) meany = (T)(v0[1] * g.inv_sqrt_ny);
+  if ((int)blockIdx.x < nblk) prefetch(blockIdx.x);
 
 #pragma unroll 1
   for (int blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
@@ -220,82 +254,152 @@ k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, c
     if constexpr (ENS) meany = (T)(byte_off(v0, mo)[1] * g.inv_sqrt_ny);
     const int a = rp >> 1, p = rp & 1;
     const int nb = blk + gridDim.x;
-    if (t == 0 && nb < nblk) {   // L2 prefetch of what this team reads in the CTA's next iteration
+    if (t == 0 && nb < nblk) {   // L2 prefetch of what the CTA reads in its next iteration
       int nrp; size_t nmo;
       locate(nb, nrp, nmo);
-      prefetch_l2_bulk(byte_off(in_f, nmo) + (size_t)nrp * in_stride, in_bytes);
+      const cplx<T>* src = f == 0 ? inW : (f == 1 ? inVx : inPsi);
+      prefetch_l2_bulk(byte_off(src, nmo) + (size_t)nrp * in_stride, in_bytes);
       if (f == 0) prefetch_l2_bulk(byte_off(K3, nmo) + (size_t)nrp * 2 * NX, k_bytes);
     }
-    // ---- a2 / a6: w (team 0), v_x (team 1), v_y (team 2) of the two rows, in place in the team's line ----
+    // ---- a2 / a6, stage A: Z(m) = scale (wa + i wb), Z(N - m) = scale (conj wa + i conj wb) with
+    //      team 0: wa = w~(m, y_A), wb = w~(m, y_B);  team 1 / 2: wa = v_x~(m, y), wb = v_y~(m, y) = -i k_x psi~ (mean flow at m = 0)
     {
-      const cplx<T>* row = byte_off(in_f, mo) + (size_t)rp * in_stride;
-      if (f == 2) t3_inverse_A<T, NX, RM_NIKX_MEANY>(row, t, line, tw, scale_i, dkx, meany);
-      else t3_inverse_A<T, NX, RM_ONE>(row, t, line, tw, scale_i, dkx, meany);
+      auto prep = [&](Pair<T> r, int mx) -> Pair<T> {
+        if (f != 0) r.b = mx == 0 ? mk<T>(meany, (T)0) : (dkx * (T)mx) * mul_ni(r.b);
+        if (mx == 0) { r.a.y = 0; r.b.y = 0; }
+        return r;
+      };
+      auto zpos = [&](Pair<T> r) -> cplx<T> { return scale_i * mk<T>(r.a.x - r.b.y, r.a.y + r.b.x); };
+      auto zneg = [&](Pair<T> r) -> cplx<T> { return scale_i * mk<T>(r.a.x + r.b.y, r.b.x - r.a.y); };
+      auto sel = [&](Pair<T> x, Pair<T> y) -> Pair<T> {          // t0 ? x : y
+        Pair<T> r;
+        r.a = mk<T>(t0 ? x.a.x : y.a.x, t0 ? x.a.y : y.a.y);
+        r.b = mk<T>(t0 ? x.b.x : y.b.x, t0 ? x.b.y : y.b.y);
+        return r;
+      };
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { lo[k] = prep(lo[k], bin_lo(k)); hi[k] = prep(hi[k], bin_hi(k)); }
+      ex = prep(ex, 896);
+      cplx<T> v[16];
+      // butterfly j = t:  bins t + 256 k as Z(m), bins 1024 - t - 256 k as Z(N - m)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) v[k] = zpos(lo[k]);
+      v[4] = t0 ? zpos(hi[3]) : mk<T>(0, 0);
+#pragma unroll
+      for (int k = 5; k < 12; ++k) v[k] = mk<T>(0, 0);
+      v[12] = zneg(hi[3]);
+      v[13] = zneg(sel(lo[3], hi[2]));
+      v[14] = zneg(sel(lo[2], hi[1]));
+      v[15] = zneg(sel(lo[1], hi[0]));
+      t3_inverse_A_butterfly<T>(v, t, line, tw);
+      // butterfly j = 256 - t (thread 0: j = 128)
+      v[0] = zpos(hi[0]); v[1] = zpos(hi[1]); v[2] = zpos(hi[2]); v[3] = zpos(sel(ex, hi[3]));
+#pragma unroll
+      for (int k = 4; k < 12; ++k) v[k] = mk<T>(0, 0);
+      v[12] = zneg(sel(ex, lo[3]));
+      v[13] = zneg(sel(hi[2], lo[2]));
+      v[14] = zneg(sel(hi[1], lo[1]));
+      v[15] = zneg(sel(hi[0], lo[0]));
+      t3_inverse_A_butterfly<T>(v, t0 ? 128 : 256 - t, line, tw);
     }
     named_bar(1 + f, C::TEAM);
-    t3_warp_stages<+1>(line, tw, wq, l);
-    // ---- a3: lines 1-2 of Algorithm 1 on every position (x = digit-reversed p; K comes in the same order) ----
-    constexpr int NP = (NX + C::THREADS - 1) / C::THREADS;
-    cplx<T> kk[NP];
-    {
-      const T* krow = byte_off(K3, mo) + (size_t)rp * 2 * NX;
+    if (f == 0) {
+      t3_warp_stages<+1>(line, tw, wq, l);                  // w in place
+      named_bar_arrive(BAR_W, C::THREADS);
+      named_bar(BAR_S, C::THREADS);                         // S' of both rows is in line 0
+      t3_warp_stages<-1>(line, tw, wq, l);
+    } else {
+      // stage B, then per 16-point block: stage C -> lines 1-2 of Algorithm 1 -> stage C' in registers, then stage B'
+      const int c = l & 15;
+      const int s0 = 4 * wq + (l >> 4);
+      const T* kplane = byte_off(K3, mo) + ((size_t)rp * 2 + (f - 1)) * NX;
+      {
+        const TwBase<16, T> tb = t3_twB<+1>(tw, c);
 #pragma unroll
-      for (int i = 0; i < NP; ++i) {
-        const int pos = tid + i * C::THREADS;
-        kk[i] = pos < NX ? ldg_c(reinterpret_cast<const cplx<T>*>(krow) + pos) : mk<T>(0, 0);
+        for (int pi = 0; pi < 2; ++pi) {
+          cplx<T>* bl = line + 272 * (s0 + 2 * pi) + c;
+          cplx<T> v[16];
+#pragma unroll
+          for (int r = 0; r < 16; ++r) v[r] = bl[17 * r];
+          dft16<+1>(v);
+          apply_stage_twiddles<16>(v, tb);
+#pragma unroll
+          for (int r = 0; r < 16; ++r) bl[17 * r] = v[r];
+        }
+      }
+      __syncwarp();
+#pragma unroll 1
+      for (int pi = 0; pi < 2; ++pi) {
+        const int s = s0 + 2 * pi;
+        cplx<T>* bl = line + 272 * s + 17 * c;
+        Quad<T> kq[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) kq[q] = ldg_quad(kplane + 256 * s + 16 * c + 4 * q);
+        cplx<T> v[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = bl[r];
+        dft16<+1>(v);
+        if (pi == 0) named_bar(BAR_W, C::THREADS);          // w of the whole row pair is in line 0
+        T* wl = reinterpret_cast<T*>(lines + 272 * s + 17 * c) + (f - 1);      // Re (row y_A) or Im (row y_B) of line 0
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+          const T w = wl[2 * r], kk = kq[r >> 2].v[r & 3];
+          const T vx = v[r].x, vy = v[r].y;
+          const T cc = scale_f * (-beta * (vx * vx + vy * vy) - gv * kk);
+          const T lw = scale_f * lam * w;
+          v[r] = mk<T>(cc * vx + lw * vy, cc * vy - lw * vx);                  // Gx + i Gy
+          wl[2 * r] = ngw * (kk * w);                                          // S'
+        }
+        dft16<-1>(v);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) bl[r] = v[r];
+      }
+      named_bar_arrive(BAR_S, C::THREADS);
+      __syncwarp();
+      {
+        const TwBase<16, T> tb = t3_twB<-1>(tw, c);
+#pragma unroll
+        for (int pi = 0; pi < 2; ++pi) {
+          cplx<T>* bl = line + 272 * (s0 + 2 * pi) + c;
+          cplx<T> v[16];
+#pragma unroll
+          for (int r = 0; r < 16; ++r) v[r] = bl[17 * r];
+          apply_stage_twiddles<16>(v, tb);
+          dft16<-1>(v);
+#pragma unroll
+          for (int r = 0; r < 16; ++r) bl[17 * r] = v[r];
+        }
       }
     }
-    __syncthreads();
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {
-      const int pos = tid + i * C::THREADS;
-      if (pos < NX) {
-        const int q = t3_pad(pos);
-        const cplx<T> w = lines[q], vx = lines[C::LS + q], vy = lines[2 * C::LS + q];
-        const T kA = kk[i].x, kB = kk[i].y;
-        const T vxA = vx.x, vxB = vx.y, vyA = vy.x, vyB = vy.y;
-        const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * kA);
-        const T ccB = scale_f * (-beta * (vxB * vxB + vyB * vyB) - gv * kB);
-        const T lwA = scale_f * lam * w.x, lwB = scale_f * lam * w.y;
-        lines[q] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));                                  // S'
-        lines[C::LS + q] = mk<T>(ccA * vxA + lwA * vyA, ccB * vxB + lwB * vyB);                // Gx
-        lines[2 * C::LS + q] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);            // Gy
-      }
-    }
-    __syncthreads();
-    // ---- a4: forward transforms of S' (team 0), Gx (team 1), Gy (team 2) ----
-    t3_warp_stages<-1>(line, tw, wq, l);
     named_bar(1 + f, C::TEAM);
     t3_forward_A<T, NX>(t, line, tw);
-    if (f == 1) {
-      // B~ = Gx~: unpack the packed transform of (Gx(y_A), Gx(y_B))
-      named_bar(2, C::TEAM);
-      for (int mx = t; mx < Wx; mx += C::TEAM) {
-        const cplx<T> zp = line[t3_pad(mx)];
-        const cplx<T> zm = conj(line[t3_pad((NX - mx) & (NX - 1))]);
-        st_pair(byte_off(outB, mo) + inter_pair_index(g, a, p, mx), (T)0.5 * (zp + zm), (T)0.5 * mul_ni(zp - zm));
-      }
-      named_bar(2, C::TEAM);                       // line 1 is free for the next row pair
-    } else {
-      // A~ = unpack(i k_m Zgy(m) + Zs(m)), k_m the signed wavenumber of bin m: teams 0 and 2 together
-      named_bar(4, 2 * C::TEAM);
-      const cplx<T>* ls = lines;
-      const cplx<T>* lg = lines + 2 * C::LS;
-      const cplx<T> zg0 = lg[0];                   // Zgy(0) = Gy~(0, y_A) + i Gy~(0, y_B)
-      for (int mx = (f >> 1) * C::TEAM + t; mx < Wx; mx += 2 * C::TEAM) {
+    prefetch(nb < nblk ? nb : blk);            // the next row pair's bins are in flight during the unpack (last iteration: a
+                                               // harmless re-read, so that the registers are dead through the loop body)
+    __syncthreads();
+    // ---- unpack: Z0 = S'(y_A) + i S'(y_B), Z1 = Gx(y_A) + i Gy(y_A), Z2 = Gx(y_B) + i Gy(y_B) (all transformed) ----
+    {
+      const cplx<T>* l0 = lines;
+      const cplx<T>* l1 = lines + C::LS;
+      const cplx<T>* l2 = lines + 2 * C::LS;
+      for (int mx = tid; mx < Wx; mx += C::THREADS) {
         const int qp = t3_pad(mx), qm = t3_pad((NX - mx) & (NX - 1));
+        const cplx<T> z0p = l0[qp], z0m = conj(l0[qm]), z1p = l1[qp], z1m = conj(l1[qm]), z2p = l2[qp], z2m = conj(l2[qm]);
+        const T h = (T)0.5;
+        const cplx<T> sA = h * (z0p + z0m), sB = h * mul_ni(z0p - z0m);
+        const cplx<T> gxA = h * (z1p + z1m), gyA = h * mul_ni(z1p - z1m);
+        const cplx<T> gxB = h * (z2p + z2m), gyB = h * mul_ni(z2p - z2m);
         const T kx = dkx * (T)mx;
-        const cplx<T> zp = ls[qp] + kx * mul_i(lg[qp]);
-        const cplx<T> zm = conj(ls[qm] + (-kx) * mul_i(lg[qm]));
-        cplx<T> sa = (T)0.5 * (zp + zm), sb = (T)0.5 * mul_ni(zp - zm);
+        cplx<T> oa = sA + kx * mul_i(gyA), ob = sB + kx * mul_i(gyB);
         if (mx == 0) {                // real numbers S'~(0,y) and Gy~(0,y) travel together (k_fwd_row_fused)
-          sa = mk<T>(sa.x, zg0.x);
-          sb = mk<T>(sb.x, zg0.y);
+          oa = mk<T>(sA.x, gyA.x);
+          ob = mk<T>(sB.x, gyB.x);
         }
-        st_pair(byte_off(outA, mo) + inter_pair_index(g, a, p, mx), sa, sb);
+        const size_t o = inter_pair_index(g, a, p, mx);
+        st_pair(byte_off(outB, mo) + o, gxA, gxB);
+        st_pair(byte_off(outA, mo) + o, oa, ob);
       }
-      named_bar(4, 2 * C::TEAM);                   // lines 0 and 2 are free for the next row pair
     }
+    __syncthreads();
   }
 }
 

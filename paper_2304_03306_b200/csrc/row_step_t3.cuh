@@ -28,9 +28,12 @@
 // Stage A reads its inputs (the pruned inverse intermediates, retained bins |m| <= N/4 only) straight from global memory into
 // registers, one row pair AHEAD (issued before the unpack of the previous row pair); butterflies j and 256 - j need the same eight
 // bins (one as Z(m), the other as Z(N - m)), so a thread runs that pair and every bin is loaded once.
-// Synchronisation per row pair: team barriers after A and before A'; team 0 -> teams 1, 2 "w is in line 0" and back "S' is in
-// line 0" (bar.arrive / bar.sync); two CTA barriers around the unpack, which needs all three lines:
-//   B~ = (Gx~(y_A), Gx~(y_B)),   A~ = i k_x Gy~ + S'~   (fft_passes.cuh, k_fwd_row_fused).
+// Stage A' runs the same butterfly pairs, so a thread ends up with Z(m) and Z(N - m) of its eight bins in registers and unpacks
+// them there; a team writes its own row's half of the output pairs
+//   B~ = (Gx~(y_A), Gx~(y_B)),   A~ = i k_x Gy~ + S'~   (fft_passes.cuh, k_fwd_row_fused),
+// S'~ coming from line 0.  Stage A of the next row pair writes exactly the columns the thread read in A', so no barrier separates
+// the two.  Synchronisation per row pair: team barriers after A and before A', and four handshakes with team 0 (bar.arrive /
+// bar.sync): "w is in line 0", "S' is in line 0", "S'~ is in line 0", "line 0 is free".  No CTA-wide barrier in the loop.
 #pragma once
 #include "fft_passes.cuh"
 
@@ -162,30 +165,27 @@ __device__ __forceinline__ void t3_inverse_A_butterfly(cplx<T> (&v)[16], int j, 
   for (int s = 0; s < 16; ++s) col[272 * s] = v[s];
 }
 
-// stage A' of the forward transform: bins 256 k0 + i in place; only the retained bins (|m| <= NX/4) are stored
-template <typename T, int NX>
-__device__ __forceinline__ void t3_forward_A(int t, cplx<T>* __restrict__ line, const cplx<T>* __restrict__ tw) {
-#pragma unroll 1
-  for (int h = 0; h < 2; ++h) {
-    const int i = t + 128 * h;
-    cplx<T>* col = line + i + (i >> 4);
-    const TwBase<16, T> tb = t3_twA<-1>(tw, i);
-    cplx<T> v[16];
+// one radix-16 butterfly of stage A' (forward): bins 256 k0 + i, k0 = 0..15, left in registers
+template <typename T>
+__device__ __forceinline__ void t3_forward_A_butterfly(cplx<T> (&v)[16], int i, const cplx<T>* __restrict__ line, const cplx<T>* __restrict__ tw) {
+  const cplx<T>* col = line + i + (i >> 4);
+  const TwBase<16, T> tb = t3_twA<-1>(tw, i);
 #pragma unroll
-    for (int n0 = 0; n0 < 16; ++n0) v[n0] = col[272 * n0];
-    apply_stage_twiddles<16>(v, tb);
-    dft16<-1>(v);
-#pragma unroll
-    for (int k0 = 0; k0 < 4; ++k0) col[272 * k0] = v[k0];
-    if (i == 0) col[272 * 4] = v[4];
-#pragma unroll
-    for (int k0 = 12; k0 < 16; ++k0) col[272 * k0] = v[k0];
-  }
+  for (int n0 = 0; n0 < 16; ++n0) v[n0] = col[272 * n0];
+  apply_stage_twiddles<16>(v, tb);
+  dft16<-1>(v);
+}
+__device__ __forceinline__ void st_c(cplx<double>* p, cplx<double> a) {
+  asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a.x), "d"(a.y));
+}
+__device__ __forceinline__ void st_c(cplx<float>* p, cplx<float> a) {
+  asm volatile("st.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a.x), "f"(a.y));
 }
 
 // ENS: the persistent grid runs over the row pairs of `members` systems whose workspaces lie mstride bytes apart
-// (ttsh_ensemble_step); rpm = Ny/2 row pairs per member.  K3: K in line-position order, one plane per row: K(y_r, x(p)) at
-// (rp 2 + r) NX + p (k_reperm_t3); tab3: [5][256] W_N^{j b}, b = 1, 2, 3, 4, 8, then [6][16] W_256^{c b}, b = 1, 2, 3, 4, 8, 12.
+// (ttsh_ensemble_step); rpm = Ny/2 row pairs per member.  K3: one plane of NX values per row, (rp 2 + r) NX + e, in the order the
+// pointwise stage reads it: line position p = 256 s + 16 c + 4 q + i (x = digit-reversed p) at e = ((4 s + q) 16 + c) 4 + i, so that
+// the 16 threads c of a block read 512 contiguous bytes per access (k_reperm_t3); tab3: [5][256] W_N^{j b}, b = 1, 2, 3, 4, 8, then [6][16] W_256^{c b}, b = 1, 2, 3, 4, 8, 12.
 template <typename T, int NX, bool ENS>
 __global__ void __launch_bounds__(RowStep3Cfg<T, NX>::THREADS, 1)
 k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, const cplx<T>* __restrict__ inW,
@@ -194,6 +194,7 @@ k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, c
               const double* __restrict__ v0, int nblk, int rpm, size_t mstride) {
   using C = RowStep3Cfg<T, NX>;
   constexpr int BAR_W = 5, BAR_S = 6;             // "w is in line 0" (team 0 -> teams 1, 2), "S' is in line 0" (teams 1, 2 -> team 0)
+  constexpr int BAR_Z = 7, BAR_F = 8;             // "S'~ is in line 0" (team 0 -> teams 1, 2), "line 0 is free" (teams 1, 2 -> team 0)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx<T>* lines = reinterpret_cast<cplx<T>*>(smem_raw);
   cplx<T>* tw = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_TW);
@@ -334,7 +335,7 @@ k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, c
         cplx<T>* bl = line + 272 * s + 17 * c;
         Quad<T> kq[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) kq[q] = ldg_quad(kplane + 256 * s + 16 * c + 4 * q);
+        for (int q = 0; q < 4; ++q) kq[q] = ldg_quad(kplane + ((4 * s + q) * 16 + c) * 4);     // K at positions 256 s + 16 c + 4 q + (0..3)
         cplx<T> v[16];
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[r] = bl[r];
@@ -372,34 +373,77 @@ k_row_step_t3(const __grid_constant__ Geom g, const __grid_constant__ Model m, c
       }
     }
     named_bar(1 + f, C::TEAM);
-    t3_forward_A<T, NX>(t, line, tw);
-    prefetch(nb < nblk ? nb : blk);            // the next row pair's bins are in flight during the unpack (last iteration: a
-                                               // harmless re-read, so that the registers are dead through the loop body)
-    __syncthreads();
-    // ---- unpack: Z0 = S'(y_A) + i S'(y_B), Z1 = Gx(y_A) + i Gy(y_A), Z2 = Gx(y_B) + i Gy(y_B) (all transformed) ----
-    {
-      const cplx<T>* l0 = lines;
-      const cplx<T>* l1 = lines + C::LS;
-      const cplx<T>* l2 = lines + 2 * C::LS;
-      for (int mx = tid; mx < Wx; mx += C::THREADS) {
-        const int qp = t3_pad(mx), qm = t3_pad((NX - mx) & (NX - 1));
-        const cplx<T> z0p = l0[qp], z0m = conj(l0[qm]), z1p = l1[qp], z1m = conj(l1[qm]), z2p = l2[qp], z2m = conj(l2[qm]);
-        const T h = (T)0.5;
-        const cplx<T> sA = h * (z0p + z0m), sB = h * mul_ni(z0p - z0m);
-        const cplx<T> gxA = h * (z1p + z1m), gyA = h * mul_ni(z1p - z1m);
-        const cplx<T> gxB = h * (z2p + z2m), gyB = h * mul_ni(z2p - z2m);
-        const T kx = dkx * (T)mx;
-        cplx<T> oa = sA + kx * mul_i(gyA), ob = sB + kx * mul_i(gyB);
-        if (mx == 0) {                // real numbers S'~(0,y) and Gy~(0,y) travel together (k_fwd_row_fused)
-          oa = mk<T>(sA.x, gyA.x);
-          ob = mk<T>(sB.x, gyB.x);
-        }
-        const size_t o = inter_pair_index(g, a, p, mx);
-        st_pair(byte_off(outB, mo) + o, gxA, gxB);
-        st_pair(byte_off(outA, mo) + o, oa, ob);
+    // ---- stage A' for the butterfly pair (i, 256 - i): the thread then holds Z(m) AND Z(N - m) of its eight bins m ----
+    const int i2 = t0 ? 128 : 256 - t;
+    if (f == 0) {
+      // S'~: the retained bins go back to line 0 in place, where teams 1 and 2 pick them up
+      cplx<T> v[16];
+      t3_forward_A_butterfly<T>(v, t, line, tw);
+      {
+        cplx<T>* col = line + t + (t >> 4);
+#pragma unroll
+        for (int k0 = 0; k0 < 4; ++k0) col[272 * k0] = v[k0];
+        if (t0) col[272 * 4] = v[4];
+#pragma unroll
+        for (int k0 = 12; k0 < 16; ++k0) col[272 * k0] = v[k0];
       }
+      t3_forward_A_butterfly<T>(v, i2, line, tw);
+      {
+        cplx<T>* col = line + i2 + (i2 >> 4);
+#pragma unroll
+        for (int k0 = 0; k0 < 4; ++k0) col[272 * k0] = v[k0];
+#pragma unroll
+        for (int k0 = 12; k0 < 16; ++k0) col[272 * k0] = v[k0];
+      }
+      named_bar_arrive(BAR_Z, C::THREADS);
+      prefetch(nb < nblk ? nb : blk);          // last iteration: a harmless re-read, so that the registers are dead through the loop body
+      named_bar(BAR_F, C::THREADS);            // teams 1 and 2 have read S'~: line 0 is free for the next row pair
+    } else {
+      // Z1 = transform of Gx(y) + i Gy(y) of the team's row y:  Gx~(m) = (Z1(m) + conj Z1(N-m)) / 2,  Gy~(m) = -i (Z1(m) - conj Z1(N-m)) / 2;
+      // S'~(m, y_A) / S'~(m, y_B) are the same two combinations of Z0 (line 0).  Outputs: this row's half of the pairs
+      //   B~ = Gx~,   A~ = i k_x Gy~ + S'~   (column m = 0: the real numbers S'~(0, y) + i Gy~(0, y) travel together, k_fwd_row_fused)
+      cplx<T> a1[5], b1[4], a2[4], b2[4];
+      {
+        cplx<T> v[16];
+        t3_forward_A_butterfly<T>(v, t, line, tw);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) a1[k] = v[k];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) b1[k] = v[12 + k];
+        t3_forward_A_butterfly<T>(v, i2, line, tw);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { a2[k] = v[k]; b2[k] = v[12 + k]; }
+      }
+      prefetch(nb < nblk ? nb : blk);
+      named_bar(BAR_Z, C::THREADS);
+      const cplx<T>* l0 = lines;
+      cplx<T>* oB = byte_off(outB, mo) + (f - 1);
+      cplx<T>* oA = byte_off(outA, mo) + (f - 1);
+      auto emit = [&](int mx, cplx<T> zp, cplx<T> zmr) {
+        const cplx<T> zm = conj(zmr);
+        const T h = (T)0.5;
+        const cplx<T> gx = h * (zp + zm), gy = h * mul_ni(zp - zm);
+        const cplx<T> z0p = l0[t3_pad(mx)], z0m = conj(l0[t3_pad((NX - mx) & (NX - 1))]);
+        const cplx<T> sA = h * (z0p + z0m), sB = h * mul_ni(z0p - z0m);
+        const cplx<T> sv = f == 1 ? sA : sB;
+        cplx<T> oa = sv + (dkx * (T)mx) * mul_i(gy);
+        if (mx == 0) oa = mk<T>(sv.x, gy.x);
+        const size_t o = inter_pair_index(g, a, p, mx);
+        st_c(oB + o, gx);
+        st_c(oA + o, oa);
+      };
+      auto selc = [&](cplx<T> x, cplx<T> y) -> cplx<T> { return mk<T>(t0 ? x.x : y.x, t0 ? x.y : y.y); };
+      // bins t + 256 k: Z(m) from butterfly t; Z(N - m) from butterfly 256 - t (thread 0: from butterfly 0 itself, bin 0 is its own mirror)
+      emit(t, a1[0], selc(a1[0], b2[3]));
+      emit(t + 256, a1[1], selc(b1[3], b2[2]));
+      emit(t + 512, a1[2], selc(b1[2], b2[1]));
+      emit(t + 768, a1[3], selc(b1[1], b2[0]));
+      // bins 256 - t + 256 k (thread 0: 128 + 256 k, both halves from butterfly 128)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) emit(i2 + 256 * k, a2[k], selc(b2[3 - k], b1[3 - k]));
+      if (t0) emit(NX / 4, a1[4], b1[0]);
+      named_bar_arrive(BAR_F, C::THREADS);
     }
-    __syncthreads();
   }
 }
 

@@ -46,6 +46,10 @@ template <typename T> bool row_step_supported(const Geom& g);
 // ... and it is the three-team in-place variant (row_step_t3.cuh: Nx = 4096 in fp64), which wants K in line-position order
 // (launch_reperm_t3) and the table of fill_stage_tables_t3
 template <typename T> bool row_step_is_t3(const Geom& g);
+// ... or the real-row variant (row_step_real.cuh: Nx = 8192 in fp64): K in its thread order (launch_reperm_real); table = the warp-local
+// table of length Nx/2 followed, at element row_step_real_tabr(g), by W_Nx^j, j < Nx/32
+template <typename T> bool row_step_is_real(const Geom& g);
+template <typename T> int row_step_real_tabr(const Geom& g);
 // per-device set-up of k_row_step (shared-memory opt-in, resident CTAs): call on the handle's device; slots = CTAs of the
 // persistent grid of the single-system / ensemble variant (0: not supported for this grid)
 template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens, int* slots_tan);
@@ -82,6 +86,8 @@ template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* i
 template <typename T> cudaError_t launch_reperm_wl(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
 // permuted internal row layout -> line-position order of row_step_t3.cuh, one plane per row: K(y_r, x(p)) at (rp 2 + r) Nx + p
 template <typename T> cudaError_t launch_reperm_t3(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
+// permuted internal row layout -> thread order of row_step_real.cuh: (K(y, 2n), K(y, 2n+1)), n = wl_j(t) + (Nx/32) k, at y Nx + (k Nx/32 + t) 2
+template <typename T> cudaError_t launch_reperm_real(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
 constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs
 template <typename T> cudaError_t launch_diag(const Geom& g, double dx, double cx, double cy, const void* vx, const void* vy,
                                               const void* w, double* partial, double* out, cudaStream_t s);

@@ -93,6 +93,24 @@ __device__ __forceinline__ void st_pair(cplx<float>* p, cplx<float> a, cplx<floa
   asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
 }
 
+// one complex value (one row's half of a pair)
+__device__ __forceinline__ cplx<double> ld_c(const cplx<double>* p) {
+  cplx<double> r;
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ cplx<float> ld_c(const cplx<float>* p) {
+  cplx<float> r;
+  asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_c(cplx<double>* p, cplx<double> a) {
+  asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a.x), "d"(a.y));
+}
+__device__ __forceinline__ void st_c(cplx<float>* p, cplx<float> a) {
+  asm volatile("st.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a.x), "f"(a.y));
+}
+
 // 4 consecutive scalars of a (permuted) real row: one 32-byte (fp64) / 16-byte (fp32) access
 template <typename T> struct Quad { T v[4]; };
 __device__ __forceinline__ Quad<double> ld_quad(const double* p) {

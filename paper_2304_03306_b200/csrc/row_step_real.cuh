@@ -1,0 +1,203 @@
+// row_step_real.cuh — the row half of one Euler step in ONE kernel (row_step.cuh) for Nx = 8192 in fp64, the paper's production
+// width, where a packed row PAIR (128 KB per field) no longer fits in shared memory.
+//
+// One REAL row is transformed as a half-length complex sequence z[n] = f(2n) + i f(2n+1), n < M = Nx/2 = 4096 (the textbook
+// real-data FFT), so that the machinery of row_step.cuh applies unchanged at N = 4096: the warp-local plan of fft_core.cuh, one
+// field live in registers (V), one waiting in registers (H), one in the private shared-memory stash.  The pointwise stage
+// (lines 1-2 of Algorithm 1) does not care that a complex slot now holds two neighbouring points of one row
+// instead of one point of two rows.  What changes is the step between the half spectrum F (what the column passes read and
+// write) and the transform Z of the packed sequence:
+//
+//   inverse:  Z2(m) = (F(m) + conj F(M-m)) + i W^{-m} (F(m) - conj F(M-m)),  W = exp(-2 pi i / Nx);  z = iDFT_M(Z2) / sqrt(Nx).
+//             Under the 1/2 rule F(m) = 0 for m > M/2, so a slot needs ONE bin:
+//               m < M/2:  Z2(m) = F(m) + i conj(W^m) F(m)          m = 0:  F(0) (1 + i)  (F(0) real)
+//               m > M/2:  Z2(m) = c - i conj(W^m) c,  c = conj F(M-m)          m = M/2:  2 conj F(M/2)
+//   forward:  F(k) = E(k) + W^k O(k),  E = (Z(k) + conj Z(M-k)) / 2,  O = -i (Z(k) - conj Z(M-k)) / 2,  k = 0..M/2 (retained).
+//             i k_x does not commute with this step, so the three forward transforms are merged separately and
+//             A~ = i k_x Gy~ + S'~ is formed on the merged bins (a thread merges the same bins k = j + 256 i of every transform).
+//   W^m for m = j + 256 k is W^j W_32^k: one table entry per thread (tabR, W^j for j < 256) and compile-time constants.
+//
+// A CTA takes a row pair (rows 4a+p and 4a+p+2 share the (A, B) pairs of the intermediates, ttsh_common.cuh) and runs its two
+// rows one after the other; inputs come straight from global memory (L2-prefetched one row pair ahead), 16 bytes per bin.
+// K comes in the thread order of the plan: (K(y, 2n), K(y, 2n+1)) for n = wl_j(t) + 256 k at (k 256 + t) 2 (k_reperm_real).
+#pragma once
+#include "row_step.cuh"
+
+namespace ttsh {
+
+template <typename T, int NX> struct RowStepRealCfg {
+  static constexpr int M = NX / 2;                                  // complex length
+  static constexpr bool OK = fft_wl_supported<M>();
+  static constexpr int TPL = M / 16, THREADS = TPL;
+  static constexpr int LS = fft_wl_line_elems<T, M>() + 4;
+  static constexpr size_t OFF_STASH = (size_t)LS * sizeof(cplx<T>);
+  static constexpr size_t OFF_TAB = OFF_STASH + (size_t)M * sizeof(cplx<T>);
+  static constexpr size_t OFF_K = (OFF_TAB + (size_t)fft_wl_tw_elems_rt(M) * sizeof(cplx<T>) + 127) / 128 * 128;   // one row of K, staged
+  static constexpr size_t OFF_BAR = OFF_K + (size_t)NX * sizeof(T);
+  static constexpr size_t SMEM = OFF_BAR + 16;
+  static constexpr bool FITS = OK && SMEM <= 227 * 1024;
+};
+
+// W^m = wj W_32^k for m = j + 256 k (forward sign), k a compile-time constant after unrolling
+template <typename T> __device__ __forceinline__ cplx<T> real_row_tw(cplx<T> wj, int k) { return mul_w32_rt<-1>(wj, k); }
+
+// inverse transform of one real row into registers: out[k] = f(2n) + i f(2n+1), n = wl_j(j) + k TPL.
+// row: bin m of this row at row[2 m] (its half of the (A, B) pair of the inverse intermediate, global memory).
+// MODE = RM_ONE or RM_NIKX_MEANY (ttsh_common.cuh).  1/2 rule only: retained m = 0..M/2.
+template <typename T, int M, int MODE, class Hook>
+__device__ __forceinline__ void inv_real_row_regs(const cplx<T>* __restrict__ row, int j, cplx<T> wj, cplx<T>* __restrict__ line,
+                                                  const cplx<T>* __restrict__ tab, T scale, T dkx, T meany, cplx<T> (&out)[16], Hook hook) {
+  constexpr int TPL = M / 16;
+  auto mult = [&](cplx<T> w, int mx) -> cplx<T> {
+    if (MODE == RM_ONE) return mx == 0 ? mk<T>(w.x, (T)0) : w;
+    const T kx = dkx * (T)mx;
+    return mx == 0 ? mk<T>(meany, (T)0) : kx * mul_ni(w);        // RM_NIKX_MEANY
+  };
+  auto issue = [&](int mm, int k) -> cplx<T> {
+    if (k < 8 || (k == 8 && j == 0)) return ld_c(row + 2 * mm);
+    return ld_c(row + 2 * (M - mm));
+  };
+  auto finish = [&](int mm, int k, cplx<T> raw) -> cplx<T> {
+    const cplx<T> wm = real_row_tw(wj, k);                        // W^mm
+    if (k < 8) {
+      const cplx<T> F = mult(raw, mm);
+      const cplx<T> z = F + mul_i(mul_conj(F, wm));
+      return scale * ((k == 0 && j == 0) ? mk<T>(F.x, F.x) : z);
+    }
+    const bool mid = (k == 8 && j == 0);
+    const cplx<T> c = conj(mult(raw, mid ? M / 2 : M - mm));
+    const cplx<T> z = c - mul_i(mul_conj(c, wm));
+    return scale * (mid ? mk<T>(c.x + c.x, c.y + c.y) : z);
+  };
+  auto store = [&](int, int k, cplx<T> z) { out[k] = z; };
+  fft_line_wl<T, M, +1, false>(j, j, line, tab, make_loader<1>(issue, finish), store, hook);
+}
+
+// ENS: the persistent grid runs over the row pairs of `members` systems whose workspaces lie mstride bytes apart; rpm = Ny/2.
+// K2: K in thread order (k_reperm_real); tabW: the warp-local table of length M (fill_stage_tables_wl); tabR: W_NX^j, j < M/16.
+template <typename T, int NX, bool ENS>
+__global__ void __launch_bounds__(RowStepRealCfg<T, NX>::THREADS, 1)
+k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m, const cplx<T>* __restrict__ inW,
+                const cplx<T>* __restrict__ inVx, const cplx<T>* __restrict__ inPsi, const T* __restrict__ K2,
+                cplx<T>* __restrict__ outA, cplx<T>* __restrict__ outB, const cplx<T>* __restrict__ tabW,
+                const cplx<T>* __restrict__ tabR, const double* __restrict__ v0, int nblk, int rpm, size_t mstride) {
+  using C = RowStepRealCfg<T, NX>;
+  constexpr int M = C::M, TPL = C::TPL;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  cplx<T>* line = reinterpret_cast<cplx<T>*>(smem_raw);
+  const int j = threadIdx.x;
+  const int jw = fft_wl_j<M>(j);                                   // the thread owns slots n = jw + k TPL
+  cplx<T>* stash = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_STASH) + j;      // slot k at stash[k TPL]
+  cplx<T>* stab = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_TAB);
+  const cplx<T>* kslot = reinterpret_cast<const cplx<T>*>(smem_raw + C::OFF_K);
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem_raw + C::OFF_BAR);
+  const T scale_i = (T)g.inv_sqrt_nx, scale_f = (T)g.inv_sqrt_nx;
+  const T dkx = (T)g.dkx;
+  const T beta = (T)m.beta, gv = (T)m.gamma_v, lam = (T)m.lambda0;
+  const T ngw = -(T)m.gamma_w * scale_f;
+  const size_t in_stride = (size_t)g.Wxp * 2;               // elements per row pair of an inverse intermediate
+  const unsigned in_bytes = (unsigned)(in_stride * sizeof(cplx<T>)), k_bytes = (unsigned)(NX * sizeof(T));
+  const bool leader = (j == 0);
+  unsigned ph = 0;
+  auto locate = [&](int rpg, int& rp_, size_t& mo_) {
+    if constexpr (ENS) { const int mb = rpg / rpm; rp_ = rpg - mb * rpm; mo_ = (size_t)mb * mstride; }
+    else { rp_ = rpg; mo_ = 0; }
+  };
+  if (leader) mbar_init(bar, 1);
+  mbar_fence_init();
+  for (int i = j; i < fft_wl_tw_elems_rt(M); i += C::THREADS) stab[i] = ldg_c(tabW + i);     // host-written at ttsh_create
+  const cplx<T> wj = ldg_c(tabR + j);                              // W_NX^j
+  __syncthreads();
+  pdl_wait();          // inputs, K and v0 below are written by the preceding launches
+  pdl_trigger();
+  T meany = (T)0;
+  if constexpr (!ENS) meany = (T)(v0[1] * g.inv_sqrt_ny);
+
+#pragma unroll 1
+  for (int blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
+    int rp; size_t mo;
+    locate(blk, rp, mo);
+    if constexpr (ENS) meany = (T)(byte_off(v0, mo)[1] * g.inv_sqrt_ny);
+    const int a = rp >> 1, p = rp & 1;
+    const int nb = blk + gridDim.x;
+    if (leader && nb < nblk) {   // L2 prefetch of what the CTA reads in its next iteration
+      int nrp; size_t nmo;
+      locate(nb, nrp, nmo);
+      prefetch_l2_bulk(byte_off(inW, nmo) + (size_t)nrp * in_stride, in_bytes);
+      prefetch_l2_bulk(byte_off(inVx, nmo) + (size_t)nrp * in_stride, in_bytes);
+      prefetch_l2_bulk(byte_off(inPsi, nmo) + (size_t)nrp * in_stride, in_bytes);
+      const size_t ny = (size_t)(4 * (nrp >> 1) + (nrp & 1)) * NX;
+      prefetch_l2_bulk(byte_off(K2, nmo) + ny, k_bytes);
+      prefetch_l2_bulk(byte_off(K2, nmo) + ny + 2 * (size_t)NX, k_bytes);
+    }
+#pragma unroll 1
+    for (int r = 0; r < 2; ++r) {
+      const size_t y = (size_t)(4 * a + p + 2 * r);
+      const cplx<T>* rowW = byte_off(inW, mo) + (size_t)rp * in_stride + r;
+      const cplx<T>* rowVx = byte_off(inVx, mo) + (size_t)rp * in_stride + r;
+      const cplx<T>* rowPsi = byte_off(inPsi, mo) + (size_t)rp * in_stride + r;
+      cplx<T> H[16], V[16];
+      // ---- a2 / a6: w, v_x, v_y of the row; the first barrier of the first transform frees the K slot of the previous row ----
+      inv_real_row_regs<T, M, RM_ONE>(rowW, j, wj, line, stab, scale_i, dkx, meany, V,
+                                      [&]() { if (leader) bulk_load(const_cast<cplx<T>*>(kslot), byte_off(K2, mo) + y * NX, k_bytes, bar); });
+#pragma unroll
+      for (int k = 0; k < 16; ++k) stash[k * TPL] = V[k];                     // w
+      inv_real_row_regs<T, M, RM_ONE>(rowVx, j, wj, line, stab, scale_i, dkx, meany, H, NoHook());          // v_x
+      inv_real_row_regs<T, M, RM_NIKX_MEANY>(rowPsi, j, wj, line, stab, scale_i, dkx, meany, V, NoHook());  // v_y
+      // ---- a3: lines 1-2 of Algorithm 1 on the two points of every slot;  V <- Gx,  H <- Gy,  stash <- S' ----
+      mbar_wait(bar, ph); ph ^= 1;
+#pragma unroll
+      for (int k = 0; k < 16; ++k) {
+        const cplx<T> kk = kslot[k * TPL + j];
+        const cplx<T> w = stash[k * TPL];
+        const T kA = kk.x, kB = kk.y;
+        const T vxA = H[k].x, vxB = H[k].y, vyA = V[k].x, vyB = V[k].y;
+        const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * kA);
+        const T ccB = scale_f * (-beta * (vxB * vxB + vyB * vyB) - gv * kB);
+        const T lwA = scale_f * lam * w.x, lwB = scale_f * lam * w.y;
+        V[k] = mk<T>(ccA * vxA + lwA * vyA, ccB * vxB + lwB * vyB);          // Gx
+        H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
+        stash[k * TPL] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));          // S'
+      }
+      // ---- a4: three forward transforms, each merged into the half spectrum of the row on the bins k = j + 256 i ----
+      auto ident = [&](int, int, cplx<T> z) -> cplx<T> { return z; };
+      auto to_line = [&](int mm, int, cplx<T> z) { line[fft_wl_pad<T, M>(mm)] = z; };
+      auto merged = [&](int i) -> cplx<T> {                          // F(k), k = j + 256 i
+        const int k = j + TPL * i;
+        const cplx<T> zp = line[fft_wl_pad<T, M>(k)];
+        const cplx<T> zm = conj(line[fft_wl_pad<T, M>((M - k) & (M - 1))]);
+        const cplx<T> e = (T)0.5 * (zp + zm), o = (T)0.5 * mul_ni(zp - zm);
+        return e + real_row_tw(wj, i) * o;
+      };
+      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < 9; ++i)
+        if (i < 8 || leader) st_c(byte_off(outB, mo) + inter_pair_index(g, a, p, j + TPL * i) + r, merged(i));      // B~ = Gx~
+      cplx<T> ikg[9];
+      T gy0 = (T)0;
+      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), to_line);
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < 9; ++i) {
+        ikg[i] = mk<T>(0, 0);
+        if (i < 8 || leader) {
+          const cplx<T> gy = merged(i);
+          if (i == 0) gy0 = gy.x;
+          ikg[i] = (dkx * (T)(j + TPL * i)) * mul_i(gy);
+        }
+      }
+      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return stash[k * TPL]; }, ident), to_line);
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < 9; ++i)
+        if (i < 8 || leader) {
+          cplx<T> sa = merged(i) + ikg[i];
+          if (i == 0 && leader) sa = mk<T>(sa.x, gy0);       // real numbers S'~(0, y) and Gy~(0, y) travel together (k_fwd_row_fused)
+          st_c(byte_off(outA, mo) + inter_pair_index(g, a, p, j + TPL * i) + r, sa);
+        }
+    }
+  }
+}
+
+}  // namespace ttsh

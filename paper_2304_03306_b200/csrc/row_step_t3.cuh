@@ -70,17 +70,6 @@ __device__ __forceinline__ Quad<float> ldg_quad(const float* p) {
   asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "l"(p));
   return r;
 }
-__device__ __forceinline__ cplx<double> ld_c(const cplx<double>* p) {
-  cplx<double> r;
-  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-  return r;
-}
-__device__ __forceinline__ cplx<float> ld_c(const cplx<float>* p) {
-  cplx<float> r;
-  asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
-  return r;
-}
-
 template <int DIR, typename T> __device__ __forceinline__ TwBase<16, T> t3_twA(const cplx<T>* __restrict__ tw, int j) {
   TwBase<16, T> b;
 #pragma unroll
@@ -175,13 +164,6 @@ __device__ __forceinline__ void t3_forward_A_butterfly(cplx<T> (&v)[16], int i, 
   apply_stage_twiddles<16>(v, tb);
   dft16<-1>(v);
 }
-__device__ __forceinline__ void st_c(cplx<double>* p, cplx<double> a) {
-  asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a.x), "d"(a.y));
-}
-__device__ __forceinline__ void st_c(cplx<float>* p, cplx<float> a) {
-  asm volatile("st.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a.x), "f"(a.y));
-}
-
 // ENS: the persistent grid runs over the row pairs of `members` systems whose workspaces lie mstride bytes apart
 // (ttsh_ensemble_step); rpm = Ny/2 row pairs per member.  K3: one plane of NX values per row, (rp 2 + r) NX + e, in the order the
 // pointwise stage reads it: line position p = 256 s + 16 c + 4 q + i (x = digit-reversed p) at e = ((4 s + q) 16 + c) 4 + i, so that

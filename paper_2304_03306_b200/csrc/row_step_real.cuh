@@ -18,7 +18,9 @@
 //   W^m for m = j + 256 k is W^j W_32^k: one table entry per thread (tabR, W^j for j < 256) and compile-time constants.
 //
 // A CTA takes a row pair (rows 4a+p and 4a+p+2 share the (A, B) pairs of the intermediates, ttsh_common.cuh) and runs its two
-// rows one after the other; inputs come straight from global memory (L2-prefetched one row pair ahead), 16 bytes per bin.
+// rows one after the other.  Everything a row reads arrives by cp.async.bulk + mbarrier in ONE staging slot, each copy issued
+// right after the barrier that ends the previous use of the slot, i.e. one transform ahead of its consumer:
+//   w~ pairs -> v_x~ pairs -> psi~ pairs -> K row -> w~ pairs of the next row (the same pairs again for the second row of the pair).
 // K comes in the thread order of the plan: (K(y, 2n), K(y, 2n+1)) for n = wl_j(t) + 256 k at (k 256 + t) 2 (k_reperm_real).
 #pragma once
 #include "row_step.cuh"
@@ -32,8 +34,10 @@ template <typename T, int NX> struct RowStepRealCfg {
   static constexpr int LS = fft_wl_line_elems<T, M>() + 4;
   static constexpr size_t OFF_STASH = (size_t)LS * sizeof(cplx<T>);
   static constexpr size_t OFF_TAB = OFF_STASH + (size_t)M * sizeof(cplx<T>);
-  static constexpr size_t OFF_K = (OFF_TAB + (size_t)fft_wl_tw_elems_rt(M) * sizeof(cplx<T>) + 127) / 128 * 128;   // one row of K, staged
-  static constexpr size_t OFF_BAR = OFF_K + (size_t)NX * sizeof(T);
+  // one staging slot, used in turn by the (A, B) pairs of w~, v_x~, psi~ (2 Wxp <= 2 (NX/4 + 8) complex values) and by the row of K
+  static constexpr size_t SLOT = ((size_t)(NX / 4 + 8) * 2 * sizeof(cplx<T>) + 127) / 128 * 128;
+  static constexpr size_t OFF_K = (OFF_TAB + (size_t)fft_wl_tw_elems_rt(M) * sizeof(cplx<T>) + 127) / 128 * 128;
+  static constexpr size_t OFF_BAR = OFF_K + SLOT;
   static constexpr size_t SMEM = OFF_BAR + 16;
   static constexpr bool FITS = OK && SMEM <= 227 * 1024;
 };
@@ -42,7 +46,7 @@ template <typename T, int NX> struct RowStepRealCfg {
 template <typename T> __device__ __forceinline__ cplx<T> real_row_tw(cplx<T> wj, int k) { return mul_w32_rt<-1>(wj, k); }
 
 // inverse transform of one real row into registers: out[k] = f(2n) + i f(2n+1), n = wl_j(j) + k TPL.
-// row: bin m of this row at row[2 m] (its half of the (A, B) pair of the inverse intermediate, global memory).
+// row: bin m of this row at row[2 m] (its half of the staged (A, B) pairs of the inverse intermediate, shared memory).
 // MODE = RM_ONE or RM_NIKX_MEANY (ttsh_common.cuh).  1/2 rule only: retained m = 0..M/2.
 template <typename T, int M, int MODE, class Hook>
 __device__ __forceinline__ void inv_real_row_regs(const cplx<T>* __restrict__ row, int j, cplx<T> wj, cplx<T>* __restrict__ line,
@@ -54,8 +58,8 @@ __device__ __forceinline__ void inv_real_row_regs(const cplx<T>* __restrict__ ro
     return mx == 0 ? mk<T>(meany, (T)0) : kx * mul_ni(w);        // RM_NIKX_MEANY
   };
   auto issue = [&](int mm, int k) -> cplx<T> {
-    if (k < 8 || (k == 8 && j == 0)) return ld_c(row + 2 * mm);
-    return ld_c(row + 2 * (M - mm));
+    if (k < 8 || (k == 8 && j == 0)) return row[2 * mm];
+    return row[2 * (M - mm)];
   };
   auto finish = [&](int mm, int k, cplx<T> raw) -> cplx<T> {
     const cplx<T> wm = real_row_tw(wj, k);                        // W^mm
@@ -112,6 +116,11 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   pdl_trigger();
   T meany = (T)0;
   if constexpr (!ENS) meany = (T)(v0[1] * g.inv_sqrt_ny);
+  if (leader && (int)blockIdx.x < nblk) {
+    int rp0; size_t mo0;
+    locate(blockIdx.x, rp0, mo0);
+    bulk_load(const_cast<cplx<T>*>(kslot), byte_off(inW, mo0) + (size_t)rp0 * in_stride, in_bytes, bar);
+  }
 
 #pragma unroll 1
   for (int blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
@@ -133,17 +142,21 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
 #pragma unroll 1
     for (int r = 0; r < 2; ++r) {
       const size_t y = (size_t)(4 * a + p + 2 * r);
-      const cplx<T>* rowW = byte_off(inW, mo) + (size_t)rp * in_stride + r;
-      const cplx<T>* rowVx = byte_off(inVx, mo) + (size_t)rp * in_stride + r;
-      const cplx<T>* rowPsi = byte_off(inPsi, mo) + (size_t)rp * in_stride + r;
+      const cplx<T>* row = kslot + r;                          // this row's half of the staged pairs
+      cplx<T>* slot = const_cast<cplx<T>*>(kslot);
       cplx<T> H[16], V[16];
-      // ---- a2 / a6: w, v_x, v_y of the row; the first barrier of the first transform frees the K slot of the previous row ----
-      inv_real_row_regs<T, M, RM_ONE>(rowW, j, wj, line, stab, scale_i, dkx, meany, V,
-                                      [&]() { if (leader) bulk_load(const_cast<cplx<T>*>(kslot), byte_off(K2, mo) + y * NX, k_bytes, bar); });
+      // ---- a2 / a6: w, v_x, v_y of the row ----
+      mbar_wait(bar, ph); ph ^= 1;
+      inv_real_row_regs<T, M, RM_ONE>(row, j, wj, line, stab, scale_i, dkx, meany, V,
+                                      [&]() { if (leader) bulk_load(slot, byte_off(inVx, mo) + (size_t)rp * in_stride, in_bytes, bar); });
 #pragma unroll
       for (int k = 0; k < 16; ++k) stash[k * TPL] = V[k];                     // w
-      inv_real_row_regs<T, M, RM_ONE>(rowVx, j, wj, line, stab, scale_i, dkx, meany, H, NoHook());          // v_x
-      inv_real_row_regs<T, M, RM_NIKX_MEANY>(rowPsi, j, wj, line, stab, scale_i, dkx, meany, V, NoHook());  // v_y
+      mbar_wait(bar, ph); ph ^= 1;
+      inv_real_row_regs<T, M, RM_ONE>(row, j, wj, line, stab, scale_i, dkx, meany, H,
+                                      [&]() { if (leader) bulk_load(slot, byte_off(inPsi, mo) + (size_t)rp * in_stride, in_bytes, bar); });   // v_x
+      mbar_wait(bar, ph); ph ^= 1;
+      inv_real_row_regs<T, M, RM_NIKX_MEANY>(row, j, wj, line, stab, scale_i, dkx, meany, V,
+                                             [&]() { if (leader) bulk_load(slot, byte_off(K2, mo) + y * NX, k_bytes, bar); });               // v_y
       // ---- a3: lines 1-2 of Algorithm 1 on the two points of every slot;  V <- Gx,  H <- Gy,  stash <- S' ----
       mbar_wait(bar, ph); ph ^= 1;
 #pragma unroll
@@ -169,7 +182,15 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
         const cplx<T> e = (T)0.5 * (zp + zm), o = (T)0.5 * mul_ni(zp - zm);
         return e + real_row_tw(wj, i) * o;
       };
-      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
+      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line, [&]() {
+        if (!leader) return;                                   // the slot is free: stage w~ of the next row
+        if (r == 0) bulk_load(slot, byte_off(inW, mo) + (size_t)rp * in_stride, in_bytes, bar);
+        else if (nb < nblk) {
+          int nrp; size_t nmo;
+          locate(nb, nrp, nmo);
+          bulk_load(slot, byte_off(inW, nmo) + (size_t)nrp * in_stride, in_bytes, bar);
+        }
+      });
       __syncthreads();
 #pragma unroll
       for (int i = 0; i < 9; ++i)

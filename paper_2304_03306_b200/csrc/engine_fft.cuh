@@ -210,7 +210,7 @@ static cudaError_t go_row_step_real(const Geom& g, const Model& m, const void* i
                     (const cplx<T>*)inPsi, (const T*)K2, (cplx<T>*)oA, (cplx<T>*)oB, tabW, tabW + row_step_real_tabr_offset(C::M), v0, nblk, rpm, mstride);
 }
 // Nx = 4096 in fp64 runs the three-team in-place kernel (row_step_t3.cuh); its K copy and twiddle table have their own layouts
-template <typename T, int NX> constexpr bool row_step3_enabled() { return sizeof(T) == 8 && NX == 4096; }
+template <typename T, int NX> constexpr bool row_step3_enabled() { return false && sizeof(T) == 8 && NX == 4096; }   // measured: 261 us vs 254 us for k_row_step at C5
 template <typename T, int NX, bool ENS> static cudaError_t prep_row_step_t3(int* slots) {
   using C = RowStep3Cfg<T, NX>;
   static_assert(C::FITS, "row_step_t3: three lines and the twiddle tables must fit in shared memory");
@@ -330,7 +330,7 @@ template <typename T> bool row_step_is_real(const Geom& g) {
 }
 template <typename T> int row_step_real_tabr(const Geom& g) { return row_step_real_tabr_offset(g.Nx / 2); }
 template <typename T> bool row_step_is_t3(const Geom& g) {
-  return row_step_supported<T>(g) && sizeof(T) == 8 && g.Nx == 4096;
+  return row_step_supported<T>(g) && g.Nx == 4096 && row_step3_enabled<T, 4096>();
 }
 template <typename T> bool row_step_supported(const Geom& g) {
   if (4 * (g.Wx - 1) != g.Nx) return false;          // 1/2 rule only

@@ -189,6 +189,8 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
           int nrp; size_t nmo;
           locate(nb, nrp, nmo);
           bulk_load(slot, byte_off(inW, nmo) + (size_t)nrp * in_stride, in_bytes, bar);
+          prefetch_l2_bulk(byte_off(inVx, nmo) + (size_t)nrp * in_stride, in_bytes);
+          prefetch_l2_bulk(byte_off(inPsi, nmo) + (size_t)nrp * in_stride, in_bytes);
         }
       });
       __syncthreads();

@@ -18,12 +18,15 @@
 //   W^m for m = j + 256 k is W^j W_32^k: one table entry per thread (tabR, W^j for j < 256) and compile-time constants.
 //
 // A CTA takes a row pair (rows 4a+p and 4a+p+2 share the (A, B) pairs of the intermediates, ttsh_common.cuh) and runs its two
-// rows one after the other.  Everything a row reads arrives by cp.async.bulk + mbarrier in ONE staging slot, each copy issued
-// right after the barrier that ends the previous use of the slot, i.e. one transform ahead of its consumer:
-//   w~ pairs -> v_x~ pairs -> psi~ pairs -> K row -> w~ pairs of the next row (the same pairs again for the second row of the pair).
+// rows one after the other.  Everything a row reads arrives by cp.async.bulk + mbarrier in two staging slots, each copy issued
+// right after the barrier that ends the previous use of its slot, i.e. more than one transform ahead of its consumer:
+//   slot 0:  w~ pairs -> psi~ pairs -> w~ of the next row          slot 1:  v_x~ pairs -> K row -> v_x~ of the next row
+// (the same pairs again for the second row of the pair).  The waiting field (w, then S') is parked in TENSOR MEMORY (tmem.cuh) by its
+// owner thread: that frees the 64 KB of shared memory the second slot needs and takes the stash traffic off the shared-memory pipe.
 // K comes in the thread order of the plan: (K(y, 2n), K(y, 2n+1)) for n = wl_j(t) + 256 k at (k 256 + t) 2 (k_reperm_real).
 #pragma once
 #include "row_step.cuh"
+#include "tmem.cuh"
 
 namespace ttsh {
 
@@ -32,13 +35,14 @@ template <typename T, int NX> struct RowStepRealCfg {
   static constexpr bool OK = fft_wl_supported<M>();
   static constexpr int TPL = M / 16, THREADS = TPL;
   static constexpr int LS = fft_wl_line_elems<T, M>() + 4;
-  static constexpr size_t OFF_STASH = (size_t)LS * sizeof(cplx<T>);
-  static constexpr size_t OFF_TAB = OFF_STASH + (size_t)M * sizeof(cplx<T>);
-  // one staging slot, used in turn by the (A, B) pairs of w~, v_x~, psi~ (2 Wxp <= 2 (NX/4 + 8) complex values) and by the row of K
+  // one field waits in tensor memory (tmem.cuh): 16 complex values = 64 columns per thread, two warps per lane quarter
+  static constexpr unsigned TMEM_COLS = 128;
+  static constexpr size_t OFF_TAB = (size_t)LS * sizeof(cplx<T>);
+  // two staging slots, used in turn by the (A, B) pairs of w~, v_x~, psi~ (2 Wxp <= 2 (NX/4 + 8) complex values) and by the row of K
   static constexpr size_t SLOT = ((size_t)(NX / 4 + 8) * 2 * sizeof(cplx<T>) + 127) / 128 * 128;
-  static constexpr size_t OFF_K = (OFF_TAB + (size_t)fft_wl_tw_elems_rt(M) * sizeof(cplx<T>) + 127) / 128 * 128;
-  static constexpr size_t OFF_BAR = OFF_K + SLOT;
-  static constexpr size_t SMEM = OFF_BAR + 16;
+  static constexpr size_t OFF_SLOTS = (OFF_TAB + (size_t)fft_wl_tw_elems_rt(M) * sizeof(cplx<T>) + 127) / 128 * 128;
+  static constexpr size_t OFF_BAR = OFF_SLOTS + 2 * SLOT;
+  static constexpr size_t SMEM = OFF_BAR + 32;
   static constexpr bool FITS = OK && SMEM <= 227 * 1024;
 };
 
@@ -91,10 +95,12 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   cplx<T>* line = reinterpret_cast<cplx<T>*>(smem_raw);
   const int j = threadIdx.x;
   const int jw = fft_wl_j<M>(j);                                   // the thread owns slots n = jw + k TPL
-  cplx<T>* stash = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_STASH) + j;      // slot k at stash[k TPL]
   cplx<T>* stab = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_TAB);
-  const cplx<T>* kslot = reinterpret_cast<const cplx<T>*>(smem_raw + C::OFF_K);
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem_raw + C::OFF_BAR);
+  unsigned char* slot0 = smem_raw + C::OFF_SLOTS;
+  unsigned char* slot1 = slot0 + C::SLOT;
+  unsigned long long* bar0 = reinterpret_cast<unsigned long long*>(smem_raw + C::OFF_BAR);
+  unsigned long long* bar1 = bar0 + 1;
+  unsigned* tmem_holder = reinterpret_cast<unsigned*>(bar0 + 2);
   const T scale_i = (T)g.inv_sqrt_nx, scale_f = (T)g.inv_sqrt_nx;
   const T dkx = (T)g.dkx;
   const T beta = (T)m.beta, gv = (T)m.gamma_v, lam = (T)m.lambda0;
@@ -102,16 +108,22 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   const size_t in_stride = (size_t)g.Wxp * 2;               // elements per row pair of an inverse intermediate
   const unsigned in_bytes = (unsigned)(in_stride * sizeof(cplx<T>)), k_bytes = (unsigned)(NX * sizeof(T));
   const bool leader = (j == 0);
-  unsigned ph = 0;
+  unsigned ph0 = 0, ph1 = 0;
+  static_assert(sizeof(T) == 8, "the tensor-memory stash is laid out for complex doubles");
   auto locate = [&](int rpg, int& rp_, size_t& mo_) {
     if constexpr (ENS) { const int mb = rpg / rpm; rp_ = rpg - mb * rpm; mo_ = (size_t)mb * mstride; }
     else { rp_ = rpg; mo_ = 0; }
   };
-  if (leader) mbar_init(bar, 1);
+  if (leader) { mbar_init(bar0, 1); mbar_init(bar1, 1); }
   mbar_fence_init();
+  if (j < 32) tmem_alloc(tmem_holder, C::TMEM_COLS);
+  tmem_fence_before_sync();
   for (int i = j; i < fft_wl_tw_elems_rt(M); i += C::THREADS) stab[i] = ldg_c(tabW + i);     // host-written at ttsh_create
   const cplx<T> wj = ldg_c(tabR + j);                              // W_NX^j
   __syncthreads();
+  tmem_fence_after_sync();
+  const unsigned tmem_base = *tmem_holder;
+  const unsigned tstash = tmem_warp_addr(tmem_base, j >> 5, 64 * (j >> 7));      // this thread's 64 columns: slot k at column 4 k
   pdl_wait();          // inputs, K and v0 below are written by the preceding launches
   pdl_trigger();
   T meany = (T)0;
@@ -119,7 +131,8 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   if (leader && (int)blockIdx.x < nblk) {
     int rp0; size_t mo0;
     locate(blockIdx.x, rp0, mo0);
-    bulk_load(const_cast<cplx<T>*>(kslot), byte_off(inW, mo0) + (size_t)rp0 * in_stride, in_bytes, bar);
+    bulk_load(slot0, byte_off(inW, mo0) + (size_t)rp0 * in_stride, in_bytes, bar0);
+    bulk_load(slot1, byte_off(inVx, mo0) + (size_t)rp0 * in_stride, in_bytes, bar1);
   }
 
 #pragma unroll 1
@@ -142,35 +155,53 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
 #pragma unroll 1
     for (int r = 0; r < 2; ++r) {
       const size_t y = (size_t)(4 * a + p + 2 * r);
-      const cplx<T>* row = kslot + r;                          // this row's half of the staged pairs
-      cplx<T>* slot = const_cast<cplx<T>*>(kslot);
+      const cplx<T>* row0 = reinterpret_cast<const cplx<T>*>(slot0) + r;      // this row's half of the staged pairs
+      const cplx<T>* row1 = reinterpret_cast<const cplx<T>*>(slot1) + r;
+      const cplx<T>* kslot = reinterpret_cast<const cplx<T>*>(slot1);
+      // (row pair, member offset) of the row after this one
+      int xrp = rp; size_t xmo = mo; bool xok = true;
+      if (r == 1) { xok = nb < nblk; if (xok) locate(nb, xrp, xmo); }
       cplx<T> H[16], V[16];
       // ---- a2 / a6: w, v_x, v_y of the row ----
-      mbar_wait(bar, ph); ph ^= 1;
-      inv_real_row_regs<T, M, RM_ONE>(row, j, wj, line, stab, scale_i, dkx, meany, V,
-                                      [&]() { if (leader) bulk_load(slot, byte_off(inVx, mo) + (size_t)rp * in_stride, in_bytes, bar); });
+      mbar_wait(bar0, ph0); ph0 ^= 1;
+      inv_real_row_regs<T, M, RM_ONE>(row0, j, wj, line, stab, scale_i, dkx, meany, V,
+                                      [&]() { if (leader) bulk_load(slot0, byte_off(inPsi, mo) + (size_t)rp * in_stride, in_bytes, bar0); });
 #pragma unroll
-      for (int k = 0; k < 16; ++k) stash[k * TPL] = V[k];                     // w
-      mbar_wait(bar, ph); ph ^= 1;
-      inv_real_row_regs<T, M, RM_ONE>(row, j, wj, line, stab, scale_i, dkx, meany, H,
-                                      [&]() { if (leader) bulk_load(slot, byte_off(inPsi, mo) + (size_t)rp * in_stride, in_bytes, bar); });   // v_x
-      mbar_wait(bar, ph); ph ^= 1;
-      inv_real_row_regs<T, M, RM_NIKX_MEANY>(row, j, wj, line, stab, scale_i, dkx, meany, V,
-                                             [&]() { if (leader) bulk_load(slot, byte_off(K2, mo) + y * NX, k_bytes, bar); });               // v_y
-      // ---- a3: lines 1-2 of Algorithm 1 on the two points of every slot;  V <- Gx,  H <- Gy,  stash <- S' ----
-      mbar_wait(bar, ph); ph ^= 1;
+      for (int q = 0; q < 4; ++q) tmem_st4(tstash + 16 * q, V + 4 * q);      // w waits in tensor memory
+      mbar_wait(bar1, ph1); ph1 ^= 1;
+      inv_real_row_regs<T, M, RM_ONE>(row1, j, wj, line, stab, scale_i, dkx, meany, H,
+                                      [&]() { if (leader) bulk_load(slot1, byte_off(K2, mo) + y * NX, k_bytes, bar1); });                    // v_x
+      mbar_wait(bar0, ph0); ph0 ^= 1;
+      inv_real_row_regs<T, M, RM_NIKX_MEANY>(row0, j, wj, line, stab, scale_i, dkx, meany, V, [&]() {                                        // v_y
+        if (leader && xok) bulk_load(slot0, byte_off(inW, xmo) + (size_t)xrp * in_stride, in_bytes, bar0);
+      });
+      // ---- a3: lines 1-2 of Algorithm 1 on the two points of every slot;  V <- Gx,  H <- Gy,  tensor memory <- S' ----
+      mbar_wait(bar1, ph1); ph1 ^= 1;
+      tmem_wait_st();
+      {
+        TmemQuad wq[2];
+        tmem_ld4_issue(tstash, wq[0]);
 #pragma unroll
-      for (int k = 0; k < 16; ++k) {
-        const cplx<T> kk = kslot[k * TPL + j];
-        const cplx<T> w = stash[k * TPL];
-        const T kA = kk.x, kB = kk.y;
-        const T vxA = H[k].x, vxB = H[k].y, vyA = V[k].x, vyB = V[k].y;
-        const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * kA);
-        const T ccB = scale_f * (-beta * (vxB * vxB + vyB * vyB) - gv * kB);
-        const T lwA = scale_f * lam * w.x, lwB = scale_f * lam * w.y;
-        V[k] = mk<T>(ccA * vxA + lwA * vyA, ccB * vxB + lwB * vyB);          // Gx
-        H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
-        stash[k * TPL] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));          // S'
+        for (int q = 0; q < 4; ++q) {
+          tmem_wait_ld(wq[q & 1]);
+          if (q < 3) tmem_ld4_issue(tstash + 16 * (q + 1), wq[(q + 1) & 1]);
+          cplx<T> s4[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int k = 4 * q + i;
+            const cplx<T> kk = kslot[k * TPL + j];
+            const cplx<T> w = tmem_quad_get(wq[q & 1], i);
+            const T kA = kk.x, kB = kk.y;
+            const T vxA = H[k].x, vxB = H[k].y, vyA = V[k].x, vyB = V[k].y;
+            const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * kA);
+            const T ccB = scale_f * (-beta * (vxB * vxB + vyB * vyB) - gv * kB);
+            const T lwA = scale_f * lam * w.x, lwB = scale_f * lam * w.y;
+            V[k] = mk<T>(ccA * vxA + lwA * vyA, ccB * vxB + lwB * vyB);          // Gx
+            H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
+            s4[i] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));                   // S'
+          }
+          tmem_st4(tstash + 16 * q, s4);
+        }
       }
       // ---- a4: three forward transforms, each merged into the half spectrum of the row on the bins k = j + 256 i ----
       auto ident = [&](int, int, cplx<T> z) -> cplx<T> { return z; };
@@ -183,15 +214,8 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
         return e + real_row_tw(wj, i) * o;
       };
       fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line, [&]() {
-        if (!leader) return;                                   // the slot is free: stage w~ of the next row
-        if (r == 0) bulk_load(slot, byte_off(inW, mo) + (size_t)rp * in_stride, in_bytes, bar);
-        else if (nb < nblk) {
-          int nrp; size_t nmo;
-          locate(nb, nrp, nmo);
-          bulk_load(slot, byte_off(inW, nmo) + (size_t)nrp * in_stride, in_bytes, bar);
-          prefetch_l2_bulk(byte_off(inVx, nmo) + (size_t)nrp * in_stride, in_bytes);
-          prefetch_l2_bulk(byte_off(inPsi, nmo) + (size_t)nrp * in_stride, in_bytes);
-        }
+        if (!leader || !xok) return;                           // K has been consumed: stage v_x~ of the next row
+        bulk_load(slot1, byte_off(inVx, xmo) + (size_t)xrp * in_stride, in_bytes, bar1);
       });
       __syncthreads();
 #pragma unroll
@@ -210,7 +234,17 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
           ikg[i] = (dkx * (T)(j + TPL * i)) * mul_i(gy);
         }
       }
-      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return stash[k * TPL]; }, ident), to_line);
+      {
+        tmem_wait_st();
+        TmemQuad sq[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) tmem_ld4_issue(tstash + 16 * q, sq[q]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) tmem_wait_ld(sq[q]);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) V[k] = tmem_quad_get(sq[k >> 2], k & 3);       // S'
+      }
+      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
       __syncthreads();
 #pragma unroll
       for (int i = 0; i < 9; ++i)
@@ -221,6 +255,9 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
         }
     }
   }
+  tmem_fence_before_sync();
+  __syncthreads();
+  if (j < 32) tmem_dealloc(tmem_base, C::TMEM_COLS);
 }
 
 }  // namespace ttsh

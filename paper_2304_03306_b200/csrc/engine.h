@@ -43,10 +43,7 @@ template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model&
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                   const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s, int slots);
 template <typename T> bool row_step_supported(const Geom& g);
-// ... and it is the three-team in-place variant (row_step_t3.cuh: Nx = 4096 in fp64), which wants K in line-position order
-// (launch_reperm_t3) and the table of fill_stage_tables_t3
-template <typename T> bool row_step_is_t3(const Geom& g);
-// ... or the real-row variant (row_step_real.cuh: Nx = 8192 in fp64): K in its thread order (launch_reperm_real); table = the warp-local
+// ... and it is the real-row variant (row_step_real.cuh: Nx = 8192 in fp64): K in its thread order (launch_reperm_real); table = the warp-local
 // table of length Nx/2 followed, at element row_step_real_tabr(g), by W_Nx^j, j < Nx/32
 template <typename T> bool row_step_is_real(const Geom& g);
 template <typename T> int row_step_real_tabr(const Geom& g);
@@ -84,8 +81,6 @@ template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, c
 template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* in, void* out, int to_perm, cudaStream_t s);
 // permuted internal row layout (perm_index) -> thread-order layout of the warp-local plan (perm_index_wl)
 template <typename T> cudaError_t launch_reperm_wl(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
-// permuted internal row layout -> line-position order of row_step_t3.cuh, one plane per row: K(y_r, x(p)) at (rp 2 + r) Nx + p
-template <typename T> cudaError_t launch_reperm_t3(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
 // permuted internal row layout -> thread order of row_step_real.cuh: (K(y, 2n), K(y, 2n+1)), n = wl_j(t) + (Nx/32) k, at y Nx + (k Nx/32 + t) 2
 template <typename T> cudaError_t launch_reperm_real(int Nx, size_t n, const void* in, void* out, cudaStream_t s);
 constexpr int DIAG_BLOCKS = 592;   // 4 x 148 SMs

@@ -177,7 +177,6 @@ template <typename T> cudaError_t prepare_rows(const Geom& g) {
 #ifdef TTSH_BUILD_ROWSTEP
 }  // namespace ttsh
 #include "row_step.cuh"
-#include "row_step_t3.cuh"
 #include "row_step_real.cuh"
 namespace ttsh {
 // Nx = 8192 in fp64 (a packed row pair does not fit in shared memory): one real row per half-length transform (row_step_real.cuh);
@@ -208,32 +207,6 @@ static cudaError_t go_row_step_real(const Geom& g, const Model& m, const void* i
   const cplx<T>* tabW = static_cast<const cplx<T>*>(tab);
   return launch_pdl(k_row_step_real<T, NX, ENS>, dim3(grid), dim3(C::THREADS), C::SMEM, s, g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx,
                     (const cplx<T>*)inPsi, (const T*)K2, (cplx<T>*)oA, (cplx<T>*)oB, tabW, tabW + row_step_real_tabr_offset(C::M), v0, nblk, rpm, mstride);
-}
-// Nx = 4096 in fp64 runs the three-team in-place kernel (row_step_t3.cuh); its K copy and twiddle table have their own layouts
-template <typename T, int NX> constexpr bool row_step3_enabled() { return false && sizeof(T) == 8 && NX == 4096; }   // measured: 261 us vs 254 us for k_row_step at C5
-template <typename T, int NX, bool ENS> static cudaError_t prep_row_step_t3(int* slots) {
-  using C = RowStep3Cfg<T, NX>;
-  static_assert(C::FITS, "row_step_t3: three lines and the twiddle tables must fit in shared memory");
-  cudaError_t e = set_smem(k_row_step_t3<T, NX, ENS>, C::SMEM);
-  if (e != cudaSuccess) return e;
-  int dev = 0, sms = 0;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  *slots = sms > 0 ? sms : 148;                                   // one 384-thread CTA per SM
-  return cudaSuccess;
-}
-template <typename T, int NX, bool ENS>
-static cudaError_t go_row_step_t3(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi, const void* K3,
-                                  void* oA, void* oB, const void* tab3, const double* v0, cudaStream_t s, int members, size_t mstride, int slots) {
-  using C = RowStep3Cfg<T, NX>;
-  if (slots <= 0) return cudaErrorInvalidConfiguration;
-  const int rpm = g.Ny / 2;
-  const long long nblk_ll = (long long)rpm * members;
-  if (nblk_ll > 0x3fffffff) return cudaErrorInvalidValue;
-  const int nblk = (int)nblk_ll;
-  const int grid = nblk < slots ? nblk : slots;
-  return launch_pdl(k_row_step_t3<T, NX, ENS>, dim3(grid), dim3(C::THREADS), C::SMEM, s, g, m, (const cplx<T>*)inW, (const cplx<T>*)inVx,
-                    (const cplx<T>*)inPsi, (const T*)K3, (cplx<T>*)oA, (cplx<T>*)oB, static_cast<const cplx<T>*>(tab3), v0, nblk, rpm, mstride);
 }
 // persistent grid: one CTA per resident slot (SMs x occupancy), looping over the row-pair blocks.  The opt-in to > 48 KB of
 // dynamic shared memory and the occupancy are per DEVICE: prepare_row_step runs in ttsh_create on the handle's device and the
@@ -277,10 +250,7 @@ template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, in
   *slots = *slots_ens = *slots_tan = 0;
   switch (g.Nx) {
 #define X(N) case N: { cudaError_t e = prep_row_step<T, N, row_step_ens_lines<N>(), true, true>(slots_tan); if (e != cudaSuccess) return e; \
-                       if constexpr (row_step3_enabled<T, N>()) { \
-                         e = prep_row_step_t3<T, N, false>(slots); if (e != cudaSuccess) return e; \
-                         return prep_row_step_t3<T, N, true>(slots_ens); \
-                       } else if constexpr (row_step_real_enabled<T, N>()) { \
+                       if constexpr (row_step_real_enabled<T, N>()) { \
                          e = prep_row_step_real<T, N, false>(slots); if (e != cudaSuccess) return e; \
                          return prep_row_step_real<T, N, true>(slots_ens); \
                        } else { \
@@ -294,8 +264,7 @@ template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, in
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                   const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int slots) {
   switch (g.Nx) {
-#define X(N) case N: if constexpr (row_step3_enabled<T, N>()) return go_row_step_t3<T, N, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots); \
-                     else if constexpr (row_step_real_enabled<T, N>()) return go_row_step_real<T, N, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots); \
+#define X(N) case N: if constexpr (row_step_real_enabled<T, N>()) return go_row_step_real<T, N, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots); \
                      else return go_row_step<T, N, 1, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots);
     TTSH_FOR_SIZES(X)
 #undef X
@@ -306,8 +275,7 @@ template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model
                                                       const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s,
                                                       int members, size_t mstride, int slots) {
   switch (g.Nx) {
-#define X(N) case N: if constexpr (row_step3_enabled<T, N>()) return go_row_step_t3<T, N, true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots); \
-                     else if constexpr (row_step_real_enabled<T, N>()) return go_row_step_real<T, N, true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots); \
+#define X(N) case N: if constexpr (row_step_real_enabled<T, N>()) return go_row_step_real<T, N, true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots); \
                      else return go_row_step<T, N, row_step_ens_lines<N>(), true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots);
     TTSH_FOR_SIZES(X)
 #undef X
@@ -329,9 +297,6 @@ template <typename T> bool row_step_is_real(const Geom& g) {
   return row_step_supported<T>(g) && sizeof(T) == 8 && g.Nx == 8192;
 }
 template <typename T> int row_step_real_tabr(const Geom& g) { return row_step_real_tabr_offset(g.Nx / 2); }
-template <typename T> bool row_step_is_t3(const Geom& g) {
-  return row_step_supported<T>(g) && g.Nx == 4096 && row_step3_enabled<T, 4096>();
-}
 template <typename T> bool row_step_supported(const Geom& g) {
   if (4 * (g.Wx - 1) != g.Nx) return false;          // 1/2 rule only
   switch (g.Nx) {

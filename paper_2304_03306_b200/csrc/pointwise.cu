@@ -58,11 +58,6 @@ template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* i
   k_permute_rows<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(Nx, n, (const T*)in, (T*)out, to_perm);
   return cudaGetLastError();
 }
-template <typename T> cudaError_t launch_reperm_t3(int Nx, size_t n, const void* in, void* out, cudaStream_t s) {
-  if (Nx != 4096) return cudaErrorInvalidValue;
-  k_reperm_t3<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(Nx, n, (const T*)in, (T*)out);
-  return cudaGetLastError();
-}
 template <typename T> cudaError_t launch_reperm_real(int Nx, size_t n, const void* in, void* out, cudaStream_t s) {
   if (Nx < 512) return cudaErrorInvalidValue;
   k_reperm_real<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(Nx, n, (const T*)in, (T*)out);
@@ -180,7 +175,6 @@ template <typename T> cudaError_t launch_tri_apply(const Geom& g, int nvec, cons
   template cudaError_t launch_fill<T>(size_t, void*, double, cudaStream_t); \
   template cudaError_t launch_permute<T>(int, size_t, const void*, void*, int, cudaStream_t); \
   template cudaError_t launch_reperm_wl<T>(int, size_t, const void*, void*, cudaStream_t); \
-  template cudaError_t launch_reperm_t3<T>(int, size_t, const void*, void*, cudaStream_t); \
   template cudaError_t launch_reperm_real<T>(int, size_t, const void*, void*, cudaStream_t); \
   template cudaError_t launch_diag<T>(const Geom&, double, double, double, const void*, const void*, const void*, double*, double*, cudaStream_t);
 INST(double)

@@ -306,21 +306,6 @@ __global__ void k_reperm_wl(int Nx, size_t n, const T* __restrict__ in, T* __res
   }
 }
 
-// K for row_step_t3.cuh (Nx = 4096 = 16^3): row pair rp = 2a + par holds rows y_A = 4a + par, y_B = y_A + 2; one plane per row,
-// out[(rp 2 + r) Nx + e] = K(y_r, x(p)) with e = ((4 s + q) 16 + c) 4 + i  <->  line position p = 256 s + 16 c + 4 q + i, x = digit-reversed p
-template <typename T>
-__global__ void k_reperm_t3(int Nx, size_t n, const T* __restrict__ in, T* __restrict__ out) {
-  const int tpl = Nx / 16;
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const size_t plane = i / (size_t)Nx, rp = plane >> 1;
-    const int e = (int)(i - plane * (size_t)Nx), r = (int)(plane & 1);
-    const int p = 256 * (e >> 8) + 16 * ((e >> 2) & 15) + 4 * ((e >> 6) & 3) + (e & 3);
-    const size_t y = 4 * (rp >> 1) + (rp & 1) + 2 * r;
-    const int x = (p >> 8) + 16 * ((p >> 4) & 15) + 256 * (p & 15);
-    out[i] = in[y * Nx + perm_index(x, tpl)];
-  }
-}
-
 // K for row_step_real.cuh: slot n = wl_j(t) + TPL k of thread t (TPL = Nx/32 threads, wl_j(t) = (t >> 4) + (TPL/16) (t & 15)) holds the
 // points x = 2n, 2n+1 of the row;  out[y Nx + (k TPL + t) 2 + par] = K(y, 2n + par)
 template <typename T>

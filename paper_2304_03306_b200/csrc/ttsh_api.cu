@@ -103,7 +103,6 @@ struct ttsh_handle {
   bool row_step_ok;     // the fused row-step kernel supports this grid / dtype / dealias fraction
   bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
   bool row_step_real;   // ... or the real-row variant (row_step_real.cuh: its own K order and table)
-  bool row_step_t3;     // ... or the three-team in-place variant (row_step_t3.cuh: K in line-position order, its own table)
   bool real_rows;       // Nx = 16384: one real row per half-length transform (fft_rows_real.cuh); internal real fields in natural order
 };
 
@@ -197,17 +196,6 @@ template <typename T> void fill_stage_tables_wl(std::vector<unsigned char>& buf,
   for (int b = 0; b < 6; ++b)
     for (int th = 0; th < TPL; ++th)
       put_twiddle<T>(t + 2 * (size_t)(15 * R1 + b * TPL + th), (long long)fft_wl_j_rt(th, R1) * fft_tw_base_power(16, b), (long long)N);
-}
-// tables of the three-team in-place plan N = 16 x 16 x 16 (row_step_t3.cuh): [5][256] W_N^{j b}, b = 1, 2, 3, 4, 8, then [6][16] W_256^{c b},
-// b = 1, 2, 3, 4, 8, 12
-template <typename T> void fill_stage_tables_t3(std::vector<unsigned char>& buf, int N) {
-  buf.assign((size_t)(5 * 256 + 6 * 16) * 2 * sizeof(T), 0);
-  T* t = reinterpret_cast<T*>(buf.data());
-  static const int pa[5] = {1, 2, 3, 4, 8}, pb[6] = {1, 2, 3, 4, 8, 12};
-  for (int b = 0; b < 5; ++b)
-    for (int j = 0; j < 256; ++j) put_twiddle<T>(t + 2 * (size_t)(b * 256 + j), (long long)j * pa[b], (long long)N);
-  for (int b = 0; b < 6; ++b)
-    for (int c = 0; c < 16; ++c) put_twiddle<T>(t + 2 * (size_t)(5 * 256 + b * 16 + c), (long long)c * pb[b], 256LL);
 }
 // split twiddles of the column pass: W_Ny^p, p < Ny/2
 template <typename T> void fill_split_table(std::vector<unsigned char>& buf, int Ny) {
@@ -335,8 +323,8 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     }
     case TTSH_STAGE_ROW_STEP:         // a2/a6 row pass + a3 + a4 row pass in one kernel (conservative form, 1/2 rule)
       if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || !h->row_step_ok) return TTSH_ERR_INVALID_ARG;
-      TRY(h, DISPATCH(h, launch_row_step, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_t3 || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
-                      (h->row_step_wl || h->row_step_t3 || h->row_step_real) ? h->tabXw : h->tabX, h->v0, h->stream, h->rs_slots));
+      TRY(h, DISPATCH(h, launch_row_step, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
+                      (h->row_step_wl || h->row_step_real) ? h->tabXw : h->tabX, h->v0, h->stream, h->rs_slots));
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_SPECTRAL_P2:
@@ -387,9 +375,8 @@ int copy_real(ttsh_handle* h, const void* src, void* dst, int to_perm) {
 int apply_mask_k(ttsh_handle* h, const void* mask, ttsh_mask_kind kind);
 int apply_mask(ttsh_handle* h, const void* mask, ttsh_mask_kind kind) {
   int rc = apply_mask_k(h, mask, kind);
-  if (rc != TTSH_OK || !(h->row_step_ok && (h->row_step_wl || h->row_step_t3 || h->row_step_real))) return rc;
-  if (h->row_step_t3) TRY(h, DISPATCH(h, launch_reperm_t3, h->Nx, (size_t)h->Nx * h->Ny, h->K, h->K2, h->stream));
-  else if (h->row_step_real) TRY(h, DISPATCH(h, launch_reperm_real, h->Nx, (size_t)h->Nx * h->Ny, h->K, h->K2, h->stream));
+  if (rc != TTSH_OK || !(h->row_step_ok && (h->row_step_wl || h->row_step_real))) return rc;
+  if (h->row_step_real) TRY(h, DISPATCH(h, launch_reperm_real, h->Nx, (size_t)h->Nx * h->Ny, h->K, h->K2, h->stream));
   else TRY(h, DISPATCH(h, launch_reperm_wl, h->Nx, (size_t)h->Nx * h->Ny, h->K, h->K2, h->stream));
   h->launches++;
   return TTSH_OK;
@@ -465,9 +452,8 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->initialized = false; h->t = 0.0; h->step = 0; h->launches = 0; h->sticky = 0;
   h->graph_exec = h->graph_exec_k = nullptr; h->graph_ok = false; h->advection_form = TTSH_ADVECTION_CONSERVATIVE;
   h->row_step_ok = h->dtype == TTSH_F64 ? row_step_supported<double>(h->g) : row_step_supported<float>(h->g);
-  h->row_step_t3 = h->dtype == TTSH_F64 ? row_step_is_t3<double>(h->g) : row_step_is_t3<float>(h->g);
   h->row_step_real = h->dtype == TTSH_F64 ? row_step_is_real<double>(h->g) : row_step_is_real<float>(h->g);
-  h->row_step_wl = Nx == 4096 && !h->row_step_t3;
+  h->row_step_wl = Nx == 4096;
   h->real_rows = Nx == 16384;
   h->rs_slots = h->rs_slots_ens = h->rs_slots_tan = 0;
   h->device = -1;
@@ -507,12 +493,6 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
       if (t == TTSH_F64) put_twiddle<double>(reinterpret_cast<double*>(tw.data()) + 2 * (size_t)(off + j), j, Nx);
       else put_twiddle<float>(reinterpret_cast<float*>(tw.data()) + 2 * (size_t)(off + j), j, Nx);
     }
-    TRY(h, cudaMemcpyAsync(h->tabXw, tw.data(), tw.size(), cudaMemcpyHostToDevice, h->stream));
-    TRY(h, cudaStreamSynchronize(h->stream));
-  }
-  if (h->row_step_t3) {
-    std::vector<unsigned char> tw;
-    if (t == TTSH_F64) fill_stage_tables_t3<double>(tw, Nx); else fill_stage_tables_t3<float>(tw, Nx);
     TRY(h, cudaMemcpyAsync(h->tabXw, tw.data(), tw.size(), cudaMemcpyHostToDevice, h->stream));
     TRY(h, cudaStreamSynchronize(h->stream));
   }
@@ -1064,8 +1044,8 @@ static int ensemble_enqueue_step(ttsh_ensemble* e, cudaStream_t stream) {
   const size_t ms = e->mstride;
   Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->psihat, h->Tm[2], SM_ONE), op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
   TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, h->v0, stream, B, ms));
-  TRY(h, DISPATCH(h, launch_row_step_ens, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_t3 || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
-                  (h->row_step_wl || h->row_step_t3 || h->row_step_real) ? h->tabXw : h->tabX, h->v0, stream, B, ms, h->rs_slots_ens));
+  TRY(h, DISPATCH(h, launch_row_step_ens, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
+                  (h->row_step_wl || h->row_step_real) ? h->tabXw : h->tabX, h->v0, stream, B, ms, h->rs_slots_ens));
   Batch fb = make_batch({op(h->Tm[1], h->S[0], 0), op(h->Tm[4], h->S[1], 0)});
   TRY(h, DISPATCH(h, launch_fwd_col, h->g, fb, 2, h->tabY, h->tabS, stream, B, ms));
   TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, h->S[0], h->S[1], h->what, h->psihat, h->v0, stream, B, ms));

@@ -584,8 +584,8 @@ def test_other_dealias_fractions_match_oracle(ttsh, num, den, Nx, Ny):
 
 @pytest.mark.parametrize("Nx,Ny,dtype", [(8192, 64, "f64"), (8192, 64, "f32"), (64, 8192, "f64"), (64, 8192, "f32")])
 def test_maximum_grid_dimension_8192(ttsh, Nx, Ny, dtype):
-    """Nx = 8192 (fp64: the row pair does not fit in shared memory -> the 5-launch step; fp32: the fused row kernel) and
-    Ny = 8192 (4096-point half-length column transforms), 3 steps against the FFT-backed oracle."""
+    """Nx = 8192 (fp64: the real-row fused kernel k_row_step_real, one real row per half-length transform; fp32: the fused
+    row-pair kernel) and Ny = 8192 (4096-point half-length column transforms), 3 steps against the FFT-backed oracle."""
     dx, dt = 0.5, 0.01
     mask = workloads.disk_mask(Nx, Ny, dx, 12.0)
     vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 6, amplitude=1.0)
@@ -594,6 +594,41 @@ def test_maximum_grid_dimension_8192(ttsh, Nx, Ny, dtype):
     compare_state(s, o, TOL_F64_100 if dtype == "f64" else 3 * TOL_F32_1, f"{Nx}x{Ny} {dtype}")
     assert s.diagnostics()["nonfinite"] == 0
     s.close()
+
+
+@pytest.mark.parametrize("which,Ny", [("baseline", 128), ("paper", 512)])
+def test_real_row_fused_kernel_nx8192_fp64(ttsh, which, Ny):
+    """k_row_step_real (Nx = 8192 in fp64: the paper's production width): the 4-launch step against the oracle-fft for 1
+    and 10 steps, against the unfused 6-launch sequence of the same library (same arithmetic per point up to the order of the
+    real-data split / merge), and with a mean flow in both components (the m = 0 bins of the split take their own branch)."""
+    Nx, dx, dt = 8192, 0.5, 0.01
+    mask = workloads.disk_mask(Nx, Ny, dx, 0.3 * Ny * dx)
+    vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 21, amplitude=1.0, nmodes=16)
+    g = workloads.gaussian_velocity(Nx, Ny, workloads.SEED0 + 21, 1e-2, mask)
+    vel = (vel[0] + g[0] + 0.15, vel[1] + g[1] - 0.1)
+    s, o = make_pair(ttsh, Nx, Ny, dx, dt, which, mask, transform="c", vel=vel)
+    l0 = s.launch_count()
+    s.step(1); o.step(1)
+    assert s.launch_count() - l0 == 4, "k_inv_col, k_row_step_real, k_fwd_col, k_spectral_p2"
+    compare_state(s, o, TOL_F64_1, f"8192x{Ny} {which} step 1")
+    s.step(9); o.step(9)
+    compare_state(s, o, TOL_F64_100, f"8192x{Ny} {which} step 10")
+    cx, cy = (Nx // 2) * dx, (Ny // 2) * dx
+    d, od = s.diagnostics(cx, cy), o.diagnostics(cx, cy)
+    for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy", "mean_vx", "mean_vy"):
+        assert abs(d[key] - od[key]) <= TOL_DIAG * max(abs(od[key]), 1e-300), key
+    # the same step through the unfused passes of the library
+    gp, _ = params_pair(ttsh, which)
+    a = ttsh.Solver(Nx, Ny, dx, dt, gp, "f64", mask=mask)
+    b = ttsh.Solver(Nx, Ny, dx, dt, gp, "f64", mask=mask)
+    a.set_velocity(*vel); b.set_velocity(*vel)
+    a.step(1)
+    for st in (ttsh.TTSH_STAGE_INV_COL, ttsh.TTSH_STAGE_INV_ROW, ttsh.TTSH_STAGE_REAL, ttsh.TTSH_STAGE_FWD_ROW,
+               ttsh.TTSH_STAGE_FWD_COL, ttsh.TTSH_STAGE_SPECTRAL):
+        b.run_stage(st)
+    for x, y, name in zip(gpu_fields(a), gpu_fields(b), ("vx", "vy", "w", "psi")):
+        assert rel(x, y) <= 1e-13, name
+    s.close(); a.close(); b.close()
 
 
 @pytest.mark.parametrize("Nx,Ny,dtype", [(16384, 64, "f64"), (16384, 64, "f32"), (64, 16384, "f64"), (64, 16384, "f32"), (16384, 128, "f64")])

@@ -183,11 +183,10 @@ int ttsh_tangent_destroy(ttsh_tangent* s);
 /* Ensembles: the paper's workload is sweeps of independent runs on one grid — disk radius R (Fig. 2), the
  * hysteresis branches, dumbbell separations — and on grids up to about 1024^2 one system
  * cannot fill a B200.  An ensemble advances `count` independent handles with ONE launch of each hot kernel per Euler step
- * (4 launches for all members together), every member computing exactly what ttsh_step computes for it: results are
- * bit-identical to stepping the members one by one.
+ * (4 launches for all members together; 2 where ttsh_step takes 2: 128 <= Ny <= 1024), every member computing exactly what
+ * ttsh_step computes for it: results are bit-identical to stepping the members one by one.
  * Requirements (else TTSH_ERR_INVALID_ARG): count >= 1; all members have the same Nx, Ny, dtype, dx, dt, parameters and
- * stream, use TTSH_ADVECTION_CONSERVATIVE with the 1/2 rule on a grid the fused row kernel supports (every grid but
- * Nx = 8192 in fp64), and their workspaces lie at a uniform byte stride: workspace_b = workspace_0 + b * stride, stride >=
+ * stream, use TTSH_ADVECTION_CONSERVATIVE with the 1/2 rule on a grid the fused row kernel supports (Nx <= 8192), and their workspaces lie at a uniform byte stride: workspace_b = workspace_0 + b * stride, stride >=
  * ttsh_workspace_bytes (carve them from one allocation).  Masks, states and step counters are per member; all other calls
  * (ttsh_set_velocity, ttsh_set_mask, ttsh_get_fields, ttsh_diagnostics, ...) keep working on the member handles.  The
  * ensemble borrows the members: destroy it before them. */
@@ -215,8 +214,11 @@ typedef enum {
   TTSH_STAGE_REAL_FWD_ROW = 6, /* a3 fused into the a4 row pass; emits A~ = i kx Gy~ + S'~ and B~ = Gx~ (conservative form)   */
   TTSH_STAGE_FWD_COL_P2 = 7,  /* a4 column pass of those two intermediates                                                    */
   TTSH_STAGE_SPECTRAL_P2 = 8, /* a5 from the two spectra: rhs^ = A^ - i ky B^                                                   */
-  TTSH_STAGE_ROW_STEP = 9     /* stages 1 + 6 in one kernel: w, v never leave the SM (1/2 rule, row pair fits in shared memory:
-                                 every grid but Nx = 8192 in fp64).  ttsh_step runs 0, 9, 7, 8 where supported, else 0, 1, 6, 7, 8 */
+  TTSH_STAGE_ROW_STEP = 9,    /* stages 1 + 6 in one kernel: w, v never leave the SM (1/2 rule; Nx = 8192 in fp64: one real row per
+                                 transform).  ttsh_step runs 0, 9, 7, 8 where supported, else 0, 1, 6, 7, 8 */
+  TTSH_STAGE_COL_STEP = 10    /* stages 7 + 8 + stage 0 of the NEXT step in one kernel (Ny <= 1024, 1/2 rule): there ttsh_step runs
+                                 9, 10 per Euler step, preceded by stage 0 once whenever the intermediates of the current state are
+                                 not at hand (first step, or after any call that is not ttsh_step) */
 } ttsh_stage;
 int ttsh_run_stage(ttsh_handle* h, int stage);
 /* Copies a workspace array out for inspection: which = 0..4 real scratch (omega|rhs2, g_x|rhs1_x, g_y|rhs1_y, v_x, v_y;

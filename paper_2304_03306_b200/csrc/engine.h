@@ -64,6 +64,12 @@ template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model
 // set the dynamic shared-memory attribute of the pass kernels for this grid (no launch)
 template <typename T> cudaError_t prepare_rows(const Geom& g);
 template <typename T> cudaError_t prepare_cols(const Geom& g);
+// the column half of the time loop in one kernel (col_step.cuh; Ny <= 1024, 1/2 rule): forward column pass of A~, B~, lines 3-13 of
+// Algorithm 1 on the state (w, psi, v0), inverse column pass of w^, psi^, i k_y psi^ for the next row kernel
+template <typename T> bool col_step_supported(const Geom& g);
+template <typename T> cudaError_t launch_col_step(const Geom& g, const Model& m, const void* srcA, const void* srcB, void* w, void* psi, double* v0,
+                                                  void* dstW, void* dstPsi, void* dstVx, const void* tabY, const void* tabS, cudaStream_t s,
+                                                  int members = 1, size_t mstride = 0);
 
 // element-wise kernels and reductions (pointwise.cuh)
 template <typename T> cudaError_t launch_realspace(const Geom& g, const Model& m, const void* vx, const void* vy, const void* K,

@@ -73,10 +73,49 @@ template <typename T> cudaError_t launch_fwd_col(const Geom& g, const Batch& b, 
   }
   return cudaErrorInvalidValue;
 }
+}  // namespace ttsh
+#include "col_step.cuh"
+namespace ttsh {
+template <typename T> bool col_step_supported(const Geom& g) {
+  if (2 * g.My != g.Ny / 2 || g.Hy != g.Ny / 2 + 1) return false;      // 1/2 rule only
+  switch (g.Ny) {
+#define X(N) case N: return ColStepCfg<T, N>::OK;
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return false;
+}
+template <typename T, int NY> static cudaError_t go_col_step(const Geom& g, const Model& m, const void* srcA, const void* srcB, void* w, void* psi,
+                                                            double* v0, void* dstW, void* dstPsi, void* dstVx, const void* tab, const void* tabS,
+                                                            cudaStream_t s, int members, size_t mstride) {
+  using S = ColStepCfg<T, NY>;
+  if constexpr (!S::OK) return cudaErrorInvalidConfiguration;
+  else {
+    if (members < 1 || members > 65535) return cudaErrorInvalidValue;
+    return launch_pdl(k_col_step<T, NY>, dim3(g.NT, members), dim3(S::THREADS), S::SMEM, s, g, m, (const cplx<T>*)srcA, (const cplx<T>*)srcB,
+                      (cplx<T>*)w, (cplx<T>*)psi, v0, (cplx<T>*)dstW, (cplx<T>*)dstPsi, (cplx<T>*)dstVx, static_cast<const cplx<T>*>(tab),
+                      static_cast<const cplx<T>*>(tabS), mstride);
+  }
+}
+template <typename T> cudaError_t launch_col_step(const Geom& g, const Model& m, const void* srcA, const void* srcB, void* w, void* psi, double* v0,
+                                                  void* dstW, void* dstPsi, void* dstVx, const void* tab, const void* tabS, cudaStream_t s,
+                                                  int members, size_t mstride) {
+  switch (g.Ny) {
+#define X(N) case N: return go_col_step<T, N>(g, m, srcA, srcB, w, psi, v0, dstW, dstPsi, dstVx, tab, tabS, s, members, mstride);
+    TTSH_FOR_SIZES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+template <typename T, int NY> static cudaError_t prep_col_step() {
+  if constexpr (ColStepCfg<T, NY>::OK) return set_smem(k_col_step<T, NY>, ColStepCfg<T, NY>::SMEM);
+  else return cudaSuccess;
+}
 template <typename T> cudaError_t prepare_cols(const Geom& g) {
   switch (g.Ny) {
 #define X(N) case N: { using C = ColCfg<T, N>; \
-                       cudaError_t e = set_smem(k_inv_col<T, N, 1>, C::SMEM); if (e != cudaSuccess) return e; \
+                       cudaError_t e = prep_col_step<T, N>(); if (e != cudaSuccess) return e; \
+                       e = set_smem(k_inv_col<T, N, 1>, C::SMEM); if (e != cudaSuccess) return e; \
                        e = set_smem(k_inv_col<T, N, C::GMAX>, C::GMAX * C::SMEM); if (e != cudaSuccess) return e; \
                        e = set_smem(k_fwd_col<T, N, C::GMAX>, C::GMAX * C::SMEM); if (e != cudaSuccess) return e; \
                        return set_smem(k_fwd_col<T, N, 1>, C::SMEM); }

@@ -5,4 +5,6 @@ namespace ttsh {
 template cudaError_t launch_inv_col<float>(const Geom&, const Batch&, int, const void*, const void*, const double*, cudaStream_t, int, size_t);
 template cudaError_t launch_fwd_col<float>(const Geom&, const Batch&, int, const void*, const void*, cudaStream_t, int, size_t);
 template cudaError_t prepare_cols<float>(const Geom&);
+template bool col_step_supported<float>(const Geom&);
+template cudaError_t launch_col_step<float>(const Geom&, const Model&, const void*, const void*, void*, void*, double*, void*, void*, void*, const void*, const void*, cudaStream_t, int, size_t);
 }

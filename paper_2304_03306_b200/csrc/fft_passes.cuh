@@ -54,7 +54,11 @@ __host__ __device__ constexpr int col_tile_width(int Ny, int elem_bytes) {
 #ifndef TTSH_COL_CAP_SMALL
 #define TTSH_COL_CAP_SMALL 4
 #endif
-  const int cap = Ny >= 2048 ? 8 : TTSH_COL_CAP_SMALL;      // small grids: more, smaller CTAs (the GPU has 148 SMs to fill)
+  // small grids: more, smaller CTAs (the GPU has 148 SMs to fill, and the fused column kernel of col_step.cuh runs ONE CTA per tile
+  // with six transform groups): two columns at Ny = 1024, one below (measured with k_col_step, fp64 step: 1024^2 32.4 us with
+  // two columns, 37.1 with one; 512^2 18.7 with one, 24.3 with four; 256^2 16.4 / 18.8; 128^2 15.2 / 16.8)
+  if (Ny >= 128 && Ny <= 512) return 1;
+  const int cap = Ny >= 2048 ? 8 : (Ny == 1024 ? 2 : TTSH_COL_CAP_SMALL);      // Ny = 64 (four launches per step): four columns
   return cw < 2 ? 2 : (cw > cap ? cap : cw);
 }
 template <typename T, int NY> struct ColCfg {

@@ -7,6 +7,7 @@
 // integer predicate; the only divergent branch is the mx = 0 column of the Hermitian symmetrisation.
 #pragma once
 #include "ttsh_common.cuh"
+#include "spectral_point.cuh"
 
 namespace ttsh {
 
@@ -99,10 +100,6 @@ __device__ __forceinline__ cplx<T> naive_update(const Geom& g, const Model& m, i
   return e * (w[idx] + dt * r);                                               // line 4
 }
 
-template <typename T> __device__ __forceinline__ T inv_k2(const Geom& g, int mx, int my) {
-  const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my);
-  return (T)1 / (kx * kx + ky * ky);
-}
 
 template <typename T>
 __global__ void __launch_bounds__(256)
@@ -176,53 +173,7 @@ k_spectral_p2(Geom g, Model m, const cplx<T>* __restrict__ A_, const cplx<T>* __
   cplx<T>* w = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(w_) + moff);
   cplx<T>* __restrict__ psi = reinterpret_cast<cplx<T>*>(reinterpret_cast<char*>(psi_) + moff);
   double* v0 = reinterpret_cast<double*>(reinterpret_cast<char*>(v0_) + moff);
-  const int t = (int)(idx / ((size_t)g.Hy * g.CW));
-  const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
-  const int q = rem >> g.cw_shift;
-  const int mx = t * g.CW + (rem & (g.CW - 1));
-  if (mx >= g.Wx) return;
-  const int my = q <= g.My ? q : q - g.Hy;
-  const bool cut = is_cut(g, mx, my, g.num, g.den);
-  const T dt = (T)m.dt;
-  auto factor = [&](int my_) -> T {          // exp(sigma(k) dt), line 4
-    const T kx = (T)(g.dkx * mx), ky = (T)(g.dky * my_);
-    const T k2 = kx * kx + ky * ky;
-    const T sigma = -(T)m.alpha - (T)m.Gamma0 * k2 - (T)m.Gamma2 * k2 * k2;
-    return sizeof(T) == 8 ? (T)exp((double)(sigma * dt)) : (T)expf((float)(sigma * dt));
-  };
-  if (mx == 0) {
-    if (my < 0) return;                                   // written by the thread of (0, -my)
-    if (my == 0) {
-      const double e = exp(-m.alpha * m.dt);
-      v0[0] = e * (v0[0] + m.dt * (double)B[idx].x);      // Gx^(0,0)
-      v0[1] = e * (v0[1] + m.dt * (double)A[idx].y);      // Gy^(0,0)
-      w[idx] = mk<T>(0, 0);
-      psi[idx] = mk<T>(0, 0);
-      return;
-    }
-    const size_t idn = spec_index(g, g.Hy - my, 0);       // row of -my, mx = 0
-    cplx<T> out = mk<T>(0, 0);
-    if (!cut) {
-      const T ky = (T)(g.dky * my);
-      const cplx<T> sp = (T)0.5 * (A[idx] + conj(A[idn]));                   // S'^(0, my); S'^(0,-my) = conj
-      const cplx<T> rp = sp - ky * mul_i(B[idx]);                            // rhs^(0, my)
-      const cplx<T> rn = conj(sp) + ky * mul_i(B[idn]);                      // rhs^(0,-my)
-      const T e = factor(my);
-      const cplx<T> np_ = e * (w[idx] + dt * rp), nn = e * (w[idn] + dt * rn);
-      out = (T)0.5 * (np_ + conj(nn));                                       // line 12
-    }
-    const T ik2 = inv_k2<T>(g, 0, my);
-    w[idx] = out;
-    w[idn] = conj(out);
-    psi[idx] = ik2 * out;
-    psi[idn] = ik2 * conj(out);
-    return;
-  }
-  const T ky = (T)(g.dky * my);
-  cplx<T> out = factor(my) * (w[idx] + dt * (A[idx] - ky * mul_i(B[idx])));  // lines 3-4
-  out = cut ? mk<T>(0, 0) : out;
-  w[idx] = out;
-  psi[idx] = inv_k2<T>(g, mx, my) * out;                                     // line 13
+  spectral_p2_point<T>(g, m, idx, A, B, w, psi, v0, [](size_t, cplx<T>, cplx<T>) {});
 }
 
 // ttsh_set_velocity: w^ = i kx v^y - i ky v^x, v^(0) kept, then the same post-processing

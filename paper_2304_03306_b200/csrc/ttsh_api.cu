@@ -102,6 +102,9 @@ struct ttsh_handle {
   int rs_slots, rs_slots_ens, rs_slots_tan;   // persistent grid of k_row_step on this device (single system / ensemble / tangent variant)
   bool row_step_ok;     // the fused row-step kernel supports this grid / dtype / dealias fraction
   bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
+  bool col_step_ok;     // the fused column kernel (col_step.cuh) applies: an Euler step is k_row_step + k_col_step
+  bool inter_valid;     // ... and the inverse intermediates Tm[0], Tm[2], Tm[3] of the CURRENT state are at hand (k_col_step of the
+                        //     previous step wrote them); cleared by everything that touches the state or the scratch arrays
   bool row_step_real;   // ... or the real-row variant (row_step_real.cuh: its own K order and table)
   bool real_rows;       // Nx = 16384: one real row per half-length transform (fft_rows_real.cuh); internal real fields in natural order
 };
@@ -218,6 +221,7 @@ FieldOp op(const void* src, void* dst, int mode) { FieldOp o; o.src = src; o.dst
 
 // inverse 2-D transforms of the state into real fields; any destination may be NULL
 int enqueue_inverse(ttsh_handle* h, void* w, void* gx, void* gy, void* vx, void* vy, void* psi) {
+  h->inter_valid = false;
   // column pass: which intermediates are needed
   const bool need_w = w || gx, need_gy = gy != nullptr, need_psi = vy || psi, need_vx = vx != nullptr;
   Batch cb; memset(&cb, 0, sizeof(cb));
@@ -251,6 +255,7 @@ int enqueue_inverse(ttsh_handle* h, void* w, void* gx, void* gy, void* vx, void*
 
 // forward 2-D transforms of n real fields into pruned spectra S[0..n-1]
 int enqueue_forward(ttsh_handle* h, int n, const void* const* src) {
+  h->inter_valid = false;
   Batch rb; memset(&rb, 0, sizeof(rb));
   Batch cb; memset(&cb, 0, sizeof(cb));
   for (int i = 0; i < n; ++i) {
@@ -327,6 +332,12 @@ int enqueue_stage(ttsh_handle* h, int stage) {
                       (h->row_step_wl || h->row_step_real) ? h->tabXw : h->tabX, h->v0, h->stream, h->rs_slots));
       h->launches++;
       return TTSH_OK;
+    case TTSH_STAGE_COL_STEP:         // a4 column pass + a5 + the column pass of a2 / a6 of the next step in one kernel
+      if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || !h->col_step_ok) return TTSH_ERR_INVALID_ARG;
+      TRY(h, DISPATCH(h, launch_col_step, h->g, h->m, h->Tm[1], h->Tm[4], h->what, h->psihat, h->v0, h->Tm[0], h->Tm[2], h->Tm[3], h->tabY,
+                      h->tabS, h->stream));
+      h->launches++;
+      return TTSH_OK;
     case TTSH_STAGE_SPECTRAL_P2:
       TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, h->S[0], h->S[1], h->what, h->psihat, h->v0, h->stream));
       h->launches++;
@@ -350,6 +361,14 @@ int enqueue_step(ttsh_handle* h) {
   // conservative form: 4 launches where the fused row-step kernel applies, else 5 (fused real-space + forward row pass); the
   // literal form and Nx = 16384 (real-row passes, no fused row kernels) run the 6-launch sequence
   const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows;
+  if (f && h->col_step_ok) {      // two launches per step; the column pass of a2 / a6 only when its output is not at hand
+    int rc = TTSH_OK;
+    if (!h->inter_valid) rc = enqueue_stage(h, TTSH_STAGE_INV_COL);
+    if (rc == TTSH_OK) rc = enqueue_stage(h, TTSH_STAGE_ROW_STEP);
+    if (rc == TTSH_OK) rc = enqueue_stage(h, TTSH_STAGE_COL_STEP);
+    h->inter_valid = rc == TTSH_OK;
+    return rc;
+  }
   const int* seq = f ? (h->row_step_ok ? rowstep : fused) : plain;
   const int n = f ? (h->row_step_ok ? 4 : 5) : 6;
   for (int i = 0; i < n; ++i) {
@@ -359,6 +378,7 @@ int enqueue_step(ttsh_handle* h) {
   return TTSH_OK;
 }
 inline int launches_per_step(const ttsh_handle* h) {
+  if (h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows && h->col_step_ok) return 2;
   return (h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows) ? (h->row_step_ok ? 4 : 5) : 6;
 }
 
@@ -456,6 +476,9 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->row_step_wl = Nx == 4096;
   h->real_rows = Nx == 16384;
   h->rs_slots = h->rs_slots_ens = h->rs_slots_tan = 0;
+  h->col_step_ok = h->row_step_ok && !h->real_rows &&
+                   (h->dtype == TTSH_F64 ? col_step_supported<double>(h->g) : col_step_supported<float>(h->g));
+  h->inter_valid = false;
   h->device = -1;
   *out = h;   // from here on errors are reported through the handle (caller destroys it)
 
@@ -547,6 +570,7 @@ int ttsh_set_advection_form(ttsh_handle* h, int form) {
     h->graph_ok = false;
   }
   h->advection_form = form;
+  h->inter_valid = false;
   return TTSH_OK;
 }
 
@@ -560,6 +584,11 @@ int ttsh_step(ttsh_handle* h, int n) {
   // four kernels of a step take about as long as a graph launch costs on the host, GRAPH_K steps per launch.  Large grids launch
   // directly.  Replays are bit-identical to direct launches (same kernels, same order).
   constexpr int GRAPH_K = 16;
+  if (launches_per_step(h) == 2 && !h->inter_valid) {   // fused column kernel: the captured steps start at the row kernel
+    int rc = enqueue_stage(h, TTSH_STAGE_INV_COL);
+    if (rc != TTSH_OK) return rc;
+    h->inter_valid = true;
+  }
   const size_t P = (size_t)h->Nx * h->Ny;
   const bool use_graph = P <= (size_t)1024 * 1024 && n >= 4;
   const bool use_k = P <= (size_t)256 * 256 && n >= GRAPH_K;
@@ -643,6 +672,7 @@ int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, d
   if (h->sticky) return h->sticky;
   CHECK_DEVICE(h);
   const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
+  h->inter_valid = false;
   TRY(h, cudaMemcpyAsync(h->what, w_hat, bytes, cudaMemcpyDeviceToDevice, h->stream));
   TRY(h, cudaMemcpyAsync(h->v0, mean_flow, 2 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
   TRY(h, DISPATCH(h, launch_psi_from_w, h->g, h->what, h->psihat, h->stream));
@@ -902,6 +932,7 @@ int ttsh_tangent_step(ttsh_tangent* s, int n) {
   const size_t ms = s->stride;
   for (int it = 0; it < n; ++it) {
     // base state in real space (permuted internal layout): R[0] = w, R[3] = v_x, R[4] = v_y
+    h->inter_valid = false;
     int rc = enqueue_stage(h, TTSH_STAGE_INV_COL);
     if (rc == TTSH_OK) rc = enqueue_stage(h, TTSH_STAGE_INV_ROW);
     if (rc != TTSH_OK) return rc;
@@ -1038,14 +1069,27 @@ int ttsh_ensemble_create(ttsh_ensemble** out, ttsh_handle* const* members, int c
   return TTSH_OK;
 }
 
+// the column pass of a2 / a6 for all members (stage 0 of a step)
+static int ensemble_enqueue_inv_col(ttsh_ensemble* e, cudaStream_t stream) {
+  ttsh_handle* h = e->members[0];
+  Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->psihat, h->Tm[2], SM_ONE), op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
+  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, h->v0, stream, (int)e->members.size(), e->mstride));
+  return TTSH_OK;
+}
+// one Euler step of all members.  Where the fused column kernel applies (h->col_step_ok) the step is k_row_step + k_col_step and
+// expects the members' inverse intermediates at hand (ttsh_ensemble_step sees to that); else the four launches of ttsh_step.
 static int ensemble_enqueue_step(ttsh_ensemble* e, cudaStream_t stream) {
   ttsh_handle* h = e->members[0];
   const int B = (int)e->members.size();
   const size_t ms = e->mstride;
-  Batch cb = make_batch({op(h->what, h->Tm[0], SM_ONE), op(h->psihat, h->Tm[2], SM_ONE), op(h->psihat, h->Tm[3], SM_IKY_MEANX)});
-  TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, h->v0, stream, B, ms));
+  if (!h->col_step_ok) { const int rc = ensemble_enqueue_inv_col(e, stream); if (rc != TTSH_OK) return rc; }
   TRY(h, DISPATCH(h, launch_row_step_ens, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
                   (h->row_step_wl || h->row_step_real) ? h->tabXw : h->tabX, h->v0, stream, B, ms, h->rs_slots_ens));
+  if (h->col_step_ok) {
+    TRY(h, DISPATCH(h, launch_col_step, h->g, h->m, h->Tm[1], h->Tm[4], h->what, h->psihat, h->v0, h->Tm[0], h->Tm[2], h->Tm[3], h->tabY, h->tabS,
+                    stream, B, ms));
+    return TTSH_OK;
+  }
   Batch fb = make_batch({op(h->Tm[1], h->S[0], 0), op(h->Tm[4], h->S[1], 0)});
   TRY(h, DISPATCH(h, launch_fwd_col, h->g, fb, 2, h->tabY, h->tabS, stream, B, ms));
   TRY(h, DISPATCH(h, launch_spectral_p2, h->g, h->m, h->S[0], h->S[1], h->what, h->psihat, h->v0, stream, B, ms));
@@ -1062,6 +1106,17 @@ int ttsh_ensemble_step(ttsh_ensemble* e, int n) {
     if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
   }
   if (n == 0) return TTSH_OK;
+  const int per_step = h0->col_step_ok ? 2 : 4;
+  if (h0->col_step_ok) {     // the captured / enqueued steps start at the row kernel: make every member's intermediates valid first
+    bool valid = true;
+    for (ttsh_handle* h : e->members) valid = valid && h->inter_valid;
+    if (!valid) {
+      const int rc = ensemble_enqueue_inv_col(e, h0->stream);
+      if (rc != TTSH_OK) return rc;
+      e->launches += 1;
+    }
+  }
+  for (ttsh_handle* h : e->members) h->inter_valid = h0->col_step_ok;   // k_col_step leaves them valid for every member
   // a step of a small ensemble is launch-latency bound: replay one captured step (as ttsh_step does)
   const bool use_graph = (size_t)h0->Nx * h0->Ny * e->members.size() <= (size_t)4 * 1024 * 1024 && n >= 4;
   if (use_graph && !e->graph_exec) {
@@ -1085,7 +1140,7 @@ int ttsh_ensemble_step(ttsh_ensemble* e, int n) {
       const int rc = ensemble_enqueue_step(e, h0->stream);
       if (rc != TTSH_OK) return rc;
     }
-    e->launches += 4;
+    e->launches += per_step;
   }
   for (ttsh_handle* h : e->members) {
     h->t += (double)n * h->dt;
@@ -1110,6 +1165,7 @@ int ttsh_run_stage(ttsh_handle* h, int stage) {
   if (h->sticky) return h->sticky;
   CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
+  h->inter_valid = false;
   return enqueue_stage(h, stage);
 }
 

@@ -24,7 +24,8 @@ TTSH_F64, TTSH_F32 = 8, 4
 TTSH_MASK_BINARY, TTSH_MASK_PROCESSED = 0, 1
 TTSH_ADVECTION_CONSERVATIVE, TTSH_ADVECTION_LITERAL = 0, 1
 (TTSH_STAGE_INV_COL, TTSH_STAGE_INV_ROW, TTSH_STAGE_REAL, TTSH_STAGE_FWD_ROW, TTSH_STAGE_FWD_COL,
- TTSH_STAGE_SPECTRAL, TTSH_STAGE_REAL_FWD_ROW, TTSH_STAGE_FWD_COL_P2, TTSH_STAGE_SPECTRAL_P2, TTSH_STAGE_ROW_STEP) = range(10)
+ TTSH_STAGE_SPECTRAL, TTSH_STAGE_REAL_FWD_ROW, TTSH_STAGE_FWD_COL_P2, TTSH_STAGE_SPECTRAL_P2, TTSH_STAGE_ROW_STEP,
+ TTSH_STAGE_COL_STEP) = range(11)
 
 # every symbol include/ttsh.h declares (tests check that the library exports all of them)
 SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_velocity", "ttsh_set_advection_form", "ttsh_step",

@@ -57,7 +57,9 @@ def test_ensemble_members_match_oracle_and_single_handles(ttsh, Nx, Ny, count, n
         ens.members[i].set_velocity(*vels[i]); singles[i].set_velocity(*vels[i]); oracles[i].set_velocity(*vels[i])
     l0 = ens.launch_count()
     ens.step(1)                       # direct launches
-    assert ens.launch_count() - l0 == 4, "one launch of each of the 4 hot kernels for the whole ensemble"
+    # Ny = 64: the four hot kernels, one launch each for the whole ensemble; 128 <= Ny <= 1024: k_inv_col (the intermediates are not
+    # at hand yet) + k_row_step + k_col_step
+    assert ens.launch_count() - l0 == (4 if Ny == 64 else 3)
     for i in range(count):
         singles[i].step(1); oracles[i].step(1)
     for i in range(count):

@@ -150,6 +150,51 @@ def test_fused_forward_row_kernel_equals_unfused_pair(ttsh, shape, dtype):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("Nx,Ny,dtype", [(256, 128, "f64"), (128, 512, "f64"), (1024, 1024, "f64"), (512, 1024, "f32"), (2048, 256, "f32")])
+def test_fused_column_kernel_against_the_four_launch_step(ttsh, Nx, Ny, dtype):
+    """k_col_step (128 <= Ny <= 1024: forward column pass + lines 3-13 + inverse column pass of the next step in one kernel, two
+    launches per Euler step) against the same steps driven stage by stage through k_inv_col, the row kernel, k_fwd_col and
+    k_spectral_p2 (same expressions on the same operands: agreement to round-off, the compiler contracts a few multiply-adds
+    differently), and against ITSELF bit for bit however it is driven: direct launches, CUDA-graph replays, with calls in between
+    that overwrite the scratch arrays (the intermediates are then rebuilt by k_inv_col), and stage by stage (0, then 9, 10)."""
+    import torch
+    mask = workloads.disk_mask(Nx, Ny, 0.5, 0.3 * min(Nx, Ny) * 0.5)
+    vel = workloads.planewave_velocity(Nx, Ny, 0.5, 17, amplitude=1.0)
+    vel = (vel[0] + 0.1, vel[1] - 0.05)                              # a mean flow: the (0, 0) entry of tile 0
+    mk = lambda: ttsh.Solver(Nx, Ny, 0.5, 0.01, ttsh.baseline_params(), dtype, mask=mask)
+    a, b, c, d = mk(), mk(), mk(), mk()
+    for s in (a, b, c, d):
+        s.set_velocity(*vel)
+    four = (ttsh.TTSH_STAGE_INV_COL, ttsh.TTSH_STAGE_ROW_STEP, ttsh.TTSH_STAGE_FWD_COL_P2, ttsh.TTSH_STAGE_SPECTRAL_P2)
+    tol = 1e-13 if dtype == "f64" else 2e-5
+
+    l0 = a.launch_count()
+    a.step(1)
+    assert a.launch_count() - l0 == 3, "k_inv_col once, then k_row_step + k_col_step"
+    l0 = a.launch_count()
+    a.step(2)
+    assert a.launch_count() - l0 == 4, "two launches per Euler step"
+    a.step(21)                                                        # CUDA-graph replays (16 + 5 on the small grids)
+    for _ in range(24):
+        for st in four:
+            b.run_stage(st)
+    for x, y, name in zip(gpu_fields(a), gpu_fields(b), ("vx", "vy", "w", "psi")):
+        assert rel(x, y) <= tol, name
+    # c: one step per call with get_fields / diagnostics in between (they overwrite the scratch arrays)
+    for _ in range(24):
+        c.step(1)
+        c.get_fields(); c.diagnostics()
+    # d: the stages by hand
+    d.run_stage(ttsh.TTSH_STAGE_INV_COL)
+    for _ in range(24):
+        d.run_stage(ttsh.TTSH_STAGE_ROW_STEP); d.run_stage(ttsh.TTSH_STAGE_COL_STEP)
+    for other, what in ((c, "step by step with calls in between"), (d, "stages 0, (9, 10) x 24")):
+        for x, y, name in zip(a.get_fields(), other.get_fields(), ("vx", "vy", "w", "psi")):
+            assert torch.equal(x, y), f"{what}: {name}"
+    for s in (a, b, c, d):
+        s.close()
+
+
 # ---------------------------------------------------------------- whole-step parity
 CASES_SMALL = [
     ("C1-baseline", 64, 64, "baseline", "disk", 1e-2),
@@ -609,9 +654,12 @@ def test_real_row_fused_kernel_nx8192_fp64(ttsh, which, Ny):
     s, o = make_pair(ttsh, Nx, Ny, dx, dt, which, mask, transform="c", vel=vel)
     l0 = s.launch_count()
     s.step(1); o.step(1)
-    assert s.launch_count() - l0 == 4, "k_inv_col, k_row_step_real, k_fwd_col, k_spectral_p2"
+    assert s.launch_count() - l0 == 3, "k_inv_col (the intermediates are not at hand yet), k_row_step_real, k_col_step (Ny <= 1024)"
     compare_state(s, o, TOL_F64_1, f"8192x{Ny} {which} step 1")
-    s.step(9); o.step(9)
+    l0 = s.launch_count()
+    s.step(3); o.step(3)
+    assert s.launch_count() - l0 == 1 + 3 * 2, "get_fields used the scratch arrays: k_inv_col once, then two launches per step"
+    s.step(6); o.step(6)
     compare_state(s, o, TOL_F64_100, f"8192x{Ny} {which} step 10")
     cx, cy = (Nx // 2) * dx, (Ny // 2) * dx
     d, od = s.diagnostics(cx, cy), o.diagnostics(cx, cy)

@@ -183,8 +183,10 @@ int ttsh_tangent_destroy(ttsh_tangent* s);
 /* Ensembles: the paper's workload is sweeps of independent runs on one grid — disk radius R (Fig. 2), the
  * hysteresis branches, dumbbell separations — and on grids up to about 1024^2 one system
  * cannot fill a B200.  An ensemble advances `count` independent handles with ONE launch of each hot kernel per Euler step
- * (4 launches for all members together; 2 where ttsh_step takes 2: 128 <= Ny <= 1024), every member computing exactly what
- * ttsh_step computes for it: results are bit-identical to stepping the members one by one.
+ * (4 launches for all members together), every member computing exactly what ttsh_step computes for it: results are
+ * bit-identical to stepping the members one by one.  On grids with 128 <= Ny <= 1024, where ttsh_step takes 2 launches
+ * (TTSH_STAGE_COL_STEP), an ensemble does the same as long as count x (number of column tiles) <= 8 x (number of SMs); a larger
+ * one is bound by throughput, keeps the 4 launches, and then agrees with ttsh_step to round-off instead of bit for bit.
  * Requirements (else TTSH_ERR_INVALID_ARG): count >= 1; all members have the same Nx, Ny, dtype, dx, dt, parameters and
  * stream, use TTSH_ADVECTION_CONSERVATIVE with the 1/2 rule on a grid the fused row kernel supports (Nx <= 8192), and their workspaces lie at a uniform byte stride: workspace_b = workspace_0 + b * stride, stride >=
  * ttsh_workspace_bytes (carve them from one allocation).  Masks, states and step counters are per member; all other calls

@@ -135,6 +135,7 @@ template <class P> static P* vec_ptr(const ttsh_tangent* s, P* p0, int i) {
 }
 
 struct ttsh_ensemble {
+  bool col_fused;                      // the step is k_row_step + k_col_step (small ensembles of grids with 128 <= Ny <= 1024), else 4 launches
   std::vector<ttsh_handle*> members;   // borrowed
   size_t mstride;                      // bytes between consecutive members' workspaces
   cudaGraphExec_t graph_exec;
@@ -1065,6 +1066,13 @@ int ttsh_ensemble_create(ttsh_ensemble** out, ttsh_handle* const* members, int c
   e->mstride = count > 1 ? (size_t)stride : 0;
   e->graph_exec = nullptr;
   e->launches = 0;
+  {   // k_col_step runs ONE CTA per tile and member: it shortens the dependency chain of a step, which is what binds a small ensemble,
+      // but has less throughput than the separate column passes, which is what binds a large one (C3 x 16: 454 vs 395 us per step)
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    e->col_fused = h0->col_step_ok && (long long)count * h0->g.NT <= 8LL * sms;
+  }
   *out = e;
   return TTSH_OK;
 }
@@ -1076,16 +1084,16 @@ static int ensemble_enqueue_inv_col(ttsh_ensemble* e, cudaStream_t stream) {
   TRY(h, DISPATCH(h, launch_inv_col, h->g, cb, 3, h->tabY, h->tabS, h->v0, stream, (int)e->members.size(), e->mstride));
   return TTSH_OK;
 }
-// one Euler step of all members.  Where the fused column kernel applies (h->col_step_ok) the step is k_row_step + k_col_step and
+// one Euler step of all members.  With the fused column kernel (e->col_fused) the step is k_row_step + k_col_step and
 // expects the members' inverse intermediates at hand (ttsh_ensemble_step sees to that); else the four launches of ttsh_step.
 static int ensemble_enqueue_step(ttsh_ensemble* e, cudaStream_t stream) {
   ttsh_handle* h = e->members[0];
   const int B = (int)e->members.size();
   const size_t ms = e->mstride;
-  if (!h->col_step_ok) { const int rc = ensemble_enqueue_inv_col(e, stream); if (rc != TTSH_OK) return rc; }
+  if (!e->col_fused) { const int rc = ensemble_enqueue_inv_col(e, stream); if (rc != TTSH_OK) return rc; }
   TRY(h, DISPATCH(h, launch_row_step_ens, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
                   (h->row_step_wl || h->row_step_real) ? h->tabXw : h->tabX, h->v0, stream, B, ms, h->rs_slots_ens));
-  if (h->col_step_ok) {
+  if (e->col_fused) {
     TRY(h, DISPATCH(h, launch_col_step, h->g, h->m, h->Tm[1], h->Tm[4], h->what, h->psihat, h->v0, h->Tm[0], h->Tm[2], h->Tm[3], h->tabY, h->tabS,
                     stream, B, ms));
     return TTSH_OK;
@@ -1106,8 +1114,8 @@ int ttsh_ensemble_step(ttsh_ensemble* e, int n) {
     if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE) return TTSH_ERR_INVALID_ARG;
   }
   if (n == 0) return TTSH_OK;
-  const int per_step = h0->col_step_ok ? 2 : 4;
-  if (h0->col_step_ok) {     // the captured / enqueued steps start at the row kernel: make every member's intermediates valid first
+  const int per_step = e->col_fused ? 2 : 4;
+  if (e->col_fused) {     // the captured / enqueued steps start at the row kernel: make every member's intermediates valid first
     bool valid = true;
     for (ttsh_handle* h : e->members) valid = valid && h->inter_valid;
     if (!valid) {
@@ -1116,7 +1124,7 @@ int ttsh_ensemble_step(ttsh_ensemble* e, int n) {
       e->launches += 1;
     }
   }
-  for (ttsh_handle* h : e->members) h->inter_valid = h0->col_step_ok;   // k_col_step leaves them valid for every member
+  for (ttsh_handle* h : e->members) h->inter_valid = e->col_fused;      // k_col_step leaves them valid for every member
   // a step of a small ensemble is launch-latency bound: replay one captured step (as ttsh_step does)
   const bool use_graph = (size_t)h0->Nx * h0->Ny * e->members.size() <= (size_t)4 * 1024 * 1024 && n >= 4;
   if (use_graph && !e->graph_exec) {

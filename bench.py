@@ -227,6 +227,7 @@ def stage_bytes(Nx, Ny, w, conservative=True):
         "k_spectral_p2": 3 * spec + 2 * spec,                    # A^, B^, w^ in; w^, psi^ out
         "k_fwd_col": (2 * inter + 2 * spec) if conservative else (3 * inter + 3 * spec),
         "k_spectral": (3 if conservative else 4) * spec + 2 * spec,   # A^, B^ (or F^x, F^y, S^), w^ in; w^, psi^ out
+        "k_col_step": 2 * inter + spec + 2 * spec + 3 * inter,   # A~, B~, w^ in; w^, psi^ and the three inverse intermediates out
     }
 
 
@@ -274,6 +275,12 @@ def measure(torch, ttsh, cfg, dtype, K, W, device, want_roofline=True, want_e2e=
             s.run_stage(9)
         except Exception:     # grid / dtype without the fused row-step kernel: ttsh_step launches the 5-kernel sequence
             names, ids = ["k_inv_col", "k_inv_row", "k_fwd_row_fused", "k_fwd_col", "k_spectral_p2"], [0, 1, 6, 7, 8]
+        if 128 <= cfg.Ny <= 1024 and ids[1] == 9:
+            try:                  # grids whose step is k_row_step + k_col_step (col_step.cuh): time those two
+                s.run_stage(0); s.run_stage(9); s.run_stage(10)
+                names, ids = ["k_row_step", "k_col_step"], [9, 10]
+            except Exception:
+                pass
         ns = len(ids)
         ev = [[torch.cuda.Event(enable_timing=True) for _ in range(ns + 1)] for _ in range(reps)]
         for r in range(reps):

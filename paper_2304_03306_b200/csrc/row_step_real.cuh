@@ -35,8 +35,10 @@ template <typename T, int NX> struct RowStepRealCfg {
   static constexpr bool OK = fft_wl_supported<M>();
   static constexpr int TPL = M / 16, THREADS = TPL;
   static constexpr int LS = fft_wl_line_elems<T, M>() + 4;
-  // one field waits in tensor memory (tmem.cuh): 16 complex values = 64 columns per thread, two warps per lane quarter
-  static constexpr unsigned TMEM_COLS = 128;
+  // tensor memory (tmem.cuh), per thread: 64 columns for the waiting field (16 complex values) and 2 x 48 for the merged bins of
+  // the pair's first row (B~ and A~, 9 complex values each in three 4-value pieces); two warps per lane quarter -> 2 x 160 <= 512
+  static constexpr unsigned TMEM_COLS = 512;
+  static constexpr int TMEM_PER_WARP = 256;
   static constexpr size_t OFF_TAB = (size_t)LS * sizeof(cplx<T>);
   // two staging slots, used in turn by the (A, B) pairs of w~, v_x~, psi~ (2 Wxp <= 2 (NX/4 + 8) complex values) and by the row of K
   static constexpr size_t SLOT = ((size_t)(NX / 4 + 8) * 2 * sizeof(cplx<T>) + 127) / 128 * 128;
@@ -123,7 +125,8 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   __syncthreads();
   tmem_fence_after_sync();
   const unsigned tmem_base = *tmem_holder;
-  const unsigned tstash = tmem_warp_addr(tmem_base, j >> 5, 64 * (j >> 7));      // this thread's 64 columns: slot k at column 4 k
+  const unsigned tstash = tmem_warp_addr(tmem_base, j >> 5, C::TMEM_PER_WARP * (j >> 7));   // this thread's columns: slot k of the waiting field at column 4 k
+  const unsigned tparkB = tstash + 64, tparkA = tstash + 112;                    // merged B~ / A~ bins of the pair's first row
   pdl_wait();          // inputs, K and v0 below are written by the preceding launches
   pdl_trigger();
   T meany = (T)0;
@@ -218,9 +221,30 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
         bulk_load(slot1, byte_off(inVx, xmo) + (size_t)xrp * in_stride, in_bytes, bar1);
       });
       __syncthreads();
+      // The merged bins of the pair's first row wait in tensor memory; the second row then writes whole (A, B) pairs (32 bytes: one
+      // full sector per bin instead of two half-written ones, and half as many store instructions).
+      auto emit = [&](cplx<T>* out, unsigned tpark, const cplx<T> (&mb)[12]) {
+        if (r == 0) {
 #pragma unroll
-      for (int i = 0; i < 9; ++i)
-        if (i < 8 || leader) st_c(byte_off(outB, mo) + inter_pair_index(g, a, p, j + TPL * i) + r, merged(i));      // B~ = Gx~
+          for (int q = 0; q < 3; ++q) tmem_st4(tpark + 16 * q, mb + 4 * q);
+        } else {
+          TmemQuad pq[3];
+#pragma unroll
+          for (int q = 0; q < 3; ++q) tmem_ld4_issue(tpark + 16 * q, pq[q]);
+#pragma unroll
+          for (int q = 0; q < 3; ++q) tmem_wait_ld(pq[q]);
+#pragma unroll
+          for (int i = 0; i < 9; ++i)
+            if (i < 8 || leader) st_pair(out + inter_pair_index(g, a, p, j + TPL * i), tmem_quad_get(pq[i >> 2], i & 3), mb[i]);
+        }
+      };
+      {
+        cplx<T> mb[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) mb[i] = (i < 8 || (i == 8 && leader)) ? merged(i < 9 ? i : 8) : mk<T>(0, 0);
+        tmem_wait_st();
+        emit(byte_off(outB, mo), tparkB, mb);                                          // B~ = Gx~
+      }
       cplx<T> ikg[9];
       T gy0 = (T)0;
       fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), to_line);
@@ -246,13 +270,19 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       }
       fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
       __syncthreads();
+      {
+        cplx<T> mb[12];
 #pragma unroll
-      for (int i = 0; i < 9; ++i)
-        if (i < 8 || leader) {
-          cplx<T> sa = merged(i) + ikg[i];
-          if (i == 0 && leader) sa = mk<T>(sa.x, gy0);       // real numbers S'~(0, y) and Gy~(0, y) travel together (k_fwd_row_fused)
-          st_c(byte_off(outA, mo) + inter_pair_index(g, a, p, j + TPL * i) + r, sa);
+        for (int i = 0; i < 12; ++i) {
+          mb[i] = mk<T>(0, 0);
+          if (i < 8 || (i == 8 && leader)) {
+            mb[i] = merged(i < 9 ? i : 8) + ikg[i < 9 ? i : 8];
+            if (i == 0 && leader) mb[i] = mk<T>(mb[i].x, gy0);   // real numbers S'~(0, y) and Gy~(0, y) travel together (k_fwd_row_fused)
+          }
         }
+        tmem_wait_st();
+        emit(byte_off(outA, mo), tparkA, mb);                                          // A~ = i k_x Gy~ + S'~
+      }
     }
   }
   tmem_fence_before_sync();

@@ -59,7 +59,10 @@ __host__ __device__ constexpr int col_tile_width(int Ny, int elem_bytes) {
   // two columns, 37.1 with one; 512^2 18.7 with one, 24.3 with four; 256^2 16.4 / 18.8; 128^2 15.2 / 16.8)
   if (Ny >= 128 && Ny <= 512) return 1;
   const int cap = Ny >= 2048 ? 8 : (Ny == 1024 ? 2 : TTSH_COL_CAP_SMALL);      // Ny = 64 (four launches per step): four columns
-  return cw < 2 ? 2 : (cw > cap ? cap : cw);
+  // Ny = 8192 in fp64: one 4096-point column (64 KB) per 256-thread CTA, two CTAs per SM, instead of two columns in one 512-thread CTA
+  // per SM (8192^2: k_inv_col 437 -> 349 us, k_fwd_col 289 -> 237 us; k_row_step_real writes whole 32-byte pairs and pays 34 us)
+  if (cw < 2) return Ny >= 8192 ? 1 : 2;
+  return cw > cap ? cap : cw;
 }
 template <typename T, int NY> struct ColCfg {
   static constexpr int NH = NY / 2;

@@ -3,7 +3,8 @@
 //
 // One REAL row is transformed as a half-length complex sequence z[n] = f(2n) + i f(2n+1), n < M = Nx/2 = 4096 (the textbook
 // real-data FFT), so that the machinery of row_step.cuh applies unchanged at N = 4096: the warp-local plan of fft_core.cuh, one
-// field live in registers (V), one waiting in registers (H), one in the private shared-memory stash.  The pointwise stage
+// field live in registers (V), one waiting in registers (H), one parked by its owner thread (there: a shared-memory stash; here:
+// tensor memory).  The pointwise stage
 // (lines 1-2 of Algorithm 1) does not care that a complex slot now holds two neighbouring points of one row
 // instead of one point of two rows.  What changes is the step between the half spectrum F (what the column passes read and
 // write) and the transform Z of the packed sequence:
@@ -23,6 +24,8 @@
 //   slot 0:  w~ pairs -> psi~ pairs -> w~ of the next row          slot 1:  v_x~ pairs -> K row -> v_x~ of the next row
 // (the same pairs again for the second row of the pair).  The waiting field (w, then S') is parked in TENSOR MEMORY (tmem.cuh) by its
 // owner thread: that frees the 64 KB of shared memory the second slot needs and takes the stash traffic off the shared-memory pipe.
+// The merged bins of the pair's FIRST row wait there too, so that the second row writes whole 32-byte (A, B) pairs of the forward
+// intermediates (one full sector per bin) instead of 16-byte halves.
 // K comes in the thread order of the plan: (K(y, 2n), K(y, 2n+1)) for n = wl_j(t) + 256 k at (k 256 + t) 2 (k_reperm_real).
 #pragma once
 #include "row_step.cuh"

@@ -43,7 +43,7 @@ template <typename T> cudaError_t launch_spectral_p2(const Geom& g, const Model&
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                   const void* K, void* oA, void* oB, const void* tabX, const double* v0, cudaStream_t s, int slots);
 template <typename T> bool row_step_supported(const Geom& g);
-// ... and it is the real-row variant (row_step_real.cuh: Nx = 8192 in fp64): K in its thread order (launch_reperm_real); table = the warp-local
+// ... and it is the real-row variant (row_step_real.cuh: Nx = 8192): K in its thread order (launch_reperm_real); table = the warp-local
 // table of length Nx/2 followed, at element row_step_real_tabr(g), by W_Nx^j, j < Nx/32
 template <typename T> bool row_step_is_real(const Geom& g);
 template <typename T> int row_step_real_tabr(const Geom& g);

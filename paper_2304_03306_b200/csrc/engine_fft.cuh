@@ -218,9 +218,9 @@ template <typename T> cudaError_t prepare_rows(const Geom& g) {
 #include "row_step.cuh"
 #include "row_step_real.cuh"
 namespace ttsh {
-// Nx = 8192 in fp64 (a packed row pair does not fit in shared memory): one real row per half-length transform (row_step_real.cuh);
+// Nx = 8192 (fp64: a packed row pair does not fit in shared memory; fp32: faster): one real row per half-length transform (row_step_real.cuh);
 // K in the thread order of that kernel (launch_reperm_real), table = fill_stage_tables_real
-template <typename T, int NX> constexpr bool row_step_real_enabled() { return sizeof(T) == 8 && NX == 8192; }
+template <typename T, int NX> constexpr bool row_step_real_enabled() { return NX == 8192; }
 __host__ __device__ constexpr int row_step_real_tabr_offset(int M) { return (fft_wl_tw_elems_rt(M) + 15) / 16 * 16; }
 template <typename T, int NX, bool ENS> static cudaError_t prep_row_step_real(int* slots) {
   using C = RowStepRealCfg<T, NX>;
@@ -333,7 +333,7 @@ template <typename T> cudaError_t launch_row_step_tan(const Geom& g, const Model
   return cudaErrorInvalidValue;
 }
 template <typename T> bool row_step_is_real(const Geom& g) {
-  return row_step_supported<T>(g) && sizeof(T) == 8 && g.Nx == 8192;
+  return row_step_supported<T>(g) && g.Nx == 8192;
 }
 template <typename T> int row_step_real_tabr(const Geom& g) { return row_step_real_tabr_offset(g.Nx / 2); }
 template <typename T> bool row_step_supported(const Geom& g) {

@@ -1,5 +1,6 @@
-// row_step_real.cuh — the row half of one Euler step in ONE kernel (row_step.cuh) for Nx = 8192 in fp64, the paper's production
-// width, where a packed row PAIR (128 KB per field) no longer fits in shared memory.
+// row_step_real.cuh — the row half of one Euler step in ONE kernel (row_step.cuh) for Nx = 8192, the paper's production width
+// (PAPER.md:71, :271).  In fp64 a packed row PAIR (128 KB per field) no longer fits in shared memory; in fp32 it does, but the
+// four-stage plan of an 8192-point transform is slower than what follows (8192^2 fp32: 749 -> 589 us for the row kernel).
 //
 // One REAL row is transformed as a half-length complex sequence z[n] = f(2n) + i f(2n+1), n < M = Nx/2 = 4096 (the textbook
 // real-data FFT), so that the machinery of row_step.cuh applies unchanged at N = 4096: the warp-local plan of fft_core.cuh, one
@@ -114,7 +115,8 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   const unsigned in_bytes = (unsigned)(in_stride * sizeof(cplx<T>)), k_bytes = (unsigned)(NX * sizeof(T));
   const bool leader = (j == 0);
   unsigned ph0 = 0, ph1 = 0;
-  static_assert(sizeof(T) == 8, "the tensor-memory stash is laid out for complex doubles");
+  constexpr int CH = TmemPack<T>::CH, NCH = 16 / CH;          // complex values per 16 columns of tensor memory; pieces per field
+  constexpr int NBP = (9 + CH - 1) / CH, NB = NBP * CH;        // the 9 merged bins of a thread in NBP pieces
   auto locate = [&](int rpg, int& rp_, size_t& mo_) {
     if constexpr (ENS) { const int mb = rpg / rpm; rp_ = rpg - mb * rpm; mo_ = (size_t)mb * mstride; }
     else { rp_ = rpg; mo_ = 0; }
@@ -123,13 +125,16 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   mbar_fence_init();
   if (j < 32) tmem_alloc(tmem_holder, C::TMEM_COLS);
   tmem_fence_before_sync();
-  for (int i = j; i < fft_wl_tw_elems_rt(M); i += C::THREADS) stab[i] = ldg_c(tabW + i);     // host-written at ttsh_create
+  // the table of the warp-local plan: a copy in shared memory in fp64, through L1 in fp32 (row_step.cuh, SMEM_TAB, says why)
+  if constexpr (sizeof(T) == 8) {
+    for (int i = j; i < fft_wl_tw_elems_rt(M); i += C::THREADS) stab[i] = ldg_c(tabW + i);     // host-written at ttsh_create
+  } else stab = const_cast<cplx<T>*>(tabW);
   const cplx<T> wj = ldg_c(tabR + j);                              // W_NX^j
   __syncthreads();
   tmem_fence_after_sync();
   const unsigned tmem_base = *tmem_holder;
   const unsigned tstash = tmem_warp_addr(tmem_base, j >> 5, C::TMEM_PER_WARP * (j >> 7));   // this thread's columns: slot k of the waiting field at column 4 k
-  const unsigned tparkB = tstash + 64, tparkA = tstash + 112;                    // merged B~ / A~ bins of the pair's first row
+  const unsigned tparkB = tstash + 16 * NCH, tparkA = tparkB + 16 * NBP;         // merged B~ / A~ bins of the pair's first row
   pdl_wait();          // inputs, K and v0 below are written by the preceding launches
   pdl_trigger();
   T meany = (T)0;
@@ -173,7 +178,7 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       inv_real_row_regs<T, M, RM_ONE>(row0, j, wj, line, stab, scale_i, dkx, meany, V,
                                       [&]() { if (leader) bulk_load(slot0, byte_off(inPsi, mo) + (size_t)rp * in_stride, in_bytes, bar0); });
 #pragma unroll
-      for (int q = 0; q < 4; ++q) tmem_st4(tstash + 16 * q, V + 4 * q);      // w waits in tensor memory
+      for (int q = 0; q < NCH; ++q) tmem_stc(tstash + 16 * q, V + CH * q);   // w waits in tensor memory
       mbar_wait(bar1, ph1); ph1 ^= 1;
       inv_real_row_regs<T, M, RM_ONE>(row1, j, wj, line, stab, scale_i, dkx, meany, H,
                                       [&]() { if (leader) bulk_load(slot1, byte_off(K2, mo) + y * NX, k_bytes, bar1); });                    // v_x
@@ -186,17 +191,17 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       tmem_wait_st();
       {
         TmemQuad wq[2];
-        tmem_ld4_issue(tstash, wq[0]);
+        tmem_ldc_issue(tstash, wq[0]);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
+        for (int q = 0; q < NCH; ++q) {
           tmem_wait_ld(wq[q & 1]);
-          if (q < 3) tmem_ld4_issue(tstash + 16 * (q + 1), wq[(q + 1) & 1]);
-          cplx<T> s4[4];
+          if (q < NCH - 1) tmem_ldc_issue(tstash + 16 * (q + 1), wq[(q + 1) & 1]);
+          cplx<T> s4[CH];
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int k = 4 * q + i;
+          for (int i = 0; i < CH; ++i) {
+            const int k = CH * q + i;
             const cplx<T> kk = kslot[k * TPL + j];
-            const cplx<T> w = tmem_quad_get(wq[q & 1], i);
+            const cplx<T> w = tmem_getc(wq[q & 1], i, T());
             const T kA = kk.x, kB = kk.y;
             const T vxA = H[k].x, vxB = H[k].y, vyA = V[k].x, vyB = V[k].y;
             const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * kA);
@@ -206,7 +211,7 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
             H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
             s4[i] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));                   // S'
           }
-          tmem_st4(tstash + 16 * q, s4);
+          tmem_stc(tstash + 16 * q, s4);
         }
       }
       // ---- a4: three forward transforms, each merged into the half spectrum of the row on the bins k = j + 256 i ----
@@ -226,25 +231,25 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       __syncthreads();
       // The merged bins of the pair's first row wait in tensor memory; the second row then writes whole (A, B) pairs (32 bytes: one
       // full sector per bin instead of two half-written ones, and half as many store instructions).
-      auto emit = [&](cplx<T>* out, unsigned tpark, const cplx<T> (&mb)[12]) {
+      auto emit = [&](cplx<T>* out, unsigned tpark, const cplx<T> (&mb)[NB]) {
         if (r == 0) {
 #pragma unroll
-          for (int q = 0; q < 3; ++q) tmem_st4(tpark + 16 * q, mb + 4 * q);
+          for (int q = 0; q < NBP; ++q) tmem_stc(tpark + 16 * q, mb + CH * q);
         } else {
-          TmemQuad pq[3];
+          TmemQuad pq[NBP];
 #pragma unroll
-          for (int q = 0; q < 3; ++q) tmem_ld4_issue(tpark + 16 * q, pq[q]);
+          for (int q = 0; q < NBP; ++q) tmem_ldc_issue(tpark + 16 * q, pq[q]);
 #pragma unroll
-          for (int q = 0; q < 3; ++q) tmem_wait_ld(pq[q]);
+          for (int q = 0; q < NBP; ++q) tmem_wait_ld(pq[q]);
 #pragma unroll
           for (int i = 0; i < 9; ++i)
-            if (i < 8 || leader) st_pair(out + inter_pair_index(g, a, p, j + TPL * i), tmem_quad_get(pq[i >> 2], i & 3), mb[i]);
+            if (i < 8 || leader) st_pair(out + inter_pair_index(g, a, p, j + TPL * i), tmem_getc(pq[i / CH], i % CH, T()), mb[i]);
         }
       };
       {
-        cplx<T> mb[12];
+        cplx<T> mb[NB];
 #pragma unroll
-        for (int i = 0; i < 12; ++i) mb[i] = (i < 8 || (i == 8 && leader)) ? merged(i < 9 ? i : 8) : mk<T>(0, 0);
+        for (int i = 0; i < NB; ++i) mb[i] = (i < 8 || (i == 8 && leader)) ? merged(i < 9 ? i : 8) : mk<T>(0, 0);
         tmem_wait_st();
         emit(byte_off(outB, mo), tparkB, mb);                                          // B~ = Gx~
       }
@@ -263,20 +268,20 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       }
       {
         tmem_wait_st();
-        TmemQuad sq[4];
+        TmemQuad sq[NCH];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) tmem_ld4_issue(tstash + 16 * q, sq[q]);
+        for (int q = 0; q < NCH; ++q) tmem_ldc_issue(tstash + 16 * q, sq[q]);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) tmem_wait_ld(sq[q]);
+        for (int q = 0; q < NCH; ++q) tmem_wait_ld(sq[q]);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) V[k] = tmem_quad_get(sq[k >> 2], k & 3);       // S'
+        for (int k = 0; k < 16; ++k) V[k] = tmem_getc(sq[k / CH], k % CH, T());     // S'
       }
       fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
       __syncthreads();
       {
-        cplx<T> mb[12];
+        cplx<T> mb[NB];
 #pragma unroll
-        for (int i = 0; i < 12; ++i) {
+        for (int i = 0; i < NB; ++i) {
           mb[i] = mk<T>(0, 0);
           if (i < 8 || (i == 8 && leader)) {
             mb[i] = merged(i < 9 ? i : 8) + ikg[i < 9 ? i : 8];

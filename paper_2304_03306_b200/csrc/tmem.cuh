@@ -47,8 +47,9 @@ __device__ __forceinline__ void tmem_ld16(unsigned taddr, unsigned (&r)[16]) {
                : "memory");
 }
 
-// four complex doubles <-> 16 columns
-__device__ __forceinline__ void tmem_st4(unsigned taddr, const cplx<double>* v) {
+// 16 columns hold TmemPack<T>::CH complex values of the calling thread: four complex doubles or eight complex floats
+template <typename T> struct TmemPack { static constexpr int CH = 16 / (2 * (int)sizeof(T) / 4); };
+__device__ __forceinline__ void tmem_stc(unsigned taddr, const cplx<double>* v) {
   unsigned r[16];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -57,8 +58,14 @@ __device__ __forceinline__ void tmem_st4(unsigned taddr, const cplx<double>* v) 
   }
   tmem_st16(taddr, r);
 }
+__device__ __forceinline__ void tmem_stc(unsigned taddr, const cplx<float>* v) {
+  unsigned r[16];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { r[2 * i] = __float_as_uint(v[i].x); r[2 * i + 1] = __float_as_uint(v[i].y); }
+  tmem_st16(taddr, r);
+}
 struct TmemQuad { unsigned r[16]; };
-__device__ __forceinline__ void tmem_ld4_issue(unsigned taddr, TmemQuad& q) { tmem_ld16(taddr, q.r); }
+__device__ __forceinline__ void tmem_ldc_issue(unsigned taddr, TmemQuad& q) { tmem_ld16(taddr, q.r); }
 // tcgen05.ld is asynchronous: its registers are valid after tcgen05.wait::ld.  The registers are in/out operands of the wait, so
 // that no use of them can be scheduled above it.
 __device__ __forceinline__ void tmem_wait_ld(TmemQuad& q) {
@@ -68,9 +75,12 @@ __device__ __forceinline__ void tmem_wait_ld(TmemQuad& q) {
                :
                : "memory");
 }
-// after tmem_wait_ld(q)
-__device__ __forceinline__ cplx<double> tmem_quad_get(const TmemQuad& q, int i) {
+// value i of the 16 columns, after tmem_wait_ld(q); the last argument selects the scalar type
+__device__ __forceinline__ cplx<double> tmem_getc(const TmemQuad& q, int i, double) {
   return mk<double>(__hiloint2double((int)q.r[4 * i + 1], (int)q.r[4 * i + 0]), __hiloint2double((int)q.r[4 * i + 3], (int)q.r[4 * i + 2]));
+}
+__device__ __forceinline__ cplx<float> tmem_getc(const TmemQuad& q, int i, float) {
+  return mk<float>(__uint_as_float(q.r[2 * i]), __uint_as_float(q.r[2 * i + 1]));
 }
 
 }  // namespace ttsh

@@ -629,8 +629,8 @@ def test_other_dealias_fractions_match_oracle(ttsh, num, den, Nx, Ny):
 
 @pytest.mark.parametrize("Nx,Ny,dtype", [(8192, 64, "f64"), (8192, 64, "f32"), (64, 8192, "f64"), (64, 8192, "f32")])
 def test_maximum_grid_dimension_8192(ttsh, Nx, Ny, dtype):
-    """Nx = 8192 (fp64: the real-row fused kernel k_row_step_real, one real row per half-length transform; fp32: the fused
-    row-pair kernel) and Ny = 8192 (4096-point half-length column transforms), 3 steps against the FFT-backed oracle."""
+    """Nx = 8192 (the real-row fused kernel k_row_step_real, one real row per half-length transform, in both precisions) and
+    Ny = 8192 (4096-point half-length column transforms), 3 steps against the FFT-backed oracle."""
     dx, dt = 0.5, 0.01
     mask = workloads.disk_mask(Nx, Ny, dx, 12.0)
     vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 6, amplitude=1.0)
@@ -641,41 +641,46 @@ def test_maximum_grid_dimension_8192(ttsh, Nx, Ny, dtype):
     s.close()
 
 
-@pytest.mark.parametrize("which,Ny", [("baseline", 128), ("paper", 512)])
-def test_real_row_fused_kernel_nx8192_fp64(ttsh, which, Ny):
-    """k_row_step_real (Nx = 8192 in fp64: the paper's production width): the 4-launch step against the oracle-fft for 1
-    and 10 steps, against the unfused 6-launch sequence of the same library (same arithmetic per point up to the order of the
-    real-data split / merge), and with a mean flow in both components (the m = 0 bins of the split take their own branch)."""
+@pytest.mark.parametrize("which,Ny,dtype", [("baseline", 128, "f64"), ("paper", 512, "f64"), ("baseline", 256, "f32")])
+def test_real_row_fused_kernel_nx8192(ttsh, which, Ny, dtype):
+    """k_row_step_real (Nx = 8192, the paper's production width; in fp64 a packed row pair does not fit in shared memory,
+    in fp32 the warp-local plan at N = 4096 beats the four-stage plan at 8192): against the oracle-fft for 1 and 10 steps, against the
+    unfused 6-launch sequence of the same library (same arithmetic per point up to the order of the real-data split / merge), and
+    with a mean flow in both components (the m = 0 bins of the split take their own branch)."""
     Nx, dx, dt = 8192, 0.5, 0.01
+    f64 = dtype == "f64"
     mask = workloads.disk_mask(Nx, Ny, dx, 0.3 * Ny * dx)
     vel = workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 21, amplitude=1.0, nmodes=16)
     g = workloads.gaussian_velocity(Nx, Ny, workloads.SEED0 + 21, 1e-2, mask)
     vel = (vel[0] + g[0] + 0.15, vel[1] + g[1] - 0.1)
-    s, o = make_pair(ttsh, Nx, Ny, dx, dt, which, mask, transform="c", vel=vel)
+    s, o = make_pair(ttsh, Nx, Ny, dx, dt, which, mask, dtype=dtype, transform="c", vel=vel)
     l0 = s.launch_count()
     s.step(1); o.step(1)
     assert s.launch_count() - l0 == 3, "k_inv_col (the intermediates are not at hand yet), k_row_step_real, k_col_step (Ny <= 1024)"
-    compare_state(s, o, TOL_F64_1, f"8192x{Ny} {which} step 1")
+    compare_state(s, o, TOL_F64_1 if f64 else TOL_F32_1, f"8192x{Ny} {which} {dtype} step 1")
     l0 = s.launch_count()
     s.step(3); o.step(3)
     assert s.launch_count() - l0 == 1 + 3 * 2, "get_fields used the scratch arrays: k_inv_col once, then two launches per step"
-    s.step(6); o.step(6)
-    compare_state(s, o, TOL_F64_100, f"8192x{Ny} {which} step 10")
-    cx, cy = (Nx // 2) * dx, (Ny // 2) * dx
-    d, od = s.diagnostics(cx, cy), o.diagnostics(cx, cy)
-    for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy", "mean_vx", "mean_vy"):
-        assert abs(d[key] - od[key]) <= TOL_DIAG * max(abs(od[key]), 1e-300), key
+    if f64:
+        s.step(6); o.step(6)
+        compare_state(s, o, TOL_F64_100, f"8192x{Ny} {which} step 10")
+        cx, cy = (Nx // 2) * dx, (Ny // 2) * dx
+        d, od = s.diagnostics(cx, cy), o.diagnostics(cx, cy)
+        for key in ("sum_speed", "sum_abs_vtheta", "kinetic_energy", "enstrophy", "mean_vx", "mean_vy"):
+            assert abs(d[key] - od[key]) <= TOL_DIAG * max(abs(od[key]), 1e-300), key
+    else:
+        compare_state(s, o, 3 * TOL_F32_1, f"8192x{Ny} f32 step 4")
     # the same step through the unfused passes of the library
     gp, _ = params_pair(ttsh, which)
-    a = ttsh.Solver(Nx, Ny, dx, dt, gp, "f64", mask=mask)
-    b = ttsh.Solver(Nx, Ny, dx, dt, gp, "f64", mask=mask)
+    a = ttsh.Solver(Nx, Ny, dx, dt, gp, dtype, mask=mask)
+    b = ttsh.Solver(Nx, Ny, dx, dt, gp, dtype, mask=mask)
     a.set_velocity(*vel); b.set_velocity(*vel)
     a.step(1)
     for st in (ttsh.TTSH_STAGE_INV_COL, ttsh.TTSH_STAGE_INV_ROW, ttsh.TTSH_STAGE_REAL, ttsh.TTSH_STAGE_FWD_ROW,
                ttsh.TTSH_STAGE_FWD_COL, ttsh.TTSH_STAGE_SPECTRAL):
         b.run_stage(st)
     for x, y, name in zip(gpu_fields(a), gpu_fields(b), ("vx", "vy", "w", "psi")):
-        assert rel(x, y) <= 1e-13, name
+        assert rel(x, y) <= (1e-13 if f64 else 2e-5), name
     s.close(); a.close(); b.close()
 
 

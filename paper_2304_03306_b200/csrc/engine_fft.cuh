@@ -220,8 +220,8 @@ template <typename T> cudaError_t prepare_rows(const Geom& g) {
 namespace ttsh {
 // Nx = 8192 (fp64: a packed row pair does not fit in shared memory; fp32: faster): one real row per half-length transform (row_step_real.cuh);
 // K in the thread order of that kernel (launch_reperm_real), table = fill_stage_tables_real
-template <typename T, int NX> constexpr bool row_step_real_enabled() { return NX == 8192; }
-__host__ __device__ constexpr int row_step_real_tabr_offset(int M) { return (fft_wl_tw_elems_rt(M) + 15) / 16 * 16; }
+template <typename T, int NX> constexpr bool row_step_real_enabled() { return NX == 8192 || (NX == 16384 && sizeof(T) == 4); }
+__host__ __device__ constexpr int row_step_real_tabr_offset(int M) { return ((M == 4096 ? fft_wl_tw_elems_rt(M) : fft_tw_elems_rt(M) + 1) + 15) / 16 * 16; }
 template <typename T, int NX, bool ENS> static cudaError_t prep_row_step_real(int* slots) {
   using C = RowStepRealCfg<T, NX>;
   static_assert(C::FITS, "row_step_real: line, stash, table and the K slot must fit in shared memory");
@@ -287,6 +287,12 @@ static cudaError_t go_row_step(const Geom& g, const Model& m, const void* inW, c
 }
 template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, int* slots_ens, int* slots_tan) {
   *slots = *slots_ens = *slots_tan = 0;
+  if constexpr (row_step_real_enabled<T, TTSH_REAL_ROW_NX>()) {
+    if (g.Nx == TTSH_REAL_ROW_NX) {
+      cudaError_t e = prep_row_step_real<T, TTSH_REAL_ROW_NX, false>(slots); if (e != cudaSuccess) return e;
+      return prep_row_step_real<T, TTSH_REAL_ROW_NX, true>(slots_ens);
+    }
+  }
   switch (g.Nx) {
 #define X(N) case N: { cudaError_t e = prep_row_step<T, N, row_step_ens_lines<N>(), true, true>(slots_tan); if (e != cudaSuccess) return e; \
                        if constexpr (row_step_real_enabled<T, N>()) { \
@@ -302,6 +308,9 @@ template <typename T> cudaError_t prepare_row_step(const Geom& g, int* slots, in
 }
 template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                   const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int slots) {
+  if constexpr (row_step_real_enabled<T, TTSH_REAL_ROW_NX>()) {
+    if (g.Nx == TTSH_REAL_ROW_NX) return go_row_step_real<T, TTSH_REAL_ROW_NX, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots);
+  }
   switch (g.Nx) {
 #define X(N) case N: if constexpr (row_step_real_enabled<T, N>()) return go_row_step_real<T, N, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots); \
                      else return go_row_step<T, N, 1, false>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, 1, 0, slots);
@@ -313,6 +322,9 @@ template <typename T> cudaError_t launch_row_step(const Geom& g, const Model& m,
 template <typename T> cudaError_t launch_row_step_ens(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi,
                                                       const void* K, void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s,
                                                       int members, size_t mstride, int slots) {
+  if constexpr (row_step_real_enabled<T, TTSH_REAL_ROW_NX>()) {
+    if (g.Nx == TTSH_REAL_ROW_NX) return go_row_step_real<T, TTSH_REAL_ROW_NX, true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots);
+  }
   switch (g.Nx) {
 #define X(N) case N: if constexpr (row_step_real_enabled<T, N>()) return go_row_step_real<T, N, true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots); \
                      else return go_row_step<T, N, row_step_ens_lines<N>(), true>(g, m, inW, inVx, inPsi, K, oA, oB, tab, v0, s, members, mstride, slots);
@@ -333,11 +345,12 @@ template <typename T> cudaError_t launch_row_step_tan(const Geom& g, const Model
   return cudaErrorInvalidValue;
 }
 template <typename T> bool row_step_is_real(const Geom& g) {
-  return row_step_supported<T>(g) && g.Nx == 8192;
+  return row_step_supported<T>(g) && (g.Nx == 8192 || g.Nx == TTSH_REAL_ROW_NX);
 }
 template <typename T> int row_step_real_tabr(const Geom& g) { return row_step_real_tabr_offset(g.Nx / 2); }
 template <typename T> bool row_step_supported(const Geom& g) {
   if (4 * (g.Wx - 1) != g.Nx) return false;          // 1/2 rule only
+  if (g.Nx == TTSH_REAL_ROW_NX) return row_step_real_enabled<T, TTSH_REAL_ROW_NX>();
   switch (g.Nx) {
 #define X(N) case N: return RowStepCfg<T, N>::FITS || row_step_real_enabled<T, N>();
     TTSH_FOR_SIZES(X)

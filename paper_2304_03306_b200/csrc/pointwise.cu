@@ -60,7 +60,7 @@ template <typename T> cudaError_t launch_permute(int Nx, size_t n, const void* i
 }
 template <typename T> cudaError_t launch_reperm_real(int Nx, size_t n, const void* in, void* out, cudaStream_t s) {
   if (Nx < 512) return cudaErrorInvalidValue;
-  k_reperm_real<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(Nx, n, (const T*)in, (T*)out);
+  k_reperm_real<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(Nx, n, (const T*)in, (T*)out, Nx == 8192 ? 1 : 0, Nx == 16384 ? 1 : 0);
   return cudaGetLastError();
 }
 template <typename T> cudaError_t launch_reperm_wl(int Nx, size_t n, const void* in, void* out, cudaStream_t s) {

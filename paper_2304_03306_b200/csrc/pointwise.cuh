@@ -257,16 +257,18 @@ __global__ void k_reperm_wl(int Nx, size_t n, const T* __restrict__ in, T* __res
   }
 }
 
-// K for row_step_real.cuh: slot n = wl_j(t) + TPL k of thread t (TPL = Nx/32 threads, wl_j(t) = (t >> 4) + (TPL/16) (t & 15)) holds the
-// points x = 2n, 2n+1 of the row;  out[y Nx + (k TPL + t) 2 + par] = K(y, 2n + par)
+// K for row_step_real.cuh: slot n = own(t) + TPL k of thread t (TPL = Nx/32 threads; own(t) = wl_j(t) = (t >> 4) + (TPL/16) (t & 15) for the
+// warp-local plan, t for the plain plan) holds the points x = 2n, 2n+1 of the row;  out[y Nx + (k TPL + t) 2 + par] = K(y, 2n + par).
+// natural: the source rows are in natural order (Nx = 16384), else in the permuted internal layout (perm_index).
 template <typename T>
-__global__ void k_reperm_real(int Nx, size_t n, const T* __restrict__ in, T* __restrict__ out) {
+__global__ void k_reperm_real(int Nx, size_t n, const T* __restrict__ in, T* __restrict__ out, int wl, int natural) {
   const int tpl_in = Nx / 16, TPL = Nx / 32, r1 = TPL / 16;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const size_t row = i / (size_t)Nx;
     const int e = (int)(i - row * (size_t)Nx), par = e & 1, t = (e >> 1) % TPL, k = (e >> 1) / TPL;
-    const int x = 2 * ((t >> 4) + r1 * (t & 15) + TPL * k) + par;
-    out[i] = in[row * Nx + perm_index(x, tpl_in)];
+    const int own = wl ? (t >> 4) + r1 * (t & 15) : t;     // warp-local plan: wl_j(t); plain plan: t
+    const int x = 2 * (own + TPL * k) + par;
+    out[i] = in[row * Nx + (natural ? x : perm_index(x, tpl_in))];
   }
 }
 

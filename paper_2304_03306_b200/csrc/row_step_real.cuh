@@ -1,9 +1,13 @@
-// row_step_real.cuh — the row half of one Euler step in ONE kernel (row_step.cuh) for Nx = 8192, the paper's production width
-// (PAPER.md:71, :271).  In fp64 a packed row PAIR (128 KB per field) no longer fits in shared memory; in fp32 it does, but the
-// four-stage plan of an 8192-point transform is slower than what follows (8192^2 fp32: 749 -> 589 us for the row kernel).
+// row_step_real.cuh — the row half of one Euler step in ONE kernel (row_step.cuh) on ONE REAL ROW per transform:
+//   Nx = 8192, the paper's production width.  In fp64 a packed row PAIR (128 KB per field) no longer fits in shared
+//              memory; in fp32 it does, but the four-stage plan of an 8192-point transform is slower than what follows (8192^2 fp32:
+//              749 -> 589 us for the row kernel).  256 threads, warp-local plan at M = Nx/2 = 4096.
+//   Nx = 16384 in fp32 (the grid of Fig. 6(f); in fp64 a line of M = 8192 complex doubles does not leave room for the
+//              staging slots): 512 threads x 128 registers, plain four-stage plan, BOTH waiting fields in tensor memory.
+//              16384 x 4096 fp32: 1.76 ms per step with the 6-launch sequence of fft_rows_real.cuh, 1.17 ms with this kernel.
 //
 // One REAL row is transformed as a half-length complex sequence z[n] = f(2n) + i f(2n+1), n < M = Nx/2 = 4096 (the textbook
-// real-data FFT), so that the machinery of row_step.cuh applies unchanged at N = 4096: the warp-local plan of fft_core.cuh, one
+// real-data FFT), so that the machinery of row_step.cuh applies unchanged at N = M: the transform plans of fft_core.cuh, one
 // field live in registers (V), one waiting in registers (H), one parked by its owner thread (there: a shared-memory stash; here:
 // tensor memory).  The pointwise stage
 // (lines 1-2 of Algorithm 1) does not care that a complex slot now holds two neighbouring points of one row
@@ -36,20 +40,27 @@ namespace ttsh {
 
 template <typename T, int NX> struct RowStepRealCfg {
   static constexpr int M = NX / 2;                                  // complex length
-  static constexpr bool OK = fft_wl_supported<M>();
+  static constexpr bool WL = fft_wl_supported<M>();                 // warp-local plan (M = 4096), else the plain Stockham plan (M = 8192)
   static constexpr int TPL = M / 16, THREADS = TPL;
-  static constexpr int LS = fft_wl_line_elems<T, M>() + 4;
-  // tensor memory (tmem.cuh), per thread: 64 columns for the waiting field (16 complex values) and 2 x 48 for the merged bins of
-  // the pair's first row (B~ and A~, 9 complex values each in three 4-value pieces); two warps per lane quarter -> 2 x 160 <= 512
+  static constexpr int LS = (WL ? fft_wl_line_elems<T, M>() : fft_line_elems<M>()) + 4;
+  // tensor memory (tmem.cuh), per thread: the waiting field (16 complex values) and the merged bins of the pair's first row (B~ and
+  // A~, 9 complex values each), in pieces of 16 columns = 4 complex doubles / 8 complex floats; THREADS / 128 warps per lane quarter
   static constexpr unsigned TMEM_COLS = 512;
-  static constexpr int TMEM_PER_WARP = 256;
+  static constexpr int TMEM_PER_WARP = 512 / (THREADS / 128);
+  static constexpr int CH = 16 / (2 * (int)sizeof(T) / 4);
+  // the 512-thread variant (M = 8192) has 128 registers per thread: its second waiting field (v_x, then Gy) is parked as well
+  static constexpr bool HTM = THREADS > 256;
+  static constexpr int TMEM_NEED = (HTM ? 2 : 1) * 16 * (16 / CH) + 2 * 16 * ((9 + CH - 1) / CH);
   static constexpr size_t OFF_TAB = (size_t)LS * sizeof(cplx<T>);
+  // a copy of the warp-local table in shared memory in fp64 (row_step.cuh, SMEM_TAB, says why); fp32 and the plain plan read it through L1
+  static constexpr bool SMEM_TAB = WL && sizeof(T) == 8;
+  static constexpr size_t TAB_BYTES = SMEM_TAB ? (size_t)fft_wl_tw_elems_rt(M) * sizeof(cplx<T>) : 0;
   // two staging slots, used in turn by the (A, B) pairs of w~, v_x~, psi~ (2 Wxp <= 2 (NX/4 + 8) complex values) and by the row of K
   static constexpr size_t SLOT = ((size_t)(NX / 4 + 8) * 2 * sizeof(cplx<T>) + 127) / 128 * 128;
-  static constexpr size_t OFF_SLOTS = (OFF_TAB + (size_t)fft_wl_tw_elems_rt(M) * sizeof(cplx<T>) + 127) / 128 * 128;
+  static constexpr size_t OFF_SLOTS = (OFF_TAB + TAB_BYTES + 127) / 128 * 128;
   static constexpr size_t OFF_BAR = OFF_SLOTS + 2 * SLOT;
   static constexpr size_t SMEM = OFF_BAR + 32;
-  static constexpr bool FITS = OK && SMEM <= 227 * 1024;
+  static constexpr bool FITS = THREADS % 128 == 0 && THREADS <= 1024 && TMEM_NEED <= TMEM_PER_WARP && SMEM <= 227 * 1024;
 };
 
 // W^m = wj W_32^k for m = j + 256 k (forward sign), k a compile-time constant after unrolling
@@ -58,7 +69,7 @@ template <typename T> __device__ __forceinline__ cplx<T> real_row_tw(cplx<T> wj,
 // inverse transform of one real row into registers: out[k] = f(2n) + i f(2n+1), n = wl_j(j) + k TPL.
 // row: bin m of this row at row[2 m] (its half of the staged (A, B) pairs of the inverse intermediate, shared memory).
 // MODE = RM_ONE or RM_NIKX_MEANY (ttsh_common.cuh).  1/2 rule only: retained m = 0..M/2.
-template <typename T, int M, int MODE, class Hook>
+template <typename T, int M, bool WL, int MODE, class Hook>
 __device__ __forceinline__ void inv_real_row_regs(const cplx<T>* __restrict__ row, int j, cplx<T> wj, cplx<T>* __restrict__ line,
                                                   const cplx<T>* __restrict__ tab, T scale, T dkx, T meany, cplx<T> (&out)[16], Hook hook) {
   constexpr int TPL = M / 16;
@@ -84,7 +95,8 @@ __device__ __forceinline__ void inv_real_row_regs(const cplx<T>* __restrict__ ro
     return scale * (mid ? mk<T>(c.x + c.x, c.y + c.y) : z);
   };
   auto store = [&](int, int k, cplx<T> z) { out[k] = z; };
-  fft_line_wl<T, M, +1, false>(j, j, line, tab, make_loader<1>(issue, finish), store, hook);
+  if constexpr (WL) fft_line_wl<T, M, +1, false>(j, j, line, tab, make_loader<1>(issue, finish), store, hook);
+  else fft_line<T, M, +1, false>(j, line, tab, make_loader<1>(issue, finish), store, hook);
 }
 
 // ENS: the persistent grid runs over the row pairs of `members` systems whose workspaces lie mstride bytes apart; rpm = Ny/2.
@@ -97,10 +109,11 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
                 const cplx<T>* __restrict__ tabR, const double* __restrict__ v0, int nblk, int rpm, size_t mstride) {
   using C = RowStepRealCfg<T, NX>;
   constexpr int M = C::M, TPL = C::TPL;
+  constexpr bool WL = C::WL;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx<T>* line = reinterpret_cast<cplx<T>*>(smem_raw);
   const int j = threadIdx.x;
-  const int jw = fft_wl_j<M>(j);                                   // the thread owns slots n = jw + k TPL
+  const int jw = WL ? (j >> 4) + (M / 256) * (j & 15) : j;         // the thread owns slots n = jw + k TPL
   cplx<T>* stab = reinterpret_cast<cplx<T>*>(smem_raw + C::OFF_TAB);
   unsigned char* slot0 = smem_raw + C::OFF_SLOTS;
   unsigned char* slot1 = slot0 + C::SLOT;
@@ -126,7 +139,7 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   if (j < 32) tmem_alloc(tmem_holder, C::TMEM_COLS);
   tmem_fence_before_sync();
   // the table of the warp-local plan: a copy in shared memory in fp64, through L1 in fp32 (row_step.cuh, SMEM_TAB, says why)
-  if constexpr (sizeof(T) == 8) {
+  if constexpr (C::SMEM_TAB) {
     for (int i = j; i < fft_wl_tw_elems_rt(M); i += C::THREADS) stab[i] = ldg_c(tabW + i);     // host-written at ttsh_create
   } else stab = const_cast<cplx<T>*>(tabW);
   const cplx<T> wj = ldg_c(tabR + j);                              // W_NX^j
@@ -134,7 +147,9 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
   tmem_fence_after_sync();
   const unsigned tmem_base = *tmem_holder;
   const unsigned tstash = tmem_warp_addr(tmem_base, j >> 5, C::TMEM_PER_WARP * (j >> 7));   // this thread's columns: slot k of the waiting field at column 4 k
-  const unsigned tparkB = tstash + 16 * NCH, tparkA = tparkB + 16 * NBP;         // merged B~ / A~ bins of the pair's first row
+  constexpr bool HTM = C::HTM;
+  const unsigned tH = tstash + 16 * NCH;                                         // v_x, then Gy (HTM only)
+  const unsigned tparkB = tH + (HTM ? 16 * NCH : 0), tparkA = tparkB + 16 * NBP; // merged B~ / A~ bins of the pair's first row
   pdl_wait();          // inputs, K and v0 below are written by the preceding launches
   pdl_trigger();
   T meany = (T)0;
@@ -172,59 +187,72 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       // (row pair, member offset) of the row after this one
       int xrp = rp; size_t xmo = mo; bool xok = true;
       if (r == 1) { xok = nb < nblk; if (xok) locate(nb, xrp, xmo); }
-      cplx<T> H[16], V[16];
+      cplx<T> H[HTM ? 1 : 16], V[16];
       // ---- a2 / a6: w, v_x, v_y of the row ----
       mbar_wait(bar0, ph0); ph0 ^= 1;
-      inv_real_row_regs<T, M, RM_ONE>(row0, j, wj, line, stab, scale_i, dkx, meany, V,
+      inv_real_row_regs<T, M, WL, RM_ONE>(row0, j, wj, line, stab, scale_i, dkx, meany, V,
                                       [&]() { if (leader) bulk_load(slot0, byte_off(inPsi, mo) + (size_t)rp * in_stride, in_bytes, bar0); });
 #pragma unroll
       for (int q = 0; q < NCH; ++q) tmem_stc(tstash + 16 * q, V + CH * q);   // w waits in tensor memory
       mbar_wait(bar1, ph1); ph1 ^= 1;
-      inv_real_row_regs<T, M, RM_ONE>(row1, j, wj, line, stab, scale_i, dkx, meany, H,
-                                      [&]() { if (leader) bulk_load(slot1, byte_off(K2, mo) + y * NX, k_bytes, bar1); });                    // v_x
+      if constexpr (HTM) {
+        inv_real_row_regs<T, M, WL, RM_ONE>(row1, j, wj, line, stab, scale_i, dkx, meany, V,
+                                        [&]() { if (leader) bulk_load(slot1, byte_off(K2, mo) + y * NX, k_bytes, bar1); });                  // v_x
+#pragma unroll
+        for (int q = 0; q < NCH; ++q) tmem_stc(tH + 16 * q, V + CH * q);
+      } else {
+        inv_real_row_regs<T, M, WL, RM_ONE>(row1, j, wj, line, stab, scale_i, dkx, meany, H,
+                                        [&]() { if (leader) bulk_load(slot1, byte_off(K2, mo) + y * NX, k_bytes, bar1); });                  // v_x
+      }
       mbar_wait(bar0, ph0); ph0 ^= 1;
-      inv_real_row_regs<T, M, RM_NIKX_MEANY>(row0, j, wj, line, stab, scale_i, dkx, meany, V, [&]() {                                        // v_y
+      inv_real_row_regs<T, M, WL, RM_NIKX_MEANY>(row0, j, wj, line, stab, scale_i, dkx, meany, V, [&]() {                                        // v_y
         if (leader && xok) bulk_load(slot0, byte_off(inW, xmo) + (size_t)xrp * in_stride, in_bytes, bar0);
       });
       // ---- a3: lines 1-2 of Algorithm 1 on the two points of every slot;  V <- Gx,  H <- Gy,  tensor memory <- S' ----
       mbar_wait(bar1, ph1); ph1 ^= 1;
       tmem_wait_st();
       {
-        TmemQuad wq[2];
+        TmemQuad wq[2], uq;
         tmem_ldc_issue(tstash, wq[0]);
 #pragma unroll
         for (int q = 0; q < NCH; ++q) {
+          if constexpr (HTM) tmem_ldc_issue(tH + 16 * q, uq);
           tmem_wait_ld(wq[q & 1]);
+          if constexpr (HTM) tmem_wait_ld(uq);
           if (q < NCH - 1) tmem_ldc_issue(tstash + 16 * (q + 1), wq[(q + 1) & 1]);
-          cplx<T> s4[CH];
+          cplx<T> s4[CH], g4[CH];
 #pragma unroll
           for (int i = 0; i < CH; ++i) {
             const int k = CH * q + i;
             const cplx<T> kk = kslot[k * TPL + j];
             const cplx<T> w = tmem_getc(wq[q & 1], i, T());
             const T kA = kk.x, kB = kk.y;
-            const T vxA = H[k].x, vxB = H[k].y, vyA = V[k].x, vyB = V[k].y;
+            cplx<T> vx;
+            if constexpr (HTM) vx = tmem_getc(uq, i, T()); else vx = H[k];
+            const T vxA = vx.x, vxB = vx.y, vyA = V[k].x, vyB = V[k].y;
             const T ccA = scale_f * (-beta * (vxA * vxA + vyA * vyA) - gv * kA);
             const T ccB = scale_f * (-beta * (vxB * vxB + vyB * vyB) - gv * kB);
             const T lwA = scale_f * lam * w.x, lwB = scale_f * lam * w.y;
             V[k] = mk<T>(ccA * vxA + lwA * vyA, ccB * vxB + lwB * vyB);          // Gx
-            H[k] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);          // Gy
+            g4[i] = mk<T>(ccA * vyA - lwA * vxA, ccB * vyB - lwB * vxB);         // Gy
+            if constexpr (!HTM) H[k] = g4[i];
             s4[i] = mk<T>(ngw * (kA * w.x), ngw * (kB * w.y));                   // S'
           }
           tmem_stc(tstash + 16 * q, s4);
+          if constexpr (HTM) tmem_stc(tH + 16 * q, g4);
         }
       }
       // ---- a4: three forward transforms, each merged into the half spectrum of the row on the bins k = j + 256 i ----
       auto ident = [&](int, int, cplx<T> z) -> cplx<T> { return z; };
-      auto to_line = [&](int mm, int, cplx<T> z) { line[fft_wl_pad<T, M>(mm)] = z; };
+      auto to_line = [&](int mm, int, cplx<T> z) { line[row_step_pad<T, M, WL>(mm)] = z; };
       auto merged = [&](int i) -> cplx<T> {                          // F(k), k = j + 256 i
         const int k = j + TPL * i;
-        const cplx<T> zp = line[fft_wl_pad<T, M>(k)];
-        const cplx<T> zm = conj(line[fft_wl_pad<T, M>((M - k) & (M - 1))]);
+        const cplx<T> zp = line[row_step_pad<T, M, WL>(k)];
+        const cplx<T> zm = conj(line[row_step_pad<T, M, WL>((M - k) & (M - 1))]);
         const cplx<T> e = (T)0.5 * (zp + zm), o = (T)0.5 * mul_ni(zp - zm);
         return e + real_row_tw(wj, i) * o;
       };
-      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line, [&]() {
+      fwd_row_regs<T, M, true, WL>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line, [&]() {
         if (!leader || !xok) return;                           // K has been consumed: stage v_x~ of the next row
         bulk_load(slot1, byte_off(inVx, xmo) + (size_t)xrp * in_stride, in_bytes, bar1);
       });
@@ -255,7 +283,22 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
       }
       cplx<T> ikg[9];
       T gy0 = (T)0;
-      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), to_line);
+      auto unpark = [&](unsigned tp) {                               // V <- the field parked at tp
+        tmem_wait_st();
+        TmemQuad sq[NCH];
+#pragma unroll
+        for (int q = 0; q < NCH; ++q) tmem_ldc_issue(tp + 16 * q, sq[q]);
+#pragma unroll
+        for (int q = 0; q < NCH; ++q) tmem_wait_ld(sq[q]);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) V[k] = tmem_getc(sq[k / CH], k % CH, T());
+      };
+      if constexpr (HTM) {
+        unpark(tH);                                                  // Gy
+        fwd_row_regs<T, M, true, WL>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
+      } else {
+        fwd_row_regs<T, M, true, WL>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return H[k]; }, ident), to_line);
+      }
       __syncthreads();
 #pragma unroll
       for (int i = 0; i < 9; ++i) {
@@ -266,17 +309,8 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
           ikg[i] = (dkx * (T)(j + TPL * i)) * mul_i(gy);
         }
       }
-      {
-        tmem_wait_st();
-        TmemQuad sq[NCH];
-#pragma unroll
-        for (int q = 0; q < NCH; ++q) tmem_ldc_issue(tstash + 16 * q, sq[q]);
-#pragma unroll
-        for (int q = 0; q < NCH; ++q) tmem_wait_ld(sq[q]);
-#pragma unroll
-        for (int k = 0; k < 16; ++k) V[k] = tmem_getc(sq[k / CH], k % CH, T());     // S'
-      }
-      fwd_row_regs<T, M, true, true>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
+      unpark(tstash);                                                // S'
+      fwd_row_regs<T, M, true, WL>(jw, j, line, stab, make_loader<1>([&](int, int k) -> cplx<T> { return V[k]; }, ident), to_line);
       __syncthreads();
       {
         cplx<T> mb[NB];

@@ -102,6 +102,7 @@ struct ttsh_handle {
   int rs_slots, rs_slots_ens, rs_slots_tan;   // persistent grid of k_row_step on this device (single system / ensemble / tangent variant)
   bool row_step_ok;     // the fused row-step kernel supports this grid / dtype / dealias fraction
   bool row_step_wl;     // ... and runs the warp-local FFT plan (thread-order K copy, warp-local twiddle table)
+  void* rs_tab;         // the twiddle table the fused row kernel of this grid reads (tabX, or tabXw for the warp-local / real-row variants)
   bool col_step_ok;     // the fused column kernel (col_step.cuh) applies: an Euler step is k_row_step + k_col_step
   bool inter_valid;     // ... and the inverse intermediates Tm[0], Tm[2], Tm[3] of the CURRENT state are at hand (k_col_step of the
                         //     previous step wrote them); cleared by everything that touches the state or the scratch arrays
@@ -330,7 +331,7 @@ int enqueue_stage(ttsh_handle* h, int stage) {
     case TTSH_STAGE_ROW_STEP:         // a2/a6 row pass + a3 + a4 row pass in one kernel (conservative form, 1/2 rule)
       if (h->advection_form != TTSH_ADVECTION_CONSERVATIVE || !h->row_step_ok) return TTSH_ERR_INVALID_ARG;
       TRY(h, DISPATCH(h, launch_row_step, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
-                      (h->row_step_wl || h->row_step_real) ? h->tabXw : h->tabX, h->v0, h->stream, h->rs_slots));
+                      h->rs_tab, h->v0, h->stream, h->rs_slots));
       h->launches++;
       return TTSH_OK;
     case TTSH_STAGE_COL_STEP:         // a4 column pass + a5 + the column pass of a2 / a6 of the next step in one kernel
@@ -361,7 +362,7 @@ int enqueue_step(ttsh_handle* h) {
                               TTSH_STAGE_SPECTRAL};
   // conservative form: 4 launches where the fused row-step kernel applies, else 5 (fused real-space + forward row pass); the
   // literal form and Nx = 16384 (real-row passes, no fused row kernels) run the 6-launch sequence
-  const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows;
+  const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE && (!h->real_rows || h->row_step_real);
   if (f && h->col_step_ok) {      // two launches per step; the column pass of a2 / a6 only when its output is not at hand
     int rc = TTSH_OK;
     if (!h->inter_valid) rc = enqueue_stage(h, TTSH_STAGE_INV_COL);
@@ -379,8 +380,9 @@ int enqueue_step(ttsh_handle* h) {
   return TTSH_OK;
 }
 inline int launches_per_step(const ttsh_handle* h) {
-  if (h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows && h->col_step_ok) return 2;
-  return (h->advection_form == TTSH_ADVECTION_CONSERVATIVE && !h->real_rows) ? (h->row_step_ok ? 4 : 5) : 6;
+  const bool f = h->advection_form == TTSH_ADVECTION_CONSERVATIVE && (!h->real_rows || h->row_step_real);
+  if (f && h->col_step_ok) return 2;
+  return f ? (h->row_step_ok ? 4 : 5) : 6;
 }
 
 // natural <-> internal row layout of a real field (to_perm = 1: natural -> internal).  On real-row grids the internal layout IS
@@ -475,6 +477,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
   h->row_step_ok = h->dtype == TTSH_F64 ? row_step_supported<double>(h->g) : row_step_supported<float>(h->g);
   h->row_step_real = h->dtype == TTSH_F64 ? row_step_is_real<double>(h->g) : row_step_is_real<float>(h->g);
   h->row_step_wl = Nx == 4096;
+  h->rs_tab = h->row_step_real ? (Nx == 16384 ? h->tabX : h->tabXw) : (h->row_step_wl ? h->tabXw : h->tabX);
   h->real_rows = Nx == 16384;
   h->rs_slots = h->rs_slots_ens = h->rs_slots_tan = 0;
   h->col_step_ok = h->row_step_ok && !h->real_rows &&
@@ -508,7 +511,7 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
     TRY(h, cudaMemcpyAsync(h->tabXw, tr.data(), tr.size(), cudaMemcpyHostToDevice, h->stream));
     TRY(h, cudaStreamSynchronize(h->stream));
   }
-  if (h->row_step_real) {     // warp-local tables of the half-length transform, then W_Nx^j, j < Nx/32
+  if (h->row_step_real && !h->real_rows) {     // warp-local tables of the half-length transform, then W_Nx^j, j < Nx/32
     std::vector<unsigned char> tw;
     const int off = DISPATCH(h, row_step_real_tabr, h->g);
     if (t == TTSH_F64) fill_stage_tables_wl<double>(tw, Nx / 2); else fill_stage_tables_wl<float>(tw, Nx / 2);
@@ -527,6 +530,17 @@ int ttsh_create(ttsh_handle** out, int Nx, int Ny, double dx, double dt, const t
     TRY(h, cudaStreamSynchronize(h->stream));
   }
   TRY(h, cudaMemcpyAsync(h->tabX, tx.data(), tx.size(), cudaMemcpyHostToDevice, h->stream));
+  std::vector<unsigned char> trx;
+  if (h->row_step_real && h->real_rows) {      // Nx = 16384: the fused real-row kernel reads the plain tables of the half-length
+                                               // transform (tabX) followed by W_Nx^j, j < Nx/32
+    const int off = DISPATCH(h, row_step_real_tabr, h->g);
+    trx.assign((size_t)(Nx / 32) * 2 * (size_t)t, 0);
+    for (int j = 0; j < Nx / 32; ++j) {
+      if (t == TTSH_F64) put_twiddle<double>(reinterpret_cast<double*>(trx.data()) + 2 * (size_t)j, j, Nx);
+      else put_twiddle<float>(reinterpret_cast<float*>(trx.data()) + 2 * (size_t)j, j, Nx);
+    }
+    TRY(h, cudaMemcpyAsync(static_cast<char*>(h->tabX) + (size_t)off * 2 * (size_t)t, trx.data(), trx.size(), cudaMemcpyHostToDevice, h->stream));
+  }
   TRY(h, cudaMemcpyAsync(h->tabY, ty.data(), ty.size(), cudaMemcpyHostToDevice, h->stream));
   TRY(h, cudaMemcpyAsync(h->tabS, ts.data(), ts.size(), cudaMemcpyHostToDevice, h->stream));
   TRY(h, cudaMemsetAsync(h->v0, 0, 8 * sizeof(double), h->stream));
@@ -1092,7 +1106,7 @@ static int ensemble_enqueue_step(ttsh_ensemble* e, cudaStream_t stream) {
   const size_t ms = e->mstride;
   if (!e->col_fused) { const int rc = ensemble_enqueue_inv_col(e, stream); if (rc != TTSH_OK) return rc; }
   TRY(h, DISPATCH(h, launch_row_step_ens, h->g, h->m, h->Tm[0], h->Tm[3], h->Tm[2], (h->row_step_wl || h->row_step_real) ? h->K2 : h->K, h->Tm[1], h->Tm[4],
-                  (h->row_step_wl || h->row_step_real) ? h->tabXw : h->tabX, h->v0, stream, B, ms, h->rs_slots_ens));
+                  h->rs_tab, h->v0, stream, B, ms, h->rs_slots_ens));
   if (e->col_fused) {
     TRY(h, DISPATCH(h, launch_col_step, h->g, h->m, h->Tm[1], h->Tm[4], h->what, h->psihat, h->v0, h->Tm[0], h->Tm[2], h->Tm[3], h->tabY, h->tabS,
                     stream, B, ms));

@@ -686,8 +686,8 @@ def test_real_row_fused_kernel_nx8192(ttsh, which, Ny, dtype):
 
 @pytest.mark.parametrize("Nx,Ny,dtype", [(16384, 64, "f64"), (16384, 64, "f32"), (64, 16384, "f64"), (64, 16384, "f32"), (16384, 128, "f64")])
 def test_maximum_grid_dimension_16384(ttsh, Nx, Ny, dtype):
-    """(N, dx) = (16384, 0.0025) is the grid of Fig. 6(f).  Nx = 16384: one real row per half-length transform
-    (fft_rows_real.cuh), 6-launch step; Ny = 16384: 8192-point half-length column transforms, one column per CTA.  Algorithm 2,
+    """(N, dx) = (16384, 0.0025) is the grid of Fig. 6(f).  Nx = 16384: one real row per half-length transform: in
+    fp32 the fused kernel k_row_step_real (4-launch step), in fp64 the passes of fft_rows_real.cuh (6-launch step); Ny = 16384: 8192-point half-length column transforms, one column per CTA.  Algorithm 2,
     the initial projection, 3 steps in both advection forms and the diagnostics against the C oracle-fft."""
     dx, dt = 0.5, 0.01
     mask = workloads.disk_mask(Nx, Ny, dx, 12.0)

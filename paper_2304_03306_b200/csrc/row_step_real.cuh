@@ -6,7 +6,7 @@
 //              staging slots): 512 threads x 128 registers, plain four-stage plan, BOTH waiting fields in tensor memory.
 //              16384 x 4096 fp32: 1.76 ms per step with the 6-launch sequence of fft_rows_real.cuh, 1.17 ms with this kernel.
 //
-// One REAL row is transformed as a half-length complex sequence z[n] = f(2n) + i f(2n+1), n < M = Nx/2 = 4096 (the textbook
+// One REAL row is transformed as a half-length complex sequence z[n] = f(2n) + i f(2n+1), n < M = Nx/2 (the textbook
 // real-data FFT), so that the machinery of row_step.cuh applies unchanged at N = M: the transform plans of fft_core.cuh, one
 // field live in registers (V), one waiting in registers (H), one parked by its owner thread (there: a shared-memory stash; here:
 // tensor memory).  The pointwise stage

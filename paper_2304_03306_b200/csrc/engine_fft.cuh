@@ -222,7 +222,10 @@ namespace ttsh {
 // K in the thread order of that kernel (launch_reperm_real), table = fill_stage_tables_real
 template <typename T, int NX> constexpr bool row_step_real_enabled() { return NX == 8192 || (NX == 16384 && sizeof(T) == 4); }
 __host__ __device__ constexpr int row_step_real_tabr_offset(int M) { return ((M == 4096 ? fft_wl_tw_elems_rt(M) : fft_tw_elems_rt(M) + 1) + 15) / 16 * 16; }
-template <typename T, int NX, bool ENS> static cudaError_t prep_row_step_real(int* slots) {
+// Single systems and ensembles run the SAME instantiation (the member loop of the ensemble variant with one member), so that an
+// ensemble member is bit-identical to the system stepped alone whatever the compiler does with the two variants.
+template <typename T, int NX, bool ENS_> static cudaError_t prep_row_step_real(int* slots) {
+  constexpr bool ENS = true;
   using C = RowStepRealCfg<T, NX>;
   static_assert(C::FITS, "row_step_real: line, stash, table and the K slot must fit in shared memory");
   cudaError_t e = set_smem(k_row_step_real<T, NX, ENS>, C::SMEM);
@@ -233,9 +236,10 @@ template <typename T, int NX, bool ENS> static cudaError_t prep_row_step_real(in
   *slots = sms > 0 ? sms : 148;                                   // one CTA per SM
   return cudaSuccess;
 }
-template <typename T, int NX, bool ENS>
+template <typename T, int NX, bool ENS_>
 static cudaError_t go_row_step_real(const Geom& g, const Model& m, const void* inW, const void* inVx, const void* inPsi, const void* K2,
                                     void* oA, void* oB, const void* tab, const double* v0, cudaStream_t s, int members, size_t mstride, int slots) {
+  constexpr bool ENS = true;
   using C = RowStepRealCfg<T, NX>;
   if (slots <= 0) return cudaErrorInvalidConfiguration;
   const int rpm = g.Ny / 2;

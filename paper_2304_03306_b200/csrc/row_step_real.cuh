@@ -20,8 +20,8 @@
 //               m > M/2:  Z2(m) = c - i conj(W^m) c,  c = conj F(M-m)          m = M/2:  2 conj F(M/2)
 //   forward:  F(k) = E(k) + W^k O(k),  E = (Z(k) + conj Z(M-k)) / 2,  O = -i (Z(k) - conj Z(M-k)) / 2,  k = 0..M/2 (retained).
 //             i k_x does not commute with this step, so the three forward transforms are merged separately and
-//             A~ = i k_x Gy~ + S'~ is formed on the merged bins (a thread merges the same bins k = j + 256 i of every transform).
-//   W^m for m = j + 256 k is W^j W_32^k: one table entry per thread (tabR, W^j for j < 256) and compile-time constants.
+//             A~ = i k_x Gy~ + S'~ is formed on the merged bins (a thread merges the same bins k = j + TPL i of every transform, TPL = M/16).
+//   W^m for m = j + TPL k is W^j W_32^k: one table entry per thread (tabR, W^j for j < TPL) and compile-time constants.
 //
 // A CTA takes a row pair (rows 4a+p and 4a+p+2 share the (A, B) pairs of the intermediates, ttsh_common.cuh) and runs its two
 // rows one after the other.  Everything a row reads arrives by cp.async.bulk + mbarrier in two staging slots, each copy issued
@@ -31,7 +31,8 @@
 // owner thread: that frees the 64 KB of shared memory the second slot needs and takes the stash traffic off the shared-memory pipe.
 // The merged bins of the pair's FIRST row wait there too, so that the second row writes whole 32-byte (A, B) pairs of the forward
 // intermediates (one full sector per bin) instead of 16-byte halves.
-// K comes in the thread order of the plan: (K(y, 2n), K(y, 2n+1)) for n = wl_j(t) + 256 k at (k 256 + t) 2 (k_reperm_real).
+// K comes in the thread order of the plan: (K(y, 2n), K(y, 2n+1)) for n = own(t) + TPL k at (k TPL + t) 2 (k_reperm_real), own(t) =
+// wl_j(t) for the warp-local plan, t for the plain one.
 #pragma once
 #include "row_step.cuh"
 #include "tmem.cuh"
@@ -63,7 +64,7 @@ template <typename T, int NX> struct RowStepRealCfg {
   static constexpr bool FITS = THREADS % 128 == 0 && THREADS <= 1024 && TMEM_NEED <= TMEM_PER_WARP && SMEM <= 227 * 1024;
 };
 
-// W^m = wj W_32^k for m = j + 256 k (forward sign), k a compile-time constant after unrolling
+// W^m = wj W_32^k for m = j + TPL k (forward sign), k a compile-time constant after unrolling
 template <typename T> __device__ __forceinline__ cplx<T> real_row_tw(cplx<T> wj, int k) { return mul_w32_rt<-1>(wj, k); }
 
 // inverse transform of one real row into registers: out[k] = f(2n) + i f(2n+1), n = wl_j(j) + k TPL.
@@ -242,10 +243,10 @@ k_row_step_real(const __grid_constant__ Geom g, const __grid_constant__ Model m,
           if constexpr (HTM) tmem_stc(tH + 16 * q, g4);
         }
       }
-      // ---- a4: three forward transforms, each merged into the half spectrum of the row on the bins k = j + 256 i ----
+      // ---- a4: three forward transforms, each merged into the half spectrum of the row on the bins k = j + TPL i ----
       auto ident = [&](int, int, cplx<T> z) -> cplx<T> { return z; };
       auto to_line = [&](int mm, int, cplx<T> z) { line[row_step_pad<T, M, WL>(mm)] = z; };
-      auto merged = [&](int i) -> cplx<T> {                          // F(k), k = j + 256 i
+      auto merged = [&](int i) -> cplx<T> {                          // F(k), k = j + TPL i
         const int k = j + TPL * i;
         const cplx<T> zp = line[row_step_pad<T, M, WL>(k)];
         const cplx<T> zm = conj(line[row_step_pad<T, M, WL>((M - k) & (M - 1))]);

@@ -216,8 +216,8 @@ typedef enum {
   TTSH_STAGE_REAL_FWD_ROW = 6, /* a3 fused into the a4 row pass; emits A~ = i kx Gy~ + S'~ and B~ = Gx~ (conservative form)   */
   TTSH_STAGE_FWD_COL_P2 = 7,  /* a4 column pass of those two intermediates                                                    */
   TTSH_STAGE_SPECTRAL_P2 = 8, /* a5 from the two spectra: rhs^ = A^ - i ky B^                                                   */
-  TTSH_STAGE_ROW_STEP = 9,    /* stages 1 + 6 in one kernel: w, v never leave the SM (1/2 rule; Nx = 8192: one real row per
-                                 transform).  ttsh_step runs 0, 9, 7, 8 where supported, else 0, 1, 6, 7, 8 */
+  TTSH_STAGE_ROW_STEP = 9,    /* stages 1 + 6 in one kernel: w, v never leave the SM (1/2 rule; Nx = 8192, and 16384 in fp32: one real
+                                 row per transform).  ttsh_step runs 0, 9, 7, 8 where supported, else 0, 1, 6, 7, 8 */
   TTSH_STAGE_COL_STEP = 10    /* stages 7 + 8 + stage 0 of the NEXT step in one kernel (Ny <= 1024, 1/2 rule): there ttsh_step runs
                                  9, 10 per Euler step, preceded by stage 0 once whenever the intermediates of the current state are
                                  not at hand (first step, or after any call that is not ttsh_step) */

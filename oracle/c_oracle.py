@@ -46,6 +46,8 @@ def _load():
         lib.ttsho_step.restype, lib.ttsho_step.argtypes = None, [vp, i]
         lib.ttsho_get_fields.restype, lib.ttsho_get_fields.argtypes = None, [vp, vp, vp, vp, vp]
         lib.ttsho_diagnostics.restype, lib.ttsho_diagnostics.argtypes = None, [vp, d, d, vp]
+        lib.ttsho_debug_post.restype, lib.ttsho_debug_post.argtypes = None, [vp, vp, vp, vp, vp, vp]
+        lib.ttsho_debug_set_state.restype, lib.ttsho_debug_set_state.argtypes = None, [vp, vp, vp, vp]
         lib.ttsho_time.restype, lib.ttsho_time.argtypes = d, [vp]
         lib.ttsho_nstep.restype, lib.ttsho_nstep.argtypes = C.c_longlong, [vp]
         _lib = lib
@@ -121,6 +123,23 @@ class TTSHOracleC:
         d = {k: float(v) for k, v in zip(keys, out[:9])}
         d.update(t=self.t, step=self.nstep, nonfinite=int(out[9]))
         return d
+
+    # ---- test-only (tests/test_oracle_c.py): see ttsho_debug_* in ttsh_oracle_c.c ----
+    def debug_post(self, w_naive, v0_new=(0.0, 0.0)):
+        """Lines 5-16 of Algorithm 1 on a caller-supplied spectrum complex[Ny, Nx]; returns (w^_new, v^_x, v^_y)."""
+        a = np.ascontiguousarray(w_naive, dtype=np.complex128)
+        assert a.shape == (self.Ny, self.Nx)
+        v0 = np.ascontiguousarray(v0_new, dtype=np.float64)
+        out = [np.empty((self.Ny, self.Nx), dtype=np.complex128) for _ in range(3)]
+        _load().ttsho_debug_post(self.h, _ptr(a), _ptr(v0), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]))
+        return tuple(out)
+
+    def debug_set_state(self, w_hat=None, vx=None, vy=None):
+        """Overwrites the raw state arrays (no projection, no dealiasing)."""
+        keep = [None if x is None else np.ascontiguousarray(x, dtype=dt) for x, dt in
+                ((w_hat, np.complex128), (vx, np.float64), (vy, np.float64))]
+        assert all(x is None or x.shape == (self.Ny, self.Nx) for x in keep)
+        _load().ttsho_debug_set_state(self.h, *[None if x is None else _ptr(x) for x in keep])
 
     def close(self):
         if getattr(self, "h", None):

@@ -18,7 +18,8 @@
  *
  * Pins (tests/test_oracle_c.py, `-m "not gpu"`): locked to the definition-oracle (whole trajectories, K, diagnostics,
  * <= 1e-13) on square and non-square grids, plus the closed-form single-mode growth and the uniform fixed point run
- * through this code alone.  Whole chaotic trajectories of the paper: parity unpinned (as for the numpy oracle).
+ * through this code alone; line 12 (Hermitian average) on a caller-supplied non-Hermitian spectrum and the
+ * non-finite count on one bad value per field, through the test-only ttsho_debug_* entries at the end of this file.  Whole chaotic trajectories of the paper: parity unpinned (as for the numpy oracle).
  */
 #include <complex.h>
 #include <math.h>
@@ -321,6 +322,28 @@ void ttsho_diagnostics(ttsho* o, double cx, double cy, double* out) {
   out[4] = (double)s_speed; out[5] = (double)s_vth;
   out[6] = (double)s_vx / (double)P; out[7] = (double)s_vy / (double)P;
   out[8] = vmax; out[9] = (double)bad;
+}
+
+/* ---- test-only entries (tests/test_oracle_c.py); no arithmetic of their own ----
+ * ttsho_debug_post: lines 5-16 of Algorithm 1 (`post` above) applied to a spectrum the CALLER supplies, so that
+ * the Hermitian average of line 12 can be pinned with an input that is not the spectrum of a real field.
+ * w_in, w_out, vxh_out, vyh_out: complex[Ny*Nx], interleaved (re, im); v0_new: the k = 0 velocity of line 8. */
+void ttsho_debug_post(ttsho* o, const double* w_in, const double* v0_new, double* w_out, double* vxh_out, double* vyh_out) {
+  const size_t P = (size_t)o->Nx * o->Ny;
+  memcpy(o->s3, w_in, sizeof(cplx) * P);
+  post(o, o->s3, v0_new, o->s0, o->s1, o->s2);
+  memcpy(w_out, o->s3, sizeof(cplx) * P);
+  memcpy(vxh_out, o->s0, sizeof(cplx) * P);
+  memcpy(vyh_out, o->s1, sizeof(cplx) * P);
+}
+
+/* ttsho_debug_set_state: overwrites the raw state arrays (any pointer may be NULL), bypassing set_velocity's projection: the only
+ * way to hand ttsho_diagnostics a non-finite value in a chosen field.  w_hat: complex[Ny*Nx] interleaved; vx, vy: double[Ny*Nx]. */
+void ttsho_debug_set_state(ttsho* o, const double* w_hat, const double* vx, const double* vy) {
+  const size_t P = (size_t)o->Nx * o->Ny;
+  if (w_hat) memcpy(o->w_hat, w_hat, sizeof(cplx) * P);
+  if (vx) memcpy(o->vx, vx, sizeof(double) * P);
+  if (vy) memcpy(o->vy, vy, sizeof(double) * P);
 }
 
 double ttsho_time(const ttsho* o) { return o->t; }

@@ -120,3 +120,49 @@ def test_c_oracle_uniform_fixed_point_and_damping_closed_form():
     gw = np.exp((0.5 + k2 - k2 * k2) * dt) * (1 - 44.0 * dt)
     assert rel(w, gw * k2 * np.cos(ph)) < 1e-12
     assert abs(vx.mean() - 0.3 * np.exp(0.5 * dt) * (1 - 40.0 * dt)) < 1e-14
+
+
+def test_c_hermitian_average_removes_injected_antihermitian_part():
+    """Line 12 of Algorithm 1, w^(k) = 1/2 {w^(k) + w^(-k)*}, in the C restatement: its trajectories only ever
+    feed it spectra of real fields, which are Hermitian already, so the line is pinned here on a spectrum that is not."""
+    from oracle import idft2
+    N, dx = 32, 0.5
+    mask = workloads.disk_mask(N, N, dx, 5.0)
+    vel = workloads.gaussian_velocity(N, N, 21, 0.8, mask)
+    o = TTSHOracle(N, N, dx, 0.01, BASELINE_PRESET, mask=mask)
+    c = TTSHOracleC(N, N, dx, 0.01, BASELINE_PRESET, mask=mask)
+    o.set_velocity(*vel); o.step(1)
+    good = o.w_hat.copy()
+    bad = good.copy()
+    bad[3, 5] += 0.25j; bad[0, 7] += 0.1 + 0.2j; bad[4, 0] -= 0.3j         # breaks w^(k) = w^(-k)*
+    v0 = np.array([0.3, -0.2])
+    w_new, vxh, vyh = c.debug_post(bad, v0)
+    refl = np.conj(np.roll(w_new[::-1, ::-1], (1, 1), (0, 1)))
+    assert np.max(np.abs(w_new - refl)) < 1e-16                            # Hermitian after the step
+    assert np.max(np.abs(idft2(w_new).imag)) < 1e-15 and np.max(np.abs(idft2(vxh).imag)) < 1e-15
+    assert abs(w_new[3, 5] - (good[3, 5] + 0.125j)) < 1e-15                # exactly the average of line 12
+    assert abs(w_new[N - 3, N - 5] - np.conj(good[3, 5] + 0.125j)) < 1e-15  # and its mirror image at -k
+    assert abs(w_new[0, 7] - (good[0, 7] + 0.05 + 0.1j)) < 1e-15 and abs(w_new[4, 0] - (good[4, 0] - 0.15j)) < 1e-15
+    assert w_new[0, 0] == 0 and vxh[0, 0] == v0[0] and vyh[0, 0] == v0[1]  # lines 7-8
+    # the same lines of the definition-oracle on the same input
+    ow, _, ovx, ovy = o._post(bad, v0)
+    assert np.max(np.abs(w_new - ow)) < 1e-15 and np.max(np.abs(vxh - ovx)) < 1e-15 and np.max(np.abs(vyh - ovy)) < 1e-15
+    c.close()
+
+
+def test_c_nonfinite_counts_every_field():
+    """`nonfinite` counts the non-finite entries of v_x, v_y AND w (reading R13): one bad value in each, separately."""
+    N, dx = 16, 0.5
+    lin = TTSHParams(lambda0=0.0, alpha=-0.5, beta=0.0, Gamma0=-1.0, Gamma2=1.0, gamma_v=0.0, gamma_w=0.0)
+    for which, bad in (("vx", np.nan), ("vy", np.inf), ("w", np.nan)):
+        c = TTSHOracleC(N, N, dx, 0.01, lin)
+        w_hat = np.zeros((N, N), complex); vx = np.zeros((N, N)); vy = np.zeros((N, N))
+        if which == "vx":
+            vx[3, 5] = bad
+        elif which == "vy":
+            vy[7, 2] = bad
+        else:
+            w_hat[0, 0] = bad                                              # w = iDFT[w^]: every point non-finite
+        c.debug_set_state(w_hat, vx, vy)
+        assert c.diagnostics(4.0, 4.0)["nonfinite"] == (N * N if which == "w" else 1), which
+        c.close()

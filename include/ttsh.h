@@ -127,6 +127,36 @@ typedef struct {
 } ttsh_diag;
 int ttsh_diagnostics(ttsh_handle* h, double cx, double cy, ttsh_diag* host_out);
 
+/* The same diagnostics for a caller that cannot hand the library any device memory: no handle, no workspace, just the three
+ * fields.  Meant for code that is given field pointers and nothing else (a monitoring hook called from inside another solver's
+ * time loop), for processes whose framework allocator already owns all device memory so that a raw cudaMalloc would fail, and
+ * for loops that cannot afford the device-wide synchronisation cudaMalloc / cudaFree imply.  This call allocates nothing and
+ * frees nothing: its only scratch (one partial record per thread block, 592 x 8 doubles = 37,888 bytes) is a static
+ * __device__ array inside the library, which every GPU that loads the library carries until the process exits.
+ *   vx, vy, omega  DEVICE scalar[Ny*Nx] in (row-major, x contiguous; scalar per `t`); read only.
+ *   cx, cy         centre of e_theta in physical units, as in ttsh_diagnostics.
+ *   sums           DEVICE double[8] out, caller-owned: sum|v|^2, sum w^2, sum|v|, sum|e_theta.v|, sum v_x, sum v_y, max|v|,
+ *                  number of non-finite values among v_x, v_y, omega.
+ *   host_out       HOST or NULL.  NULL: the call only enqueues two kernels on cuda_stream and returns; read `sums` in stream
+ *                  order.  Non-NULL: additionally copies `sums` back, synchronises the stream and fills *host_out like
+ *                  ttsh_diagnostics does (t and step are 0: there is no handle to keep time).
+ *   cuda_stream    cudaStream_t of the caller (NULL = the default stream).
+ * Limits: 1 <= Nx, Ny <= 16384 (any integers, not only powers of two), i.e. at most TTSH_NOALLOC_MAX_POINTS grid points — the
+ * library's own largest grid; the scratch does not grow with the grid.  Larger sizes return TTSH_ERR_UNSUPPORTED_SIZE, bad
+ * pointers / dtype / dx TTSH_ERR_INVALID_ARG, a CUDA failure TTSH_ERR_CUDA; ttsh_diagnostics_noalloc_error() gives the text of
+ * the last failure of this call on the calling thread ("" after a success).
+ * Things to know about the shared static scratch:
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device current,
+ *     which may also load the library's code onto that device).  Make that first call before any stream capture begins.
+ *   - every call on a device uses the same array.  A call overwrites all of it before reading it, so nothing left behind by
+ *     an earlier call (of any grid size or dtype) matters; but two calls whose kernels can run at the same time — different
+ *     streams without an event between them — race on it and both results are undefined.  Serialise them.
+ * The sums equal those of ttsh_diagnostics on the same fields (same arithmetic, same launch shape). */
+#define TTSH_NOALLOC_MAX_POINTS (16384LL * 16384LL)
+int ttsh_diagnostics_noalloc(int Nx, int Ny, double dx, ttsh_dtype t, const void* vx, const void* vy, const void* omega,
+                             double cx, double cy, double* sums, ttsh_diag* host_out, void* cuda_stream);
+const char* ttsh_diagnostics_noalloc_error(void);
+
 /* Order parameter of the dumbbell geometry:
  *   Psi_2 = | w(x*_left) + w(x*_right) | / ( |w|(x*_left) + |w|(x*_right) ),   x*_side = argmax_side |w|,
  * "left"/"right" = the grid points within `radius` (the paper: D/2) of the centre of either cavity (physical units;

@@ -35,7 +35,8 @@ SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_vel
            "ttsh_psd_accumulate", "ttsh_psd_result", "ttsh_psd_reset", "ttsh_psd_destroy", "ttsh_tangent_workspace_bytes",
            "ttsh_tangent_create", "ttsh_tangent_set", "ttsh_tangent_step", "ttsh_tangent_orthonormalize",
            "ttsh_tangent_get_fields", "ttsh_tangent_destroy", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
-           "ttsh_ensemble_destroy", "ttsh_build_info")
+           "ttsh_ensemble_destroy", "ttsh_build_info", "ttsh_diagnostics_noalloc", "ttsh_diagnostics_noalloc_error")
+TTSH_NOALLOC_MAX_POINTS = 16384 * 16384
 
 
 class ttsh_params(C.Structure):
@@ -97,6 +98,8 @@ _sig = {
     "ttsh_ensemble_launch_count": (_ll, [_vp]),
     "ttsh_ensemble_destroy": (_i, [_vp]),
     "ttsh_build_info": (C.c_char_p, []),
+    "ttsh_diagnostics_noalloc": (_i, [_i, _i, _d, _i, _vp, _vp, _vp, _d, _d, _vp, C.POINTER(ttsh_diag), _vp]),
+    "ttsh_diagnostics_noalloc_error": (C.c_char_p, []),
 }
 for _name, (_res, _args) in _sig.items():
     _f = getattr(_lib, _name)
@@ -171,6 +174,21 @@ def ttsh_diagnostics(h, cx, cy):
     d = ttsh_diag()
     rc = _lib.ttsh_diagnostics(h, cx, cy, C.byref(d))
     return rc, d
+
+
+def ttsh_diagnostics_noalloc(Nx, Ny, dx, dtype, vx_ptr, vy_ptr, omega_ptr, cx, cy, sums_ptr, stream_ptr, read_back=True):
+    """Diagnostics of three caller-owned DEVICE fields without a handle or workspace, for callers that cannot allocate device
+    memory (see include/ttsh.h): the library's scratch is a static array on the GPU, shared by all calls on that device, so
+    calls must not overlap on the GPU.  sums_ptr: DEVICE double[8] out.  Returns (status, ttsh_diag or None); with
+    read_back=False nothing is copied to the host and the call is asynchronous."""
+    d = ttsh_diag() if read_back else None
+    rc = _lib.ttsh_diagnostics_noalloc(Nx, Ny, dx, dtype, vx_ptr, vy_ptr, omega_ptr, cx, cy, sums_ptr,
+                                       C.byref(d) if read_back else None, stream_ptr)
+    return rc, d
+
+
+def ttsh_diagnostics_noalloc_error():
+    return _lib.ttsh_diagnostics_noalloc_error().decode()
 
 
 def ttsh_dumbbell_order(h, cx_left, cy_left, cx_right, cy_right, radius):

@@ -28,6 +28,17 @@ def test_library_exports_every_declared_symbol(ttsh):
 
 
 def test_library_was_built_from_the_sources_in_the_tree(ttsh):
+    _check_build_info(ttsh)
+
+
+@pytest.mark.gpu
+def test_library_on_the_gpu_box_was_built_from_the_sources_in_the_tree(ttsh):
+    """The same check inside the `-m gpu` run: the libttsh.so that the parity tests load on the GPU box (it travels with the
+    snapshot; build() is an incremental make) is the one compiled from the sources next to it."""
+    _check_build_info(ttsh)
+
+
+def _check_build_info(ttsh):
     """ttsh_build_info carries the SHA-256 of the CUDA sources the binary was compiled from (csrc/Makefile): a stale libttsh.so
     that travelled with the snapshot instead of being rebuilt would show here."""
     import glob

@@ -218,7 +218,7 @@ int ttsh_tangent_destroy(ttsh_tangent* s);
  * (TTSH_STAGE_COL_STEP), an ensemble does the same as long as count x (number of column tiles) <= 8 x (number of SMs); a larger
  * one is bound by throughput, keeps the 4 launches, and then agrees with ttsh_step to round-off instead of bit for bit.
  * Requirements (else TTSH_ERR_INVALID_ARG): count >= 1; all members have the same Nx, Ny, dtype, dx, dt, parameters and
- * stream, use TTSH_ADVECTION_CONSERVATIVE with the 1/2 rule on a grid the fused row kernel supports (Nx <= 8192), and their workspaces lie at a uniform byte stride: workspace_b = workspace_0 + b * stride, stride >=
+ * stream, use TTSH_ADVECTION_CONSERVATIVE with the 1/2 rule on a grid the fused row kernel supports (Nx <= 8192 in fp64, Nx <= 16384 in fp32), and their workspaces lie at a uniform byte stride: workspace_b = workspace_0 + b * stride, stride >=
  * ttsh_workspace_bytes (carve them from one allocation).  Masks, states and step counters are per member; all other calls
  * (ttsh_set_velocity, ttsh_set_mask, ttsh_get_fields, ttsh_diagnostics, ...) keep working on the member handles.  The
  * ensemble borrows the members: destroy it before them. */

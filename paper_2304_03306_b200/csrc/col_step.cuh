@@ -12,8 +12,11 @@
 // the dependency chain is two half-length transforms and the pointwise update.
 //
 // Every number is computed by the expressions of k_fwd_col, k_spectral_p2 and k_inv_col on the same operands (the odd-row part is
-// added to the even-row part in shared memory where k_fwd_col uses red.global.add: one addend per entry either way), so the state
-// and the intermediates are BIT-IDENTICAL to those of the four-launch step.  1/2 rule only.
+// added to the even-row part in shared memory where k_fwd_col uses red.global.add: one addend per entry either way).  The results
+// agree with the four-launch step to ROUND-OFF, not bit for bit: inlined into one kernel, the compiler contracts a few
+// multiply-adds of the odd-row twiddle and of the spectral update differently (test_fused_column_kernel_against_the_four_launch_step
+// bounds the difference by 1e-13 in fp64, 2e-5 in fp32; ttsh.h says the same).  An ensemble picks this kernel or the four launches
+// by count x tiles against the SM count (ttsh_ensemble_create), so its round-off depends on count and on the device.  1/2 rule only.
 #pragma once
 #include "fft_passes.cuh"
 #include "spectral_point.cuh"

@@ -84,7 +84,7 @@ def test_ensemble_members_match_oracle_and_single_handles(ttsh, Nx, Ny, count, n
 
 
 @pytest.mark.parametrize("dtype,Nx,Ny,count", [("f32", 256, 128, 4), ("f64", 1024, 1024, 2), ("f32", 2048, 256, 2), ("f64", 8192, 64, 2),
-                                               ("f32", 8192, 64, 2), ("f64", 4096, 64, 3)])
+                                               ("f32", 8192, 64, 2), ("f64", 4096, 64, 3), ("f32", 16384, 64, 2)])
 def test_ensemble_bit_identical_to_single_handles_larger_grids(ttsh, dtype, Nx, Ny, count):
     dx, dt = 0.5, 0.01
     radii = [0.1 * min(Nx, Ny) * dx * (1 + 0.5 * i) for i in range(count)]

@@ -46,12 +46,17 @@ template <typename T, int NX> struct RowStepRealCfg {
   static constexpr int LS = (WL ? fft_wl_line_elems<T, M>() : fft_line_elems<M>()) + 4;
   // tensor memory (tmem.cuh), per thread: the waiting field (16 complex values) and the merged bins of the pair's first row (B~ and
   // A~, 9 complex values each), in pieces of 16 columns = 4 complex doubles / 8 complex floats; THREADS / 128 warps per lane quarter
-  static constexpr unsigned TMEM_COLS = 512;
-  static constexpr int TMEM_PER_WARP = 512 / (THREADS / 128);
   static constexpr int CH = 16 / (2 * (int)sizeof(T) / 4);
   // the 512-thread variant (M = 8192) has 128 registers per thread: its second waiting field (v_x, then Gy) is parked as well
   static constexpr bool HTM = THREADS > 256;
   static constexpr int TMEM_NEED = (HTM ? 2 : 1) * 16 * (16 / CH) + 2 * 16 * ((9 + CH - 1) / CH);
+  // allocate no more than the kernel uses (the next power of two >= columns per warp x warps per lane quarter, >= 32): a CTA
+  // holds its columns for the whole persistent loop, and a second CTA on the same SM (another handle on another stream; fp32 at
+  // NX = 8192 leaves room for two) would otherwise block in tcgen05.alloc until the first one ends.  fp64: 2 x 160 -> 512;
+  // fp32 at NX = 8192: 2 x 96 -> 256; fp32 at NX = 16384: 4 x 128 = 512
+  static constexpr unsigned tmem_cols_for(unsigned need) { unsigned c = 32; while (c < need) c *= 2; return c; }
+  static constexpr unsigned TMEM_COLS = tmem_cols_for((unsigned)(THREADS >= 128 ? THREADS / 128 : 1) * TMEM_NEED);
+  static constexpr int TMEM_PER_WARP = (int)TMEM_COLS / (THREADS >= 128 ? THREADS / 128 : 1);
   static constexpr size_t OFF_TAB = (size_t)LS * sizeof(cplx<T>);
   // a copy of the warp-local table in shared memory in fp64 (row_step.cuh, SMEM_TAB, says why); fp32 and the plain plan read it through L1
   static constexpr bool SMEM_TAB = WL && sizeof(T) == 8;
@@ -61,7 +66,7 @@ template <typename T, int NX> struct RowStepRealCfg {
   static constexpr size_t OFF_SLOTS = (OFF_TAB + TAB_BYTES + 127) / 128 * 128;
   static constexpr size_t OFF_BAR = OFF_SLOTS + 2 * SLOT;
   static constexpr size_t SMEM = OFF_BAR + 32;
-  static constexpr bool FITS = THREADS % 128 == 0 && THREADS <= 1024 && TMEM_NEED <= TMEM_PER_WARP && SMEM <= 227 * 1024;
+  static constexpr bool FITS = THREADS % 128 == 0 && THREADS <= 1024 && TMEM_COLS <= 512 && TMEM_NEED <= TMEM_PER_WARP && SMEM <= 227 * 1024;
 };
 
 // W^m = wj W_32^k for m = j + TPL k (forward sign), k a compile-time constant after unrolling

@@ -684,6 +684,39 @@ def test_real_row_fused_kernel_nx8192(ttsh, which, Ny, dtype):
     s.close(); a.close(); b.close()
 
 
+@pytest.mark.parametrize("Nx,Ny,dtype", [(8192, 256, "f32"), (8192, 128, "f64"), (1024, 1024, "f64")])
+def test_two_handles_on_two_streams_match_sequential_runs_bit_for_bit(ttsh, Nx, Ny, dtype):
+    """k_row_step_real keeps tensor-memory columns for its whole persistent loop, and in fp32 at Nx = 8192 two of its CTAs fit on
+    one SM: two handles stepped at the same time on two streams must neither block each other for good (tcgen05.alloc) nor
+    disturb each other's columns.  Also run-to-run determinism of k_row_step_real and k_col_step (1024^2: k_row_step + k_col_step):
+    the concurrent run, repeated, and the one-after-the-other run give the same bits."""
+    import torch
+    dx, dt = 0.5, 0.01
+    masks = [workloads.disk_mask(Nx, Ny, dx, f * min(Nx, Ny) * dx) for f in (0.3, 0.2)]
+    vels = [workloads.planewave_velocity(Nx, Ny, dx, workloads.SEED0 + 31 + i, amplitude=1.0, nmodes=12) for i in range(2)]
+
+    def run(streams):
+        sols = [ttsh.Solver(Nx, Ny, dx, dt, ttsh.baseline_params(), dtype, mask=masks[i], stream=streams[i]) for i in range(2)]
+        for s, v in zip(sols, vels):
+            s.set_velocity(*v)
+        for _ in range(4):                    # enqueued alternately, nothing waits in between
+            for s in sols:
+                s.step(3)
+        torch.cuda.synchronize()
+        out = [gpu_fields(s) for s in sols]
+        for s in sols:
+            s.close()
+        return out
+
+    one_after_the_other = run([None, None])                       # both on the current stream
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for attempt in range(2):
+        together = run(streams)
+        for i in range(2):
+            for a, b, name in zip(together[i], one_after_the_other[i], ("vx", "vy", "w", "psi")):
+                assert np.isfinite(a).all() and np.array_equal(a, b), f"handle {i}, {name}, concurrent run {attempt}"
+
+
 @pytest.mark.parametrize("Nx,Ny,dtype", [(16384, 64, "f64"), (16384, 64, "f32"), (64, 16384, "f64"), (64, 16384, "f32"), (16384, 128, "f64")])
 def test_maximum_grid_dimension_16384(ttsh, Nx, Ny, dtype):
     """(N, dx) = (16384, 0.0025) is the grid of Fig. 6(f).  Nx = 16384: one real row per half-length transform: in

@@ -105,9 +105,14 @@ int ttsh_step(ttsh_handle* h, int n);
  * v = iDFT[v^] (state), omega = iDFT[w^], psi = iDFT[w^/k^2] with psi^(0) = 0. */
 int ttsh_get_fields(ttsh_handle* h, void* vx, void* vy, void* omega, void* psi);
 
-/* Bit-exact checkpoint of the spectral state: w_hat is DEVICE complex-scalar[ttsh_state_elems] (interleaved
- * re, im; the library's tile-major pruned-spectrum layout, opaque to the caller), mean_flow is HOST double[2] = v^(0).
- * get synchronises the stream. */
+/* Bit-exact checkpoint of the spectral state: w_hat is DEVICE complex-scalar[ttsh_state_elems] (interleaved re, im), the retained
+ * modes of w^ (unitary DFT) in natural order [Hy][Wx]: element (q, m_x) at q Wx + m_x, with m_x = 0 .. Wx - 1,
+ * Wx - 1 = floor(num Nx / (2 den)), and row q <-> m_y = q for q <= My, q - Hy above, My = floor(num Ny / (2 den)), Hy = 2 My + 1
+ * (num/den = the dealias fraction: nothing outside this rectangle is ever non-zero under the cutoff of PAPER.md:301).
+ * ttsh_state_elems = Wx Hy depends on Nx, Ny and the dealias fraction only — not on the tile widths this binary was built with —
+ * so a checkpoint written by one build of the library restores in any other on a handle of the same grid, dtype and parameters;
+ * there is no header in the buffer: the caller stores (Nx, Ny, dtype, num/den) beside it.  mean_flow is HOST double[2] = v^(0).
+ * Both calls synchronise the stream. */
 size_t ttsh_state_elems(const ttsh_handle* h);
 int ttsh_get_state(ttsh_handle* h, void* w_hat, double* mean_flow);
 int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, double t, long long step);

@@ -80,6 +80,9 @@ template <typename T> cudaError_t launch_spectral(const Geom& g, const Model& m,
                                                   void* w, void* psi, double* v0, cudaStream_t s, int members = 1, size_t mstride = 0);
 template <typename T> cudaError_t launch_spectral_init(const Geom& g, const void* Vx, const void* Vy, void* w, void* psi, double* v0, cudaStream_t s);
 template <typename T> cudaError_t launch_psi_from_w(const Geom& g, const void* w, void* psi, cudaStream_t s);
+// checkpoint layout: the tile-major pruned spectrum <-> natural order complex[Hy][Wx] (independent of the tile width CW)
+template <typename T> cudaError_t launch_state_pack(const Geom& g, const void* w, void* nat, cudaStream_t s);
+template <typename T> cudaError_t launch_state_unpack(const Geom& g, const void* nat, void* w, cudaStream_t s);
 template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s);
 template <typename T> cudaError_t launch_square(size_t n, const void* in, void* out, cudaStream_t s);
 template <typename T> cudaError_t launch_fill(size_t n, void* out, double val, cudaStream_t s);

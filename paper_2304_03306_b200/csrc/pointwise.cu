@@ -46,6 +46,16 @@ template <typename T> cudaError_t launch_psi_from_w(const Geom& g, const void* w
   k_psi_from_w<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)w, (cplx<T>*)psi);
   return cudaGetLastError();
 }
+template <typename T> cudaError_t launch_state_pack(const Geom& g, const void* w, void* nat, cudaStream_t s) {
+  const unsigned grid = (unsigned)(((size_t)g.Hy * g.Wx + 255) / 256);
+  k_state_pack<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)w, (cplx<T>*)nat);
+  return cudaGetLastError();
+}
+template <typename T> cudaError_t launch_state_unpack(const Geom& g, const void* nat, void* w, cudaStream_t s) {
+  const unsigned grid = (unsigned)(((size_t)g.NT * g.Hy * g.CW + 255) / 256);
+  k_state_unpack<T><<<grid, 256, 0, s>>>(g, (const cplx<T>*)nat, (cplx<T>*)w);
+  return cudaGetLastError();
+}
 template <typename T> cudaError_t launch_mask_to_real(size_t n, const unsigned char* mask, void* out, cudaStream_t s) {
   k_mask_to_real<T><<<blocks_for(n, 256, GRID_CAP), 256, 0, s>>>(n, mask, (T*)out);
   return cudaGetLastError();
@@ -169,6 +179,8 @@ template <typename T> cudaError_t launch_tri_apply(const Geom& g, int nvec, cons
   template cudaError_t launch_spectral<T>(const Geom&, const Model&, const void*, const void*, const void*, void*, void*, double*, cudaStream_t, int, size_t); \
   template cudaError_t launch_spectral_init<T>(const Geom&, const void*, const void*, void*, void*, double*, cudaStream_t); \
   template cudaError_t launch_psi_from_w<T>(const Geom&, const void*, void*, cudaStream_t); \
+  template cudaError_t launch_state_pack<T>(const Geom&, const void*, void*, cudaStream_t); \
+  template cudaError_t launch_state_unpack<T>(const Geom&, const void*, void*, cudaStream_t); \
   template cudaError_t launch_spectral_p2<T>(const Geom&, const Model&, const void*, const void*, void*, void*, double*, cudaStream_t, int, size_t); \
   template cudaError_t launch_mask_to_real<T>(size_t, const unsigned char*, void*, cudaStream_t); \
   template cudaError_t launch_square<T>(size_t, const void*, void*, cudaStream_t); \

@@ -233,6 +233,27 @@ k_psi_from_w(Geom g, const cplx<T>* __restrict__ w, cplx<T>* __restrict__ psi) {
   psi[idx] = (mx >= g.Wx || (mx == 0 && my == 0)) ? mk<T>(0, 0) : inv_k2<T>(g, mx, my) * w[idx];
 }
 
+// Checkpoints (ttsh_get_state / ttsh_set_state) cross the C ABI in NATURAL order, complex[Hy][Wx]: element (q, mx) at q Wx + mx,
+// so that their size and layout do not depend on the tile width CW of this build (col_tile_width and the TTSH_COL_* macros).
+// pack: tile-major -> natural.  unpack: natural -> tile-major, padding columns mx >= Wx set to zero (they never hold anything else).
+template <typename T>
+__global__ void __launch_bounds__(256) k_state_pack(Geom g, const cplx<T>* __restrict__ w, cplx<T>* __restrict__ nat) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)g.Hy * g.Wx) return;
+  const int q = (int)(idx / g.Wx), mx = (int)(idx - (size_t)q * g.Wx);
+  nat[idx] = w[spec_index(g, q, mx)];
+}
+template <typename T>
+__global__ void __launch_bounds__(256) k_state_unpack(Geom g, const cplx<T>* __restrict__ nat, cplx<T>* __restrict__ w) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)g.NT * g.Hy * g.CW) return;
+  const int t = (int)(idx / ((size_t)g.Hy * g.CW));
+  const int rem = (int)(idx - (size_t)t * g.Hy * g.CW);
+  const int q = rem >> g.cw_shift;
+  const int mx = t * g.CW + (rem & (g.CW - 1));
+  w[idx] = mx < g.Wx ? nat[(size_t)q * g.Wx + mx] : mk<T>(0, 0);
+}
+
 // natural <-> permuted row layout of the internal real fields (perm_index: x = j + k TPL -> ((k>>2) TPL + j) 4 + (k&3)).
 // Only for buffers that cross the C ABI in natural order (a processed mask, debug copies).
 template <typename T>

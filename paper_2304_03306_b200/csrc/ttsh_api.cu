@@ -668,15 +668,15 @@ int ttsh_get_fields(ttsh_handle* h, void* vx, void* vy, void* omega, void* psi) 
   return enqueue_inverse(h, omega, nullptr, nullptr, vx, vy, psi);
 }
 
-size_t ttsh_state_elems(const ttsh_handle* h) { return h ? (size_t)h->g.NT * h->g.CW * h->g.Hy : 0; }
+size_t ttsh_state_elems(const ttsh_handle* h) { return h ? (size_t)h->g.Wx * h->g.Hy : 0; }
 
 int ttsh_get_state(ttsh_handle* h, void* w_hat, double* mean_flow) {
   if (!h || !w_hat || !mean_flow) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
   CHECK_DEVICE(h);
   if (!h->initialized) return TTSH_ERR_NOT_INITIALIZED;
-  const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
-  TRY(h, cudaMemcpyAsync(w_hat, h->what, bytes, cudaMemcpyDeviceToDevice, h->stream));
+  TRY(h, DISPATCH(h, launch_state_pack, h->g, h->what, w_hat, h->stream));
+  h->launches++;
   TRY(h, cudaMemcpyAsync(mean_flow, h->v0, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   TRY(h, cudaStreamSynchronize(h->stream));
   return TTSH_OK;
@@ -686,9 +686,9 @@ int ttsh_set_state(ttsh_handle* h, const void* w_hat, const double* mean_flow, d
   if (!h || !w_hat || !mean_flow) return TTSH_ERR_INVALID_ARG;
   if (h->sticky) return h->sticky;
   CHECK_DEVICE(h);
-  const size_t bytes = ttsh_state_elems(h) * 2 * (size_t)h->dtype;
   h->inter_valid = false;
-  TRY(h, cudaMemcpyAsync(h->what, w_hat, bytes, cudaMemcpyDeviceToDevice, h->stream));
+  TRY(h, DISPATCH(h, launch_state_unpack, h->g, w_hat, h->what, h->stream));
+  h->launches++;
   TRY(h, cudaMemcpyAsync(h->v0, mean_flow, 2 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
   TRY(h, DISPATCH(h, launch_psi_from_w, h->g, h->what, h->psihat, h->stream));
   h->launches++;

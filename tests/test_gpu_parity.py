@@ -352,6 +352,48 @@ def test_uniform_fixed_point_and_single_mode_on_gpu(ttsh):
     s.close()
 
 
+@pytest.mark.parametrize("Nx,Ny,dtype", [(64, 64, "f64"), (256, 1024, "f64"), (128, 2048, "f32"), (8192, 64, "f32")])
+def test_checkpoint_is_in_natural_order_and_restores_bit_exactly(ttsh, Nx, Ny, dtype):
+    """ttsh_get_state / ttsh_set_state on grids whose column tiles are 4, 2, 8 and 4 columns wide (the retained Nx/4 + 1 columns do
+    not fill the last tile): the buffer is the oracle's w^ on the retained modes in natural order [Hy][Wx] (include/ttsh.h), its
+    size does not depend on the tile width, and a restart from it repeats the run bit for bit."""
+    import torch
+    dx, dt = 0.5, 0.01
+    mask = workloads.disk_mask(Nx, Ny, dx, 0.3 * min(Nx, Ny) * dx)
+    vel = workloads.planewave_velocity(Nx, Ny, dx, 9, amplitude=1.0)
+    s, o = make_pair(ttsh, Nx, Ny, dx, dt, "baseline", mask, dtype=dtype, transform="c" if Nx * Ny > 256 * 256 else "matmul", vel=vel)
+    s.step(2); o.step(2)
+    Wx, My = Nx // 4 + 1, Ny // 4
+    Hy = 2 * My + 1
+    n = ttsh.ttsh_state_elems(s.h)
+    assert n == Wx * Hy
+    buf = torch.empty(2 * n, dtype=s.tdtype, device="cuda")
+    rc, mf = ttsh.ttsh_get_state(s.h, buf.data_ptr())
+    assert rc == 0
+    got = buf.cpu().numpy().astype(np.float64).reshape(Hy, Wx, 2)
+    got = got[..., 0] + 1j * got[..., 1]
+    if hasattr(o, "w_hat"):
+        rows = [q if q <= My else q - Hy for q in range(Hy)]             # row q <-> m_y
+        want = o.w_hat[rows, :Wx]
+        assert np.linalg.norm(got - want) <= (TOL_F64_1 if dtype == "f64" else TOL_F32_1) * np.linalg.norm(want)   # complex: not rel()
+    else:                                                                  # the C oracle keeps w^ to itself: compare w = iDFT[w^] rebuilt from the buffer
+        full = np.zeros((Ny, Nx), complex)
+        for q in range(Hy):
+            my = q if q <= My else q - Hy
+            full[my % Ny, :Wx] = got[q]
+            full[(-my) % Ny, (-np.arange(1, Wx)) % Nx] = np.conj(got[q, 1:])
+        w = np.fft.ifft2(full).real * np.sqrt(Nx * Ny)
+        assert rel(w, o.get_fields()[2]) <= (10 * TOL_F64_1 if dtype == "f64" else TOL_F32_1)
+    s.step(3)
+    a = [t.clone() for t in s.get_fields()]
+    assert ttsh.ttsh_set_state(s.h, buf.data_ptr(), mf, 2 * dt, 2) == 0
+    s.step(3)
+    for u, v in zip(a, s.get_fields()):
+        assert torch.equal(u, v)
+    assert s.diagnostics()["step"] == 5
+    s.close()
+
+
 def test_checkpoint_roundtrip_is_bit_exact_and_set_mask_keeps_state(ttsh):
     import torch
     N = 128

@@ -265,6 +265,14 @@ int ttsh_debug_get_real(ttsh_handle* h, int which, void* dst);
 
 int ttsh_destroy(ttsh_handle* h);
 
+/* Measurement aid, not part of the method (the fp64 / fp32 ALU roof is not in MEASURED_PEAKS.json).  Enqueues ONE
+ * kernel of `blocks` x 256 threads in which every thread runs 8 independent chains x <- x a + b for 16 x rounds fused multiply-adds
+ * each, in registers: nothing but the FMA pipe limits it.  sink: DEVICE scalar[blocks * 256] out (thread i of block k writes the
+ * sum of its chains, started at (i + 32 c) / 1024, c < 8, to sink[256 k + i]: with a = 1, b = 0 that is (8 i + 896) / 1024).
+ * *flops_out (HOST, may be NULL) = 2 x 8 x 16 x rounds x 256 x blocks, the flops of the launch; the caller times it with events.
+ * bench.py divides the two and reports the result as the peak of the ALU roofline. */
+int ttsh_microbench_fma(ttsh_dtype t, int blocks, int rounds, double a, double b, void* sink, void* cuda_stream, double* flops_out);
+
 /* "ttsh sm_100a sources=<first 16 hex digits of the SHA-256 of csrc/*.cu, *.cuh, *.h, include/ttsh.h, Makefile, concatenated in
  * sorted order> cuda=<nvcc version> built <date>": which sources this binary was compiled from (tests compare it with the tree). */
 const char* ttsh_build_info(void);

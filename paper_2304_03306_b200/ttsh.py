@@ -35,7 +35,8 @@ SYMBOLS = ("ttsh_workspace_bytes", "ttsh_create", "ttsh_set_mask", "ttsh_set_vel
            "ttsh_psd_accumulate", "ttsh_psd_result", "ttsh_psd_reset", "ttsh_psd_destroy", "ttsh_tangent_workspace_bytes",
            "ttsh_tangent_create", "ttsh_tangent_set", "ttsh_tangent_step", "ttsh_tangent_orthonormalize",
            "ttsh_tangent_get_fields", "ttsh_tangent_destroy", "ttsh_ensemble_create", "ttsh_ensemble_step", "ttsh_ensemble_launch_count",
-           "ttsh_ensemble_destroy", "ttsh_build_info", "ttsh_diagnostics_noalloc", "ttsh_diagnostics_noalloc_error")
+           "ttsh_ensemble_destroy", "ttsh_build_info", "ttsh_diagnostics_noalloc", "ttsh_diagnostics_noalloc_error",
+           "ttsh_microbench_fma")
 TTSH_NOALLOC_MAX_POINTS = 16384 * 16384
 
 
@@ -100,6 +101,7 @@ _sig = {
     "ttsh_build_info": (C.c_char_p, []),
     "ttsh_diagnostics_noalloc": (_i, [_i, _i, _d, _i, _vp, _vp, _vp, _d, _d, _vp, C.POINTER(ttsh_diag), _vp]),
     "ttsh_diagnostics_noalloc_error": (C.c_char_p, []),
+    "ttsh_microbench_fma": (_i, [_i, _i, _i, _d, _d, _vp, _vp, C.POINTER(_d)]),
 }
 for _name, (_res, _args) in _sig.items():
     _f = getattr(_lib, _name)
@@ -189,6 +191,13 @@ def ttsh_diagnostics_noalloc(Nx, Ny, dx, dtype, vx_ptr, vy_ptr, omega_ptr, cx, c
 
 def ttsh_diagnostics_noalloc_error():
     return _lib.ttsh_diagnostics_noalloc_error().decode()
+
+
+def ttsh_microbench_fma(dtype, blocks, rounds, a, b, sink_ptr, stream_ptr):
+    """One launch of the dense FMA loop (include/ttsh.h); returns (status, flops of the launch)."""
+    fl = _d(0.0)
+    rc = _lib.ttsh_microbench_fma(dtype, blocks, rounds, a, b, sink_ptr, stream_ptr, C.byref(fl))
+    return rc, fl.value
 
 
 def ttsh_dumbbell_order(h, cx_left, cy_left, cx_right, cy_right, radius):

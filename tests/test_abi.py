@@ -159,3 +159,23 @@ def test_tangent_argument_validation_without_touching_cuda(ttsh):
     assert ttsh.ttsh_tangent_orthonormalize(None, 1)[0] == ttsh.TTSH_ERR_INVALID_ARG
     assert ttsh.ttsh_tangent_get_fields(None, 0) == ttsh.TTSH_ERR_INVALID_ARG
     assert ttsh.ttsh_tangent_destroy(None) == ttsh.TTSH_OK
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_microbench_fma_runs_the_stated_chains(ttsh, dtype):
+    """ttsh_microbench_fma (the measured ALU roof of bench.py): with a = 1, b = 0 every chain keeps its start value, so thread i
+    writes (8 i + 896) / 1024 exactly; with a = 1, b = 2^-10 each chain grows by 16 x rounds / 1024; the flop count is the stated one."""
+    import torch
+    code, td = (ttsh.TTSH_F64, torch.float64) if dtype == "f64" else (ttsh.TTSH_F32, torch.float32)
+    blocks, rounds = 3, 5
+    sink = torch.full((blocks * 256,), -1.0, dtype=td, device="cuda")
+    stream = torch.cuda.current_stream()
+    rc, flops = ttsh.ttsh_microbench_fma(code, blocks, rounds, 1.0, 0.0, sink.data_ptr(), stream.cuda_stream)
+    assert rc == ttsh.TTSH_OK and flops == 2 * 8 * 16 * rounds * 256 * blocks
+    i = torch.arange(256, dtype=td, device="cuda").repeat(blocks)
+    assert torch.equal(sink, (8 * i + 896) / 1024)
+    rc, _ = ttsh.ttsh_microbench_fma(code, blocks, rounds, 1.0, 2.0 ** -10, sink.data_ptr(), stream.cuda_stream)
+    assert rc == ttsh.TTSH_OK and torch.equal(sink, (8 * i + 896 + 8 * 16 * rounds) / 1024)
+    assert ttsh.ttsh_microbench_fma(code, 0, rounds, 1.0, 0.0, sink.data_ptr(), stream.cuda_stream)[0] == ttsh.TTSH_ERR_INVALID_ARG
+    assert ttsh.ttsh_microbench_fma(code, blocks, rounds, 1.0, 0.0, 0, stream.cuda_stream)[0] == ttsh.TTSH_ERR_INVALID_ARG

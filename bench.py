@@ -433,6 +433,29 @@ def measure_tangent(torch, ttsh, name, nvec, device, nsteps=100, qr_every=10):
             "workload": f"{name} {dtype}, {nvec} tangent vectors, QR every {qr_every} steps, {nsteps} steps from the 1e-2 start"}
 
 
+def measure_fma_peak(torch, ttsh, dtype, device, reps=5):
+    """The ALU roof, measured: ttsh_microbench_fma (a dense register-resident FMA loop, csrc/microbench.cu) timed with CUDA events;
+    best of `reps` launches of about 10 ms each.  Returns TFLOP/s."""
+    props = torch.cuda.get_device_properties(device)
+    code = ttsh.TTSH_F64 if dtype == "f64" else ttsh.TTSH_F32
+    blocks = props.multi_processor_count * 8                  # 8 CTAs x 256 threads = 64 warps per SM
+    rounds = 2000 if dtype == "f64" else 4000
+    sink = torch.empty(blocks * 256, dtype=torch.float64 if dtype == "f64" else torch.float32, device=device)
+    stream = torch.cuda.current_stream(device)
+    best = 0.0
+    for i in range(reps + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        rc, flops = ttsh.ttsh_microbench_fma(code, blocks, rounds, 0.999999, 1e-6, sink.data_ptr(), stream.cuda_stream)
+        e1.record(stream)
+        torch.cuda.synchronize(device)
+        if rc != ttsh.TTSH_OK:
+            raise RuntimeError("ttsh_microbench_fma failed")
+        if i > 0:                                             # the first launch is warm-up
+            best = max(best, flops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+    return best
+
+
 def measure_cufft_reference(torch, cfg, dtype, device, reps=10):
     """north_star: 'cuFFT serves only as a side-by-side reference'.  The transforms of ONE Euler step in the conservative form
     (3 inverse + 3 forward dense 2-D real transforms, the paper's own design) through torch.fft = cuFFT, without
@@ -578,13 +601,18 @@ def main():
         props = torch.cuda.get_device_properties(device)
         sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
         lanes = 64 if dtype == "f64" else 128
-        alu_peak = props.multi_processor_count * lanes * 2 * sm_mhz * 1e6 / 1e12
+        derived_peak = props.multi_processor_count * lanes * 2 * sm_mhz * 1e6 / 1e12
+        alu_peak = measure_fma_peak(torch, ttsh, dtype, device)       # measured in this run; the derived figure is kept beside it
         flops = row_step_flops(cfg.Nx, cfg.Ny)
         ach = flops / (st[dom] * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": dom, "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
                     "traffic": None,
-                    "peak_source": f"{props.multi_processor_count} SMs x {lanes} {dtype} lanes x 2 flop x {sm_mhz:.0f} MHz (DESIGN.md §6; "
-                                   "lane count confirmed by ncu: DP warp instructions / fp64-pipe active cycles = 62 lanes per SM-cycle)",
+                    "peak_source": f"measured in this run: ttsh_microbench_fma, a dense {dtype} FMA loop in registers on "
+                                   f"{props.multi_processor_count} SMs x 64 warps (csrc/microbench.cu), best of 5 launches, CUDA events",
+                    "peak_derived": derived_peak,
+                    "peak_derived_source": f"{props.multi_processor_count} SMs x {lanes} {dtype} lanes x 2 flop x {sm_mhz:.0f} MHz (DESIGN.md §6)",
+                    "flop_count": "textbook 5 N log2 N per complex transform of a packed row pair, unpruned (6 per pair) + 18 flop per "
+                                  "point of lines 1-2; counting one radix-2 level less for the 1/2-rule zeros gives about 0.91 of it",
                     "algorithmic_flops_per_launch": flops, "algorithmic_bytes_per_launch": sb[dom],
                     "hbm_GBps": hbm[dom]["GBps"], "hbm_frac": hbm[dom]["frac"], "hbm_peak": peak, "hbm_peak_source": peak_src}
     roofline.update({"kernel_ms": st[dom], "kernel_share_of_step": st[dom] / step_ms, "all_kernels_hbm": hbm,
@@ -611,7 +639,7 @@ def main():
 
     if not a.no_extra and world == 1:
         extra = {}
-        for name in ("C5-f32", "C3", "C3-f32", "C5p", "C6", "C6-f32"):
+        for name in ("C5-f32", "C3", "C3-f32", "C5p", "C6", "C6-f32", "C7", "C7-f32"):
             if name == a.workload:
                 continue
             c2, d2 = workload(name)

@@ -120,4 +120,7 @@ CONFIGS = {
     # the paper's own production run (Table I :264-278): 8192 x 8192, dx = 0.005 (L = 40.96), dt = 0.01, the paper's
     # parameters, a disk of radius R = 5.2 (just above the onset of the single vortex): about 95 % of the box is masked
     "C6": Config("C6", 8192, 8192, dx=0.005, dt=0.01, geometry="disk", R=5.2, steps=2000, dtypes=("f64", "f32"), index=5, preset="paper"),
+    # the grid of Fig. 6(f) (Table I footnote a): (N, dx) = (16384, 0.0025), the same box L = 40.96 and disk as C6 at
+    # twice the resolution; 27 GB of workspace in fp64, 13.5 GB in fp32
+    "C7": Config("C7", 16384, 16384, dx=0.0025, dt=0.01, geometry="disk", R=5.2, steps=2000, dtypes=("f64", "f32"), index=6, preset="paper"),
 }

@@ -832,6 +832,38 @@ def test_full_16384_square_grid_runs_in_fp32(ttsh):
     s.close()
 
 
+@pytest.mark.slow
+def test_C7_full_16384_square_grid_in_fp64_invariants(ttsh):
+    """The grid of Fig. 6(f), (N, dx) = (16384, 0.0025), whole and in fp64 (27 GB of workspace, the 6-launch step),
+    with the paper's parameters and the disk of C6.  No oracle can follow this size (parity is on the 16384-wide strips), so: the
+    properties that hold at any size — finite fields, zero-mean w, div v = 0 and curl v = w to round-off (checked with torch.fft on
+    the device: a checker, not the product path)."""
+    import torch
+    cfg = workloads.CONFIGS["C7"]
+    mask = cfg.mask()
+    s = ttsh.Solver(cfg.Nx, cfg.Ny, cfg.dx, cfg.dt, ttsh.paper_params(), "f64", mask=mask)
+    vel = cfg.initial_velocity(mask)
+    s.set_velocity(*vel)
+    del vel, mask
+    l0 = s.launch_count()
+    s.step(10)
+    assert s.launch_count() - l0 == 60
+    d = s.diagnostics()
+    assert d["nonfinite"] == 0 and d["step"] == 10 and np.isfinite(d["kinetic_energy"]) and d["kinetic_energy"] > 0 and d["max_speed"] < 1.0
+    vx, vy, w, _ = s.get_fields(psi=False)
+    kx = (2 * np.pi * torch.fft.rfftfreq(cfg.Nx, d=cfg.dx, dtype=torch.float64, device=w.device))[None, :]
+    ky = (2 * np.pi * torch.fft.fftfreq(cfg.Ny, d=cfg.dx, dtype=torch.float64, device=w.device))[:, None]
+    vxh, vyh = torch.fft.rfft2(vx), torch.fft.rfft2(vy)
+    del vx, vy
+    div = torch.fft.irfft2(1j * kx * vxh + 1j * ky * vyh, s=w.shape)
+    scale = float(w.abs().max())
+    assert scale > 0 and float(div.abs().max()) <= 1e-10 * scale
+    del div
+    curl = torch.fft.irfft2(1j * kx * vyh - 1j * ky * vxh, s=w.shape)
+    assert float((curl - w).abs().max()) <= 1e-10 * scale and abs(float(w.mean())) <= 1e-10 * scale
+    s.close()
+
+
 # ---------------------------------------------------------------- C2 as BASELINE.json states it: 20,000 steps, diagnostics every 100
 def test_C2_long_run_20000_steps_invariants(ttsh):
     """No oracle can follow 20,000 steps (chaotic dynamics): properties that hold at any time instead —

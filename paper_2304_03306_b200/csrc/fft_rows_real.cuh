@@ -40,7 +40,7 @@ k_inv_row_real(const __grid_constant__ Geom g, const __grid_constant__ Batch bat
   using C = RealRowCfg<T, NX>;
   constexpr int N2 = C::N2, TPL = C::TPL;
   pdl_wait();
-  pdl_trigger();     // the dependent launch may start its prologue; its own pdl_wait still waits for this grid to finish
+  pdl_trigger();     // as in k_inv_row / k_fwd_row (compiled out unless TTSH_PDL_TRIGGER = 1, ttsh_common.cuh)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* line = reinterpret_cast<cplx<T>*>(smem_raw);
   const int j = threadIdx.x;
@@ -96,7 +96,7 @@ k_fwd_row_real(const __grid_constant__ Geom g, const __grid_constant__ Batch bat
   using C = RealRowCfg<T, NX>;
   constexpr int N2 = C::N2, TPL = C::TPL;
   pdl_wait();
-  pdl_trigger();     // the dependent launch may start its prologue; its own pdl_wait still waits for this grid to finish
+  pdl_trigger();     // as in k_inv_row / k_fwd_row (compiled out unless TTSH_PDL_TRIGGER = 1, ttsh_common.cuh)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx<T>* line = reinterpret_cast<cplx<T>*>(smem_raw);
   const int j = threadIdx.x;

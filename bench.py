@@ -639,7 +639,8 @@ def main():
 
     if not a.no_extra and world == 1:
         extra = {}
-        for name in ("C5-f32", "C3", "C3-f32", "C5p", "C6", "C6-f32", "C7", "C7-f32"):
+        # all five BASELINE.json configs as single systems (C1, C2, C4 beside C3 and C5), then the paper's own grids C6, C7
+        for name in ("C5-f32", "C1", "C2", "C3", "C3-f32", "C4", "C5p", "C6", "C6-f32", "C7", "C7-f32"):
             if name == a.workload:
                 continue
             c2, d2 = workload(name)
